@@ -1,0 +1,172 @@
+"""ctypes wrapper around oracle/omni_oracle.c  -- TEST INFRASTRUCTURE, NOT THE PRODUCT.
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference leg may import
+this module.  It never imports paper_2311_16935_b200 and shares nothing with the CUDA path.
+Everything here is argument marshalling for the C functions; the arithmetic lives in omni_oracle.c,
+each function citing the PAPER.md passage it follows.
+"""
+import ctypes as C
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "omni_oracle.c")
+_LIB = os.path.join(_HERE, "libomni_oracle.so")
+_lib = None
+
+
+def build(force=False):
+    """gcc -O2 -ffp-contract=off -fopenmp (no fast-math); rebuilt when the source is newer."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        cmd = ["gcc", "-O2", "-ffp-contract=off", "-fopenmp", "-shared", "-fPIC", "-o", _LIB, _SRC, "-lm"]
+        subprocess.run(cmd, check=True)
+    return _LIB
+
+
+class Info(C.Structure):
+    _fields_ = [("outer_iters", C.c_int), ("cg_iters_total", C.c_longlong), ("eps_R_final", C.c_double),
+                ("norm_S", C.c_double), ("converged", C.c_int)]
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        _lib = C.CDLL(build())
+        _lib.oracle_far_face_constant.restype = C.c_double
+        _lib.oracle_far_face_constant.argtypes = [C.c_double] * 3
+        _lib.oracle_dot.restype = C.c_double
+        _lib.oracle_num_threads.restype = C.c_int
+    return _lib
+
+
+def _p(a):
+    return None if a is None else a.ctypes.data_as(C.c_void_p)
+
+
+def _f64(a):
+    return None if a is None else np.ascontiguousarray(a, dtype=np.float64)
+
+
+def _dims(shape):
+    """shape is numpy order (nz, ny, nx) or (ny, nx); returns nx, ny, nz."""
+    if len(shape) == 2:
+        return shape[1], shape[0], 1
+    return shape[2], shape[1], shape[0]
+
+
+def num_threads():
+    return int(lib().oracle_num_threads())
+
+
+def constants(nx, ny, nz, dx, dy, dz):
+    """dict F[3], A_tot, c[3][3]  (Eq. 5/8/17 2D; Eq. 23/24/32-35 3D)."""
+    out = np.zeros(13)
+    lib().oracle_constants(C.c_int(nx), C.c_int(ny), C.c_int(nz), C.c_double(dx), C.c_double(dy), C.c_double(dz), _p(out))
+    return {"F": out[0:3].copy(), "A_tot": float(out[3]), "c": out[4:13].reshape(3, 3).copy()}
+
+
+def far_face_constant(da, db, dc):
+    return float(lib().oracle_far_face_constant(da, db, dc))
+
+
+def validity(gx, gy, gz=None, mask=None):
+    gx, gy, gz = _f64(gx), _f64(gy), _f64(gz)
+    nx, ny, nz = _dims(gx.shape)
+    m = None if mask is None else np.ascontiguousarray(mask, dtype=np.uint8)
+    v = np.zeros(gx.shape, dtype=np.uint8)
+    lib().oracle_validity(C.c_int(nx), C.c_int(ny), C.c_int(nz), _p(gx), _p(gy), _p(gz), _p(m), _p(v))
+    return v
+
+
+def weights(v, dx, dy, dz=1.0):
+    """returns w1[6,...], w0[6,...], w0C[...] (Eq. 10) for a validity array v."""
+    v = np.ascontiguousarray(v, dtype=np.uint8)
+    nx, ny, nz = _dims(v.shape)
+    w1 = np.zeros((6,) + v.shape)
+    w0 = np.zeros((6,) + v.shape)
+    w0C = np.zeros(v.shape)
+    lib().oracle_weights(C.c_int(nx), C.c_int(ny), C.c_int(nz), C.c_double(dx), C.c_double(dy), C.c_double(dz),
+                         _p(v), _p(w1), _p(w0), _p(w0C))
+    return w1, w0, w0C
+
+
+def source(v, w1, w0, gx, gy, gz, dx, dy, dz=1.0):
+    v = np.ascontiguousarray(v, dtype=np.uint8)
+    nx, ny, nz = _dims(v.shape)
+    gx, gy = _f64(gx), _f64(gy)
+    gz = _f64(gz) if gz is not None else np.zeros_like(gx)
+    S = np.zeros(v.shape)
+    lib().oracle_source(C.c_int(nx), C.c_int(ny), C.c_int(nz), C.c_double(dx), C.c_double(dy), C.c_double(dz),
+                        _p(v), _p(w1), _p(w0), _p(gx), _p(gy), _p(gz), _p(S))
+    return S
+
+
+def apply_M(v, w1, p):
+    v = np.ascontiguousarray(v, dtype=np.uint8)
+    nx, ny, nz = _dims(v.shape)
+    p = _f64(p)
+    q = np.zeros(v.shape)
+    lib().oracle_apply_M(C.c_int(nx), C.c_int(ny), C.c_int(nz), _p(v), _p(w1), _p(p), _p(q))
+    return q
+
+
+def apply_Wn(v, w0, w0C, p):
+    v = np.ascontiguousarray(v, dtype=np.uint8)
+    nx, ny, nz = _dims(v.shape)
+    p = _f64(p)
+    q = np.zeros(v.shape)
+    lib().oracle_apply_Wn(C.c_int(nx), C.c_int(ny), C.c_int(nz), _p(v), _p(w0), _p(w0C), _p(p), _p(q))
+    return q
+
+
+def cg(v, w1, rhs, x0, thresh, max_cg):
+    """textbook CG on M x = rhs from x0; returns (x, iterations)."""
+    v = np.ascontiguousarray(v, dtype=np.uint8)
+    nx, ny, nz = _dims(v.shape)
+    rhs = _f64(rhs)
+    x = np.array(x0, dtype=np.float64, order="C", copy=True)
+    r, p, q = np.zeros(v.shape), np.zeros(v.shape), np.zeros(v.shape)
+    f = lib().oracle_cg
+    f.restype = C.c_int
+    k = f(C.c_int(nx), C.c_int(ny), C.c_int(nz), _p(v), _p(w1), _p(rhs), _p(x), C.c_double(thresh), C.c_int(max_cg),
+          _p(r), _p(p), _p(q))
+    return x, int(k)
+
+
+def solve(gx, gy, gz, mask, dx, dy, dz, tol, max_outer, max_cg, hist_cap=0):
+    """Algorithm 1.  Arrays in numpy order (nz,ny,nx) or (ny,nx).  Returns (P, info dict[, hist])."""
+    gx, gy = _f64(gx), _f64(gy)
+    nx, ny, nz = _dims(gx.shape)
+    gz = _f64(gz) if gz is not None else None
+    if nz > 1 and gz is None:
+        raise ValueError("gz required in 3D")
+    m = None if mask is None else np.ascontiguousarray(mask, dtype=np.uint8)
+    P = np.zeros(gx.shape)
+    info = Info()
+    hist = np.full(max(hist_cap, 1), np.nan)
+    f = lib().oracle_solve
+    f.restype = C.c_int
+    rc = f(C.c_int(nx), C.c_int(ny), C.c_int(nz), C.c_double(dx), C.c_double(dy), C.c_double(dz),
+           _p(gx), _p(gy), _p(gz if gz is not None else gx), _p(m), _p(P), C.c_double(tol), C.c_int(max_outer),
+           C.c_int(max_cg), C.byref(info), _p(hist) if hist_cap else None, C.c_int(hist_cap))
+    if rc != 0:
+        raise MemoryError("oracle_solve: allocation failed")
+    d = {"outer_iters": info.outer_iters, "cg_iters_total": info.cg_iters_total, "eps_R_final": info.eps_R_final,
+         "norm_S": info.norm_S, "converged": bool(info.converged)}
+    return (P, d, hist) if hist_cap else (P, d)
+
+
+def sample(v, gx, gy, gz, x, cells, dx, dy, dz=1.0):
+    """Per-cell S_C, (M x)_C, (W^n x)_C at linear indices `cells` (full-size spot checks)."""
+    v = np.ascontiguousarray(v, dtype=np.uint8)
+    nx, ny, nz = _dims(v.shape)
+    gx, gy, gz, x = _f64(gx), _f64(gy), _f64(gz), _f64(x)
+    if gx is not None and gz is None:
+        gz = gx
+    cells = np.ascontiguousarray(cells, dtype=np.int64)
+    S, Mx, Wx = np.zeros(len(cells)), np.zeros(len(cells)), np.zeros(len(cells))
+    lib().oracle_sample(C.c_int(nx), C.c_int(ny), C.c_int(nz), C.c_double(dx), C.c_double(dy), C.c_double(dz),
+                        _p(v), _p(gx), _p(gy), _p(gz), _p(x), C.c_longlong(len(cells)), _p(cells), _p(S), _p(Mx), _p(Wx))
+    return S, Mx, Wx

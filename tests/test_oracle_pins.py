@@ -1,0 +1,464 @@
+"""Pins of the CPU oracle against what the paper and the mathematics fix (no GPU, no CUDA path).
+
+Each test names the passage it pins (PAPER.md:<line>).  Nothing here compares the oracle with itself:
+expected values are the paper's printed numbers/tables (tests/golden/), closed forms, numpy dense algebra,
+or brute-force ray counting.
+"""
+import math
+import os
+
+import numpy as np
+import pytest
+
+from workloads import make_field
+
+GOLD = os.path.join(os.path.dirname(__file__), "golden")
+DIRS = ["E", "W", "N", "S", "F", "B"]
+
+
+# ----------------------------------------------------------------------------- constants
+
+def test_2d_constants_eq5_6_7_17(oracle):
+    """Eq. 5 (:75) A_E = 2 dy; Eq. 6 (:86) = c_xy; Eq. 7 (:89) = c_xy + c_xx; Eq. 8 (:94)."""
+    dx, dy = 0.3, 0.7
+    K = oracle.constants(5, 5, 1, dx, dy, 1.0)
+    dd = math.hypot(dx, dy)
+    assert K["F"][0] == pytest.approx(2 * dy, rel=1e-15)
+    assert K["F"][1] == pytest.approx(2 * dx, rel=1e-15)
+    assert K["A_tot"] == pytest.approx(4 * (dx + dy), rel=1e-15)
+    assert K["c"][0, 1] == pytest.approx(dx + dy - dd, rel=1e-14)              # Eq. 6
+    assert K["c"][0, 1] + K["c"][0, 0] == pytest.approx(dy - dx + dd, rel=1e-14)  # Eq. 7
+    # Eq. 6 is printed as an integral too (:84): evaluate it numerically
+    al = math.atan(dy / dx)
+    th = np.linspace(0, al, 200001)
+    i1 = np.trapezoid(dx * np.sin(th), th)
+    th = np.linspace(al, math.pi / 2, 200001)
+    i2 = np.trapezoid(dy * np.cos(th), th)
+    assert K["c"][0, 1] == pytest.approx(i1 + i2, rel=1e-9)
+
+
+def test_appendix_constants_eq45_46(oracle):
+    D = 0.37
+    K = oracle.constants(3, 3, 1, D, D, 1.0)
+    assert K["c"][0, 0] == pytest.approx(D * (2 * math.sqrt(2) - 2), rel=1e-14)
+    assert K["c"][1, 1] == pytest.approx(D * (2 * math.sqrt(2) - 2), rel=1e-14)
+    assert K["c"][0, 1] == pytest.approx(D * (2 - math.sqrt(2)), rel=1e-14)
+    assert K["A_tot"] == pytest.approx(8 * D, rel=1e-15)                      # :585
+
+
+def test_3d_isotropic_constants_eq34_35(oracle):
+    """Eq. 34-35 (:322-326) to the 13 digits printed; Eq. 24 (:262); sum rule = pi D^2 (Eq. 23)."""
+    for D in (1.0, 0.25):
+        K = oracle.constants(4, 4, 4, D, D, D)
+        assert K["c"][0, 0] / D**2 == pytest.approx(0.6277684243304, abs=5e-14)
+        assert K["c"][0, 1] / D**2 == pytest.approx(0.6284560573148, abs=5e-14)
+        assert K["A_tot"] == pytest.approx(6 * math.pi * D * D, rel=1e-15)
+        assert K["c"][0, 0] + 4 * K["c"][0, 1] == pytest.approx(math.pi * D * D, rel=1e-13)
+    # the general-spacing quadrature (reading A7) reproduces Eq. 34 at dx=dy=dz
+    assert oracle.far_face_constant(1.0, 1.0, 1.0) == pytest.approx(0.6277684243304, abs=5e-13)
+
+
+def test_3d_general_constants_symmetry_and_sum_rule(oracle):
+    """c_jk = c_kj (:304); every face's pieces sum to its total pi*d*d (Eq. 23 :258, Eq. 25 :266)."""
+    dx, dy, dz = 1.0, 0.7, 1.9
+    K = oracle.constants(4, 4, 4, dx, dy, dz)
+    c, F = K["c"], K["F"]
+    assert np.allclose(c, c.T, rtol=0, atol=0)
+    assert np.all(c > 0)
+    for a in range(3):
+        b, cc = (a + 1) % 3, (a + 2) % 3
+        assert c[a, a] + 2 * c[a, b] + 2 * c[a, cc] == pytest.approx(F[a], rel=1e-13)
+    assert F[1] == pytest.approx(math.pi * dx * dz)
+    # near-isotropic spacing must approach the closed forms continuously
+    Kn = oracle.constants(4, 4, 4, 1.0, 1.0, 1.0 + 1e-9)
+    Ki = oracle.constants(4, 4, 4, 1.0, 1.0, 1.0)
+    assert np.allclose(Kn["c"], Ki["c"], rtol=1e-8)
+
+
+# ----------------------------------------------------------------------------- brute-force ray counts (P11)
+
+def _mc_fractions(da, db, dc, n, rng, three_d):
+    """Rays leave the shared face into Q (size da along the face normal) with the cosine-weighted measure of
+    Eq. 4/22 (:71, :253); returns the fractions that leave Q through far, +b, -b, +c, -c faces."""
+    if not three_d:
+        y0 = rng.uniform(-db / 2, db / 2, n)
+        sin_t = rng.uniform(-1, 1, n)                 # pdf ~ cos(theta) d theta
+        tan_t = sin_t / np.sqrt(1 - sin_t**2)
+        y = y0 + da * tan_t
+        return np.array([np.mean(np.abs(y) <= db / 2), np.mean(y > db / 2), np.mean(y < -db / 2), 0.0, 0.0])
+    y0 = rng.uniform(-db / 2, db / 2, n)
+    z0 = rng.uniform(-dc / 2, dc / 2, n)
+    s2 = rng.uniform(0, 1, n)                         # sin^2(theta) uniform: pdf ~ cos sin d theta
+    st, ct = np.sqrt(s2), np.sqrt(1 - s2)
+    ph = rng.uniform(0, 2 * np.pi, n)
+    vy, vz = st * np.cos(ph), st * np.sin(ph)
+    with np.errstate(divide="ignore"):
+        t_far = da / ct
+        t_b = np.where(vy > 0, (db / 2 - y0) / vy, (-db / 2 - y0) / vy)
+        t_c = np.where(vz > 0, (dc / 2 - z0) / vz, (-dc / 2 - z0) / vz)
+    first = np.argmin(np.stack([t_far, t_b, t_c]), axis=0)
+    return np.array([np.mean(first == 0), np.mean((first == 1) & (vy > 0)), np.mean((first == 1) & (vy < 0)),
+                     np.mean((first == 2) & (vz > 0)), np.mean((first == 2) & (vz < 0))])
+
+
+@pytest.mark.parametrize("spacing", [(1.0, 1.0, None), (0.3, 0.7, None), (1.0, 1.0, 1.0), (1.0, 0.7, 1.9)])
+def test_constants_vs_monte_carlo_ray_count(oracle, spacing):
+    """c_aa / F_a and c_ab / F_a are the fractions of rays through face a that crossed the far / side faces of the
+    neighbour cell (Fig. 4 :185, Eq. 14 :191, Fig. 5 :245).  Statistical pin: 4e6 rays, 5 sigma."""
+    dx, dy, dz = spacing
+    three_d = dz is not None
+    K = oracle.constants(4, 4, 4 if three_d else 1, dx, dy, dz if three_d else 1.0)
+    d = [dx, dy, dz if three_d else 1.0]
+    rng = np.random.default_rng(1234)
+    n = 4_000_000
+    for a in range(3 if three_d else 2):
+        if three_d:
+            b, c = (a + 1) % 3, (a + 2) % 3
+        else:
+            b, c = 1 - a, 2
+        fr = _mc_fractions(d[a], d[b], d[c], n, rng, three_d)
+        exp = np.array([K["c"][a, a], K["c"][a, b], K["c"][a, b], K["c"][a, c], K["c"][a, c]]) / K["F"][a]
+        sig = np.sqrt(np.maximum(exp * (1 - exp), 1e-12) / n)
+        assert np.all(np.abs(fr - exp) < 5 * sig + 1e-12), (a, fr, exp)
+
+
+def test_weights_vs_monte_carlo_on_masked_grid(oracle):
+    """Whole weight assembly (Eq. 15, 16, 18, 25) from first principles on a tiny masked 3D grid with anisotropic
+    spacing: trace rays back one cell, classify by the validity of the cell they came from."""
+    rng = np.random.default_rng(7)
+    shape = (4, 5, 4)
+    v = (rng.random(shape) > 0.3).astype(np.uint8)
+    dx, dy, dz = 1.0, 0.8, 1.3
+    d = [dx, dy, dz]
+    w1, w0, w0C = oracle.weights(v, dx, dy, dz)
+    K = oracle.constants(4, 5, 4, dx, dy, dz)
+    nz, ny, nx = shape
+
+    def valid(i, j, k):
+        return 0 <= i < nx and 0 <= j < ny and 0 <= k < nz and v[k, j, i]
+
+    n = 400_000
+    checked = 0
+    cells = [tuple(c) for c in np.argwhere(v == 1)[::5]]
+    for (k, j, i) in cells:
+        C = np.array([i, j, k])
+        AC = 0.0
+        for dd in range(6):
+            a, sg = dd // 2, (1 if dd % 2 == 0 else -1)
+            b, c = (a + 1) % 3, (a + 2) % 3
+            e = np.zeros(3, int); e[a] = sg
+            Q = C + e
+            share = K["F"][a] / K["A_tot"]
+            if not valid(*Q):
+                AC += share
+                assert w1[dd, k, j, i] == 0 and w0[dd, k, j, i] == 0
+                continue
+            fr = _mc_fractions(d[a], d[b], d[c], n, rng, True)
+            eb = np.zeros(3, int); eb[b] = 1
+            ec = np.zeros(3, int); ec[c] = 1
+            origin = [Q + e, Q + eb, Q - eb, Q + ec, Q - ec]
+            new = sum(f for f, o in zip(fr, origin) if valid(*o)) * share
+            old = sum(f for f, o in zip(fr, origin) if not valid(*o)) * share
+            tol = 5 * math.sqrt(0.25 / n) * share * 2
+            assert abs(w1[dd, k, j, i] - new) < tol
+            assert abs(w0[dd, k, j, i] - old) < tol
+            checked += 1
+        assert w0C[k, j, i] == pytest.approx(AC, rel=1e-12, abs=1e-15)
+    assert checked >= 10
+
+
+# ----------------------------------------------------------------------------- Table 1 (P1) and S (P2)
+
+def _parse_table1():
+    rows, fixes = {}, []
+    for line in open(os.path.join(GOLD, "table1_3x3.txt")):
+        line = line.strip()
+        if not line or line.startswith("#"):
+            continue
+        t = line.split()
+        if t[0] == "FIX":
+            fixes.append((t[1], int(t[2]), t[3]))
+        else:
+            rows[t[0]] = t[1:]
+            assert len(t) == 10
+    return rows, fixes
+
+
+def _tok(tok, D):
+    s2 = math.sqrt(2)
+    val = {"0": 0.0, "2D": 2 * D, "4D": 4 * D, "cxx": D * (2 * s2 - 2), "cyy": D * (2 * s2 - 2), "cxy": D * (2 - s2),
+           "2cxy": 2 * D * (2 - s2)}
+    return sum(val[p] for p in tok.split("+"))
+
+
+def test_table1_3x3_example(oracle):
+    """All ten A_j^i of all nine cells; 88 entries verbatim + the 2 of erratum A10."""
+    D = 0.5
+    v = np.ones((3, 3), np.uint8)
+    w1, w0, w0C = oracle.weights(v, D, D)
+    Atot = 8 * D
+    rows, fixes = _parse_table1()
+    # cell number (1..9, row-major from the top) -> numpy index (j, i) with j up
+    pos = {c: (2 - (c - 1) // 3, (c - 1) % 3) for c in range(1, 10)}
+    ours = {}
+    for c, (j, i) in pos.items():
+        ours[("A_C^n", c)] = w0C[j, i] * Atot
+        ours[("A_C^n+1", c)] = 0.0                                   # Eq. 11 :113
+        for dd, name in enumerate(DIRS[:4]):
+            ours[(f"A_{name}^n+1", c)] = w1[dd, j, i] * Atot
+            ours[(f"A_{name}^n", c)] = w0[dd, j, i] * Atot
+    fixed = {(r, c): tok for r, c, tok in fixes}
+    n_verbatim = 0
+    for r, toks in rows.items():
+        for c in range(1, 10):
+            tok = fixed.get((r, c), toks[c - 1])
+            assert ours[(r, c)] == pytest.approx(_tok(tok, D), abs=1e-14), (r, c, tok)
+            n_verbatim += (r, c) not in fixed
+    assert n_verbatim == 88 and len(fixed) == 2
+    # the verbatim cell-4 entries break the table's own mirror symmetries (justifies A10)
+    assert rows["A_N^n"][3] != rows["A_N^n"][5] and rows["A_N^n"][3] != rows["A_S^n"][3]
+    # "all coefficients sum to A_tot, which is always required" (:631)
+    for c in range(1, 10):
+        assert sum(val for (r, cc), val in ours.items() if cc == c) == pytest.approx(Atot, rel=1e-14)
+
+
+def test_source_eq49_50(oracle):
+    """S_1 and S_5 of the 3x3 example (Eq. 49-50 :656-662): signs, 1/2 face average, missing-neighbour rule."""
+    D = 0.25
+    rng = np.random.default_rng(3)
+    fx, fy = rng.normal(size=(3, 3)), rng.normal(size=(3, 3))
+    v = np.ones((3, 3), np.uint8)
+    w1, w0, _ = oracle.weights(v, D, D)
+    S = oracle.source(v, w1, w0, fx, fy, None, D, D)
+    pos = {c: (2 - (c - 1) // 3, (c - 1) % 3) for c in range(1, 10)}
+    f_x = {c: fx[pos[c]] for c in pos}
+    f_y = {c: fy[pos[c]] for c in pos}
+    S1 = -(D / 8) * (f_x[2] + f_x[1] - f_y[4] - f_y[1])
+    S5 = -(D / 8) * (f_x[6] - f_x[4] + f_y[2] - f_y[8])
+    assert S[pos[1]] == pytest.approx(S1, rel=1e-13)
+    assert S[pos[5]] == pytest.approx(S5, rel=1e-13)
+
+
+# ----------------------------------------------------------------------------- invariants (P4)
+
+@pytest.mark.parametrize("shape,sp", [((9, 11), (0.3, 0.5, 1.0)), ((6, 7, 8), (1.0, 1.0, 1.0)), ((6, 7, 8), (0.4, 1.1, 0.7)),
+                                      ((1, 9), (1.0, 1.0, 1.0)), ((5, 1, 6), (1.0, 2.0, 1.0))])
+def test_weights_sum_to_one_and_nonnegative(oracle, shape, sp):
+    """w_C^n + sum_j (w_j^{n+1} + w_j^n) = 1 at every valid cell, any mask/spacing (:631, Eq. 8, Eq. 24)."""
+    rng = np.random.default_rng(11)
+    v = (rng.random(shape) > 0.25).astype(np.uint8)
+    w1, w0, w0C = oracle.weights(v, *sp)
+    tot = w0C + w1.sum(0) + w0.sum(0)
+    assert np.allclose(tot[v == 1], 1.0, rtol=0, atol=1e-14)
+    assert np.all(tot[v == 0] == 0)
+    assert w1.min() >= 0 and w0.min() >= -1e-16 and w0C.min() >= 0
+    # interior cell of a full box: only new-iteration weights, w = F_a / A_tot (Eq. 5)
+    full = np.ones(shape, np.uint8)
+    w1f, w0f, w0Cf = oracle.weights(full, *sp)
+    K = oracle.constants(shape[-1], shape[-2], shape[0] if len(shape) == 3 else 1, *sp)
+    if min(shape) >= 5:
+        ctr = tuple(s // 2 for s in shape)
+        for dd in range(2 * len(shape)):
+            assert w1f[(dd,) + ctr] == pytest.approx(K["F"][dd // 2] / K["A_tot"], rel=1e-14)
+            assert w0f[(dd,) + ctr] == pytest.approx(0.0, abs=1e-16)
+
+
+def test_validity_eq13(oracle):
+    """NaN in any used component or mask == 0 marks a cell missing (Eq. 13 :176, :158)."""
+    gx, gy, gz = np.zeros((2, 3, 4)), np.zeros((2, 3, 4)), np.zeros((2, 3, 4))
+    gx[0, 0, 1] = np.nan
+    gz[1, 2, 3] = np.nan
+    mask = np.ones((2, 3, 4), np.uint8)
+    mask[1, 1, 1] = 0
+    v = oracle.validity(gx, gy, gz, mask)
+    exp = np.ones((2, 3, 4), np.uint8)
+    exp[0, 0, 1] = exp[1, 2, 3] = exp[1, 1, 1] = 0
+    assert np.array_equal(v, exp)
+    # 2D ignores gz
+    v2 = oracle.validity(gx[0], gy[0], None, None)
+    assert v2.sum() == 11
+
+
+# ----------------------------------------------------------------------------- dense algebra pins (P5, P6)
+
+def _dense(v, w1, w0=None, w0C=None):
+    """M (and W^n) as dense numpy matrices, filled entry by entry from the stored weights (Eq. 12 :119 with the
+    sign convention of reading A1), then handed to numpy.linalg."""
+    shape = v.shape
+    N = v.size
+    idx = np.arange(N).reshape(shape)
+    M = np.zeros((N, N))
+    W = np.zeros((N, N))
+    nd = len(shape)
+    for C in np.ndindex(shape):
+        if not v[C]:
+            continue
+        r = idx[C]
+        M[r, r] = 1.0
+        if w0C is not None:
+            W[r, r] = w0C[C]
+        for dd in range(2 * nd):
+            a, sg = dd // 2, (1 if dd % 2 == 0 else -1)
+            Q = list(C)
+            Q[nd - 1 - a] += sg
+            if not (0 <= Q[nd - 1 - a] < shape[nd - 1 - a]):
+                continue
+            q = idx[tuple(Q)]
+            M[r, q] -= w1[(dd,) + C]
+            if w0 is not None:
+                W[r, q] += w0[(dd,) + C]
+    return M, W
+
+
+@pytest.mark.parametrize("shape,sp", [((10, 12), (1.0, 0.6, 1.0)), ((5, 6, 6), (1.0, 1.0, 1.0))])
+def test_inner_cg_vs_dense_lu(oracle, shape, sp):
+    """Textbook CG on the non-symmetric M (reading A2) reaches the dense-LU solution on random masks."""
+    rng = np.random.default_rng(5)
+    v = (rng.random(shape) > 0.15).astype(np.uint8)
+    w1, w0, w0C = oracle.weights(v, *sp)
+    M, _ = _dense(v, w1)
+    assert np.abs(M - M.T).max() > 1e-3            # the operator really is non-symmetric next to boundaries
+    rhs = rng.normal(size=shape) * v
+    x, k = oracle.cg(v, w1, rhs, np.zeros(shape), 1e-13 * np.linalg.norm(rhs), 2000)
+    keep = v.ravel() == 1
+    xs = np.linalg.solve(M[np.ix_(keep, keep)], rhs.ravel()[keep])
+    assert k < 2000
+    assert np.linalg.norm(x.ravel()[keep] - xs) / np.linalg.norm(xs) < 1e-10
+    # apply_M agrees with the densely assembled matrix (pins the operator's indexing/signs through numpy)
+    p = rng.normal(size=shape) * v
+    assert np.allclose(oracle.apply_M(v, w1, p).ravel(), M @ p.ravel(), rtol=0, atol=1e-14)
+
+
+@pytest.mark.parametrize("shape,sp", [((9, 10), (1.0, 0.6, 1.0)), ((5, 5, 6), (1.0, 1.3, 0.8))])
+def test_outer_iteration_vs_dense_solves(oracle, shape, sp):
+    """Algorithm 1 (:128-150) with numpy dense solves of Eq. 12, iteration by iteration, against oracle.solve with a
+    tight inner CG; and the limit: the fixed point solves L P = S, L = weighted graph Laplacian F_a/A_tot (P5)."""
+    rng = np.random.default_rng(9)
+    f = make_field("gaussians2d" if len(shape) == 2 else "fourier3d", shape, seed=2, noise=0.05, kmax=2.0)
+    mask = (rng.random(shape) > 0.12).astype(np.uint8)
+    d = sp
+    g = f["g"] + [None] * (3 - len(f["g"]))
+    v = oracle.validity(g[0], g[1], g[2], mask)
+    w1, w0, w0C = oracle.weights(v, *d)
+    S = oracle.source(v, w1, w0, g[0], g[1], g[2], *d)
+    M, W = _dense(v, w1, w0, w0C)
+    keep = v.ravel() == 1
+    Mk, Wk, Sk = M[np.ix_(keep, keep)], W[np.ix_(keep, keep)], S.ravel()[keep]
+    P = np.zeros(keep.sum())
+    for n in range(1, 6):
+        P = np.linalg.solve(Mk, Wk @ P + Sk)
+        Po, info = oracle.solve(g[0], g[1], g[2], mask, *d, tol=0.0, max_outer=n, max_cg=400)
+        assert info["outer_iters"] == n
+        assert np.linalg.norm(Po.ravel()[keep] - P) / np.linalg.norm(P) < 1e-10
+        assert np.all(np.isnan(Po.ravel()[~keep]))
+    # fixed point: (M - W) P = S.  L is built here from its definition, not from the oracle's weights.
+    K = oracle.constants(shape[-1], shape[-2], shape[0] if len(shape) == 3 else 1, *d)
+    t = K["F"] / K["A_tot"]
+    N = v.size
+    idx = np.arange(N).reshape(shape)
+    L = np.zeros((N, N))
+    nd = len(shape)
+    for C in np.ndindex(shape):
+        if not v[C]:
+            continue
+        for a in range(nd):
+            for sg in (1, -1):
+                Q = list(C); Q[nd - 1 - a] += sg
+                if 0 <= Q[nd - 1 - a] < shape[nd - 1 - a] and v[tuple(Q)]:
+                    L[idx[C], idx[C]] += t[a]
+                    L[idx[C], idx[tuple(Q)]] -= t[a]
+    Lk = L[np.ix_(keep, keep)]
+    assert np.allclose(Lk, Mk - Wk, rtol=0, atol=1e-14)
+    assert np.allclose(Lk, Lk.T)
+    Pstar = np.linalg.lstsq(Lk, Sk, rcond=None)[0]
+    Po, info = oracle.solve(g[0], g[1], g[2], mask, *d, tol=1e-11, max_outer=20000, max_cg=400)
+    assert info["converged"]
+    # compare per connected component after mean removal (reading A12)
+    from scipy.sparse import csr_matrix
+    from scipy.sparse.csgraph import connected_components
+    ncomp, lab = connected_components(csr_matrix(np.abs(Lk) > 0), directed=False)
+    a, b = Po.ravel()[keep].copy(), Pstar.copy()
+    for cpt in range(ncomp):
+        m = lab == cpt
+        a[m] -= a[m].mean(); b[m] -= b[m].mean()
+    assert np.linalg.norm(a - b) / np.linalg.norm(b) < 1e-8
+
+
+# ----------------------------------------------------------------------------- analytic pins (P7, P8, P9)
+
+@pytest.mark.parametrize("shape,sp", [((12, 10), (0.1, 0.07, 1.0)), ((7, 8, 6), (0.2, 0.15, 0.3))])
+def test_exact_on_quadratics(oracle, shape, sp):
+    """The face average of f is exact for quadratic P (:78 'second-order accurate'), so the converged field equals
+    P up to a constant to rounding, for any mask and spacing."""
+    rng = np.random.default_rng(21)
+    nd = len(shape)
+    ax = [np.arange(m) * s for m, s in zip(shape[::-1], sp)]          # x, y, (z)
+    X = np.meshgrid(*ax[::-1], indexing="ij")[::-1]                    # X[0]=x ...
+    A = rng.normal(size=(nd, nd)); A = A + A.T
+    b = rng.normal(size=nd)
+    P = sum(b[i] * X[i] for i in range(nd)) + 0.5 * sum(A[i, j] * X[i] * X[j] for i in range(nd) for j in range(nd))
+    g = [b[i] + sum(A[i, j] * X[j] for j in range(nd)) for i in range(nd)] + [None] * (3 - nd)
+    mask = np.ones(shape, np.uint8)
+    mask[tuple(s // 2 for s in shape)] = 0
+    mask[(1,) * nd] = 0
+    Po, info = oracle.solve(g[0], g[1], g[2], mask, *sp, tol=1e-13, max_outer=50000, max_cg=500)
+    assert info["converged"]
+    m = mask == 1
+    e = (Po[m] - Po[m].mean()) - (P[m] - P[m].mean())
+    assert np.linalg.norm(e) / np.linalg.norm(P[m] - P[m].mean()) < 1e-10
+
+
+def test_second_order_convergence(oracle):
+    """Smooth P from exact gradients: discretisation error falls as h^2 (:78, :105)."""
+    errs = []
+    for n in (17, 33, 65):
+        f = make_field("gaussians2d", (n, n), seed=0, noise=0.0)
+        Po, info = oracle.solve(f["g"][0], f["g"][1], None, None, *f["d"], tol=1e-9, max_outer=20000, max_cg=60)
+        assert info["converged"]
+        e = (Po - Po.mean()) - (f["P"] - f["P"].mean())
+        errs.append(np.linalg.norm(e) / np.linalg.norm(f["P"] - f["P"].mean()))
+    assert 3.5 < errs[0] / errs[1] < 4.5 and 3.5 < errs[1] / errs[2] < 4.5, errs
+
+
+def test_zero_gradient_gives_zero_field(oracle):
+    """S = 0 -> P = 0 (constant), no iterations (Alg. 1 :139, reading A4)."""
+    z = np.zeros((6, 7, 8))
+    mask = np.ones(z.shape, np.uint8); mask[2, 3, 4] = 0
+    Po, info = oracle.solve(z, z, z, mask, 1.0, 1.0, 1.0, tol=1e-8, max_outer=10, max_cg=10)
+    assert info["outer_iters"] == 0 and info["cg_iters_total"] == 0 and info["norm_S"] == 0
+    assert np.all(Po[mask == 1] == 0) and np.isnan(Po[2, 3, 4])
+
+
+def test_conservation_and_residual_definition(oracle):
+    """1^T S = 0 on a full box (every face term appears twice with opposite sign); eps_R (Eq. 41 :442) equals
+    |S - (M - W^n) P| / |S| recomputed from the operators; eps_R^0 = 1 for P^0 = 0 (:445)."""
+    f = make_field("gaussians2d", (20, 24), seed=4, noise=0.05)
+    d = f["d"]
+    Po, info, hist = oracle.solve(f["g"][0], f["g"][1], None, None, *d, tol=0.0, max_outer=7, max_cg=30, hist_cap=16)
+    v = np.ones((20, 24), np.uint8)
+    w1, w0, w0C = oracle.weights(v, *d)
+    S = oracle.source(v, w1, w0, f["g"][0], f["g"][1], None, *d)
+    assert abs(S.sum()) < 1e-12 * np.abs(S).sum()
+    r = S - (oracle.apply_M(v, w1, Po) - oracle.apply_Wn(v, w0, w0C, Po))
+    assert np.linalg.norm(r) / np.linalg.norm(S) == pytest.approx(info["eps_R_final"], rel=1e-9)
+    assert hist[0] == pytest.approx(1.0, rel=1e-12)
+    assert np.all(np.diff(hist[:8]) < 0)
+
+
+def test_sample_matches_stored_weight_path(oracle):
+    """oracle.sample (per-cell evaluation for full-size spot checks) agrees with the stored-weight operators,
+    which the pins above fix."""
+    rng = np.random.default_rng(17)
+    shape = (7, 9, 8)
+    f = make_field("fourier3d", shape, seed=6, noise=0.1, kmax=2.0)
+    mask = (rng.random(shape) > 0.2).astype(np.uint8)
+    d = (0.5, 0.7, 0.9)
+    v = oracle.validity(*f["g"], mask)
+    w1, w0, w0C = oracle.weights(v, *d)
+    S = oracle.source(v, w1, w0, *f["g"], *d)
+    x = rng.normal(size=shape) * v
+    cells = rng.choice(v.size, 200, replace=False)
+    Ss, Ms, Ws = oracle.sample(v, *f["g"], x, cells, *d)
+    assert np.allclose(Ss, S.ravel()[cells], rtol=1e-14, atol=1e-16)
+    assert np.allclose(Ms, oracle.apply_M(v, w1, x).ravel()[cells], rtol=1e-14, atol=1e-16)
+    assert np.allclose(Ws, oracle.apply_Wn(v, w0, w0C, x).ravel()[cells], rtol=1e-14, atol=1e-16)
