@@ -1,0 +1,135 @@
+/* omni.h -- C ABI of the B200-native hot path of the matrix-based omnidirectional pressure integration
+ * (Zigunov & Charonko, arXiv 2311.16935; citations are PAPER.md:<line>).
+ *
+ * Problem statement (PAPER.md:26, :51, :122, Algorithm 1 :128-150, :158): given a measured pressure-gradient field
+ * f = grad P on a uniform rectangular grid with some cells missing, return P on the valid cells, up to an additive
+ * constant per connected region, by iterating  [W^{n+1}]{P^{n+1}} = [W^n]{P^n} + {S}  (Eq. 12 :119) from P^0 = 0,
+ * each system solved by conjugate gradients warm-started from P^n (:124, :489).
+ *
+ * Conventions for every entry point
+ *   - x is the fastest index: idx = i + nx*(j + ny*k).  nz == 1 selects the 2D scheme (Eq. 8, 14-20); dz and gz are
+ *     then ignored and gz may be NULL.  E/W = +/-x, N/S = +/-y, F/B = +/-z (:103).
+ *   - a cell is MISSING if it is outside the box, or mask[idx] == 0, or any used component of g is NaN (Eq. 13 :176).
+ *   - pointers named d_* are DEVICE memory owned by the caller (for example a torch tensor); pointers named h_* are
+ *     HOST memory owned by the caller.  The library never frees or keeps caller memory.
+ *   - `stream` is a cudaStream_t passed as void* (NULL = legacy default stream).  All device work is enqueued on it.
+ *   - errors are return codes only: nothing is printed, thrown or exit()ed.  Invalid arguments are rejected before
+ *     anything is enqueued.  Negative codes are errors; OMNI_NOT_CONVERGED (1) still writes the last iterate.
+ *   - same inputs give bit-identical outputs (fixed reduction order, no floating-point atomics).
+ *   - there is no CPU fallback: without a CUDA device every compute entry point returns OMNI_ERR_CUDA.
+ */
+#ifndef OMNI_H
+#define OMNI_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+    OMNI_OK = 0,
+    OMNI_NOT_CONVERGED = 1,    /* max_outer reached with eps_R > tol; result written                      */
+    OMNI_ERR_INVALID_ARG = -1,
+    OMNI_ERR_CUDA = -2,        /* a CUDA runtime call failed (or no device)                                */
+    OMNI_ERR_ALLOC = -3,       /* workspace allocation failed / caller workspace too small                 */
+    OMNI_ERR_BREAKDOWN = -4    /* non-finite scalar or p.Mp <= 0 seen on the device (M is not symmetric)   */
+} omni_status;
+
+typedef struct {
+    int outer_iters;           /* n: number of Eq. 12 solves performed (Algorithm 1 :141-149)              */
+    long long cg_iters_total;  /* CG iterations summed over all outer iterations                           */
+    double eps_R_final;        /* momentum residual of the returned field, Eq. 41 :442                     */
+    double norm_S;             /* ||S||_2, the denominator of Eq. 41                                       */
+    int status;                /* same value as the function's return code                                 */
+} omni_info;
+
+enum { OMNI_F32 = 0, OMNI_F64 = 1 };
+
+/* ---- the whole hot path: Algorithm 1 (:128-150) -------------------------------------
+ * d_gx, d_gy, d_gz : [nx*ny*nz] pressure-gradient components (Eq. 1 :23), NaN = missing (:158).
+ * d_mask           : [nx*ny*nz] bytes, 1 = valid, 0 = missing; NULL = all cells valid.
+ * d_P_out          : [nx*ny*nz] result; quiet NaN at missing cells.  Not mean-shifted (the caller pins the constant).
+ * tol              : outer stop eps_R <= tol (Eq. 41); inner CG stops at ||r_k|| <= 0.1*tol*||S|| (A3).
+ * max_outer,max_cg : caps on outer iterations / CG iterations per outer iteration (>= 0).  tol = 0 runs exactly
+ *                    max_outer x max_cg iterations (fixed-count trajectories).
+ * info             : host, may be NULL.  If NULL the call returns right after enqueueing (no synchronisation and
+ *                    the return code covers argument / launch errors only); otherwise the call synchronises `stream`
+ *                    once at the end and fills *info.
+ * _f32: g, S, the CG vectors and the stencil arithmetic are fp32; dot products accumulate in fp64; the master
+ * pressure and the outer residual (Eq. 41) are fp64 (A9).  dx, dy, dz, tol are double in both variants.
+ * Workspace is taken from the stream-ordered allocator (cudaMallocAsync) and released before returning. */
+int omni_solve_f64(int nx, int ny, int nz, double dx, double dy, double dz,
+                   const double* d_gx, const double* d_gy, const double* d_gz, const unsigned char* d_mask,
+                   double* d_P_out, double tol, int max_outer, int max_cg, void* stream, omni_info* info);
+int omni_solve_f32(int nx, int ny, int nz, double dx, double dy, double dz,
+                   const float* d_gx, const float* d_gy, const float* d_gz, const unsigned char* d_mask,
+                   float* d_P_out, double tol, int max_outer, int max_cg, void* stream, omni_info* info);
+
+/* Same with a caller-supplied device workspace (no allocation inside): d_workspace must hold at least
+ * omni_workspace_bytes(nx, ny, nz, dtype) bytes, 256-byte aligned; contents are scratch. */
+size_t omni_workspace_bytes(int nx, int ny, int nz, int dtype /* OMNI_F32 | OMNI_F64 */);
+int omni_solve_f64_ws(int nx, int ny, int nz, double dx, double dy, double dz,
+                      const double* d_gx, const double* d_gy, const double* d_gz, const unsigned char* d_mask,
+                      double* d_P_out, double tol, int max_outer, int max_cg,
+                      void* d_workspace, size_t workspace_bytes, void* stream, omni_info* info);
+int omni_solve_f32_ws(int nx, int ny, int nz, double dx, double dy, double dz,
+                      const float* d_gx, const float* d_gy, const float* d_gz, const unsigned char* d_mask,
+                      float* d_P_out, double tol, int max_outer, int max_cg,
+                      void* d_workspace, size_t workspace_bytes, void* stream, omni_info* info);
+
+/* Same with HOST buffers: allocates device memory, copies h_g* / h_mask to the device, solves, copies P back and
+ * synchronises.  h_* buffers may be pageable or pinned. */
+int omni_solve_host_f64(int nx, int ny, int nz, double dx, double dy, double dz,
+                        const double* h_gx, const double* h_gy, const double* h_gz, const unsigned char* h_mask,
+                        double* h_P_out, double tol, int max_outer, int max_cg, void* stream, omni_info* info);
+int omni_solve_host_f32(int nx, int ny, int nz, double dx, double dy, double dz,
+                        const float* h_gx, const float* h_gy, const float* h_gz, const unsigned char* h_mask,
+                        float* h_P_out, double tol, int max_outer, int max_cg, void* stream, omni_info* info);
+
+/* ---- single steps of the path (each runs the same device code the solve runs; used by the parity tests) ----------
+ * a0  geometry constants (host only, no device needed).  out[0..2] = face totals F_x,F_y,F_z (Eq. 5 :75 / Eq. 23 :258),
+ *     out[3] = A_tot (Eq. 8 :94 / Eq. 24 :262), out[4..12] = c_jk row-major 3x3 (Eq. 17 :207 / Eq. 32-35 :314-326 /
+ *     parallel-rectangle measure for general spacing, A7).  2D: every entry with a z index is 0. */
+int omni_constants(int nx, int ny, int nz, double dx, double dy, double dz, double* h_out13);
+
+/* a1+a2  source vector S (last sum of Eq. 9 :100; Eq. 49-50 :656-662), 0 at missing cells; *h_norm_S (host, may be
+ *     NULL) receives ||S||_2.  Synchronises `stream`. */
+int omni_source_f64(int nx, int ny, int nz, double dx, double dy, double dz,
+                    const double* d_gx, const double* d_gy, const double* d_gz, const unsigned char* d_mask,
+                    double* d_S_out, double* h_norm_S, void* stream);
+int omni_source_f32(int nx, int ny, int nz, double dx, double dy, double dz,
+                    const float* d_gx, const float* d_gy, const float* d_gz, const unsigned char* d_mask,
+                    float* d_S_out, double* h_norm_S, void* stream);
+
+/* a1+a4  q = [W^{n+1}] p = M p with M = I - W1_off (Eq. 9 rearranged, A1), through the CG operator kernel
+ *     (K4's recomputation path); validity from d_mask only (NULL = full box); q = 0 at missing cells; values of p at
+ *     missing cells are ignored.  *h_pq (host, may be NULL) receives p.Mp over valid cells.  Synchronises. */
+int omni_apply_M_f64(int nx, int ny, int nz, double dx, double dy, double dz, const unsigned char* d_mask,
+                     const double* d_p, double* d_q, double* h_pq, void* stream);
+int omni_apply_M_f32(int nx, int ny, int nz, double dx, double dy, double dz, const unsigned char* d_mask,
+                     const float* d_p, float* d_q, double* h_pq, void* stream);
+
+/* a3  outer residual r = S + [W^n]P - [W^{n+1}]P = S - L P (Eq. 12 :119, Eq. 41 :442) for a given field P (values at
+ *     missing cells ignored), r = 0 at missing cells; *h_eps_R (host, may be NULL) = ||r|| / ||S||.  Synchronises.
+ *     _f32: g, S and r are fp32, P is fp64 (the fp32 solve keeps its master pressure in fp64, A9). */
+int omni_residual_f64(int nx, int ny, int nz, double dx, double dy, double dz,
+                      const double* d_gx, const double* d_gy, const double* d_gz, const unsigned char* d_mask,
+                      const double* d_P, double* d_r_out, double* h_eps_R, void* stream);
+int omni_residual_f32(int nx, int ny, int nz, double dx, double dy, double dz,
+                      const float* d_gx, const float* d_gy, const float* d_gz, const unsigned char* d_mask,
+                      const double* d_P, float* d_r_out, double* h_eps_R, void* stream);
+
+/* ---- misc ---------------------------------------------------------------------------------------------------- */
+/* Kernel launches issued by this library since the last reset (counts launches on any thread; for bench.py). */
+long long omni_launch_count(int reset);
+/* 0 = CUDA-graph loop with device-side conditional WHILE nodes (default), 1 = host-driven loop that synchronises
+ * once per outer iteration (debug / drivers without conditional nodes).  Returns the previous mode. */
+int omni_set_loop_mode(int mode);
+const char* omni_status_string(int status);
+int omni_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* OMNI_H */

@@ -77,21 +77,27 @@ static void gauss_legendre(int n, double *x, double *w)
  * (projected area integrated over direction, as in Eq. 22 :253) of those that entered
  * Q through its far face, a parallel db x dc rectangle at distance da:
  *   c_aa = 4 * int_0^db int_0^dc (db-u)(dc-v) da^2 / (u^2+v^2+da^2)^2 dv du.
- * Composite Gauss-Legendre, 16 panels x 16 points per axis. */
+ * Composite Gauss-Legendre: 16 points on each of 24 dyadic panels [L 2^-m, L 2^-(m-1)] per axis, refined
+ * towards 0 where the integrand peaks (width ~ da), so strongly anisotropic spacings keep ~1e-13. */
 static double far_face_constant(double da, double db, double dc)
 {
-    enum { NP = 16, NG = 16 };
+    enum { NP = 24, NG = 16 };
     double gx[NG], gw[NG];
     gauss_legendre(NG, gx, gw);
+    double lo[NP], hi[NP];                     /* panel bounds as fractions of the interval */
+    for (int m = 0; m < NP; ++m) {
+        hi[m] = ldexp(1.0, -m);
+        lo[m] = (m == NP - 1) ? 0.0 : ldexp(1.0, -(m + 1));
+    }
     long double acc = 0.0L;
     for (int pu = 0; pu < NP; ++pu)
         for (int iu = 0; iu < NG; ++iu) {
-            double u = (pu + 0.5 * (gx[iu] + 1.0)) * db / NP;
-            double wu = 0.5 * gw[iu] * db / NP;
+            double u = (lo[pu] + 0.5 * (gx[iu] + 1.0) * (hi[pu] - lo[pu])) * db;
+            double wu = 0.5 * gw[iu] * (hi[pu] - lo[pu]) * db;
             for (int pv = 0; pv < NP; ++pv)
                 for (int iv = 0; iv < NG; ++iv) {
-                    double v = (pv + 0.5 * (gx[iv] + 1.0)) * dc / NP;
-                    double wv = 0.5 * gw[iv] * dc / NP;
+                    double v = (lo[pv] + 0.5 * (gx[iv] + 1.0) * (hi[pv] - lo[pv])) * dc;
+                    double wv = 0.5 * gw[iv] * (hi[pv] - lo[pv]) * dc;
                     double r2 = u * u + v * v + da * da;
                     acc += (long double)(wu * wv * (db - u) * (dc - v) * da * da / (r2 * r2));
                 }

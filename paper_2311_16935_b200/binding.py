@@ -1,0 +1,213 @@
+"""Thin ctypes binding of include/omni.h: argument marshalling only.
+
+Every step of the path runs in the CUDA kernels of libomni.so; torch is used for device memory and streams.
+There is no CPU fallback: a missing library or a missing CUDA device raises.
+Arrays are torch tensors in C order with x the fastest index: shape (nz, ny, nx) or (ny, nx).
+"""
+import ctypes as C
+import os
+
+from . import build as _build
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_lib = None
+
+OMNI_OK, OMNI_NOT_CONVERGED = 0, 1
+STATUS_NAMES = {0: "OMNI_OK", 1: "OMNI_NOT_CONVERGED", -1: "OMNI_ERR_INVALID_ARG", -2: "OMNI_ERR_CUDA",
+                -3: "OMNI_ERR_ALLOC", -4: "OMNI_ERR_BREAKDOWN"}
+# every symbol include/omni.h declares
+SYMBOLS = ["omni_solve_f64", "omni_solve_f32", "omni_workspace_bytes", "omni_solve_f64_ws", "omni_solve_f32_ws",
+           "omni_solve_host_f64", "omni_solve_host_f32", "omni_constants", "omni_source_f64", "omni_source_f32",
+           "omni_apply_M_f64", "omni_apply_M_f32", "omni_residual_f64", "omni_residual_f32", "omni_launch_count",
+           "omni_set_loop_mode", "omni_status_string", "omni_version"]
+
+
+class OmniError(RuntimeError):
+    def __init__(self, code, what):
+        super().__init__(f"{what}: {STATUS_NAMES.get(code, code)} ({status_string(code)})")
+        self.code = code
+
+
+class Info(C.Structure):
+    _fields_ = [("outer_iters", C.c_int), ("cg_iters_total", C.c_longlong), ("eps_R_final", C.c_double),
+                ("norm_S", C.c_double), ("status", C.c_int)]
+
+    def as_dict(self):
+        return {"outer_iters": self.outer_iters, "cg_iters_total": self.cg_iters_total,
+                "eps_R_final": self.eps_R_final, "norm_S": self.norm_S, "status": self.status}
+
+
+def lib():
+    """Loads libomni.so (building it in-tree first if nvcc is available and the sources are newer)."""
+    global _lib
+    if _lib is None:
+        path = os.path.join(_HERE, "libomni.so")
+        try:
+            path = _build.build()
+        except Exception:
+            if not os.path.exists(path):
+                raise
+        L = C.CDLL(path)
+        L.omni_workspace_bytes.restype = C.c_size_t
+        L.omni_launch_count.restype = C.c_longlong
+        L.omni_status_string.restype = C.c_char_p
+        _lib = L
+    return _lib
+
+
+def status_string(code):
+    return lib().omni_status_string(C.c_int(code)).decode()
+
+
+def version():
+    return int(lib().omni_version())
+
+
+def launch_count(reset=False):
+    return int(lib().omni_launch_count(C.c_int(1 if reset else 0)))
+
+
+def set_loop_mode(mode):
+    """0 = CUDA-graph loop (default), 1 = host-driven debug loop.  Returns the previous mode."""
+    return int(lib().omni_set_loop_mode(C.c_int(mode)))
+
+
+def constants(nx, ny, nz, dx, dy, dz):
+    out = (C.c_double * 13)()
+    rc = lib().omni_constants(C.c_int(nx), C.c_int(ny), C.c_int(nz), C.c_double(dx), C.c_double(dy), C.c_double(dz), out)
+    if rc != 0:
+        raise OmniError(rc, "omni_constants")
+    v = list(out)
+    return {"F": v[0:3], "A_tot": v[3], "c": [v[4:7], v[7:10], v[10:13]]}
+
+
+def workspace_bytes(nx, ny, nz, dtype):
+    return int(lib().omni_workspace_bytes(C.c_int(nx), C.c_int(ny), C.c_int(nz), C.c_int(0 if dtype == "f32" else 1)))
+
+
+# ----------------------------------------------------------------------------------------------- marshalling
+
+def _dims(t):
+    if t.dim() == 2:
+        return t.shape[1], t.shape[0], 1
+    if t.dim() == 3:
+        return t.shape[2], t.shape[1], t.shape[0]
+    raise ValueError("expected a 2D (ny, nx) or 3D (nz, ny, nx) tensor")
+
+
+def _suffix(t):
+    import torch
+    if t.dtype == torch.float32:
+        return "f32"
+    if t.dtype == torch.float64:
+        return "f64"
+    raise TypeError("fp32 or fp64 tensors only")
+
+
+def _ptr(t):
+    return C.c_void_p(0 if t is None else t.data_ptr())
+
+
+def _check(ts, device_type):
+    for t in ts:
+        if t is None:
+            continue
+        if not t.is_contiguous():
+            raise ValueError("tensors must be contiguous")
+        if t.device.type != device_type:
+            raise ValueError(f"tensor on {t.device}, expected {device_type}")
+
+
+def _stream(dev):
+    import torch
+    if not torch.cuda.is_available():
+        raise RuntimeError("paper_2311_16935_b200 needs a CUDA device: there is no CPU fallback")
+    return C.c_void_p(torch.cuda.current_stream(dev).cuda_stream)
+
+
+def _geom(gx, d):
+    nx, ny, nz = _dims(gx)
+    dx, dy = float(d[0]), float(d[1])
+    dz = float(d[2]) if len(d) > 2 else 1.0
+    return (C.c_int(nx), C.c_int(ny), C.c_int(nz), C.c_double(dx), C.c_double(dy), C.c_double(dz))
+
+
+def solve(gx, gy, gz, mask, d, tol, max_outer, max_cg, out=None, workspace=None, want_info=True):
+    """Algorithm 1 (omni_solve_f32/f64[_ws]) on device tensors, or omni_solve_host_* on CPU tensors.
+
+    d = (dx, dy[, dz]).  Returns (P, info dict or None).  Raises OmniError on negative status codes."""
+    import torch
+    sfx = _suffix(gx)
+    host = gx.device.type == "cpu"
+    _check([gx, gy, gz, mask, out], "cpu" if host else "cuda")
+    if mask is not None and mask.dtype != torch.uint8:
+        raise TypeError("mask must be uint8")
+    P = out if out is not None else torch.empty_like(gx)
+    info = Info()
+    geom = _geom(gx, d)
+    tail = (C.c_double(tol), C.c_int(max_outer), C.c_int(max_cg))
+    if host:
+        dev = torch.device("cuda", torch.cuda.current_device()) if torch.cuda.is_available() else None
+        fn = getattr(lib(), f"omni_solve_host_{sfx}")
+        rc = fn(*geom, _ptr(gx), _ptr(gy), _ptr(gz), _ptr(mask), _ptr(P), *tail, _stream(dev), C.byref(info))
+    else:
+        with torch.cuda.device(gx.device):
+            st = _stream(gx.device)
+            ip = C.byref(info) if want_info else None
+            if workspace is not None:
+                fn = getattr(lib(), f"omni_solve_{sfx}_ws")
+                rc = fn(*geom, _ptr(gx), _ptr(gy), _ptr(gz), _ptr(mask), _ptr(P), *tail, _ptr(workspace),
+                        C.c_size_t(workspace.numel() * workspace.element_size()), st, ip)
+            else:
+                fn = getattr(lib(), f"omni_solve_{sfx}")
+                rc = fn(*geom, _ptr(gx), _ptr(gy), _ptr(gz), _ptr(mask), _ptr(P), *tail, st, ip)
+    if rc < 0:
+        raise OmniError(rc, f"omni_solve_{sfx}")
+    return P, (info.as_dict() if (want_info or host) else None)
+
+
+def source(gx, gy, gz, mask, d):
+    """S of Eq. 9 (omni_source_*).  Returns (S, ||S||)."""
+    import torch
+    sfx = _suffix(gx)
+    _check([gx, gy, gz, mask], "cuda")
+    S = torch.empty_like(gx)
+    nrm = C.c_double(0.0)
+    with torch.cuda.device(gx.device):
+        rc = getattr(lib(), f"omni_source_{sfx}")(*_geom(gx, d), _ptr(gx), _ptr(gy), _ptr(gz), _ptr(mask), _ptr(S),
+                                                  C.byref(nrm), _stream(gx.device))
+    if rc < 0:
+        raise OmniError(rc, f"omni_source_{sfx}")
+    return S, nrm.value
+
+
+def apply_M(p, mask, d):
+    """q = M p (omni_apply_M_*).  Returns (q, p.Mp)."""
+    sfx = _suffix(p)
+    _check([p, mask], "cuda")
+    import torch
+    q = torch.empty_like(p)
+    pq = C.c_double(0.0)
+    with torch.cuda.device(p.device):
+        rc = getattr(lib(), f"omni_apply_M_{sfx}")(*_geom(p, d), _ptr(mask), _ptr(p), _ptr(q), C.byref(pq),
+                                                   _stream(p.device))
+    if rc < 0:
+        raise OmniError(rc, f"omni_apply_M_{sfx}")
+    return q, pq.value
+
+
+def residual(gx, gy, gz, mask, P, d):
+    """r = S - L P and eps_R of Eq. 41 (omni_residual_*); P is fp64.  Returns (r, eps_R)."""
+    import torch
+    sfx = _suffix(gx)
+    _check([gx, gy, gz, mask, P], "cuda")
+    if P.dtype != torch.float64:
+        raise TypeError("P must be fp64")
+    r = torch.empty_like(gx)
+    eps = C.c_double(0.0)
+    with torch.cuda.device(gx.device):
+        rc = getattr(lib(), f"omni_residual_{sfx}")(*_geom(gx, d), _ptr(gx), _ptr(gy), _ptr(gz), _ptr(mask), _ptr(P),
+                                                    _ptr(r), C.byref(eps), _stream(gx.device))
+    if rc < 0:
+        raise OmniError(rc, f"omni_residual_{sfx}")
+    return r, eps.value

@@ -1,0 +1,25 @@
+"""Builds libomni.so (the C-ABI library of include/omni.h) in-tree with nvcc for sm_100a."""
+import os
+import subprocess
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+SRC = [os.path.join(HERE, "csrc", "omni_api.cu")]
+DEPS = SRC + [os.path.join(HERE, "csrc", "omni_kernels.cuh"), os.path.join(os.path.dirname(HERE), "include", "omni.h")]
+LIB = os.path.join(HERE, "libomni.so")
+NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
+              "-Xcompiler", "-fPIC", "-shared", "-cudart", "static"]
+
+
+def build(force=False, verbose=False):
+    """Compile if libomni.so is missing or older than its sources; returns the library path."""
+    if not force and os.path.exists(LIB) and all(os.path.getmtime(LIB) >= os.path.getmtime(d) for d in DEPS):
+        return LIB
+    nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
+    cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-o", LIB] + SRC
+    subprocess.run(cmd, check=True)
+    return LIB
+
+
+if __name__ == "__main__":
+    import sys
+    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))

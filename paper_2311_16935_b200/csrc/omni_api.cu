@@ -1,0 +1,721 @@
+// omni_api.cu -- C ABI (include/omni.h) over the kernels of omni_kernels.cuh.
+// Host logic only: argument validation, geometry constants (a0), workspace carving, launch configuration and the
+// loop driver (CUDA graph with device-side conditional WHILE nodes, or a host-driven debug loop).
+#include "omni_kernels.cuh"
+#include "../../include/omni.h"
+
+#include <atomic>
+#include <cmath>
+#include <cstdio>
+#include <cstdlib>
+#include <type_traits>
+
+using namespace omni;
+
+namespace {
+
+std::atomic<long long> g_launches{0};
+std::atomic<int> g_loop_mode{0};
+
+#define CK(call)                                       \
+    do {                                               \
+        cudaError_t e__ = (call);                      \
+        if (e__ != cudaSuccess) return OMNI_ERR_CUDA;  \
+    } while (0)
+
+inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+// ------------------------------------------------------------------------------------------------ a0 constants
+
+// c_aa for general spacing: measure of the rays that cross two directly opposed, parallel db x dc rectangles a
+// distance da apart (A7; the geometry of PAPER.md:273 / Fig. 5b), written with the closed form of the
+// classical radiative configuration factor between aligned parallel rectangles, X = db/da, Y = dc/da:
+//   c_aa = 2 da^2 { ln sqrt[(1+X^2)(1+Y^2)/(1+X^2+Y^2)] + X sqrt(1+Y^2) atan(X/sqrt(1+Y^2))
+//                   + Y sqrt(1+X^2) atan(Y/sqrt(1+X^2)) - X atan X - Y atan Y }.
+double far_face_measure(double da, double db, double dc)
+{
+    const double X = db / da, Y = dc / da;
+    const double X2 = 1.0 + X * X, Y2 = 1.0 + Y * Y;
+    const double sx = std::sqrt(X2), sy = std::sqrt(Y2);
+    const double v = 0.5 * std::log(X2 * Y2 / (X2 + Y2 - 1.0)) + X * sy * std::atan(X / sy) + Y * sx * std::atan(Y / sx)
+                     - X * std::atan(X) - Y * std::atan(Y);
+    return 2.0 * da * da * v;
+}
+
+struct HostConst {
+    double F[3], Atot, c[3][3];
+};
+
+void host_constants(int nz, double dx, double dy, double dz, HostConst& H)
+{
+    const double PI = 3.14159265358979323846;
+    for (int a = 0; a < 3; ++a)
+        for (int b = 0; b < 3; ++b) H.c[a][b] = 0.0;
+    if (nz == 1) {                                             // 2D scheme
+        const double dd = std::hypot(dx, dy);
+        H.F[0] = 2.0 * dy; H.F[1] = 2.0 * dx; H.F[2] = 0.0;     // Eq. 5 :75
+        H.Atot = 4.0 * (dx + dy);                              // Eq. 8 :94
+        H.c[0][0] = 2.0 * (dd - dx);                           // Eq. 17 :207-212
+        H.c[1][1] = 2.0 * (dd - dy);
+        H.c[0][1] = H.c[1][0] = dx + dy - dd;
+        return;
+    }
+    const double d[3] = { dx, dy, dz };
+    H.F[0] = PI * dy * dz; H.F[1] = PI * dx * dz; H.F[2] = PI * dx * dy;      // Eq. 23 :258
+    H.Atot = 2.0 * PI * (dx * dy + dx * dz + dy * dz);                       // Eq. 24 :262
+    double s[3];
+    for (int a = 0; a < 3; ++a) {
+        H.c[a][a] = far_face_measure(d[a], d[(a + 1) % 3], d[(a + 2) % 3]);
+        s[a] = 0.5 * (H.F[a] - H.c[a][a]);      // c_ab + c_ac: the pieces of face a add up to F_a (Eq. 25 :266)
+    }
+    H.c[0][1] = H.c[1][0] = 0.5 * (s[0] + s[1] - s[2]);                      // c_jk = c_kj (:304)
+    H.c[0][2] = H.c[2][0] = 0.5 * (s[0] + s[2] - s[1]);
+    H.c[1][2] = H.c[2][1] = 0.5 * (s[1] + s[2] - s[0]);
+}
+
+template <typename T>
+Coef<T> make_coef(const HostConst& H, double dx, double dy, double dz)
+{
+    Coef<T> K;
+    const double d[3] = { dx, dy, dz };
+    for (int a = 0; a < 3; ++a) {
+        K.t[a] = (T)(H.F[a] / H.Atot);
+        K.caa[a] = (T)(H.c[a][a] / H.Atot);
+        K.cab[a] = (T)(H.c[a][(a + 1) % 3] / H.Atot);
+        K.cac[a] = (T)(H.c[a][(a + 2) % 3] / H.Atot);
+        K.hs[a] = (T)(d[a] * (H.F[a] / H.Atot) * 0.5);
+    }
+    return K;
+}
+
+// ------------------------------------------------------------------------------------------------ geometry / workspace
+
+bool make_geom(int nx, int ny, int nz, Geom& g)
+{
+    if (nx < 1 || ny < 1 || nz < 1) return false;
+    const long long px = ((long long)nx + 7) / 8 * 8;
+    const long long npad = px * (long long)ny * (long long)nz;
+    if (npad > (1LL << 40) || px > 0x7fffffff) return false;
+    g.nx = nx; g.ny = ny; g.nz = nz; g.px = (int)px;
+    g.pplane = px * ny;
+    g.npad = npad;
+    return true;
+}
+
+template <typename T>
+struct Workspace {
+    uint8_t* link; uint32_t* wcode; uint32_t* flags;
+    T *S, *r, *p0, *p1, *delta;
+    double* P; double* partial; Scalars* sc;
+};
+
+size_t partial_slots(const Geom& g)
+{
+    // 1D kernels: ceil(npad / 256) blocks; march kernels never exceed that
+    return (size_t)((g.npad + 255) / 256) * 2 + 64;
+}
+
+template <typename T>
+size_t carve(const Geom& g, char* base, Workspace<T>* w)
+{
+    size_t off = 0;
+    auto take = [&](size_t bytes) {
+        char* p = base ? base + off : nullptr;
+        off += align_up(bytes, 256);
+        return p;
+    };
+    const size_t n = (size_t)g.npad;
+    char* link = take(n);
+    char* wcode = take(n * 4);
+    char* flags = take(((n / 4 + 31) / 32 + 1) * 4);
+    char* S = take(n * sizeof(T));
+    char* r = take(n * sizeof(T));
+    char* p0 = take(n * sizeof(T));
+    char* p1 = take(n * sizeof(T));
+    char* delta = take(n * sizeof(T));
+    char* P = take(n * sizeof(double));
+    char* partial = take(partial_slots(g) * sizeof(double));
+    char* sc = take(sizeof(Scalars));
+    if (w) {
+        w->link = (uint8_t*)link; w->wcode = (uint32_t*)wcode; w->flags = (uint32_t*)flags;
+        w->S = (T*)S; w->r = (T*)r; w->p0 = (T*)p0; w->p1 = (T*)p1; w->delta = (T*)delta;
+        w->P = (double*)P; w->partial = (double*)partial; w->sc = (Scalars*)sc;
+    }
+    return off;
+}
+
+__global__ void init_scalars_kernel(Scalars* sc, double tol, int max_outer, int max_cg)
+{
+    Scalars s;
+    memset(&s, 0, sizeof(s));
+    s.tol = tol; s.max_outer = max_outer; s.max_cg = max_cg;
+    s.inner_go = 0; s.outer_go = 1; s.status = ST_OK;
+    *sc = s;
+}
+
+// ------------------------------------------------------------------------------------------------ launch configuration
+
+struct MarchCfg { dim3 grid, block; int zlen; };
+
+// z segments: minimise (waves) x (planes per CTA incl. the two halo planes)
+template <class Op>
+MarchCfg march_config(const Geom& g)
+{
+    constexpr int W = 32 * Op::V, TYO = Op::TYR - 2;
+    static int slots_cache = 0;
+    if (slots_cache == 0) {
+        int dev = 0, sms = 148, occ = 1;
+        cudaGetDevice(&dev);
+        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, march_kernel<Op>, 32 * Op::TYR, 0);
+        if (occ < 1) occ = 1;
+        slots_cache = sms * occ;
+    }
+    const int slots = slots_cache;
+    const int ntx = (g.px + W - 1) / W, nty = (g.ny + TYO - 1) / TYO;
+    const long long tiles = (long long)ntx * nty;
+    int best = 1;
+    double best_cost = 1e300;
+    const int max_seg = g.nz;
+    for (int ns = 1; ns <= max_seg; ns = (ns < 16 ? ns + 1 : ns + ns / 8)) {
+        const int zlen = (g.nz + ns - 1) / ns;
+        const int nseg = (g.nz + zlen - 1) / zlen;
+        const long long ctas = tiles * nseg;
+        const long long waves = (ctas + slots - 1) / slots;
+        const double cost = (double)waves * (zlen + (nseg > 1 ? 2 : 0) + 3);   // +3: per-CTA prologue/epilogue
+        if (cost < best_cost) { best_cost = cost; best = nseg; }
+        if (zlen <= 4) break;
+    }
+    MarchCfg c;
+    c.zlen = (g.nz + best - 1) / best;
+    const int nseg = (g.nz + c.zlen - 1) / c.zlen;
+    c.grid = dim3(ntx, nty, nseg);
+    c.block = dim3(32, Op::TYR, 1);
+    return c;
+}
+
+template <class Op>
+cudaError_t launch_march(const Geom& g, const typename Op::Args& a, cudaStream_t st)
+{
+    const MarchCfg c = march_config<Op>(g);
+    march_kernel<Op><<<c.grid, c.block, 0, st>>>(g, c.zlen, a);
+    g_launches.fetch_add(1, std::memory_order_relaxed);
+    return cudaGetLastError();
+}
+
+// tile shapes: 16 rows (14 output) x 1 KB wide; register budgets checked with -Xptxas -v
+template <typename T> using K3 = OpK3<T, 16, 1>;
+template <typename T> using K4 = OpK4<T, 16, 1>;
+template <typename T> using K2 = OpK2<T, 16, 1>;
+
+inline unsigned blocks_for(long long n, int bs) { return (unsigned)((n + bs - 1) / bs); }
+
+// ------------------------------------------------------------------------------------------------ setup shared by all entry points
+
+template <typename T>
+int setup_codes(const Geom& g, const Workspace<T>& w, const T* gx, const T* gy, const T* gz, const uint8_t* mask,
+                cudaStream_t st)
+{
+    uint8_t* vbyte = reinterpret_cast<uint8_t*>(w.p0);       // scratch: p0 is cleared afterwards
+    validity_kernel<T><<<blocks_for(g.npad, 256), 256, 0, st>>>(g, gx, gy, gz, mask, vbyte);
+    CK(cudaGetLastError());
+    codes_kernel<<<blocks_for(g.npad / 4, 256), 256, 0, st>>>(g, vbyte, w.link, w.wcode, w.flags);
+    CK(cudaGetLastError());
+    g_launches.fetch_add(2, std::memory_order_relaxed);
+    const size_t n = (size_t)g.npad;
+    CK(cudaMemsetAsync(w.p0, 0, n * sizeof(T), st));
+    CK(cudaMemsetAsync(w.p1, 0, n * sizeof(T), st));
+    CK(cudaMemsetAsync(w.delta, 0, n * sizeof(T), st));
+    CK(cudaMemsetAsync(w.P, 0, n * sizeof(double), st));
+    return OMNI_OK;
+}
+
+template <typename T>
+int launch_source(const Geom& g, const Workspace<T>& w, const Coef<T>& K, const T* gx, const T* gy, const T* gz,
+                  cudaStream_t st)
+{
+    source_kernel<T><<<blocks_for(g.npad, 256), 256, 0, st>>>(g, gx, gy, gz, w.link, K, w.S, w.sc, w.partial);
+    g_launches.fetch_add(1, std::memory_order_relaxed);
+    CK(cudaGetLastError());
+    return OMNI_OK;
+}
+
+template <typename T>
+typename K2<T>::Args k2_args(const Workspace<T>& w, const HostConst& H, CondHandles ch, int fold)
+{
+    typename K2<T>::Args a;
+    a.P = w.P; a.delta = w.delta; a.S = w.S; a.r = w.r; a.link = w.link; a.flags = w.flags;
+    for (int i = 0; i < 3; ++i) a.t[i] = H.F[i] / H.Atot;
+    a.sc = w.sc; a.partial = w.partial; a.cond = ch; a.fold_delta = fold;
+    return a;
+}
+template <typename T>
+typename K3<T>::Args k3_args(const Workspace<T>& w, const Coef<T>& K, CondHandles ch)
+{
+    typename K3<T>::Args a;
+    a.r = w.r; a.pbuf[0] = w.p0; a.pbuf[1] = w.p1; a.wcode = w.wcode; a.flags = w.flags;
+    a.K = K; a.sc = w.sc; a.partial = w.partial; a.cond = ch;
+    return a;
+}
+template <typename T>
+typename K4<T>::Args k4_args(const Workspace<T>& w, const Coef<T>& K, CondHandles ch)
+{
+    typename K4<T>::Args a;
+    a.r = w.r; a.delta = w.delta; a.pbuf[0] = w.p0; a.pbuf[1] = w.p1; a.wcode = w.wcode; a.flags = w.flags;
+    a.K = K; a.sc = w.sc; a.partial = w.partial; a.cond = ch; a.q_out = nullptr;
+    return a;
+}
+
+// ------------------------------------------------------------------------------------------------ loop drivers
+
+// Host-driven loop (debug): one synchronisation per outer iteration (plus one per 16 CG iterations).
+template <typename T>
+int run_loop_host(const Geom& g, const Workspace<T>& w, const HostConst& H, const Coef<T>& K, int max_outer, int max_cg,
+                  cudaStream_t st)
+{
+    CondHandles ch{ 0, 0, 0 };
+    const auto a2 = k2_args<T>(w, H, ch, 1);
+    const auto a3 = k3_args<T>(w, K, ch);
+    const auto a4 = k4_args<T>(w, K, ch);
+    Scalars h;
+    for (long long it = 0; it <= (long long)max_outer; ++it) {
+        CK(launch_march<K2<T>>(g, a2, st));
+        int done = 0;
+        while (done < max_cg) {
+            const int batch = (max_cg - done < 16) ? (max_cg - done) : 16;
+            for (int c = 0; c < batch; ++c) {
+                CK(launch_march<K3<T>>(g, a3, st));
+                CK(launch_march<K4<T>>(g, a4, st));
+            }
+            done += batch;
+            CK(cudaMemcpyAsync(&h, w.sc, sizeof(Scalars), cudaMemcpyDeviceToHost, st));
+            CK(cudaStreamSynchronize(st));
+            if (!h.inner_go) break;
+        }
+        if (max_cg == 0) {
+            CK(cudaMemcpyAsync(&h, w.sc, sizeof(Scalars), cudaMemcpyDeviceToHost, st));
+            CK(cudaStreamSynchronize(st));
+        }
+        if (!h.outer_go) break;
+    }
+    return OMNI_OK;
+}
+
+// CUDA-graph loop: outer WHILE { K2 ; inner WHILE { K3 ; K4 } }, conditions written by the kernels' last CTAs.
+template <typename T>
+int run_loop_graph(const Geom& g, const Workspace<T>& w, const HostConst& H, const Coef<T>& K, cudaStream_t st)
+{
+    cudaGraph_t G = nullptr;
+    cudaGraphExec_t exec = nullptr;
+    cudaStream_t cap = nullptr;
+    int rc = OMNI_ERR_CUDA;
+    // occupancy queries happen here, outside any stream capture (results are cached per kernel)
+    (void)march_config<K2<T>>(g); (void)march_config<K3<T>>(g); (void)march_config<K4<T>>(g);
+    do {
+        if (cudaGraphCreate(&G, 0) != cudaSuccess) break;
+        cudaGraphConditionalHandle hOuter, hInner;
+        if (cudaGraphConditionalHandleCreate(&hOuter, G, 1, cudaGraphCondAssignDefault) != cudaSuccess) break;
+        if (cudaGraphConditionalHandleCreate(&hInner, G, 0, cudaGraphCondAssignDefault) != cudaSuccess) break;
+        CondHandles ch{ (unsigned long long)hOuter, (unsigned long long)hInner, 1 };
+
+        cudaGraphNodeParams po = {};
+        po.type = cudaGraphNodeTypeConditional;
+        po.conditional.handle = hOuter;
+        po.conditional.type = cudaGraphCondTypeWhile;
+        po.conditional.size = 1;
+        cudaGraphNode_t nOuter;
+        if (cudaGraphAddNode(&nOuter, G, nullptr, 0, &po) != cudaSuccess) break;
+        cudaGraph_t bodyOuter = po.conditional.phGraph_out[0];
+
+        if (cudaStreamCreateWithFlags(&cap, cudaStreamNonBlocking) != cudaSuccess) break;
+        // K2 into the outer body
+        if (cudaStreamBeginCaptureToGraph(cap, bodyOuter, nullptr, nullptr, 0, cudaStreamCaptureModeThreadLocal) != cudaSuccess) break;
+        cudaError_t e = launch_march<K2<T>>(g, k2_args<T>(w, H, ch, 1), cap);
+        cudaGraph_t tmp = nullptr;
+        if (cudaStreamEndCapture(cap, &tmp) != cudaSuccess || e != cudaSuccess) break;
+        cudaGraphNode_t k2node;
+        size_t nn = 1;
+        if (cudaGraphGetNodes(bodyOuter, &k2node, &nn) != cudaSuccess || nn != 1) break;
+
+        cudaGraphNodeParams pi = {};
+        pi.type = cudaGraphNodeTypeConditional;
+        pi.conditional.handle = hInner;
+        pi.conditional.type = cudaGraphCondTypeWhile;
+        pi.conditional.size = 1;
+        cudaGraphNode_t nInner;
+        if (cudaGraphAddNode(&nInner, bodyOuter, &k2node, 1, &pi) != cudaSuccess) break;
+        cudaGraph_t bodyInner = pi.conditional.phGraph_out[0];
+
+        if (cudaStreamBeginCaptureToGraph(cap, bodyInner, nullptr, nullptr, 0, cudaStreamCaptureModeThreadLocal) != cudaSuccess) break;
+        cudaError_t e3 = launch_march<K3<T>>(g, k3_args<T>(w, K, ch), cap);
+        cudaError_t e4 = launch_march<K4<T>>(g, k4_args<T>(w, K, ch), cap);
+        if (cudaStreamEndCapture(cap, &tmp) != cudaSuccess || e3 != cudaSuccess || e4 != cudaSuccess) break;
+        g_launches.fetch_sub(3, std::memory_order_relaxed);     // captured, not launched; counted from the device state
+
+        if (cudaGraphInstantiate(&exec, G, 0) != cudaSuccess) break;
+        if (cudaGraphLaunch(exec, st) != cudaSuccess) break;
+        rc = OMNI_OK;
+    } while (0);
+    if (rc != OMNI_OK) cudaGetLastError();
+    // an executable graph in flight is freed asynchronously on completion
+    if (exec) cudaGraphExecDestroy(exec);
+    if (G) cudaGraphDestroy(G);
+    if (cap) cudaStreamDestroy(cap);
+    return rc;
+}
+
+bool valid_common(int nx, int ny, int nz, double dx, double dy, double dz, double tol, int max_outer, int max_cg)
+{
+    if (nx < 1 || ny < 1 || nz < 1) return false;
+    if (!(dx > 0.0) || !(dy > 0.0) || !std::isfinite(dx) || !std::isfinite(dy)) return false;
+    if (nz > 1 && (!(dz > 0.0) || !std::isfinite(dz))) return false;
+    if (!(tol >= 0.0) || !std::isfinite(tol) || max_outer < 0 || max_cg < 0) return false;
+    return true;
+}
+
+template <typename T>
+int solve_ws(int nx, int ny, int nz, double dx, double dy, double dz, const T* gx, const T* gy, const T* gz,
+             const unsigned char* mask, T* P_out, double tol, int max_outer, int max_cg, void* ws, size_t ws_bytes,
+             void* stream, omni_info* info)
+{
+    Geom g;
+    if (!valid_common(nx, ny, nz, dx, dy, dz, tol, max_outer, max_cg) || !make_geom(nx, ny, nz, g)) return OMNI_ERR_INVALID_ARG;
+    if (!gx || !gy || (nz > 1 && !gz) || !P_out || !ws) return OMNI_ERR_INVALID_ARG;
+    if (((uintptr_t)ws & 255) != 0) return OMNI_ERR_INVALID_ARG;
+    if (ws_bytes < carve<T>(g, nullptr, nullptr)) return OMNI_ERR_ALLOC;
+    cudaStream_t st = (cudaStream_t)stream;
+    Workspace<T> w;
+    carve<T>(g, (char*)ws, &w);
+    HostConst H;
+    host_constants(nz, dx, dy, dz, H);
+    const Coef<T> K = make_coef<T>(H, dx, dy, dz);
+
+    init_scalars_kernel<<<1, 1, 0, st>>>(w.sc, tol, max_outer, max_cg);
+    CK(cudaGetLastError());
+    g_launches.fetch_add(1, std::memory_order_relaxed);
+    int rc = setup_codes<T>(g, w, gx, gy, gz, mask, st);
+    if (rc != OMNI_OK) return rc;
+    rc = launch_source<T>(g, w, K, gx, gy, gz, st);
+    if (rc != OMNI_OK) return rc;
+
+    const int mode = g_loop_mode.load();
+    rc = (mode == 1) ? run_loop_host<T>(g, w, H, K, max_outer, max_cg, st) : run_loop_graph<T>(g, w, H, K, st);
+    if (rc != OMNI_OK) return rc;
+
+    finalize_kernel<T><<<blocks_for((long long)nx * ny * nz, 256), 256, 0, st>>>(g, w.P, w.link, P_out);
+    CK(cudaGetLastError());
+    g_launches.fetch_add(1, std::memory_order_relaxed);
+
+    if (info) {
+        Scalars h;
+        CK(cudaMemcpyAsync(&h, w.sc, sizeof(Scalars), cudaMemcpyDeviceToHost, st));
+        CK(cudaStreamSynchronize(st));
+        info->outer_iters = h.n;
+        info->cg_iters_total = h.cg_total;
+        info->norm_S = std::sqrt(h.normS2);
+        info->eps_R_final = (h.normS2 > 0.0) ? std::sqrt(h.epsR2 / h.normS2) : 0.0;
+        info->status = h.status;
+        if (mode != 1) g_launches.fetch_add((long long)(h.normS2 > 0.0 ? h.n + 1 : 0) + 2 * h.cg_total, std::memory_order_relaxed);
+        return h.status;
+    }
+    return OMNI_OK;
+}
+
+template <typename T>
+int solve_alloc(int nx, int ny, int nz, double dx, double dy, double dz, const T* gx, const T* gy, const T* gz,
+                const unsigned char* mask, T* P_out, double tol, int max_outer, int max_cg, void* stream, omni_info* info)
+{
+    Geom g;
+    if (!valid_common(nx, ny, nz, dx, dy, dz, tol, max_outer, max_cg) || !make_geom(nx, ny, nz, g)) return OMNI_ERR_INVALID_ARG;
+    cudaStream_t st = (cudaStream_t)stream;
+    const size_t bytes = carve<T>(g, nullptr, nullptr);
+    void* ws = nullptr;
+    if (cudaMallocAsync(&ws, bytes, st) != cudaSuccess) { cudaGetLastError(); return OMNI_ERR_ALLOC; }
+    int rc = solve_ws<T>(nx, ny, nz, dx, dy, dz, gx, gy, gz, mask, P_out, tol, max_outer, max_cg, ws, bytes, stream, info);
+    cudaFreeAsync(ws, st);
+    return rc;
+}
+
+template <typename T>
+int solve_host(int nx, int ny, int nz, double dx, double dy, double dz, const T* gx, const T* gy, const T* gz,
+               const unsigned char* mask, T* P_out, double tol, int max_outer, int max_cg, void* stream, omni_info* info)
+{
+    Geom g;
+    if (!valid_common(nx, ny, nz, dx, dy, dz, tol, max_outer, max_cg) || !make_geom(nx, ny, nz, g)) return OMNI_ERR_INVALID_ARG;
+    if (!gx || !gy || (nz > 1 && !gz) || !P_out) return OMNI_ERR_INVALID_ARG;
+    cudaStream_t st = (cudaStream_t)stream;
+    const size_t n = (size_t)nx * ny * nz;
+    const int ncomp = (nz > 1) ? 3 : 2;
+    T* dbuf = nullptr;
+    uint8_t* dmask = nullptr;
+    if (cudaMallocAsync((void**)&dbuf, (ncomp + 1) * n * sizeof(T), st) != cudaSuccess) { cudaGetLastError(); return OMNI_ERR_ALLOC; }
+    if (mask && cudaMallocAsync((void**)&dmask, n, st) != cudaSuccess) { cudaGetLastError(); cudaFreeAsync(dbuf, st); return OMNI_ERR_ALLOC; }
+    int rc = OMNI_ERR_CUDA;
+    omni_info local;
+    do {
+        if (cudaMemcpyAsync(dbuf, gx, n * sizeof(T), cudaMemcpyHostToDevice, st) != cudaSuccess) break;
+        if (cudaMemcpyAsync(dbuf + n, gy, n * sizeof(T), cudaMemcpyHostToDevice, st) != cudaSuccess) break;
+        if (ncomp == 3 && cudaMemcpyAsync(dbuf + 2 * n, gz, n * sizeof(T), cudaMemcpyHostToDevice, st) != cudaSuccess) break;
+        if (mask && cudaMemcpyAsync(dmask, mask, n, cudaMemcpyHostToDevice, st) != cudaSuccess) break;
+        T* dP = dbuf + (size_t)ncomp * n;
+        rc = solve_alloc<T>(nx, ny, nz, dx, dy, dz, dbuf, dbuf + n, ncomp == 3 ? dbuf + 2 * n : nullptr, dmask, dP, tol,
+                            max_outer, max_cg, stream, &local);
+        if (rc < 0) break;
+        if (cudaMemcpyAsync(P_out, dP, n * sizeof(T), cudaMemcpyDeviceToHost, st) != cudaSuccess) { rc = OMNI_ERR_CUDA; break; }
+        if (cudaStreamSynchronize(st) != cudaSuccess) { rc = OMNI_ERR_CUDA; break; }
+        if (info) *info = local;
+    } while (0);
+    cudaFreeAsync(dbuf, st);
+    if (dmask) cudaFreeAsync(dmask, st);
+    if (rc == OMNI_ERR_CUDA) cudaGetLastError();
+    return rc;
+}
+
+// ------------------------------------------------------------------------------------------------ step entry points
+
+template <typename T>
+struct StepCtx {
+    Geom g; Workspace<T> w; HostConst H; Coef<T> K; void* ws; cudaStream_t st;
+};
+
+template <typename T>
+int step_begin(StepCtx<T>& c, int nx, int ny, int nz, double dx, double dy, double dz, const T* gx, const T* gy,
+               const T* gz, const unsigned char* mask, void* stream)
+{
+    if (!valid_common(nx, ny, nz, dx, dy, dz, 0.0, 0, 0) || !make_geom(nx, ny, nz, c.g)) return OMNI_ERR_INVALID_ARG;
+    c.st = (cudaStream_t)stream;
+    const size_t bytes = carve<T>(c.g, nullptr, nullptr);
+    c.ws = nullptr;
+    if (cudaMallocAsync(&c.ws, bytes, c.st) != cudaSuccess) { cudaGetLastError(); return OMNI_ERR_ALLOC; }
+    carve<T>(c.g, (char*)c.ws, &c.w);
+    host_constants(nz, dx, dy, dz, c.H);
+    c.K = make_coef<T>(c.H, dx, dy, dz);
+    init_scalars_kernel<<<1, 1, 0, c.st>>>(c.w.sc, 0.0, 0, 0);
+    g_launches.fetch_add(1, std::memory_order_relaxed);
+    int rc = setup_codes<T>(c.g, c.w, gx, gy, gz, mask, c.st);
+    return rc;
+}
+
+template <typename T>
+int step_end(StepCtx<T>& c, int rc, Scalars* h)
+{
+    if (rc == OMNI_OK && h) {
+        if (cudaMemcpyAsync(h, c.w.sc, sizeof(Scalars), cudaMemcpyDeviceToHost, c.st) != cudaSuccess) rc = OMNI_ERR_CUDA;
+    }
+    if (cudaStreamSynchronize(c.st) != cudaSuccess) rc = OMNI_ERR_CUDA;
+    if (c.ws) cudaFreeAsync(c.ws, c.st);
+    if (rc == OMNI_ERR_CUDA) cudaGetLastError();
+    return rc;
+}
+
+template <typename T>
+int source_step(int nx, int ny, int nz, double dx, double dy, double dz, const T* gx, const T* gy, const T* gz,
+                const unsigned char* mask, T* S_out, double* norm_S, void* stream)
+{
+    if (!gx || !gy || (nz > 1 && !gz) || !S_out) return OMNI_ERR_INVALID_ARG;
+    StepCtx<T> c;
+    int rc = step_begin<T>(c, nx, ny, nz, dx, dy, dz, gx, gy, gz, mask, stream);
+    if (rc == OMNI_ERR_INVALID_ARG || rc == OMNI_ERR_ALLOC) return rc;
+    Scalars h;
+    if (rc == OMNI_OK) rc = launch_source<T>(c.g, c.w, c.K, gx, gy, gz, c.st);
+    if (rc == OMNI_OK) {
+        pad_copy_kernel<T, T><<<blocks_for(c.g.npad, 256), 256, 0, c.st>>>(c.g, c.w.S, S_out, 0, c.w.link);
+        g_launches.fetch_add(1, std::memory_order_relaxed);
+        if (cudaGetLastError() != cudaSuccess) rc = OMNI_ERR_CUDA;
+    }
+    rc = step_end<T>(c, rc, &h);
+    if (rc == OMNI_OK && norm_S) *norm_S = std::sqrt(h.normS2);
+    return rc;
+}
+
+__global__ void force_go_kernel(Scalars* sc, double alpha)
+{
+    sc->inner_go = 1; sc->outer_go = 1; sc->k = 0; sc->alpha = alpha; sc->beta = 0.0;
+}
+
+template <typename T>
+int apply_M_step(int nx, int ny, int nz, double dx, double dy, double dz, const unsigned char* mask, const T* p, T* q,
+                 double* pq, void* stream)
+{
+    if (!p || !q) return OMNI_ERR_INVALID_ARG;
+    StepCtx<T> c;
+    int rc = step_begin<T>(c, nx, ny, nz, dx, dy, dz, (const T*)nullptr, (const T*)nullptr, (const T*)nullptr, mask, stream);
+    if (rc == OMNI_ERR_INVALID_ARG || rc == OMNI_ERR_ALLOC) return rc;
+    Scalars h;
+    if (rc == OMNI_OK) {
+        const unsigned nb = blocks_for(c.g.npad, 256);
+        pad_copy_kernel<T, T><<<nb, 256, 0, c.st>>>(c.g, p, c.w.p0, 1, c.w.link);
+        force_go_kernel<<<1, 1, 0, c.st>>>(c.w.sc, 0.0);
+        CondHandles ch{ 0, 0, 0 };
+        auto a4 = k4_args<T>(c.w, c.K, ch);
+        a4.pbuf[0] = c.w.p0; a4.pbuf[1] = c.w.p0;
+        a4.q_out = c.w.r;
+        cudaError_t e = launch_march<K4<T>>(c.g, a4, c.st);
+        pad_copy_kernel<T, T><<<nb, 256, 0, c.st>>>(c.g, c.w.r, q, 0, c.w.link);
+        g_launches.fetch_add(3, std::memory_order_relaxed);
+        if (e != cudaSuccess || cudaGetLastError() != cudaSuccess) rc = OMNI_ERR_CUDA;
+    }
+    rc = step_end<T>(c, rc, &h);
+    if (rc == OMNI_OK && pq) *pq = h.gamma;
+    return rc;
+}
+
+template <typename T>
+int residual_step(int nx, int ny, int nz, double dx, double dy, double dz, const T* gx, const T* gy, const T* gz,
+                  const unsigned char* mask, const double* P, T* r_out, double* eps_R, void* stream)
+{
+    if (!gx || !gy || (nz > 1 && !gz) || !P || !r_out) return OMNI_ERR_INVALID_ARG;
+    StepCtx<T> c;
+    int rc = step_begin<T>(c, nx, ny, nz, dx, dy, dz, gx, gy, gz, mask, stream);
+    if (rc == OMNI_ERR_INVALID_ARG || rc == OMNI_ERR_ALLOC) return rc;
+    Scalars h;
+    if (rc == OMNI_OK) rc = launch_source<T>(c.g, c.w, c.K, gx, gy, gz, c.st);
+    if (rc == OMNI_OK) {
+        const unsigned nb = blocks_for(c.g.npad, 256);
+        pad_copy_kernel<double, double><<<nb, 256, 0, c.st>>>(c.g, P, c.w.P, 1, c.w.link);
+        force_go_kernel<<<1, 1, 0, c.st>>>(c.w.sc, 0.0);
+        CondHandles ch{ 0, 0, 0 };
+        cudaError_t e = launch_march<K2<T>>(c.g, k2_args<T>(c.w, c.H, ch, 0), c.st);
+        pad_copy_kernel<T, T><<<nb, 256, 0, c.st>>>(c.g, c.w.r, r_out, 0, c.w.link);
+        g_launches.fetch_add(3, std::memory_order_relaxed);
+        if (e != cudaSuccess || cudaGetLastError() != cudaSuccess) rc = OMNI_ERR_CUDA;
+    }
+    rc = step_end<T>(c, rc, &h);
+    if (rc == OMNI_OK && eps_R) *eps_R = (h.normS2 > 0.0) ? std::sqrt(h.epsR2 / h.normS2) : 0.0;
+    return rc;
+}
+
+}  // namespace
+
+// ================================================================================================ C ABI
+
+extern "C" {
+
+int omni_solve_f64(int nx, int ny, int nz, double dx, double dy, double dz, const double* d_gx, const double* d_gy,
+                   const double* d_gz, const unsigned char* d_mask, double* d_P_out, double tol, int max_outer,
+                   int max_cg, void* stream, omni_info* info)
+{
+    if (!d_gx || !d_gy || (nz > 1 && !d_gz) || !d_P_out) return OMNI_ERR_INVALID_ARG;
+    return solve_alloc<double>(nx, ny, nz, dx, dy, dz, d_gx, d_gy, d_gz, d_mask, d_P_out, tol, max_outer, max_cg, stream, info);
+}
+
+int omni_solve_f32(int nx, int ny, int nz, double dx, double dy, double dz, const float* d_gx, const float* d_gy,
+                   const float* d_gz, const unsigned char* d_mask, float* d_P_out, double tol, int max_outer,
+                   int max_cg, void* stream, omni_info* info)
+{
+    if (!d_gx || !d_gy || (nz > 1 && !d_gz) || !d_P_out) return OMNI_ERR_INVALID_ARG;
+    return solve_alloc<float>(nx, ny, nz, dx, dy, dz, d_gx, d_gy, d_gz, d_mask, d_P_out, tol, max_outer, max_cg, stream, info);
+}
+
+size_t omni_workspace_bytes(int nx, int ny, int nz, int dtype)
+{
+    Geom g;
+    if (!make_geom(nx, ny, nz, g)) return 0;
+    if (dtype == OMNI_F32) return carve<float>(g, nullptr, nullptr);
+    if (dtype == OMNI_F64) return carve<double>(g, nullptr, nullptr);
+    return 0;
+}
+
+int omni_solve_f64_ws(int nx, int ny, int nz, double dx, double dy, double dz, const double* d_gx, const double* d_gy,
+                      const double* d_gz, const unsigned char* d_mask, double* d_P_out, double tol, int max_outer,
+                      int max_cg, void* d_workspace, size_t workspace_bytes, void* stream, omni_info* info)
+{
+    return solve_ws<double>(nx, ny, nz, dx, dy, dz, d_gx, d_gy, d_gz, d_mask, d_P_out, tol, max_outer, max_cg, d_workspace,
+                            workspace_bytes, stream, info);
+}
+
+int omni_solve_f32_ws(int nx, int ny, int nz, double dx, double dy, double dz, const float* d_gx, const float* d_gy,
+                      const float* d_gz, const unsigned char* d_mask, float* d_P_out, double tol, int max_outer,
+                      int max_cg, void* d_workspace, size_t workspace_bytes, void* stream, omni_info* info)
+{
+    return solve_ws<float>(nx, ny, nz, dx, dy, dz, d_gx, d_gy, d_gz, d_mask, d_P_out, tol, max_outer, max_cg, d_workspace,
+                           workspace_bytes, stream, info);
+}
+
+int omni_solve_host_f64(int nx, int ny, int nz, double dx, double dy, double dz, const double* h_gx, const double* h_gy,
+                        const double* h_gz, const unsigned char* h_mask, double* h_P_out, double tol, int max_outer,
+                        int max_cg, void* stream, omni_info* info)
+{
+    return solve_host<double>(nx, ny, nz, dx, dy, dz, h_gx, h_gy, h_gz, h_mask, h_P_out, tol, max_outer, max_cg, stream, info);
+}
+
+int omni_solve_host_f32(int nx, int ny, int nz, double dx, double dy, double dz, const float* h_gx, const float* h_gy,
+                        const float* h_gz, const unsigned char* h_mask, float* h_P_out, double tol, int max_outer,
+                        int max_cg, void* stream, omni_info* info)
+{
+    return solve_host<float>(nx, ny, nz, dx, dy, dz, h_gx, h_gy, h_gz, h_mask, h_P_out, tol, max_outer, max_cg, stream, info);
+}
+
+int omni_constants(int nx, int ny, int nz, double dx, double dy, double dz, double* h_out13)
+{
+    if (!h_out13 || !valid_common(nx, ny, nz, dx, dy, dz, 0.0, 0, 0)) return OMNI_ERR_INVALID_ARG;
+    HostConst H;
+    host_constants(nz, dx, dy, dz, H);
+    h_out13[0] = H.F[0]; h_out13[1] = H.F[1]; h_out13[2] = H.F[2]; h_out13[3] = H.Atot;
+    for (int a = 0; a < 3; ++a)
+        for (int b = 0; b < 3; ++b) h_out13[4 + 3 * a + b] = H.c[a][b];
+    return OMNI_OK;
+}
+
+int omni_source_f64(int nx, int ny, int nz, double dx, double dy, double dz, const double* d_gx, const double* d_gy,
+                    const double* d_gz, const unsigned char* d_mask, double* d_S_out, double* h_norm_S, void* stream)
+{
+    return source_step<double>(nx, ny, nz, dx, dy, dz, d_gx, d_gy, d_gz, d_mask, d_S_out, h_norm_S, stream);
+}
+int omni_source_f32(int nx, int ny, int nz, double dx, double dy, double dz, const float* d_gx, const float* d_gy,
+                    const float* d_gz, const unsigned char* d_mask, float* d_S_out, double* h_norm_S, void* stream)
+{
+    return source_step<float>(nx, ny, nz, dx, dy, dz, d_gx, d_gy, d_gz, d_mask, d_S_out, h_norm_S, stream);
+}
+
+int omni_apply_M_f64(int nx, int ny, int nz, double dx, double dy, double dz, const unsigned char* d_mask,
+                     const double* d_p, double* d_q, double* h_pq, void* stream)
+{
+    return apply_M_step<double>(nx, ny, nz, dx, dy, dz, d_mask, d_p, d_q, h_pq, stream);
+}
+int omni_apply_M_f32(int nx, int ny, int nz, double dx, double dy, double dz, const unsigned char* d_mask,
+                     const float* d_p, float* d_q, double* h_pq, void* stream)
+{
+    return apply_M_step<float>(nx, ny, nz, dx, dy, dz, d_mask, d_p, d_q, h_pq, stream);
+}
+
+int omni_residual_f64(int nx, int ny, int nz, double dx, double dy, double dz, const double* d_gx, const double* d_gy,
+                      const double* d_gz, const unsigned char* d_mask, const double* d_P, double* d_r_out,
+                      double* h_eps_R, void* stream)
+{
+    return residual_step<double>(nx, ny, nz, dx, dy, dz, d_gx, d_gy, d_gz, d_mask, d_P, d_r_out, h_eps_R, stream);
+}
+int omni_residual_f32(int nx, int ny, int nz, double dx, double dy, double dz, const float* d_gx, const float* d_gy,
+                      const float* d_gz, const unsigned char* d_mask, const double* d_P, float* d_r_out,
+                      double* h_eps_R, void* stream)
+{
+    return residual_step<float>(nx, ny, nz, dx, dy, dz, d_gx, d_gy, d_gz, d_mask, d_P, d_r_out, h_eps_R, stream);
+}
+
+long long omni_launch_count(int reset)
+{
+    return reset ? g_launches.exchange(0) : g_launches.load();
+}
+
+int omni_set_loop_mode(int mode)
+{
+    if (mode != 0 && mode != 1) return g_loop_mode.load();
+    return g_loop_mode.exchange(mode);
+}
+
+const char* omni_status_string(int status)
+{
+    switch (status) {
+    case OMNI_OK: return "ok";
+    case OMNI_NOT_CONVERGED: return "not converged: max_outer reached (last iterate written)";
+    case OMNI_ERR_INVALID_ARG: return "invalid argument";
+    case OMNI_ERR_CUDA: return "CUDA runtime error (or no CUDA device)";
+    case OMNI_ERR_ALLOC: return "workspace allocation failed or workspace too small";
+    case OMNI_ERR_BREAKDOWN: return "CG breakdown: non-finite scalar or p.Mp <= 0";
+    default: return "unknown status";
+    }
+}
+
+int omni_version(void) { return 100; }
+
+}  // extern "C"

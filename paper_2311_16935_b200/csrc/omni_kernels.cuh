@@ -1,0 +1,707 @@
+// omni_kernels.cuh -- sm_100a kernels of the matrix-based omnidirectional pressure integration hot path.
+// Zigunov & Charonko, arXiv 2311.16935 (citations: PAPER.md:<line>); notation of DESIGN.md section 2.
+//
+//   K0a validity, K0b stencil codes + interior flags        (Eq. 13 :176; Eq. 16/18/19/20 :202-227; Eq. 25 :266)
+//   K1  source vector S + ||S||^2                              (last sum of Eq. 9 :100; Eq. 49-50 :656)
+//   K2  outer boundary update: P += delta, r = S - L P, eps_R  (Eq. 12 :119; Eq. 41 :442; Alg. 1 :141-148)
+//   K3  p = r + beta p (fused), gamma = p . M p                (CG, :124)
+//   K4  q = M p recomputed, delta += alpha p, r -= alpha q, rho' = r.r
+//   K7  P_out with NaN at missing cells                        (:158)
+// K2/K3/K4 share one z-marching tile engine (march_kernel): a CTA owns a (32*V cells) x (TYR-2 rows) column of the
+// grid, streams it plane by plane with a register pipeline (planes k-1, k, k+1), exchanges the current plane's y
+// neighbours through shared memory and its x neighbours by warp shuffles, and finishes with a deterministic
+// grid-wide reduction (fixed-slot partials + last-arriving CTA) whose scalars stay on the device.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <string.h>
+
+namespace omni {
+
+struct Geom {
+    int nx, ny, nz;      // logical grid
+    int px;              // padded row pitch in cells (multiple of 8); cells nx..px-1 are permanently missing
+    long long pplane;    // px * ny
+    long long npad;      // px * ny * nz
+};
+
+// stencil coefficients, already divided by A_tot (Eq. 10 :109), in the arithmetic type T
+template <typename T>
+struct Coef {
+    T t[3];    // F_a / A_tot: weight of a fully interior link (Eq. 5 :75 / Eq. 23 :258); also the L-operator weight
+    T caa[3];  // c_aa / A_tot         far-face constant       (Eq. 17 :207 / Eq. 32 :314)
+    T cab[3];  // c_{a,(a+1)%3} / A_tot  side-face constants   (Eq. 17 / Eq. 33 :317)
+    T cac[3];  // c_{a,(a+2)%3} / A_tot
+    T hs[3];   // Delta_a * t_a / 2: face-average factor of the source term (Eq. 9 :100)
+};
+
+// device-resident loop state: no scalar ever visits the host inside the iteration
+struct Scalars {
+    double rho, gamma, alpha, beta;
+    double normS2;     // ||S||^2
+    double thresh2;    // (0.1 * tol)^2 * ||S||^2   inner stop (A3)
+    double tol2S;      // tol^2 * ||S||^2           outer stop (Eq. 41)
+    double epsR2;      // ||r0||^2 of the last outer check
+    double tol;
+    long long cg_total;
+    int k;             // CG iteration index inside the current outer iteration
+    int n;             // outer iterations done
+    int inner_go, outer_go;
+    int status;        // omni_status
+    int max_cg, max_outer;
+    unsigned int ticket[4];
+};
+
+struct CondHandles {
+    unsigned long long h_outer, h_inner;   // cudaGraphConditionalHandle
+    int use;                               // 1 inside the conditional-node graph
+};
+
+enum { ST_OK = 0, ST_NOT_CONVERGED = 1, ST_BREAKDOWN = -4 };
+
+// per-cell code layout.  wcode: for direction d (0..5 = E W N S F B, axis a = d/2) bits [5d, 5d+5) hold
+// far (1 bit: v(Q+d)), nb (2 bits: v(Q+e_b)+v(Q-e_b), b=(a+1)%3), nc (2 bits, c=(a+2)%3), all zero when the link is
+// absent; bit 30 = cell valid.  link: bits 0..5 = v(C+d), bit 6 = cell valid.
+constexpr uint32_t WCODE_VALID = 1u << 30;
+constexpr uint8_t LINK_VALID = 1u << 6;
+
+// ------------------------------------------------------------------------------------------------ small helpers
+
+template <typename T, int V>
+__device__ __forceinline__ void ld_chunk(const T* __restrict__ p, T (&v)[V])
+{
+    constexpr int NV = V * (int)sizeof(T) / 16;
+    static_assert(NV * 16 == V * (int)sizeof(T), "chunk must be a multiple of 16 bytes");
+    uint4 u[NV];
+#pragma unroll
+    for (int i = 0; i < NV; ++i) u[i] = reinterpret_cast<const uint4*>(p)[i];
+    memcpy(v, u, sizeof(u));
+}
+
+template <typename T, int V>
+__device__ __forceinline__ void st_chunk(T* __restrict__ p, const T (&v)[V])
+{
+    constexpr int NV = V * (int)sizeof(T) / 16;
+    uint4 u[NV];
+    memcpy(u, v, sizeof(u));
+#pragma unroll
+    for (int i = 0; i < NV; ++i) reinterpret_cast<uint4*>(p)[i] = u[i];
+}
+
+template <typename T, int V>
+__device__ __forceinline__ void zero_chunk(T (&v)[V])
+{
+#pragma unroll
+    for (int i = 0; i < V; ++i) v[i] = T(0);
+}
+
+__device__ __forceinline__ double warp_sum(double v)
+{
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+
+// weight of one link from its 5 code bits (Eq. 16/19 :202/:223, Eq. 25 :266, divided by A_tot)
+template <typename T>
+__device__ __forceinline__ T link_weight(uint32_t bits, const Coef<T>& K, int a)
+{
+    return T(bits & 1u) * K.caa[a] + T((bits >> 1) & 3u) * K.cab[a] + T((bits >> 3) & 3u) * K.cac[a];
+}
+
+// (M p)_C = p_C - sum_d w1_d p_{C+d}   (Eq. 9 rearranged, A1); general (coded) cell
+template <typename T>
+__device__ __forceinline__ T apply_M_coded(uint32_t code, T c, T e, T w, T n, T s, T f, T b, const Coef<T>& K)
+{
+    if (!(code & WCODE_VALID)) return T(0);
+    T acc = c;
+    acc -= link_weight(code, K, 0) * e;
+    acc -= link_weight(code >> 5, K, 0) * w;
+    acc -= link_weight(code >> 10, K, 1) * n;
+    acc -= link_weight(code >> 15, K, 1) * s;
+    acc -= link_weight(code >> 20, K, 2) * f;
+    acc -= link_weight(code >> 25, K, 2) * b;
+    return acc;
+}
+
+// interior cell: every link carries its full face share t_a (Eq. 5 :75: A^{n+1} = F_a, A^n = 0)
+template <typename T>
+__device__ __forceinline__ T apply_M_interior(T c, T e, T w, T n, T s, T f, T b, const Coef<T>& K)
+{
+    return c - K.t[0] * (e + w) - K.t[1] * (n + s) - K.t[2] * (f + b);
+}
+
+// q = M p for the V cells of one thread; fb = interior-flag bits of the thread's 4-cell groups (0 = all interior)
+template <typename T, int V>
+__device__ __forceinline__ void apply_M_chunk(T (&q)[V], const T (&vm)[V], const T (&vc)[V], const T (&vp)[V],
+                                              const T (&vn)[V], const T (&vs)[V], T xl, T xr, uint32_t fb,
+                                              const uint32_t* __restrict__ wcode, long long idx, const Coef<T>& K)
+{
+    if (fb == 0) {
+#pragma unroll
+        for (int i = 0; i < V; ++i) {
+            T w = (i == 0) ? xl : vc[i - 1];
+            T e = (i == V - 1) ? xr : vc[i + 1];
+            q[i] = apply_M_interior(vc[i], e, w, vn[i], vs[i], vp[i], vm[i], K);
+        }
+    } else {
+        uint32_t code[V];
+        ld_chunk<uint32_t, V>(wcode + idx, code);
+#pragma unroll
+        for (int i = 0; i < V; ++i) {
+            T w = (i == 0) ? xl : vc[i - 1];
+            T e = (i == V - 1) ? xr : vc[i + 1];
+            q[i] = apply_M_coded(code[i], vc[i], e, w, vn[i], vs[i], vp[i], vm[i], K);
+        }
+    }
+}
+
+// interior-flag bits of the V/4 groups starting at padded cell idx (one bit per 4 cells, global linear bit index)
+template <int V>
+__device__ __forceinline__ uint32_t flag_bits(const uint32_t* __restrict__ flags, long long idx)
+{
+    long long g = idx >> 2;
+    return (flags[g >> 5] >> (unsigned)(g & 31)) & ((1u << (V / 4)) - 1u);
+}
+
+// ------------------------------------------------------------------------------------------------ tile engine
+//
+// Op supplies: VT (value type of the stencil input), V (cells per thread, 32 bytes of the widest streamed array),
+// TYR (rows per CTA incl. the two halo rows), MINB, NACC, TICKET, Args, Ctx, Raw (+ load / convert), Extra
+// (+ load_extra), emit, active, finalize.
+
+template <class Op>
+__global__ void __launch_bounds__(32 * Op::TYR, Op::MINB)
+march_kernel(const Geom g, const int zlen, const typename Op::Args a)
+{
+    using VT = typename Op::VT;
+    constexpr int V = Op::V, TYR = Op::TYR, TYO = TYR - 2, W = 32 * V, NACC = Op::NACC;
+    __shared__ __align__(16) VT sm[2][TYR][W];
+    __shared__ double red[NACC][TYR];
+    __shared__ int is_last;
+
+    if (!Op::active(a)) return;
+
+    const int lane = threadIdx.x, ty = threadIdx.y;
+    const int x = blockIdx.x * W + lane * V;
+    const int j = blockIdx.y * TYO + ty - 1;
+    const int k0 = blockIdx.z * zlen;
+    const int k1 = min(g.nz, k0 + zlen);
+    const bool ldok = (x < g.px) && (j >= 0) && (j < g.ny);
+    const bool outrow = ldok && (ty >= 1) && (ty <= TYO);
+    const bool lok = ldok && (lane == 0) && (x > 0);
+    const bool rok = ldok && (lane == 31) && (x + V < g.px);
+    const long long rowbase = (long long)j * g.px + x;
+
+    const typename Op::Ctx ctx(a);
+    VT vm[V], vc[V], vp[V], hlc, hrc, hlp, hrp;
+    typename Op::Raw raw;
+    typename Op::Extra exc, exn;
+    double acc[NACC];
+#pragma unroll
+    for (int i = 0; i < NACC; ++i) acc[i] = 0.0;
+
+    {   // prologue: planes k0-1, k0, k0+1
+        VT d0, d1;
+        Op::load(raw, a, ctx, rowbase + (long long)(k0 - 1) * g.pplane, ldok && k0 > 0, false, false);
+        Op::convert(raw, ctx, vm, d0, d1);
+        Op::load(raw, a, ctx, rowbase + (long long)k0 * g.pplane, ldok, lok, rok);
+        Op::convert(raw, ctx, vc, hlc, hrc);
+        Op::load(raw, a, ctx, rowbase + (long long)(k0 + 1) * g.pplane, ldok && (k0 + 1 < g.nz), lok && (k0 + 1 < g.nz),
+                 rok && (k0 + 1 < g.nz));
+        Op::convert(raw, ctx, vp, hlp, hrp);
+        Op::load_extra(exc, a, rowbase + (long long)k0 * g.pplane, outrow);
+    }
+
+    int buf = 0;
+    for (int k = k0; k < k1; ++k) {
+        const long long idx = rowbase + (long long)k * g.pplane;
+        // prefetch plane k+2 (needed as plane k+1 of the next step; the plane after the segment is its halo)
+        const bool nxt = (k + 2 <= k1) && (k + 2 < g.nz);
+        Op::load(raw, a, ctx, idx + 2 * g.pplane, ldok && nxt, lok && nxt, rok && nxt);
+        Op::load_extra(exn, a, idx + g.pplane, outrow && (k + 1 < k1));
+
+        st_chunk<VT, V>(&sm[buf][ty][lane * V], vc);
+        __syncthreads();
+
+        VT xl = __shfl_up_sync(0xffffffffu, vc[V - 1], 1);
+        VT xr = __shfl_down_sync(0xffffffffu, vc[0], 1);
+        if (lane == 0) xl = hlc;
+        if (lane == 31) xr = hrc;
+
+        if (outrow) {
+            VT vn[V], vs[V];
+            ld_chunk<VT, V>(&sm[buf][ty + 1][lane * V], vn);
+            ld_chunk<VT, V>(&sm[buf][ty - 1][lane * V], vs);
+            Op::emit(a, ctx, idx, vm, vc, vp, vn, vs, xl, xr, exc, acc);
+        }
+#pragma unroll
+        for (int i = 0; i < V; ++i) { vm[i] = vc[i]; vc[i] = vp[i]; }
+        hlc = hlp; hrc = hrp;
+        Op::convert(raw, ctx, vp, hlp, hrp);
+        exc = exn;
+        buf ^= 1;
+    }
+
+    // deterministic grid reduction: CTA partial -> fixed slot -> last-arriving CTA sums all slots in slot order
+    const int tid = ty * 32 + lane, nthr = 32 * TYR;
+    const unsigned int nblk = gridDim.x * gridDim.y * gridDim.z;
+    const unsigned int bid = blockIdx.x + gridDim.x * (blockIdx.y + gridDim.y * blockIdx.z);
+#pragma unroll
+    for (int i = 0; i < NACC; ++i) {
+        double s = warp_sum(acc[i]);
+        if (lane == 0) red[i][ty] = s;
+    }
+    __syncthreads();
+    if (tid == 0) {
+#pragma unroll
+        for (int i = 0; i < NACC; ++i) {
+            double s = 0.0;
+            for (int w = 0; w < TYR; ++w) s += red[i][w];
+            a.partial[(size_t)i * nblk + bid] = s;
+        }
+        __threadfence();
+        unsigned int t = atomicAdd(&a.sc->ticket[Op::TICKET], 1u);
+        is_last = (t == nblk - 1);
+    }
+    __syncthreads();
+    if (is_last) {
+        __threadfence();
+        double tot[NACC];
+#pragma unroll
+        for (int i = 0; i < NACC; ++i) {
+            double s = 0.0;
+            for (unsigned int b = tid; b < nblk; b += nthr) s += __ldcg(&a.partial[(size_t)i * nblk + b]);
+            s = warp_sum(s);
+            __syncthreads();
+            if (lane == 0) red[i][ty] = s;
+            __syncthreads();
+            s = 0.0;
+            for (int w = 0; w < TYR; ++w) s += red[i][w];
+            tot[i] = s;
+        }
+        if (tid == 0) {
+            a.sc->ticket[Op::TICKET] = 0;
+            Op::finalize(a, tot);
+        }
+    }
+}
+
+__device__ __forceinline__ void set_cond(const CondHandles& h, int outer, int inner)
+{
+#if defined(__CUDA_ARCH__)
+    if (h.use) {
+        if (outer >= 0) cudaGraphSetConditional((cudaGraphConditionalHandle)h.h_outer, (unsigned)outer);
+        if (inner >= 0) cudaGraphSetConditional((cudaGraphConditionalHandle)h.h_inner, (unsigned)inner);
+    }
+#endif
+}
+
+// ------------------------------------------------------------------------------------------------ K3
+// p_new = r + beta p_old on the fly (also in the halo), store p_new, gamma = p_new . M p_new; alpha = rho / gamma.
+template <typename T, int TYR_, int MINB_>
+struct OpK3 {
+    using VT = T;
+    enum { V = 32 / sizeof(T), TYR = TYR_, MINB = MINB_, NACC = 1, TICKET = 0 };
+    struct Args {
+        const T* r; T* pbuf[2]; const uint32_t* wcode; const uint32_t* flags;
+        Coef<T> K; Scalars* sc; double* partial; CondHandles cond;
+    };
+    struct Ctx {
+        T beta; const T* pold; T* pnew;
+        __device__ Ctx(const Args& a)
+        {
+            beta = (T)a.sc->beta;
+            int par = a.sc->k & 1;
+            pold = a.pbuf[par]; pnew = a.pbuf[par ^ 1];
+        }
+    };
+    struct Raw { T r[V], p[V], rl, pl, rr, pr; };
+    struct Extra {};
+    __device__ static bool active(const Args& a) { return a.sc->inner_go != 0; }
+    __device__ static void load(Raw& w, const Args& a, const Ctx& c, long long idx, bool ok, bool lok, bool rok)
+    {
+        if (ok) { ld_chunk<T, V>(a.r + idx, w.r); ld_chunk<T, V>(c.pold + idx, w.p); }
+        else { zero_chunk<T, V>(w.r); zero_chunk<T, V>(w.p); }
+        w.rl = lok ? a.r[idx - 1] : T(0); w.pl = lok ? c.pold[idx - 1] : T(0);
+        w.rr = rok ? a.r[idx + V] : T(0); w.pr = rok ? c.pold[idx + V] : T(0);
+    }
+    __device__ static void convert(const Raw& w, const Ctx& c, T (&v)[V], T& hl, T& hr)
+    {
+#pragma unroll
+        for (int i = 0; i < V; ++i) v[i] = w.r[i] + c.beta * w.p[i];
+        hl = w.rl + c.beta * w.pl;
+        hr = w.rr + c.beta * w.pr;
+    }
+    __device__ static void load_extra(Extra&, const Args&, long long, bool) {}
+    __device__ static void emit(const Args& a, const Ctx& c, long long idx, const T (&vm)[V], const T (&vc)[V],
+                                const T (&vp)[V], const T (&vn)[V], const T (&vs)[V], T xl, T xr, const Extra&,
+                                double (&acc)[1])
+    {
+        st_chunk<T, V>(c.pnew + idx, vc);
+        T q[V];
+        apply_M_chunk<T, V>(q, vm, vc, vp, vn, vs, xl, xr, flag_bits<V>(a.flags, idx), a.wcode, idx, a.K);
+#pragma unroll
+        for (int i = 0; i < V; ++i) acc[0] += (double)vc[i] * (double)q[i];
+    }
+    __device__ static void finalize(const Args& a, const double (&tot)[1])
+    {
+        Scalars* s = a.sc;
+        double gamma = tot[0];
+        s->gamma = gamma;
+        if (!(gamma > 0.0) || !isfinite(gamma)) {      // also catches NaN
+            s->status = ST_BREAKDOWN; s->inner_go = 0; s->outer_go = 0;
+            set_cond(a.cond, 0, 0);
+        } else {
+            s->alpha = s->rho / gamma;
+        }
+    }
+};
+
+// ------------------------------------------------------------------------------------------------ K4
+// q = M p recomputed from p (never stored), delta += alpha p, r -= alpha q, rho' = r.r; beta = rho'/rho; loop test.
+template <typename T, int TYR_, int MINB_>
+struct OpK4 {
+    using VT = T;
+    enum { V = 32 / sizeof(T), TYR = TYR_, MINB = MINB_, NACC = 1, TICKET = 1 };
+    struct Args {
+        T* r; T* delta; const T* pbuf[2]; const uint32_t* wcode; const uint32_t* flags;
+        Coef<T> K; Scalars* sc; double* partial; CondHandles cond;
+        T* q_out;        // only for omni_apply_M: store q, leave r/delta untouched (NULL inside the solve)
+    };
+    struct Ctx {
+        T alpha; const T* p; bool first;
+        __device__ Ctx(const Args& a)
+        {
+            alpha = (T)a.sc->alpha;
+            first = (a.sc->k == 0);
+            p = a.pbuf[(a.sc->k & 1) ^ 1];
+        }
+    };
+    struct Raw { T p[V], pl, pr; };
+    struct Extra { T r[V], d[V]; };
+    __device__ static bool active(const Args& a) { return a.sc->inner_go != 0; }
+    __device__ static void load(Raw& w, const Args&, const Ctx& c, long long idx, bool ok, bool lok, bool rok)
+    {
+        if (ok) ld_chunk<T, V>(c.p + idx, w.p); else zero_chunk<T, V>(w.p);
+        w.pl = lok ? c.p[idx - 1] : T(0);
+        w.pr = rok ? c.p[idx + V] : T(0);
+    }
+    __device__ static void convert(const Raw& w, const Ctx&, T (&v)[V], T& hl, T& hr)
+    {
+#pragma unroll
+        for (int i = 0; i < V; ++i) v[i] = w.p[i];
+        hl = w.pl; hr = w.pr;
+    }
+    __device__ static void load_extra(Extra& e, const Args& a, long long idx, bool ok)
+    {
+        if (ok && a.q_out == nullptr) { ld_chunk<T, V>(a.r + idx, e.r); ld_chunk<T, V>(a.delta + idx, e.d); }
+        else { zero_chunk<T, V>(e.r); zero_chunk<T, V>(e.d); }
+    }
+    __device__ static void emit(const Args& a, const Ctx& c, long long idx, const T (&vm)[V], const T (&vc)[V],
+                                const T (&vp)[V], const T (&vn)[V], const T (&vs)[V], T xl, T xr, const Extra& e,
+                                double (&acc)[1])
+    {
+        T q[V];
+        apply_M_chunk<T, V>(q, vm, vc, vp, vn, vs, xl, xr, flag_bits<V>(a.flags, idx), a.wcode, idx, a.K);
+        if (a.q_out != nullptr) {           // operator-only mode (omni_apply_M): q and p.q
+            st_chunk<T, V>(a.q_out + idx, q);
+#pragma unroll
+            for (int i = 0; i < V; ++i) acc[0] += (double)vc[i] * (double)q[i];
+            return;
+        }
+        T rn[V], dn[V];
+#pragma unroll
+        for (int i = 0; i < V; ++i) {
+            rn[i] = e.r[i] - c.alpha * q[i];
+            dn[i] = (c.first ? T(0) : e.d[i]) + c.alpha * vc[i];
+            acc[0] += (double)rn[i] * (double)rn[i];
+        }
+        st_chunk<T, V>(a.r + idx, rn);
+        st_chunk<T, V>(a.delta + idx, dn);
+    }
+    __device__ static void finalize(const Args& a, const double (&tot)[1])
+    {
+        Scalars* s = a.sc;
+        if (a.q_out != nullptr) { s->gamma = tot[0]; return; }
+        double rho1 = tot[0];
+        if (!isfinite(rho1)) {
+            s->status = ST_BREAKDOWN; s->inner_go = 0; s->outer_go = 0;
+            set_cond(a.cond, 0, 0);
+            return;
+        }
+        s->beta = rho1 / s->rho;
+        s->rho = rho1;
+        s->k += 1;
+        s->cg_total += 1;
+        int go = (rho1 > s->thresh2) && (rho1 != 0.0) && (s->k < s->max_cg);
+        s->inner_go = go;
+        set_cond(a.cond, -1, go);
+    }
+};
+
+// ------------------------------------------------------------------------------------------------ K2
+// outer boundary update (Eq. 12 collapsed): P <- P + delta; r0 = S - L P with
+// (L P)_C = sum_d v(C+d) t_a (P_C - P_{C+d}) = ([W^{n+1}] - [W^n]) P; eps_R^2 ||S||^2 = ||r0||^2 (Eq. 41).
+// P is always fp64 (master pressure, A9); delta, S, r are T.
+template <typename T, int TYR_, int MINB_>
+struct OpK2 {
+    using VT = double;
+    enum { V = 4, TYR = TYR_, MINB = MINB_, NACC = 2, TICKET = 2 };
+    struct Args {
+        double* P; const T* delta; const T* S; T* r; const uint8_t* link; const uint32_t* flags;
+        double t[3]; Scalars* sc; double* partial; CondHandles cond;
+        int fold_delta;   // 0: residual of P as given (omni_residual); 1: inside the solve
+    };
+    struct Ctx { __device__ Ctx(const Args&) {} };
+    struct Raw { double P[V]; T d[V]; double Pl, Pr; T dl, dr; };
+    struct Extra { T S[V]; };
+    __device__ static bool active(const Args& a) { return a.sc->outer_go != 0; }
+    __device__ static void load(Raw& w, const Args& a, const Ctx&, long long idx, bool ok, bool lok, bool rok)
+    {
+        if (ok) { ld_chunk<double, V>(a.P + idx, w.P); ld_chunk<T, V>(a.delta + idx, w.d); }
+        else { zero_chunk<double, V>(w.P); zero_chunk<T, V>(w.d); }
+        w.Pl = lok ? a.P[idx - 1] : 0.0; w.dl = lok ? a.delta[idx - 1] : T(0);
+        w.Pr = rok ? a.P[idx + V] : 0.0; w.dr = rok ? a.delta[idx + V] : T(0);
+    }
+    __device__ static void convert(const Raw& w, const Ctx&, double (&v)[V], double& hl, double& hr)
+    {
+#pragma unroll
+        for (int i = 0; i < V; ++i) v[i] = w.P[i] + (double)w.d[i];
+        hl = w.Pl + (double)w.dl;
+        hr = w.Pr + (double)w.dr;
+    }
+    __device__ static void load_extra(Extra& e, const Args& a, long long idx, bool ok)
+    {
+        if (ok) ld_chunk<T, V>(a.S + idx, e.S); else zero_chunk<T, V>(e.S);
+    }
+    __device__ static void emit(const Args& a, const Ctx&, long long idx, const double (&vm)[V], const double (&vc)[V],
+                                const double (&vp)[V], const double (&vn)[V], const double (&vs)[V], double xl,
+                                double xr, const Extra& e, double (&acc)[2])
+    {
+        if (a.fold_delta) st_chunk<double, V>(a.P + idx, vc);
+        uint32_t fb = flag_bits<V>(a.flags, idx);
+        uint32_t lk = 0x7f7f7f7fu;
+        if (fb) lk = *reinterpret_cast<const uint32_t*>(a.link + idx);
+        T rn[V];
+#pragma unroll
+        for (int i = 0; i < V; ++i) {
+            double w = (i == 0) ? xl : vc[i - 1];
+            double ee = (i == V - 1) ? xr : vc[i + 1];
+            uint32_t l = (lk >> (8 * i)) & 0xffu;
+            double LP = 0.0;
+            if (l & 1u) LP += a.t[0] * (vc[i] - ee);
+            if (l & 2u) LP += a.t[0] * (vc[i] - w);
+            if (l & 4u) LP += a.t[1] * (vc[i] - vn[i]);
+            if (l & 8u) LP += a.t[1] * (vc[i] - vs[i]);
+            if (l & 16u) LP += a.t[2] * (vc[i] - vp[i]);
+            if (l & 32u) LP += a.t[2] * (vc[i] - vm[i]);
+            double rr = (l & LINK_VALID) ? ((double)e.S[i] - LP) : 0.0;
+            rn[i] = (T)rr;
+            acc[0] += rr * rr;
+            acc[1] += (double)rn[i] * (double)rn[i];
+        }
+        st_chunk<T, V>(a.r + idx, rn);
+    }
+    __device__ static void finalize(const Args& a, const double (&tot)[2])
+    {
+        Scalars* s = a.sc;
+        s->epsR2 = tot[0];
+        if (!a.fold_delta) return;
+        if (!isfinite(tot[0])) {
+            s->status = ST_BREAKDOWN; s->inner_go = 0; s->outer_go = 0;
+            set_cond(a.cond, 0, 0);
+            return;
+        }
+        if (tot[0] <= s->tol2S || s->n >= s->max_outer) {
+            s->status = (tot[0] <= s->tol2S) ? ST_OK : ST_NOT_CONVERGED;
+            s->inner_go = 0; s->outer_go = 0;
+            set_cond(a.cond, 0, 0);
+            return;
+        }
+        s->n += 1;
+        s->k = 0;
+        s->beta = 0.0;
+        s->rho = tot[1];
+        int go = (tot[1] > s->thresh2) && (tot[1] != 0.0) && (s->max_cg > 0);
+        s->inner_go = go;
+        set_cond(a.cond, 1, go);
+    }
+};
+
+// ------------------------------------------------------------------------------------------------ K0a validity
+template <typename T>
+__global__ void validity_kernel(Geom g, const T* __restrict__ gx, const T* __restrict__ gy, const T* __restrict__ gz,
+                                const uint8_t* __restrict__ mask, uint8_t* __restrict__ vbyte)
+{
+    long long pid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (pid >= g.npad) return;
+    int i = (int)(pid % g.px);
+    long long row = pid / g.px;                   // j + ny*k
+    uint8_t ok = 0;
+    if (i < g.nx) {
+        long long u = row * g.nx + i;             // user-layout index
+        ok = (mask == nullptr) || (mask[u] != 0);
+        if (gx != nullptr) {
+            if (isnan(gx[u]) || isnan(gy[u])) ok = 0;
+            if (g.nz > 1 && isnan(gz[u])) ok = 0;
+        }
+    }
+    vbyte[pid] = ok;
+}
+
+// ------------------------------------------------------------------------------------------------ K0b codes
+__device__ __forceinline__ int vget(const Geom& g, const uint8_t* __restrict__ v, int i, int j, int k)
+{
+    if (i < 0 || j < 0 || k < 0 || i >= g.nx || j >= g.ny || k >= g.nz) return 0;
+    return v[i + (long long)g.px * (j + (long long)g.ny * k)];
+}
+
+// one thread per 4-cell group; a warp's 32 groups fill exactly one flag word
+__global__ void codes_kernel(Geom g, const uint8_t* __restrict__ vbyte, uint8_t* __restrict__ link,
+                             uint32_t* __restrict__ wcode, uint32_t* __restrict__ flags)
+{
+    const long long grp = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const long long ngrp = g.npad >> 2;
+    bool flagged = false;
+    if (grp < ngrp) {
+        const long long base = grp << 2;
+        const int i0 = (int)(base % g.px);
+        const long long row = base / g.px;
+        const int j = (int)(row % g.ny), k = (int)(row / g.ny);
+        const int naxes = (g.nz > 1) ? 3 : 2;
+        uint32_t codes[4];
+        uint32_t links = 0;
+#pragma unroll
+        for (int c = 0; c < 4; ++c) {
+            const int i = i0 + c;
+            uint32_t code = 0, lk = 0;
+            bool interior = false;
+            if (vget(g, vbyte, i, j, k)) {
+                code = WCODE_VALID; lk = LINK_VALID; interior = true;
+                for (int d = 0; d < 6; ++d) {
+                    const int a = d >> 1, sg = (d & 1) ? -1 : 1;
+                    int e[3] = { 0, 0, 0 };
+                    e[a] = sg;
+                    const int qi = i + e[0], qj = j + e[1], qk = k + e[2];
+                    if (a >= naxes) continue;                       // 2D scheme: no F/B links at all
+                    if (!vget(g, vbyte, qi, qj, qk)) { interior = false; continue; }
+                    lk |= 1u << d;
+                    const int b = (a + 1) % 3, cc = (a + 2) % 3;
+                    int eb[3] = { 0, 0, 0 }, ec[3] = { 0, 0, 0 };
+                    eb[b] = 1; ec[cc] = 1;
+                    uint32_t far = vget(g, vbyte, qi + e[0], qj + e[1], qk + e[2]);
+                    uint32_t nb = vget(g, vbyte, qi + eb[0], qj + eb[1], qk + eb[2]) +
+                                  vget(g, vbyte, qi - eb[0], qj - eb[1], qk - eb[2]);
+                    uint32_t nc = vget(g, vbyte, qi + ec[0], qj + ec[1], qk + ec[2]) +
+                                  vget(g, vbyte, qi - ec[0], qj - ec[1], qk - ec[2]);
+                    code |= (far | (nb << 1) | (nc << 3)) << (5 * d);
+                    const uint32_t nb_full = (b < naxes) ? 2u : 0u, nc_full = (cc < naxes) ? 2u : 0u;
+                    if (far != 1u || nb != nb_full || nc != nc_full) interior = false;
+                }
+            }
+            codes[c] = code;
+            links |= lk << (8 * c);
+            flagged |= !interior;
+        }
+        *reinterpret_cast<uint4*>(wcode + base) = make_uint4(codes[0], codes[1], codes[2], codes[3]);
+        *reinterpret_cast<uint32_t*>(link + base) = links;
+    }
+    const uint32_t word = __ballot_sync(0xffffffffu, flagged);
+    if ((threadIdx.x & 31) == 0 && grp < ngrp) flags[grp >> 5] = word;
+}
+
+// ------------------------------------------------------------------------------------------------ K1 source
+// S_C = - sum_d v(C+d) sgn(d) (Delta_a t_a / 2) (g_a(C+d) + g_a(C))     (Eq. 9 :100, w^{n+1}+w^n = t_a)
+template <typename T>
+__global__ void __launch_bounds__(256)
+source_kernel(Geom g, const T* __restrict__ gx, const T* __restrict__ gy, const T* __restrict__ gz,
+              const uint8_t* __restrict__ link, Coef<T> K, T* __restrict__ S, Scalars* sc, double* partial)
+{
+    __shared__ double red[8];
+    __shared__ int is_last;
+    const long long pid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    double sq = 0.0;
+    if (pid < g.npad) {
+        const int i = (int)(pid % g.px);
+        const long long row = pid / g.px;
+        T s = T(0);
+        const uint32_t l = link[pid];
+        if (l & LINK_VALID) {
+            const long long u = row * g.nx + i;
+            const long long sy = g.nx, sz = (long long)g.nx * g.ny;
+            const T cx = gx[u], cy = gy[u];
+            if (l & 1u) s -= K.hs[0] * (gx[u + 1] + cx);
+            if (l & 2u) s += K.hs[0] * (gx[u - 1] + cx);
+            if (l & 4u) s -= K.hs[1] * (gy[u + sy] + cy);
+            if (l & 8u) s += K.hs[1] * (gy[u - sy] + cy);
+            if (l & 48u) {
+                const T cz = gz[u];
+                if (l & 16u) s -= K.hs[2] * (gz[u + sz] + cz);
+                if (l & 32u) s += K.hs[2] * (gz[u - sz] + cz);
+            }
+        }
+        S[pid] = s;
+        sq = (double)s * (double)s;
+    }
+    sq = warp_sum(sq);
+    if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = sq;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double t = 0.0;
+        for (int w = 0; w < 8; ++w) t += red[w];
+        partial[blockIdx.x] = t;
+        __threadfence();
+        is_last = (atomicAdd(&sc->ticket[3], 1u) == gridDim.x - 1);
+    }
+    __syncthreads();
+    if (is_last) {
+        __threadfence();
+        double t = 0.0;
+        for (unsigned int b = threadIdx.x; b < gridDim.x; b += 256) t += __ldcg(&partial[b]);
+        t = warp_sum(t);
+        __syncthreads();
+        if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = t;
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            double n2 = 0.0;
+            for (int w = 0; w < 8; ++w) n2 += red[w];
+            sc->ticket[3] = 0;
+            sc->normS2 = n2;
+            sc->thresh2 = (0.1 * sc->tol) * (0.1 * sc->tol) * n2;
+            sc->tol2S = sc->tol * sc->tol * n2;
+            if (!(n2 > 0.0)) {                 // zero (or NaN) source: P = 0, no iterations (A4)
+                sc->outer_go = 0; sc->inner_go = 0;
+                if (!isfinite(n2)) sc->status = ST_BREAKDOWN;
+            }
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------------ K7 finalize
+template <typename T>
+__global__ void finalize_kernel(Geom g, const double* __restrict__ P, const uint8_t* __restrict__ link,
+                                T* __restrict__ out)
+{
+    long long u = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    long long nuser = (long long)g.nx * g.ny * g.nz;
+    if (u >= nuser) return;
+    int i = (int)(u % g.nx);
+    long long pid = (u / g.nx) * g.px + i;
+    out[u] = (link[pid] & LINK_VALID) ? (T)P[pid] : (T)nan("");
+}
+
+// copies between the caller's unpadded layout and the padded internal layout (step entry points only)
+template <typename TI, typename TO>
+__global__ void pad_copy_kernel(Geom g, const TI* __restrict__ in, TO* __restrict__ out, int to_padded,
+                                const uint8_t* __restrict__ link)
+{
+    long long pid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (pid >= g.npad) return;
+    int i = (int)(pid % g.px);
+    long long u = (pid / g.px) * g.nx + i;
+    if (to_padded) out[pid] = (i < g.nx && (link[pid] & LINK_VALID)) ? (TO)in[u] : TO(0);
+    else if (i < g.nx) out[u] = (TO)in[pid];
+}
+
+}  // namespace omni

@@ -1,0 +1,211 @@
+"""Parity of the CUDA path (through the C ABI) with the CPU oracle, element by element, on seeded inputs.
+
+Tolerances: fp64 rel-L2 after mean removal <= 1e-9, fp32 <= 2e-4 (north_star); single-step
+operators are compared entry-wise with a bound derived from the arithmetic (a handful of roundings of terms of size
+max|term|): 1e-13 relative to the largest entry in fp64, 2e-6 in fp32.
+"""
+import numpy as np
+import pytest
+
+import paper_2311_16935_b200 as omni
+from workloads import make_config, make_field
+
+from util import rel_l2_after_mean_removal, to_dev
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+TOL_STEP = {"f64": 1e-13, "f32": 2e-6}
+TOL_SOLVE = {"f64": 1e-9, "f32": 2e-4}
+TDT = {"f64": torch.float64, "f32": torch.float32}
+
+
+def _inputs(f, dtype, mask=None):
+    """Device tensors + the values the oracle must consume (fp32 runs: the fp32-rounded inputs)."""
+    np_dt = np.float32 if dtype == "f32" else np.float64
+    g_host = [np.ascontiguousarray(c.astype(np_dt)) for c in f["g"]]
+    g_dev = [to_dev(c) for c in g_host] + [None] * (3 - len(g_host))
+    g_or = [c.astype(np.float64) for c in g_host] + [None] * (3 - len(g_host))
+    m = f["mask"] if mask is None else mask
+    return g_dev, g_or, (None if m is None else to_dev(m.astype(np.uint8))), m
+
+
+def _random_mask(shape, seed, frac):
+    rng = np.random.default_rng(seed)
+    return (rng.random(shape) > frac).astype(np.uint8)
+
+
+SHAPES = [((37, 300), 0.1), ((9, 31, 150), 0.1), ((5, 16, 264), 0.0), ((17, 29, 9), 0.3), ((1, 77), 0.0), ((40, 3, 20), 0.05)]
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("shape,frac", SHAPES)
+def test_source_and_operator_steps(oracle, dtype, shape, frac):
+    """a1+a2 (S), a4 (q = M p) and a3 (r = S - L P) against the oracle's stored-weight operators: ragged sizes
+    spanning several tiles, random masks, anisotropic spacing."""
+    kind = "gaussians2d" if len(shape) == 2 else "fourier3d"
+    f = make_field(kind, shape, seed=11, noise=0.1, kmax=3.0)
+    mask = _random_mask(shape, 5, frac) if frac > 0 else None
+    g_dev, g_or, m_dev, m = _inputs(f, dtype, mask)
+    d = f["d"]
+    v = oracle.validity(g_or[0], g_or[1], g_or[2], m)
+    w1, w0, w0C = oracle.weights(v, *d)
+    S_or = oracle.source(v, w1, w0, g_or[0], g_or[1], g_or[2], *d)
+
+    S, nS = omni.source(g_dev[0], g_dev[1], g_dev[2], m_dev, d)
+    S = S.cpu().numpy().astype(np.float64)
+    scale = np.abs(S_or).max()
+    assert np.abs(S - S_or).max() <= TOL_STEP[dtype] * scale * 4
+    assert nS == pytest.approx(np.linalg.norm(S_or), rel=10 * TOL_STEP[dtype])
+    assert np.all(S[v == 0] == 0)
+
+    rng = np.random.default_rng(3)
+    p = rng.normal(size=shape)
+    p_dev = to_dev(p, TDT[dtype])
+    p_or = p_dev.cpu().numpy().astype(np.float64) * v
+    q, pq = omni.apply_M(p_dev, m_dev if m is not None else None, d)
+    # validity for apply_M comes from the mask alone; these inputs carry no NaN so it equals v
+    q = q.cpu().numpy().astype(np.float64)
+    q_or = oracle.apply_M(v, w1, p_or)
+    assert np.abs(q - q_or).max() <= TOL_STEP[dtype] * np.abs(q_or).max() * 8
+    assert pq == pytest.approx(float(np.sum(p_or * q_or)), rel=1e-5 if dtype == "f32" else 1e-11)
+    assert np.all(q[v == 0] == 0)
+
+    P = rng.normal(size=shape)
+    r, eps = omni.residual(g_dev[0], g_dev[1], g_dev[2], m_dev, to_dev(P), d)
+    r = r.cpu().numpy().astype(np.float64)
+    Pv = P * v
+    r_or = S_or + oracle.apply_Wn(v, w0, w0C, Pv) - oracle.apply_M(v, w1, Pv)
+    assert np.abs(r - r_or).max() <= TOL_STEP[dtype] * max(np.abs(r_or).max(), np.abs(Pv).max()) * 8
+    assert eps == pytest.approx(np.linalg.norm(r_or) / np.linalg.norm(S_or), rel=1e-5 if dtype == "f32" else 1e-10)
+
+
+def _solve_both(oracle, f, dtype, tol, max_outer, max_cg, mask=None, nan_mask=False):
+    g_dev, g_or, m_dev, m = _inputs(f, dtype, mask)
+    d = f["d"]
+    P, info = omni.solve(g_dev[0], g_dev[1], g_dev[2], m_dev, d, tol, max_outer, max_cg)
+    torch.cuda.synchronize()
+    Po, io = oracle.solve(g_or[0], g_or[1], g_or[2], m, *d, tol=tol, max_outer=max_outer, max_cg=max_cg)
+    return P.cpu().numpy(), info, Po, io
+
+
+TRAJ = [("gaussians2d", (64, 64), None), ("lamb_oseen2d", (150, 130), None), ("fourier3d", (20, 33, 140), None),
+        ("sphere3d", (40, 36, 44), None), ("fourier3d", (12, 30, 270), 0.15)]
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("kind,shape,frac", TRAJ)
+def test_trajectory_parity(oracle, dtype, kind, shape, frac):
+    """Same inputs, tol = 0, fixed iteration counts: both sides execute identical steps (SURVEY 8c protocol i)."""
+    f = make_field(kind, shape, seed=7, noise=0.05, kmax=4.0)
+    mask = None
+    if frac:
+        mask = _random_mask(shape, 9, frac)
+    P, info, Po, io = _solve_both(oracle, f, dtype, 0.0, 6, 20, mask)
+    valid = ~np.isnan(Po)
+    assert np.array_equal(np.isnan(P), ~valid)
+    assert info["outer_iters"] == io["outer_iters"] == 6
+    assert info["cg_iters_total"] == io["cg_iters_total"]
+    assert info["status"] == omni.binding.OMNI_NOT_CONVERGED
+    err = rel_l2_after_mean_removal(P, Po, valid)
+    assert err <= TOL_SOLVE[dtype], err
+    assert info["norm_S"] == pytest.approx(io["norm_S"], rel=1e-5 if dtype == "f32" else 1e-12)
+    assert info["eps_R_final"] == pytest.approx(io["eps_R_final"], rel=2e-3 if dtype == "f32" else 1e-7)
+
+
+def test_converged_parity_config0(oracle):
+    """BASELINE configs[0]: 64^2 fp64, tol 1e-8, converged on both sides with the same stopping rules; and the
+    recovered field matches the analytic P up to a constant at the discretisation + noise level."""
+    f = make_config(0)
+    P, info, Po, io = _solve_both(oracle, f, "f64", 1e-8, 100000, 1000)
+    assert info["status"] == 0 and io["converged"]
+    assert info["outer_iters"] == io["outer_iters"]
+    assert info["cg_iters_total"] == io["cg_iters_total"]
+    valid = np.ones(P.shape, bool)
+    assert rel_l2_after_mean_removal(P, Po, valid) <= 1e-9
+    assert info["eps_R_final"] <= 1e-8
+    assert rel_l2_after_mean_removal(P, f["P"], valid) < 0.05
+
+
+@pytest.mark.parametrize("dtype,tol", [("f64", 1e-8), ("f32", 1e-5)])
+def test_converged_parity_small_standins(oracle, dtype, tol):
+    """Small stand-ins of configs 1 and 3 (masked 2D vortex 96^2, masked sphere flow 32^3), converged."""
+    for idx, n in ((1, 96), (3, 32)):
+        f = make_config(idx, n)
+        P, info, Po, io = _solve_both(oracle, f, dtype, tol, 200000, 64)
+        assert info["status"] == 0 and io["converged"], (idx, info, io)
+        valid = ~np.isnan(Po)
+        assert rel_l2_after_mean_removal(P, Po, valid) <= TOL_SOLVE[dtype]
+        if dtype == "f64":
+            assert info["outer_iters"] == io["outer_iters"]
+
+
+def test_graph_and_host_loops_are_bit_identical():
+    f = make_field("sphere3d", (24, 30, 40), seed=2, noise=0.05)
+    for dtype in ("f64", "f32"):
+        g_dev, _, m_dev, _ = _inputs(f, dtype)
+        res = []
+        for mode in (0, 1):
+            prev = omni.set_loop_mode(mode)
+            try:
+                P, info = omni.solve(g_dev[0], g_dev[1], g_dev[2], m_dev, f["d"], 1e-4, 50, 12)
+            finally:
+                omni.set_loop_mode(prev)
+            res.append((P.cpu().numpy(), info))
+        assert res[0][1] == res[1][1]
+        assert np.array_equal(res[0][0], res[1][0], equal_nan=True)
+        # determinism: same call twice, same bits
+        P2, _ = omni.solve(g_dev[0], g_dev[1], g_dev[2], m_dev, f["d"], 1e-4, 50, 12)
+        assert np.array_equal(res[0][0], P2.cpu().numpy(), equal_nan=True)
+
+
+def test_edge_cases(oracle):
+    dev = "cuda"
+    # zero gradient -> P = 0, no iterations
+    z = torch.zeros(6, 7, 8, dtype=torch.float64, device=dev)
+    m = torch.ones(6, 7, 8, dtype=torch.uint8, device=dev)
+    m[2, 3, 4] = 0
+    P, info = omni.solve(z, z, z, m, (1.0, 1.0, 1.0), 1e-8, 10, 10)
+    assert info["outer_iters"] == 0 and info["cg_iters_total"] == 0 and info["norm_S"] == 0 and info["status"] == 0
+    Pn = P.cpu().numpy()
+    assert np.isnan(Pn[2, 3, 4]) and np.all(Pn[m.cpu().numpy() == 1] == 0)
+    # everything masked
+    P, info = omni.solve(z, z, z, torch.zeros_like(m), (1.0, 1.0, 1.0), 1e-8, 10, 10)
+    assert np.all(np.isnan(P.cpu().numpy())) and info["outer_iters"] == 0
+    # single cell, single row, single column
+    one = torch.ones(1, 1, dtype=torch.float64, device=dev)
+    P, info = omni.solve(one, one, None, None, (1.0, 1.0), 1e-8, 10, 10)
+    assert float(P[0, 0]) == 0.0 and info["outer_iters"] == 0
+    # NaN-marked missing data equals mask-marked missing data (Eq. 13)
+    f = make_field("lamb_oseen2d", (60, 70), seed=1, noise=0.05)
+    fn = make_field("lamb_oseen2d", (60, 70), seed=1, noise=0.05, nan_mask=True)
+    Pm, im = omni.solve(to_dev(f["g"][0]), to_dev(f["g"][1]), None, to_dev(f["mask"]), f["d"], 1e-6, 500, 20)
+    Pn, inn = omni.solve(to_dev(fn["g"][0]), to_dev(fn["g"][1]), None, None, fn["d"], 1e-6, 500, 20)
+    assert im == inn and np.array_equal(Pm.cpu().numpy(), Pn.cpu().numpy(), equal_nan=True)
+    # max_outer = 0 and max_cg = 0 terminate
+    g = to_dev(f["g"][0])
+    P, info = omni.solve(g, to_dev(f["g"][1]), None, to_dev(f["mask"]), f["d"], 1e-6, 0, 5)
+    assert info["outer_iters"] == 0 and info["status"] == 1 and info["eps_R_final"] == pytest.approx(1.0)
+    P, info = omni.solve(g, to_dev(f["g"][1]), None, to_dev(f["mask"]), f["d"], 1e-6, 3, 0)
+    assert info["outer_iters"] == 3 and info["cg_iters_total"] == 0
+    # the 3x3 appendix example runs (all cells are boundary cells)
+    rng = np.random.default_rng(0)
+    fx, fy = rng.normal(size=(3, 3)), rng.normal(size=(3, 3))
+    P, info = omni.solve(to_dev(fx), to_dev(fy), None, None, (0.5, 0.5), 0.0, 4, 9)
+    Po, io = oracle.solve(fx, fy, None, None, 0.5, 0.5, 1.0, tol=0.0, max_outer=4, max_cg=9)
+    assert rel_l2_after_mean_removal(P.cpu().numpy(), Po, np.ones((3, 3), bool)) < 1e-9
+
+
+def test_host_buffers_and_workspace_entry_points(oracle):
+    f = make_field("fourier3d", (10, 20, 30), seed=4, noise=0.05, kmax=2.0)
+    g = [torch.from_numpy(c) for c in f["g"]]
+    Ph, ih = omni.solve(g[0], g[1], g[2], None, f["d"], 1e-6, 100, 10)          # host path
+    gd = [c.cuda() for c in g]
+    Pd, idv = omni.solve(gd[0], gd[1], gd[2], None, f["d"], 1e-6, 100, 10)
+    assert ih == idv and np.array_equal(Ph.numpy(), Pd.cpu().numpy())
+    ws = torch.empty(omni.workspace_bytes(30, 20, 10, "f64"), dtype=torch.uint8, device="cuda")
+    Pw, iw = omni.solve(gd[0], gd[1], gd[2], None, f["d"], 1e-6, 100, 10, workspace=ws)
+    assert iw == idv and np.array_equal(Pw.cpu().numpy(), Pd.cpu().numpy())
+    small = torch.empty(1024, dtype=torch.uint8, device="cuda")
+    with pytest.raises(omni.OmniError):
+        omni.solve(gd[0], gd[1], gd[2], None, f["d"], 1e-6, 100, 10, workspace=small)

@@ -1,0 +1,66 @@
+"""CPU-side checks of the CUDA library: it loads, exports every symbol of include/omni.h, validates arguments, and
+its host-side geometry constants (step a0) agree with the oracle's independent computation."""
+import ctypes as C
+import os
+import re
+
+import numpy as np
+import pytest
+
+import paper_2311_16935_b200 as omni
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def test_library_exports_every_declared_symbol():
+    hdr = open(os.path.join(ROOT, "include", "omni.h")).read()
+    declared = set(re.findall(r"\b(omni_[a-z0-9_A-Z]+)\s*\(", hdr))
+    assert declared == set(omni.SYMBOLS), declared ^ set(omni.SYMBOLS)
+    L = omni.lib()
+    for s in declared:
+        assert hasattr(L, s), s
+    assert omni.version() >= 100
+    assert "invalid" in omni.status_string(-1)
+
+
+def test_argument_validation_needs_no_device():
+    L = omni.lib()
+    bad = [dict(nx=0), dict(dx=0.0), dict(dx=float("nan")), dict(tol=-1.0), dict(max_outer=-1), dict(gx=0), dict(P=0)]
+    for b in bad:
+        a = dict(nx=4, ny=4, nz=1, dx=1.0, dy=1.0, dz=1.0, gx=8, gy=8, gz=0, mask=0, P=8, tol=1e-8, max_outer=1, max_cg=1)
+        a.update(b)
+        rc = L.omni_solve_f64(C.c_int(a["nx"]), C.c_int(a["ny"]), C.c_int(a["nz"]), C.c_double(a["dx"]), C.c_double(a["dy"]),
+                              C.c_double(a["dz"]), C.c_void_p(a["gx"]), C.c_void_p(a["gy"]), C.c_void_p(a["gz"]),
+                              C.c_void_p(a["mask"]), C.c_void_p(a["P"]), C.c_double(a["tol"]), C.c_int(a["max_outer"]),
+                              C.c_int(a["max_cg"]), None, None)
+        assert rc == -1, b
+    # 3D needs gz
+    rc = L.omni_solve_f32(C.c_int(4), C.c_int(4), C.c_int(4), C.c_double(1), C.c_double(1), C.c_double(1), C.c_void_p(8),
+                          C.c_void_p(8), C.c_void_p(0), None, C.c_void_p(8), C.c_double(0), C.c_int(1), C.c_int(1), None, None)
+    assert rc == -1
+    assert omni.workspace_bytes(64, 64, 1, "f64") > 64 * 64 * 8 * 6
+    assert omni.workspace_bytes(500, 500, 500, "f32") < 6 * 2**30
+
+
+@pytest.mark.parametrize("dims,sp", [((9, 9, 1), (0.3, 0.7, 1.0)), ((5, 5, 5), (1.0, 1.0, 1.0)), ((5, 5, 5), (0.25, 0.25, 0.25)),
+                                     ((5, 6, 7), (1.0, 0.7, 1.9)), ((4, 4, 4), (0.01, 0.013, 0.0047)),
+                                     ((264, 16, 5), (1 / 263, 1 / 15, 1 / 4)), ((5, 16, 264), (0.25, 1 / 15, 1 / 263))])
+def test_constants_a0_match_oracle(oracle, dims, sp):
+    """Two independent routes to c_jk: closed-form parallel-rectangle measure (library) vs Eq. 17 / Eq. 32-33 /
+    Gauss-Legendre quadrature of the defining integral (oracle)."""
+    K = omni.constants(*dims, *sp)
+    Ko = oracle.constants(*dims, *sp)
+    assert np.allclose(K["F"], Ko["F"], rtol=1e-14)
+    assert K["A_tot"] == pytest.approx(Ko["A_tot"], rel=1e-14)
+    # what enters the stencil is c / A_tot (Eq. 10): relative 2e-12, or 1e-15 absolute for the tiny far-face
+    # constants of strongly anisotropic cells, where the closed form loses digits to cancellation
+    assert np.allclose(np.array(K["c"]) / K["A_tot"], Ko["c"] / Ko["A_tot"], rtol=2e-12, atol=1e-15)
+
+
+def test_no_cpu_fallback():
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("GPU present")
+    g = torch.zeros(8, 8, dtype=torch.float64)
+    with pytest.raises(RuntimeError):
+        omni.solve(g, g, None, None, (1.0, 1.0), 1e-8, 1, 1)
