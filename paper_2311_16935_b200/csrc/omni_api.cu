@@ -106,7 +106,7 @@ template <typename T>
 struct Workspace {
     uint8_t* link; uint32_t* wcode; uint32_t* flags;
     T *S, *r, *p0, *p1, *delta;
-    double* P; double* partial; Scalars* sc;
+    double* P; double* P1; double* partial; Scalars* sc;
 };
 
 size_t partial_slots(const Geom& g)
@@ -134,12 +134,13 @@ size_t carve(const Geom& g, char* base, Workspace<T>* w)
     char* p1 = take(n * sizeof(T));
     char* delta = take(n * sizeof(T));
     char* P = take(n * sizeof(double));
+    char* P1 = take(n * sizeof(double));
     char* partial = take(partial_slots(g) * sizeof(double));
     char* sc = take(sizeof(Scalars));
     if (w) {
         w->link = (uint8_t*)link; w->wcode = (uint32_t*)wcode; w->flags = (uint32_t*)flags;
         w->S = (T*)S; w->r = (T*)r; w->p0 = (T*)p0; w->p1 = (T*)p1; w->delta = (T*)delta;
-        w->P = (double*)P; w->partial = (double*)partial; w->sc = (Scalars*)sc;
+        w->P = (double*)P; w->P1 = (double*)P1; w->partial = (double*)partial; w->sc = (Scalars*)sc;
     }
     return off;
 }
@@ -227,6 +228,7 @@ int setup_codes(const Geom& g, const Workspace<T>& w, const T* gx, const T* gy, 
     CK(cudaMemsetAsync(w.p1, 0, n * sizeof(T), st));
     CK(cudaMemsetAsync(w.delta, 0, n * sizeof(T), st));
     CK(cudaMemsetAsync(w.P, 0, n * sizeof(double), st));
+    CK(cudaMemsetAsync(w.P1, 0, n * sizeof(double), st));
     return OMNI_OK;
 }
 
@@ -244,7 +246,7 @@ template <typename T>
 typename K2<T>::Args k2_args(const Workspace<T>& w, const HostConst& H, CondHandles ch, int fold)
 {
     typename K2<T>::Args a;
-    a.P = w.P; a.delta = w.delta; a.S = w.S; a.r = w.r; a.link = w.link; a.flags = w.flags;
+    a.Pbuf[0] = w.P; a.Pbuf[1] = fold ? w.P1 : w.P; a.delta = w.delta; a.S = w.S; a.r = w.r; a.link = w.link; a.flags = w.flags;
     for (int i = 0; i < 3; ++i) a.t[i] = H.F[i] / H.Atot;
     a.sc = w.sc; a.partial = w.partial; a.cond = ch; a.fold_delta = fold;
     return a;
@@ -402,7 +404,7 @@ int solve_ws(int nx, int ny, int nz, double dx, double dy, double dz, const T* g
     rc = (mode == 1) ? run_loop_host<T>(g, w, H, K, max_outer, max_cg, st) : run_loop_graph<T>(g, w, H, K, st);
     if (rc != OMNI_OK) return rc;
 
-    finalize_kernel<T><<<blocks_for((long long)nx * ny * nz, 256), 256, 0, st>>>(g, w.P, w.link, P_out);
+    finalize_kernel<T><<<blocks_for((long long)nx * ny * nz, 256), 256, 0, st>>>(g, w.P, w.P1, w.sc, w.link, P_out);
     CK(cudaGetLastError());
     g_launches.fetch_add(1, std::memory_order_relaxed);
 

@@ -170,6 +170,8 @@ __device__ __forceinline__ uint32_t flag_bits(const uint32_t* __restrict__ flags
 // TYR (rows per CTA incl. the two halo rows), MINB, NACC, TICKET, Args, Ctx, Raw (+ load / convert), Extra
 // (+ load_extra), emit, active, finalize.
 
+__device__ __forceinline__ void set_cond(const CondHandles& h, int outer, int inner);
+
 template <class Op>
 __global__ void __launch_bounds__(32 * Op::TYR, Op::MINB)
 march_kernel(const Geom g, const int zlen, const typename Op::Args a)
@@ -180,7 +182,10 @@ march_kernel(const Geom g, const int zlen, const typename Op::Args a)
     __shared__ double red[NACC][TYR];
     __shared__ int is_last;
 
-    if (!Op::active(a)) return;
+    if (!Op::active(a)) {       // uniform: the device-side loop state says this launch has nothing to do
+        if (threadIdx.x == 0 && threadIdx.y == 0 && blockIdx.x == 0 && blockIdx.y == 0 && blockIdx.z == 0) Op::idle(a);
+        return;
+    }
 
     const int lane = threadIdx.x, ty = threadIdx.y;
     const int x = blockIdx.x * W + lane * V;
@@ -319,6 +324,7 @@ struct OpK3 {
     struct Raw { T r[V], p[V], rl, pl, rr, pr; };
     struct Extra {};
     __device__ static bool active(const Args& a) { return a.sc->inner_go != 0; }
+    __device__ static void idle(const Args& a) { set_cond(a.cond, -1, 0); }
     __device__ static void load(Raw& w, const Args& a, const Ctx& c, long long idx, bool ok, bool lok, bool rok)
     {
         if (ok) { ld_chunk<T, V>(a.r + idx, w.r); ld_chunk<T, V>(c.pold + idx, w.p); }
@@ -381,6 +387,7 @@ struct OpK4 {
     struct Raw { T p[V], pl, pr; };
     struct Extra { T r[V], d[V]; };
     __device__ static bool active(const Args& a) { return a.sc->inner_go != 0; }
+    __device__ static void idle(const Args& a) { set_cond(a.cond, -1, 0); }
     __device__ static void load(Raw& w, const Args&, const Ctx& c, long long idx, bool ok, bool lok, bool rok)
     {
         if (ok) ld_chunk<T, V>(c.p + idx, w.p); else zero_chunk<T, V>(w.p);
@@ -443,26 +450,31 @@ struct OpK4 {
 // ------------------------------------------------------------------------------------------------ K2
 // outer boundary update (Eq. 12 collapsed): P <- P + delta; r0 = S - L P with
 // (L P)_C = sum_d v(C+d) t_a (P_C - P_{C+d}) = ([W^{n+1}] - [W^n]) P; eps_R^2 ||S||^2 = ||r0||^2 (Eq. 41).
-// P is always fp64 (master pressure, A9); delta, S, r are T.
+// P is always fp64 (master pressure, A9); delta, S, r are T.  P is double-buffered: neighbouring CTAs read
+// P + delta in their halos, so the folded field goes to the other buffer (read Pbuf[n&1], write Pbuf[(n&1)^1]).
 template <typename T, int TYR_, int MINB_>
 struct OpK2 {
     using VT = double;
     enum { V = 4, TYR = TYR_, MINB = MINB_, NACC = 2, TICKET = 2 };
     struct Args {
-        double* P; const T* delta; const T* S; T* r; const uint8_t* link; const uint32_t* flags;
+        double* Pbuf[2]; const T* delta; const T* S; T* r; const uint8_t* link; const uint32_t* flags;
         double t[3]; Scalars* sc; double* partial; CondHandles cond;
         int fold_delta;   // 0: residual of P as given (omni_residual); 1: inside the solve
     };
-    struct Ctx { __device__ Ctx(const Args&) {} };
+    struct Ctx {
+        const double* Pin; double* Pout;
+        __device__ Ctx(const Args& a) { int par = a.sc->n & 1; Pin = a.Pbuf[par]; Pout = a.Pbuf[par ^ 1]; }
+    };
     struct Raw { double P[V]; T d[V]; double Pl, Pr; T dl, dr; };
     struct Extra { T S[V]; };
     __device__ static bool active(const Args& a) { return a.sc->outer_go != 0; }
-    __device__ static void load(Raw& w, const Args& a, const Ctx&, long long idx, bool ok, bool lok, bool rok)
+    __device__ static void idle(const Args& a) { set_cond(a.cond, 0, 0); }
+    __device__ static void load(Raw& w, const Args& a, const Ctx& c, long long idx, bool ok, bool lok, bool rok)
     {
-        if (ok) { ld_chunk<double, V>(a.P + idx, w.P); ld_chunk<T, V>(a.delta + idx, w.d); }
+        if (ok) { ld_chunk<double, V>(c.Pin + idx, w.P); ld_chunk<T, V>(a.delta + idx, w.d); }
         else { zero_chunk<double, V>(w.P); zero_chunk<T, V>(w.d); }
-        w.Pl = lok ? a.P[idx - 1] : 0.0; w.dl = lok ? a.delta[idx - 1] : T(0);
-        w.Pr = rok ? a.P[idx + V] : 0.0; w.dr = rok ? a.delta[idx + V] : T(0);
+        w.Pl = lok ? c.Pin[idx - 1] : 0.0; w.dl = lok ? a.delta[idx - 1] : T(0);
+        w.Pr = rok ? c.Pin[idx + V] : 0.0; w.dr = rok ? a.delta[idx + V] : T(0);
     }
     __device__ static void convert(const Raw& w, const Ctx&, double (&v)[V], double& hl, double& hr)
     {
@@ -475,11 +487,11 @@ struct OpK2 {
     {
         if (ok) ld_chunk<T, V>(a.S + idx, e.S); else zero_chunk<T, V>(e.S);
     }
-    __device__ static void emit(const Args& a, const Ctx&, long long idx, const double (&vm)[V], const double (&vc)[V],
+    __device__ static void emit(const Args& a, const Ctx& c, long long idx, const double (&vm)[V], const double (&vc)[V],
                                 const double (&vp)[V], const double (&vn)[V], const double (&vs)[V], double xl,
                                 double xr, const Extra& e, double (&acc)[2])
     {
-        if (a.fold_delta) st_chunk<double, V>(a.P + idx, vc);
+        if (a.fold_delta) st_chunk<double, V>(c.Pout + idx, vc);
         uint32_t fb = flag_bits<V>(a.flags, idx);
         uint32_t lk = 0x7f7f7f7fu;
         if (fb) lk = *reinterpret_cast<const uint32_t*>(a.link + idx);
@@ -680,9 +692,10 @@ source_kernel(Geom g, const T* __restrict__ gx, const T* __restrict__ gy, const 
 
 // ------------------------------------------------------------------------------------------------ K7 finalize
 template <typename T>
-__global__ void finalize_kernel(Geom g, const double* __restrict__ P, const uint8_t* __restrict__ link,
-                                T* __restrict__ out)
+__global__ void finalize_kernel(Geom g, const double* P0, const double* P1, const Scalars* sc,
+                                const uint8_t* __restrict__ link, T* __restrict__ out)
 {
+    const double* __restrict__ P = (sc->n & 1) ? P0 : P1;      // the last K2 wrote Pbuf[(n & 1) ^ 1]
     long long u = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     long long nuser = (long long)g.nx * g.ny * g.nz;
     if (u >= nuser) return;
