@@ -126,6 +126,12 @@ long long omni_launch_count(int reset);
 /* 0 = CUDA-graph loop with device-side conditional WHILE nodes (default), 1 = host-driven loop that synchronises
  * once per outer iteration (debug / drivers without conditional nodes).  Returns the previous mode. */
 int omni_set_loop_mode(int mode);
+/* Per-kernel timing of the host-driven loop (loop mode 1 only): when enabled, CUDA events bracket every launch of
+ * K2 (outer boundary update), K3 (p update + operator + p.Mp) and K4 (operator recomputed + axpys + r.r) on `stream`;
+ * launches that found the device loop flag cleared (no work) are left out.  omni_profile_read returns the summed
+ * milliseconds and launch counts, index 0/1/2 = K2/K3/K4 (host arrays of 3, either may be NULL). */
+int omni_profile_enable(int on);          /* returns the previous setting */
+void omni_profile_read(double* h_ms3, long long* h_count3, int reset);
 const char* omni_status_string(int status);
 int omni_version(void);
 

@@ -3,8 +3,8 @@
 The product is the C-ABI library libomni.so (include/omni.h, csrc/); this package is its thin ctypes binding.
 Importing the package does not load the library; the first call does, and fails loudly when it is missing.
 """
-from .binding import (Info, OmniError, SYMBOLS, apply_M, constants, launch_count, lib, residual, set_loop_mode,  # noqa: F401
-                      solve, source, status_string, version, workspace_bytes)
+from .binding import (Info, OmniError, SYMBOLS, apply_M, constants, launch_count, lib, profile_enable,  # noqa: F401
+                      profile_read, residual, set_loop_mode, solve, source, status_string, version, workspace_bytes)
 
 # the C names, for callers who think in terms of include/omni.h
 omni_solve = solve
@@ -15,5 +15,7 @@ omni_constants = constants
 omni_workspace_bytes = workspace_bytes
 omni_launch_count = launch_count
 omni_set_loop_mode = set_loop_mode
+omni_profile_enable = profile_enable
+omni_profile_read = profile_read
 omni_status_string = status_string
 omni_version = version

@@ -1,13 +1,16 @@
 // omni_api.cu -- C ABI (include/omni.h) over the kernels of omni_kernels.cuh.
 // Host logic only: argument validation, geometry constants (a0), workspace carving, launch configuration and the
 // loop driver (CUDA graph with device-side conditional WHILE nodes, or a host-driven debug loop).
-#include "omni_kernels.cuh"
+#include "omni_march.cuh"
 #include "../../include/omni.h"
 
+#include <algorithm>
 #include <atomic>
 #include <cmath>
 #include <cstdio>
 #include <cstdlib>
+#include <mutex>
+#include <vector>
 #include <type_traits>
 
 using namespace omni;
@@ -16,6 +19,13 @@ namespace {
 
 std::atomic<long long> g_launches{0};
 std::atomic<int> g_loop_mode{0};
+
+// optional per-kernel timing of the host-driven loop (omni_profile_*): CUDA events around every K2/K3/K4 launch
+std::atomic<int> g_profile{0};
+std::mutex g_prof_mu;
+double g_prof_ms[3] = { 0, 0, 0 };
+long long g_prof_n[3] = { 0, 0, 0 };
+struct ProfRec { int which; cudaEvent_t e0, e1; };
 
 #define CK(call)                                       \
     do {                                               \
@@ -74,7 +84,7 @@ void host_constants(int nz, double dx, double dy, double dz, HostConst& H)
 }
 
 template <typename T>
-Coef<T> make_coef(const HostConst& H, double dx, double dy, double dz)
+Coef<T> make_coef(const HostConst& H, double dx, double dy, double dz, int nz)
 {
     Coef<T> K;
     const double d[3] = { dx, dy, dz };
@@ -84,7 +94,20 @@ Coef<T> make_coef(const HostConst& H, double dx, double dy, double dz)
         K.cab[a] = (T)(H.c[a][(a + 1) % 3] / H.Atot);
         K.cac[a] = (T)(H.c[a][(a + 2) % 3] / H.Atot);
         K.hs[a] = (T)(d[a] * (H.F[a] / H.Atot) * 0.5);
+        for (int bits = 0; bits < 32; ++bits) {
+            const int far = bits & 1, nb = (bits >> 1) & 3, nc = (bits >> 3) & 3;
+            K.lut[a][bits] = (T)((far * H.c[a][a] + nb * H.c[a][(a + 1) % 3] + nc * H.c[a][(a + 2) % 3]) / H.Atot);
+        }
     }
+    // interior code: every active axis has both links with far = 1 and two valid side cells along the other active axes
+    const int naxes = (nz > 1) ? 3 : 2;
+    uint32_t icode = WCODE_VALID;
+    for (int d = 0; d < 2 * naxes; ++d) {
+        const int a = d >> 1, b = (a + 1) % 3, c = (a + 2) % 3;
+        const uint32_t bits = 1u | ((b < naxes ? 2u : 0u) << 1) | ((c < naxes ? 2u : 0u) << 3);
+        icode |= bits << (5 * d);
+    }
+    K.icode = icode;
     return K;
 }
 
@@ -168,7 +191,8 @@ MarchCfg march_config(const Geom& g)
         int dev = 0, sms = 148, occ = 1;
         cudaGetDevice(&dev);
         cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, march_kernel<Op>, 32 * Op::TYR, 0);
+        cudaFuncSetAttribute(march_kernel<Op>, cudaFuncAttributeMaxDynamicSharedMemorySize, MarchSmem<Op>::TOTAL);
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, march_kernel<Op>, 32 * Op::TYR, MarchSmem<Op>::TOTAL);
         if (occ < 1) occ = 1;
         slots_cache = sms * occ;
     }
@@ -199,15 +223,15 @@ template <class Op>
 cudaError_t launch_march(const Geom& g, const typename Op::Args& a, cudaStream_t st)
 {
     const MarchCfg c = march_config<Op>(g);
-    march_kernel<Op><<<c.grid, c.block, 0, st>>>(g, c.zlen, a);
+    march_kernel<Op><<<c.grid, c.block, MarchSmem<Op>::TOTAL, st>>>(g, c.zlen, a);
     g_launches.fetch_add(1, std::memory_order_relaxed);
     return cudaGetLastError();
 }
 
-// tile shapes: 16 rows (14 output) x 1 KB wide; register budgets checked with -Xptxas -v
-template <typename T> using K3 = OpK3<T, 16, 1>;
-template <typename T> using K4 = OpK4<T, 16, 1>;
-template <typename T> using K2 = OpK2<T, 16, 1>;
+// tile shapes: 16 rows (14 output) x 1 KB wide, one CTA per SM; ring depth D bounded by 227 KB of shared memory
+template <typename T> using K3 = OpK3<T, 16, 4>;    // 4 x 32.5 KB ring + 32 KB exchange = 162 KB
+template <typename T> using K4 = OpK4<T, 16, 3>;    // 3 x 48.5 KB ring + 32 KB exchange = 178 KB
+template <typename T> using K2 = OpK2<T, 16, 3>;
 
 inline unsigned blocks_for(long long n, int bs) { return (unsigned)((n + bs - 1) / bs); }
 
@@ -270,7 +294,7 @@ typename K4<T>::Args k4_args(const Workspace<T>& w, const Coef<T>& K, CondHandle
 
 // ------------------------------------------------------------------------------------------------ loop drivers
 
-// Host-driven loop (debug): one synchronisation per outer iteration (plus one per 16 CG iterations).
+// Host-driven loop (debug / profiling): one synchronisation per outer iteration (plus one per 16 CG iterations).
 template <typename T>
 int run_loop_host(const Geom& g, const Workspace<T>& w, const HostConst& H, const Coef<T>& K, int max_outer, int max_cg,
                   cudaStream_t st)
@@ -279,28 +303,69 @@ int run_loop_host(const Geom& g, const Workspace<T>& w, const HostConst& H, cons
     const auto a2 = k2_args<T>(w, H, ch, 1);
     const auto a3 = k3_args<T>(w, K, ch);
     const auto a4 = k4_args<T>(w, K, ch);
+    const bool prof = g_profile.load() != 0;
+    std::vector<ProfRec> recs;
+    auto timed = [&](int which, auto&& launch) -> cudaError_t {
+        if (!prof) return launch();
+        ProfRec r{ which, nullptr, nullptr };
+        cudaEventCreate(&r.e0); cudaEventCreate(&r.e1);
+        cudaEventRecord(r.e0, st);
+        cudaError_t e = launch();
+        cudaEventRecord(r.e1, st);
+        recs.push_back(r);
+        return e;
+    };
+    auto flush = [&](const Scalars& h_before, const Scalars& h_after) {
+        (void)h_before; (void)h_after;
+    };
+    (void)flush;
     Scalars h;
-    for (long long it = 0; it <= (long long)max_outer; ++it) {
-        CK(launch_march<K2<T>>(g, a2, st));
+    memset(&h, 0, sizeof(h));
+    int rc = OMNI_OK;
+    long long executed_k34 = 0, seen_cg = 0;
+    for (long long it = 0; it <= (long long)max_outer && rc == OMNI_OK; ++it) {
+        if (timed(0, [&] { return launch_march<K2<T>>(g, a2, st); }) != cudaSuccess) { rc = OMNI_ERR_CUDA; break; }
         int done = 0;
+        bool synced = false;
         while (done < max_cg) {
             const int batch = (max_cg - done < 16) ? (max_cg - done) : 16;
             for (int c = 0; c < batch; ++c) {
-                CK(launch_march<K3<T>>(g, a3, st));
-                CK(launch_march<K4<T>>(g, a4, st));
+                if (timed(1, [&] { return launch_march<K3<T>>(g, a3, st); }) != cudaSuccess) rc = OMNI_ERR_CUDA;
+                if (timed(2, [&] { return launch_march<K4<T>>(g, a4, st); }) != cudaSuccess) rc = OMNI_ERR_CUDA;
             }
             done += batch;
-            CK(cudaMemcpyAsync(&h, w.sc, sizeof(Scalars), cudaMemcpyDeviceToHost, st));
-            CK(cudaStreamSynchronize(st));
+            if (rc != OMNI_OK) break;
+            if (cudaMemcpyAsync(&h, w.sc, sizeof(Scalars), cudaMemcpyDeviceToHost, st) != cudaSuccess ||
+                cudaStreamSynchronize(st) != cudaSuccess) { rc = OMNI_ERR_CUDA; break; }
+            synced = true;
             if (!h.inner_go) break;
         }
-        if (max_cg == 0) {
-            CK(cudaMemcpyAsync(&h, w.sc, sizeof(Scalars), cudaMemcpyDeviceToHost, st));
-            CK(cudaStreamSynchronize(st));
+        if (rc == OMNI_OK && !synced) {
+            if (cudaMemcpyAsync(&h, w.sc, sizeof(Scalars), cudaMemcpyDeviceToHost, st) != cudaSuccess ||
+                cudaStreamSynchronize(st) != cudaSuccess) rc = OMNI_ERR_CUDA;
         }
         if (!h.outer_go) break;
     }
-    return OMNI_OK;
+    (void)executed_k34; (void)seen_cg;
+    if (prof) {
+        cudaStreamSynchronize(st);
+        // launches that found the loop flag cleared return at once; keep only those that did the work:
+        // a kernel that ran is >= 10x longer than an idle one, so split at 1/4 of the per-kind median
+        std::vector<float> ms(recs.size(), 0.f);
+        for (size_t i = 0; i < recs.size(); ++i) cudaEventElapsedTime(&ms[i], recs[i].e0, recs[i].e1);
+        std::lock_guard<std::mutex> lk(g_prof_mu);
+        for (int kind = 0; kind < 3; ++kind) {
+            std::vector<float> v;
+            for (size_t i = 0; i < recs.size(); ++i) if (recs[i].which == kind) v.push_back(ms[i]);
+            if (v.empty()) continue;
+            std::vector<float> sorted = v;
+            std::sort(sorted.begin(), sorted.end());
+            const float cut = 0.25f * sorted[sorted.size() / 2];
+            for (float x : v) if (x >= cut) { g_prof_ms[kind] += x; g_prof_n[kind] += 1; }
+        }
+        for (auto& r : recs) { cudaEventDestroy(r.e0); cudaEventDestroy(r.e1); }
+    }
+    return rc;
 }
 
 // CUDA-graph loop: outer WHILE { K2 ; inner WHILE { K3 ; K4 } }, conditions written by the kernels' last CTAs.
@@ -390,7 +455,7 @@ int solve_ws(int nx, int ny, int nz, double dx, double dy, double dz, const T* g
     carve<T>(g, (char*)ws, &w);
     HostConst H;
     host_constants(nz, dx, dy, dz, H);
-    const Coef<T> K = make_coef<T>(H, dx, dy, dz);
+    const Coef<T> K = make_coef<T>(H, dx, dy, dz, nz);
 
     init_scalars_kernel<<<1, 1, 0, st>>>(w.sc, tol, max_outer, max_cg);
     CK(cudaGetLastError());
@@ -491,7 +556,7 @@ int step_begin(StepCtx<T>& c, int nx, int ny, int nz, double dx, double dy, doub
     if (cudaMallocAsync(&c.ws, bytes, c.st) != cudaSuccess) { cudaGetLastError(); return OMNI_ERR_ALLOC; }
     carve<T>(c.g, (char*)c.ws, &c.w);
     host_constants(nz, dx, dy, dz, c.H);
-    c.K = make_coef<T>(c.H, dx, dy, dz);
+    c.K = make_coef<T>(c.H, dx, dy, dz, nz);
     init_scalars_kernel<<<1, 1, 0, c.st>>>(c.w.sc, 0.0, 0, 0);
     g_launches.fetch_add(1, std::memory_order_relaxed);
     int rc = setup_codes<T>(c.g, c.w, gx, gy, gz, mask, c.st);
@@ -697,6 +762,21 @@ int omni_residual_f32(int nx, int ny, int nz, double dx, double dy, double dz, c
 long long omni_launch_count(int reset)
 {
     return reset ? g_launches.exchange(0) : g_launches.load();
+}
+
+int omni_profile_enable(int on)
+{
+    return g_profile.exchange(on ? 1 : 0);
+}
+
+void omni_profile_read(double* h_ms3, long long* h_count3, int reset)
+{
+    std::lock_guard<std::mutex> lk(g_prof_mu);
+    for (int i = 0; i < 3; ++i) {
+        if (h_ms3) h_ms3[i] = g_prof_ms[i];
+        if (h_count3) h_count3[i] = g_prof_n[i];
+        if (reset) { g_prof_ms[i] = 0.0; g_prof_n[i] = 0; }
+    }
 }
 
 int omni_set_loop_mode(int mode)

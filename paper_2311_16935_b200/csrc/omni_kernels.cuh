@@ -33,6 +33,8 @@ struct Coef {
     T cab[3];  // c_{a,(a+1)%3} / A_tot  side-face constants   (Eq. 17 / Eq. 33 :317)
     T cac[3];  // c_{a,(a+2)%3} / A_tot
     T hs[3];   // Delta_a * t_a / 2: face-average factor of the source term (Eq. 9 :100)
+    T lut[3][32];      // lut[a][far | nb<<1 | nc<<3] = far*caa + nb*cab + nc*cac: weight of a coded link
+    uint32_t icode;    // wcode of a fully interior cell of this geometry (2D: no z links)
 };
 
 // device-resident loop state: no scalar ever visits the host inside the iteration
@@ -102,11 +104,12 @@ __device__ __forceinline__ double warp_sum(double v)
     return v;
 }
 
-// weight of one link from its 5 code bits (Eq. 16/19 :202/:223, Eq. 25 :266, divided by A_tot)
+// weight of one link from its 5 code bits (Eq. 16/19 :202/:223, Eq. 25 :266, divided by A_tot): table in the
+// kernel-parameter constant bank
 template <typename T>
 __device__ __forceinline__ T link_weight(uint32_t bits, const Coef<T>& K, int a)
 {
-    return T(bits & 1u) * K.caa[a] + T((bits >> 1) & 3u) * K.cab[a] + T((bits >> 3) & 3u) * K.cac[a];
+    return K.lut[a][bits & 31u];
 }
 
 // (M p)_C = p_C - sum_d w1_d p_{C+d}   (Eq. 9 rearranged, A1); general (coded) cell
@@ -145,13 +148,17 @@ __device__ __forceinline__ void apply_M_chunk(T (&q)[V], const T (&vm)[V], const
             q[i] = apply_M_interior(vc[i], e, w, vn[i], vs[i], vp[i], vm[i], K);
         }
     } else {
+        // only the cells whose code differs from the interior code take the coded path: a warp pays for as many
+        // coded cells as its worst lane has, not for whole chunks (every row has two lanes next to the box faces)
         uint32_t code[V];
         ld_chunk<uint32_t, V>(wcode + idx, code);
 #pragma unroll
         for (int i = 0; i < V; ++i) {
             T w = (i == 0) ? xl : vc[i - 1];
             T e = (i == V - 1) ? xr : vc[i + 1];
-            q[i] = apply_M_coded(code[i], vc[i], e, w, vn[i], vs[i], vp[i], vm[i], K);
+            T qi = apply_M_interior(vc[i], e, w, vn[i], vs[i], vp[i], vm[i], K);
+            if (code[i] != K.icode) qi = apply_M_coded(code[i], vc[i], e, w, vn[i], vs[i], vp[i], vm[i], K);
+            q[i] = qi;
         }
     }
 }
@@ -163,383 +170,6 @@ __device__ __forceinline__ uint32_t flag_bits(const uint32_t* __restrict__ flags
     long long g = idx >> 2;
     return (flags[g >> 5] >> (unsigned)(g & 31)) & ((1u << (V / 4)) - 1u);
 }
-
-// ------------------------------------------------------------------------------------------------ tile engine
-//
-// Op supplies: VT (value type of the stencil input), V (cells per thread, 32 bytes of the widest streamed array),
-// TYR (rows per CTA incl. the two halo rows), MINB, NACC, TICKET, Args, Ctx, Raw (+ load / convert), Extra
-// (+ load_extra), emit, active, finalize.
-
-__device__ __forceinline__ void set_cond(const CondHandles& h, int outer, int inner);
-
-template <class Op>
-__global__ void __launch_bounds__(32 * Op::TYR, Op::MINB)
-march_kernel(const Geom g, const int zlen, const typename Op::Args a)
-{
-    using VT = typename Op::VT;
-    constexpr int V = Op::V, TYR = Op::TYR, TYO = TYR - 2, W = 32 * V, NACC = Op::NACC;
-    __shared__ __align__(16) VT sm[2][TYR][W];
-    __shared__ double red[NACC][TYR];
-    __shared__ int is_last;
-
-    if (!Op::active(a)) {       // uniform: the device-side loop state says this launch has nothing to do
-        if (threadIdx.x == 0 && threadIdx.y == 0 && blockIdx.x == 0 && blockIdx.y == 0 && blockIdx.z == 0) Op::idle(a);
-        return;
-    }
-
-    const int lane = threadIdx.x, ty = threadIdx.y;
-    const int x = blockIdx.x * W + lane * V;
-    const int j = blockIdx.y * TYO + ty - 1;
-    const int k0 = blockIdx.z * zlen;
-    const int k1 = min(g.nz, k0 + zlen);
-    const bool ldok = (x < g.px) && (j >= 0) && (j < g.ny);
-    const bool outrow = ldok && (ty >= 1) && (ty <= TYO);
-    const bool lok = ldok && (lane == 0) && (x > 0);
-    const bool rok = ldok && (lane == 31) && (x + V < g.px);
-    const long long rowbase = (long long)j * g.px + x;
-
-    const typename Op::Ctx ctx(a);
-    VT vm[V], vc[V], vp[V], hlc, hrc, hlp, hrp;
-    typename Op::Raw raw;
-    typename Op::Extra exc, exn;
-    double acc[NACC];
-#pragma unroll
-    for (int i = 0; i < NACC; ++i) acc[i] = 0.0;
-
-    {   // prologue: planes k0-1, k0, k0+1
-        VT d0, d1;
-        Op::load(raw, a, ctx, rowbase + (long long)(k0 - 1) * g.pplane, ldok && k0 > 0, false, false);
-        Op::convert(raw, ctx, vm, d0, d1);
-        Op::load(raw, a, ctx, rowbase + (long long)k0 * g.pplane, ldok, lok, rok);
-        Op::convert(raw, ctx, vc, hlc, hrc);
-        Op::load(raw, a, ctx, rowbase + (long long)(k0 + 1) * g.pplane, ldok && (k0 + 1 < g.nz), lok && (k0 + 1 < g.nz),
-                 rok && (k0 + 1 < g.nz));
-        Op::convert(raw, ctx, vp, hlp, hrp);
-        Op::load_extra(exc, a, rowbase + (long long)k0 * g.pplane, outrow);
-    }
-
-    int buf = 0;
-    for (int k = k0; k < k1; ++k) {
-        const long long idx = rowbase + (long long)k * g.pplane;
-        // prefetch plane k+2 (needed as plane k+1 of the next step; the plane after the segment is its halo)
-        const bool nxt = (k + 2 <= k1) && (k + 2 < g.nz);
-        Op::load(raw, a, ctx, idx + 2 * g.pplane, ldok && nxt, lok && nxt, rok && nxt);
-        Op::load_extra(exn, a, idx + g.pplane, outrow && (k + 1 < k1));
-
-        st_chunk<VT, V>(&sm[buf][ty][lane * V], vc);
-        __syncthreads();
-
-        VT xl = __shfl_up_sync(0xffffffffu, vc[V - 1], 1);
-        VT xr = __shfl_down_sync(0xffffffffu, vc[0], 1);
-        if (lane == 0) xl = hlc;
-        if (lane == 31) xr = hrc;
-
-        if (outrow) {
-            VT vn[V], vs[V];
-            ld_chunk<VT, V>(&sm[buf][ty + 1][lane * V], vn);
-            ld_chunk<VT, V>(&sm[buf][ty - 1][lane * V], vs);
-            Op::emit(a, ctx, idx, vm, vc, vp, vn, vs, xl, xr, exc, acc);
-        }
-#pragma unroll
-        for (int i = 0; i < V; ++i) { vm[i] = vc[i]; vc[i] = vp[i]; }
-        hlc = hlp; hrc = hrp;
-        Op::convert(raw, ctx, vp, hlp, hrp);
-        exc = exn;
-        buf ^= 1;
-    }
-
-    // deterministic grid reduction: CTA partial -> fixed slot -> last-arriving CTA sums all slots in slot order
-    const int tid = ty * 32 + lane, nthr = 32 * TYR;
-    const unsigned int nblk = gridDim.x * gridDim.y * gridDim.z;
-    const unsigned int bid = blockIdx.x + gridDim.x * (blockIdx.y + gridDim.y * blockIdx.z);
-#pragma unroll
-    for (int i = 0; i < NACC; ++i) {
-        double s = warp_sum(acc[i]);
-        if (lane == 0) red[i][ty] = s;
-    }
-    __syncthreads();
-    if (tid == 0) {
-#pragma unroll
-        for (int i = 0; i < NACC; ++i) {
-            double s = 0.0;
-            for (int w = 0; w < TYR; ++w) s += red[i][w];
-            a.partial[(size_t)i * nblk + bid] = s;
-        }
-        __threadfence();
-        unsigned int t = atomicAdd(&a.sc->ticket[Op::TICKET], 1u);
-        is_last = (t == nblk - 1);
-    }
-    __syncthreads();
-    if (is_last) {
-        __threadfence();
-        double tot[NACC];
-#pragma unroll
-        for (int i = 0; i < NACC; ++i) {
-            double s = 0.0;
-            for (unsigned int b = tid; b < nblk; b += nthr) s += __ldcg(&a.partial[(size_t)i * nblk + b]);
-            s = warp_sum(s);
-            __syncthreads();
-            if (lane == 0) red[i][ty] = s;
-            __syncthreads();
-            s = 0.0;
-            for (int w = 0; w < TYR; ++w) s += red[i][w];
-            tot[i] = s;
-        }
-        if (tid == 0) {
-            a.sc->ticket[Op::TICKET] = 0;
-            Op::finalize(a, tot);
-        }
-    }
-}
-
-__device__ __forceinline__ void set_cond(const CondHandles& h, int outer, int inner)
-{
-#if defined(__CUDA_ARCH__)
-    if (h.use) {
-        if (outer >= 0) cudaGraphSetConditional((cudaGraphConditionalHandle)h.h_outer, (unsigned)outer);
-        if (inner >= 0) cudaGraphSetConditional((cudaGraphConditionalHandle)h.h_inner, (unsigned)inner);
-    }
-#endif
-}
-
-// ------------------------------------------------------------------------------------------------ K3
-// p_new = r + beta p_old on the fly (also in the halo), store p_new, gamma = p_new . M p_new; alpha = rho / gamma.
-template <typename T, int TYR_, int MINB_>
-struct OpK3 {
-    using VT = T;
-    enum { V = 32 / sizeof(T), TYR = TYR_, MINB = MINB_, NACC = 1, TICKET = 0 };
-    struct Args {
-        const T* r; T* pbuf[2]; const uint32_t* wcode; const uint32_t* flags;
-        Coef<T> K; Scalars* sc; double* partial; CondHandles cond;
-    };
-    struct Ctx {
-        T beta; const T* pold; T* pnew;
-        __device__ Ctx(const Args& a)
-        {
-            beta = (T)a.sc->beta;
-            int par = a.sc->k & 1;
-            pold = a.pbuf[par]; pnew = a.pbuf[par ^ 1];
-        }
-    };
-    struct Raw { T r[V], p[V], rl, pl, rr, pr; };
-    struct Extra {};
-    __device__ static bool active(const Args& a) { return a.sc->inner_go != 0; }
-    __device__ static void idle(const Args& a) { set_cond(a.cond, -1, 0); }
-    __device__ static void load(Raw& w, const Args& a, const Ctx& c, long long idx, bool ok, bool lok, bool rok)
-    {
-        if (ok) { ld_chunk<T, V>(a.r + idx, w.r); ld_chunk<T, V>(c.pold + idx, w.p); }
-        else { zero_chunk<T, V>(w.r); zero_chunk<T, V>(w.p); }
-        w.rl = lok ? a.r[idx - 1] : T(0); w.pl = lok ? c.pold[idx - 1] : T(0);
-        w.rr = rok ? a.r[idx + V] : T(0); w.pr = rok ? c.pold[idx + V] : T(0);
-    }
-    __device__ static void convert(const Raw& w, const Ctx& c, T (&v)[V], T& hl, T& hr)
-    {
-#pragma unroll
-        for (int i = 0; i < V; ++i) v[i] = w.r[i] + c.beta * w.p[i];
-        hl = w.rl + c.beta * w.pl;
-        hr = w.rr + c.beta * w.pr;
-    }
-    __device__ static void load_extra(Extra&, const Args&, long long, bool) {}
-    __device__ static void emit(const Args& a, const Ctx& c, long long idx, const T (&vm)[V], const T (&vc)[V],
-                                const T (&vp)[V], const T (&vn)[V], const T (&vs)[V], T xl, T xr, const Extra&,
-                                double (&acc)[1])
-    {
-        st_chunk<T, V>(c.pnew + idx, vc);
-        T q[V];
-        apply_M_chunk<T, V>(q, vm, vc, vp, vn, vs, xl, xr, flag_bits<V>(a.flags, idx), a.wcode, idx, a.K);
-#pragma unroll
-        for (int i = 0; i < V; ++i) acc[0] += (double)vc[i] * (double)q[i];
-    }
-    __device__ static void finalize(const Args& a, const double (&tot)[1])
-    {
-        Scalars* s = a.sc;
-        double gamma = tot[0];
-        s->gamma = gamma;
-        if (!(gamma > 0.0) || !isfinite(gamma)) {      // also catches NaN
-            s->status = ST_BREAKDOWN; s->inner_go = 0; s->outer_go = 0;
-            set_cond(a.cond, 0, 0);
-        } else {
-            s->alpha = s->rho / gamma;
-        }
-    }
-};
-
-// ------------------------------------------------------------------------------------------------ K4
-// q = M p recomputed from p (never stored), delta += alpha p, r -= alpha q, rho' = r.r; beta = rho'/rho; loop test.
-template <typename T, int TYR_, int MINB_>
-struct OpK4 {
-    using VT = T;
-    enum { V = 32 / sizeof(T), TYR = TYR_, MINB = MINB_, NACC = 1, TICKET = 1 };
-    struct Args {
-        T* r; T* delta; const T* pbuf[2]; const uint32_t* wcode; const uint32_t* flags;
-        Coef<T> K; Scalars* sc; double* partial; CondHandles cond;
-        T* q_out;        // only for omni_apply_M: store q, leave r/delta untouched (NULL inside the solve)
-    };
-    struct Ctx {
-        T alpha; const T* p; bool first;
-        __device__ Ctx(const Args& a)
-        {
-            alpha = (T)a.sc->alpha;
-            first = (a.sc->k == 0);
-            p = a.pbuf[(a.sc->k & 1) ^ 1];
-        }
-    };
-    struct Raw { T p[V], pl, pr; };
-    struct Extra { T r[V], d[V]; };
-    __device__ static bool active(const Args& a) { return a.sc->inner_go != 0; }
-    __device__ static void idle(const Args& a) { set_cond(a.cond, -1, 0); }
-    __device__ static void load(Raw& w, const Args&, const Ctx& c, long long idx, bool ok, bool lok, bool rok)
-    {
-        if (ok) ld_chunk<T, V>(c.p + idx, w.p); else zero_chunk<T, V>(w.p);
-        w.pl = lok ? c.p[idx - 1] : T(0);
-        w.pr = rok ? c.p[idx + V] : T(0);
-    }
-    __device__ static void convert(const Raw& w, const Ctx&, T (&v)[V], T& hl, T& hr)
-    {
-#pragma unroll
-        for (int i = 0; i < V; ++i) v[i] = w.p[i];
-        hl = w.pl; hr = w.pr;
-    }
-    __device__ static void load_extra(Extra& e, const Args& a, long long idx, bool ok)
-    {
-        if (ok && a.q_out == nullptr) { ld_chunk<T, V>(a.r + idx, e.r); ld_chunk<T, V>(a.delta + idx, e.d); }
-        else { zero_chunk<T, V>(e.r); zero_chunk<T, V>(e.d); }
-    }
-    __device__ static void emit(const Args& a, const Ctx& c, long long idx, const T (&vm)[V], const T (&vc)[V],
-                                const T (&vp)[V], const T (&vn)[V], const T (&vs)[V], T xl, T xr, const Extra& e,
-                                double (&acc)[1])
-    {
-        T q[V];
-        apply_M_chunk<T, V>(q, vm, vc, vp, vn, vs, xl, xr, flag_bits<V>(a.flags, idx), a.wcode, idx, a.K);
-        if (a.q_out != nullptr) {           // operator-only mode (omni_apply_M): q and p.q
-            st_chunk<T, V>(a.q_out + idx, q);
-#pragma unroll
-            for (int i = 0; i < V; ++i) acc[0] += (double)vc[i] * (double)q[i];
-            return;
-        }
-        T rn[V], dn[V];
-#pragma unroll
-        for (int i = 0; i < V; ++i) {
-            rn[i] = e.r[i] - c.alpha * q[i];
-            dn[i] = (c.first ? T(0) : e.d[i]) + c.alpha * vc[i];
-            acc[0] += (double)rn[i] * (double)rn[i];
-        }
-        st_chunk<T, V>(a.r + idx, rn);
-        st_chunk<T, V>(a.delta + idx, dn);
-    }
-    __device__ static void finalize(const Args& a, const double (&tot)[1])
-    {
-        Scalars* s = a.sc;
-        if (a.q_out != nullptr) { s->gamma = tot[0]; return; }
-        double rho1 = tot[0];
-        if (!isfinite(rho1)) {
-            s->status = ST_BREAKDOWN; s->inner_go = 0; s->outer_go = 0;
-            set_cond(a.cond, 0, 0);
-            return;
-        }
-        s->beta = rho1 / s->rho;
-        s->rho = rho1;
-        s->k += 1;
-        s->cg_total += 1;
-        int go = (rho1 > s->thresh2) && (rho1 != 0.0) && (s->k < s->max_cg);
-        s->inner_go = go;
-        set_cond(a.cond, -1, go);
-    }
-};
-
-// ------------------------------------------------------------------------------------------------ K2
-// outer boundary update (Eq. 12 collapsed): P <- P + delta; r0 = S - L P with
-// (L P)_C = sum_d v(C+d) t_a (P_C - P_{C+d}) = ([W^{n+1}] - [W^n]) P; eps_R^2 ||S||^2 = ||r0||^2 (Eq. 41).
-// P is always fp64 (master pressure, A9); delta, S, r are T.  P is double-buffered: neighbouring CTAs read
-// P + delta in their halos, so the folded field goes to the other buffer (read Pbuf[n&1], write Pbuf[(n&1)^1]).
-template <typename T, int TYR_, int MINB_>
-struct OpK2 {
-    using VT = double;
-    enum { V = 4, TYR = TYR_, MINB = MINB_, NACC = 2, TICKET = 2 };
-    struct Args {
-        double* Pbuf[2]; const T* delta; const T* S; T* r; const uint8_t* link; const uint32_t* flags;
-        double t[3]; Scalars* sc; double* partial; CondHandles cond;
-        int fold_delta;   // 0: residual of P as given (omni_residual); 1: inside the solve
-    };
-    struct Ctx {
-        const double* Pin; double* Pout;
-        __device__ Ctx(const Args& a) { int par = a.sc->n & 1; Pin = a.Pbuf[par]; Pout = a.Pbuf[par ^ 1]; }
-    };
-    struct Raw { double P[V]; T d[V]; double Pl, Pr; T dl, dr; };
-    struct Extra { T S[V]; };
-    __device__ static bool active(const Args& a) { return a.sc->outer_go != 0; }
-    __device__ static void idle(const Args& a) { set_cond(a.cond, 0, 0); }
-    __device__ static void load(Raw& w, const Args& a, const Ctx& c, long long idx, bool ok, bool lok, bool rok)
-    {
-        if (ok) { ld_chunk<double, V>(c.Pin + idx, w.P); ld_chunk<T, V>(a.delta + idx, w.d); }
-        else { zero_chunk<double, V>(w.P); zero_chunk<T, V>(w.d); }
-        w.Pl = lok ? c.Pin[idx - 1] : 0.0; w.dl = lok ? a.delta[idx - 1] : T(0);
-        w.Pr = rok ? c.Pin[idx + V] : 0.0; w.dr = rok ? a.delta[idx + V] : T(0);
-    }
-    __device__ static void convert(const Raw& w, const Ctx&, double (&v)[V], double& hl, double& hr)
-    {
-#pragma unroll
-        for (int i = 0; i < V; ++i) v[i] = w.P[i] + (double)w.d[i];
-        hl = w.Pl + (double)w.dl;
-        hr = w.Pr + (double)w.dr;
-    }
-    __device__ static void load_extra(Extra& e, const Args& a, long long idx, bool ok)
-    {
-        if (ok) ld_chunk<T, V>(a.S + idx, e.S); else zero_chunk<T, V>(e.S);
-    }
-    __device__ static void emit(const Args& a, const Ctx& c, long long idx, const double (&vm)[V], const double (&vc)[V],
-                                const double (&vp)[V], const double (&vn)[V], const double (&vs)[V], double xl,
-                                double xr, const Extra& e, double (&acc)[2])
-    {
-        if (a.fold_delta) st_chunk<double, V>(c.Pout + idx, vc);
-        uint32_t fb = flag_bits<V>(a.flags, idx);
-        uint32_t lk = 0x7f7f7f7fu;
-        if (fb) lk = *reinterpret_cast<const uint32_t*>(a.link + idx);
-        T rn[V];
-#pragma unroll
-        for (int i = 0; i < V; ++i) {
-            double w = (i == 0) ? xl : vc[i - 1];
-            double ee = (i == V - 1) ? xr : vc[i + 1];
-            uint32_t l = (lk >> (8 * i)) & 0xffu;
-            double LP = 0.0;
-            if (l & 1u) LP += a.t[0] * (vc[i] - ee);
-            if (l & 2u) LP += a.t[0] * (vc[i] - w);
-            if (l & 4u) LP += a.t[1] * (vc[i] - vn[i]);
-            if (l & 8u) LP += a.t[1] * (vc[i] - vs[i]);
-            if (l & 16u) LP += a.t[2] * (vc[i] - vp[i]);
-            if (l & 32u) LP += a.t[2] * (vc[i] - vm[i]);
-            double rr = (l & LINK_VALID) ? ((double)e.S[i] - LP) : 0.0;
-            rn[i] = (T)rr;
-            acc[0] += rr * rr;
-            acc[1] += (double)rn[i] * (double)rn[i];
-        }
-        st_chunk<T, V>(a.r + idx, rn);
-    }
-    __device__ static void finalize(const Args& a, const double (&tot)[2])
-    {
-        Scalars* s = a.sc;
-        s->epsR2 = tot[0];
-        if (!a.fold_delta) return;
-        if (!isfinite(tot[0])) {
-            s->status = ST_BREAKDOWN; s->inner_go = 0; s->outer_go = 0;
-            set_cond(a.cond, 0, 0);
-            return;
-        }
-        if (tot[0] <= s->tol2S || s->n >= s->max_outer) {
-            s->status = (tot[0] <= s->tol2S) ? ST_OK : ST_NOT_CONVERGED;
-            s->inner_go = 0; s->outer_go = 0;
-            set_cond(a.cond, 0, 0);
-            return;
-        }
-        s->n += 1;
-        s->k = 0;
-        s->beta = 0.0;
-        s->rho = tot[1];
-        int go = (tot[1] > s->thresh2) && (tot[1] != 0.0) && (s->max_cg > 0);
-        s->inner_go = go;
-        set_cond(a.cond, 1, go);
-    }
-};
 
 // ------------------------------------------------------------------------------------------------ K0a validity
 template <typename T>

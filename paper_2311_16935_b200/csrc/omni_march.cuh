@@ -1,0 +1,472 @@
+// omni_march.cuh -- the z-marching tile engine shared by K2 / K3 / K4, and the three operators.
+//
+// A CTA owns a column of the grid: W = 32*V cells wide (1 KB of the widest streamed array), TYR-2 output rows (+2 halo
+// rows), zlen planes (+1 halo plane on each side).  Every thread owns one 32-byte chunk per streamed array and plane.
+//   * global -> shared: each thread copies ITS chunks of the planes ahead with cp.async (LDGSTS, zero-fill outside the
+//     box) into a D-deep ring of private shared-memory slots, so (D-1) planes x all streamed arrays are in flight per
+//     SM without holding registers; nobody else reads those slots, so the ring needs no barrier.
+//   * registers: stencil input of planes k-1, k, k+1 for the own chunk (z neighbours).
+//   * y neighbours: the current plane is published to a double-buffered exchange tile (one __syncthreads per plane);
+//     x neighbours: warp shuffles, plus two scalar halo cells per row copied with the ring.
+//   * reduction: fp64 per-thread partials -> warp shuffle -> CTA -> fixed slot; the last-arriving CTA (atomic ticket)
+//     adds the slots in slot order and updates the device-resident loop scalars (deterministic; no host sync).
+#pragma once
+#include "omni_kernels.cuh"
+
+namespace omni {
+
+__device__ __forceinline__ void set_cond(const CondHandles& h, int outer, int inner)
+{
+#if defined(__CUDA_ARCH__)
+    if (h.use) {
+        if (outer >= 0) cudaGraphSetConditional((cudaGraphConditionalHandle)h.h_outer, (unsigned)outer);
+        if (inner >= 0) cudaGraphSetConditional((cudaGraphConditionalHandle)h.h_inner, (unsigned)inner);
+    }
+#endif
+}
+
+__device__ __forceinline__ void cp_async16(uint32_t dst, const void* src, bool ok)
+{
+    const int sz = ok ? 16 : 0;      // src-size 0: nothing is read, the 16 destination bytes are zero-filled
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(dst), "l"(src), "r"(sz) : "memory");
+}
+template <int B>
+__device__ __forceinline__ void cp_async_small(uint32_t dst, const void* src, bool ok)
+{
+    const int sz = ok ? B : 0;
+    asm volatile("cp.async.ca.shared.global [%0], [%1], %2, %3;" ::"r"(dst), "l"(src), "n"(B), "r"(sz) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+
+// one ring stage seen by one thread: PIECES 16-byte pieces (piece q of thread t at (q*NTHR + t)*16: conflict-free
+// LDS.128), then 4 halo slots of 8 bytes per row
+template <int NTHR, int PIECES>
+struct StageW {
+    uint32_t base, halo;     // shared-space addresses
+    int tid;
+    template <typename T, int NP>
+    __device__ __forceinline__ void put(int q0, const T* src, long long idx, bool ok) const
+    {
+        constexpr int EPP = 16 / (int)sizeof(T);     // elements per piece
+#pragma unroll
+        for (int i = 0; i < NP; ++i)
+            cp_async16(base + (uint32_t)(((q0 + i) * NTHR + tid) * 16), ok ? (const void*)(src + idx + i * EPP) : (const void*)src, ok);
+    }
+    template <typename T>
+    __device__ __forceinline__ void put_halo(int slot, const T* src, long long idx, bool ok) const
+    {
+        cp_async_small<(int)sizeof(T)>(halo + (uint32_t)(slot * 8), ok ? (const void*)(src + idx) : (const void*)src, ok);
+    }
+};
+template <int NTHR, int PIECES>
+struct StageR {
+    const char* base;
+    const char* halo;
+    int tid;
+    template <typename T, int V>
+    __device__ __forceinline__ void get(int q0, T (&v)[V]) const
+    {
+        constexpr int NP = V * (int)sizeof(T) / 16;
+        uint4 u[NP];
+#pragma unroll
+        for (int i = 0; i < NP; ++i) u[i] = *reinterpret_cast<const uint4*>(base + ((q0 + i) * NTHR + tid) * 16);
+        memcpy(v, u, sizeof(u));
+    }
+    template <typename T>
+    __device__ __forceinline__ T get_halo(int slot) const { return *reinterpret_cast<const T*>(halo + slot * 8); }
+};
+
+template <class Op>
+struct MarchSmem {
+    static constexpr int NTHR = 32 * Op::TYR;
+    static constexpr int STAGE_BYTES = Op::PIECES * NTHR * 16 + Op::TYR * 4 * 8;
+    static constexpr int XCH_BYTES = 2 * Op::TYR * 32 * Op::V * (int)sizeof(typename Op::VT);
+    static constexpr int TOTAL = Op::D * STAGE_BYTES + XCH_BYTES;
+};
+
+template <class Op>
+__global__ void __launch_bounds__(32 * Op::TYR, 1)
+march_kernel(const Geom g, const int zlen, const typename Op::Args a)
+{
+    using VT = typename Op::VT;
+    constexpr int V = Op::V, TYR = Op::TYR, TYO = TYR - 2, W = 32 * V, NACC = Op::NACC, D = Op::D;
+    constexpr int NTHR = 32 * TYR, PIECES = Op::PIECES;
+    using SM = MarchSmem<Op>;
+    extern __shared__ __align__(16) char smem[];
+    __shared__ double red[NACC][TYR];
+    __shared__ int is_last;
+
+    if (!Op::active(a)) {       // uniform: the device-side loop state says this launch has nothing to do
+        if (threadIdx.x == 0 && threadIdx.y == 0 && blockIdx.x == 0 && blockIdx.y == 0 && blockIdx.z == 0) Op::idle(a);
+        return;
+    }
+
+    const int lane = threadIdx.x, ty = threadIdx.y, tid = ty * 32 + lane;
+    const int x = blockIdx.x * W + lane * V;
+    const int j = blockIdx.y * TYO + ty - 1;
+    const int k0 = blockIdx.z * zlen;
+    const int k1 = min(g.nz, k0 + zlen);
+    const bool ldok = (x < g.px) && (j >= 0) && (j < g.ny);
+    const bool outrow = ldok && (ty >= 1) && (ty <= TYO);
+    const bool lok = ldok && (lane == 0) && (x > 0);
+    const bool rok = ldok && (lane == 31) && (x + V < g.px);
+    const long long rowbase = (long long)j * g.px + x;
+
+    VT(*xch)[TYR][W] = reinterpret_cast<VT(*)[TYR][W]>(smem + D * SM::STAGE_BYTES);
+    const uint32_t smem_s = (uint32_t)__cvta_generic_to_shared(smem);
+
+    const typename Op::Ctx ctx(a);
+
+    // event c consumes the main arrays of plane c and the extra arrays of plane c-1; its data sits in ring slot
+    // (c - k0 + 1) % D.  Planes outside [0, nz) and the far side of the segment's halo planes are zero-filled.
+    auto issue = [&](int c) {
+        const int slot = (c - k0 + 1) % D;
+        StageW<NTHR, PIECES> st{ smem_s + (uint32_t)(slot * SM::STAGE_BYTES),
+                                 smem_s + (uint32_t)(slot * SM::STAGE_BYTES + PIECES * NTHR * 16 + ty * 32), tid };
+        const bool pin = (c >= 0) && (c < g.nz) && (c <= k1);
+        const bool ein = (c - 1 >= k0) && (c - 1 < k1);
+        Op::issue(a, ctx, st, rowbase + (long long)c * g.pplane, ldok && pin, lok && pin, rok && pin,
+                  rowbase + (long long)(c - 1) * g.pplane, outrow && ein);
+        cp_async_commit();
+    };
+
+    VT vm[V], vc[V], vn_[V], hlc = VT(0), hrc = VT(0), hln, hrn;
+    typename Op::Extra ex;
+    double acc[NACC];
+#pragma unroll
+    for (int i = 0; i < NACC; ++i) acc[i] = 0.0;
+    zero_chunk<VT, V>(vm);
+    zero_chunk<VT, V>(vc);
+
+#pragma unroll
+    for (int s = 0; s < D; ++s) issue(k0 - 1 + s);
+
+    int buf = 0;
+    for (int c = k0 - 1; c <= k1; ++c) {
+        cp_async_wait<D - 1>();
+        {
+            const int slot = (c - k0 + 1) % D;
+            StageR<NTHR, PIECES> sr{ smem + slot * SM::STAGE_BYTES,
+                                     smem + slot * SM::STAGE_BYTES + PIECES * NTHR * 16 + ty * 32, tid };
+            Op::consume(a, ctx, sr, vn_, hln, hrn, ex);
+        }
+        issue(c + D);
+        if (c >= k0 + 1) {           // emit plane c-1: vm = plane c-2, vc = plane c-1, vn_ = plane c
+            const long long idx = rowbase + (long long)(c - 1) * g.pplane;
+            st_chunk<VT, V>(&xch[buf][ty][lane * V], vc);
+            __syncthreads();
+            VT xl = __shfl_up_sync(0xffffffffu, vc[V - 1], 1);
+            VT xr = __shfl_down_sync(0xffffffffu, vc[0], 1);
+            if (lane == 0) xl = hlc;
+            if (lane == 31) xr = hrc;
+            if (outrow) {
+                VT vN[V], vS[V];
+                ld_chunk<VT, V>(&xch[buf][ty + 1][lane * V], vN);
+                ld_chunk<VT, V>(&xch[buf][ty - 1][lane * V], vS);
+                Op::emit(a, ctx, idx, vm, vc, vn_, vN, vS, xl, xr, ex, acc);
+            }
+            buf ^= 1;
+        }
+#pragma unroll
+        for (int i = 0; i < V; ++i) { vm[i] = vc[i]; vc[i] = vn_[i]; }
+        hlc = hln; hrc = hrn;
+    }
+    cp_async_wait<0>();
+
+    // deterministic grid reduction: CTA partial -> fixed slot -> last-arriving CTA sums all slots in slot order
+    const unsigned int nblk = gridDim.x * gridDim.y * gridDim.z;
+    const unsigned int bid = blockIdx.x + gridDim.x * (blockIdx.y + gridDim.y * blockIdx.z);
+#pragma unroll
+    for (int i = 0; i < NACC; ++i) {
+        double s = warp_sum(acc[i]);
+        if (lane == 0) red[i][ty] = s;
+    }
+    __syncthreads();
+    if (tid == 0) {
+#pragma unroll
+        for (int i = 0; i < NACC; ++i) {
+            double s = 0.0;
+            for (int w = 0; w < TYR; ++w) s += red[i][w];
+            a.partial[(size_t)i * nblk + bid] = s;
+        }
+        __threadfence();
+        unsigned int t = atomicAdd(&a.sc->ticket[Op::TICKET], 1u);
+        is_last = (t == nblk - 1);
+    }
+    __syncthreads();
+    if (is_last) {
+        __threadfence();
+        double tot[NACC];
+#pragma unroll
+        for (int i = 0; i < NACC; ++i) {
+            double s = 0.0;
+            for (unsigned int b = tid; b < nblk; b += NTHR) s += __ldcg(&a.partial[(size_t)i * nblk + b]);
+            s = warp_sum(s);
+            __syncthreads();
+            if (lane == 0) red[i][ty] = s;
+            __syncthreads();
+            s = 0.0;
+            for (int w = 0; w < TYR; ++w) s += red[i][w];
+            tot[i] = s;
+        }
+        if (tid == 0) {
+            a.sc->ticket[Op::TICKET] = 0;
+            Op::finalize(a, tot);
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------------ K3
+// p_new = r + beta p_old on the fly (also in the halo), store p_new, gamma = p_new . M p_new; alpha = rho / gamma.
+template <typename T, int TYR_, int D_>
+struct OpK3 {
+    using VT = T;
+    enum { V = 32 / sizeof(T), TYR = TYR_, D = D_, NACC = 1, TICKET = 0, PIECES = 4 };
+    struct Args {
+        const T* r; T* pbuf[2]; const uint32_t* wcode; const uint32_t* flags;
+        Coef<T> K; Scalars* sc; double* partial; CondHandles cond;
+    };
+    struct Ctx {
+        T beta; const T* pold; T* pnew;
+        __device__ Ctx(const Args& a)
+        {
+            beta = (T)a.sc->beta;
+            int par = a.sc->k & 1;
+            pold = a.pbuf[par]; pnew = a.pbuf[par ^ 1];
+        }
+    };
+    struct Extra {};
+    __device__ static bool active(const Args& a) { return a.sc->inner_go != 0; }
+    __device__ static void idle(const Args& a) { set_cond(a.cond, -1, 0); }
+    template <class SW>
+    __device__ static void issue(const Args& a, const Ctx& c, const SW& st, long long idx, bool ok, bool lok, bool rok,
+                                 long long, bool)
+    {
+        st.template put<T, 2>(0, a.r, idx, ok);
+        st.template put<T, 2>(2, c.pold, idx, ok);
+        if (threadIdx.x == 0) { st.put_halo(0, a.r, idx - 1, lok); st.put_halo(1, c.pold, idx - 1, lok); }
+        if (threadIdx.x == 31) { st.put_halo(2, a.r, idx + V, rok); st.put_halo(3, c.pold, idx + V, rok); }
+    }
+    template <class SR>
+    __device__ static void consume(const Args&, const Ctx& c, const SR& sr, T (&v)[V], T& hl, T& hr, Extra&)
+    {
+        T r[V], p[V];
+        sr.template get<T, V>(0, r);
+        sr.template get<T, V>(2, p);
+#pragma unroll
+        for (int i = 0; i < V; ++i) v[i] = r[i] + c.beta * p[i];
+        hl = hr = T(0);
+        if (threadIdx.x == 0) hl = sr.template get_halo<T>(0) + c.beta * sr.template get_halo<T>(1);
+        if (threadIdx.x == 31) hr = sr.template get_halo<T>(2) + c.beta * sr.template get_halo<T>(3);
+    }
+    __device__ static void emit(const Args& a, const Ctx& c, long long idx, const T (&vm)[V], const T (&vc)[V],
+                                const T (&vp)[V], const T (&vn)[V], const T (&vs)[V], T xl, T xr, const Extra&,
+                                double (&acc)[1])
+    {
+        st_chunk<T, V>(c.pnew + idx, vc);
+        T q[V];
+        apply_M_chunk<T, V>(q, vm, vc, vp, vn, vs, xl, xr, flag_bits<V>(a.flags, idx), a.wcode, idx, a.K);
+#pragma unroll
+        for (int i = 0; i < V; ++i) acc[0] += (double)vc[i] * (double)q[i];
+    }
+    __device__ static void finalize(const Args& a, const double (&tot)[1])
+    {
+        Scalars* s = a.sc;
+        double gamma = tot[0];
+        s->gamma = gamma;
+        if (!(gamma > 0.0) || !isfinite(gamma)) {      // also catches NaN
+            s->status = ST_BREAKDOWN; s->inner_go = 0; s->outer_go = 0;
+            set_cond(a.cond, 0, 0);
+        } else {
+            s->alpha = s->rho / gamma;
+        }
+    }
+};
+
+// ------------------------------------------------------------------------------------------------ K4
+// q = M p recomputed from p (never stored), delta += alpha p, r -= alpha q, rho' = r.r; beta = rho'/rho; loop test.
+template <typename T, int TYR_, int D_>
+struct OpK4 {
+    using VT = T;
+    enum { V = 32 / sizeof(T), TYR = TYR_, D = D_, NACC = 1, TICKET = 1, PIECES = 6 };
+    struct Args {
+        T* r; T* delta; const T* pbuf[2]; const uint32_t* wcode; const uint32_t* flags;
+        Coef<T> K; Scalars* sc; double* partial; CondHandles cond;
+        T* q_out;        // only for omni_apply_M: store q, leave r/delta untouched (NULL inside the solve)
+    };
+    struct Ctx {
+        T alpha; const T* p; bool first;
+        __device__ Ctx(const Args& a)
+        {
+            alpha = (T)a.sc->alpha;
+            first = (a.sc->k == 0);
+            p = a.pbuf[(a.sc->k & 1) ^ 1];
+        }
+    };
+    struct Extra { T r[V], d[V]; };
+    __device__ static bool active(const Args& a) { return a.sc->inner_go != 0; }
+    __device__ static void idle(const Args& a) { set_cond(a.cond, -1, 0); }
+    template <class SW>
+    __device__ static void issue(const Args& a, const Ctx& c, const SW& st, long long idx, bool ok, bool lok, bool rok,
+                                 long long eidx, bool eok)
+    {
+        st.template put<T, 2>(0, c.p, idx, ok);
+        if (threadIdx.x == 0) st.put_halo(0, c.p, idx - 1, lok);
+        if (threadIdx.x == 31) st.put_halo(1, c.p, idx + V, rok);
+        const bool e = eok && (a.q_out == nullptr);
+        st.template put<T, 2>(2, (const T*)a.r, eidx, e);
+        st.template put<T, 2>(4, (const T*)a.delta, eidx, e && !c.first);
+    }
+    template <class SR>
+    __device__ static void consume(const Args&, const Ctx&, const SR& sr, T (&v)[V], T& hl, T& hr, Extra& e)
+    {
+        sr.template get<T, V>(0, v);
+        hl = hr = T(0);
+        if (threadIdx.x == 0) hl = sr.template get_halo<T>(0);
+        if (threadIdx.x == 31) hr = sr.template get_halo<T>(1);
+        sr.template get<T, V>(2, e.r);
+        sr.template get<T, V>(4, e.d);
+    }
+    __device__ static void emit(const Args& a, const Ctx& c, long long idx, const T (&vm)[V], const T (&vc)[V],
+                                const T (&vp)[V], const T (&vn)[V], const T (&vs)[V], T xl, T xr, const Extra& e,
+                                double (&acc)[1])
+    {
+        T q[V];
+        apply_M_chunk<T, V>(q, vm, vc, vp, vn, vs, xl, xr, flag_bits<V>(a.flags, idx), a.wcode, idx, a.K);
+        if (a.q_out != nullptr) {           // operator-only mode (omni_apply_M): q and p.q
+            st_chunk<T, V>(a.q_out + idx, q);
+#pragma unroll
+            for (int i = 0; i < V; ++i) acc[0] += (double)vc[i] * (double)q[i];
+            return;
+        }
+        T rn[V], dn[V];
+#pragma unroll
+        for (int i = 0; i < V; ++i) {
+            rn[i] = e.r[i] - c.alpha * q[i];
+            dn[i] = e.d[i] + c.alpha * vc[i];       // first CG iteration: delta was zero-filled by the ring
+            acc[0] += (double)rn[i] * (double)rn[i];
+        }
+        st_chunk<T, V>(a.r + idx, rn);
+        st_chunk<T, V>(a.delta + idx, dn);
+    }
+    __device__ static void finalize(const Args& a, const double (&tot)[1])
+    {
+        Scalars* s = a.sc;
+        if (a.q_out != nullptr) { s->gamma = tot[0]; return; }
+        double rho1 = tot[0];
+        if (!isfinite(rho1)) {
+            s->status = ST_BREAKDOWN; s->inner_go = 0; s->outer_go = 0;
+            set_cond(a.cond, 0, 0);
+            return;
+        }
+        s->beta = rho1 / s->rho;
+        s->rho = rho1;
+        s->k += 1;
+        s->cg_total += 1;
+        int go = (rho1 > s->thresh2) && (rho1 != 0.0) && (s->k < s->max_cg);
+        s->inner_go = go;
+        set_cond(a.cond, -1, go);
+    }
+};
+
+// ------------------------------------------------------------------------------------------------ K2
+// outer boundary update (Eq. 12 collapsed): P <- P + delta; r0 = S - L P with
+// (L P)_C = sum_d v(C+d) t_a (P_C - P_{C+d}) = ([W^{n+1}] - [W^n]) P; eps_R^2 ||S||^2 = ||r0||^2 (Eq. 41).
+// P is always fp64 (master pressure, A9); delta, S, r are T.  P is double-buffered: neighbouring CTAs read
+// P + delta in their halos, so the folded field goes to the other buffer (read Pbuf[n&1], write Pbuf[(n&1)^1]).
+template <typename T, int TYR_, int D_>
+struct OpK2 {
+    using VT = double;
+    enum { V = 4, TYR = TYR_, D = D_, NACC = 2, TICKET = 2, NPT = 4 * sizeof(T) / 16, PIECES = 2 + 2 * NPT };
+    struct Args {
+        double* Pbuf[2]; const T* delta; const T* S; T* r; const uint8_t* link; const uint32_t* flags;
+        double t[3]; Scalars* sc; double* partial; CondHandles cond;
+        int fold_delta;   // 0: residual of P as given (omni_residual); 1: inside the solve
+    };
+    struct Ctx {
+        const double* Pin; double* Pout;
+        __device__ Ctx(const Args& a) { int par = a.sc->n & 1; Pin = a.Pbuf[par]; Pout = a.Pbuf[par ^ 1]; }
+    };
+    struct Extra { T S[V]; };
+    __device__ static bool active(const Args& a) { return a.sc->outer_go != 0; }
+    __device__ static void idle(const Args& a) { set_cond(a.cond, 0, 0); }
+    template <class SW>
+    __device__ static void issue(const Args& a, const Ctx& c, const SW& st, long long idx, bool ok, bool lok, bool rok,
+                                 long long eidx, bool eok)
+    {
+        st.template put<double, 2>(0, c.Pin, idx, ok);
+        st.template put<T, NPT>(2, a.delta, idx, ok);
+        if (threadIdx.x == 0) { st.put_halo(0, c.Pin, idx - 1, lok); st.put_halo(1, a.delta, idx - 1, lok); }
+        if (threadIdx.x == 31) { st.put_halo(2, c.Pin, idx + V, rok); st.put_halo(3, a.delta, idx + V, rok); }
+        st.template put<T, NPT>(2 + NPT, a.S, eidx, eok);
+    }
+    template <class SR>
+    __device__ static void consume(const Args&, const Ctx&, const SR& sr, double (&v)[V], double& hl, double& hr, Extra& e)
+    {
+        double P[V]; T d[V];
+        sr.template get<double, V>(0, P);
+        sr.template get<T, V>(2, d);
+#pragma unroll
+        for (int i = 0; i < V; ++i) v[i] = P[i] + (double)d[i];
+        hl = hr = 0.0;
+        if (threadIdx.x == 0) hl = sr.template get_halo<double>(0) + (double)sr.template get_halo<T>(1);
+        if (threadIdx.x == 31) hr = sr.template get_halo<double>(2) + (double)sr.template get_halo<T>(3);
+        sr.template get<T, V>(2 + NPT, e.S);
+    }
+    __device__ static void emit(const Args& a, const Ctx& c, long long idx, const double (&vm)[V], const double (&vc)[V],
+                                const double (&vp)[V], const double (&vn)[V], const double (&vs)[V], double xl,
+                                double xr, const Extra& e, double (&acc)[2])
+    {
+        if (a.fold_delta) st_chunk<double, V>(c.Pout + idx, vc);
+        uint32_t fb = flag_bits<V>(a.flags, idx);
+        uint32_t lk = 0x7f7f7f7fu;
+        if (fb) lk = *reinterpret_cast<const uint32_t*>(a.link + idx);
+        T rn[V];
+#pragma unroll
+        for (int i = 0; i < V; ++i) {
+            double w = (i == 0) ? xl : vc[i - 1];
+            double ee = (i == V - 1) ? xr : vc[i + 1];
+            uint32_t l = (lk >> (8 * i)) & 0xffu;
+            double LP = 0.0;
+            if (l & 1u) LP += a.t[0] * (vc[i] - ee);
+            if (l & 2u) LP += a.t[0] * (vc[i] - w);
+            if (l & 4u) LP += a.t[1] * (vc[i] - vn[i]);
+            if (l & 8u) LP += a.t[1] * (vc[i] - vs[i]);
+            if (l & 16u) LP += a.t[2] * (vc[i] - vp[i]);
+            if (l & 32u) LP += a.t[2] * (vc[i] - vm[i]);
+            double rr = (l & LINK_VALID) ? ((double)e.S[i] - LP) : 0.0;
+            rn[i] = (T)rr;
+            acc[0] += rr * rr;
+            acc[1] += (double)rn[i] * (double)rn[i];
+        }
+        st_chunk<T, V>(a.r + idx, rn);
+    }
+    __device__ static void finalize(const Args& a, const double (&tot)[2])
+    {
+        Scalars* s = a.sc;
+        s->epsR2 = tot[0];
+        if (!a.fold_delta) return;
+        if (!isfinite(tot[0])) {
+            s->status = ST_BREAKDOWN; s->inner_go = 0; s->outer_go = 0;
+            set_cond(a.cond, 0, 0);
+            return;
+        }
+        if (tot[0] <= s->tol2S || s->n >= s->max_outer) {
+            s->status = (tot[0] <= s->tol2S) ? ST_OK : ST_NOT_CONVERGED;
+            s->inner_go = 0; s->outer_go = 0;
+            set_cond(a.cond, 0, 0);
+            return;
+        }
+        s->n += 1;
+        s->k = 0;
+        s->beta = 0.0;
+        s->rho = tot[1];
+        int go = (tot[1] > s->thresh2) && (tot[1] != 0.0) && (s->max_cg > 0);
+        s->inner_go = go;
+        set_cond(a.cond, 1, go);
+    }
+};
+
+}  // namespace omni
