@@ -84,7 +84,7 @@ void host_constants(int nz, double dx, double dy, double dz, HostConst& H)
 }
 
 template <typename T>
-Coef<T> make_coef(const HostConst& H, double dx, double dy, double dz, int nz)
+Coef<T> make_coef(const HostConst& H, double dx, double dy, double dz, const Geom& g)
 {
     Coef<T> K;
     const double d[3] = { dx, dy, dz };
@@ -99,29 +99,56 @@ Coef<T> make_coef(const HostConst& H, double dx, double dy, double dz, int nz)
             K.lut[a][bits] = (T)((far * H.c[a][a] + nb * H.c[a][(a + 1) % 3] + nc * H.c[a][(a + 2) % 3]) / H.Atot);
         }
     }
-    // interior code: every active axis has both links with far = 1 and two valid side cells along the other active axes
-    const int naxes = (nz > 1) ? 3 : 2;
-    uint32_t icode = WCODE_VALID;
-    for (int d = 0; d < 2 * naxes; ++d) {
-        const int a = d >> 1, b = (a + 1) % 3, c = (a + 2) % 3;
-        const uint32_t bits = 1u | ((b < naxes ? 2u : 0u) << 1) | ((c < naxes ? 2u : 0u) << 3);
-        icode |= bits << (5 * d);
-    }
-    K.icode = icode;
+    K.icode = g.icode;
+    for (int cls = 0; cls < 4; ++cls)
+        for (int d = 0; d < 6; ++d) {
+            const int a = d >> 1;
+            const uint32_t bits = (g.stdc[cls] >> (5 * d)) & 31u;
+            const int far = bits & 1, nb = (bits >> 1) & 3, nc = (bits >> 3) & 3;
+            const double w = (far * H.c[a][a] + nb * H.c[a][(a + 1) % 3] + nc * H.c[a][(a + 2) % 3]) / H.Atot;
+            K.xc[cls][d] = (T)(H.F[a] / H.Atot - w);
+        }
     return K;
 }
 
 // ------------------------------------------------------------------------------------------------ geometry / workspace
 
-bool make_geom(int nx, int ny, int nz, Geom& g)
+// wcode of cell i of a row whose y/z neighbourhood is complete (mirrors codes_kernel with only x bounded)
+uint32_t std_xcode(int i, int nx, int naxes)
+{
+    auto vx = [&](int ii) { return (ii >= 0 && ii < nx) ? 1u : 0u; };
+    uint32_t code = WCODE_VALID;
+    for (int d = 0; d < 2 * naxes; ++d) {
+        const int a = d >> 1, sg = (d & 1) ? -1 : 1;
+        const int qi = i + (a == 0 ? sg : 0);
+        if (!vx(qi)) continue;
+        const int b = (a + 1) % 3, c = (a + 2) % 3;
+        const uint32_t far = vx(qi + (a == 0 ? sg : 0));
+        auto side = [&](int ax) -> uint32_t {
+            if (ax >= naxes) return 0u;
+            if (ax == 0) return vx(qi + 1) + vx(qi - 1);
+            return 2u;
+        };
+        code |= (far | (side(b) << 1) | (side(c) << 3)) << (5 * d);
+    }
+    return code;
+}
+
+bool make_geom(int nx, int ny, int nz, int elem_size, Geom& g)
 {
     if (nx < 1 || ny < 1 || nz < 1) return false;
-    const long long px = ((long long)nx + 7) / 8 * 8;
+    const long long pad = (elem_size == 4) ? 8 : 4;        // one thread chunk = 32 bytes
+    const long long px = ((long long)nx + pad - 1) / pad * pad;
     const long long npad = px * (long long)ny * (long long)nz;
     if (npad > (1LL << 40) || px > 0x7fffffff) return false;
     g.nx = nx; g.ny = ny; g.nz = nz; g.px = (int)px;
     g.pplane = px * ny;
     g.npad = npad;
+    const int naxes = (nz > 1) ? 3 : 2;
+    g.xfix = (nx >= 4) ? 1 : 0;
+    g.icode = std_xcode(2, 5, naxes);
+    g.stdc[0] = std_xcode(0, nx, naxes); g.stdc[1] = std_xcode(1, nx, naxes);
+    g.stdc[2] = std_xcode(nx - 2, nx, naxes); g.stdc[3] = std_xcode(nx - 1, nx, naxes);
     return true;
 }
 
@@ -446,7 +473,7 @@ int solve_ws(int nx, int ny, int nz, double dx, double dy, double dz, const T* g
              void* stream, omni_info* info)
 {
     Geom g;
-    if (!valid_common(nx, ny, nz, dx, dy, dz, tol, max_outer, max_cg) || !make_geom(nx, ny, nz, g)) return OMNI_ERR_INVALID_ARG;
+    if (!valid_common(nx, ny, nz, dx, dy, dz, tol, max_outer, max_cg) || !make_geom(nx, ny, nz, (int)sizeof(T), g)) return OMNI_ERR_INVALID_ARG;
     if (!gx || !gy || (nz > 1 && !gz) || !P_out || !ws) return OMNI_ERR_INVALID_ARG;
     if (((uintptr_t)ws & 255) != 0) return OMNI_ERR_INVALID_ARG;
     if (ws_bytes < carve<T>(g, nullptr, nullptr)) return OMNI_ERR_ALLOC;
@@ -455,7 +482,7 @@ int solve_ws(int nx, int ny, int nz, double dx, double dy, double dz, const T* g
     carve<T>(g, (char*)ws, &w);
     HostConst H;
     host_constants(nz, dx, dy, dz, H);
-    const Coef<T> K = make_coef<T>(H, dx, dy, dz, nz);
+    const Coef<T> K = make_coef<T>(H, dx, dy, dz, g);
 
     init_scalars_kernel<<<1, 1, 0, st>>>(w.sc, tol, max_outer, max_cg);
     CK(cudaGetLastError());
@@ -493,7 +520,7 @@ int solve_alloc(int nx, int ny, int nz, double dx, double dy, double dz, const T
                 const unsigned char* mask, T* P_out, double tol, int max_outer, int max_cg, void* stream, omni_info* info)
 {
     Geom g;
-    if (!valid_common(nx, ny, nz, dx, dy, dz, tol, max_outer, max_cg) || !make_geom(nx, ny, nz, g)) return OMNI_ERR_INVALID_ARG;
+    if (!valid_common(nx, ny, nz, dx, dy, dz, tol, max_outer, max_cg) || !make_geom(nx, ny, nz, (int)sizeof(T), g)) return OMNI_ERR_INVALID_ARG;
     cudaStream_t st = (cudaStream_t)stream;
     const size_t bytes = carve<T>(g, nullptr, nullptr);
     void* ws = nullptr;
@@ -508,7 +535,7 @@ int solve_host(int nx, int ny, int nz, double dx, double dy, double dz, const T*
                const unsigned char* mask, T* P_out, double tol, int max_outer, int max_cg, void* stream, omni_info* info)
 {
     Geom g;
-    if (!valid_common(nx, ny, nz, dx, dy, dz, tol, max_outer, max_cg) || !make_geom(nx, ny, nz, g)) return OMNI_ERR_INVALID_ARG;
+    if (!valid_common(nx, ny, nz, dx, dy, dz, tol, max_outer, max_cg) || !make_geom(nx, ny, nz, (int)sizeof(T), g)) return OMNI_ERR_INVALID_ARG;
     if (!gx || !gy || (nz > 1 && !gz) || !P_out) return OMNI_ERR_INVALID_ARG;
     cudaStream_t st = (cudaStream_t)stream;
     const size_t n = (size_t)nx * ny * nz;
@@ -549,14 +576,14 @@ template <typename T>
 int step_begin(StepCtx<T>& c, int nx, int ny, int nz, double dx, double dy, double dz, const T* gx, const T* gy,
                const T* gz, const unsigned char* mask, void* stream)
 {
-    if (!valid_common(nx, ny, nz, dx, dy, dz, 0.0, 0, 0) || !make_geom(nx, ny, nz, c.g)) return OMNI_ERR_INVALID_ARG;
+    if (!valid_common(nx, ny, nz, dx, dy, dz, 0.0, 0, 0) || !make_geom(nx, ny, nz, (int)sizeof(T), c.g)) return OMNI_ERR_INVALID_ARG;
     c.st = (cudaStream_t)stream;
     const size_t bytes = carve<T>(c.g, nullptr, nullptr);
     c.ws = nullptr;
     if (cudaMallocAsync(&c.ws, bytes, c.st) != cudaSuccess) { cudaGetLastError(); return OMNI_ERR_ALLOC; }
     carve<T>(c.g, (char*)c.ws, &c.w);
     host_constants(nz, dx, dy, dz, c.H);
-    c.K = make_coef<T>(c.H, dx, dy, dz, nz);
+    c.K = make_coef<T>(c.H, dx, dy, dz, c.g);
     init_scalars_kernel<<<1, 1, 0, c.st>>>(c.w.sc, 0.0, 0, 0);
     g_launches.fetch_add(1, std::memory_order_relaxed);
     int rc = setup_codes<T>(c.g, c.w, gx, gy, gz, mask, c.st);
@@ -677,10 +704,9 @@ int omni_solve_f32(int nx, int ny, int nz, double dx, double dy, double dz, cons
 size_t omni_workspace_bytes(int nx, int ny, int nz, int dtype)
 {
     Geom g;
-    if (!make_geom(nx, ny, nz, g)) return 0;
-    if (dtype == OMNI_F32) return carve<float>(g, nullptr, nullptr);
-    if (dtype == OMNI_F64) return carve<double>(g, nullptr, nullptr);
-    return 0;
+    if (dtype != OMNI_F32 && dtype != OMNI_F64) return 0;
+    if (!make_geom(nx, ny, nz, dtype == OMNI_F32 ? 4 : 8, g)) return 0;
+    return dtype == OMNI_F32 ? carve<float>(g, nullptr, nullptr) : carve<double>(g, nullptr, nullptr);
 }
 
 int omni_solve_f64_ws(int nx, int ny, int nz, double dx, double dy, double dz, const double* d_gx, const double* d_gy,

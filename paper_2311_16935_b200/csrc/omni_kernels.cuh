@@ -23,6 +23,11 @@ struct Geom {
     int px;              // padded row pitch in cells (multiple of 8); cells nx..px-1 are permanently missing
     long long pplane;    // px * ny
     long long npad;      // px * ny * nz
+    // x-edge classes of an otherwise regular row (y, z neighbourhood complete): wcode of cells 0, 1, nx-2, nx-1.
+    // Groups whose codes are the interior code or these are NOT flagged: the fast path plus a per-lane correction
+    // (xedge_fix) covers them, so the box faces normal to x cost no divergent coded path in every warp.
+    uint32_t icode, stdc[4];
+    int xfix;            // 1 iff nx >= 4 (the four classes are distinct cells)
 };
 
 // stencil coefficients, already divided by A_tot (Eq. 10 :109), in the arithmetic type T
@@ -34,8 +39,26 @@ struct Coef {
     T cac[3];  // c_{a,(a+2)%3} / A_tot
     T hs[3];   // Delta_a * t_a / 2: face-average factor of the source term (Eq. 9 :100)
     T lut[3][32];      // lut[a][far | nb<<1 | nc<<3] = far*caa + nb*cab + nc*cac: weight of a coded link
+    T xc[4][6];        // xc[class][d] = t_a - w_d(stdc[class]): what the fast path over-subtracts at x-edge cells
     uint32_t icode;    // wcode of a fully interior cell of this geometry (2D: no z links)
 };
+
+// which x-edge cells a thread's chunk holds (thread constants)
+struct XEdge {
+    bool L, A, B;      // holds cells {0,1} / cell nx-2 / cell nx-1
+    int posA, posB;    // their positions inside the chunk
+};
+template <int V>
+__device__ __forceinline__ XEdge make_xedge(const Geom& g, int x)
+{
+    XEdge e;
+    const bool on = g.xfix != 0;
+    e.L = on && (x == 0);
+    e.posA = (g.nx - 2) % V; e.posB = (g.nx - 1) % V;
+    e.A = on && (x == g.nx - 2 - e.posA);
+    e.B = on && (x == g.nx - 1 - e.posB);
+    return e;
+}
 
 // device-resident loop state: no scalar ever visits the host inside the iteration
 struct Scalars {
@@ -134,31 +157,72 @@ __device__ __forceinline__ T apply_M_interior(T c, T e, T w, T n, T s, T f, T b,
     return c - K.t[0] * (e + w) - K.t[1] * (n + s) - K.t[2] * (f + b);
 }
 
-// q = M p for the V cells of one thread; fb = interior-flag bits of the thread's 4-cell groups (0 = all interior)
+// q[I] += sum_d xc[cls][d] * neighbour_d: turns the interior formula into the exact one at an x-edge cell
+template <int I, typename T, int V>
+__device__ __forceinline__ void xfix_cell(T (&q)[V], const T (&vm)[V], const T (&vc)[V], const T (&vp)[V],
+                                          const T (&vn)[V], const T (&vs)[V], T xl, T xr, const T (&c)[6])
+{
+    const T w = (I == 0) ? xl : vc[I > 0 ? I - 1 : 0];
+    const T e = (I == V - 1) ? xr : vc[I < V - 1 ? I + 1 : V - 1];
+    q[I] += c[0] * e + c[1] * w + c[2] * vn[I] + c[3] * vs[I] + c[4] * vp[I] + c[5] * vm[I];
+}
+template <int I, typename T, int V>
+__device__ __forceinline__ void xfix_zero_after(T (&q)[V])
+{
+#pragma unroll
+    for (int i = I + 1; i < V; ++i) q[i] = T(0);      // pad cells nx..px-1
+}
+
+template <typename T, int V>
+__device__ __forceinline__ void xedge_fix(T (&q)[V], const T (&vm)[V], const T (&vc)[V], const T (&vp)[V],
+                                          const T (&vn)[V], const T (&vs)[V], T xl, T xr, const XEdge& xe,
+                                          const Coef<T>& K)
+{
+    if (xe.L) {
+        xfix_cell<0, T, V>(q, vm, vc, vp, vn, vs, xl, xr, K.xc[0]);
+        xfix_cell<1, T, V>(q, vm, vc, vp, vn, vs, xl, xr, K.xc[1]);
+    }
+    if (xe.A) {
+        switch (xe.posA) {
+#define OMNI_CASE(I) case I: if (I < V) xfix_cell<(I < V ? I : 0), T, V>(q, vm, vc, vp, vn, vs, xl, xr, K.xc[2]); break;
+            OMNI_CASE(0) OMNI_CASE(1) OMNI_CASE(2) OMNI_CASE(3) OMNI_CASE(4) OMNI_CASE(5) OMNI_CASE(6) OMNI_CASE(7)
+#undef OMNI_CASE
+        }
+    }
+    if (xe.B) {
+        switch (xe.posB) {
+#define OMNI_CASE(I) case I: if (I < V) { xfix_cell<(I < V ? I : 0), T, V>(q, vm, vc, vp, vn, vs, xl, xr, K.xc[3]); \
+                                          xfix_zero_after<(I < V ? I : 0), T, V>(q); } break;
+            OMNI_CASE(0) OMNI_CASE(1) OMNI_CASE(2) OMNI_CASE(3) OMNI_CASE(4) OMNI_CASE(5) OMNI_CASE(6) OMNI_CASE(7)
+#undef OMNI_CASE
+        }
+    }
+}
+
+// q = M p for the V cells of one thread; fb = flag bits of the thread's 4-cell groups (0 = interior or regular
+// x-edge: fast path; else the chunk's codes are read and the cells that need it take the coded path)
 template <typename T, int V>
 __device__ __forceinline__ void apply_M_chunk(T (&q)[V], const T (&vm)[V], const T (&vc)[V], const T (&vp)[V],
                                               const T (&vn)[V], const T (&vs)[V], T xl, T xr, uint32_t fb,
-                                              const uint32_t* __restrict__ wcode, long long idx, const Coef<T>& K)
+                                              const uint32_t* __restrict__ wcode, long long idx, const Coef<T>& K,
+                                              const XEdge& xe)
 {
-    if (fb == 0) {
 #pragma unroll
-        for (int i = 0; i < V; ++i) {
-            T w = (i == 0) ? xl : vc[i - 1];
-            T e = (i == V - 1) ? xr : vc[i + 1];
-            q[i] = apply_M_interior(vc[i], e, w, vn[i], vs[i], vp[i], vm[i], K);
-        }
+    for (int i = 0; i < V; ++i) {
+        T w = (i == 0) ? xl : vc[i - 1];
+        T e = (i == V - 1) ? xr : vc[i + 1];
+        q[i] = apply_M_interior(vc[i], e, w, vn[i], vs[i], vp[i], vm[i], K);
+    }
+    if (fb == 0) {
+        if (xe.L || xe.A || xe.B) xedge_fix<T, V>(q, vm, vc, vp, vn, vs, xl, xr, xe, K);
     } else {
-        // only the cells whose code differs from the interior code take the coded path: a warp pays for as many
-        // coded cells as its worst lane has, not for whole chunks (every row has two lanes next to the box faces)
         uint32_t code[V];
         ld_chunk<uint32_t, V>(wcode + idx, code);
 #pragma unroll
         for (int i = 0; i < V; ++i) {
             T w = (i == 0) ? xl : vc[i - 1];
             T e = (i == V - 1) ? xr : vc[i + 1];
-            T qi = apply_M_interior(vc[i], e, w, vn[i], vs[i], vp[i], vm[i], K);
-            if (code[i] != K.icode) qi = apply_M_coded(code[i], vc[i], e, w, vn[i], vs[i], vp[i], vm[i], K);
-            q[i] = qi;
+            if (code[i] != K.icode) q[i] = apply_M_coded(code[i], vc[i], e, w, vn[i], vs[i], vp[i], vm[i], K);
         }
     }
 }
@@ -218,16 +282,15 @@ __global__ void codes_kernel(Geom g, const uint8_t* __restrict__ vbyte, uint8_t*
         for (int c = 0; c < 4; ++c) {
             const int i = i0 + c;
             uint32_t code = 0, lk = 0;
-            bool interior = false;
             if (vget(g, vbyte, i, j, k)) {
-                code = WCODE_VALID; lk = LINK_VALID; interior = true;
+                code = WCODE_VALID; lk = LINK_VALID;
                 for (int d = 0; d < 6; ++d) {
                     const int a = d >> 1, sg = (d & 1) ? -1 : 1;
                     int e[3] = { 0, 0, 0 };
                     e[a] = sg;
                     const int qi = i + e[0], qj = j + e[1], qk = k + e[2];
                     if (a >= naxes) continue;                       // 2D scheme: no F/B links at all
-                    if (!vget(g, vbyte, qi, qj, qk)) { interior = false; continue; }
+                    if (!vget(g, vbyte, qi, qj, qk)) continue;
                     lk |= 1u << d;
                     const int b = (a + 1) % 3, cc = (a + 2) % 3;
                     int eb[3] = { 0, 0, 0 }, ec[3] = { 0, 0, 0 };
@@ -238,13 +301,19 @@ __global__ void codes_kernel(Geom g, const uint8_t* __restrict__ vbyte, uint8_t*
                     uint32_t nc = vget(g, vbyte, qi + ec[0], qj + ec[1], qk + ec[2]) +
                                   vget(g, vbyte, qi - ec[0], qj - ec[1], qk - ec[2]);
                     code |= (far | (nb << 1) | (nc << 3)) << (5 * d);
-                    const uint32_t nb_full = (b < naxes) ? 2u : 0u, nc_full = (cc < naxes) ? 2u : 0u;
-                    if (far != 1u || nb != nb_full || nc != nc_full) interior = false;
                 }
             }
             codes[c] = code;
             links |= lk << (8 * c);
-            flagged |= !interior;
+            uint32_t expect = g.icode;
+            if (g.xfix) {
+                if (i >= g.nx) expect = 0u;
+                else if (i == 0) expect = g.stdc[0];
+                else if (i == 1) expect = g.stdc[1];
+                else if (i == g.nx - 2) expect = g.stdc[2];
+                else if (i == g.nx - 1) expect = g.stdc[3];
+            }
+            flagged |= (code != expect);
         }
         *reinterpret_cast<uint4*>(wcode + base) = make_uint4(codes[0], codes[1], codes[2], codes[3]);
         *reinterpret_cast<uint32_t*>(link + base) = links;

@@ -118,17 +118,16 @@ march_kernel(const Geom g, const int zlen, const typename Op::Args a)
     const uint32_t smem_s = (uint32_t)__cvta_generic_to_shared(smem);
 
     const typename Op::Ctx ctx(a);
+    const typename Op::TC tc = Op::thread_init(g, x);
 
     // event c consumes the main arrays of plane c and the extra arrays of plane c-1; its data sits in ring slot
     // (c - k0 + 1) % D.  Planes outside [0, nz) and the far side of the segment's halo planes are zero-filled.
-    auto issue = [&](int c) {
-        const int slot = (c - k0 + 1) % D;
+    auto issue = [&](int c, int slot, long long off) {      // off = rowbase + c * pplane
         StageW<NTHR, PIECES> st{ smem_s + (uint32_t)(slot * SM::STAGE_BYTES),
                                  smem_s + (uint32_t)(slot * SM::STAGE_BYTES + PIECES * NTHR * 16 + ty * 32), tid };
         const bool pin = (c >= 0) && (c < g.nz) && (c <= k1);
         const bool ein = (c - 1 >= k0) && (c - 1 < k1);
-        Op::issue(a, ctx, st, rowbase + (long long)c * g.pplane, ldok && pin, lok && pin, rok && pin,
-                  rowbase + (long long)(c - 1) * g.pplane, outrow && ein);
+        Op::issue(a, ctx, st, off, ldok && pin, lok && pin, rok && pin, off - g.pplane, outrow && ein);
         cp_async_commit();
     };
 
@@ -140,21 +139,26 @@ march_kernel(const Geom g, const int zlen, const typename Op::Args a)
     zero_chunk<VT, V>(vm);
     zero_chunk<VT, V>(vc);
 
+    long long off = rowbase + (long long)(k0 - 1) * g.pplane;     // offset of plane c
 #pragma unroll
-    for (int s = 0; s < D; ++s) issue(k0 - 1 + s);
+    for (int s = 0; s < D; ++s) issue(k0 - 1 + s, s, off + s * g.pplane);
+    const long long doff = (long long)D * g.pplane;
 
-    int buf = 0;
+    // flag word of the plane emitted at the NEXT event, fetched one event early so that its latency is hidden
+    uint32_t fw_next = 0, fw_cur = 0;
+    int slot = 0, buf = 0;
     for (int c = k0 - 1; c <= k1; ++c) {
         cp_async_wait<D - 1>();
         {
-            const int slot = (c - k0 + 1) % D;
             StageR<NTHR, PIECES> sr{ smem + slot * SM::STAGE_BYTES,
                                      smem + slot * SM::STAGE_BYTES + PIECES * NTHR * 16 + ty * 32, tid };
             Op::consume(a, ctx, sr, vn_, hln, hrn, ex);
         }
-        issue(c + D);
+        issue(c + D, slot, off + doff);
+        fw_cur = fw_next;
+        if (outrow && c >= k0 && c < k1) fw_next = a.flags[(off >> 2) >> 5];     // plane c is emitted at event c+1
         if (c >= k0 + 1) {           // emit plane c-1: vm = plane c-2, vc = plane c-1, vn_ = plane c
-            const long long idx = rowbase + (long long)(c - 1) * g.pplane;
+            const long long idx = off - g.pplane;
             st_chunk<VT, V>(&xch[buf][ty][lane * V], vc);
             __syncthreads();
             VT xl = __shfl_up_sync(0xffffffffu, vc[V - 1], 1);
@@ -165,13 +169,16 @@ march_kernel(const Geom g, const int zlen, const typename Op::Args a)
                 VT vN[V], vS[V];
                 ld_chunk<VT, V>(&xch[buf][ty + 1][lane * V], vN);
                 ld_chunk<VT, V>(&xch[buf][ty - 1][lane * V], vS);
-                Op::emit(a, ctx, idx, vm, vc, vn_, vN, vS, xl, xr, ex, acc);
+                const uint32_t fb = (fw_cur >> (unsigned)((idx >> 2) & 31)) & ((1u << (V / 4)) - 1u);
+                Op::emit(a, ctx, idx, vm, vc, vn_, vN, vS, xl, xr, ex, fb, tc, acc);
             }
             buf ^= 1;
         }
 #pragma unroll
         for (int i = 0; i < V; ++i) { vm[i] = vc[i]; vc[i] = vn_[i]; }
         hlc = hln; hrc = hrn;
+        off += g.pplane;
+        slot = (slot + 1 == D) ? 0 : slot + 1;
     }
     cp_async_wait<0>();
 
@@ -238,6 +245,8 @@ struct OpK3 {
         }
     };
     struct Extra {};
+    using TC = XEdge;
+    __device__ static TC thread_init(const Geom& g, int x) { return make_xedge<V>(g, x); }
     __device__ static bool active(const Args& a) { return a.sc->inner_go != 0; }
     __device__ static void idle(const Args& a) { set_cond(a.cond, -1, 0); }
     template <class SW>
@@ -263,11 +272,11 @@ struct OpK3 {
     }
     __device__ static void emit(const Args& a, const Ctx& c, long long idx, const T (&vm)[V], const T (&vc)[V],
                                 const T (&vp)[V], const T (&vn)[V], const T (&vs)[V], T xl, T xr, const Extra&,
-                                double (&acc)[1])
+                                uint32_t fb, const TC& xe, double (&acc)[1])
     {
         st_chunk<T, V>(c.pnew + idx, vc);
         T q[V];
-        apply_M_chunk<T, V>(q, vm, vc, vp, vn, vs, xl, xr, flag_bits<V>(a.flags, idx), a.wcode, idx, a.K);
+        apply_M_chunk<T, V>(q, vm, vc, vp, vn, vs, xl, xr, fb, a.wcode, idx, a.K, xe);
 #pragma unroll
         for (int i = 0; i < V; ++i) acc[0] += (double)vc[i] * (double)q[i];
     }
@@ -306,6 +315,8 @@ struct OpK4 {
         }
     };
     struct Extra { T r[V], d[V]; };
+    using TC = XEdge;
+    __device__ static TC thread_init(const Geom& g, int x) { return make_xedge<V>(g, x); }
     __device__ static bool active(const Args& a) { return a.sc->inner_go != 0; }
     __device__ static void idle(const Args& a) { set_cond(a.cond, -1, 0); }
     template <class SW>
@@ -331,10 +342,10 @@ struct OpK4 {
     }
     __device__ static void emit(const Args& a, const Ctx& c, long long idx, const T (&vm)[V], const T (&vc)[V],
                                 const T (&vp)[V], const T (&vn)[V], const T (&vs)[V], T xl, T xr, const Extra& e,
-                                double (&acc)[1])
+                                uint32_t fb, const TC& xe, double (&acc)[1])
     {
         T q[V];
-        apply_M_chunk<T, V>(q, vm, vc, vp, vn, vs, xl, xr, flag_bits<V>(a.flags, idx), a.wcode, idx, a.K);
+        apply_M_chunk<T, V>(q, vm, vc, vp, vn, vs, xl, xr, fb, a.wcode, idx, a.K, xe);
         if (a.q_out != nullptr) {           // operator-only mode (omni_apply_M): q and p.q
             st_chunk<T, V>(a.q_out + idx, q);
 #pragma unroll
@@ -390,6 +401,25 @@ struct OpK2 {
         __device__ Ctx(const Args& a) { int par = a.sc->n & 1; Pin = a.Pbuf[par]; Pout = a.Pbuf[par ^ 1]; }
     };
     struct Extra { T S[V]; };
+    // thread constant: link bytes of an unflagged chunk (all six links, minus the box faces normal to x, pads invalid)
+    using TC = uint32_t;
+    __device__ static TC thread_init(const Geom& g, int x)
+    {
+        uint32_t lk = 0;
+#pragma unroll
+        for (int i = 0; i < V; ++i) {
+            const int gi = x + i;
+            uint32_t l = 0x7fu;
+            if (g.nz == 1) l &= ~48u;
+            if (g.xfix) {
+                if (gi == 0) l &= ~2u;
+                if (gi == g.nx - 1) l &= ~1u;
+                if (gi >= g.nx) l = 0;
+            }
+            lk |= l << (8 * i);
+        }
+        return lk;
+    }
     __device__ static bool active(const Args& a) { return a.sc->outer_go != 0; }
     __device__ static void idle(const Args& a) { set_cond(a.cond, 0, 0); }
     template <class SW>
@@ -417,11 +447,10 @@ struct OpK2 {
     }
     __device__ static void emit(const Args& a, const Ctx& c, long long idx, const double (&vm)[V], const double (&vc)[V],
                                 const double (&vp)[V], const double (&vn)[V], const double (&vs)[V], double xl,
-                                double xr, const Extra& e, double (&acc)[2])
+                                double xr, const Extra& e, uint32_t fb, const TC& lk_const, double (&acc)[2])
     {
         if (a.fold_delta) st_chunk<double, V>(c.Pout + idx, vc);
-        uint32_t fb = flag_bits<V>(a.flags, idx);
-        uint32_t lk = 0x7f7f7f7fu;
+        uint32_t lk = lk_const;
         if (fb) lk = *reinterpret_cast<const uint32_t*>(a.link + idx);
         T rn[V];
 #pragma unroll
