@@ -1,0 +1,273 @@
+#!/usr/bin/env python
+"""bench.py -- grid-point CG updates/s of the omnidirectional pressure-integration hot path on B200.
+
+A step = one omni_solve call (all rows a0-a8 of SURVEY.md section 8(a): constants, codes, source term, outer
+boundary updates, CG inner loops under a CUDA graph, finalize) on one synthetic gradient field, with the outer and
+inner iteration caps fixed (STEP_MAX_OUTER x STEP_MAX_CG) so that every step does the same, bounded work.
+Unit of work: one grid point updated by one CG iteration.  See DESIGN.md section 8 for every figure printed here.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config 0..4] [--dtype f32|f64] [--impl ours|reference]
+
+N > 1 (torchrun): replicas only -- every rank solves its own copy of the workload, no data-path collective.
+--impl reference times the CPU oracle (oracle/, test infrastructure) on a bounded sample of the same workload.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+STEP_MAX_OUTER = 8
+STEP_MAX_CG = 25
+METRIC = "grid-point CG updates/s"
+UNIT = "grid-point CG updates/s"
+CPU_SAMPLE_EDGE = 200                   # 3D: edge of the corner crop the oracle is timed on (2D: the whole grid)
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel (K4) from the ncu --set full capture
+# summarised in profiles/r1_ncu_k3_k4_500cube_f32.md; only valid for that workload.
+NCU_TRAFFIC_K4 = {(4, "f32"): 1.527892e9 + 0.952720e9}
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=4)
+    ap.add_argument("--dtype", default=None)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    return ap.parse_args()
+
+
+def measured_peak():
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            return float(json.load(f)["hbm_gbs"]), "MEASURED_PEAKS.json hbm_gbs (of measured)"
+    except Exception:
+        return 6650.0, "B200_PROFILING.md fallback 6.65 TB/s (of fallback)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled during the timed region (B200_PROFILING.md recipe)."""
+    Q = "clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown," \
+        "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap"
+
+    def __init__(self, index):
+        self.rows, self.stop, self.index = [], threading.Event(), index
+        self.t = threading.Thread(target=self.run, daemon=True)
+
+    def run(self):
+        while not self.stop.is_set():
+            try:
+                out = subprocess.run(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                                      "--format=csv,noheader,nounits"], capture_output=True, text=True, timeout=5).stdout
+                self.rows.append([c.strip() for c in out.strip().split(",")])
+            except Exception:
+                pass
+            self.stop.wait(0.2)
+
+    def __enter__(self):
+        self.t.start()
+        return self
+
+    def __exit__(self, *a):
+        self.stop.set()
+        self.t.join(timeout=6)
+
+    def summary(self):
+        sm = sorted(int(r[0]) for r in self.rows if len(r) >= 6 and r[0].isdigit())
+        reasons = set()
+        for r in self.rows:
+            if len(r) >= 6:
+                for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), r[2:6]):
+                    if v.lower().startswith("active"):
+                        reasons.add(name)
+        mx = max((int(r[1]) for r in self.rows if len(r) >= 6 and r[1].isdigit()), default=None)
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": mx, "reasons": sorted(reasons),
+                "samples": len(sm)}
+
+
+def cpu_sample(f, ndim):
+    """Bounded sample of the workload for the oracle: the corner crop [0:e]^ndim of the same arrays."""
+    import numpy as np
+    e = min(CPU_SAMPLE_EDGE if ndim == 3 else 1024, f["g"][0].shape[0])
+    sl = (slice(0, e),) * ndim
+    g = [np.ascontiguousarray(c[sl]) for c in f["g"]]
+    m = None if f["mask"] is None else np.ascontiguousarray(f["mask"][sl])
+    return g, m, e
+
+
+def run_oracle(f, dtype, steps, warmup):
+    """CPU oracle, as it stands, on the bounded sample; returns (updates/s, cores, sample description)."""
+    import numpy as np
+    from oracle import omni_oracle as orc
+    ndim = f["g"][0].ndim
+    g, m, e = cpu_sample(f, ndim)
+    if dtype == "f32":
+        g = [c.astype(np.float32).astype(np.float64) for c in g]
+    g = g + [None] * (3 - len(g))
+    tol = 1e-5 if dtype == "f32" else 1e-8
+    mo, mc = 4, 25
+    for _ in range(warmup):
+        orc.solve(g[0], g[1], g[2], m, *f["d"], tol=tol, max_outer=mo, max_cg=mc)
+    t0 = time.perf_counter()
+    units = 0
+    for _ in range(steps):
+        _, info = orc.solve(g[0], g[1], g[2], m, *f["d"], tol=tol, max_outer=mo, max_cg=mc)
+        units += g[0].size * info["cg_iters_total"]
+    dt = time.perf_counter() - t0
+    desc = f"corner crop {e}^{ndim} of the same field, omni oracle solve max_outer={mo} max_cg={mc}, {steps} step(s)"
+    return units / dt, orc.num_threads(), desc, dt / steps
+
+
+def main():
+    args = parse()
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    from workloads import CONFIGS, make_config
+    cfg = CONFIGS[args.config]
+    dtype = args.dtype or ("f32" if "f32" in cfg["dtypes"] else "f64")
+    n = cfg["n"]
+    ndim = 2 if cfg["kind"].endswith("2d") else 3
+    workload = f"configs[{args.config}] {cfg['kind']} {n}^{ndim} {dtype} noise={cfg['noise']}"
+    config = {"workload": workload, "step": f"omni_solve tol={'1e-5' if dtype == 'f32' else '1e-8'} "
+              f"max_outer={STEP_MAX_OUTER} max_cg={STEP_MAX_CG} (fixed caps)", "parallelism": f"replicas x{world}",
+              "l2": "inputs larger than L2 (no flush)" if n ** ndim * (4 if dtype == "f32" else 8) > 126e6
+              else "CG state fits L2: numbers are L2-resident, flushed between steps by the solve's own setup passes"}
+
+    if args.impl == "reference":
+        if rank != 0:
+            return
+        f = make_config(args.config)
+        v, cores, desc, spstep = run_oracle(f, dtype, args.steps, args.warmup)
+        print(json.dumps({"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus,
+                          "steps": args.steps, "warmup": args.warmup, "ms_per_step": spstep * 1e3,
+                          "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+                          "data": "synthetic", "config": config,
+                          "cpu_baseline": {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc},
+                          "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}))
+        return
+
+    import torch
+    import paper_2311_16935_b200 as omni
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (no CPU fallback)")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=dev)
+
+    f = make_config(args.config, device=f"cuda:{local_rank}")
+    tdt = torch.float32 if dtype == "f32" else torch.float64
+    g_host = [torch.from_numpy(c).to(tdt).pin_memory() for c in f["g"]]
+    m_host = None if f["mask"] is None else torch.from_numpy(f["mask"]).pin_memory()
+    g = [c.to(dev) for c in g_host] + [None] * (3 - len(g_host))
+    m = None if m_host is None else m_host.to(dev)
+    g_host = g_host + [None] * (3 - len(g_host))
+    d = f["d"]
+    tol = 1e-5 if dtype == "f32" else 1e-8
+    N = g[0].numel()
+    esz = 4 if dtype == "f32" else 8
+    P = torch.empty_like(g[0])
+
+    def step(info=False):
+        return omni.solve(g[0], g[1], g[2], m, d, tol, STEP_MAX_OUTER, STEP_MAX_CG, out=P, want_info=info)
+
+    # warm-up (also gives the deterministic iteration and launch counts of one step)
+    omni.launch_count(reset=True)
+    _, info = step(info=True)
+    launches_per_step = omni.launch_count(reset=True)
+    for _ in range(max(args.warmup - 1, 0)):
+        step()
+    torch.cuda.synchronize()
+    units_per_step = N * info["cg_iters_total"]
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    with ClockSampler(local_rank) as clk:
+        barrier()
+        e0.record()
+        for _ in range(args.steps):
+            step()
+        e1.record()
+        barrier()
+        ms = e0.elapsed_time(e1)
+        # end to end through the C ABI with HOST buffers (pinned): H2D of g/mask and D2H of P inside the timed region
+        P_host = torch.empty_like(g_host[0]).pin_memory()
+        omni.solve(g_host[0], g_host[1], g_host[2], m_host, d, tol, STEP_MAX_OUTER, STEP_MAX_CG, out=P_host)
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(args.steps):
+            omni.solve(g_host[0], g_host[1], g_host[2], m_host, d, tol, STEP_MAX_OUTER, STEP_MAX_CG, out=P_host)
+        torch.cuda.synchronize()
+        e2e_s = time.perf_counter() - t0
+    clocks = clk.summary()
+
+    if world > 1:
+        t = torch.tensor([ms, e2e_s], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms, e2e_s = float(t[0]), float(t[1])
+
+    # per-kernel live timing of the same step (host-driven loop, CUDA events around each launch on the same stream)
+    prev = omni.set_loop_mode(1)
+    omni.profile_enable(1)
+    omni.profile_read(reset=True)
+    step(info=True)
+    prof = omni.profile_read(reset=True)
+    omni.profile_enable(0)
+    omni.set_loop_mode(prev)
+    peak, peak_src = measured_peak()
+    k3_ms, k3_n = prof["K3"]
+    k4_ms, k4_n = prof["K4"]
+    k2_ms, k2_n = prof["K2"]
+    t4 = k4_ms / max(k4_n, 1) * 1e-3
+    t3 = k3_ms / max(k3_n, 1) * 1e-3
+    alg4, alg3 = 5 * esz * N, 3 * esz * N          # K4: R p,r,delta W r,delta ; K3: R r,p W p
+    ach = alg4 / t4 / 1e9 if t4 > 0 else 0.0
+    roofline = {"bound": "hbm", "kernel": "K4 march_kernel<OpK4> (operator recomputed + axpys + r.r)",
+                "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak, "peak_source": peak_src,
+                "traffic": NCU_TRAFFIC_K4.get((args.config, dtype)),
+                "algorithmic_bytes_per_launch": alg4, "us_per_launch": t4 * 1e6,
+                "k3": {"achieved": alg3 / t3 / 1e9 if t3 > 0 else 0.0, "us_per_launch": t3 * 1e6,
+                       "algorithmic_bytes_per_launch": alg3},
+                "cg_iteration": {"us": (t3 + t4) * 1e6, "achieved": (alg3 + alg4) / (t3 + t4) / 1e9 if t3 + t4 > 0 else 0.0,
+                                 "frac": (alg3 + alg4) / (t3 + t4) / 1e9 / peak if t3 + t4 > 0 else 0.0,
+                                 "updates_per_s_in_loop": N / (t3 + t4) if t3 + t4 > 0 else 0.0},
+                "k2_us_per_launch": k2_ms / max(k2_n, 1) * 1e3,
+                "share_of_step": {"K2": k2_ms, "K3": k3_ms, "K4": k4_ms}}
+
+    if rank != 0:
+        return
+    out = {"metric": METRIC, "value": world * units_per_step * args.steps / (ms * 1e-3), "unit": UNIT,
+           "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms / args.steps,
+           "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": dtype, "data": "synthetic",
+           "config": config, "clocks": clocks, "gpu_launches": launches_per_step * args.steps,
+           "e2e": {"value": world * units_per_step * args.steps / e2e_s, "unit": UNIT,
+                   "h2d_bytes_per_step": sum(c.numel() * c.element_size() for c in g_host if c is not None)
+                   + (0 if m_host is None else m_host.numel()), "d2h_bytes_per_step": N * esz,
+                   "ms_per_step": e2e_s / args.steps * 1e3},
+           "step_info": {"outer_iters": info["outer_iters"], "cg_iters": info["cg_iters_total"],
+                         "eps_R": info["eps_R_final"], "status": info["status"]},
+           "roofline": roofline}
+    if world == 1:
+        del g, P
+        torch.cuda.empty_cache()
+        v, cores, desc, _ = run_oracle(f, dtype, 1, 0)
+        out["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc}
+    print(json.dumps(out))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

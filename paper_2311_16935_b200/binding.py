@@ -41,12 +41,14 @@ def lib():
     """Loads libomni.so (building it in-tree first if nvcc is available and the sources are newer)."""
     global _lib
     if _lib is None:
-        path = os.path.join(_HERE, "libomni.so")
-        try:
-            path = _build.build()
-        except Exception:
-            if not os.path.exists(path):
-                raise
+        path = os.environ.get("OMNI_LIB")          # debug: load an alternative build of the same library
+        if not path:
+            path = os.path.join(_HERE, "libomni.so")
+            try:
+                path = _build.build()
+            except Exception:
+                if not os.path.exists(path):
+                    raise
         L = C.CDLL(path)
         L.omni_workspace_bytes.restype = C.c_size_t
         L.omni_launch_count.restype = C.c_longlong

@@ -256,9 +256,15 @@ cudaError_t launch_march(const Geom& g, const typename Op::Args& a, cudaStream_t
 }
 
 // tile shapes: 16 rows (14 output) x 1 KB wide, one CTA per SM; ring depth D bounded by 227 KB of shared memory
-template <typename T> using K3 = OpK3<T, 16, 4>;    // 4 x 32.5 KB ring + 32 KB exchange = 162 KB
-template <typename T> using K4 = OpK4<T, 16, 3>;    // 3 x 48.5 KB ring + 32 KB exchange = 178 KB
-template <typename T> using K2 = OpK2<T, 16, 3>;
+// measured on B200 (profiles/r1_tile_variants.md): fp32 prefers 8-row CTAs, two per SM; fp64 16-row CTAs, one per SM
+#ifdef OMNI_TYR
+template <typename T> using K3 = OpK3<T, OMNI_TYR, OMNI_D3, OMNI_MINB>;
+template <typename T> using K4 = OpK4<T, OMNI_TYR, OMNI_D4, OMNI_MINB>;
+#else
+template <typename T> using K3 = OpK3<T, (sizeof(T) == 4 ? 8 : 16), 4, (sizeof(T) == 4 ? 2 : 1)>;
+template <typename T> using K4 = OpK4<T, (sizeof(T) == 4 ? 8 : 16), 3, (sizeof(T) == 4 ? 2 : 1)>;
+#endif
+template <typename T> using K2 = OpK2<T, 16, 3, 1>;
 
 inline unsigned blocks_for(long long n, int bs) { return (unsigned)((n + bs - 1) / bs); }
 

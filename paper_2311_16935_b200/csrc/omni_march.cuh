@@ -87,7 +87,7 @@ struct MarchSmem {
 };
 
 template <class Op>
-__global__ void __launch_bounds__(32 * Op::TYR, 1)
+__global__ void __launch_bounds__(32 * Op::TYR, Op::MINB)
 march_kernel(const Geom g, const int zlen, const typename Op::Args a)
 {
     using VT = typename Op::VT;
@@ -227,10 +227,10 @@ march_kernel(const Geom g, const int zlen, const typename Op::Args a)
 
 // ------------------------------------------------------------------------------------------------ K3
 // p_new = r + beta p_old on the fly (also in the halo), store p_new, gamma = p_new . M p_new; alpha = rho / gamma.
-template <typename T, int TYR_, int D_>
+template <typename T, int TYR_, int D_, int MINB_>
 struct OpK3 {
     using VT = T;
-    enum { V = 32 / sizeof(T), TYR = TYR_, D = D_, NACC = 1, TICKET = 0, PIECES = 4 };
+    enum { V = 32 / sizeof(T), TYR = TYR_, D = D_, MINB = MINB_, NACC = 1, TICKET = 0, PIECES = 4 };
     struct Args {
         const T* r; T* pbuf[2]; const uint32_t* wcode; const uint32_t* flags;
         Coef<T> K; Scalars* sc; double* partial; CondHandles cond;
@@ -296,10 +296,10 @@ struct OpK3 {
 
 // ------------------------------------------------------------------------------------------------ K4
 // q = M p recomputed from p (never stored), delta += alpha p, r -= alpha q, rho' = r.r; beta = rho'/rho; loop test.
-template <typename T, int TYR_, int D_>
+template <typename T, int TYR_, int D_, int MINB_>
 struct OpK4 {
     using VT = T;
-    enum { V = 32 / sizeof(T), TYR = TYR_, D = D_, NACC = 1, TICKET = 1, PIECES = 6 };
+    enum { V = 32 / sizeof(T), TYR = TYR_, D = D_, MINB = MINB_, NACC = 1, TICKET = 1, PIECES = 6 };
     struct Args {
         T* r; T* delta; const T* pbuf[2]; const uint32_t* wcode; const uint32_t* flags;
         Coef<T> K; Scalars* sc; double* partial; CondHandles cond;
@@ -387,10 +387,10 @@ struct OpK4 {
 // (L P)_C = sum_d v(C+d) t_a (P_C - P_{C+d}) = ([W^{n+1}] - [W^n]) P; eps_R^2 ||S||^2 = ||r0||^2 (Eq. 41).
 // P is always fp64 (master pressure, A9); delta, S, r are T.  P is double-buffered: neighbouring CTAs read
 // P + delta in their halos, so the folded field goes to the other buffer (read Pbuf[n&1], write Pbuf[(n&1)^1]).
-template <typename T, int TYR_, int D_>
+template <typename T, int TYR_, int D_, int MINB_>
 struct OpK2 {
     using VT = double;
-    enum { V = 4, TYR = TYR_, D = D_, NACC = 2, TICKET = 2, NPT = 4 * sizeof(T) / 16, PIECES = 2 + 2 * NPT };
+    enum { V = 4, TYR = TYR_, D = D_, MINB = MINB_, NACC = 2, TICKET = 2, NPT = 4 * sizeof(T) / 16, PIECES = 2 + 2 * NPT };
     struct Args {
         double* Pbuf[2]; const T* delta; const T* S; T* r; const uint8_t* link; const uint32_t* flags;
         double t[3]; Scalars* sc; double* partial; CondHandles cond;
