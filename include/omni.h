@@ -126,6 +126,9 @@ long long omni_launch_count(int reset);
 /* 0 = CUDA-graph loop with device-side conditional WHILE nodes (default), 1 = host-driven loop that synchronises
  * once per outer iteration (debug / drivers without conditional nodes).  Returns the previous mode. */
 int omni_set_loop_mode(int mode);
+/* Workspace of the non-_ws entry points comes from a library-owned stream-ordered memory pool (one per device) that
+ * keeps freed blocks mapped between calls; this returns the unused memory to the driver. */
+void omni_release_memory(void);
 /* Per-kernel timing of the host-driven loop (loop mode 1 only): when enabled, CUDA events bracket every launch of
  * K2 (outer boundary update), K3 (p update + operator + p.Mp) and K4 (operator recomputed + axpys + r.r) on `stream`;
  * launches that found the device loop flag cleared (no work) are left out.  omni_profile_read returns the summed

@@ -4,7 +4,7 @@ The product is the C-ABI library libomni.so (include/omni.h, csrc/); this packag
 Importing the package does not load the library; the first call does, and fails loudly when it is missing.
 """
 from .binding import (Info, OmniError, SYMBOLS, apply_M, constants, launch_count, lib, profile_enable,  # noqa: F401
-                      profile_read, residual, set_loop_mode, solve, source, status_string, version, workspace_bytes)
+                      profile_read, release_memory, residual, set_loop_mode, solve, source, status_string, version, workspace_bytes)
 
 # the C names, for callers who think in terms of include/omni.h
 omni_solve = solve
@@ -15,6 +15,7 @@ omni_constants = constants
 omni_workspace_bytes = workspace_bytes
 omni_launch_count = launch_count
 omni_set_loop_mode = set_loop_mode
+omni_release_memory = release_memory
 omni_profile_enable = profile_enable
 omni_profile_read = profile_read
 omni_status_string = status_string

@@ -19,7 +19,7 @@ STATUS_NAMES = {0: "OMNI_OK", 1: "OMNI_NOT_CONVERGED", -1: "OMNI_ERR_INVALID_ARG
 SYMBOLS = ["omni_solve_f64", "omni_solve_f32", "omni_workspace_bytes", "omni_solve_f64_ws", "omni_solve_f32_ws",
            "omni_solve_host_f64", "omni_solve_host_f32", "omni_constants", "omni_source_f64", "omni_source_f32",
            "omni_apply_M_f64", "omni_apply_M_f32", "omni_residual_f64", "omni_residual_f32", "omni_launch_count",
-           "omni_set_loop_mode", "omni_profile_enable", "omni_profile_read", "omni_status_string", "omni_version"]
+           "omni_set_loop_mode", "omni_release_memory", "omni_profile_enable", "omni_profile_read", "omni_status_string", "omni_version"]
 
 
 class OmniError(RuntimeError):
@@ -72,6 +72,10 @@ def launch_count(reset=False):
 def set_loop_mode(mode):
     """0 = CUDA-graph loop (default), 1 = host-driven debug loop.  Returns the previous mode."""
     return int(lib().omni_set_loop_mode(C.c_int(mode)))
+
+
+def release_memory():
+    lib().omni_release_memory()
 
 
 def profile_enable(on):

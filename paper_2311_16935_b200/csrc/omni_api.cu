@@ -35,6 +35,40 @@ struct ProfRec { int which; cudaEvent_t e0, e1; };
 
 inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
+// Workspace comes from a library-owned stream-ordered pool per device whose release threshold is unbounded: freed
+// blocks stay mapped between calls (re-mapping ~5 GB costs ~10 ms per call with the default pool, measured on B200).
+// omni_release_memory() trims it.
+std::mutex g_pool_mu;
+cudaMemPool_t g_pools[64] = {};
+
+cudaMemPool_t device_pool()
+{
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) return nullptr;
+    std::lock_guard<std::mutex> lk(g_pool_mu);
+    if (!g_pools[dev]) {
+        cudaMemPoolProps props = {};
+        props.allocType = cudaMemAllocationTypePinned;
+        props.handleTypes = cudaMemHandleTypeNone;
+        props.location.type = cudaMemLocationTypeDevice;
+        props.location.id = dev;
+        cudaMemPool_t pool = nullptr;
+        if (cudaMemPoolCreate(&pool, &props) != cudaSuccess) { cudaGetLastError(); return nullptr; }
+        unsigned long long thr = ~0ULL;
+        cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &thr);
+        g_pools[dev] = pool;
+    }
+    return g_pools[dev];
+}
+
+template <typename P>
+cudaError_t pool_alloc(P** ptr, size_t bytes, cudaStream_t st)
+{
+    cudaMemPool_t pool = device_pool();
+    if (!pool) return cudaMallocAsync((void**)ptr, bytes, st);
+    return cudaMallocFromPoolAsync((void**)ptr, bytes, pool, st);
+}
+
 // ------------------------------------------------------------------------------------------------ a0 constants
 
 // c_aa for general spacing: measure of the rays that cross two directly opposed, parallel db x dc rectangles a
@@ -530,7 +564,7 @@ int solve_alloc(int nx, int ny, int nz, double dx, double dy, double dz, const T
     cudaStream_t st = (cudaStream_t)stream;
     const size_t bytes = carve<T>(g, nullptr, nullptr);
     void* ws = nullptr;
-    if (cudaMallocAsync(&ws, bytes, st) != cudaSuccess) { cudaGetLastError(); return OMNI_ERR_ALLOC; }
+    if (pool_alloc(&ws, bytes, st) != cudaSuccess) { cudaGetLastError(); return OMNI_ERR_ALLOC; }
     int rc = solve_ws<T>(nx, ny, nz, dx, dy, dz, gx, gy, gz, mask, P_out, tol, max_outer, max_cg, ws, bytes, stream, info);
     cudaFreeAsync(ws, st);
     return rc;
@@ -548,8 +582,8 @@ int solve_host(int nx, int ny, int nz, double dx, double dy, double dz, const T*
     const int ncomp = (nz > 1) ? 3 : 2;
     T* dbuf = nullptr;
     uint8_t* dmask = nullptr;
-    if (cudaMallocAsync((void**)&dbuf, (ncomp + 1) * n * sizeof(T), st) != cudaSuccess) { cudaGetLastError(); return OMNI_ERR_ALLOC; }
-    if (mask && cudaMallocAsync((void**)&dmask, n, st) != cudaSuccess) { cudaGetLastError(); cudaFreeAsync(dbuf, st); return OMNI_ERR_ALLOC; }
+    if (pool_alloc((void**)&dbuf, (ncomp + 1) * n * sizeof(T), st) != cudaSuccess) { cudaGetLastError(); return OMNI_ERR_ALLOC; }
+    if (mask && pool_alloc((void**)&dmask, n, st) != cudaSuccess) { cudaGetLastError(); cudaFreeAsync(dbuf, st); return OMNI_ERR_ALLOC; }
     int rc = OMNI_ERR_CUDA;
     omni_info local;
     do {
@@ -586,7 +620,7 @@ int step_begin(StepCtx<T>& c, int nx, int ny, int nz, double dx, double dy, doub
     c.st = (cudaStream_t)stream;
     const size_t bytes = carve<T>(c.g, nullptr, nullptr);
     c.ws = nullptr;
-    if (cudaMallocAsync(&c.ws, bytes, c.st) != cudaSuccess) { cudaGetLastError(); return OMNI_ERR_ALLOC; }
+    if (pool_alloc(&c.ws, bytes, c.st) != cudaSuccess) { cudaGetLastError(); return OMNI_ERR_ALLOC; }
     carve<T>(c.g, (char*)c.ws, &c.w);
     host_constants(nz, dx, dy, dz, c.H);
     c.K = make_coef<T>(c.H, dx, dy, dz, c.g);
@@ -809,6 +843,13 @@ void omni_profile_read(double* h_ms3, long long* h_count3, int reset)
         if (h_count3) h_count3[i] = g_prof_n[i];
         if (reset) { g_prof_ms[i] = 0.0; g_prof_n[i] = 0; }
     }
+}
+
+void omni_release_memory(void)
+{
+    std::lock_guard<std::mutex> lk(g_pool_mu);
+    for (auto& p : g_pools)
+        if (p) cudaMemPoolTrimTo(p, 0);
 }
 
 int omni_set_loop_mode(int mode)
