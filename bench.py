@@ -91,6 +91,22 @@ class ClockSampler:
                 "samples": len(sm)}
 
 
+def max_over_ranks(values, world, device="cpu"):
+    """Per-rank timings -> the maximum over ranks (the job finishes with its slowest replica)."""
+    if world <= 1:
+        return [float(v) for v in values]
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor(values, dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return [float(v) for v in t]
+
+
+def aggregate_value(units_per_step_per_rank, steps, world, seconds_max):
+    """Whole-job throughput of N independent replicas (weak scaling): all ranks' units over the slowest rank's time."""
+    return world * units_per_step_per_rank * steps / seconds_max
+
+
 def cpu_sample(f, ndim):
     """Bounded sample of the workload for the oracle: the corner crop [0:e]^ndim of the same arrays."""
     import numpy as np
@@ -213,10 +229,7 @@ def main():
         e2e_s = time.perf_counter() - t0
     clocks = clk.summary()
 
-    if world > 1:
-        t = torch.tensor([ms, e2e_s], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms, e2e_s = float(t[0]), float(t[1])
+    ms, e2e_s = max_over_ranks([ms, e2e_s], world, dev)
 
     # per-kernel live timing of the same step (host-driven loop, CUDA events around each launch on the same stream)
     prev = omni.set_loop_mode(1)
@@ -248,11 +261,11 @@ def main():
 
     if rank != 0:
         return
-    out = {"metric": METRIC, "value": world * units_per_step * args.steps / (ms * 1e-3), "unit": UNIT,
+    out = {"metric": METRIC, "value": aggregate_value(units_per_step, args.steps, world, ms * 1e-3), "unit": UNIT,
            "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms / args.steps,
            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": dtype, "data": "synthetic",
            "config": config, "clocks": clocks, "gpu_launches": launches_per_step * args.steps,
-           "e2e": {"value": world * units_per_step * args.steps / e2e_s, "unit": UNIT,
+           "e2e": {"value": aggregate_value(units_per_step, args.steps, world, e2e_s), "unit": UNIT,
                    "h2d_bytes_per_step": sum(c.numel() * c.element_size() for c in g_host if c is not None)
                    + (0 if m_host is None else m_host.numel()), "d2h_bytes_per_step": N * esz,
                    "ms_per_step": e2e_s / args.steps * 1e3},

@@ -1,0 +1,99 @@
+"""BASELINE.json's full-size configs, in the launch configuration bench.py times, against the oracle:
+step outputs at sampled cells (the oracle evaluates S_C, (M x)_C, (W^n x)_C one cell at a time), the device
+reductions against fp64 sums of the full device arrays, and a short fixed-count trajectory against a full oracle
+solve where host memory allows it."""
+import numpy as np
+import pytest
+
+import paper_2311_16935_b200 as omni
+from workloads import CONFIGS, make_config
+
+from util import rel_l2_after_mean_removal
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+NSAMP = 20000
+CASES = [(1, "f32"), (1, "f64"), (2, "f64"), (3, "f32"), (3, "f64"), (4, "f32")]
+TOL_STEP = {"f64": 1e-12, "f32": 4e-6}
+TOL_SOLVE = {"f64": 1e-9, "f32": 2e-4}
+
+
+def _host_mem_gb():
+    try:
+        import psutil
+        return psutil.virtual_memory().available / 2**30
+    except Exception:
+        return 0.0
+
+
+@pytest.mark.parametrize("idx,dtype", CASES)
+def test_fullsize_config(oracle, idx, dtype):
+    f = make_config(idx, device="cuda")
+    d = f["d"]
+    tdt = torch.float32 if dtype == "f32" else torch.float64
+    g_dev = [torch.from_numpy(c).to(tdt).cuda() for c in f["g"]]
+    g_or = [c.cpu().numpy().astype(np.float64) for c in g_dev]           # the values the device consumed
+    g_dev += [None] * (3 - len(g_dev))
+    g_or += [None] * (3 - len(g_or))
+    mask = f["mask"]
+    m_dev = None if mask is None else torch.from_numpy(mask).cuda()
+    shape = f["g"][0].shape
+    N = int(np.prod(shape))
+    v = oracle.validity(g_or[0], g_or[1], g_or[2], mask)
+    rng = np.random.default_rng(100 + idx)
+    # sampled cells: uniform + every kind of boundary (box faces, edges, corners, mask surface)
+    cells = rng.choice(N, NSAMP, replace=False)
+    edge = np.array([0, 1, shape[-1] - 2, shape[-1] - 1, shape[-1], N - 1, N - 2, N - shape[-1], N // 2])
+    cells = np.unique(np.concatenate([cells, edge]))
+    if mask is not None:
+        from scipy import ndimage
+        surf = np.flatnonzero((ndimage.binary_dilation(mask == 0) & (mask == 1)).ravel())
+        cells = np.unique(np.concatenate([cells, rng.choice(surf, min(len(surf), 4000), replace=False)]))
+
+    # a2: source term
+    S, nS = omni.source(g_dev[0], g_dev[1], g_dev[2], m_dev, d)
+    x = rng.standard_normal(shape)
+    x_dev = torch.from_numpy(x).to(tdt).cuda()
+    x_or = x_dev.cpu().numpy().astype(np.float64) * v
+    S_or, Mx_or, Wx_or = oracle.sample(v, g_or[0], g_or[1], g_or[2], x_or, cells, *d)
+    S_s = S.flatten()[torch.from_numpy(cells).cuda()].cpu().numpy().astype(np.float64)
+    assert np.abs(S_s - S_or).max() <= TOL_STEP[dtype] * np.abs(S_or).max() * 4
+    assert nS == pytest.approx(float(torch.linalg.vector_norm(S.double())), rel=1e-12)
+    # a4: operator through the CG kernel
+    q, pq = omni.apply_M(x_dev, m_dev, d)
+    q_s = q.flatten()[torch.from_numpy(cells).cuda()].cpu().numpy().astype(np.float64)
+    assert np.abs(q_s - Mx_or).max() <= TOL_STEP[dtype] * np.abs(Mx_or).max() * 8
+    xv = x_dev.double() * torch.from_numpy(v).cuda()
+    assert pq == pytest.approx(float((xv * q.double()).sum()), rel=1e-10)
+    del q, xv
+
+    # the whole path in bench.py's launch configuration (fixed caps, graph loop)
+    tol = 1e-5 if dtype == "f32" else 1e-8
+    P, info = omni.solve(g_dev[0], g_dev[1], g_dev[2], m_dev, d, tol, 8, 25)
+    assert info["status"] in (0, 1) and info["cg_iters_total"] > 0
+    assert info["norm_S"] == pytest.approx(nS, rel=1e-12)
+    Pn = torch.nan_to_num(P.double(), nan=0.0)
+    assert bool((torch.isnan(P) == (torch.from_numpy(v).cuda() == 0)).all())
+    # a3 on the returned field: r at sampled cells against the oracle, eps_R against the full device arrays
+    r, eps = omni.residual(g_dev[0], g_dev[1], g_dev[2], m_dev, Pn, d)
+    _, MP, WP = oracle.sample(v, None, None, None, Pn.cpu().numpy(), cells, *d)
+    r_or = S_or + WP - MP
+    r_s = r.flatten()[torch.from_numpy(cells).cuda()].cpu().numpy().astype(np.float64)
+    scale = max(np.abs(r_or).max(), np.abs(MP).max() * 1e-3)
+    assert np.abs(r_s - r_or).max() <= TOL_STEP[dtype] * 16 * max(np.abs(MP).max(), np.abs(S_or).max())
+    assert eps == pytest.approx(float(torch.linalg.vector_norm(r.double())) / nS, rel=1e-6 if dtype == "f32" else 1e-10)
+    # the solve's own eps_R (fp64 master pressure) agrees with the residual of the (rounded) returned field
+    assert info["eps_R_final"] == pytest.approx(eps, rel=5e-2 if dtype == "f32" else 1e-6)
+    assert scale > 0
+    del r, Pn, S, x_dev
+
+    # short fixed-count trajectory against a full oracle solve (needs ~18 fp64 fields on the host)
+    if N * 8 * 20 / 2**30 < 0.6 * _host_mem_gb():
+        mo, mc = (2, 5) if N > 5e7 else (3, 8)
+        Pg, ig = omni.solve(g_dev[0], g_dev[1], g_dev[2], m_dev, d, 0.0, mo, mc)
+        Po, io = oracle.solve(g_or[0], g_or[1], g_or[2], mask, *d, tol=0.0, max_outer=mo, max_cg=mc)
+        assert ig["cg_iters_total"] == io["cg_iters_total"] == mo * mc
+        err = rel_l2_after_mean_removal(Pg.cpu().numpy(), Po, v == 1)
+        assert err <= TOL_SOLVE[dtype], err
+        assert ig["eps_R_final"] == pytest.approx(io["eps_R_final"], rel=1e-3 if dtype == "f32" else 1e-8)
