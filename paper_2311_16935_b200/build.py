@@ -4,7 +4,8 @@ import subprocess
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 SRC = [os.path.join(HERE, "csrc", "omni_api.cu")]
-DEPS = SRC + [os.path.join(HERE, "csrc", "omni_kernels.cuh"), os.path.join(os.path.dirname(HERE), "include", "omni.h")]
+DEPS = [os.path.join(HERE, "csrc", f) for f in sorted(os.listdir(os.path.join(HERE, "csrc")))] + \
+       [os.path.join(os.path.dirname(HERE), "include", "omni.h")]
 LIB = os.path.join(HERE, "libomni.so")
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-Xcompiler", "-fPIC", "-shared", "-cudart", "static"]

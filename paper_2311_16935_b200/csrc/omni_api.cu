@@ -1,7 +1,7 @@
 // omni_api.cu -- C ABI (include/omni.h) over the kernels of omni_kernels.cuh.
 // Host logic only: argument validation, geometry constants (a0), workspace carving, launch configuration and the
 // loop driver (CUDA graph with device-side conditional WHILE nodes, or a host-driven debug loop).
-#include "omni_march.cuh"
+#include "omni_tma.cuh"
 #include "../../include/omni.h"
 
 #include <algorithm>
@@ -289,16 +289,95 @@ cudaError_t launch_march(const Geom& g, const typename Op::Args& a, cudaStream_t
     return cudaGetLastError();
 }
 
-// tile shapes: 16 rows (14 output) x 1 KB wide, one CTA per SM; ring depth D bounded by 227 KB of shared memory
-// measured on B200 (profiles/r1_tile_variants.md): fp32 prefers 8-row CTAs, two per SM; fp64 16-row CTAs, one per SM
-#ifdef OMNI_TYR
-template <typename T> using K3 = OpK3<T, OMNI_TYR, OMNI_D3, OMNI_MINB>;
-template <typename T> using K4 = OpK4<T, OMNI_TYR, OMNI_D4, OMNI_MINB>;
-#else
-template <typename T> using K3 = OpK3<T, (sizeof(T) == 4 ? 8 : 16), 4, (sizeof(T) == 4 ? 2 : 1)>;
-template <typename T> using K4 = OpK4<T, (sizeof(T) == 4 ? 8 : 16), 3, (sizeof(T) == 4 ? 2 : 1)>;
+// K3 / K4: TMA + mbarrier pipeline (omni_tma.cuh): 512-byte x 8-row tiles, 8 consumer warps + 1 producer warp,
+// several CTAs per SM (shared memory: K3 6 stages x 10.8 KB, K4 5 stages x 13.4 KB).  K2: cp.async engine.
+#ifndef OMNI_BY
+#define OMNI_BY 8
+#define OMNI_D3 6
+#define OMNI_D4 5
+#define OMNI_MINB 3
 #endif
+template <typename T> using K3 = OpT3<T, OMNI_BY, OMNI_D3, OMNI_MINB>;
+template <typename T> using K4 = OpT4<T, OMNI_BY, OMNI_D4, OMNI_MINB>;
 template <typename T> using K2 = OpK2<T, 16, 3, 1>;
+
+
+template <class Op>
+MarchCfg tma_config(const Geom& g)
+{
+    using TG = typename Op::TG;
+    constexpr int SMEM = Op::D * Op::STAGE_BYTES + 128;
+    static int slots_cache = 0;
+    if (slots_cache == 0) {
+        int dev = 0, sms = 148, occ = 1;
+        cudaGetDevice(&dev);
+        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+        cudaFuncSetAttribute(tma_kernel<Op>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM);
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, tma_kernel<Op>, TG::NTHR, SMEM);
+        if (occ < 1) occ = 1;
+        slots_cache = sms * occ;
+    }
+    const int slots = slots_cache;
+    const int ntx = (g.px + TG::BX - 1) / TG::BX, nty = (g.ny + TG::BY - 1) / TG::BY;
+    const long long tiles = (long long)ntx * nty;
+    int best = 1;
+    double best_cost = 1e300;
+    for (int ns = 1; ns <= g.nz; ns = (ns < 16 ? ns + 1 : ns + ns / 8)) {
+        const int zlen = (g.nz + ns - 1) / ns;
+        const int nseg = (g.nz + zlen - 1) / zlen;
+        const long long ctas = tiles * nseg;
+        const long long waves = (ctas + slots - 1) / slots;
+        const double cost = (double)waves * (zlen + (nseg > 1 ? 2 : 0) + 3);
+        if (cost < best_cost) { best_cost = cost; best = nseg; }
+        if (zlen <= 4) break;
+    }
+    MarchCfg c;
+    c.zlen = (g.nz + best - 1) / best;
+    const int nseg = (g.nz + c.zlen - 1) / c.zlen;
+    c.grid = dim3(ntx, nty, nseg);
+    c.block = dim3(TG::NTHR, 1, 1);
+    return c;
+}
+
+template <class Op>
+cudaError_t launch_tma(const Geom& g, const typename Op::Args& a, const TmaSet& maps, cudaStream_t st)
+{
+    const MarchCfg c = tma_config<Op>(g);
+    tma_kernel<Op><<<c.grid, c.block, Op::D * Op::STAGE_BYTES + 128, st>>>(g, c.zlen, a, maps);
+    g_launches.fetch_add(1, std::memory_order_relaxed);
+    return cudaGetLastError();
+}
+
+// host-side tensor maps (driver entry point fetched through the runtime: no link-time dependency on libcuda)
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+EncodeTiledFn encode_fn()
+{
+    static EncodeTiledFn fn = nullptr;
+    if (!fn) {
+        void* p = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess &&
+            q == cudaDriverEntryPointSuccess)
+            fn = (EncodeTiledFn)p;
+    }
+    return fn;
+}
+
+template <typename T>
+bool encode_map(CUtensorMap* m, const Geom& g, const T* base, int bx, int by)
+{
+    EncodeTiledFn fn = encode_fn();
+    if (!fn) return false;
+    const cuuint64_t dims[3] = { (cuuint64_t)g.px, (cuuint64_t)g.ny, (cuuint64_t)g.nz };
+    const cuuint64_t strides[2] = { (cuuint64_t)g.px * sizeof(T), (cuuint64_t)g.pplane * sizeof(T) };
+    const cuuint32_t box[3] = { (cuuint32_t)bx, (cuuint32_t)by, 1u };
+    const cuuint32_t estr[3] = { 1u, 1u, 1u };
+    const CUtensorMapDataType dt = (sizeof(T) == 4) ? CU_TENSOR_MAP_DATA_TYPE_FLOAT32 : CU_TENSOR_MAP_DATA_TYPE_FLOAT64;
+    return fn(m, dt, 3, (void*)base, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+              CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
 
 inline unsigned blocks_for(long long n, int bs) { return (unsigned)((n + bs - 1) / bs); }
 
@@ -346,7 +425,7 @@ template <typename T>
 typename K3<T>::Args k3_args(const Workspace<T>& w, const Coef<T>& K, CondHandles ch)
 {
     typename K3<T>::Args a;
-    a.r = w.r; a.pbuf[0] = w.p0; a.pbuf[1] = w.p1; a.wcode = w.wcode; a.flags = w.flags;
+    a.pbuf[0] = w.p0; a.pbuf[1] = w.p1; a.wcode = w.wcode; a.flags = w.flags;
     a.K = K; a.sc = w.sc; a.partial = w.partial; a.cond = ch;
     return a;
 }
@@ -354,9 +433,18 @@ template <typename T>
 typename K4<T>::Args k4_args(const Workspace<T>& w, const Coef<T>& K, CondHandles ch)
 {
     typename K4<T>::Args a;
-    a.r = w.r; a.delta = w.delta; a.pbuf[0] = w.p0; a.pbuf[1] = w.p1; a.wcode = w.wcode; a.flags = w.flags;
+    a.r = w.r; a.delta = w.delta; a.p_fixed = -1; a.wcode = w.wcode; a.flags = w.flags;
     a.K = K; a.sc = w.sc; a.partial = w.partial; a.cond = ch; a.q_out = nullptr;
     return a;
+}
+template <typename T>
+bool make_tma_set(const Geom& g, const Workspace<T>& w, TmaSet& m)
+{
+    using TG = typename K3<T>::TG;
+    const int hx = TG::BX + 2 * TG::HX, hy = TG::BY + 2;
+    return encode_map<T>(&m.r_h, g, w.r, hx, hy) && encode_map<T>(&m.p_h[0], g, w.p0, hx, hy) &&
+           encode_map<T>(&m.p_h[1], g, w.p1, hx, hy) && encode_map<T>(&m.r_c, g, w.r, TG::BX, TG::BY) &&
+           encode_map<T>(&m.d_c, g, w.delta, TG::BX, TG::BY);
 }
 
 // ------------------------------------------------------------------------------------------------ loop drivers
@@ -370,6 +458,8 @@ int run_loop_host(const Geom& g, const Workspace<T>& w, const HostConst& H, cons
     const auto a2 = k2_args<T>(w, H, ch, 1);
     const auto a3 = k3_args<T>(w, K, ch);
     const auto a4 = k4_args<T>(w, K, ch);
+    TmaSet maps;
+    if (!make_tma_set<T>(g, w, maps)) return OMNI_ERR_CUDA;
     const bool prof = g_profile.load() != 0;
     std::vector<ProfRec> recs;
     auto timed = [&](int which, auto&& launch) -> cudaError_t {
@@ -397,8 +487,8 @@ int run_loop_host(const Geom& g, const Workspace<T>& w, const HostConst& H, cons
         while (done < max_cg) {
             const int batch = (max_cg - done < 16) ? (max_cg - done) : 16;
             for (int c = 0; c < batch; ++c) {
-                if (timed(1, [&] { return launch_march<K3<T>>(g, a3, st); }) != cudaSuccess) rc = OMNI_ERR_CUDA;
-                if (timed(2, [&] { return launch_march<K4<T>>(g, a4, st); }) != cudaSuccess) rc = OMNI_ERR_CUDA;
+                if (timed(1, [&] { return launch_tma<K3<T>>(g, a3, maps, st); }) != cudaSuccess) rc = OMNI_ERR_CUDA;
+                if (timed(2, [&] { return launch_tma<K4<T>>(g, a4, maps, st); }) != cudaSuccess) rc = OMNI_ERR_CUDA;
             }
             done += batch;
             if (rc != OMNI_OK) break;
@@ -444,7 +534,9 @@ int run_loop_graph(const Geom& g, const Workspace<T>& w, const HostConst& H, con
     cudaStream_t cap = nullptr;
     int rc = OMNI_ERR_CUDA;
     // occupancy queries happen here, outside any stream capture (results are cached per kernel)
-    (void)march_config<K2<T>>(g); (void)march_config<K3<T>>(g); (void)march_config<K4<T>>(g);
+    (void)march_config<K2<T>>(g); (void)tma_config<K3<T>>(g); (void)tma_config<K4<T>>(g);
+    TmaSet maps;
+    if (!make_tma_set<T>(g, w, maps)) return OMNI_ERR_CUDA;
     do {
         if (cudaGraphCreate(&G, 0) != cudaSuccess) break;
         cudaGraphConditionalHandle hOuter, hInner;
@@ -481,8 +573,8 @@ int run_loop_graph(const Geom& g, const Workspace<T>& w, const HostConst& H, con
         cudaGraph_t bodyInner = pi.conditional.phGraph_out[0];
 
         if (cudaStreamBeginCaptureToGraph(cap, bodyInner, nullptr, nullptr, 0, cudaStreamCaptureModeThreadLocal) != cudaSuccess) break;
-        cudaError_t e3 = launch_march<K3<T>>(g, k3_args<T>(w, K, ch), cap);
-        cudaError_t e4 = launch_march<K4<T>>(g, k4_args<T>(w, K, ch), cap);
+        cudaError_t e3 = launch_tma<K3<T>>(g, k3_args<T>(w, K, ch), maps, cap);
+        cudaError_t e4 = launch_tma<K4<T>>(g, k4_args<T>(w, K, ch), maps, cap);
         if (cudaStreamEndCapture(cap, &tmp) != cudaSuccess || e3 != cudaSuccess || e4 != cudaSuccess) break;
         g_launches.fetch_sub(3, std::memory_order_relaxed);     // captured, not launched; counted from the device state
 
@@ -682,9 +774,10 @@ int apply_M_step(int nx, int ny, int nz, double dx, double dy, double dz, const 
         force_go_kernel<<<1, 1, 0, c.st>>>(c.w.sc, 0.0);
         CondHandles ch{ 0, 0, 0 };
         auto a4 = k4_args<T>(c.w, c.K, ch);
-        a4.pbuf[0] = c.w.p0; a4.pbuf[1] = c.w.p0;
+        a4.p_fixed = 0;
         a4.q_out = c.w.r;
-        cudaError_t e = launch_march<K4<T>>(c.g, a4, c.st);
+        TmaSet maps;
+        cudaError_t e = make_tma_set<T>(c.g, c.w, maps) ? launch_tma<K4<T>>(c.g, a4, maps, c.st) : cudaErrorUnknown;
         pad_copy_kernel<T, T><<<nb, 256, 0, c.st>>>(c.g, c.w.r, q, 0, c.w.link);
         g_launches.fetch_add(3, std::memory_order_relaxed);
         if (e != cudaSuccess || cudaGetLastError() != cudaSuccess) rc = OMNI_ERR_CUDA;

@@ -95,22 +95,35 @@ constexpr uint8_t LINK_VALID = 1u << 6;
 template <typename T, int V>
 __device__ __forceinline__ void ld_chunk(const T* __restrict__ p, T (&v)[V])
 {
-    constexpr int NV = V * (int)sizeof(T) / 16;
-    static_assert(NV * 16 == V * (int)sizeof(T), "chunk must be a multiple of 16 bytes");
-    uint4 u[NV];
+    constexpr int BYTES = V * (int)sizeof(T);
+    static_assert(BYTES == 8 || BYTES % 16 == 0, "chunk must be 8 bytes or a multiple of 16");
+    if constexpr (BYTES == 8) {
+        uint2 u = *reinterpret_cast<const uint2*>(p);
+        memcpy(v, &u, 8);
+    } else {
+        constexpr int NV = BYTES / 16;
+        uint4 u[NV];
 #pragma unroll
-    for (int i = 0; i < NV; ++i) u[i] = reinterpret_cast<const uint4*>(p)[i];
-    memcpy(v, u, sizeof(u));
+        for (int i = 0; i < NV; ++i) u[i] = reinterpret_cast<const uint4*>(p)[i];
+        memcpy(v, u, sizeof(u));
+    }
 }
 
 template <typename T, int V>
 __device__ __forceinline__ void st_chunk(T* __restrict__ p, const T (&v)[V])
 {
-    constexpr int NV = V * (int)sizeof(T) / 16;
-    uint4 u[NV];
-    memcpy(u, v, sizeof(u));
+    constexpr int BYTES = V * (int)sizeof(T);
+    if constexpr (BYTES == 8) {
+        uint2 u;
+        memcpy(&u, v, 8);
+        *reinterpret_cast<uint2*>(p) = u;
+    } else {
+        constexpr int NV = BYTES / 16;
+        uint4 u[NV];
+        memcpy(u, v, sizeof(u));
 #pragma unroll
-    for (int i = 0; i < NV; ++i) reinterpret_cast<uint4*>(p)[i] = u[i];
+        for (int i = 0; i < NV; ++i) reinterpret_cast<uint4*>(p)[i] = u[i];
+    }
 }
 
 template <typename T, int V>
@@ -232,7 +245,7 @@ template <int V>
 __device__ __forceinline__ uint32_t flag_bits(const uint32_t* __restrict__ flags, long long idx)
 {
     long long g = idx >> 2;
-    return (flags[g >> 5] >> (unsigned)(g & 31)) & ((1u << (V / 4)) - 1u);
+    return (flags[g >> 5] >> (unsigned)(g & 31)) & ((1u << (V >= 4 ? V / 4 : 1)) - 1u);
 }
 
 // ------------------------------------------------------------------------------------------------ K0a validity

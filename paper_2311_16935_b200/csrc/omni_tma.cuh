@@ -1,0 +1,350 @@
+// omni_tma.cuh -- K3 / K4 on a TMA + mbarrier producer/consumer pipeline (sm_100a).
+//
+// A CTA owns a column of the grid: BX = 32*V cells (512 bytes) x BY rows x zlen planes.  One producer warp issues,
+// per plane, a few cp.async.bulk.tensor (TMA) box loads -- the tile of every streamed array, the stencil input with
+// its one-cell halo in x and y -- into a D-deep ring of shared-memory stages; out-of-box coordinates (box faces, the
+// planes before/after the grid) are zero-filled by the TMA unit, so the kernels carry no bounds logic.  BY consumer
+// warps (one row each, V cells per lane) wait on the stage's "full" mbarrier, read the centre / N / S chunks of plane
+// c-1 and the own chunk of planes c-2 and c from the three resident stages (x neighbours by shuffle), evaluate the
+// operator, store, and release the oldest stage through its "empty" mbarrier.  Warps only ever wait for data, never
+// for each other: there is no CTA-wide barrier in the loop and no state carried in registers across planes.
+// The grid reduction at the end is the deterministic fixed-slot + last-CTA scheme of omni_march.cuh.
+#pragma once
+#include <cuda.h>
+#include "omni_march.cuh"
+
+namespace omni {
+
+// ------------------------------------------------------------------------------------------------ PTX wrappers
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
+{
+    uint32_t done;
+    do {
+        asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.b32 %0, 1, 0, p;\n\t}"
+                     : "=r"(done) : "r"(bar), "r"(parity) : "memory");
+    } while (!done);
+}
+__device__ __forceinline__ void tma_load_3d(uint32_t dst, const CUtensorMap* map, uint32_t bar, int c0, int c1, int c2)
+{
+    asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5}], [%2];"
+                 ::"r"(dst), "l"((unsigned long long)map), "r"(bar), "r"(c0), "r"(c1), "r"(c2) : "memory");
+}
+
+// tensor maps of one solve (host-encoded, passed as a __grid_constant__ kernel parameter)
+struct alignas(64) TmaSet {
+    CUtensorMap r_h, p_h[2];     // boxes with halo: (BX + 2 HX) x (BY + 2) x 1
+    CUtensorMap r_c, d_c;        // plain boxes: BX x BY x 1
+};
+
+template <typename T, int BY_>
+struct TileGeom {
+    static constexpr int V = 16 / (int)sizeof(T);          // cells per lane (one 16-byte piece)
+    static constexpr int BX = 32 * V;                      // 512 bytes per row
+    static constexpr int BY = BY_;
+    static constexpr int HX = 16 / (int)sizeof(T);         // x halo in cells (16 bytes: TMA box rows are 16 B multiples)
+    static constexpr int PITCH_H = (BX + 2 * HX) * (int)sizeof(T);       // 544 bytes
+    static constexpr int TILE_H = ((BY + 2) * PITCH_H + 127) / 128 * 128;
+    static constexpr int TILE_C = BY * BX * (int)sizeof(T);              // multiple of 512
+    static constexpr int NTHR = 32 * (BY + 1);             // BY consumer warps + 1 producer warp
+};
+
+// chunk accessors into a haloed / plain tile for (row w, lane l)
+template <typename T, int V>
+__device__ __forceinline__ void lds_chunk(const char* p, T (&v)[V])
+{
+    static_assert(V * sizeof(T) == 16, "one 16-byte piece per lane");
+    uint4 u = *reinterpret_cast<const uint4*>(p);
+    memcpy(v, &u, 16);
+}
+
+template <class Op>
+__global__ void __launch_bounds__(Op::TG::NTHR, Op::MINB)
+tma_kernel(const Geom g, const int zlen, const typename Op::Args a, const __grid_constant__ TmaSet maps)
+{
+    using TG = typename Op::TG;
+    using T = typename Op::VT;
+    constexpr int V = TG::V, BX = TG::BX, BY = TG::BY, D = Op::D, NACC = 1;
+    extern __shared__ __align__(128) char smem_raw[];
+    __shared__ double red[BY + 1];
+    __shared__ int is_last;
+    __shared__ __align__(8) unsigned long long bars[2 * D];
+
+    if (!Op::active(a)) {
+        if (threadIdx.x == 0 && blockIdx.x == 0 && blockIdx.y == 0 && blockIdx.z == 0) Op::idle(a);
+        return;
+    }
+    // dynamic shared memory is only guaranteed 16-byte aligned: round up to 128 for the TMA destinations
+    char* smem = reinterpret_cast<char*>((reinterpret_cast<uintptr_t>(smem_raw) + 127) & ~uintptr_t(127));
+    const uint32_t smem_s = (uint32_t)__cvta_generic_to_shared(smem);
+    const uint32_t bar_s = (uint32_t)__cvta_generic_to_shared(bars);
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int x0 = blockIdx.x * BX, y0 = blockIdx.y * BY;
+    const int k0 = blockIdx.z * zlen, k1 = min(g.nz, k0 + zlen);
+    const int E = k1 - k0 + 2;                       // events: planes k0-1 .. k1
+    const typename Op::Ctx ctx(a);
+
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < D; ++s) { mbar_init(bar_s + 8 * s, 1); mbar_init(bar_s + 8 * (D + s), BY); }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    }
+    __syncthreads();
+
+    double acc = 0.0;
+    if (warp == BY) {
+        // ---------------------------------------------------------------- producer warp (one elected lane)
+        if (lane == 0) {
+            for (int e = 0; e < E; ++e) {
+                const int s = e % D;
+                if (e >= D) mbar_wait(bar_s + 8 * (D + s), (uint32_t)((e / D - 1) & 1));
+                const int c = k0 - 1 + e;
+                Op::produce(a, ctx, maps, smem_s + (uint32_t)(s * Op::STAGE_BYTES), bar_s + 8 * s, x0, y0, c,
+                            (c >= k0) && (c < k1));
+            }
+        }
+    } else {
+        // ---------------------------------------------------------------- consumer warps: row = y0 + warp
+        const int x = x0 + lane * V, j = y0 + warp;
+        const bool out = (x < g.nx) && (j < g.ny);      // chunks made only of pad cells (x >= nx) stay zero
+        const typename Op::TC tc = Op::thread_init(g, x);
+        const long long rowbase = (long long)j * g.px + x;
+        uint32_t fw_next = 0, fw_cur = 0;
+        for (int e = 0; e < E; ++e) {
+            const int s = e % D;
+            mbar_wait(bar_s + 8 * s, (uint32_t)((e / D) & 1));
+            const int c = k0 - 1 + e;
+            fw_cur = fw_next;
+            if (out && c >= k0 && c < k1) fw_next = a.flags[((rowbase + (long long)c * g.pplane) >> 2) >> 5];
+            if (e >= 2) {                            // emit plane c-1 from stages e-2 (B), e-1 (centre), e (F)
+                const long long idx = rowbase + (long long)(c - 1) * g.pplane;
+                const char* sB = smem + ((e - 2) % D) * Op::STAGE_BYTES;
+                const char* sC = smem + ((e - 1) % D) * Op::STAGE_BYTES;
+                const char* sF = smem + s * Op::STAGE_BYTES;
+                const uint32_t fb = (fw_cur >> (unsigned)((idx >> 2) & 31)) & 1u;
+                Op::emit(a, ctx, g, idx, sB, sC, sF, warp, lane, out, fb, tc, acc);
+                __syncwarp();
+                if (lane == 0) mbar_arrive(bar_s + 8 * (D + (e - 2) % D));
+            }
+        }
+    }
+
+    // deterministic grid reduction (all warps, the producer contributes 0)
+    const unsigned int nblk = gridDim.x * gridDim.y * gridDim.z;
+    const unsigned int bid = blockIdx.x + gridDim.x * (blockIdx.y + gridDim.y * blockIdx.z);
+    {
+        double sacc = warp_sum(acc);
+        if (lane == 0) red[warp] = sacc;
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double s = 0.0;
+        for (int w = 0; w < BY; ++w) s += red[w];
+        a.partial[bid] = s;
+        __threadfence();
+        unsigned int t = atomicAdd(&a.sc->ticket[Op::TICKET], 1u);
+        is_last = (t == nblk - 1);
+    }
+    __syncthreads();
+    if (is_last) {
+        __threadfence();
+        double s = 0.0;
+        for (unsigned int b = threadIdx.x; b < nblk; b += TG::NTHR) s += __ldcg(&a.partial[b]);
+        s = warp_sum(s);
+        __syncthreads();
+        if (lane == 0) red[warp] = s;
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            double tot[NACC] = { 0.0 };
+            for (int w = 0; w <= BY; ++w) tot[0] += red[w];
+            a.sc->ticket[Op::TICKET] = 0;
+            Op::finalize(a, tot);
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------------ K3 (TMA)
+// p_new = r + beta p_old evaluated from the raw r / p_old tiles wherever the stencil needs it (centre, N, S, F, B
+// chunks and the two x-halo cells); store p_new; gamma = p_new . M p_new; last CTA: alpha = rho / gamma.
+template <typename T, int BY_, int D_, int MINB_>
+struct OpT3 {
+    using VT = T;
+    using TG = TileGeom<T, BY_>;
+    enum { V = TG::V, D = D_, MINB = MINB_, TICKET = 0, STAGE_BYTES = 2 * TG::TILE_H,
+           BOX_H = (BY_ + 2) * TG::PITCH_H };
+    struct Args {
+        T* pbuf[2]; const uint32_t* wcode; const uint32_t* flags;
+        Coef<T> K; Scalars* sc; double* partial; CondHandles cond;
+    };
+    struct Ctx {
+        T beta; int par; T* pnew;
+        __device__ Ctx(const Args& a) { beta = (T)a.sc->beta; par = a.sc->k & 1; pnew = a.pbuf[par ^ 1]; }
+    };
+    using TC = XEdge;
+    __device__ static TC thread_init(const Geom& g, int x) { return make_xedge<V>(g, x); }
+    __device__ static bool active(const Args& a) { return a.sc->inner_go != 0; }
+    __device__ static void idle(const Args& a) { set_cond(a.cond, -1, 0); }
+    __device__ static void produce(const Args&, const Ctx& c, const TmaSet& m, uint32_t stage, uint32_t bar, int x0, int y0,
+                                   int plane, bool)
+    {
+        mbar_expect_tx(bar, 2 * BOX_H);
+        tma_load_3d(stage, &m.r_h, bar, x0 - TG::HX, y0 - 1, plane);
+        tma_load_3d(stage + TG::TILE_H, &m.p_h[c.par], bar, x0 - TG::HX, y0 - 1, plane);
+    }
+    __device__ static void pnew_chunk(const char* st, int off, T beta, T (&v)[V])
+    {
+        T r[V], p[V];
+        lds_chunk<T, V>(st + off, r);
+        lds_chunk<T, V>(st + TG::TILE_H + off, p);
+#pragma unroll
+        for (int i = 0; i < V; ++i) v[i] = r[i] + beta * p[i];
+    }
+    __device__ static void emit(const Args& a, const Ctx& c, const Geom&, long long idx, const char* sB, const char* sC,
+                                const char* sF, int warp, int lane, bool out, uint32_t fb, const TC& xe, double& acc)
+    {
+        const int row = (warp + 1) * TG::PITCH_H;
+        const int off = row + (TG::HX + lane * V) * (int)sizeof(T);
+        T vm[V], vc[V], vp[V], vn[V], vs[V];
+        pnew_chunk(sC, off, c.beta, vc);
+        pnew_chunk(sC, off + TG::PITCH_H, c.beta, vn);
+        pnew_chunk(sC, off - TG::PITCH_H, c.beta, vs);
+        pnew_chunk(sF, off, c.beta, vp);
+        pnew_chunk(sB, off, c.beta, vm);
+        // x neighbours: shuffles inside the warp, the row's two halo cells (same address for all lanes) at its ends
+        const int hl_off = row + (TG::HX - 1) * (int)sizeof(T), hr_off = row + (TG::HX + TG::BX) * (int)sizeof(T);
+        const T hl = *reinterpret_cast<const T*>(sC + hl_off) + c.beta * *reinterpret_cast<const T*>(sC + TG::TILE_H + hl_off);
+        const T hr = *reinterpret_cast<const T*>(sC + hr_off) + c.beta * *reinterpret_cast<const T*>(sC + TG::TILE_H + hr_off);
+        T xl = __shfl_up_sync(0xffffffffu, vc[V - 1], 1);
+        T xr = __shfl_down_sync(0xffffffffu, vc[0], 1);
+        if (lane == 0) xl = hl;
+        if (lane == 31) xr = hr;
+        if (!out) return;
+        st_chunk<T, V>(c.pnew + idx, vc);
+        T q[V];
+        apply_M_chunk<T, V>(q, vm, vc, vp, vn, vs, xl, xr, fb, a.wcode, idx, a.K, xe);
+#pragma unroll
+        for (int i = 0; i < V; ++i) acc += (double)vc[i] * (double)q[i];
+    }
+    __device__ static void finalize(const Args& a, const double (&tot)[1])
+    {
+        Scalars* s = a.sc;
+        const double gamma = tot[0];
+        s->gamma = gamma;
+        if (!(gamma > 0.0) || !isfinite(gamma)) {
+            s->status = ST_BREAKDOWN; s->inner_go = 0; s->outer_go = 0;
+            set_cond(a.cond, 0, 0);
+        } else {
+            s->alpha = s->rho / gamma;
+        }
+    }
+};
+
+// ------------------------------------------------------------------------------------------------ K4 (TMA)
+// q = M p recomputed from the haloed p tile; delta += alpha p; r -= alpha q; rho' = r.r; beta, loop test.
+template <typename T, int BY_, int D_, int MINB_>
+struct OpT4 {
+    using VT = T;
+    using TG = TileGeom<T, BY_>;
+    enum { V = TG::V, D = D_, MINB = MINB_, TICKET = 1, STAGE_BYTES = TG::TILE_H + 2 * TG::TILE_C,
+           BOX_H = (BY_ + 2) * TG::PITCH_H };
+    struct Args {
+        T* r; T* delta; int p_fixed;      // p_fixed >= 0: read p from pbuf[p_fixed] (omni_apply_M), else by parity
+        const uint32_t* wcode; const uint32_t* flags;
+        Coef<T> K; Scalars* sc; double* partial; CondHandles cond;
+        T* q_out;                         // only for omni_apply_M: store q, leave r / delta untouched
+    };
+    struct Ctx {
+        T alpha; int pidx; bool first;
+        __device__ Ctx(const Args& a)
+        {
+            alpha = (T)a.sc->alpha;
+            first = (a.sc->k == 0);
+            pidx = (a.p_fixed >= 0) ? a.p_fixed : ((a.sc->k & 1) ^ 1);
+        }
+    };
+    using TC = XEdge;
+    __device__ static TC thread_init(const Geom& g, int x) { return make_xedge<V>(g, x); }
+    __device__ static bool active(const Args& a) { return a.sc->inner_go != 0; }
+    __device__ static void idle(const Args& a) { set_cond(a.cond, -1, 0); }
+    __device__ static void produce(const Args& a, const Ctx& c, const TmaSet& m, uint32_t stage, uint32_t bar, int x0,
+                                   int y0, int plane, bool inner)
+    {
+        const bool ext = inner && (a.q_out == nullptr);
+        const bool dl = ext && !c.first;           // first CG iteration: delta counts as zero, never read
+        mbar_expect_tx(bar, BOX_H + (ext ? TG::TILE_C : 0) + (dl ? TG::TILE_C : 0));
+        tma_load_3d(stage, &m.p_h[c.pidx], bar, x0 - TG::HX, y0 - 1, plane);
+        if (ext) tma_load_3d(stage + TG::TILE_H, &m.r_c, bar, x0, y0, plane);
+        if (dl) tma_load_3d(stage + TG::TILE_H + TG::TILE_C, &m.d_c, bar, x0, y0, plane);
+    }
+    __device__ static void emit(const Args& a, const Ctx& c, const Geom&, long long idx, const char* sB, const char* sC,
+                                const char* sF, int warp, int lane, bool out, uint32_t fb, const TC& xe, double& acc)
+    {
+        const int row = (warp + 1) * TG::PITCH_H;
+        const int off = row + (TG::HX + lane * V) * (int)sizeof(T);
+        T vm[V], vc[V], vp[V], vn[V], vs[V];
+        lds_chunk<T, V>(sC + off, vc);
+        lds_chunk<T, V>(sC + off + TG::PITCH_H, vn);
+        lds_chunk<T, V>(sC + off - TG::PITCH_H, vs);
+        lds_chunk<T, V>(sF + off, vp);
+        lds_chunk<T, V>(sB + off, vm);
+        const T hl = *reinterpret_cast<const T*>(sC + row + (TG::HX - 1) * (int)sizeof(T));
+        const T hr = *reinterpret_cast<const T*>(sC + row + (TG::HX + TG::BX) * (int)sizeof(T));
+        T xl = __shfl_up_sync(0xffffffffu, vc[V - 1], 1);
+        T xr = __shfl_down_sync(0xffffffffu, vc[0], 1);
+        if (lane == 0) xl = hl;
+        if (lane == 31) xr = hr;
+        if (!out) return;
+        T q[V];
+        apply_M_chunk<T, V>(q, vm, vc, vp, vn, vs, xl, xr, fb, a.wcode, idx, a.K, xe);
+        if (a.q_out != nullptr) {
+            st_chunk<T, V>(a.q_out + idx, q);
+#pragma unroll
+            for (int i = 0; i < V; ++i) acc += (double)vc[i] * (double)q[i];
+            return;
+        }
+        const int eoff = TG::TILE_H + (warp * TG::BX + lane * V) * (int)sizeof(T);
+        T er[V], ed[V], rn[V], dn[V];
+        lds_chunk<T, V>(sC + eoff, er);
+        if (c.first) zero_chunk<T, V>(ed); else lds_chunk<T, V>(sC + eoff + TG::TILE_C, ed);
+#pragma unroll
+        for (int i = 0; i < V; ++i) {
+            rn[i] = er[i] - c.alpha * q[i];
+            dn[i] = ed[i] + c.alpha * vc[i];
+            acc += (double)rn[i] * (double)rn[i];
+        }
+        st_chunk<T, V>(a.r + idx, rn);
+        st_chunk<T, V>(a.delta + idx, dn);
+    }
+    __device__ static void finalize(const Args& a, const double (&tot)[1])
+    {
+        Scalars* s = a.sc;
+        if (a.q_out != nullptr) { s->gamma = tot[0]; return; }
+        const double rho1 = tot[0];
+        if (!isfinite(rho1)) {
+            s->status = ST_BREAKDOWN; s->inner_go = 0; s->outer_go = 0;
+            set_cond(a.cond, 0, 0);
+            return;
+        }
+        s->beta = rho1 / s->rho;
+        s->rho = rho1;
+        s->k += 1;
+        s->cg_total += 1;
+        const int go = (rho1 > s->thresh2) && (rho1 != 0.0) && (s->k < s->max_cg);
+        s->inner_go = go;
+        set_cond(a.cond, -1, go);
+    }
+};
+
+}  // namespace omni
