@@ -60,13 +60,27 @@ struct TileGeom {
     static constexpr int NTHR = 32 * (BY + 1);             // BY consumer warps + 1 producer warp
 };
 
-// chunk accessors into a haloed / plain tile for (row w, lane l)
+// explicit shared-space loads (generic LD through a computed pointer costs an address-space check and a longer
+// scoreboard): addresses are 32-bit shared-window offsets
 template <typename T, int V>
-__device__ __forceinline__ void lds_chunk(const char* p, T (&v)[V])
+__device__ __forceinline__ void lds_chunk(uint32_t addr, T (&v)[V])
 {
     static_assert(V * sizeof(T) == 16, "one 16-byte piece per lane");
-    uint4 u = *reinterpret_cast<const uint4*>(p);
+    uint4 u;
+    asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(u.x), "=r"(u.y), "=r"(u.z), "=r"(u.w) : "r"(addr));
     memcpy(v, &u, 16);
+}
+__device__ __forceinline__ float lds_scalar(uint32_t addr, float)
+{
+    float v;
+    asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(addr));
+    return v;
+}
+__device__ __forceinline__ double lds_scalar(uint32_t addr, double)
+{
+    double v;
+    asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(addr));
+    return v;
 }
 
 template <class Op>
@@ -107,12 +121,15 @@ tma_kernel(const Geom g, const int zlen, const typename Op::Args a, const __grid
     if (warp == BY) {
         // ---------------------------------------------------------------- producer warp (one elected lane)
         if (lane == 0) {
+            int s = 0;
+            uint32_t phase = 1;                     // parity of the previous use of slot s (first pass: no wait)
             for (int e = 0; e < E; ++e) {
-                const int s = e % D;
-                if (e >= D) mbar_wait(bar_s + 8 * (D + s), (uint32_t)((e / D - 1) & 1));
+                if (e >= D) mbar_wait(bar_s + 8 * (D + s), phase);
                 const int c = k0 - 1 + e;
                 Op::produce(a, ctx, maps, smem_s + (uint32_t)(s * Op::STAGE_BYTES), bar_s + 8 * s, x0, y0, c,
                             (c >= k0) && (c < k1));
+                s = (s + 1 == D) ? 0 : s + 1;
+                phase ^= (s == 0);
             }
         }
     } else {
@@ -122,22 +139,29 @@ tma_kernel(const Geom g, const int zlen, const typename Op::Args a, const __grid
         const typename Op::TC tc = Op::thread_init(g, x);
         const long long rowbase = (long long)j * g.px + x;
         uint32_t fw_next = 0, fw_cur = 0;
+        // running state instead of per-event div/mod: slot of event e, its phase bit, the shared addresses of the
+        // stages of events e-2 / e-1 / e, the cell offset of plane c
+        int s = 0, sB = 0;
+        uint32_t phase = 0;
+        uint32_t aB = smem_s, aC = smem_s, aF = smem_s;
+        long long off = rowbase + (long long)(k0 - 1) * g.pplane;
         for (int e = 0; e < E; ++e) {
-            const int s = e % D;
-            mbar_wait(bar_s + 8 * s, (uint32_t)((e / D) & 1));
-            const int c = k0 - 1 + e;
+            mbar_wait(bar_s + 8 * s, phase);
             fw_cur = fw_next;
-            if (out && c >= k0 && c < k1) fw_next = a.flags[((rowbase + (long long)c * g.pplane) >> 2) >> 5];
+            if (out && e >= 1 && e <= E - 2) fw_next = a.flags[(off >> 2) >> 5];      // plane c is emitted at event e+1
             if (e >= 2) {                            // emit plane c-1 from stages e-2 (B), e-1 (centre), e (F)
-                const long long idx = rowbase + (long long)(c - 1) * g.pplane;
-                const char* sB = smem + ((e - 2) % D) * Op::STAGE_BYTES;
-                const char* sC = smem + ((e - 1) % D) * Op::STAGE_BYTES;
-                const char* sF = smem + s * Op::STAGE_BYTES;
+                const long long idx = off - g.pplane;
                 const uint32_t fb = (fw_cur >> (unsigned)((idx >> 2) & 31)) & 1u;
-                Op::emit(a, ctx, g, idx, sB, sC, sF, warp, lane, out, fb, tc, acc);
+                Op::emit(a, ctx, idx, aB, aC, aF, warp, lane, out, fb, tc, acc);
                 __syncwarp();
-                if (lane == 0) mbar_arrive(bar_s + 8 * (D + (e - 2) % D));
+                if (lane == 0) mbar_arrive(bar_s + 8 * (D + sB));
+                sB = (sB + 1 == D) ? 0 : sB + 1;
             }
+            off += g.pplane;
+            aB = aC; aC = aF;
+            s = (s + 1 == D) ? 0 : s + 1;
+            phase ^= (s == 0);
+            aF = smem_s + (uint32_t)(s * Op::STAGE_BYTES);
         }
     }
 
@@ -203,7 +227,7 @@ struct OpT3 {
         tma_load_3d(stage, &m.r_h, bar, x0 - TG::HX, y0 - 1, plane);
         tma_load_3d(stage + TG::TILE_H, &m.p_h[c.par], bar, x0 - TG::HX, y0 - 1, plane);
     }
-    __device__ static void pnew_chunk(const char* st, int off, T beta, T (&v)[V])
+    __device__ static void pnew_chunk(uint32_t st, int off, T beta, T (&v)[V])
     {
         T r[V], p[V];
         lds_chunk<T, V>(st + off, r);
@@ -211,8 +235,8 @@ struct OpT3 {
 #pragma unroll
         for (int i = 0; i < V; ++i) v[i] = r[i] + beta * p[i];
     }
-    __device__ static void emit(const Args& a, const Ctx& c, const Geom&, long long idx, const char* sB, const char* sC,
-                                const char* sF, int warp, int lane, bool out, uint32_t fb, const TC& xe, double& acc)
+    __device__ static void emit(const Args& a, const Ctx& c, long long idx, uint32_t sB, uint32_t sC, uint32_t sF,
+                                int warp, int lane, bool out, uint32_t fb, const TC& xe, double& acc)
     {
         const int row = (warp + 1) * TG::PITCH_H;
         const int off = row + (TG::HX + lane * V) * (int)sizeof(T);
@@ -224,8 +248,8 @@ struct OpT3 {
         pnew_chunk(sB, off, c.beta, vm);
         // x neighbours: shuffles inside the warp, the row's two halo cells (same address for all lanes) at its ends
         const int hl_off = row + (TG::HX - 1) * (int)sizeof(T), hr_off = row + (TG::HX + TG::BX) * (int)sizeof(T);
-        const T hl = *reinterpret_cast<const T*>(sC + hl_off) + c.beta * *reinterpret_cast<const T*>(sC + TG::TILE_H + hl_off);
-        const T hr = *reinterpret_cast<const T*>(sC + hr_off) + c.beta * *reinterpret_cast<const T*>(sC + TG::TILE_H + hr_off);
+        const T hl = lds_scalar(sC + hl_off, T()) + c.beta * lds_scalar(sC + TG::TILE_H + hl_off, T());
+        const T hr = lds_scalar(sC + hr_off, T()) + c.beta * lds_scalar(sC + TG::TILE_H + hr_off, T());
         T xl = __shfl_up_sync(0xffffffffu, vc[V - 1], 1);
         T xr = __shfl_down_sync(0xffffffffu, vc[0], 1);
         if (lane == 0) xl = hl;
@@ -288,8 +312,8 @@ struct OpT4 {
         if (ext) tma_load_3d(stage + TG::TILE_H, &m.r_c, bar, x0, y0, plane);
         if (dl) tma_load_3d(stage + TG::TILE_H + TG::TILE_C, &m.d_c, bar, x0, y0, plane);
     }
-    __device__ static void emit(const Args& a, const Ctx& c, const Geom&, long long idx, const char* sB, const char* sC,
-                                const char* sF, int warp, int lane, bool out, uint32_t fb, const TC& xe, double& acc)
+    __device__ static void emit(const Args& a, const Ctx& c, long long idx, uint32_t sB, uint32_t sC, uint32_t sF,
+                                int warp, int lane, bool out, uint32_t fb, const TC& xe, double& acc)
     {
         const int row = (warp + 1) * TG::PITCH_H;
         const int off = row + (TG::HX + lane * V) * (int)sizeof(T);
@@ -299,8 +323,8 @@ struct OpT4 {
         lds_chunk<T, V>(sC + off - TG::PITCH_H, vs);
         lds_chunk<T, V>(sF + off, vp);
         lds_chunk<T, V>(sB + off, vm);
-        const T hl = *reinterpret_cast<const T*>(sC + row + (TG::HX - 1) * (int)sizeof(T));
-        const T hr = *reinterpret_cast<const T*>(sC + row + (TG::HX + TG::BX) * (int)sizeof(T));
+        const T hl = lds_scalar(sC + row + (TG::HX - 1) * (int)sizeof(T), T());
+        const T hr = lds_scalar(sC + row + (TG::HX + TG::BX) * (int)sizeof(T), T());
         T xl = __shfl_up_sync(0xffffffffu, vc[V - 1], 1);
         T xr = __shfl_down_sync(0xffffffffu, vc[0], 1);
         if (lane == 0) xl = hl;
