@@ -40,7 +40,41 @@ def parse():
     ap.add_argument("--config", type=int, default=4)
     ap.add_argument("--dtype", default=None)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--converge", action="store_true",
+                    help="instead of the fixed-cap step: time ONE solve to the config's tolerance (BASELINE.md table)")
+    ap.add_argument("--max-cg", type=int, default=1000, help="--converge: CG cap per outer iteration")
+    ap.add_argument("--max-outer", type=int, default=200000, help="--converge: outer iteration cap")
     return ap.parse_args()
+
+
+def converge(args, cfg, dtype):
+    """Time-to-converged P of one configuration (whole omni_solve call, CUDA events, inputs resident)."""
+    import numpy as np
+    import torch
+    import paper_2311_16935_b200 as omni
+    from workloads import make_config
+    f = make_config(args.config, device="cuda")
+    tdt = torch.float32 if dtype == "f32" else torch.float64
+    g = [torch.from_numpy(c).to(tdt).cuda() for c in f["g"]] + [None] * (3 - len(f["g"]))
+    m = None if f["mask"] is None else torch.from_numpy(f["mask"]).cuda()
+    tol = 1e-5 if dtype == "f32" else 1e-8
+    omni.solve(g[0], g[1], g[2], m, f["d"], tol, 2, 2)                       # warm-up (module load, pool)
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    P, info = omni.solve(g[0], g[1], g[2], m, f["d"], tol, args.max_outer, args.max_cg)
+    e1.record()
+    torch.cuda.synchronize()
+    sec = e0.elapsed_time(e1) * 1e-3
+    Pn = P.double().cpu().numpy()
+    valid = ~np.isnan(Pn)
+    a, b = Pn[valid] - Pn[valid].mean(), f["P"][valid] - f["P"][valid].mean()
+    N = g[0].numel()
+    print(json.dumps({"converge": True, "workload": f"configs[{args.config}] {cfg['kind']} {cfg['n']} {dtype}", "tol": tol,
+                      "max_cg": args.max_cg, "outer_iters": info["outer_iters"], "cg_iters": info["cg_iters_total"],
+                      "seconds": sec, "eps_R": info["eps_R_final"], "status": info["status"],
+                      "updates_per_s": N * info["cg_iters_total"] / sec,
+                      "rel_l2_vs_analytic_P": float(np.linalg.norm(a - b) / np.linalg.norm(b))}))
 
 
 def measured_peak():
@@ -156,6 +190,10 @@ def main():
               "l2": "inputs larger than L2 (no flush)" if n ** ndim * (4 if dtype == "f32" else 8) > 126e6
               else "CG state fits L2: numbers are L2-resident, flushed between steps by the solve's own setup passes"}
 
+    if args.converge:
+        if rank == 0:
+            converge(args, cfg, dtype)
+        return
     if args.impl == "reference":
         if rank != 0:
             return

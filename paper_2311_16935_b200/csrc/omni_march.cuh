@@ -1,4 +1,5 @@
-// omni_march.cuh -- the z-marching tile engine shared by K2 / K3 / K4, and the three operators.
+// omni_march.cuh -- the cp.async z-marching tile engine and the K2 operator (outer boundary update).
+// (K3 / K4, the CG inner loop, run on the TMA + mbarrier pipeline of omni_tma.cuh.)
 //
 // A CTA owns a column of the grid: W = 32*V cells wide (1 KB of the widest streamed array), TYR-2 output rows (+2 halo
 // rows), zlen planes (+1 halo plane on each side).  Every thread owns one 32-byte chunk per streamed array and plane.
@@ -224,163 +225,6 @@ march_kernel(const Geom g, const int zlen, const typename Op::Args a)
         }
     }
 }
-
-// ------------------------------------------------------------------------------------------------ K3
-// p_new = r + beta p_old on the fly (also in the halo), store p_new, gamma = p_new . M p_new; alpha = rho / gamma.
-template <typename T, int TYR_, int D_, int MINB_>
-struct OpK3 {
-    using VT = T;
-    enum { V = 32 / sizeof(T), TYR = TYR_, D = D_, MINB = MINB_, NACC = 1, TICKET = 0, PIECES = 4 };
-    struct Args {
-        const T* r; T* pbuf[2]; const uint32_t* wcode; const uint32_t* flags;
-        Coef<T> K; Scalars* sc; double* partial; CondHandles cond;
-    };
-    struct Ctx {
-        T beta; const T* pold; T* pnew;
-        __device__ Ctx(const Args& a)
-        {
-            beta = (T)a.sc->beta;
-            int par = a.sc->k & 1;
-            pold = a.pbuf[par]; pnew = a.pbuf[par ^ 1];
-        }
-    };
-    struct Extra {};
-    using TC = XEdge;
-    __device__ static TC thread_init(const Geom& g, int x) { return make_xedge<V>(g, x); }
-    __device__ static bool active(const Args& a) { return a.sc->inner_go != 0; }
-    __device__ static void idle(const Args& a) { set_cond(a.cond, -1, 0); }
-    template <class SW>
-    __device__ static void issue(const Args& a, const Ctx& c, const SW& st, long long idx, bool ok, bool lok, bool rok,
-                                 long long, bool)
-    {
-        st.template put<T, 2>(0, a.r, idx, ok);
-        st.template put<T, 2>(2, c.pold, idx, ok);
-        if (threadIdx.x == 0) { st.put_halo(0, a.r, idx - 1, lok); st.put_halo(1, c.pold, idx - 1, lok); }
-        if (threadIdx.x == 31) { st.put_halo(2, a.r, idx + V, rok); st.put_halo(3, c.pold, idx + V, rok); }
-    }
-    template <class SR>
-    __device__ static void consume(const Args&, const Ctx& c, const SR& sr, T (&v)[V], T& hl, T& hr, Extra&)
-    {
-        T r[V], p[V];
-        sr.template get<T, V>(0, r);
-        sr.template get<T, V>(2, p);
-#pragma unroll
-        for (int i = 0; i < V; ++i) v[i] = r[i] + c.beta * p[i];
-        hl = hr = T(0);
-        if (threadIdx.x == 0) hl = sr.template get_halo<T>(0) + c.beta * sr.template get_halo<T>(1);
-        if (threadIdx.x == 31) hr = sr.template get_halo<T>(2) + c.beta * sr.template get_halo<T>(3);
-    }
-    __device__ static void emit(const Args& a, const Ctx& c, long long idx, const T (&vm)[V], const T (&vc)[V],
-                                const T (&vp)[V], const T (&vn)[V], const T (&vs)[V], T xl, T xr, const Extra&,
-                                uint32_t fb, const TC& xe, double (&acc)[1])
-    {
-        st_chunk<T, V>(c.pnew + idx, vc);
-        T q[V];
-        apply_M_chunk<T, V>(q, vm, vc, vp, vn, vs, xl, xr, fb, a.wcode, idx, a.K, xe);
-#pragma unroll
-        for (int i = 0; i < V; ++i) acc[0] += (double)vc[i] * (double)q[i];
-    }
-    __device__ static void finalize(const Args& a, const double (&tot)[1])
-    {
-        Scalars* s = a.sc;
-        double gamma = tot[0];
-        s->gamma = gamma;
-        if (!(gamma > 0.0) || !isfinite(gamma)) {      // also catches NaN
-            s->status = ST_BREAKDOWN; s->inner_go = 0; s->outer_go = 0;
-            set_cond(a.cond, 0, 0);
-        } else {
-            s->alpha = s->rho / gamma;
-        }
-    }
-};
-
-// ------------------------------------------------------------------------------------------------ K4
-// q = M p recomputed from p (never stored), delta += alpha p, r -= alpha q, rho' = r.r; beta = rho'/rho; loop test.
-template <typename T, int TYR_, int D_, int MINB_>
-struct OpK4 {
-    using VT = T;
-    enum { V = 32 / sizeof(T), TYR = TYR_, D = D_, MINB = MINB_, NACC = 1, TICKET = 1, PIECES = 6 };
-    struct Args {
-        T* r; T* delta; const T* pbuf[2]; const uint32_t* wcode; const uint32_t* flags;
-        Coef<T> K; Scalars* sc; double* partial; CondHandles cond;
-        T* q_out;        // only for omni_apply_M: store q, leave r/delta untouched (NULL inside the solve)
-    };
-    struct Ctx {
-        T alpha; const T* p; bool first;
-        __device__ Ctx(const Args& a)
-        {
-            alpha = (T)a.sc->alpha;
-            first = (a.sc->k == 0);
-            p = a.pbuf[(a.sc->k & 1) ^ 1];
-        }
-    };
-    struct Extra { T r[V], d[V]; };
-    using TC = XEdge;
-    __device__ static TC thread_init(const Geom& g, int x) { return make_xedge<V>(g, x); }
-    __device__ static bool active(const Args& a) { return a.sc->inner_go != 0; }
-    __device__ static void idle(const Args& a) { set_cond(a.cond, -1, 0); }
-    template <class SW>
-    __device__ static void issue(const Args& a, const Ctx& c, const SW& st, long long idx, bool ok, bool lok, bool rok,
-                                 long long eidx, bool eok)
-    {
-        st.template put<T, 2>(0, c.p, idx, ok);
-        if (threadIdx.x == 0) st.put_halo(0, c.p, idx - 1, lok);
-        if (threadIdx.x == 31) st.put_halo(1, c.p, idx + V, rok);
-        const bool e = eok && (a.q_out == nullptr);
-        st.template put<T, 2>(2, (const T*)a.r, eidx, e);
-        st.template put<T, 2>(4, (const T*)a.delta, eidx, e && !c.first);
-    }
-    template <class SR>
-    __device__ static void consume(const Args&, const Ctx&, const SR& sr, T (&v)[V], T& hl, T& hr, Extra& e)
-    {
-        sr.template get<T, V>(0, v);
-        hl = hr = T(0);
-        if (threadIdx.x == 0) hl = sr.template get_halo<T>(0);
-        if (threadIdx.x == 31) hr = sr.template get_halo<T>(1);
-        sr.template get<T, V>(2, e.r);
-        sr.template get<T, V>(4, e.d);
-    }
-    __device__ static void emit(const Args& a, const Ctx& c, long long idx, const T (&vm)[V], const T (&vc)[V],
-                                const T (&vp)[V], const T (&vn)[V], const T (&vs)[V], T xl, T xr, const Extra& e,
-                                uint32_t fb, const TC& xe, double (&acc)[1])
-    {
-        T q[V];
-        apply_M_chunk<T, V>(q, vm, vc, vp, vn, vs, xl, xr, fb, a.wcode, idx, a.K, xe);
-        if (a.q_out != nullptr) {           // operator-only mode (omni_apply_M): q and p.q
-            st_chunk<T, V>(a.q_out + idx, q);
-#pragma unroll
-            for (int i = 0; i < V; ++i) acc[0] += (double)vc[i] * (double)q[i];
-            return;
-        }
-        T rn[V], dn[V];
-#pragma unroll
-        for (int i = 0; i < V; ++i) {
-            rn[i] = e.r[i] - c.alpha * q[i];
-            dn[i] = e.d[i] + c.alpha * vc[i];       // first CG iteration: delta was zero-filled by the ring
-            acc[0] += (double)rn[i] * (double)rn[i];
-        }
-        st_chunk<T, V>(a.r + idx, rn);
-        st_chunk<T, V>(a.delta + idx, dn);
-    }
-    __device__ static void finalize(const Args& a, const double (&tot)[1])
-    {
-        Scalars* s = a.sc;
-        if (a.q_out != nullptr) { s->gamma = tot[0]; return; }
-        double rho1 = tot[0];
-        if (!isfinite(rho1)) {
-            s->status = ST_BREAKDOWN; s->inner_go = 0; s->outer_go = 0;
-            set_cond(a.cond, 0, 0);
-            return;
-        }
-        s->beta = rho1 / s->rho;
-        s->rho = rho1;
-        s->k += 1;
-        s->cg_total += 1;
-        int go = (rho1 > s->thresh2) && (rho1 != 0.0) && (s->k < s->max_cg);
-        s->inner_go = go;
-        set_cond(a.cond, -1, go);
-    }
-};
 
 // ------------------------------------------------------------------------------------------------ K2
 // outer boundary update (Eq. 12 collapsed): P <- P + delta; r0 = S - L P with
