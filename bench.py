@@ -29,7 +29,7 @@ UNIT = "grid-point CG updates/s"
 CPU_SAMPLE_EDGE = 200                   # 3D: edge of the corner crop the oracle is timed on (2D: the whole grid)
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel (K4) from the ncu --set full capture
 # summarised in profiles/r1_ncu_k3_k4_500cube_f32.md; only valid for that workload.
-NCU_TRAFFIC_K4 = {(4, "f32"): 1.527892e9 + 0.952720e9}
+NCU_TRAFFIC_K4 = {(4, "f32"): 1.537037e9 + 0.957180e9}
 
 
 def parse():
@@ -285,7 +285,7 @@ def main():
     t3 = k3_ms / max(k3_n, 1) * 1e-3
     alg4, alg3 = 5 * esz * N, 3 * esz * N          # K4: R p,r,delta W r,delta ; K3: R r,p W p
     ach = alg4 / t4 / 1e9 if t4 > 0 else 0.0
-    roofline = {"bound": "hbm", "kernel": "K4 march_kernel<OpK4> (operator recomputed + axpys + r.r)",
+    roofline = {"bound": "hbm", "kernel": "K4 tma_kernel<OpT4> (operator recomputed + axpys + r.r)",
                 "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak, "peak_source": peak_src,
                 "traffic": NCU_TRAFFIC_K4.get((args.config, dtype)),
                 "algorithmic_bytes_per_launch": alg4, "us_per_launch": t4 * 1e6,
