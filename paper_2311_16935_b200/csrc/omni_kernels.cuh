@@ -46,6 +46,7 @@ struct Coef {
 // which x-edge cells a thread's chunk holds (thread constants)
 struct XEdge {
     bool L, A, B;      // holds cells {0,1} / cell nx-2 / cell nx-1
+    bool any;          // L || A || B
     int posA, posB;    // their positions inside the chunk
 };
 template <int V>
@@ -57,6 +58,7 @@ __device__ __forceinline__ XEdge make_xedge(const Geom& g, int x)
     e.posA = (g.nx - 2) % V; e.posB = (g.nx - 1) % V;
     e.A = on && (x == g.nx - 2 - e.posA);
     e.B = on && (x == g.nx - 1 - e.posB);
+    e.any = e.L || e.A || e.B;
     return e;
 }
 
@@ -227,7 +229,7 @@ __device__ __forceinline__ void apply_M_chunk(T (&q)[V], const T (&vm)[V], const
         q[i] = apply_M_interior(vc[i], e, w, vn[i], vs[i], vp[i], vm[i], K);
     }
     if (fb == 0) {
-        if (xe.L || xe.A || xe.B) xedge_fix<T, V>(q, vm, vc, vp, vn, vs, xl, xr, xe, K);
+        if (xe.any) xedge_fix<T, V>(q, vm, vc, vp, vn, vs, xl, xr, xe, K);
     } else {
         uint32_t code[V];
         ld_chunk<uint32_t, V>(wcode + idx, code);

@@ -30,11 +30,9 @@ __device__ __forceinline__ void mbar_arrive(uint32_t bar)
 }
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
 {
-    uint32_t done;
-    do {
-        asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.b32 %0, 1, 0, p;\n\t}"
-                     : "=r"(done) : "r"(bar), "r"(parity) : "memory");
-    } while (!done);
+    // labels are local to the PTX block scope, so the loop can be inlined any number of times
+    asm volatile("{\n\t.reg .pred p;\n\tWAIT_LOOP:\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
+                 "@p bra WAIT_DONE;\n\tbra WAIT_LOOP;\n\tWAIT_DONE:\n\t}" ::"r"(bar), "r"(parity) : "memory");
 }
 __device__ __forceinline__ void tma_load_3d(uint32_t dst, const CUtensorMap* map, uint32_t bar, int c0, int c1, int c2)
 {
@@ -145,14 +143,16 @@ tma_kernel(const Geom g, const int zlen, const typename Op::Args a, const __grid
         uint32_t phase = 0;
         uint32_t aB = smem_s, aC = smem_s, aF = smem_s;
         long long off = rowbase + (long long)(k0 - 1) * g.pplane;
+        typename Op::State st;
         for (int e = 0; e < E; ++e) {
             mbar_wait(bar_s + 8 * s, phase);
+            Op::advance(st, ctx, aF, warp, lane);
             fw_cur = fw_next;
             if (out && e >= 1 && e <= E - 2) fw_next = a.flags[(off >> 2) >> 5];      // plane c is emitted at event e+1
             if (e >= 2) {                            // emit plane c-1 from stages e-2 (B), e-1 (centre), e (F)
                 const long long idx = off - g.pplane;
                 const uint32_t fb = (fw_cur >> (unsigned)((idx >> 2) & 31)) & 1u;
-                Op::emit(a, ctx, idx, aB, aC, aF, warp, lane, out, fb, tc, acc);
+                Op::emit(a, ctx, st, idx, aB, aC, aF, warp, lane, out, fb, tc, acc);
                 __syncwarp();
                 if (lane == 0) mbar_arrive(bar_s + 8 * (D + sB));
                 sB = (sB + 1 == D) ? 0 : sB + 1;
@@ -235,17 +235,30 @@ struct OpT3 {
 #pragma unroll
         for (int i = 0; i < V; ++i) v[i] = r[i] + beta * p[i];
     }
-    __device__ static void emit(const Args& a, const Ctx& c, long long idx, uint32_t sB, uint32_t sC, uint32_t sF,
+    // own-chunk p_new of the last three planes: each plane's chunk is formed once (when its stage arrives) and reused
+    // as F, centre and B neighbour of three consecutive emissions
+    struct State {
+        T m[V], c[V], f[V];
+        __device__ State() { zero_chunk<T, V>(m); zero_chunk<T, V>(c); zero_chunk<T, V>(f); }
+    };
+    __device__ static void advance(State& st, const Ctx& c, uint32_t sF, int warp, int lane)
+    {
+        const int off = (warp + 1) * TG::PITCH_H + (TG::HX + lane * V) * (int)sizeof(T);
+#pragma unroll
+        for (int i = 0; i < V; ++i) { st.m[i] = st.c[i]; st.c[i] = st.f[i]; }
+        pnew_chunk(sF, off, c.beta, st.f);
+    }
+    __device__ static void emit(const Args& a, const Ctx& c, const State& st, long long idx, uint32_t, uint32_t sC, uint32_t,
                                 int warp, int lane, bool out, uint32_t fb, const TC& xe, double& acc)
     {
         const int row = (warp + 1) * TG::PITCH_H;
         const int off = row + (TG::HX + lane * V) * (int)sizeof(T);
-        T vm[V], vc[V], vp[V], vn[V], vs[V];
-        pnew_chunk(sC, off, c.beta, vc);
+        T vn[V], vs[V];
+        const T (&vm)[V] = st.m;
+        const T (&vc)[V] = st.c;
+        const T (&vp)[V] = st.f;
         pnew_chunk(sC, off + TG::PITCH_H, c.beta, vn);
         pnew_chunk(sC, off - TG::PITCH_H, c.beta, vs);
-        pnew_chunk(sF, off, c.beta, vp);
-        pnew_chunk(sB, off, c.beta, vm);
         // x neighbours: shuffles inside the warp, the row's two halo cells (same address for all lanes) at its ends
         const int hl_off = row + (TG::HX - 1) * (int)sizeof(T), hr_off = row + (TG::HX + TG::BX) * (int)sizeof(T);
         const T hl = lds_scalar(sC + hl_off, T()) + c.beta * lds_scalar(sC + TG::TILE_H + hl_off, T());
@@ -312,7 +325,9 @@ struct OpT4 {
         if (ext) tma_load_3d(stage + TG::TILE_H, &m.r_c, bar, x0, y0, plane);
         if (dl) tma_load_3d(stage + TG::TILE_H + TG::TILE_C, &m.d_c, bar, x0, y0, plane);
     }
-    __device__ static void emit(const Args& a, const Ctx& c, long long idx, uint32_t sB, uint32_t sC, uint32_t sF,
+    struct State {};
+    __device__ static void advance(State&, const Ctx&, uint32_t, int, int) {}
+    __device__ static void emit(const Args& a, const Ctx& c, const State&, long long idx, uint32_t sB, uint32_t sC, uint32_t sF,
                                 int warp, int lane, bool out, uint32_t fb, const TC& xe, double& acc)
     {
         const int row = (warp + 1) * TG::PITCH_H;
