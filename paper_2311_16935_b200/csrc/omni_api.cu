@@ -15,6 +15,13 @@
 
 using namespace omni;
 
+#ifndef OMNI_BY
+#define OMNI_BY 8
+#define OMNI_D3 6
+#define OMNI_D4 5
+#define OMNI_MINB 3
+#endif
+
 namespace {
 
 std::atomic<long long> g_launches{0};
@@ -117,6 +124,8 @@ void host_constants(int nz, double dx, double dy, double dz, HostConst& H)
     H.c[1][2] = H.c[2][1] = 0.5 * (s[1] + s[2] - s[0]);
 }
 
+uint32_t std_axis_code(int ax, int pos, int n, int naxes);
+
 template <typename T>
 Coef<T> make_coef(const HostConst& H, double dx, double dy, double dz, const Geom& g)
 {
@@ -134,33 +143,39 @@ Coef<T> make_coef(const HostConst& H, double dx, double dy, double dz, const Geo
         }
     }
     K.icode = g.icode;
-    for (int cls = 0; cls < 4; ++cls)
-        for (int d = 0; d < 6; ++d) {
-            const int a = d >> 1;
-            const uint32_t bits = (g.stdc[cls] >> (5 * d)) & 31u;
-            const int far = bits & 1, nb = (bits >> 1) & 3, nc = (bits >> 3) & 3;
-            const double w = (far * H.c[a][a] + nb * H.c[a][(a + 1) % 3] + nc * H.c[a][(a + 2) % 3]) / H.Atot;
-            K.xc[cls][d] = (T)(H.F[a] / H.Atot - w);
+    const int naxes = (g.nz > 1) ? 3 : 2;
+    const int n3[3] = { g.nx, g.ny, g.nz };
+    for (int ax = 0; ax < 3; ++ax)
+        for (int cls = 0; cls < 4; ++cls) {
+            const int pos = (cls < 2) ? cls : n3[ax] - 4 + cls;          // cells 0, 1, n-2, n-1
+            const uint32_t code = (ax < naxes && n3[ax] >= 4) ? std_axis_code(ax, pos, n3[ax], naxes) : g.icode;
+            for (int d = 0; d < 6; ++d) {
+                const int a = d >> 1;
+                const uint32_t bits = (code >> (5 * d)) & 31u;
+                const int far = bits & 1, nb = (bits >> 1) & 3, nc = (bits >> 3) & 3;
+                const double w = (far * H.c[a][a] + nb * H.c[a][(a + 1) % 3] + nc * H.c[a][(a + 2) % 3]) / H.Atot;
+                K.fc[ax][cls][d] = (T)(H.F[a] / H.Atot - w);
+            }
         }
     return K;
 }
 
 // ------------------------------------------------------------------------------------------------ geometry / workspace
 
-// wcode of cell i of a row whose y/z neighbourhood is complete (mirrors codes_kernel with only x bounded)
-uint32_t std_xcode(int i, int nx, int naxes)
+// wcode of the cell at position pos of axis ax (length n) when only that axis is bounded (mirrors codes_kernel)
+uint32_t std_axis_code(int ax, int pos, int n, int naxes)
 {
-    auto vx = [&](int ii) { return (ii >= 0 && ii < nx) ? 1u : 0u; };
+    auto vx = [&](int ii) { return (ii >= 0 && ii < n) ? 1u : 0u; };
     uint32_t code = WCODE_VALID;
     for (int d = 0; d < 2 * naxes; ++d) {
         const int a = d >> 1, sg = (d & 1) ? -1 : 1;
-        const int qi = i + (a == 0 ? sg : 0);
-        if (!vx(qi)) continue;
+        const int q = pos + (a == ax ? sg : 0);
+        if (!vx(q)) continue;
         const int b = (a + 1) % 3, c = (a + 2) % 3;
-        const uint32_t far = vx(qi + (a == 0 ? sg : 0));
-        auto side = [&](int ax) -> uint32_t {
-            if (ax >= naxes) return 0u;
-            if (ax == 0) return vx(qi + 1) + vx(qi - 1);
+        const uint32_t far = vx(q + (a == ax ? sg : 0));
+        auto side = [&](int s_ax) -> uint32_t {
+            if (s_ax >= naxes) return 0u;
+            if (s_ax == ax) return vx(q + 1) + vx(q - 1);
             return 2u;
         };
         code |= (far | (side(b) << 1) | (side(c) << 3)) << (5 * d);
@@ -179,16 +194,19 @@ bool make_geom(int nx, int ny, int nz, int elem_size, Geom& g)
     g.pplane = px * ny;
     g.npad = npad;
     const int naxes = (nz > 1) ? 3 : 2;
-    g.xfix = (nx >= 4) ? 1 : 0;
-    g.icode = std_xcode(2, 5, naxes);
-    g.stdc[0] = std_xcode(0, nx, naxes); g.stdc[1] = std_xcode(1, nx, naxes);
-    g.stdc[2] = std_xcode(nx - 2, nx, naxes); g.stdc[3] = std_xcode(nx - 1, nx, naxes);
+    const int n3[3] = { nx, ny, nz };
+    for (int a = 0; a < 3; ++a) g.fix[a] = (a < naxes && n3[a] >= 4) ? 1 : 0;
+    g.xfix = g.fix[0];
+    g.icode = std_axis_code(0, 2, 5, naxes);
+    g.tbx = 512 / elem_size; g.tby = OMNI_BY;                 // the K3/K4 tile (omni_tma.cuh TileGeom)
+    g.ntx = (g.px + g.tbx - 1) / g.tbx; g.nty = (ny + g.tby - 1) / g.tby;
+    g.twords = (nz + 31) / 32;
     return true;
 }
 
 template <typename T>
 struct Workspace {
-    uint8_t* link; uint32_t* wcode; uint32_t* flags;
+    uint8_t* link; uint32_t* wcode; uint32_t* flags; uint32_t* tflags;
     T *S, *r, *p0, *p1, *delta;
     double* P; double* P1; double* partial; Scalars* sc;
 };
@@ -212,6 +230,7 @@ size_t carve(const Geom& g, char* base, Workspace<T>* w)
     char* link = take(n);
     char* wcode = take(n * 4);
     char* flags = take(((n / 4 + 31) / 32 + 1) * 4);
+    char* tflags = take((size_t)g.ntx * g.nty * g.twords * 4);
     char* S = take(n * sizeof(T));
     char* r = take(n * sizeof(T));
     char* p0 = take(n * sizeof(T));
@@ -222,7 +241,7 @@ size_t carve(const Geom& g, char* base, Workspace<T>* w)
     char* partial = take(partial_slots(g) * sizeof(double));
     char* sc = take(sizeof(Scalars));
     if (w) {
-        w->link = (uint8_t*)link; w->wcode = (uint32_t*)wcode; w->flags = (uint32_t*)flags;
+        w->link = (uint8_t*)link; w->wcode = (uint32_t*)wcode; w->flags = (uint32_t*)flags; w->tflags = (uint32_t*)tflags;
         w->S = (T*)S; w->r = (T*)r; w->p0 = (T*)p0; w->p1 = (T*)p1; w->delta = (T*)delta;
         w->P = (double*)P; w->P1 = (double*)P1; w->partial = (double*)partial; w->sc = (Scalars*)sc;
     }
@@ -291,14 +310,8 @@ cudaError_t launch_march(const Geom& g, const typename Op::Args& a, cudaStream_t
 
 // K3 / K4: TMA + mbarrier pipeline (omni_tma.cuh): 512-byte x 8-row tiles, 8 consumer warps + 1 producer warp,
 // several CTAs per SM (shared memory: K3 6 stages x 10.8 KB, K4 5 stages x 13.4 KB).  K2: cp.async engine.
-#ifndef OMNI_BY
-#define OMNI_BY 8
-#define OMNI_D3 6
-#define OMNI_D4 5
-#define OMNI_MINB 3
-#endif
 template <typename T> using K3 = OpT3<T, OMNI_BY, OMNI_D3, OMNI_MINB>;
-template <typename T> using K4 = OpT4<T, OMNI_BY, OMNI_D4, OMNI_MINB>;
+template <typename T> using K4 = OpT4<T, OMNI_BY, OMNI_D4, (sizeof(T) == 8 ? 2 : OMNI_MINB)>;   // fp64 K4: 72 registers spill
 template <typename T> using K2 = OpK2<T, 16, 3, 1>;
 
 
@@ -327,7 +340,9 @@ MarchCfg tma_config(const Geom& g)
         const int nseg = (g.nz + zlen - 1) / zlen;
         const long long ctas = tiles * nseg;
         const long long waves = (ctas + slots - 1) / slots;
-        const double cost = (double)waves * (zlen + (nseg > 1 ? 2 : 0) + 3);
+        // CTAs next to masked cells run the slower general loop: with fewer than three waves a few of them become
+        // the tail of the launch, so shallow schedules are penalised (measured on the masked 256^3 case)
+        const double cost = (double)waves * (zlen + (nseg > 1 ? 2 : 0) + 3) * (waves < 3 ? 1.25 : 1.0);
         if (cost < best_cost) { best_cost = cost; best = nseg; }
         if (zlen <= 4) break;
     }
@@ -390,7 +405,8 @@ int setup_codes(const Geom& g, const Workspace<T>& w, const T* gx, const T* gy, 
     uint8_t* vbyte = reinterpret_cast<uint8_t*>(w.p0);       // scratch: p0 is cleared afterwards
     validity_kernel<T><<<blocks_for(g.npad, 256), 256, 0, st>>>(g, gx, gy, gz, mask, vbyte);
     CK(cudaGetLastError());
-    codes_kernel<<<blocks_for(g.npad / 4, 256), 256, 0, st>>>(g, vbyte, w.link, w.wcode, w.flags);
+    CK(cudaMemsetAsync(w.tflags, 0, (size_t)g.ntx * g.nty * g.twords * 4, st));
+    codes_kernel<<<blocks_for(g.npad / 4, 256), 256, 0, st>>>(g, vbyte, w.link, w.wcode, w.flags, w.tflags);
     CK(cudaGetLastError());
     g_launches.fetch_add(2, std::memory_order_relaxed);
     const size_t n = (size_t)g.npad;
@@ -413,19 +429,20 @@ int launch_source(const Geom& g, const Workspace<T>& w, const Coef<T>& K, const 
 }
 
 template <typename T>
-typename K2<T>::Args k2_args(const Workspace<T>& w, const HostConst& H, CondHandles ch, int fold)
+typename K2<T>::Args k2_args(const Geom& g, const Workspace<T>& w, const HostConst& H, CondHandles ch, int fold)
 {
     typename K2<T>::Args a;
     a.Pbuf[0] = w.P; a.Pbuf[1] = fold ? w.P1 : w.P; a.delta = w.delta; a.S = w.S; a.r = w.r; a.link = w.link; a.flags = w.flags;
     for (int i = 0; i < 3; ++i) a.t[i] = H.F[i] / H.Atot;
     a.sc = w.sc; a.partial = w.partial; a.cond = ch; a.fold_delta = fold;
+    a.nz = g.nz; a.fixz = g.fix[2];
     return a;
 }
 template <typename T>
 typename K3<T>::Args k3_args(const Workspace<T>& w, const Coef<T>& K, CondHandles ch)
 {
     typename K3<T>::Args a;
-    a.pbuf[0] = w.p0; a.pbuf[1] = w.p1; a.wcode = w.wcode; a.flags = w.flags;
+    a.pbuf[0] = w.p0; a.pbuf[1] = w.p1; a.wcode = w.wcode; a.flags = w.flags; a.tflags = w.tflags;
     a.K = K; a.sc = w.sc; a.partial = w.partial; a.cond = ch;
     return a;
 }
@@ -433,7 +450,7 @@ template <typename T>
 typename K4<T>::Args k4_args(const Workspace<T>& w, const Coef<T>& K, CondHandles ch)
 {
     typename K4<T>::Args a;
-    a.r = w.r; a.delta = w.delta; a.p_fixed = -1; a.wcode = w.wcode; a.flags = w.flags;
+    a.r = w.r; a.delta = w.delta; a.p_fixed = -1; a.wcode = w.wcode; a.flags = w.flags; a.tflags = w.tflags;
     a.K = K; a.sc = w.sc; a.partial = w.partial; a.cond = ch; a.q_out = nullptr;
     return a;
 }
@@ -455,7 +472,7 @@ int run_loop_host(const Geom& g, const Workspace<T>& w, const HostConst& H, cons
                   cudaStream_t st)
 {
     CondHandles ch{ 0, 0, 0 };
-    const auto a2 = k2_args<T>(w, H, ch, 1);
+    const auto a2 = k2_args<T>(g, w, H, ch, 1);
     const auto a3 = k3_args<T>(w, K, ch);
     const auto a4 = k4_args<T>(w, K, ch);
     TmaSet maps;
@@ -556,7 +573,7 @@ int run_loop_graph(const Geom& g, const Workspace<T>& w, const HostConst& H, con
         if (cudaStreamCreateWithFlags(&cap, cudaStreamNonBlocking) != cudaSuccess) break;
         // K2 into the outer body
         if (cudaStreamBeginCaptureToGraph(cap, bodyOuter, nullptr, nullptr, 0, cudaStreamCaptureModeThreadLocal) != cudaSuccess) break;
-        cudaError_t e = launch_march<K2<T>>(g, k2_args<T>(w, H, ch, 1), cap);
+        cudaError_t e = launch_march<K2<T>>(g, k2_args<T>(g, w, H, ch, 1), cap);
         cudaGraph_t tmp = nullptr;
         if (cudaStreamEndCapture(cap, &tmp) != cudaSuccess || e != cudaSuccess) break;
         cudaGraphNode_t k2node;
@@ -802,7 +819,7 @@ int residual_step(int nx, int ny, int nz, double dx, double dy, double dz, const
         pad_copy_kernel<double, double><<<nb, 256, 0, c.st>>>(c.g, P, c.w.P, 1, c.w.link);
         force_go_kernel<<<1, 1, 0, c.st>>>(c.w.sc, 0.0);
         CondHandles ch{ 0, 0, 0 };
-        cudaError_t e = launch_march<K2<T>>(c.g, k2_args<T>(c.w, c.H, ch, 0), c.st);
+        cudaError_t e = launch_march<K2<T>>(c.g, k2_args<T>(c.g, c.w, c.H, ch, 0), c.st);
         pad_copy_kernel<T, T><<<nb, 256, 0, c.st>>>(c.g, c.w.r, r_out, 0, c.w.link);
         g_launches.fetch_add(3, std::memory_order_relaxed);
         if (e != cudaSuccess || cudaGetLastError() != cudaSuccess) rc = OMNI_ERR_CUDA;

@@ -23,11 +23,16 @@ struct Geom {
     int px;              // padded row pitch in cells (multiple of 8); cells nx..px-1 are permanently missing
     long long pplane;    // px * ny
     long long npad;      // px * ny * nz
-    // x-edge classes of an otherwise regular row (y, z neighbourhood complete): wcode of cells 0, 1, nx-2, nx-1.
-    // Groups whose codes are the interior code or these are NOT flagged: the fast path plus a per-lane correction
-    // (xedge_fix) covers them, so the box faces normal to x cost no divergent coded path in every warp.
-    uint32_t icode, stdc[4];
-    int xfix;            // 1 iff nx >= 4 (the four classes are distinct cells)
+    // Box faces never flag a group: a cell whose code equals the code it would have in a mask-free box is handled by the
+    // fast path plus additive per-axis corrections (x: per lane, y: per row, z: per plane; face_fix / xedge_fix).  A
+    // group is flagged only if a mask / NaN cell changes some code.  fix[a] = 1 iff axis a is long enough (n_a >= 4)
+    // for its four face classes (cells 0, 1, n-2, n-1) to be distinct cells; otherwise that axis' faces do flag.
+    uint32_t icode;
+    int fix[3];
+    int xfix;            // = fix[0]
+    // tile-plane flags for the K3/K4 tiles (tbx x tby cells): bit (k & 31) of tflags[(ty*ntx + tx)*twords + (k >> 5)]
+    // is set iff some group of tile (tx, ty) is flagged in plane k; unset bits let a warp skip the per-row flag word
+    int tbx, tby, ntx, nty, twords;
 };
 
 // stencil coefficients, already divided by A_tot (Eq. 10 :109), in the arithmetic type T
@@ -39,7 +44,7 @@ struct Coef {
     T cac[3];  // c_{a,(a+2)%3} / A_tot
     T hs[3];   // Delta_a * t_a / 2: face-average factor of the source term (Eq. 9 :100)
     T lut[3][32];      // lut[a][far | nb<<1 | nc<<3] = far*caa + nb*cab + nc*cac: weight of a coded link
-    T xc[4][6];        // xc[class][d] = t_a - w_d(stdc[class]): what the fast path over-subtracts at x-edge cells
+    T fc[3][4][6];     // fc[axis][class][d] = t_a(d) - w_d(face-class code): what the fast path over-subtracts there
     uint32_t icode;    // wcode of a fully interior cell of this geometry (2D: no z links)
 };
 
@@ -188,25 +193,49 @@ __device__ __forceinline__ void xfix_zero_after(T (&q)[V])
     for (int i = I + 1; i < V; ++i) q[i] = T(0);      // pad cells nx..px-1
 }
 
+// face class of position i on an axis of length n: 0, 1 (cells 0, 1), 2, 3 (cells n-2, n-1), -1 otherwise / axis off
+__device__ __forceinline__ int face_class(int i, int n, int on)
+{
+    if (!on) return -1;
+    if (i == 0) return 0;
+    if (i == 1) return 1;
+    if (i == n - 2) return 2;
+    if (i == n - 1) return 3;
+    return -1;
+}
+
+// whole-chunk correction for a row (y class) or plane (z class) next to a box face: uniform over the warp
+template <typename T, int V>
+__device__ __forceinline__ void face_fix(T (&q)[V], const T (&vm)[V], const T (&vc)[V], const T (&vp)[V],
+                                         const T (&vn)[V], const T (&vs)[V], T xl, T xr, const T (&c)[6])
+{
+#pragma unroll
+    for (int i = 0; i < V; ++i) {
+        const T w = (i == 0) ? xl : vc[i > 0 ? i - 1 : 0];
+        const T e = (i == V - 1) ? xr : vc[i < V - 1 ? i + 1 : V - 1];
+        q[i] += c[0] * e + c[1] * w + c[2] * vn[i] + c[3] * vs[i] + c[4] * vp[i] + c[5] * vm[i];
+    }
+}
+
 template <typename T, int V>
 __device__ __forceinline__ void xedge_fix(T (&q)[V], const T (&vm)[V], const T (&vc)[V], const T (&vp)[V],
                                           const T (&vn)[V], const T (&vs)[V], T xl, T xr, const XEdge& xe,
                                           const Coef<T>& K)
 {
     if (xe.L) {
-        xfix_cell<0, T, V>(q, vm, vc, vp, vn, vs, xl, xr, K.xc[0]);
-        xfix_cell<1, T, V>(q, vm, vc, vp, vn, vs, xl, xr, K.xc[1]);
+        xfix_cell<0, T, V>(q, vm, vc, vp, vn, vs, xl, xr, K.fc[0][0]);
+        xfix_cell<1, T, V>(q, vm, vc, vp, vn, vs, xl, xr, K.fc[0][1]);
     }
     if (xe.A) {
         switch (xe.posA) {
-#define OMNI_CASE(I) case I: if (I < V) xfix_cell<(I < V ? I : 0), T, V>(q, vm, vc, vp, vn, vs, xl, xr, K.xc[2]); break;
+#define OMNI_CASE(I) case I: if (I < V) xfix_cell<(I < V ? I : 0), T, V>(q, vm, vc, vp, vn, vs, xl, xr, K.fc[0][2]); break;
             OMNI_CASE(0) OMNI_CASE(1) OMNI_CASE(2) OMNI_CASE(3) OMNI_CASE(4) OMNI_CASE(5) OMNI_CASE(6) OMNI_CASE(7)
 #undef OMNI_CASE
         }
     }
     if (xe.B) {
         switch (xe.posB) {
-#define OMNI_CASE(I) case I: if (I < V) { xfix_cell<(I < V ? I : 0), T, V>(q, vm, vc, vp, vn, vs, xl, xr, K.xc[3]); \
+#define OMNI_CASE(I) case I: if (I < V) { xfix_cell<(I < V ? I : 0), T, V>(q, vm, vc, vp, vn, vs, xl, xr, K.fc[0][3]); \
                                           xfix_zero_after<(I < V ? I : 0), T, V>(q); } break;
             OMNI_CASE(0) OMNI_CASE(1) OMNI_CASE(2) OMNI_CASE(3) OMNI_CASE(4) OMNI_CASE(5) OMNI_CASE(6) OMNI_CASE(7)
 #undef OMNI_CASE
@@ -214,13 +243,14 @@ __device__ __forceinline__ void xedge_fix(T (&q)[V], const T (&vm)[V], const T (
     }
 }
 
-// q = M p for the V cells of one thread; fb = flag bits of the thread's 4-cell groups (0 = interior or regular
-// x-edge: fast path; else the chunk's codes are read and the cells that need it take the coded path)
+// q = M p for the V cells of one thread; fb = flag bit of the thread's 4-cell group (0 = interior or box face: fast
+// path + face corrections; else `code` holds the chunk's codes -- fetched a plane ahead by the caller -- and the
+// cells that need it take the coded path)
 template <typename T, int V>
 __device__ __forceinline__ void apply_M_chunk(T (&q)[V], const T (&vm)[V], const T (&vc)[V], const T (&vp)[V],
                                               const T (&vn)[V], const T (&vs)[V], T xl, T xr, uint32_t fb,
-                                              const uint32_t* __restrict__ wcode, long long idx, const Coef<T>& K,
-                                              const XEdge& xe)
+                                              const uint32_t (&code)[V], const Coef<T>& K,
+                                              const XEdge& xe, int ycls, int zcls)
 {
 #pragma unroll
     for (int i = 0; i < V; ++i) {
@@ -229,10 +259,10 @@ __device__ __forceinline__ void apply_M_chunk(T (&q)[V], const T (&vm)[V], const
         q[i] = apply_M_interior(vc[i], e, w, vn[i], vs[i], vp[i], vm[i], K);
     }
     if (fb == 0) {
-        if (xe.any) xedge_fix<T, V>(q, vm, vc, vp, vn, vs, xl, xr, xe, K);
+        if (ycls >= 0) face_fix<T, V>(q, vm, vc, vp, vn, vs, xl, xr, K.fc[1][ycls]);      // warp-uniform
+        if (zcls >= 0) face_fix<T, V>(q, vm, vc, vp, vn, vs, xl, xr, K.fc[2][zcls]);      // CTA-uniform
+        if (xe.any) xedge_fix<T, V>(q, vm, vc, vp, vn, vs, xl, xr, xe, K);               // last: zeroes the pad cells
     } else {
-        uint32_t code[V];
-        ld_chunk<uint32_t, V>(wcode + idx, code);
 #pragma unroll
         for (int i = 0; i < V; ++i) {
             T w = (i == 0) ? xl : vc[i - 1];
@@ -278,9 +308,43 @@ __device__ __forceinline__ int vget(const Geom& g, const uint8_t* __restrict__ v
     return v[i + (long long)g.px * (j + (long long)g.ny * k)];
 }
 
+// validity in the mask-free box, seen by the face corrections: axes whose faces are corrected (fix[a]) end at the box,
+// the others are treated as unbounded (their face cells then differ from this code and get flagged); an inactive z axis
+// (2D) has no neighbours at all
+__device__ __forceinline__ uint32_t vbox(const Geom& g, int i, int j, int k)
+{
+    if (g.fix[0] && (i < 0 || i >= g.nx)) return 0u;
+    if (g.fix[1] && (j < 0 || j >= g.ny)) return 0u;
+    if (g.nz == 1) return (k == 0) ? 1u : 0u;
+    if (g.fix[2] && (k < 0 || k >= g.nz)) return 0u;
+    return 1u;
+}
+__device__ __forceinline__ uint32_t box_code(const Geom& g, int i, int j, int k)
+{
+    if (i >= g.nx) return g.fix[0] ? 0u : g.icode;      // pad cells: expected only where xedge_fix zeroes them
+    if (!vbox(g, i, j, k)) return 0u;
+    const int naxes = (g.nz > 1) ? 3 : 2;
+    uint32_t code = WCODE_VALID;
+    for (int d = 0; d < 2 * naxes; ++d) {
+        const int a = d >> 1, sg = (d & 1) ? -1 : 1;
+        int e[3] = { 0, 0, 0 };
+        e[a] = sg;
+        const int qi = i + e[0], qj = j + e[1], qk = k + e[2];
+        if (!vbox(g, qi, qj, qk)) continue;
+        const int b = (a + 1) % 3, cc = (a + 2) % 3;
+        int eb[3] = { 0, 0, 0 }, ec[3] = { 0, 0, 0 };
+        eb[b] = 1; ec[cc] = 1;
+        const uint32_t far = vbox(g, qi + e[0], qj + e[1], qk + e[2]);
+        const uint32_t nb = vbox(g, qi + eb[0], qj + eb[1], qk + eb[2]) + vbox(g, qi - eb[0], qj - eb[1], qk - eb[2]);
+        const uint32_t nc = vbox(g, qi + ec[0], qj + ec[1], qk + ec[2]) + vbox(g, qi - ec[0], qj - ec[1], qk - ec[2]);
+        code |= (far | (nb << 1) | (nc << 3)) << (5 * d);
+    }
+    return code;
+}
+
 // one thread per 4-cell group; a warp's 32 groups fill exactly one flag word
 __global__ void codes_kernel(Geom g, const uint8_t* __restrict__ vbyte, uint8_t* __restrict__ link,
-                             uint32_t* __restrict__ wcode, uint32_t* __restrict__ flags)
+                             uint32_t* __restrict__ wcode, uint32_t* __restrict__ flags, uint32_t* __restrict__ tflags)
 {
     const long long grp = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     const long long ngrp = g.npad >> 2;
@@ -320,18 +384,15 @@ __global__ void codes_kernel(Geom g, const uint8_t* __restrict__ vbyte, uint8_t*
             }
             codes[c] = code;
             links |= lk << (8 * c);
-            uint32_t expect = g.icode;
-            if (g.xfix) {
-                if (i >= g.nx) expect = 0u;
-                else if (i == 0) expect = g.stdc[0];
-                else if (i == 1) expect = g.stdc[1];
-                else if (i == g.nx - 2) expect = g.stdc[2];
-                else if (i == g.nx - 1) expect = g.stdc[3];
-            }
+            const uint32_t expect = box_code(g, i, j, k);
             flagged |= (code != expect);
         }
         *reinterpret_cast<uint4*>(wcode + base) = make_uint4(codes[0], codes[1], codes[2], codes[3]);
         *reinterpret_cast<uint32_t*>(link + base) = links;
+        if (flagged) {
+            const int tile = (j / g.tby) * g.ntx + (i0 / g.tbx);
+            atomicOr(&tflags[(size_t)tile * g.twords + (k >> 5)], 1u << (k & 31));
+        }
     }
     const uint32_t word = __ballot_sync(0xffffffffu, flagged);
     if ((threadIdx.x & 31) == 0 && grp < ngrp) flags[grp >> 5] = word;

@@ -119,7 +119,7 @@ march_kernel(const Geom g, const int zlen, const typename Op::Args a)
     const uint32_t smem_s = (uint32_t)__cvta_generic_to_shared(smem);
 
     const typename Op::Ctx ctx(a);
-    const typename Op::TC tc = Op::thread_init(g, x);
+    const typename Op::TC tc = Op::thread_init(g, x, j);
 
     // event c consumes the main arrays of plane c and the extra arrays of plane c-1; its data sits in ring slot
     // (c - k0 + 1) % D.  Planes outside [0, nz) and the far side of the segment's halo planes are zero-filled.
@@ -171,7 +171,7 @@ march_kernel(const Geom g, const int zlen, const typename Op::Args a)
                 ld_chunk<VT, V>(&xch[buf][ty + 1][lane * V], vN);
                 ld_chunk<VT, V>(&xch[buf][ty - 1][lane * V], vS);
                 const uint32_t fb = (fw_cur >> (unsigned)((idx >> 2) & 31)) & ((1u << (V / 4)) - 1u);
-                Op::emit(a, ctx, idx, vm, vc, vn_, vN, vS, xl, xr, ex, fb, tc, acc);
+                Op::emit(a, ctx, idx, c - 1, vm, vc, vn_, vN, vS, xl, xr, ex, fb, tc, acc);
             }
             buf ^= 1;
         }
@@ -239,6 +239,7 @@ struct OpK2 {
         double* Pbuf[2]; const T* delta; const T* S; T* r; const uint8_t* link; const uint32_t* flags;
         double t[3]; Scalars* sc; double* partial; CondHandles cond;
         int fold_delta;   // 0: residual of P as given (omni_residual); 1: inside the solve
+        int nz, fixz;     // box faces normal to z are not flagged either: their links are cleared per plane
     };
     struct Ctx {
         const double* Pin; double* Pout;
@@ -247,7 +248,7 @@ struct OpK2 {
     struct Extra { T S[V]; };
     // thread constant: link bytes of an unflagged chunk (all six links, minus the box faces normal to x, pads invalid)
     using TC = uint32_t;
-    __device__ static TC thread_init(const Geom& g, int x)
+    __device__ static TC thread_init(const Geom& g, int x, int j)
     {
         uint32_t lk = 0;
 #pragma unroll
@@ -255,10 +256,14 @@ struct OpK2 {
             const int gi = x + i;
             uint32_t l = 0x7fu;
             if (g.nz == 1) l &= ~48u;
-            if (g.xfix) {
+            if (g.fix[0]) {
                 if (gi == 0) l &= ~2u;
                 if (gi == g.nx - 1) l &= ~1u;
                 if (gi >= g.nx) l = 0;
+            }
+            if (g.fix[1]) {                      // box faces normal to y (rows are not flagged for them)
+                if (j == 0) l &= ~8u;
+                if (j == g.ny - 1) l &= ~4u;
             }
             lk |= l << (8 * i);
         }
@@ -289,12 +294,16 @@ struct OpK2 {
         if (threadIdx.x == 31) hr = sr.template get_halo<double>(2) + (double)sr.template get_halo<T>(3);
         sr.template get<T, V>(2 + NPT, e.S);
     }
-    __device__ static void emit(const Args& a, const Ctx& c, long long idx, const double (&vm)[V], const double (&vc)[V],
+    __device__ static void emit(const Args& a, const Ctx& c, long long idx, int kp, const double (&vm)[V], const double (&vc)[V],
                                 const double (&vp)[V], const double (&vn)[V], const double (&vs)[V], double xl,
                                 double xr, const Extra& e, uint32_t fb, const TC& lk_const, double (&acc)[2])
     {
         if (a.fold_delta) st_chunk<double, V>(c.Pout + idx, vc);
         uint32_t lk = lk_const;
+        if (a.fixz) {
+            if (kp == 0) lk &= ~0x20202020u;
+            if (kp == a.nz - 1) lk &= ~0x10101010u;
+        }
         if (fb) lk = *reinterpret_cast<const uint32_t*>(a.link + idx);
         T rn[V];
 #pragma unroll

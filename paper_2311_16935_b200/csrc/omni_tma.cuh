@@ -11,6 +11,7 @@
 // The grid reduction at the end is the deterministic fixed-slot + last-CTA scheme of omni_march.cuh.
 #pragma once
 #include <cuda.h>
+#include <type_traits>
 #include "omni_march.cuh"
 
 namespace omni {
@@ -135,34 +136,72 @@ tma_kernel(const Geom g, const int zlen, const typename Op::Args a, const __grid
         const int x = x0 + lane * V, j = y0 + warp;
         const bool out = (x < g.nx) && (j < g.ny);      // chunks made only of pad cells (x >= nx) stay zero
         const typename Op::TC tc = Op::thread_init(g, x);
+        const int ycls = face_class(j, g.ny, g.fix[1]);  // rows next to the box faces normal to y (uniform per warp)
         const long long rowbase = (long long)j * g.px + x;
-        uint32_t fw_next = 0, fw_cur = 0;
-        // running state instead of per-event div/mod: slot of event e, its phase bit, the shared addresses of the
-        // stages of events e-2 / e-1 / e, the cell offset of plane c
-        int s = 0, sB = 0;
-        uint32_t phase = 0;
-        uint32_t aB = smem_s, aC = smem_s, aF = smem_s;
-        long long off = rowbase + (long long)(k0 - 1) * g.pplane;
-        typename Op::State st;
-        for (int e = 0; e < E; ++e) {
-            mbar_wait(bar_s + 8 * s, phase);
-            Op::advance(st, ctx, aF, warp, lane);
-            fw_cur = fw_next;
-            if (out && e >= 1 && e <= E - 2) fw_next = a.flags[(off >> 2) >> 5];      // plane c is emitted at event e+1
-            if (e >= 2) {                            // emit plane c-1 from stages e-2 (B), e-1 (centre), e (F)
-                const long long idx = off - g.pplane;
-                const uint32_t fb = (fw_cur >> (unsigned)((idx >> 2) & 31)) & 1u;
-                Op::emit(a, ctx, st, idx, aB, aC, aF, warp, lane, out, fb, tc, acc);
-                __syncwarp();
-                if (lane == 0) mbar_arrive(bar_s + 8 * (D + sB));
-                sB = (sB + 1 == D) ? 0 : sB + 1;
-            }
-            off += g.pplane;
-            aB = aC; aC = aF;
-            s = (s + 1 == D) ? 0 : s + 1;
-            phase ^= (s == 0);
-            aF = smem_s + (uint32_t)(s * Op::STAGE_BYTES);
+        // tile-plane flag bits (a group of this tile is flagged in plane k): a CTA whose planes are all clear -- every
+        // CTA of a mask-free box -- runs the CLEAN loop, compiled without the coded path, the flag words and their
+        // branches; only CTAs next to masked cells run the general loop
+        const uint32_t* tf = a.tflags + (size_t)(blockIdx.y * gridDim.x + blockIdx.x) * g.twords;
+        uint32_t anyf = 0;
+        for (int w = k0 >> 5; w <= (k1 - 1) >> 5; ++w) {
+            uint32_t m = tf[w];
+            if (w == (k0 >> 5)) m &= ~0u << (k0 & 31);
+            if (w == ((k1 - 1) >> 5)) m &= (2u << ((k1 - 1) & 31)) - 1u;
+            anyf |= m;
         }
+        auto run = [&](auto clean_tag) {
+            constexpr bool CLEAN = decltype(clean_tag)::value;
+            // running state instead of per-event div/mod: slot of event e, its phase bit, the shared addresses of
+            // the stages of events e-2 / e-1 / e, the cell offset of plane c
+            int s = 0, sB = 0;
+            uint32_t phase = 0;
+            uint32_t aB = smem_s, aC = smem_s, aF = smem_s;
+            long long off = rowbase + (long long)(k0 - 1) * g.pplane;
+            typename Op::State st;
+            // general loop only: the row's flag words of the planes kp, kp+1 (and kp+2, fetched now) and the chunk's
+            // stencil codes of planes kp and kp+1 -- every global load is issued at least one plane before its use
+            uint32_t fwA = 0, fwB = 0, codeA[V], codeB[V];
+#pragma unroll
+            for (int i = 0; i < V; ++i) codeA[i] = codeB[i] = 0u;
+            auto flag_word = [&](long long cell) { return a.flags[(cell >> 2) >> 5]; };
+            auto flag_bit = [&](uint32_t w, long long cell) { return (w >> (unsigned)((cell >> 2) & 31)) & 1u; };
+            if (!CLEAN && out) {
+                const long long c0 = rowbase + (long long)k0 * g.pplane;
+                fwA = flag_word(c0);
+                if (k0 + 1 < k1) fwB = flag_word(c0 + g.pplane);
+                if (flag_bit(fwA, c0)) ld_chunk<uint32_t, V>(a.wcode + c0, codeA);
+            }
+            for (int e = 0; e < E; ++e) {
+                mbar_wait(bar_s + 8 * s, phase);
+                Op::advance(st, ctx, aF, warp, lane);
+                if (e >= 2) {                        // emit plane c-1 from stages e-2 (B), e-1 (centre), e (F)
+                    const int kp = k0 + e - 2;       // the plane being emitted
+                    const int zcls = face_class(kp, g.nz, g.fix[2]);
+                    const long long idx = off - g.pplane;
+                    uint32_t fb = 0, fwC = 0;
+                    if (!CLEAN && out) {
+                        fb = flag_bit(fwA, idx);
+                        if (kp + 2 < k1) fwC = flag_word(idx + 2 * g.pplane);
+                        if (kp + 1 < k1 && flag_bit(fwB, off)) ld_chunk<uint32_t, V>(a.wcode + off, codeB);
+                    }
+                    Op::template emit<CLEAN>(a, ctx, st, idx, aB, aC, aF, warp, lane, out, fb, codeA, tc, ycls, zcls, acc);
+                    if (!CLEAN) {
+                        fwA = fwB; fwB = fwC;
+#pragma unroll
+                        for (int i = 0; i < V; ++i) codeA[i] = codeB[i];
+                    }
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive(bar_s + 8 * (D + sB));
+                    sB = (sB + 1 == D) ? 0 : sB + 1;
+                }
+                off += g.pplane;
+                aB = aC; aC = aF;
+                s = (s + 1 == D) ? 0 : s + 1;
+                phase ^= (s == 0);
+                aF = smem_s + (uint32_t)(s * Op::STAGE_BYTES);
+            }
+        };
+        if (anyf) run(std::false_type{}); else run(std::true_type{});
     }
 
     // deterministic grid reduction (all warps, the producer contributes 0)
@@ -209,7 +248,7 @@ struct OpT3 {
     enum { V = TG::V, D = D_, MINB = MINB_, TICKET = 0, STAGE_BYTES = 2 * TG::TILE_H,
            BOX_H = (BY_ + 2) * TG::PITCH_H };
     struct Args {
-        T* pbuf[2]; const uint32_t* wcode; const uint32_t* flags;
+        T* pbuf[2]; const uint32_t* wcode; const uint32_t* flags; const uint32_t* tflags;
         Coef<T> K; Scalars* sc; double* partial; CondHandles cond;
     };
     struct Ctx {
@@ -248,8 +287,10 @@ struct OpT3 {
         for (int i = 0; i < V; ++i) { st.m[i] = st.c[i]; st.c[i] = st.f[i]; }
         pnew_chunk(sF, off, c.beta, st.f);
     }
+    template <bool CLEAN>
     __device__ static void emit(const Args& a, const Ctx& c, const State& st, long long idx, uint32_t, uint32_t sC, uint32_t,
-                                int warp, int lane, bool out, uint32_t fb, const TC& xe, double& acc)
+                                int warp, int lane, bool out, uint32_t fb, const uint32_t (&code)[V], const TC& xe, int ycls, int zcls,
+                                double& acc)
     {
         const int row = (warp + 1) * TG::PITCH_H;
         const int off = row + (TG::HX + lane * V) * (int)sizeof(T);
@@ -270,7 +311,7 @@ struct OpT3 {
         if (!out) return;
         st_chunk<T, V>(c.pnew + idx, vc);
         T q[V];
-        apply_M_chunk<T, V>(q, vm, vc, vp, vn, vs, xl, xr, fb, a.wcode, idx, a.K, xe);
+        apply_M_chunk<T, V>(q, vm, vc, vp, vn, vs, xl, xr, CLEAN ? 0u : fb, code, a.K, xe, ycls, zcls);
 #pragma unroll
         for (int i = 0; i < V; ++i) acc += (double)vc[i] * (double)q[i];
     }
@@ -298,7 +339,7 @@ struct OpT4 {
            BOX_H = (BY_ + 2) * TG::PITCH_H };
     struct Args {
         T* r; T* delta; int p_fixed;      // p_fixed >= 0: read p from pbuf[p_fixed] (omni_apply_M), else by parity
-        const uint32_t* wcode; const uint32_t* flags;
+        const uint32_t* wcode; const uint32_t* flags; const uint32_t* tflags;
         Coef<T> K; Scalars* sc; double* partial; CondHandles cond;
         T* q_out;                         // only for omni_apply_M: store q, leave r / delta untouched
     };
@@ -327,8 +368,10 @@ struct OpT4 {
     }
     struct State {};
     __device__ static void advance(State&, const Ctx&, uint32_t, int, int) {}
+    template <bool CLEAN>
     __device__ static void emit(const Args& a, const Ctx& c, const State&, long long idx, uint32_t sB, uint32_t sC, uint32_t sF,
-                                int warp, int lane, bool out, uint32_t fb, const TC& xe, double& acc)
+                                int warp, int lane, bool out, uint32_t fb, const uint32_t (&code)[V], const TC& xe, int ycls, int zcls,
+                                double& acc)
     {
         const int row = (warp + 1) * TG::PITCH_H;
         const int off = row + (TG::HX + lane * V) * (int)sizeof(T);
@@ -346,7 +389,7 @@ struct OpT4 {
         if (lane == 31) xr = hr;
         if (!out) return;
         T q[V];
-        apply_M_chunk<T, V>(q, vm, vc, vp, vn, vs, xl, xr, fb, a.wcode, idx, a.K, xe);
+        apply_M_chunk<T, V>(q, vm, vc, vp, vn, vs, xl, xr, CLEAN ? 0u : fb, code, a.K, xe, ycls, zcls);
         if (a.q_out != nullptr) {
             st_chunk<T, V>(a.q_out + idx, q);
 #pragma unroll
