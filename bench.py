@@ -29,7 +29,7 @@ UNIT = "grid-point CG updates/s"
 CPU_SAMPLE_EDGE = 200                   # 3D: edge of the corner crop the oracle is timed on (2D: the whole grid)
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel (K4) from the ncu --set full capture
 # summarised in profiles/r1_ncu_k3_k4_500cube_f32.md; only valid for that workload.
-NCU_TRAFFIC_K4 = {(4, "f32"): 1.537037e9 + 0.957180e9}
+NCU_TRAFFIC_K4 = {(4, "f32"): 1.526446e9 + 0.955657e9}
 
 
 def parse():

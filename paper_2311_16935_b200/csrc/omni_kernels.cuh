@@ -384,7 +384,9 @@ __global__ void codes_kernel(Geom g, const uint8_t* __restrict__ vbyte, uint8_t*
             }
             codes[c] = code;
             links |= lk << (8 * c);
-            const uint32_t expect = box_code(g, i, j, k);
+            // two or more cells away from every face the mask-free box code is the interior code
+            const bool deep = (i >= 2 && i < g.nx - 2) && (j >= 2 && j < g.ny - 2) && (g.nz == 1 || (k >= 2 && k < g.nz - 2));
+            const uint32_t expect = deep ? g.icode : box_code(g, i, j, k);
             flagged |= (code != expect);
         }
         *reinterpret_cast<uint4*>(wcode + base) = make_uint4(codes[0], codes[1], codes[2], codes[3]);
