@@ -115,6 +115,33 @@ def test_trajectory_parity(oracle, dtype, kind, shape, frac):
     assert info["eps_R_final"] == pytest.approx(io["eps_R_final"], rel=2e-3 if dtype == "f32" else 1e-7)
 
 
+SMALL = [(4, 4, 4), (5, 4, 9), (3, 7, 12), (2, 6, 10), (4, 9), (3, 5), (2, 2), (6, 1, 7), (1, 1, 9), (7, 5, 4), (9, 4, 5)]
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("shape", SMALL)
+def test_small_and_thin_grids(oracle, dtype, shape):
+    """Axes of length 1..5: every cell is a face / edge / corner cell, the per-axis face corrections overlap, and
+    axes shorter than 4 fall back to flagged groups (coded path).  With and without a masked cell."""
+    rng = np.random.default_rng(sum(shape))
+    g = [rng.normal(size=shape) for _ in range(len(shape))]
+    f = dict(g=g, mask=None, d=tuple(0.3 + 0.2 * a for a in range(3)))
+    for with_mask in (False, True):
+        mask = None
+        if with_mask:
+            mask = np.ones(shape, np.uint8)
+            mask[tuple(s // 2 for s in shape)] = 0
+            if mask.sum() == 0:
+                continue
+        P, info, Po, io = _solve_both(oracle, f, dtype, 0.0, 4, 6, mask)
+        valid = ~np.isnan(Po)
+        assert np.array_equal(np.isnan(P), ~valid)
+        assert info["cg_iters_total"] == io["cg_iters_total"]
+        if valid.sum() > 1 and np.nanmax(np.abs(Po)) > 0:
+            Pz, Poz = np.nan_to_num(P), np.nan_to_num(Po)
+            assert np.abs(Pz - Poz).max() <= (1e-10 if dtype == "f64" else 2e-4) * np.abs(Poz).max(), (shape, with_mask)
+
+
 def test_converged_parity_config0(oracle):
     """BASELINE configs[0]: 64^2 fp64, tol 1e-8, converged on both sides with the same stopping rules; and the
     recovered field matches the analytic P up to a constant at the discretisation + noise level."""
