@@ -1,4 +1,4 @@
-// omni_api.cu -- C ABI (include/omni.h) over the kernels of omni_kernels.cuh.
+// omni_api.cu -- C ABI (include/omni.h) over the kernels of omni_kernels.cuh and omni_tma.cuh.
 // Host logic only: argument validation, geometry constants (a0), workspace carving, launch configuration and the
 // loop driver (CUDA graph with device-side conditional WHILE nodes, or a host-driven debug loop).
 #include "omni_tma.cuh"
@@ -261,58 +261,11 @@ __global__ void init_scalars_kernel(Scalars* sc, double tol, int max_outer, int 
 
 struct MarchCfg { dim3 grid, block; int zlen; };
 
-// z segments: minimise (waves) x (planes per CTA incl. the two halo planes)
-template <class Op>
-MarchCfg march_config(const Geom& g)
-{
-    constexpr int W = 32 * Op::V, TYO = Op::TYR - 2;
-    static int slots_cache = 0;
-    if (slots_cache == 0) {
-        int dev = 0, sms = 148, occ = 1;
-        cudaGetDevice(&dev);
-        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-        cudaFuncSetAttribute(march_kernel<Op>, cudaFuncAttributeMaxDynamicSharedMemorySize, MarchSmem<Op>::TOTAL);
-        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, march_kernel<Op>, 32 * Op::TYR, MarchSmem<Op>::TOTAL);
-        if (occ < 1) occ = 1;
-        slots_cache = sms * occ;
-    }
-    const int slots = slots_cache;
-    const int ntx = (g.px + W - 1) / W, nty = (g.ny + TYO - 1) / TYO;
-    const long long tiles = (long long)ntx * nty;
-    int best = 1;
-    double best_cost = 1e300;
-    const int max_seg = g.nz;
-    for (int ns = 1; ns <= max_seg; ns = (ns < 16 ? ns + 1 : ns + ns / 8)) {
-        const int zlen = (g.nz + ns - 1) / ns;
-        const int nseg = (g.nz + zlen - 1) / zlen;
-        const long long ctas = tiles * nseg;
-        const long long waves = (ctas + slots - 1) / slots;
-        const double cost = (double)waves * (zlen + (nseg > 1 ? 2 : 0) + 3);   // +3: per-CTA prologue/epilogue
-        if (cost < best_cost) { best_cost = cost; best = nseg; }
-        if (zlen <= 4) break;
-    }
-    MarchCfg c;
-    c.zlen = (g.nz + best - 1) / best;
-    const int nseg = (g.nz + c.zlen - 1) / c.zlen;
-    c.grid = dim3(ntx, nty, nseg);
-    c.block = dim3(32, Op::TYR, 1);
-    return c;
-}
-
-template <class Op>
-cudaError_t launch_march(const Geom& g, const typename Op::Args& a, cudaStream_t st)
-{
-    const MarchCfg c = march_config<Op>(g);
-    march_kernel<Op><<<c.grid, c.block, MarchSmem<Op>::TOTAL, st>>>(g, c.zlen, a);
-    g_launches.fetch_add(1, std::memory_order_relaxed);
-    return cudaGetLastError();
-}
-
-// K3 / K4: TMA + mbarrier pipeline (omni_tma.cuh): 512-byte x 8-row tiles, 8 consumer warps + 1 producer warp,
-// several CTAs per SM (shared memory: K3 6 stages x 10.8 KB, K4 5 stages x 13.4 KB).  K2: cp.async engine.
+// K2 / K3 / K4: TMA + mbarrier pipeline (omni_tma.cuh): 512-byte x 8-row tiles, 8 consumer warps + 1 producer warp,
+// several CTAs per SM (shared memory: K3 6 stages x 10.8 KB, K4 5 x 13.4 KB, K2 5 x 10.3 KB fp32 / 4 x 14.8 KB fp64).
 template <typename T> using K3 = OpT3<T, OMNI_BY, OMNI_D3, OMNI_MINB>;
 template <typename T> using K4 = OpT4<T, OMNI_BY, OMNI_D4, (sizeof(T) == 8 ? 2 : OMNI_MINB)>;   // fp64 K4: 72 registers spill
-template <typename T> using K2 = OpK2<T, 16, 3, 1>;
+template <typename T> using K2 = OpT2<T, OMNI_BY, (sizeof(T) == 8 ? 4 : 5), OMNI_MINB>;
 
 
 template <class Op>
@@ -413,6 +366,7 @@ int setup_codes(const Geom& g, const Workspace<T>& w, const T* gx, const T* gy, 
     CK(cudaMemsetAsync(w.p0, 0, n * sizeof(T), st));
     CK(cudaMemsetAsync(w.p1, 0, n * sizeof(T), st));
     CK(cudaMemsetAsync(w.delta, 0, n * sizeof(T), st));
+    CK(cudaMemsetAsync(w.r, 0, n * sizeof(T), st));          // pad cells of r are never written afterwards
     CK(cudaMemsetAsync(w.P, 0, n * sizeof(double), st));
     CK(cudaMemsetAsync(w.P1, 0, n * sizeof(double), st));
     return OMNI_OK;
@@ -431,11 +385,11 @@ int launch_source(const Geom& g, const Workspace<T>& w, const Coef<T>& K, const 
 template <typename T>
 typename K2<T>::Args k2_args(const Geom& g, const Workspace<T>& w, const HostConst& H, CondHandles ch, int fold)
 {
+    (void)g;
     typename K2<T>::Args a;
-    a.Pbuf[0] = w.P; a.Pbuf[1] = fold ? w.P1 : w.P; a.delta = w.delta; a.S = w.S; a.r = w.r; a.link = w.link; a.flags = w.flags;
+    a.Pbuf[0] = w.P; a.Pbuf[1] = fold ? w.P1 : w.P; a.r = w.r; a.link = w.link; a.flags = w.flags; a.tflags = w.tflags;
     for (int i = 0; i < 3; ++i) a.t[i] = H.F[i] / H.Atot;
     a.sc = w.sc; a.partial = w.partial; a.cond = ch; a.fold_delta = fold;
-    a.nz = g.nz; a.fixz = g.fix[2];
     return a;
 }
 template <typename T>
@@ -461,7 +415,10 @@ bool make_tma_set(const Geom& g, const Workspace<T>& w, TmaSet& m)
     const int hx = TG::BX + 2 * TG::HX, hy = TG::BY + 2;
     return encode_map<T>(&m.r_h, g, w.r, hx, hy) && encode_map<T>(&m.p_h[0], g, w.p0, hx, hy) &&
            encode_map<T>(&m.p_h[1], g, w.p1, hx, hy) && encode_map<T>(&m.r_c, g, w.r, TG::BX, TG::BY) &&
-           encode_map<T>(&m.d_c, g, w.delta, TG::BX, TG::BY);
+           encode_map<T>(&m.d_c, g, w.delta, TG::BX, TG::BY) &&
+           encode_map<double>(&m.P_h[0], g, w.P, 64 + 4, TG::BY + 2) && encode_map<double>(&m.P_h[1], g, w.P1, 64 + 4, TG::BY + 2) &&
+           encode_map<T>(&m.d2_h, g, w.delta, 64 + 2 * (16 / (int)sizeof(T)), TG::BY + 2) &&
+           encode_map<T>(&m.S_c, g, w.S, 64, TG::BY);
 }
 
 // ------------------------------------------------------------------------------------------------ loop drivers
@@ -498,7 +455,7 @@ int run_loop_host(const Geom& g, const Workspace<T>& w, const HostConst& H, cons
     int rc = OMNI_OK;
     long long executed_k34 = 0, seen_cg = 0;
     for (long long it = 0; it <= (long long)max_outer && rc == OMNI_OK; ++it) {
-        if (timed(0, [&] { return launch_march<K2<T>>(g, a2, st); }) != cudaSuccess) { rc = OMNI_ERR_CUDA; break; }
+        if (timed(0, [&] { return launch_tma<K2<T>>(g, a2, maps, st); }) != cudaSuccess) { rc = OMNI_ERR_CUDA; break; }
         int done = 0;
         bool synced = false;
         while (done < max_cg) {
@@ -551,7 +508,7 @@ int run_loop_graph(const Geom& g, const Workspace<T>& w, const HostConst& H, con
     cudaStream_t cap = nullptr;
     int rc = OMNI_ERR_CUDA;
     // occupancy queries happen here, outside any stream capture (results are cached per kernel)
-    (void)march_config<K2<T>>(g); (void)tma_config<K3<T>>(g); (void)tma_config<K4<T>>(g);
+    (void)tma_config<K2<T>>(g); (void)tma_config<K3<T>>(g); (void)tma_config<K4<T>>(g);
     TmaSet maps;
     if (!make_tma_set<T>(g, w, maps)) return OMNI_ERR_CUDA;
     do {
@@ -573,7 +530,7 @@ int run_loop_graph(const Geom& g, const Workspace<T>& w, const HostConst& H, con
         if (cudaStreamCreateWithFlags(&cap, cudaStreamNonBlocking) != cudaSuccess) break;
         // K2 into the outer body
         if (cudaStreamBeginCaptureToGraph(cap, bodyOuter, nullptr, nullptr, 0, cudaStreamCaptureModeThreadLocal) != cudaSuccess) break;
-        cudaError_t e = launch_march<K2<T>>(g, k2_args<T>(g, w, H, ch, 1), cap);
+        cudaError_t e = launch_tma<K2<T>>(g, k2_args<T>(g, w, H, ch, 1), maps, cap);
         cudaGraph_t tmp = nullptr;
         if (cudaStreamEndCapture(cap, &tmp) != cudaSuccess || e != cudaSuccess) break;
         cudaGraphNode_t k2node;
@@ -819,7 +776,8 @@ int residual_step(int nx, int ny, int nz, double dx, double dy, double dz, const
         pad_copy_kernel<double, double><<<nb, 256, 0, c.st>>>(c.g, P, c.w.P, 1, c.w.link);
         force_go_kernel<<<1, 1, 0, c.st>>>(c.w.sc, 0.0);
         CondHandles ch{ 0, 0, 0 };
-        cudaError_t e = launch_march<K2<T>>(c.g, k2_args<T>(c.g, c.w, c.H, ch, 0), c.st);
+        TmaSet maps;
+        cudaError_t e = make_tma_set<T>(c.g, c.w, maps) ? launch_tma<K2<T>>(c.g, k2_args<T>(c.g, c.w, c.H, ch, 0), maps, c.st) : cudaErrorUnknown;
         pad_copy_kernel<T, T><<<nb, 256, 0, c.st>>>(c.g, c.w.r, r_out, 0, c.w.link);
         g_launches.fetch_add(3, std::memory_order_relaxed);
         if (e != cudaSuccess || cudaGetLastError() != cudaSuccess) rc = OMNI_ERR_CUDA;

@@ -7,10 +7,8 @@
 //   K3  p = r + beta p (fused), gamma = p . M p                (CG, :124)
 //   K4  q = M p recomputed, delta += alpha p, r -= alpha q, rho' = r.r
 //   K7  P_out with NaN at missing cells                        (:158)
-// K2/K3/K4 share one z-marching tile engine (march_kernel): a CTA owns a (32*V cells) x (TYR-2 rows) column of the
-// grid, streams it plane by plane with a register pipeline (planes k-1, k, k+1), exchanges the current plane's y
-// neighbours through shared memory and its x neighbours by warp shuffles, and finishes with a deterministic
-// grid-wide reduction (fixed-slot partials + last-arriving CTA) whose scalars stay on the device.
+// K2/K3/K4 run on the TMA + mbarrier tile pipeline of omni_tma.cuh; this header holds the shared device helpers
+// (geometry, coefficient tables, operator evaluation, face corrections) and the one-off kernels K0, K1, K7.
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>

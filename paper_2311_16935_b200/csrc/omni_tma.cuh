@@ -1,4 +1,4 @@
-// omni_tma.cuh -- K3 / K4 on a TMA + mbarrier producer/consumer pipeline (sm_100a).
+// omni_tma.cuh -- K2 / K3 / K4 on a TMA + mbarrier producer/consumer pipeline (sm_100a).
 //
 // A CTA owns a column of the grid: BX = 32*V cells (512 bytes) x BY rows x zlen planes.  One producer warp issues,
 // per plane, a few cp.async.bulk.tensor (TMA) box loads -- the tile of every streamed array, the stencil input with
@@ -8,13 +8,25 @@
 // c-1 and the own chunk of planes c-2 and c from the three resident stages (x neighbours by shuffle), evaluate the
 // operator, store, and release the oldest stage through its "empty" mbarrier.  Warps only ever wait for data, never
 // for each other: there is no CTA-wide barrier in the loop and no state carried in registers across planes.
-// The grid reduction at the end is the deterministic fixed-slot + last-CTA scheme of omni_march.cuh.
+// The grid reduction at the end is deterministic: fp64 per-thread partials -> warp shuffle -> CTA -> fixed slot; the
+// last-arriving CTA (atomic ticket) adds the slots in slot order and updates the device-resident loop scalars.
 #pragma once
 #include <cuda.h>
 #include <type_traits>
-#include "omni_march.cuh"
+#include "omni_kernels.cuh"
 
 namespace omni {
+
+// loop conditions of the CUDA-graph WHILE nodes, written by a kernel's last CTA (no-op outside the graph)
+__device__ __forceinline__ void set_cond(const CondHandles& h, int outer, int inner)
+{
+#if defined(__CUDA_ARCH__)
+    if (h.use) {
+        if (outer >= 0) cudaGraphSetConditional((cudaGraphConditionalHandle)h.h_outer, (unsigned)outer);
+        if (inner >= 0) cudaGraphSetConditional((cudaGraphConditionalHandle)h.h_inner, (unsigned)inner);
+    }
+#endif
+}
 
 // ------------------------------------------------------------------------------------------------ PTX wrappers
 __device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count)
@@ -45,6 +57,9 @@ __device__ __forceinline__ void tma_load_3d(uint32_t dst, const CUtensorMap* map
 struct alignas(64) TmaSet {
     CUtensorMap r_h, p_h[2];     // boxes with halo: (BX + 2 HX) x (BY + 2) x 1
     CUtensorMap r_c, d_c;        // plain boxes: BX x BY x 1
+    // K2 (64-cell tiles: the fp64 master pressure sets the 16-byte lane chunk)
+    CUtensorMap P_h[2], d2_h;    // haloed: P (fp64, both buffers), delta (T)
+    CUtensorMap S_c;             // plain: S (T)
 };
 
 template <typename T, int BY_>
@@ -88,9 +103,9 @@ tma_kernel(const Geom g, const int zlen, const typename Op::Args a, const __grid
 {
     using TG = typename Op::TG;
     using T = typename Op::VT;
-    constexpr int V = TG::V, BX = TG::BX, BY = TG::BY, D = Op::D, NACC = 1;
+    constexpr int V = TG::V, BX = TG::BX, BY = TG::BY, D = Op::D, NACC = Op::NACC;
     extern __shared__ __align__(128) char smem_raw[];
-    __shared__ double red[BY + 1];
+    __shared__ double red[NACC][BY + 1];
     __shared__ int is_last;
     __shared__ __align__(8) unsigned long long bars[2 * D];
 
@@ -116,7 +131,9 @@ tma_kernel(const Geom g, const int zlen, const typename Op::Args a, const __grid
     }
     __syncthreads();
 
-    double acc = 0.0;
+    double acc[NACC];
+#pragma unroll
+    for (int i = 0; i < NACC; ++i) acc[i] = 0.0;
     if (warp == BY) {
         // ---------------------------------------------------------------- producer warp (one elected lane)
         if (lane == 0) {
@@ -141,7 +158,7 @@ tma_kernel(const Geom g, const int zlen, const typename Op::Args a, const __grid
         // tile-plane flag bits (a group of this tile is flagged in plane k): a CTA whose planes are all clear -- every
         // CTA of a mask-free box -- runs the CLEAN loop, compiled without the coded path, the flag words and their
         // branches; only CTAs next to masked cells run the general loop
-        const uint32_t* tf = a.tflags + (size_t)(blockIdx.y * gridDim.x + blockIdx.x) * g.twords;
+        const uint32_t* tf = a.tflags + (size_t)(blockIdx.y * g.ntx + x0 / g.tbx) * g.twords;
         uint32_t anyf = 0;
         for (int w = k0 >> 5; w <= (k1 - 1) >> 5; ++w) {
             uint32_t m = tf[w];
@@ -169,7 +186,7 @@ tma_kernel(const Geom g, const int zlen, const typename Op::Args a, const __grid
                 const long long c0 = rowbase + (long long)k0 * g.pplane;
                 fwA = flag_word(c0);
                 if (k0 + 1 < k1) fwB = flag_word(c0 + g.pplane);
-                if (flag_bit(fwA, c0)) ld_chunk<uint32_t, V>(a.wcode + c0, codeA);
+                if (flag_bit(fwA, c0)) Op::load_codes(a, c0, codeA);
             }
             for (int e = 0; e < E; ++e) {
                 mbar_wait(bar_s + 8 * s, phase);
@@ -182,7 +199,7 @@ tma_kernel(const Geom g, const int zlen, const typename Op::Args a, const __grid
                     if (!CLEAN && out) {
                         fb = flag_bit(fwA, idx);
                         if (kp + 2 < k1) fwC = flag_word(idx + 2 * g.pplane);
-                        if (kp + 1 < k1 && flag_bit(fwB, off)) ld_chunk<uint32_t, V>(a.wcode + off, codeB);
+                        if (kp + 1 < k1 && flag_bit(fwB, off)) Op::load_codes(a, off, codeB);
                     }
                     Op::template emit<CLEAN>(a, ctx, st, idx, aB, aC, aF, warp, lane, out, fb, codeA, tc, ycls, zcls, acc);
                     if (!CLEAN) {
@@ -207,15 +224,19 @@ tma_kernel(const Geom g, const int zlen, const typename Op::Args a, const __grid
     // deterministic grid reduction (all warps, the producer contributes 0)
     const unsigned int nblk = gridDim.x * gridDim.y * gridDim.z;
     const unsigned int bid = blockIdx.x + gridDim.x * (blockIdx.y + gridDim.y * blockIdx.z);
-    {
-        double sacc = warp_sum(acc);
-        if (lane == 0) red[warp] = sacc;
+#pragma unroll
+    for (int i = 0; i < NACC; ++i) {
+        double sacc = warp_sum(acc[i]);
+        if (lane == 0) red[i][warp] = sacc;
     }
     __syncthreads();
     if (threadIdx.x == 0) {
-        double s = 0.0;
-        for (int w = 0; w < BY; ++w) s += red[w];
-        a.partial[bid] = s;
+#pragma unroll
+        for (int i = 0; i < NACC; ++i) {
+            double s = 0.0;
+            for (int w = 0; w < BY; ++w) s += red[i][w];
+            a.partial[(size_t)i * nblk + bid] = s;
+        }
         __threadfence();
         unsigned int t = atomicAdd(&a.sc->ticket[Op::TICKET], 1u);
         is_last = (t == nblk - 1);
@@ -223,15 +244,20 @@ tma_kernel(const Geom g, const int zlen, const typename Op::Args a, const __grid
     __syncthreads();
     if (is_last) {
         __threadfence();
-        double s = 0.0;
-        for (unsigned int b = threadIdx.x; b < nblk; b += TG::NTHR) s += __ldcg(&a.partial[b]);
-        s = warp_sum(s);
-        __syncthreads();
-        if (lane == 0) red[warp] = s;
-        __syncthreads();
+        double tot[NACC];
+#pragma unroll
+        for (int i = 0; i < NACC; ++i) {
+            double s = 0.0;
+            for (unsigned int b = threadIdx.x; b < nblk; b += TG::NTHR) s += __ldcg(&a.partial[(size_t)i * nblk + b]);
+            s = warp_sum(s);
+            __syncthreads();
+            if (lane == 0) red[i][warp] = s;
+            __syncthreads();
+            s = 0.0;
+            for (int w = 0; w <= BY; ++w) s += red[i][w];
+            tot[i] = s;
+        }
         if (threadIdx.x == 0) {
-            double tot[NACC] = { 0.0 };
-            for (int w = 0; w <= BY; ++w) tot[0] += red[w];
             a.sc->ticket[Op::TICKET] = 0;
             Op::finalize(a, tot);
         }
@@ -245,7 +271,7 @@ template <typename T, int BY_, int D_, int MINB_>
 struct OpT3 {
     using VT = T;
     using TG = TileGeom<T, BY_>;
-    enum { V = TG::V, D = D_, MINB = MINB_, TICKET = 0, STAGE_BYTES = 2 * TG::TILE_H,
+    enum { V = TG::V, D = D_, MINB = MINB_, NACC = 1, TICKET = 0, STAGE_BYTES = 2 * TG::TILE_H,
            BOX_H = (BY_ + 2) * TG::PITCH_H };
     struct Args {
         T* pbuf[2]; const uint32_t* wcode; const uint32_t* flags; const uint32_t* tflags;
@@ -259,6 +285,7 @@ struct OpT3 {
     __device__ static TC thread_init(const Geom& g, int x) { return make_xedge<V>(g, x); }
     __device__ static bool active(const Args& a) { return a.sc->inner_go != 0; }
     __device__ static void idle(const Args& a) { set_cond(a.cond, -1, 0); }
+    __device__ static void load_codes(const Args& a, long long cell, uint32_t (&code)[V]) { ld_chunk<uint32_t, V>(a.wcode + cell, code); }
     __device__ static void produce(const Args&, const Ctx& c, const TmaSet& m, uint32_t stage, uint32_t bar, int x0, int y0,
                                    int plane, bool)
     {
@@ -290,8 +317,9 @@ struct OpT3 {
     template <bool CLEAN>
     __device__ static void emit(const Args& a, const Ctx& c, const State& st, long long idx, uint32_t, uint32_t sC, uint32_t,
                                 int warp, int lane, bool out, uint32_t fb, const uint32_t (&code)[V], const TC& xe, int ycls, int zcls,
-                                double& acc)
+                                double (&accs)[1])
     {
+        double& acc = accs[0];
         const int row = (warp + 1) * TG::PITCH_H;
         const int off = row + (TG::HX + lane * V) * (int)sizeof(T);
         T vn[V], vs[V];
@@ -335,7 +363,7 @@ template <typename T, int BY_, int D_, int MINB_>
 struct OpT4 {
     using VT = T;
     using TG = TileGeom<T, BY_>;
-    enum { V = TG::V, D = D_, MINB = MINB_, TICKET = 1, STAGE_BYTES = TG::TILE_H + 2 * TG::TILE_C,
+    enum { V = TG::V, D = D_, MINB = MINB_, NACC = 1, TICKET = 1, STAGE_BYTES = TG::TILE_H + 2 * TG::TILE_C,
            BOX_H = (BY_ + 2) * TG::PITCH_H };
     struct Args {
         T* r; T* delta; int p_fixed;      // p_fixed >= 0: read p from pbuf[p_fixed] (omni_apply_M), else by parity
@@ -356,6 +384,7 @@ struct OpT4 {
     __device__ static TC thread_init(const Geom& g, int x) { return make_xedge<V>(g, x); }
     __device__ static bool active(const Args& a) { return a.sc->inner_go != 0; }
     __device__ static void idle(const Args& a) { set_cond(a.cond, -1, 0); }
+    __device__ static void load_codes(const Args& a, long long cell, uint32_t (&code)[V]) { ld_chunk<uint32_t, V>(a.wcode + cell, code); }
     __device__ static void produce(const Args& a, const Ctx& c, const TmaSet& m, uint32_t stage, uint32_t bar, int x0,
                                    int y0, int plane, bool inner)
     {
@@ -371,8 +400,9 @@ struct OpT4 {
     template <bool CLEAN>
     __device__ static void emit(const Args& a, const Ctx& c, const State&, long long idx, uint32_t sB, uint32_t sC, uint32_t sF,
                                 int warp, int lane, bool out, uint32_t fb, const uint32_t (&code)[V], const TC& xe, int ycls, int zcls,
-                                double& acc)
+                                double (&accs)[1])
     {
+        double& acc = accs[0];
         const int row = (warp + 1) * TG::PITCH_H;
         const int off = row + (TG::HX + lane * V) * (int)sizeof(T);
         T vm[V], vc[V], vp[V], vn[V], vs[V];
@@ -426,6 +456,162 @@ struct OpT4 {
         const int go = (rho1 > s->thresh2) && (rho1 != 0.0) && (s->k < s->max_cg);
         s->inner_go = go;
         set_cond(a.cond, -1, go);
+    }
+};
+
+// ------------------------------------------------------------------------------------------------ K2 (TMA)
+// outer boundary update (Eq. 12 collapsed): P <- P + delta (into the other P buffer);
+// r0 = S - L P with (L P)_C = sum_d v(C+d) t_a (P_C - P_{C+d}) = ([W^{n+1}] - [W^n]) P; eps_R^2 ||S||^2 = ||r0||^2 (Eq. 41).
+// P is always fp64 (master pressure, A9), so a lane's 16-byte chunk is 2 cells and the tile is 64 cells wide;
+// delta, S, r are T.  Links of unflagged chunks come from the position (box faces); flagged chunks read their link bytes.
+__device__ __forceinline__ void lds_pair(uint32_t addr, float (&v)[2])
+{
+    asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(v[0]), "=f"(v[1]) : "r"(addr));
+}
+__device__ __forceinline__ void lds_pair(uint32_t addr, double (&v)[2])
+{
+    asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(v[0]), "=d"(v[1]) : "r"(addr));
+}
+
+template <typename T, int BY_, int D_, int MINB_>
+struct OpT2 {
+    using VT = double;
+    struct TG {
+        static constexpr int V = 2, BX = 64, BY = BY_, NTHR = 32 * (BY_ + 1);
+        static constexpr int HXP = 2, PITCH_P = (BX + 2 * HXP) * 8;                      // 544 bytes
+        static constexpr int HXD = 16 / (int)sizeof(T), PITCH_D = (BX + 2 * HXD) * (int)sizeof(T);
+        static constexpr int BOX_P = (BY_ + 2) * PITCH_P, BOX_D = (BY_ + 2) * PITCH_D;
+        static constexpr int TILE_P = (BOX_P + 127) / 128 * 128, TILE_D = (BOX_D + 127) / 128 * 128;
+        static constexpr int TILE_S = BY_ * BX * (int)sizeof(T);
+    };
+    enum { V = 2, D = D_, MINB = MINB_, NACC = 2, TICKET = 2, STAGE_BYTES = TG::TILE_P + TG::TILE_D + TG::TILE_S };
+    struct Args {
+        double* Pbuf[2]; T* r; const uint8_t* link; const uint32_t* flags; const uint32_t* tflags;
+        double t[3]; Scalars* sc; double* partial; CondHandles cond;
+        int fold_delta;   // 0: residual of P as given (omni_residual); 1: inside the solve
+    };
+    struct Ctx {
+        int par; double* Pout;
+        __device__ Ctx(const Args& a) { par = a.fold_delta ? (a.sc->n & 1) : 0; Pout = a.Pbuf[par ^ 1]; }
+    };
+    // thread constant: link bytes of an unflagged chunk as far as x decides (box faces normal to x, pad cells)
+    using TC = uint32_t;
+    __device__ static TC thread_init(const Geom& g, int x)
+    {
+        uint32_t lk = 0;
+#pragma unroll
+        for (int i = 0; i < V; ++i) {
+            const int gi = x + i;
+            uint32_t l = 0x7fu;
+            if (g.nz == 1) l &= ~48u;
+            if (g.fix[0]) {
+                if (gi == 0) l &= ~2u;
+                if (gi == g.nx - 1) l &= ~1u;
+                if (gi >= g.nx) l = 0;
+            }
+            lk |= l << (8 * i);
+        }
+        return lk;
+    }
+    __device__ static bool active(const Args& a) { return a.sc->outer_go != 0; }
+    __device__ static void idle(const Args& a) { set_cond(a.cond, 0, 0); }
+    __device__ static void load_codes(const Args& a, long long cell, uint32_t (&code)[V])
+    {
+        code[0] = *reinterpret_cast<const unsigned short*>(a.link + cell);
+        code[1] = 0u;
+    }
+    __device__ static void produce(const Args&, const Ctx& c, const TmaSet& m, uint32_t stage, uint32_t bar, int x0, int y0,
+                                   int plane, bool inner)
+    {
+        mbar_expect_tx(bar, TG::BOX_P + TG::BOX_D + (inner ? TG::TILE_S : 0));
+        tma_load_3d(stage, &m.P_h[c.par], bar, x0 - TG::HXP, y0 - 1, plane);
+        tma_load_3d(stage + TG::TILE_P, &m.d2_h, bar, x0 - TG::HXD, y0 - 1, plane);
+        if (inner) tma_load_3d(stage + TG::TILE_P + TG::TILE_D, &m.S_c, bar, x0, y0, plane);
+    }
+    struct State {};
+    __device__ static void advance(State&, const Ctx&, uint32_t, int, int) {}
+    __device__ static void value(uint32_t st, int offP, int offD, double (&v)[V])
+    {
+        double P[2]; T d[2];
+        lds_pair(st + offP, P);
+        lds_pair(st + TG::TILE_P + offD, d);
+        v[0] = P[0] + (double)d[0];
+        v[1] = P[1] + (double)d[1];
+    }
+    template <bool CLEAN>
+    __device__ static void emit(const Args& a, const Ctx& c, const State&, long long idx, uint32_t sB, uint32_t sC, uint32_t sF,
+                                int warp, int lane, bool out, uint32_t fb, const uint32_t (&code)[V], const TC& lk_x, int ycls,
+                                int zcls, double (&acc)[2])
+    {
+        const int rowP = (warp + 1) * TG::PITCH_P, rowD = (warp + 1) * TG::PITCH_D;
+        const int offP = rowP + (TG::HXP + lane * V) * 8, offD = rowD + (TG::HXD + lane * V) * (int)sizeof(T);
+        double vm[V], vc[V], vp[V], vn[V], vs[V];
+        value(sC, offP, offD, vc);
+        value(sC, offP + TG::PITCH_P, offD + TG::PITCH_D, vn);
+        value(sC, offP - TG::PITCH_P, offD - TG::PITCH_D, vs);
+        value(sF, offP, offD, vp);
+        value(sB, offP, offD, vm);
+        const double hl = lds_scalar(sC + rowP + (TG::HXP - 1) * 8, double()) +
+                          (double)lds_scalar(sC + TG::TILE_P + rowD + (TG::HXD - 1) * (int)sizeof(T), T());
+        const double hr = lds_scalar(sC + rowP + (TG::HXP + TG::BX) * 8, double()) +
+                          (double)lds_scalar(sC + TG::TILE_P + rowD + (TG::HXD + TG::BX) * (int)sizeof(T), T());
+        double xl = __shfl_up_sync(0xffffffffu, vc[V - 1], 1);
+        double xr = __shfl_down_sync(0xffffffffu, vc[0], 1);
+        if (lane == 0) xl = hl;
+        if (lane == 31) xr = hr;
+        if (!out) return;
+        if (a.fold_delta) st_chunk<double, V>(c.Pout + idx, vc);
+        uint32_t lk = lk_x;
+        if (ycls == 0) lk &= ~0x0808u;          // row 0: no S link; last row: no N link (faces normal to y)
+        if (ycls == 3) lk &= ~0x0404u;
+        if (zcls == 0) lk &= ~0x2020u;          // first plane: no B link; last plane: no F link
+        if (zcls == 3) lk &= ~0x1010u;
+        if (!CLEAN && fb) lk = code[0];
+        T S[2];
+        lds_pair(sC + TG::TILE_P + TG::TILE_D + (warp * TG::BX + lane * V) * (int)sizeof(T), S);
+        T rn[V];
+#pragma unroll
+        for (int i = 0; i < V; ++i) {
+            const double w = (i == 0) ? xl : vc[0];
+            const double ee = (i == V - 1) ? xr : vc[1];
+            const uint32_t l = (lk >> (8 * i)) & 0xffu;
+            double LP = 0.0;
+            if (l & 1u) LP += a.t[0] * (vc[i] - ee);
+            if (l & 2u) LP += a.t[0] * (vc[i] - w);
+            if (l & 4u) LP += a.t[1] * (vc[i] - vn[i]);
+            if (l & 8u) LP += a.t[1] * (vc[i] - vs[i]);
+            if (l & 16u) LP += a.t[2] * (vc[i] - vp[i]);
+            if (l & 32u) LP += a.t[2] * (vc[i] - vm[i]);
+            const double rr = (l & LINK_VALID) ? ((double)S[i] - LP) : 0.0;
+            rn[i] = (T)rr;
+            acc[0] += rr * rr;
+            acc[1] += (double)rn[i] * (double)rn[i];
+        }
+        st_chunk<T, V>(a.r + idx, rn);
+    }
+    __device__ static void finalize(const Args& a, const double (&tot)[2])
+    {
+        Scalars* s = a.sc;
+        s->epsR2 = tot[0];
+        if (!a.fold_delta) return;
+        if (!isfinite(tot[0])) {
+            s->status = ST_BREAKDOWN; s->inner_go = 0; s->outer_go = 0;
+            set_cond(a.cond, 0, 0);
+            return;
+        }
+        if (tot[0] <= s->tol2S || s->n >= s->max_outer) {
+            s->status = (tot[0] <= s->tol2S) ? ST_OK : ST_NOT_CONVERGED;
+            s->inner_go = 0; s->outer_go = 0;
+            set_cond(a.cond, 0, 0);
+            return;
+        }
+        s->n += 1;
+        s->k = 0;
+        s->beta = 0.0;
+        s->rho = tot[1];
+        const int go = (tot[1] > s->thresh2) && (tot[1] != 0.0) && (s->max_cg > 0);
+        s->inner_go = go;
+        set_cond(a.cond, 1, go);
     }
 };
 

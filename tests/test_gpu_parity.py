@@ -236,6 +236,10 @@ def test_host_buffers_and_workspace_entry_points(oracle):
     ws = torch.empty(omni.workspace_bytes(30, 20, 10, "f64"), dtype=torch.uint8, device="cuda")
     Pw, iw = omni.solve(gd[0], gd[1], gd[2], None, f["d"], 1e-6, 100, 10, workspace=ws)
     assert iw == idv and np.array_equal(Pw.cpu().numpy(), Pd.cpu().numpy())
+    # a workspace full of NaN bit patterns must not leak into the result (every array is initialised by the solve)
+    ws.fill_(0xFF)
+    Pw2, iw2 = omni.solve(gd[0], gd[1], gd[2], None, f["d"], 1e-6, 100, 10, workspace=ws)
+    assert iw2 == idv and np.array_equal(Pw2.cpu().numpy(), Pd.cpu().numpy())
     small = torch.empty(1024, dtype=torch.uint8, device="cuda")
     with pytest.raises(omni.OmniError):
         omni.solve(gd[0], gd[1], gd[2], None, f["d"], 1e-6, 100, 10, workspace=small)
