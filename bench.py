@@ -26,7 +26,8 @@ STEP_MAX_OUTER = 8
 STEP_MAX_CG = 25
 METRIC = "grid-point CG updates/s"
 UNIT = "grid-point CG updates/s"
-CPU_SAMPLE_EDGE = 200                   # 3D: edge of the corner crop the oracle is timed on (2D: the whole grid)
+CPU_SAMPLE_EDGE = 320                   # 3D: edge of the corner crop the oracle is timed on (2D: the whole grid);
+                                        # with the step's own caps that is ~10 s of work on 16 host threads
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel (K4) from the ncu --set full capture
 # summarised in profiles/r1_ncu_k3_k4_500cube_f32.md; only valid for that workload.
 NCU_TRAFFIC_K4 = {(4, "f32"): 1.526446e9 + 0.955657e9}
@@ -161,7 +162,7 @@ def run_oracle(f, dtype, steps, warmup):
         g = [c.astype(np.float32).astype(np.float64) for c in g]
     g = g + [None] * (3 - len(g))
     tol = 1e-5 if dtype == "f32" else 1e-8
-    mo, mc = 4, 25
+    mo, mc = STEP_MAX_OUTER, STEP_MAX_CG
     for _ in range(warmup):
         orc.solve(g[0], g[1], g[2], m, *f["d"], tol=tol, max_outer=mo, max_cg=mc)
     t0 = time.perf_counter()
