@@ -142,6 +142,38 @@ def test_small_and_thin_grids(oracle, dtype, shape):
             assert np.abs(Pz - Poz).max() <= (1e-10 if dtype == "f64" else 2e-4) * np.abs(Poz).max(), (shape, with_mask)
 
 
+@pytest.mark.parametrize("seed", range(24))
+def test_fuzz_random_shapes_masks_spacings(oracle, seed):
+    """Seeded fuzz: random 2D/3D shapes (tile tails, pad-only chunks, thin axes), random mask densities including
+    masks touching the box faces, random anisotropic spacing; operator, residual and a short solve against the oracle."""
+    rng = np.random.default_rng(1000 + seed)
+    nd = 2 if seed % 3 == 0 else 3
+    shape = tuple(int(rng.integers(1, 12)) for _ in range(nd - 1)) + (int(rng.integers(1, 200)),)
+    dtype = "f64" if seed % 2 == 0 else "f32"
+    d = tuple(float(rng.uniform(0.2, 2.0)) for _ in range(3))
+    frac = [0.0, 0.05, 0.3][seed % 3]
+    mask = (rng.random(shape) > frac).astype(np.uint8) if frac > 0 else None
+    g = [rng.normal(size=shape) for _ in range(nd)]
+    f = dict(g=g, mask=mask, d=d)
+    g_dev, g_or, m_dev, m = _inputs(f, dtype, mask)
+    v = oracle.validity(g_or[0], g_or[1], g_or[2], m)
+    if v.sum() == 0:
+        pytest.skip("everything masked")
+    w1, w0, w0C = oracle.weights(v, *d)
+    p = rng.normal(size=shape)
+    p_dev = to_dev(p, TDT[dtype])
+    p_or = p_dev.cpu().numpy().astype(np.float64) * v
+    q, _ = omni.apply_M(p_dev, m_dev, d)
+    q_or = oracle.apply_M(v, w1, p_or)
+    assert np.abs(q.cpu().numpy() - q_or).max() <= TOL_STEP[dtype] * 8 * max(np.abs(q_or).max(), 1e-30), (shape, dtype)
+    P, info, Po, io = _solve_both(oracle, f, dtype, 0.0, 3, 5, mask)
+    assert info["cg_iters_total"] == io["cg_iters_total"]
+    assert np.array_equal(np.isnan(P), np.isnan(Po))
+    scale = np.nanmax(np.abs(Po)) if np.isfinite(Po).any() else 0.0
+    if scale > 0:
+        assert np.nanmax(np.abs(np.nan_to_num(P) - np.nan_to_num(Po))) <= (1e-10 if dtype == "f64" else 2e-4) * scale, (shape, dtype)
+
+
 def test_converged_parity_config0(oracle):
     """BASELINE configs[0]: 64^2 fp64, tol 1e-8, converged on both sides with the same stopping rules; and the
     recovered field matches the analytic P up to a constant at the discretisation + noise level."""
