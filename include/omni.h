@@ -87,6 +87,21 @@ int omni_solve_host_f32(int nx, int ny, int nz, double dx, double dy, double dz,
                         const float* h_gx, const float* h_gy, const float* h_gz, const unsigned char* h_mask,
                         float* h_P_out, double tol, int max_outer, int max_cg, void* stream, omni_info* info);
 
+/* ---- batched 2D snapshots with an optional first guess (SURVEY.md 8(f) NEXT-1; time-resolved PIV: PAPER.md:365, :503) ----
+ * nb independent 2D gradient fields [nb][ny][nx] on ONE mask [ny][nx] (NULL = all valid) are stacked and solved as one
+ * block-diagonal system with the 2D scheme: stencil codes are built once, every stencil sweep serves all snapshots,
+ * and the tile pipeline marches through the snapshots like through the planes of a volume.  The CG scalars and eps_R
+ * (Eq. 41) are those of the stacked system: on return EVERY snapshot satisfies Eq. 12 to the joint tolerance, and each
+ * converged P_b equals the single-snapshot result within tol.  d_P_init [nb][ny][nx] (may be NULL = zeros) is the
+ * first guess P^0, e.g. the previous time step's pressure ("zero ... or any other arbitrary value");
+ * its values at missing cells are ignored.  Everything else as omni_solve_*. */
+int omni_solve_batch2d_f64(int nx, int ny, int nb, double dx, double dy, const double* d_gx, const double* d_gy,
+                           const unsigned char* d_mask2d, const double* d_P_init, double* d_P_out, double tol,
+                           int max_outer, int max_cg, void* stream, omni_info* info);
+int omni_solve_batch2d_f32(int nx, int ny, int nb, double dx, double dy, const float* d_gx, const float* d_gy,
+                           const unsigned char* d_mask2d, const float* d_P_init, float* d_P_out, double tol,
+                           int max_outer, int max_cg, void* stream, omni_info* info);
+
 /* ---- single steps of the path (each runs the same device code the solve runs; used by the parity tests) ----------
  * a0  geometry constants (host only, no device needed).  out[0..2] = face totals F_x,F_y,F_z (Eq. 5 :75 / Eq. 23 :258),
  *     out[3] = A_tot (Eq. 8 :94 / Eq. 24 :262), out[4..12] = c_jk row-major 3x3 (Eq. 17 :207 / Eq. 32-35 :314-326 /

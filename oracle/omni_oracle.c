@@ -109,12 +109,18 @@ static double far_face_constant(double da, double db, double dc)
  * out[3]     = A_tot              (Eq. 8 :94 / Eq. 24 :262)
  * out[4..12] = c[a][b] row-major  (Eq. 17 :207-212 / Eq. 32-35 :314-326 / A7)
  * nz == 1 -> 2D scheme: F_z = 0 and every c with a z index = 0. */
+/* Batched 2D snapshots (SURVEY NEXT-1; PAPER.md:365 "26 Taylor vortex snapshots", :503): nb independent 2D fields on
+ * one mask are stacked along z and solved as ONE block-diagonal system with the 2D constants.  Every constant with a
+ * z index is then 0, so all weights across planes vanish (Eq. 16/18 with c_xz = c_yz = c_zz = 0, F_z = 0) and no other
+ * routine needs to know.  The flag is set only inside oracle_solve_batch2d (test infrastructure: not thread safe). */
+static int g_batch2d = 0;
+
 void oracle_constants(int nx, int ny, int nz, double dx, double dy, double dz, double *out)
 {
     (void)nx; (void)ny;
     double F[3], c[3][3], Atot;
     memset(c, 0, sizeof c);
-    if (nz == 1) {
+    if (nz == 1 || g_batch2d) {
         double dd = sqrt(dx * dx + dy * dy);          /* :214 */
         F[0] = 2.0 * dy; F[1] = 2.0 * dx; F[2] = 0.0; /* Eq. 5 :75, :96 */
         Atot = 4.0 * (dx + dy);                       /* Eq. 8 :94 */
@@ -353,10 +359,43 @@ typedef struct {
 
 /* P_out: pressure at valid cells, NaN at missing cells (:158).  hist (may be NULL) receives eps_R of every outer
  * iteration visited, up to hist_cap entries.  Returns 0, or -1 on allocation failure. */
+static int solve_impl(int nx, int ny, int nz, double dx, double dy, double dz,
+                      const double *gx, const double *gy, const double *gz, const unsigned char *mask,
+                      const double *P_init, double *P_out, double tol, int max_outer, int max_cg, oracle_info *info,
+                      double *hist, int hist_cap);
+
 int oracle_solve(int nx, int ny, int nz, double dx, double dy, double dz,
                  const double *gx, const double *gy, const double *gz, const unsigned char *mask,
                  double *P_out, double tol, int max_outer, int max_cg, oracle_info *info,
                  double *hist, int hist_cap)
+{
+    return solve_impl(nx, ny, nz, dx, dy, dz, gx, gy, gz, mask, NULL, P_out, tol, max_outer, max_cg, info, hist, hist_cap);
+}
+
+/* nb snapshots [nb][ny][nx] on one mask [ny][nx] (NULL = all valid), optional first guess P_init [nb][ny][nx]
+ * ("initialized to zero ... or any other arbitrary value"; NULL = 0).  eps_R and the CG scalars are those
+ * of the stacked system. */
+int oracle_solve_batch2d(int nx, int ny, int nb, double dx, double dy,
+                         const double *gx, const double *gy, const unsigned char *mask2d, const double *P_init,
+                         double *P_out, double tol, int max_outer, int max_cg, oracle_info *info)
+{
+    unsigned char *m = NULL;
+    if (mask2d) {
+        m = (unsigned char *)malloc((size_t)nx * ny * nb);
+        if (!m) return -1;
+        for (int b = 0; b < nb; ++b) memcpy(m + (size_t)b * nx * ny, mask2d, (size_t)nx * ny);
+    }
+    g_batch2d = 1;
+    int rc = solve_impl(nx, ny, nb, dx, dy, 1.0, gx, gy, NULL, m, P_init, P_out, tol, max_outer, max_cg, info, NULL, 0);
+    g_batch2d = 0;
+    free(m);
+    return rc;
+}
+
+static int solve_impl(int nx, int ny, int nz, double dx, double dy, double dz,
+                      const double *gx, const double *gy, const double *gz, const unsigned char *mask,
+                      const double *P_init, double *P_out, double tol, int max_outer, int max_cg, oracle_info *info,
+                      double *hist, int hist_cap)
 {
     i64 N = (i64)nx * ny * nz;
     size_t nb = sizeof(double) * (size_t)N;
@@ -370,8 +409,10 @@ int oracle_solve(int nx, int ny, int nz, double dx, double dy, double dz,
 
     oracle_validity(nx, ny, nz, gx, gy, gz, mask, v);
     oracle_weights(nx, ny, nz, dx, dy, dz, v, w1, w0, w0C);
-    oracle_source(nx, ny, nz, dx, dy, dz, v, w1, w0, gx, gy, gz, S);
+    oracle_source(nx, ny, nz, dx, dy, dz, v, w1, w0, gx, gy, gz ? gz : gx, S);
     double normS = sqrt(dot(N, nx, S, S));
+    if (P_init)
+        for (i64 c = 0; c < N; ++c) P[c] = v[c] ? P_init[c] : 0.0;
 
     int n = 0;
     i64 cg_total = 0;

@@ -97,12 +97,12 @@ struct HostConst {
     double F[3], Atot, c[3][3];
 };
 
-void host_constants(int nz, double dx, double dy, double dz, HostConst& H)
+void host_constants(int naxes, double dx, double dy, double dz, HostConst& H)
 {
     const double PI = 3.14159265358979323846;
     for (int a = 0; a < 3; ++a)
         for (int b = 0; b < 3; ++b) H.c[a][b] = 0.0;
-    if (nz == 1) {                                             // 2D scheme
+    if (naxes == 2) {                                          // 2D scheme
         const double dd = std::hypot(dx, dy);
         H.F[0] = 2.0 * dy; H.F[1] = 2.0 * dx; H.F[2] = 0.0;     // Eq. 5 :75
         H.Atot = 4.0 * (dx + dy);                              // Eq. 8 :94
@@ -143,7 +143,7 @@ Coef<T> make_coef(const HostConst& H, double dx, double dy, double dz, const Geo
         }
     }
     K.icode = g.icode;
-    const int naxes = (g.nz > 1) ? 3 : 2;
+    const int naxes = g.naxes;
     const int n3[3] = { g.nx, g.ny, g.nz };
     for (int ax = 0; ax < 3; ++ax)
         for (int cls = 0; cls < 4; ++cls) {
@@ -183,7 +183,7 @@ uint32_t std_axis_code(int ax, int pos, int n, int naxes)
     return code;
 }
 
-bool make_geom(int nx, int ny, int nz, int elem_size, Geom& g)
+bool make_geom(int nx, int ny, int nz, int elem_size, Geom& g, int batch = 0)
 {
     if (nx < 1 || ny < 1 || nz < 1) return false;
     const long long pad = (elem_size == 4) ? 8 : 4;        // one thread chunk = 32 bytes
@@ -193,7 +193,8 @@ bool make_geom(int nx, int ny, int nz, int elem_size, Geom& g)
     g.nx = nx; g.ny = ny; g.nz = nz; g.px = (int)px;
     g.pplane = px * ny;
     g.npad = npad;
-    const int naxes = (nz > 1) ? 3 : 2;
+    const int naxes = (nz > 1 && !batch) ? 3 : 2;
+    g.naxes = naxes; g.batch = batch ? 1 : 0;
     const int n3[3] = { nx, ny, nz };
     for (int a = 0; a < 3; ++a) g.fix[a] = (a < naxes && n3[a] >= 4) ? 1 : 0;
     g.xfix = g.fix[0];
@@ -576,18 +577,18 @@ bool valid_common(int nx, int ny, int nz, double dx, double dy, double dz, doubl
 template <typename T>
 int solve_ws(int nx, int ny, int nz, double dx, double dy, double dz, const T* gx, const T* gy, const T* gz,
              const unsigned char* mask, T* P_out, double tol, int max_outer, int max_cg, void* ws, size_t ws_bytes,
-             void* stream, omni_info* info)
+             void* stream, omni_info* info, int batch = 0, const T* P_init = nullptr)
 {
     Geom g;
-    if (!valid_common(nx, ny, nz, dx, dy, dz, tol, max_outer, max_cg) || !make_geom(nx, ny, nz, (int)sizeof(T), g)) return OMNI_ERR_INVALID_ARG;
-    if (!gx || !gy || (nz > 1 && !gz) || !P_out || !ws) return OMNI_ERR_INVALID_ARG;
+    if (!valid_common(nx, ny, batch ? 1 : nz, dx, dy, dz, tol, max_outer, max_cg) || !make_geom(nx, ny, nz, (int)sizeof(T), g, batch)) return OMNI_ERR_INVALID_ARG;
+    if (!gx || !gy || (g.naxes == 3 && !gz) || !P_out || !ws) return OMNI_ERR_INVALID_ARG;
     if (((uintptr_t)ws & 255) != 0) return OMNI_ERR_INVALID_ARG;
     if (ws_bytes < carve<T>(g, nullptr, nullptr)) return OMNI_ERR_ALLOC;
     cudaStream_t st = (cudaStream_t)stream;
     Workspace<T> w;
     carve<T>(g, (char*)ws, &w);
     HostConst H;
-    host_constants(nz, dx, dy, dz, H);
+    host_constants(g.naxes, dx, dy, dz, H);
     const Coef<T> K = make_coef<T>(H, dx, dy, dz, g);
 
     init_scalars_kernel<<<1, 1, 0, st>>>(w.sc, tol, max_outer, max_cg);
@@ -597,6 +598,13 @@ int solve_ws(int nx, int ny, int nz, double dx, double dy, double dz, const T* g
     if (rc != OMNI_OK) return rc;
     rc = launch_source<T>(g, w, K, gx, gy, gz, st);
     if (rc != OMNI_OK) return rc;
+    if (P_init) {       // first guess P^0 ("zero ... or any other arbitrary value"); 0 at missing cells
+        const unsigned nbk = blocks_for(g.npad, 256);
+        pad_copy_kernel<T, double><<<nbk, 256, 0, st>>>(g, P_init, w.P, 1, w.link);
+        pad_copy_kernel<T, double><<<nbk, 256, 0, st>>>(g, P_init, w.P1, 1, w.link);
+        CK(cudaGetLastError());
+        g_launches.fetch_add(2, std::memory_order_relaxed);
+    }
 
     const int mode = g_loop_mode.load();
     rc = (mode == 1) ? run_loop_host<T>(g, w, H, K, max_outer, max_cg, st) : run_loop_graph<T>(g, w, H, K, st);
@@ -623,15 +631,17 @@ int solve_ws(int nx, int ny, int nz, double dx, double dy, double dz, const T* g
 
 template <typename T>
 int solve_alloc(int nx, int ny, int nz, double dx, double dy, double dz, const T* gx, const T* gy, const T* gz,
-                const unsigned char* mask, T* P_out, double tol, int max_outer, int max_cg, void* stream, omni_info* info)
+                const unsigned char* mask, T* P_out, double tol, int max_outer, int max_cg, void* stream, omni_info* info,
+                int batch = 0, const T* P_init = nullptr)
 {
     Geom g;
-    if (!valid_common(nx, ny, nz, dx, dy, dz, tol, max_outer, max_cg) || !make_geom(nx, ny, nz, (int)sizeof(T), g)) return OMNI_ERR_INVALID_ARG;
+    if (!valid_common(nx, ny, batch ? 1 : nz, dx, dy, dz, tol, max_outer, max_cg) || !make_geom(nx, ny, nz, (int)sizeof(T), g, batch)) return OMNI_ERR_INVALID_ARG;
     cudaStream_t st = (cudaStream_t)stream;
     const size_t bytes = carve<T>(g, nullptr, nullptr);
     void* ws = nullptr;
     if (pool_alloc(&ws, bytes, st) != cudaSuccess) { cudaGetLastError(); return OMNI_ERR_ALLOC; }
-    int rc = solve_ws<T>(nx, ny, nz, dx, dy, dz, gx, gy, gz, mask, P_out, tol, max_outer, max_cg, ws, bytes, stream, info);
+    int rc = solve_ws<T>(nx, ny, nz, dx, dy, dz, gx, gy, gz, mask, P_out, tol, max_outer, max_cg, ws, bytes, stream, info,
+                         batch, P_init);
     cudaFreeAsync(ws, st);
     return rc;
 }
@@ -688,7 +698,7 @@ int step_begin(StepCtx<T>& c, int nx, int ny, int nz, double dx, double dy, doub
     c.ws = nullptr;
     if (pool_alloc(&c.ws, bytes, c.st) != cudaSuccess) { cudaGetLastError(); return OMNI_ERR_ALLOC; }
     carve<T>(c.g, (char*)c.ws, &c.w);
-    host_constants(nz, dx, dy, dz, c.H);
+    host_constants(c.g.naxes, dx, dy, dz, c.H);
     c.K = make_coef<T>(c.H, dx, dy, dz, c.g);
     init_scalars_kernel<<<1, 1, 0, c.st>>>(c.w.sc, 0.0, 0, 0);
     g_launches.fetch_add(1, std::memory_order_relaxed);
@@ -847,11 +857,29 @@ int omni_solve_host_f32(int nx, int ny, int nz, double dx, double dy, double dz,
     return solve_host<float>(nx, ny, nz, dx, dy, dz, h_gx, h_gy, h_gz, h_mask, h_P_out, tol, max_outer, max_cg, stream, info);
 }
 
+int omni_solve_batch2d_f64(int nx, int ny, int nb, double dx, double dy, const double* d_gx, const double* d_gy,
+                           const unsigned char* d_mask2d, const double* d_P_init, double* d_P_out, double tol,
+                           int max_outer, int max_cg, void* stream, omni_info* info)
+{
+    if (!d_gx || !d_gy || !d_P_out || nb < 1) return OMNI_ERR_INVALID_ARG;
+    return solve_alloc<double>(nx, ny, nb, dx, dy, 1.0, d_gx, d_gy, nullptr, d_mask2d, d_P_out, tol, max_outer, max_cg, stream,
+                               info, 1, d_P_init);
+}
+
+int omni_solve_batch2d_f32(int nx, int ny, int nb, double dx, double dy, const float* d_gx, const float* d_gy,
+                           const unsigned char* d_mask2d, const float* d_P_init, float* d_P_out, double tol,
+                           int max_outer, int max_cg, void* stream, omni_info* info)
+{
+    if (!d_gx || !d_gy || !d_P_out || nb < 1) return OMNI_ERR_INVALID_ARG;
+    return solve_alloc<float>(nx, ny, nb, dx, dy, 1.0, d_gx, d_gy, nullptr, d_mask2d, d_P_out, tol, max_outer, max_cg, stream,
+                              info, 1, d_P_init);
+}
+
 int omni_constants(int nx, int ny, int nz, double dx, double dy, double dz, double* h_out13)
 {
     if (!h_out13 || !valid_common(nx, ny, nz, dx, dy, dz, 0.0, 0, 0)) return OMNI_ERR_INVALID_ARG;
     HostConst H;
-    host_constants(nz, dx, dy, dz, H);
+    host_constants(nz > 1 ? 3 : 2, dx, dy, dz, H);
     h_out13[0] = H.F[0]; h_out13[1] = H.F[1]; h_out13[2] = H.F[2]; h_out13[3] = H.Atot;
     for (int a = 0; a < 3; ++a)
         for (int b = 0; b < 3; ++b) h_out13[4 + 3 * a + b] = H.c[a][b];

@@ -17,7 +17,9 @@
 namespace omni {
 
 struct Geom {
-    int nx, ny, nz;      // logical grid
+    int nx, ny, nz;      // logical grid (batch mode: nz = number of stacked 2D snapshots)
+    int naxes;           // 2: 2D scheme (nz == 1, or nz stacked 2D snapshots with no coupling across planes); 3: 3D
+    int batch;           // 1: stacked 2D snapshots; the mask, if any, is one plane shared by all snapshots
     int px;              // padded row pitch in cells (multiple of 8); cells nx..px-1 are permanently missing
     long long pplane;    // px * ny
     long long npad;      // px * ny * nz
@@ -290,10 +292,10 @@ __global__ void validity_kernel(Geom g, const T* __restrict__ gx, const T* __res
     uint8_t ok = 0;
     if (i < g.nx) {
         long long u = row * g.nx + i;             // user-layout index
-        ok = (mask == nullptr) || (mask[u] != 0);
+        ok = (mask == nullptr) || (mask[g.batch ? (u % ((long long)g.nx * g.ny)) : u] != 0);
         if (gx != nullptr) {
             if (isnan(gx[u]) || isnan(gy[u])) ok = 0;
-            if (g.nz > 1 && isnan(gz[u])) ok = 0;
+            if (g.naxes == 3 && isnan(gz[u])) ok = 0;
         }
     }
     vbyte[pid] = ok;
@@ -313,7 +315,7 @@ __device__ __forceinline__ uint32_t vbox(const Geom& g, int i, int j, int k)
 {
     if (g.fix[0] && (i < 0 || i >= g.nx)) return 0u;
     if (g.fix[1] && (j < 0 || j >= g.ny)) return 0u;
-    if (g.nz == 1) return (k == 0) ? 1u : 0u;
+    if (g.naxes == 2) return 1u;              // planes are independent 2D problems: k is never offset (see box_code)
     if (g.fix[2] && (k < 0 || k >= g.nz)) return 0u;
     return 1u;
 }
@@ -321,7 +323,7 @@ __device__ __forceinline__ uint32_t box_code(const Geom& g, int i, int j, int k)
 {
     if (i >= g.nx) return g.fix[0] ? 0u : g.icode;      // pad cells: expected only where xedge_fix zeroes them
     if (!vbox(g, i, j, k)) return 0u;
-    const int naxes = (g.nz > 1) ? 3 : 2;
+    const int naxes = g.naxes;
     uint32_t code = WCODE_VALID;
     for (int d = 0; d < 2 * naxes; ++d) {
         const int a = d >> 1, sg = (d & 1) ? -1 : 1;
@@ -333,8 +335,8 @@ __device__ __forceinline__ uint32_t box_code(const Geom& g, int i, int j, int k)
         int eb[3] = { 0, 0, 0 }, ec[3] = { 0, 0, 0 };
         eb[b] = 1; ec[cc] = 1;
         const uint32_t far = vbox(g, qi + e[0], qj + e[1], qk + e[2]);
-        const uint32_t nb = vbox(g, qi + eb[0], qj + eb[1], qk + eb[2]) + vbox(g, qi - eb[0], qj - eb[1], qk - eb[2]);
-        const uint32_t nc = vbox(g, qi + ec[0], qj + ec[1], qk + ec[2]) + vbox(g, qi - ec[0], qj - ec[1], qk - ec[2]);
+        const uint32_t nb = (b < naxes) ? vbox(g, qi + eb[0], qj + eb[1], qk + eb[2]) + vbox(g, qi - eb[0], qj - eb[1], qk - eb[2]) : 0u;
+        const uint32_t nc = (cc < naxes) ? vbox(g, qi + ec[0], qj + ec[1], qk + ec[2]) + vbox(g, qi - ec[0], qj - ec[1], qk - ec[2]) : 0u;
         code |= (far | (nb << 1) | (nc << 3)) << (5 * d);
     }
     return code;
@@ -352,13 +354,13 @@ __global__ void codes_kernel(Geom g, const uint8_t* __restrict__ vbyte, uint8_t*
         const int i0 = (int)(base % g.px);
         const long long row = base / g.px;
         const int j = (int)(row % g.ny), k = (int)(row / g.ny);
-        const int naxes = (g.nz > 1) ? 3 : 2;
+        const int naxes = g.naxes;
         uint32_t codes[4];
         uint32_t links = 0;
         // fast path: a group at least two cells away from every face whose 25-cell neighbourhoods are all valid (23
         // aligned word loads instead of ~150 byte loads) is interior: nothing to decode, nothing flagged
         const bool deep_grp = (i0 >= 4) && (i0 + 8 <= g.nx) && (j >= 2) && (j < g.ny - 2) &&
-                              (g.nz == 1 || (k >= 2 && k < g.nz - 2));
+                              (g.naxes == 2 || (k >= 2 && k < g.nz - 2));
         bool all_valid = false;
         if (deep_grp) {
             const long long sy = g.px, sz = g.pplane;
@@ -366,14 +368,14 @@ __global__ void codes_kernel(Geom g, const uint8_t* __restrict__ vbyte, uint8_t*
             auto w = [&](long long off) { return *reinterpret_cast<const uint32_t*>(c0 + off); };
             uint32_t m = w(-4) & w(0) & w(4);
             m &= w(-sy - 4) & w(-sy) & w(-sy + 4) & w(sy - 4) & w(sy) & w(sy + 4) & w(-2 * sy) & w(2 * sy);
-            if (g.nz > 1)
+            if (g.naxes == 3)
                 m &= w(-sz - 4) & w(-sz) & w(-sz + 4) & w(sz - 4) & w(sz) & w(sz + 4) & w(-2 * sz) & w(2 * sz) &
                      w(-sz - sy) & w(-sz + sy) & w(sz - sy) & w(sz + sy);
             all_valid = (m == 0x01010101u);
         }
         if (all_valid) {
             *reinterpret_cast<uint4*>(wcode + base) = make_uint4(g.icode, g.icode, g.icode, g.icode);
-            *reinterpret_cast<uint32_t*>(link + base) = (g.nz > 1) ? 0x7f7f7f7fu : 0x4f4f4f4fu;
+            *reinterpret_cast<uint32_t*>(link + base) = (g.naxes == 3) ? 0x7f7f7f7fu : 0x4f4f4f4fu;
         } else {
 #pragma unroll
         for (int c = 0; c < 4; ++c) {
@@ -393,17 +395,17 @@ __global__ void codes_kernel(Geom g, const uint8_t* __restrict__ vbyte, uint8_t*
                     int eb[3] = { 0, 0, 0 }, ec[3] = { 0, 0, 0 };
                     eb[b] = 1; ec[cc] = 1;
                     uint32_t far = vget(g, vbyte, qi + e[0], qj + e[1], qk + e[2]);
-                    uint32_t nb = vget(g, vbyte, qi + eb[0], qj + eb[1], qk + eb[2]) +
-                                  vget(g, vbyte, qi - eb[0], qj - eb[1], qk - eb[2]);
-                    uint32_t nc = vget(g, vbyte, qi + ec[0], qj + ec[1], qk + ec[2]) +
-                                  vget(g, vbyte, qi - ec[0], qj - ec[1], qk - ec[2]);
+                    uint32_t nb = (b < naxes) ? vget(g, vbyte, qi + eb[0], qj + eb[1], qk + eb[2]) +
+                                                vget(g, vbyte, qi - eb[0], qj - eb[1], qk - eb[2]) : 0u;
+                    uint32_t nc = (cc < naxes) ? vget(g, vbyte, qi + ec[0], qj + ec[1], qk + ec[2]) +
+                                                 vget(g, vbyte, qi - ec[0], qj - ec[1], qk - ec[2]) : 0u;
                     code |= (far | (nb << 1) | (nc << 3)) << (5 * d);
                 }
             }
             codes[c] = code;
             links |= lk << (8 * c);
             // two or more cells away from every face the mask-free box code is the interior code
-            const bool deep = (i >= 2 && i < g.nx - 2) && (j >= 2 && j < g.ny - 2) && (g.nz == 1 || (k >= 2 && k < g.nz - 2));
+            const bool deep = (i >= 2 && i < g.nx - 2) && (j >= 2 && j < g.ny - 2) && (g.naxes == 2 || (k >= 2 && k < g.nz - 2));
             const uint32_t expect = deep ? g.icode : box_code(g, i, j, k);
             flagged |= (code != expect);
         }

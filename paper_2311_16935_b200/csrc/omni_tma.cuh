@@ -503,7 +503,7 @@ struct OpT2 {
         for (int i = 0; i < V; ++i) {
             const int gi = x + i;
             uint32_t l = 0x7fu;
-            if (g.nz == 1) l &= ~48u;
+            if (g.naxes == 2) l &= ~48u;
             if (g.fix[0]) {
                 if (gi == 0) l &= ~2u;
                 if (gi == g.nx - 1) l &= ~1u;

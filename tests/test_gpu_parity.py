@@ -174,6 +174,42 @@ def test_fuzz_random_shapes_masks_spacings(oracle, seed):
         assert np.nanmax(np.abs(np.nan_to_num(P) - np.nan_to_num(Po))) <= (1e-10 if dtype == "f64" else 2e-4) * scale, (shape, dtype)
 
 
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_batch2d_and_first_guess(oracle, dtype):
+    """omni_solve_batch2d_*: stacked 2D snapshots on one mask against the oracle's stacked solve (same joint CG scalars),
+    with and without a first guess; nb = 1 is bit-identical to omni_solve_*; a converged first guess stops at once."""
+    fs = [make_field("lamb_oseen2d", (45, 140), seed=s, noise=0.05) for s in range(5)]
+    np_dt = np.float32 if dtype == "f32" else np.float64
+    gx = np.stack([f["g"][0] for f in fs]).astype(np_dt); gy = np.stack([f["g"][1] for f in fs]).astype(np_dt)
+    m, d = fs[0]["mask"], fs[0]["d"]
+    gxd, gyd, md = to_dev(gx), to_dev(gy), to_dev(m)
+    tolp = 1e-9 if dtype == "f64" else 2e-4
+    rng = np.random.default_rng(5)
+    P0 = (0.1 * rng.normal(size=gx.shape)).astype(np_dt)
+    for init in (None, P0):
+        P, info = omni.solve_batch2d(gxd, gyd, md, d, 0.0, 5, 12, P_init=None if init is None else to_dev(init))
+        Po, io = oracle.solve_batch2d(gx.astype(np.float64), gy.astype(np.float64), m, d[0], d[1], 0.0, 5, 12,
+                                      P_init=None if init is None else init.astype(np.float64))
+        assert info["cg_iters_total"] == io["cg_iters_total"] == 60
+        Pn = P.cpu().numpy()
+        assert np.array_equal(np.isnan(Pn), np.isnan(Po))
+        for b in range(5):
+            valid = ~np.isnan(Po[b])
+            assert rel_l2_after_mean_removal(Pn[b], Po[b], valid) <= tolp
+        assert info["eps_R_final"] == pytest.approx(io["eps_R_final"], rel=2e-3 if dtype == "f32" else 1e-7)
+    # nb = 1: same bits as the plain 2D entry point
+    Pb, ib = omni.solve_batch2d(gxd[:1].contiguous(), gyd[:1].contiguous(), md, d, 1e-4, 50, 12)
+    Ps, is_ = omni.solve(gxd[0].contiguous(), gyd[0].contiguous(), None, md, d, 1e-4, 50, 12)
+    assert ib == is_ and np.array_equal(Pb[0].cpu().numpy(), Ps.cpu().numpy(), equal_nan=True)
+    # converged field as first guess: no iteration; P returned unchanged (to the dtype)
+    tol = 1e-5 if dtype == "f32" else 1e-8
+    Pc, ic = omni.solve_batch2d(gxd, gyd, md, d, tol, 100000, 32)
+    assert ic["status"] == 0
+    Pw, iw = omni.solve_batch2d(gxd, gyd, md, d, 2 * tol, 100, 32, P_init=torch.nan_to_num(Pc))
+    assert iw["outer_iters"] == 0 and iw["cg_iters_total"] == 0
+    assert torch.allclose(torch.nan_to_num(Pw), torch.nan_to_num(Pc), rtol=0, atol=1e-6 if dtype == "f32" else 1e-13)
+
+
 def test_converged_parity_config0(oracle):
     """BASELINE configs[0]: 64^2 fp64, tol 1e-8, converged on both sides with the same stopping rules; and the
     recovered field matches the analytic P up to a constant at the discretisation + noise level."""

@@ -462,3 +462,33 @@ def test_sample_matches_stored_weight_path(oracle):
     assert np.allclose(Ss, S.ravel()[cells], rtol=1e-14, atol=1e-16)
     assert np.allclose(Ms, oracle.apply_M(v, w1, x).ravel()[cells], rtol=1e-14, atol=1e-16)
     assert np.allclose(Ws, oracle.apply_Wn(v, w0, w0C, x).ravel()[cells], rtol=1e-14, atol=1e-16)
+
+
+# ----------------------------------------------------------------------------- batched snapshots / first guess (NEXT-1)
+
+def test_batch2d_oracle_pins(oracle):
+    """Stacked 2D snapshots solved as one block-diagonal system (2D constants, no coupling across planes):
+    nb = 1 is bit-identical to the plain 2D solve; converged, every snapshot equals its own single solve (pinned above)
+    within the tolerance; a first guess equal to the converged field needs no iteration (:82 'any other arbitrary
+    value'); the fixed point does not depend on the first guess."""
+    fs = [make_field("lamb_oseen2d", (26, 30), seed=s, noise=0.05) for s in range(3)]
+    gx = np.stack([f["g"][0] for f in fs]); gy = np.stack([f["g"][1] for f in fs])
+    m, d = fs[0]["mask"], fs[0]["d"]
+    P1, i1 = oracle.solve_batch2d(gx[:1], gy[:1], m, d[0], d[1], 0.0, 5, 10)
+    P2, i2 = oracle.solve(gx[0], gy[0], None, m, d[0], d[1], 1.0, tol=0.0, max_outer=5, max_cg=10)
+    assert np.array_equal(P1[0], P2, equal_nan=True) and i1["eps_R_final"] == i2["eps_R_final"]
+    Pb, ib = oracle.solve_batch2d(gx, gy, m, d[0], d[1], 1e-10, 100000, 400)
+    assert ib["converged"]
+    for b in range(3):
+        Pi, ii = oracle.solve(gx[b], gy[b], None, m, d[0], d[1], 1.0, tol=1e-10, max_outer=100000, max_cg=400)
+        v = ~np.isnan(Pi)
+        a, c = Pb[b][v] - Pb[b][v].mean(), Pi[v] - Pi[v].mean()
+        assert np.linalg.norm(a - c) / np.linalg.norm(c) < 2e-9
+    Pw, iw = oracle.solve_batch2d(gx, gy, m, d[0], d[1], 1e-9, 100, 50, P_init=np.nan_to_num(Pb))
+    assert iw["outer_iters"] == 0 and iw["cg_iters_total"] == 0
+    rng = np.random.default_rng(0)
+    Pr, ir = oracle.solve_batch2d(gx, gy, m, d[0], d[1], 1e-10, 100000, 400, P_init=rng.normal(size=gx.shape))
+    v = ~np.isnan(Pb)
+    for b in range(3):
+        a, c = Pr[b][v[b]] - Pr[b][v[b]].mean(), Pb[b][v[b]] - Pb[b][v[b]].mean()
+        assert np.linalg.norm(a - c) / np.linalg.norm(c) < 1e-7
