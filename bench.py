@@ -45,6 +45,9 @@ def parse():
                     help="instead of the fixed-cap step: time ONE solve to the config's tolerance (BASELINE.md table)")
     ap.add_argument("--max-cg", type=int, default=1000, help="--converge: CG cap per outer iteration")
     ap.add_argument("--max-outer", type=int, default=200000, help="--converge: outer iteration cap")
+    ap.add_argument("--batch", type=int, default=1,
+                    help="--converge on a 2D config: solve this many snapshots (same mask, different noise seeds) in one "
+                         "omni_solve_batch2d call")
     return ap.parse_args()
 
 
@@ -54,25 +57,42 @@ def converge(args, cfg, dtype):
     import torch
     import paper_2311_16935_b200 as omni
     from workloads import make_config
-    f = make_config(args.config, device="cuda")
     tdt = torch.float32 if dtype == "f32" else torch.float64
-    g = [torch.from_numpy(c).to(tdt).cuda() for c in f["g"]] + [None] * (3 - len(f["g"]))
-    m = None if f["mask"] is None else torch.from_numpy(f["mask"]).cuda()
     tol = 1e-5 if dtype == "f32" else 1e-8
-    omni.solve(g[0], g[1], g[2], m, f["d"], tol, 2, 2)                       # warm-up (module load, pool)
-    torch.cuda.synchronize()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    e0.record()
-    P, info = omni.solve(g[0], g[1], g[2], m, f["d"], tol, args.max_outer, args.max_cg)
-    e1.record()
-    torch.cuda.synchronize()
+    if args.batch > 1:
+        from workloads import CONFIGS, make_field
+        c = CONFIGS[args.config]
+        fs = [make_field(c["kind"], (c["n"], c["n"]), seed=1000 + b, noise=c["noise"]) for b in range(args.batch)]
+        f = fs[0]
+        gx = torch.from_numpy(np.stack([x["g"][0] for x in fs])).to(tdt).cuda()
+        gy = torch.from_numpy(np.stack([x["g"][1] for x in fs])).to(tdt).cuda()
+        m = None if f["mask"] is None else torch.from_numpy(f["mask"]).cuda()
+        omni.solve_batch2d(gx, gy, m, f["d"], tol, 2, 2)
+        torch.cuda.synchronize()
+        e0.record()
+        P, info = omni.solve_batch2d(gx, gy, m, f["d"], tol, args.max_outer, args.max_cg)
+        e1.record()
+        torch.cuda.synchronize()
+        Pn = P[0].double().cpu().numpy()
+        N = gx.numel()
+    else:
+        f = make_config(args.config, device="cuda")
+        g = [torch.from_numpy(c).to(tdt).cuda() for c in f["g"]] + [None] * (3 - len(f["g"]))
+        m = None if f["mask"] is None else torch.from_numpy(f["mask"]).cuda()
+        omni.solve(g[0], g[1], g[2], m, f["d"], tol, 2, 2)                       # warm-up (module load, pool)
+        torch.cuda.synchronize()
+        e0.record()
+        P, info = omni.solve(g[0], g[1], g[2], m, f["d"], tol, args.max_outer, args.max_cg)
+        e1.record()
+        torch.cuda.synchronize()
+        Pn = P.double().cpu().numpy()
+        N = g[0].numel()
     sec = e0.elapsed_time(e1) * 1e-3
-    Pn = P.double().cpu().numpy()
     valid = ~np.isnan(Pn)
     a, b = Pn[valid] - Pn[valid].mean(), f["P"][valid] - f["P"][valid].mean()
-    N = g[0].numel()
     print(json.dumps({"converge": True, "workload": f"configs[{args.config}] {cfg['kind']} {cfg['n']} {dtype}", "tol": tol,
-                      "max_cg": args.max_cg, "outer_iters": info["outer_iters"], "cg_iters": info["cg_iters_total"],
+                      "max_cg": args.max_cg, "batch": args.batch, "outer_iters": info["outer_iters"], "cg_iters": info["cg_iters_total"],
                       "seconds": sec, "eps_R": info["eps_R_final"], "status": info["status"],
                       "updates_per_s": N * info["cg_iters_total"] / sec,
                       "rel_l2_vs_analytic_P": float(np.linalg.norm(a - b) / np.linalg.norm(b))}))
