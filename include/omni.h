@@ -138,8 +138,14 @@ int omni_residual_f32(int nx, int ny, int nz, double dx, double dy, double dz,
 /* ---- misc ---------------------------------------------------------------------------------------------------- */
 /* Kernel launches issued by this library since the last reset (counts launches on any thread; for bench.py). */
 long long omni_launch_count(int reset);
-/* 0 = CUDA-graph loop with device-side conditional WHILE nodes (default), 1 = host-driven loop that synchronises
- * once per outer iteration (debug / drivers without conditional nodes).  Returns the previous mode. */
+/* How the iteration (Alg. 1) is driven; every mode runs the same per-cell arithmetic.
+ *   0  automatic (default): mode 3 for grids of up to 1.5 M padded cells, mode 2 above
+ *   1  host-driven loop that synchronises once per outer iteration (debug / per-kernel profiling)
+ *   2  CUDA graph with device-side conditional WHILE nodes around the tile kernels K2 / K3 / K4
+ *   3  one persistent cooperative kernel: phases separated by grid barriers that double as the reductions
+ *      (state is L2-resident; falls back to mode 2 if the device cannot co-schedule the grid)
+ * The environment variable OMNI_PERSIST_MAX_CELLS overrides the automatic threshold.  Modes 1 and 2 give bit-identical
+ * results; mode 3 sums its reductions in a different (fixed) order.  Returns the previous mode; other values are ignored. */
 int omni_set_loop_mode(int mode);
 /* Workspace of the non-_ws entry points comes from a library-owned stream-ordered memory pool (one per device) that
  * keeps freed blocks mapped between calls; this returns the unused memory to the driver. */

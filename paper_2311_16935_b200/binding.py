@@ -70,7 +70,8 @@ def launch_count(reset=False):
 
 
 def set_loop_mode(mode):
-    """0 = CUDA-graph loop (default), 1 = host-driven debug loop.  Returns the previous mode."""
+    """0 = automatic (default), 1 = host-driven debug loop, 2 = CUDA-graph loop, 3 = persistent cooperative kernel
+    (include/omni.h).  Returns the previous mode."""
     return int(lib().omni_set_loop_mode(C.c_int(mode)))
 
 

@@ -2,6 +2,7 @@
 // Host logic only: argument validation, geometry constants (a0), workspace carving, launch configuration and the
 // loop driver (CUDA graph with device-side conditional WHILE nodes, or a host-driven debug loop).
 #include "omni_tma.cuh"
+#include "omni_persist.cuh"
 #include "../../include/omni.h"
 
 #include <algorithm>
@@ -20,6 +21,8 @@ using namespace omni;
 #define OMNI_D3 6
 #define OMNI_D4 5
 #define OMNI_MINB 3
+#define OMNI_PERSIST_MAX_CELLS 1500000LL   // automatic mode: grids up to this many padded cells take the persistent loop
+#define OMNI_PERSIST_SMALL_CELLS 65536LL   // persistent loop: 512-thread CTAs up to here, 1024-thread CTAs above
 #endif
 
 namespace {
@@ -210,6 +213,7 @@ struct Workspace {
     uint8_t* link; uint32_t* wcode; uint32_t* flags; uint32_t* tflags;
     T *S, *r, *p0, *p1, *delta;
     double* P; double* P1; double* partial; Scalars* sc;
+    double* slots;                // exchange slots of the persistent loop's grid barrier
 };
 
 size_t partial_slots(const Geom& g)
@@ -241,7 +245,9 @@ size_t carve(const Geom& g, char* base, Workspace<T>* w)
     char* P1 = take(n * sizeof(double));
     char* partial = take(partial_slots(g) * sizeof(double));
     char* sc = take(sizeof(Scalars));
+    char* slots = take(PERSIST_SLOT_BYTES);
     if (w) {
+        w->slots = (double*)slots;
         w->link = (uint8_t*)link; w->wcode = (uint32_t*)wcode; w->flags = (uint32_t*)flags; w->tflags = (uint32_t*)tflags;
         w->S = (T*)S; w->r = (T*)r; w->p0 = (T*)p0; w->p1 = (T*)p1; w->delta = (T*)delta;
         w->P = (double*)P; w->P1 = (double*)P1; w->partial = (double*)partial; w->sc = (Scalars*)sc;
@@ -565,6 +571,67 @@ int run_loop_graph(const Geom& g, const Workspace<T>& w, const HostConst& H, con
     return rc;
 }
 
+// Persistent loop: the whole iteration in one cooperative launch (omni_persist.cuh).  Returns -100 if the device cannot
+// co-schedule the grid (the caller then falls back to the graph loop).  NT = threads per CTA: 512 (up to 128 registers)
+// for the smallest grids, where one row segment per warp is all there is; 1024 where a warp has several segments and
+// twice the warps in flight hide more of the L2 latency.
+template <typename T, int NT>
+int launch_persist(const Geom& g, const Workspace<T>& w, const HostConst& H, const Coef<T>& K, int nsm, cudaStream_t st)
+{
+    int occ = 0;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, persist_kernel<T, NT>, NT, 0) != cudaSuccess || occ < 1) {
+        cudaGetLastError();
+        return -100;
+    }
+    PersistArgs<T> a;
+    a.r = w.r; a.pbuf[0] = w.p0; a.pbuf[1] = w.p1; a.delta = w.delta; a.S = w.S; a.Pbuf[0] = w.P; a.Pbuf[1] = w.P1;
+    a.link = w.link; a.wcode = w.wcode; a.flags = w.flags; a.K = K;
+    for (int i = 0; i < 3; ++i) a.t[i] = H.F[i] / H.Atot;
+    a.sc = w.sc; a.slots = w.slots;
+    // one warp per 64-cell row segment of K2 (the finest phase), at most one CTA per SM, at most PERSIST_MAX_CTAS slots
+    const long long tasks = (long long)g.ny * g.nz * ((g.nx + 63) / 64);
+    const int nw = NT / 32;
+    long long G = (tasks + nw - 1) / nw;
+    if (G > nsm) G = nsm;
+    if (G > PERSIST_MAX_CTAS) G = PERSIST_MAX_CTAS;
+    if (G < 1) G = 1;
+    CK(cudaMemsetAsync(w.slots, 0, (size_t)8 * G * sizeof(double), st));
+    Geom gg = g;
+    void* params[2] = { (void*)&gg, (void*)&a };
+    CK(cudaLaunchCooperativeKernel((const void*)persist_kernel<T, NT>, dim3((unsigned)G), dim3(NT), params, 0, st));
+    g_launches.fetch_add(1, std::memory_order_relaxed);
+    return OMNI_OK;
+}
+
+template <typename T>
+int run_loop_persist(const Geom& g, const Workspace<T>& w, const HostConst& H, const Coef<T>& K, cudaStream_t st)
+{
+    static int nsm = 0, coop = 0;
+    if (nsm == 0) {
+        int dev = 0;
+        if (cudaGetDevice(&dev) != cudaSuccess) return OMNI_ERR_CUDA;
+        cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev);
+        cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
+    }
+    if (!coop || nsm < 1) return -100;
+    if ((long long)g.ny * g.nz * ((g.nx + 63) / 64) >= (1LL << 31)) return -100;      // 32-bit task indices
+    return (g.npad <= OMNI_PERSIST_SMALL_CELLS) ? launch_persist<T, 512>(g, w, H, K, nsm, st)
+                                                : launch_persist<T, 1024>(g, w, H, K, nsm, st);
+}
+
+// loop selection: g_loop_mode 0 = automatic (persistent kernel for grids up to OMNI_PERSIST_MAX_CELLS padded cells, CUDA graph above),
+// 1 = host-driven, 2 = CUDA graph, 3 = persistent kernel
+long long persist_max_cells()
+{
+    static long long v = -1;
+    if (v < 0) {
+        const char* e = getenv("OMNI_PERSIST_MAX_CELLS");
+        v = e ? atoll(e) : OMNI_PERSIST_MAX_CELLS;
+        if (v < 0) v = 0;
+    }
+    return v;
+}
+
 bool valid_common(int nx, int ny, int nz, double dx, double dy, double dz, double tol, int max_outer, int max_cg)
 {
     if (nx < 1 || ny < 1 || nz < 1) return false;
@@ -606,8 +673,14 @@ int solve_ws(int nx, int ny, int nz, double dx, double dy, double dz, const T* g
         g_launches.fetch_add(2, std::memory_order_relaxed);
     }
 
-    const int mode = g_loop_mode.load();
-    rc = (mode == 1) ? run_loop_host<T>(g, w, H, K, max_outer, max_cg, st) : run_loop_graph<T>(g, w, H, K, st);
+    int mode = g_loop_mode.load();
+    if (mode == 0) mode = (g.npad <= persist_max_cells()) ? 3 : 2;
+    if (mode == 3) {
+        rc = run_loop_persist<T>(g, w, H, K, st);
+        if (rc == -100) mode = 2;
+    }
+    if (mode == 1) rc = run_loop_host<T>(g, w, H, K, max_outer, max_cg, st);
+    else if (mode == 2) rc = run_loop_graph<T>(g, w, H, K, st);
     if (rc != OMNI_OK) return rc;
 
     finalize_kernel<T><<<blocks_for((long long)nx * ny * nz, 256), 256, 0, st>>>(g, w.P, w.P1, w.sc, w.link, P_out);
@@ -623,7 +696,7 @@ int solve_ws(int nx, int ny, int nz, double dx, double dy, double dz, const T* g
         info->norm_S = std::sqrt(h.normS2);
         info->eps_R_final = (h.normS2 > 0.0) ? std::sqrt(h.epsR2 / h.normS2) : 0.0;
         info->status = h.status;
-        if (mode != 1) g_launches.fetch_add((long long)(h.normS2 > 0.0 ? h.n + 1 : 0) + 2 * h.cg_total, std::memory_order_relaxed);
+        if (mode == 2) g_launches.fetch_add((long long)(h.normS2 > 0.0 ? h.n + 1 : 0) + 2 * h.cg_total, std::memory_order_relaxed);
         return h.status;
     }
     return OMNI_OK;
@@ -950,7 +1023,7 @@ void omni_release_memory(void)
 
 int omni_set_loop_mode(int mode)
 {
-    if (mode != 0 && mode != 1) return g_loop_mode.load();
+    if (mode < 0 || mode > 3) return g_loop_mode.load();
     return g_loop_mode.exchange(mode);
 }
 

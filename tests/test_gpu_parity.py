@@ -80,11 +80,19 @@ def test_source_and_operator_steps(oracle, dtype, shape, frac):
     assert eps == pytest.approx(np.linalg.norm(r_or) / np.linalg.norm(S_or), rel=1e-5 if dtype == "f32" else 1e-10)
 
 
-def _solve_both(oracle, f, dtype, tol, max_outer, max_cg, mask=None, nan_mask=False):
+LOOPS = {"graph": 2, "persistent": 3}       # omni_set_loop_mode; the default (0) picks one of the two by grid size
+
+
+def _solve_both(oracle, f, dtype, tol, max_outer, max_cg, mask=None, nan_mask=False, loop=None):
     g_dev, g_or, m_dev, m = _inputs(f, dtype, mask)
     d = f["d"]
-    P, info = omni.solve(g_dev[0], g_dev[1], g_dev[2], m_dev, d, tol, max_outer, max_cg)
-    torch.cuda.synchronize()
+    prev = omni.set_loop_mode(LOOPS[loop]) if loop else None
+    try:
+        P, info = omni.solve(g_dev[0], g_dev[1], g_dev[2], m_dev, d, tol, max_outer, max_cg)
+        torch.cuda.synchronize()
+    finally:
+        if loop:
+            omni.set_loop_mode(prev)
     Po, io = oracle.solve(g_or[0], g_or[1], g_or[2], m, *d, tol=tol, max_outer=max_outer, max_cg=max_cg)
     return P.cpu().numpy(), info, Po, io
 
@@ -95,15 +103,16 @@ TRAJ = [("gaussians2d", (64, 64), None), ("lamb_oseen2d", (150, 130), None), ("f
         ("gaussians2d", (21, 132), None), ("fourier3d", (9, 19, 66), None)]
 
 
+@pytest.mark.parametrize("loop", list(LOOPS))
 @pytest.mark.parametrize("dtype", ["f64", "f32"])
 @pytest.mark.parametrize("kind,shape,frac", TRAJ)
-def test_trajectory_parity(oracle, dtype, kind, shape, frac):
+def test_trajectory_parity(oracle, dtype, kind, shape, frac, loop):
     """Same inputs, tol = 0, fixed iteration counts: both sides execute identical steps (SURVEY 8c protocol i)."""
     f = make_field(kind, shape, seed=7, noise=0.05, kmax=4.0)
     mask = None
     if frac:
         mask = _random_mask(shape, 9, frac)
-    P, info, Po, io = _solve_both(oracle, f, dtype, 0.0, 6, 20, mask)
+    P, info, Po, io = _solve_both(oracle, f, dtype, 0.0, 6, 20, mask, loop=loop)
     valid = ~np.isnan(Po)
     assert np.array_equal(np.isnan(P), ~valid)
     assert info["outer_iters"] == io["outer_iters"] == 6
@@ -118,9 +127,10 @@ def test_trajectory_parity(oracle, dtype, kind, shape, frac):
 SMALL = [(4, 4, 4), (5, 4, 9), (3, 7, 12), (2, 6, 10), (4, 9), (3, 5), (2, 2), (6, 1, 7), (1, 1, 9), (7, 5, 4), (9, 4, 5)]
 
 
+@pytest.mark.parametrize("loop", list(LOOPS))
 @pytest.mark.parametrize("dtype", ["f64", "f32"])
 @pytest.mark.parametrize("shape", SMALL)
-def test_small_and_thin_grids(oracle, dtype, shape):
+def test_small_and_thin_grids(oracle, dtype, shape, loop):
     """Axes of length 1..5: every cell is a face / edge / corner cell, the per-axis face corrections overlap, and
     axes shorter than 4 fall back to flagged groups (coded path).  With and without a masked cell."""
     rng = np.random.default_rng(sum(shape))
@@ -133,7 +143,7 @@ def test_small_and_thin_grids(oracle, dtype, shape):
             mask[tuple(s // 2 for s in shape)] = 0
             if mask.sum() == 0:
                 continue
-        P, info, Po, io = _solve_both(oracle, f, dtype, 0.0, 4, 6, mask)
+        P, info, Po, io = _solve_both(oracle, f, dtype, 0.0, 4, 6, mask, loop=loop)
         valid = ~np.isnan(Po)
         assert np.array_equal(np.isnan(P), ~valid)
         assert info["cg_iters_total"] == io["cg_iters_total"]
@@ -142,8 +152,9 @@ def test_small_and_thin_grids(oracle, dtype, shape):
             assert np.abs(Pz - Poz).max() <= (1e-10 if dtype == "f64" else 2e-4) * np.abs(Poz).max(), (shape, with_mask)
 
 
+@pytest.mark.parametrize("loop", list(LOOPS))
 @pytest.mark.parametrize("seed", range(24))
-def test_fuzz_random_shapes_masks_spacings(oracle, seed):
+def test_fuzz_random_shapes_masks_spacings(oracle, seed, loop):
     """Seeded fuzz: random 2D/3D shapes (tile tails, pad-only chunks, thin axes), random mask densities including
     masks touching the box faces, random anisotropic spacing; operator, residual and a short solve against the oracle."""
     rng = np.random.default_rng(1000 + seed)
@@ -166,7 +177,7 @@ def test_fuzz_random_shapes_masks_spacings(oracle, seed):
     q, _ = omni.apply_M(p_dev, m_dev, d)
     q_or = oracle.apply_M(v, w1, p_or)
     assert np.abs(q.cpu().numpy() - q_or).max() <= TOL_STEP[dtype] * 8 * max(np.abs(q_or).max(), 1e-30), (shape, dtype)
-    P, info, Po, io = _solve_both(oracle, f, dtype, 0.0, 3, 5, mask)
+    P, info, Po, io = _solve_both(oracle, f, dtype, 0.0, 3, 5, mask, loop=loop)
     assert info["cg_iters_total"] == io["cg_iters_total"]
     assert np.array_equal(np.isnan(P), np.isnan(Po))
     scale = np.nanmax(np.abs(Po)) if np.isfinite(Po).any() else 0.0
@@ -243,7 +254,7 @@ def test_graph_and_host_loops_are_bit_identical():
     for dtype in ("f64", "f32"):
         g_dev, _, m_dev, _ = _inputs(f, dtype)
         res = []
-        for mode in (0, 1):
+        for mode in (2, 1):
             prev = omni.set_loop_mode(mode)
             try:
                 P, info = omni.solve(g_dev[0], g_dev[1], g_dev[2], m_dev, f["d"], 1e-4, 50, 12)
@@ -252,9 +263,53 @@ def test_graph_and_host_loops_are_bit_identical():
             res.append((P.cpu().numpy(), info))
         assert res[0][1] == res[1][1]
         assert np.array_equal(res[0][0], res[1][0], equal_nan=True)
-        # determinism: same call twice, same bits
-        P2, _ = omni.solve(g_dev[0], g_dev[1], g_dev[2], m_dev, f["d"], 1e-4, 50, 12)
-        assert np.array_equal(res[0][0], P2.cpu().numpy(), equal_nan=True)
+        # determinism: same call twice, same bits -- in the graph loop and in the persistent kernel, whose reductions
+        # run in another (fixed) order: same iteration counts, fields equal to rounding
+        for mode in (2, 3):
+            prev = omni.set_loop_mode(mode)
+            try:
+                Pa, ia = omni.solve(g_dev[0], g_dev[1], g_dev[2], m_dev, f["d"], 1e-4, 50, 12)
+                Pb, ib = omni.solve(g_dev[0], g_dev[1], g_dev[2], m_dev, f["d"], 1e-4, 50, 12)
+            finally:
+                omni.set_loop_mode(prev)
+            assert ia == ib and np.array_equal(Pa.cpu().numpy(), Pb.cpu().numpy(), equal_nan=True)
+            if mode == 2:
+                assert np.array_equal(res[0][0], Pa.cpu().numpy(), equal_nan=True)
+            else:
+                assert ia["outer_iters"] == res[0][1]["outer_iters"] and ia["cg_iters_total"] == res[0][1]["cg_iters_total"]
+                valid = ~np.isnan(res[0][0])
+                assert rel_l2_after_mean_removal(Pa.cpu().numpy(), res[0][0], valid) <= (1e-11 if dtype == "f64" else 1e-5)
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_persistent_loop_stress(dtype):
+    """The persistent kernel's grid barrier under every mix of phases (max_cg = 0, 1, 2, 3, 16: the outer and the
+    inner barriers interleave differently), on grids from one CTA to one CTA per SM, repeated: every repetition gives
+    the same bits, the same iteration counts as the graph loop, and the same field to rounding."""
+    cases = [("gaussians2d", (64, 64)), ("lamb_oseen2d", (700, 300)), ("sphere3d", (48, 40, 36)), ("fourier3d", (9, 19, 66))]
+    for kind, shape in cases:
+        f = make_field(kind, shape, seed=3, noise=0.05, kmax=4.0)
+        g_dev, _, m_dev, _ = _inputs(f, dtype)
+        for max_outer, max_cg in ((3, 0), (12, 1), (9, 2), (7, 3), (5, 16)):
+            out = {}
+            for mode, reps in ((2, 1), (3, 4)):
+                prev = omni.set_loop_mode(mode)
+                try:
+                    out[mode] = [omni.solve(g_dev[0], g_dev[1], g_dev[2], m_dev, f["d"], 0.0, max_outer, max_cg) for _ in range(reps)]
+                finally:
+                    omni.set_loop_mode(prev)
+            Pg, ig = out[2][0]
+            Pg = Pg.cpu().numpy()
+            valid = ~np.isnan(Pg)
+            P0 = out[3][0][0].cpu().numpy()
+            for P, info in out[3]:
+                assert info == out[3][0][1], (kind, shape, max_outer, max_cg)
+                assert np.array_equal(P.cpu().numpy(), P0, equal_nan=True), (kind, shape, max_outer, max_cg)
+            assert out[3][0][1]["cg_iters_total"] == ig["cg_iters_total"] and out[3][0][1]["outer_iters"] == ig["outer_iters"]
+            if max_cg > 0:
+                assert rel_l2_after_mean_removal(P0, Pg, valid) <= (1e-11 if dtype == "f64" else 1e-5), (kind, shape, max_outer, max_cg)
+            else:
+                assert np.array_equal(P0, Pg, equal_nan=True)
 
 
 def test_edge_cases(oracle):
