@@ -20,7 +20,8 @@
  * Pins (tests/test_oracle_*.py, all -m "not gpu"): Table 1 (:637-650), Eq. 5-7,
  * Eq. 17, Eq. 34-35, Eq. 49-50, the A_tot sum rule (:631), dense L^+ S fixed point,
  * dense LU inner solve, exactness on quadratics, 2nd-order refinement, Monte-Carlo
- * ray counts.  The per-iteration trajectory P^n (finite n) is "parity unpinned" by
+ * ray counts; oracle_solve_direct: dense pinv(L) S and the dense textbook CG iterates.
+ * The per-iteration trajectory P^n (finite n) is "parity unpinned" by
  * the paper (it prints no intermediate values); it is pinned only through the pins
  * of every operator that generates it.
  *
@@ -114,6 +115,8 @@ static double far_face_constant(double da, double db, double dc)
  * z index is then 0, so all weights across planes vanish (Eq. 16/18 with c_xz = c_yz = c_zz = 0, F_z = 0) and no other
  * routine needs to know.  The flag is set only inside oracle_solve_batch2d (test infrastructure: not thread safe). */
 static int g_batch2d = 0;
+/* set by oracle_solve_direct around solve_impl: the inner systems are L P = S instead of Eq. 12 */
+static int g_direct = 0;
 
 void oracle_constants(int nx, int ny, int nz, double dx, double dy, double dz, double *out)
 {
@@ -321,19 +324,35 @@ double oracle_dot(i64 N, int nx, const double *a, const double *b) { return dot(
 
 /* ------------------------------------------------------------------ inner CG (textbook recurrences, O6) */
 
-/* Solves M x = rhs starting from x (in/out).  Stops when sqrt(rho) <= thresh, rho == 0, or k == max_cg.
- * Work arrays r, p, q of size N.  Returns the number of iterations done. */
-int oracle_cg(int nx, int ny, int nz, const unsigned char *v, const double *w1, const double *rhs, double *x,
-              double thresh, int max_cg, double *r, double *p, double *q)
+/* q = A p with A = M = I - W1_off (Eq. 12 :119), or, for the fixed-point solve below, A = L = M - W^n: moving the
+ * boundary term W^n P of Eq. 12 to the left gives L P = S, the equation every fixed point of Alg. 1 satisfies
+ * (L_CC = sum_d v t_a, L_C,C+d = -v t_a: w1 + w0 = t_a on every valid link, Eq. 10 :109).  tmp: N work doubles. */
+static void apply_op(int direct, int nx, int ny, int nz, const unsigned char *v, const double *w1, const double *w0,
+                     const double *w0C, const double *p, double *q, double *tmp)
+{
+    oracle_apply_M(nx, ny, nz, v, w1, p, q);
+    if (direct) {
+        i64 N = (i64)nx * ny * nz;
+        oracle_apply_Wn(nx, ny, nz, v, w0, w0C, p, tmp);
+#pragma omp parallel for if (N > OMP_MIN_N)
+        for (i64 c = 0; c < N; ++c) q[c] -= tmp[c];
+    }
+}
+
+/* Solves A x = rhs starting from x (in/out).  Stops when sqrt(rho) <= thresh, rho == 0, or k == max_cg.
+ * Work arrays r, p, q (and tmp if direct) of size N.  Returns the number of iterations done. */
+static int cg_op(int direct, int nx, int ny, int nz, const unsigned char *v, const double *w1, const double *w0,
+                 const double *w0C, const double *rhs, double *x, double thresh, int max_cg, double *r, double *p,
+                 double *q, double *tmp)
 {
     i64 N = (i64)nx * ny * nz;
-    oracle_apply_M(nx, ny, nz, v, w1, x, q);
+    apply_op(direct, nx, ny, nz, v, w1, w0, w0C, x, q, tmp);
 #pragma omp parallel for if (N > OMP_MIN_N)
     for (i64 c = 0; c < N; ++c) { r[c] = rhs[c] - q[c]; p[c] = r[c]; }
     double rho = dot(N, nx, r, r);
     int k = 0;
     while (sqrt(rho) > thresh && rho != 0.0 && k < max_cg) {
-        oracle_apply_M(nx, ny, nz, v, w1, p, q);
+        apply_op(direct, nx, ny, nz, v, w1, w0, w0C, p, q, tmp);
         double alpha = rho / dot(N, nx, p, q);
 #pragma omp parallel for if (N > OMP_MIN_N)
         for (i64 c = 0; c < N; ++c) { x[c] += alpha * p[c]; r[c] -= alpha * q[c]; }
@@ -345,6 +364,12 @@ int oracle_cg(int nx, int ny, int nz, const unsigned char *v, const double *w1, 
         ++k;
     }
     return k;
+}
+
+int oracle_cg(int nx, int ny, int nz, const unsigned char *v, const double *w1, const double *rhs, double *x,
+              double thresh, int max_cg, double *r, double *p, double *q)
+{
+    return cg_op(0, nx, ny, nz, v, w1, NULL, NULL, rhs, x, thresh, max_cg, r, p, q, NULL);
 }
 
 /* ------------------------------------------------------------------ Algorithm 1 (:128-150) */
@@ -370,6 +395,21 @@ int oracle_solve(int nx, int ny, int nz, double dx, double dy, double dz,
                  double *hist, int hist_cap)
 {
     return solve_impl(nx, ny, nz, dx, dy, dz, gx, gy, gz, mask, NULL, P_out, tol, max_outer, max_cg, info, hist, hist_cap);
+}
+
+/* The fixed point of Alg. 1 computed without the boundary iteration: at convergence P^{n+1} = P^n, so Eq. 12 reads
+ * (M - W^n) P = S, i.e. L P = S with L the symmetric positive semi-definite weighted graph Laplacian of the valid
+ * cells (constant null space per connected component; S sums to zero on each).  CG on it from P = 0 returns the
+ * solution with zero mean on every component.  NOT the paper's algorithm (SURVEY 8(f) NEXT-2 iii): same converged
+ * field, a different iteration.  Same arguments and stopping rules as oracle_solve. */
+int oracle_solve_direct(int nx, int ny, int nz, double dx, double dy, double dz,
+                        const double *gx, const double *gy, const double *gz, const unsigned char *mask,
+                        double *P_out, double tol, int max_outer, int max_cg, oracle_info *info)
+{
+    g_direct = 1;
+    int rc = solve_impl(nx, ny, nz, dx, dy, dz, gx, gy, gz, mask, NULL, P_out, tol, max_outer, max_cg, info, NULL, 0);
+    g_direct = 0;
+    return rc;
 }
 
 /* nb snapshots [nb][ny][nx] on one mask [ny][nx] (NULL = all valid), optional first guess P_init [nb][ny][nx]
@@ -403,8 +443,9 @@ static int solve_impl(int nx, int ny, int nz, double dx, double dy, double dz,
     double *w1 = (double *)malloc(6 * nb), *w0 = (double *)malloc(6 * nb), *w0C = (double *)malloc(nb);
     double *S = (double *)malloc(nb), *P = (double *)calloc((size_t)N, sizeof(double));
     double *rhs = (double *)malloc(nb), *r = (double *)malloc(nb), *p = (double *)malloc(nb), *q = (double *)malloc(nb);
+    double *tmp = (double *)malloc(nb);
     int rc = -1;
-    if (!v || !w1 || !w0 || !w0C || !S || !P || !rhs || !r || !p || !q) goto done;
+    if (!v || !w1 || !w0 || !w0C || !S || !P || !rhs || !r || !p || !q || !tmp) goto done;
     rc = 0;
 
     oracle_validity(nx, ny, nz, gx, gy, gz, mask, v);
@@ -427,8 +468,11 @@ static int solve_impl(int nx, int ny, int nz, double dx, double dy, double dz,
             epsR = sqrt(dot(N, nx, r, r)) / normS;
             if (hist && n < hist_cap) hist[n] = epsR;
             if (epsR <= tol || n == max_outer) break;
-            /* Solve Eq. 12 for P^{n+1} by CG, first guess P^n (:489); inner threshold: reading A3 */
-            cg_total += oracle_cg(nx, ny, nz, v, w1, rhs, P, 0.1 * tol * normS, max_cg, r, p, q);
+            /* Solve Eq. 12 for P^{n+1} by CG, first guess P^n (:489); inner threshold: reading A3.
+             * Fixed-point variant (oracle_solve_direct): the same loop with the system L P = S; eps_R above is its
+             * residual too (r0 = S - L P^n), so the outer loop only restarts a CG that hit max_cg. */
+            if (g_direct) memcpy(rhs, S, nb);
+            cg_total += cg_op(g_direct, nx, ny, nz, v, w1, w0, w0C, rhs, P, 0.1 * tol * normS, max_cg, r, p, q, tmp);
             ++n;
         }
     }
@@ -438,7 +482,7 @@ static int solve_impl(int nx, int ny, int nz, double dx, double dy, double dz,
         info->norm_S = normS; info->converged = (epsR <= tol);
     }
 done:
-    free(v); free(w1); free(w0); free(w0C); free(S); free(P); free(rhs); free(r); free(p); free(q);
+    free(v); free(w1); free(w0); free(w0C); free(S); free(P); free(rhs); free(r); free(p); free(q); free(tmp);
     return rc;
 }
 

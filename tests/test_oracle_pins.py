@@ -384,6 +384,74 @@ def test_outer_iteration_vs_dense_solves(oracle, shape, sp):
     assert np.linalg.norm(a - b) / np.linalg.norm(b) < 1e-8
 
 
+def _dense_laplacian(v, t):
+    """L from its definition (valid links carry t_a = F_a / A_tot), independent of the oracle's weights."""
+    shape, nd = v.shape, v.ndim
+    idx = np.arange(v.size).reshape(shape)
+    L = np.zeros((v.size, v.size))
+    for C in np.ndindex(shape):
+        if not v[C]:
+            continue
+        for a in range(nd):
+            for sg in (1, -1):
+                Q = list(C); Q[nd - 1 - a] += sg
+                if 0 <= Q[nd - 1 - a] < shape[nd - 1 - a] and v[tuple(Q)]:
+                    L[idx[C], idx[C]] += t[a]
+                    L[idx[C], idx[tuple(Q)]] -= t[a]
+    return L
+
+
+@pytest.mark.parametrize("shape,sp", [((9, 10), (1.0, 0.6, 1.0)), ((5, 5, 6), (1.0, 1.3, 0.8))])
+def test_direct_solve_vs_dense_pseudo_inverse(oracle, shape, sp):
+    """oracle.solve_direct (CG on L P = S from P = 0, SURVEY 8(f) NEXT-2 iii) returns pinv(L) S -- the solution with
+    zero mean on every connected component -- with L assembled here from its definition; its truncated iterates are the
+    textbook CG iterates of that dense system (numpy recurrence); and its limit is the fixed point Algorithm 1 reaches."""
+    rng = np.random.default_rng(9)
+    f = make_field("gaussians2d" if len(shape) == 2 else "fourier3d", shape, seed=2, noise=0.05, kmax=2.0)
+    mask = (rng.random(shape) > 0.12).astype(np.uint8)
+    g = f["g"] + [None] * (3 - len(f["g"]))
+    v = oracle.validity(g[0], g[1], g[2], mask)
+    w1, w0, w0C = oracle.weights(v, *sp)
+    S = oracle.source(v, w1, w0, g[0], g[1], g[2], *sp)
+    K = oracle.constants(shape[-1], shape[-2], shape[0] if len(shape) == 3 else 1, *sp)
+    keep = v.ravel() == 1
+    Lk = _dense_laplacian(v, K["F"] / K["A_tot"])[np.ix_(keep, keep)]
+    Sk = S.ravel()[keep]
+    Pstar = np.linalg.pinv(Lk, rcond=1e-12) @ Sk
+    Po, info = oracle.solve_direct(g[0], g[1], g[2], mask, *sp, tol=1e-12, max_outer=5, max_cg=2000)
+    assert info["converged"] and info["outer_iters"] == 1
+    assert np.all(np.isnan(Po.ravel()[~keep]))
+    assert np.linalg.norm(Po.ravel()[keep] - Pstar) / np.linalg.norm(Pstar) < 1e-9
+    # truncated: k textbook CG steps on the dense system
+    for k in (1, 3, 7):
+        x = np.zeros_like(Sk); r = Sk.copy(); pv = r.copy(); rho = r @ r
+        for _ in range(k):
+            q = Lk @ pv
+            al = rho / (pv @ q)
+            x += al * pv; r -= al * q
+            rho1 = r @ r
+            pv = r + (rho1 / rho) * pv
+            rho = rho1
+        Pk, ik = oracle.solve_direct(g[0], g[1], g[2], mask, *sp, tol=0.0, max_outer=1, max_cg=k)
+        assert ik["cg_iters_total"] == k
+        assert np.linalg.norm(Pk.ravel()[keep] - x) / np.linalg.norm(x) < 1e-11
+    # restart: max_cg = 4 with several outer iterations continues to the same limit
+    Pr, ir = oracle.solve_direct(g[0], g[1], g[2], mask, *sp, tol=1e-9, max_outer=10000, max_cg=4)
+    assert ir["converged"]
+    # the two-level iteration converges to the same field up to a constant per connected component
+    P2, i2 = oracle.solve(g[0], g[1], g[2], mask, *sp, tol=1e-11, max_outer=20000, max_cg=400)
+    assert i2["converged"]
+    from scipy.sparse import csr_matrix
+    from scipy.sparse.csgraph import connected_components
+    ncomp, lab = connected_components(csr_matrix(np.abs(Lk) > 0), directed=False)
+    for other, bound in ((P2, 1e-8), (Pr, 1e-6)):
+        a, b = other.ravel()[keep].copy(), Pstar.copy()
+        for cpt in range(ncomp):
+            m = lab == cpt
+            a[m] -= a[m].mean(); b[m] -= b[m].mean()
+        assert np.linalg.norm(a - b) / np.linalg.norm(b) < bound
+
+
 # ----------------------------------------------------------------------------- analytic pins (P7, P8, P9)
 
 @pytest.mark.parametrize("shape,sp", [((12, 10), (0.1, 0.07, 1.0)), ((7, 8, 6), (0.2, 0.15, 0.3))])
