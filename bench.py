@@ -45,6 +45,8 @@ def parse():
                     help="instead of the fixed-cap step: time ONE solve to the config's tolerance (BASELINE.md table)")
     ap.add_argument("--max-cg", type=int, default=1000, help="--converge: CG cap per outer iteration")
     ap.add_argument("--max-outer", type=int, default=200000, help="--converge: outer iteration cap")
+    ap.add_argument("--direct", action="store_true",
+                    help="--converge: omni_solve_direct (CG on the fixed-point system L P = S) instead of Algorithm 1")
     ap.add_argument("--batch", type=int, default=1,
                     help="--converge on a 2D config: solve this many snapshots (same mask, different noise seeds) in one "
                          "omni_solve_batch2d call")
@@ -80,10 +82,11 @@ def converge(args, cfg, dtype):
         f = make_config(args.config, device="cuda")
         g = [torch.from_numpy(c).to(tdt).cuda() for c in f["g"]] + [None] * (3 - len(f["g"]))
         m = None if f["mask"] is None else torch.from_numpy(f["mask"]).cuda()
-        omni.solve(g[0], g[1], g[2], m, f["d"], tol, 2, 2)                       # warm-up (module load, pool)
+        fn = omni.solve_direct if args.direct else omni.solve
+        fn(g[0], g[1], g[2], m, f["d"], tol, 2, 2)                               # warm-up (module load, pool)
         torch.cuda.synchronize()
         e0.record()
-        P, info = omni.solve(g[0], g[1], g[2], m, f["d"], tol, args.max_outer, args.max_cg)
+        P, info = fn(g[0], g[1], g[2], m, f["d"], tol, args.max_outer, args.max_cg)
         e1.record()
         torch.cuda.synchronize()
         Pn = P.double().cpu().numpy()
@@ -92,7 +95,7 @@ def converge(args, cfg, dtype):
     valid = ~np.isnan(Pn)
     a, b = Pn[valid] - Pn[valid].mean(), f["P"][valid] - f["P"][valid].mean()
     print(json.dumps({"converge": True, "workload": f"configs[{args.config}] {cfg['kind']} {cfg['n']} {dtype}", "tol": tol,
-                      "max_cg": args.max_cg, "batch": args.batch, "outer_iters": info["outer_iters"], "cg_iters": info["cg_iters_total"],
+                      "max_cg": args.max_cg, "batch": args.batch, "direct": bool(args.direct), "outer_iters": info["outer_iters"], "cg_iters": info["cg_iters_total"],
                       "seconds": sec, "eps_R": info["eps_R_final"], "status": info["status"],
                       "updates_per_s": N * info["cg_iters_total"] / sec,
                       "rel_l2_vs_analytic_P": float(np.linalg.norm(a - b) / np.linalg.norm(b))}))

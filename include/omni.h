@@ -87,6 +87,23 @@ int omni_solve_host_f32(int nx, int ny, int nz, double dx, double dy, double dz,
                         const float* h_gx, const float* h_gy, const float* h_gz, const unsigned char* h_mask,
                         float* h_P_out, double tol, int max_outer, int max_cg, void* stream, omni_info* info);
 
+/* ---- fixed point of Algorithm 1 without the boundary iteration (SURVEY.md 8(f) NEXT-2 iii) -----------------------------
+ * NOT the paper's iteration: at a fixed point P^{n+1} = P^n of Alg. 1, Eq. 12 reads (M - W^n) P = S,
+ * i.e. L P = S with L the symmetric positive semi-definite weighted graph Laplacian of the valid cells
+ * ((L P)_C = sum_d v(C+d) (F_a / A_tot) (P_C - P_{C+d}), Eq. 10 :109: w^{n+1} + w^n = F_a / A_tot on a valid link).
+ * These entry points run CG on that system directly -- same kernels, same S, same stopping rules, the CG kernels
+ * applying L instead of M -- inside the same outer loop, which here is an fp64 iterative refinement (the true
+ * residual S - L P is re-evaluated from the fp64 master pressure, eps_R of Eq. 41, and the CG restarted on it).
+ * It returns the field Alg. 1 converges to (zero mean on every connected component) in O(n) instead of O(n^2) CG
+ * iterations for an n-cell-wide domain.  Typical caps: max_outer 10, max_cg a few thousand.  Arguments, layout,
+ * ownership, status codes and omni_info as omni_solve_*. */
+int omni_solve_direct_f64(int nx, int ny, int nz, double dx, double dy, double dz,
+                          const double* d_gx, const double* d_gy, const double* d_gz, const unsigned char* d_mask,
+                          double* d_P_out, double tol, int max_outer, int max_cg, void* stream, omni_info* info);
+int omni_solve_direct_f32(int nx, int ny, int nz, double dx, double dy, double dz,
+                          const float* d_gx, const float* d_gy, const float* d_gz, const unsigned char* d_mask,
+                          float* d_P_out, double tol, int max_outer, int max_cg, void* stream, omni_info* info);
+
 /* ---- batched 2D snapshots with an optional first guess (SURVEY.md 8(f) NEXT-1; time-resolved PIV: PAPER.md:365, :503) ----
  * nb independent 2D gradient fields [nb][ny][nx] on ONE mask [ny][nx] (NULL = all valid) are stacked and solved as one
  * block-diagonal system with the 2D scheme: stencil codes are built once, every stencil sweep serves all snapshots,

@@ -270,8 +270,8 @@ struct MarchCfg { dim3 grid, block; int zlen; };
 
 // K2 / K3 / K4: TMA + mbarrier pipeline (omni_tma.cuh): 512-byte x 8-row tiles, 8 consumer warps + 1 producer warp,
 // several CTAs per SM (shared memory: K3 6 stages x 10.8 KB, K4 5 x 13.4 KB, K2 5 x 10.3 KB fp32 / 4 x 14.8 KB fp64).
-template <typename T> using K3 = OpT3<T, OMNI_BY, OMNI_D3, OMNI_MINB>;
-template <typename T> using K4 = OpT4<T, OMNI_BY, OMNI_D4, (sizeof(T) == 8 ? 2 : OMNI_MINB)>;   // fp64 K4: 72 registers spill
+template <typename T, bool LOP = false> using K3 = OpT3<T, OMNI_BY, OMNI_D3, OMNI_MINB, LOP>;
+template <typename T, bool LOP = false> using K4 = OpT4<T, OMNI_BY, OMNI_D4, (sizeof(T) == 8 ? 2 : OMNI_MINB), LOP>;   // fp64 K4: 72 registers spill
 template <typename T> using K2 = OpT2<T, OMNI_BY, (sizeof(T) == 8 ? 4 : 5), OMNI_MINB>;
 
 
@@ -399,19 +399,19 @@ typename K2<T>::Args k2_args(const Geom& g, const Workspace<T>& w, const HostCon
     a.sc = w.sc; a.partial = w.partial; a.cond = ch; a.fold_delta = fold;
     return a;
 }
-template <typename T>
-typename K3<T>::Args k3_args(const Workspace<T>& w, const Coef<T>& K, CondHandles ch)
+template <typename T, bool LOP = false>
+typename K3<T, LOP>::Args k3_args(const Workspace<T>& w, const Coef<T>& K, CondHandles ch)
 {
-    typename K3<T>::Args a;
-    a.pbuf[0] = w.p0; a.pbuf[1] = w.p1; a.wcode = w.wcode; a.flags = w.flags; a.tflags = w.tflags;
+    typename K3<T, LOP>::Args a;
+    a.pbuf[0] = w.p0; a.pbuf[1] = w.p1; a.wcode = w.wcode; a.link = w.link; a.flags = w.flags; a.tflags = w.tflags;
     a.K = K; a.sc = w.sc; a.partial = w.partial; a.cond = ch;
     return a;
 }
-template <typename T>
-typename K4<T>::Args k4_args(const Workspace<T>& w, const Coef<T>& K, CondHandles ch)
+template <typename T, bool LOP = false>
+typename K4<T, LOP>::Args k4_args(const Workspace<T>& w, const Coef<T>& K, CondHandles ch)
 {
-    typename K4<T>::Args a;
-    a.r = w.r; a.delta = w.delta; a.p_fixed = -1; a.wcode = w.wcode; a.flags = w.flags; a.tflags = w.tflags;
+    typename K4<T, LOP>::Args a;
+    a.r = w.r; a.delta = w.delta; a.p_fixed = -1; a.wcode = w.wcode; a.link = w.link; a.flags = w.flags; a.tflags = w.tflags;
     a.K = K; a.sc = w.sc; a.partial = w.partial; a.cond = ch; a.q_out = nullptr;
     return a;
 }
@@ -431,14 +431,14 @@ bool make_tma_set(const Geom& g, const Workspace<T>& w, TmaSet& m)
 // ------------------------------------------------------------------------------------------------ loop drivers
 
 // Host-driven loop (debug / profiling): one synchronisation per outer iteration (plus one per 16 CG iterations).
-template <typename T>
+template <typename T, bool LOP>
 int run_loop_host(const Geom& g, const Workspace<T>& w, const HostConst& H, const Coef<T>& K, int max_outer, int max_cg,
                   cudaStream_t st)
 {
     CondHandles ch{ 0, 0, 0 };
     const auto a2 = k2_args<T>(g, w, H, ch, 1);
-    const auto a3 = k3_args<T>(w, K, ch);
-    const auto a4 = k4_args<T>(w, K, ch);
+    const auto a3 = k3_args<T, LOP>(w, K, ch);
+    const auto a4 = k4_args<T, LOP>(w, K, ch);
     TmaSet maps;
     if (!make_tma_set<T>(g, w, maps)) return OMNI_ERR_CUDA;
     const bool prof = g_profile.load() != 0;
@@ -468,8 +468,8 @@ int run_loop_host(const Geom& g, const Workspace<T>& w, const HostConst& H, cons
         while (done < max_cg) {
             const int batch = (max_cg - done < 16) ? (max_cg - done) : 16;
             for (int c = 0; c < batch; ++c) {
-                if (timed(1, [&] { return launch_tma<K3<T>>(g, a3, maps, st); }) != cudaSuccess) rc = OMNI_ERR_CUDA;
-                if (timed(2, [&] { return launch_tma<K4<T>>(g, a4, maps, st); }) != cudaSuccess) rc = OMNI_ERR_CUDA;
+                if (timed(1, [&] { return launch_tma<K3<T, LOP>>(g, a3, maps, st); }) != cudaSuccess) rc = OMNI_ERR_CUDA;
+                if (timed(2, [&] { return launch_tma<K4<T, LOP>>(g, a4, maps, st); }) != cudaSuccess) rc = OMNI_ERR_CUDA;
             }
             done += batch;
             if (rc != OMNI_OK) break;
@@ -507,7 +507,7 @@ int run_loop_host(const Geom& g, const Workspace<T>& w, const HostConst& H, cons
 }
 
 // CUDA-graph loop: outer WHILE { K2 ; inner WHILE { K3 ; K4 } }, conditions written by the kernels' last CTAs.
-template <typename T>
+template <typename T, bool LOP>
 int run_loop_graph(const Geom& g, const Workspace<T>& w, const HostConst& H, const Coef<T>& K, cudaStream_t st)
 {
     cudaGraph_t G = nullptr;
@@ -515,7 +515,7 @@ int run_loop_graph(const Geom& g, const Workspace<T>& w, const HostConst& H, con
     cudaStream_t cap = nullptr;
     int rc = OMNI_ERR_CUDA;
     // occupancy queries happen here, outside any stream capture (results are cached per kernel)
-    (void)tma_config<K2<T>>(g); (void)tma_config<K3<T>>(g); (void)tma_config<K4<T>>(g);
+    (void)tma_config<K2<T>>(g); (void)tma_config<K3<T, LOP>>(g); (void)tma_config<K4<T, LOP>>(g);
     TmaSet maps;
     if (!make_tma_set<T>(g, w, maps)) return OMNI_ERR_CUDA;
     do {
@@ -554,8 +554,8 @@ int run_loop_graph(const Geom& g, const Workspace<T>& w, const HostConst& H, con
         cudaGraph_t bodyInner = pi.conditional.phGraph_out[0];
 
         if (cudaStreamBeginCaptureToGraph(cap, bodyInner, nullptr, nullptr, 0, cudaStreamCaptureModeThreadLocal) != cudaSuccess) break;
-        cudaError_t e3 = launch_tma<K3<T>>(g, k3_args<T>(w, K, ch), maps, cap);
-        cudaError_t e4 = launch_tma<K4<T>>(g, k4_args<T>(w, K, ch), maps, cap);
+        cudaError_t e3 = launch_tma<K3<T, LOP>>(g, k3_args<T, LOP>(w, K, ch), maps, cap);
+        cudaError_t e4 = launch_tma<K4<T, LOP>>(g, k4_args<T, LOP>(w, K, ch), maps, cap);
         if (cudaStreamEndCapture(cap, &tmp) != cudaSuccess || e3 != cudaSuccess || e4 != cudaSuccess) break;
         g_launches.fetch_sub(3, std::memory_order_relaxed);     // captured, not launched; counted from the device state
 
@@ -575,11 +575,11 @@ int run_loop_graph(const Geom& g, const Workspace<T>& w, const HostConst& H, con
 // co-schedule the grid (the caller then falls back to the graph loop).  NT = threads per CTA: 512 (up to 128 registers)
 // for the smallest grids, where one row segment per warp is all there is; 1024 where a warp has several segments and
 // twice the warps in flight hide more of the L2 latency.
-template <typename T, int NT>
+template <typename T, int NT, bool LOP>
 int launch_persist(const Geom& g, const Workspace<T>& w, const HostConst& H, const Coef<T>& K, int nsm, cudaStream_t st)
 {
     int occ = 0;
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, persist_kernel<T, NT>, NT, 0) != cudaSuccess || occ < 1) {
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, persist_kernel<T, NT, LOP>, NT, 0) != cudaSuccess || occ < 1) {
         cudaGetLastError();
         return -100;
     }
@@ -598,12 +598,12 @@ int launch_persist(const Geom& g, const Workspace<T>& w, const HostConst& H, con
     CK(cudaMemsetAsync(w.slots, 0, (size_t)8 * G * sizeof(double), st));
     Geom gg = g;
     void* params[2] = { (void*)&gg, (void*)&a };
-    CK(cudaLaunchCooperativeKernel((const void*)persist_kernel<T, NT>, dim3((unsigned)G), dim3(NT), params, 0, st));
+    CK(cudaLaunchCooperativeKernel((const void*)persist_kernel<T, NT, LOP>, dim3((unsigned)G), dim3(NT), params, 0, st));
     g_launches.fetch_add(1, std::memory_order_relaxed);
     return OMNI_OK;
 }
 
-template <typename T>
+template <typename T, bool LOP>
 int run_loop_persist(const Geom& g, const Workspace<T>& w, const HostConst& H, const Coef<T>& K, cudaStream_t st)
 {
     static int nsm = 0, coop = 0;
@@ -615,8 +615,8 @@ int run_loop_persist(const Geom& g, const Workspace<T>& w, const HostConst& H, c
     }
     if (!coop || nsm < 1) return -100;
     if ((long long)g.ny * g.nz * ((g.nx + 63) / 64) >= (1LL << 31)) return -100;      // 32-bit task indices
-    return (g.npad <= OMNI_PERSIST_SMALL_CELLS) ? launch_persist<T, 512>(g, w, H, K, nsm, st)
-                                                : launch_persist<T, 1024>(g, w, H, K, nsm, st);
+    return (g.npad <= OMNI_PERSIST_SMALL_CELLS) ? launch_persist<T, 512, LOP>(g, w, H, K, nsm, st)
+                                                : launch_persist<T, 1024, LOP>(g, w, H, K, nsm, st);
 }
 
 // loop selection: g_loop_mode 0 = automatic (persistent kernel for grids up to OMNI_PERSIST_MAX_CELLS padded cells, CUDA graph above),
@@ -644,7 +644,7 @@ bool valid_common(int nx, int ny, int nz, double dx, double dy, double dz, doubl
 template <typename T>
 int solve_ws(int nx, int ny, int nz, double dx, double dy, double dz, const T* gx, const T* gy, const T* gz,
              const unsigned char* mask, T* P_out, double tol, int max_outer, int max_cg, void* ws, size_t ws_bytes,
-             void* stream, omni_info* info, int batch = 0, const T* P_init = nullptr)
+             void* stream, omni_info* info, int batch = 0, const T* P_init = nullptr, int lop = 0)
 {
     Geom g;
     if (!valid_common(nx, ny, batch ? 1 : nz, dx, dy, dz, tol, max_outer, max_cg) || !make_geom(nx, ny, nz, (int)sizeof(T), g, batch)) return OMNI_ERR_INVALID_ARG;
@@ -675,12 +675,13 @@ int solve_ws(int nx, int ny, int nz, double dx, double dy, double dz, const T* g
 
     int mode = g_loop_mode.load();
     if (mode == 0) mode = (g.npad <= persist_max_cells()) ? 3 : 2;
+    // lop: the CG kernels apply L instead of M (omni_solve_direct); everything else -- K2, scalars, loop control -- is shared
     if (mode == 3) {
-        rc = run_loop_persist<T>(g, w, H, K, st);
+        rc = lop ? run_loop_persist<T, true>(g, w, H, K, st) : run_loop_persist<T, false>(g, w, H, K, st);
         if (rc == -100) mode = 2;
     }
-    if (mode == 1) rc = run_loop_host<T>(g, w, H, K, max_outer, max_cg, st);
-    else if (mode == 2) rc = run_loop_graph<T>(g, w, H, K, st);
+    if (mode == 1) rc = lop ? run_loop_host<T, true>(g, w, H, K, max_outer, max_cg, st) : run_loop_host<T, false>(g, w, H, K, max_outer, max_cg, st);
+    else if (mode == 2) rc = lop ? run_loop_graph<T, true>(g, w, H, K, st) : run_loop_graph<T, false>(g, w, H, K, st);
     if (rc != OMNI_OK) return rc;
 
     finalize_kernel<T><<<blocks_for((long long)nx * ny * nz, 256), 256, 0, st>>>(g, w.P, w.P1, w.sc, w.link, P_out);
@@ -705,7 +706,7 @@ int solve_ws(int nx, int ny, int nz, double dx, double dy, double dz, const T* g
 template <typename T>
 int solve_alloc(int nx, int ny, int nz, double dx, double dy, double dz, const T* gx, const T* gy, const T* gz,
                 const unsigned char* mask, T* P_out, double tol, int max_outer, int max_cg, void* stream, omni_info* info,
-                int batch = 0, const T* P_init = nullptr)
+                int batch = 0, const T* P_init = nullptr, int lop = 0)
 {
     Geom g;
     if (!valid_common(nx, ny, batch ? 1 : nz, dx, dy, dz, tol, max_outer, max_cg) || !make_geom(nx, ny, nz, (int)sizeof(T), g, batch)) return OMNI_ERR_INVALID_ARG;
@@ -714,7 +715,7 @@ int solve_alloc(int nx, int ny, int nz, double dx, double dy, double dz, const T
     void* ws = nullptr;
     if (pool_alloc(&ws, bytes, st) != cudaSuccess) { cudaGetLastError(); return OMNI_ERR_ALLOC; }
     int rc = solve_ws<T>(nx, ny, nz, dx, dy, dz, gx, gy, gz, mask, P_out, tol, max_outer, max_cg, ws, bytes, stream, info,
-                         batch, P_init);
+                         batch, P_init, lop);
     cudaFreeAsync(ws, st);
     return rc;
 }
@@ -946,6 +947,22 @@ int omni_solve_batch2d_f32(int nx, int ny, int nb, double dx, double dy, const f
     if (!d_gx || !d_gy || !d_P_out || nb < 1) return OMNI_ERR_INVALID_ARG;
     return solve_alloc<float>(nx, ny, nb, dx, dy, 1.0, d_gx, d_gy, nullptr, d_mask2d, d_P_out, tol, max_outer, max_cg, stream,
                               info, 1, d_P_init);
+}
+
+int omni_solve_direct_f64(int nx, int ny, int nz, double dx, double dy, double dz, const double* d_gx, const double* d_gy,
+                          const double* d_gz, const unsigned char* d_mask, double* d_P_out, double tol, int max_outer,
+                          int max_cg, void* stream, omni_info* info)
+{
+    return solve_alloc<double>(nx, ny, nz, dx, dy, dz, d_gx, d_gy, d_gz, d_mask, d_P_out, tol, max_outer, max_cg, stream, info,
+                               0, nullptr, 1);
+}
+
+int omni_solve_direct_f32(int nx, int ny, int nz, double dx, double dy, double dz, const float* d_gx, const float* d_gy,
+                          const float* d_gz, const unsigned char* d_mask, float* d_P_out, double tol, int max_outer,
+                          int max_cg, void* stream, omni_info* info)
+{
+    return solve_alloc<float>(nx, ny, nz, dx, dy, dz, d_gx, d_gy, d_gz, d_mask, d_P_out, tol, max_outer, max_cg, stream, info,
+                              0, nullptr, 1);
 }
 
 int omni_constants(int nx, int ny, int nz, double dx, double dy, double dz, double* h_out13)

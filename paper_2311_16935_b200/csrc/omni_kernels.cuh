@@ -272,6 +272,83 @@ __device__ __forceinline__ void apply_M_chunk(T (&q)[V], const T (&vm)[V], const
     }
 }
 
+// q = L p for the V cells of one thread, (L p)_C = sum_d v(C+d) t_a (p_C - p_{C+d}): the operator of the fixed-point
+// system L P = S (M - W^n of Eq. 12 :119 at P^{n+1} = P^n), used by omni_solve_direct.  Unflagged chunks have the
+// links of the mask-free box: the interior formula already sees zeros beyond the faces (TMA zero fill, pad cells), so
+// only the diagonal loses t_a per missing face link.  Flagged chunks: lk[i] = link byte of cell i.
+template <typename T, int V>
+__device__ __forceinline__ void apply_L_chunk(T (&q)[V], const T (&vm)[V], const T (&vc)[V], const T (&vp)[V],
+                                              const T (&vn)[V], const T (&vs)[V], T xl, T xr, uint32_t fb,
+                                              const uint32_t (&lk)[V], const Coef<T>& K,
+                                              const XEdge& xe, int ycls, int zcls)
+{
+    if (fb == 0) {
+        T dg = T(0);
+        if (ycls == 0 || ycls == 3) dg += K.t[1];
+        if (zcls == 0 || zcls == 3) dg += K.t[2];
+#pragma unroll
+        for (int i = 0; i < V; ++i) {
+            T w = (i == 0) ? xl : vc[i - 1];
+            T e = (i == V - 1) ? xr : vc[i + 1];
+            q[i] = apply_M_interior(vc[i], e, w, vn[i], vs[i], vp[i], vm[i], K) - dg * vc[i];
+        }
+        if (xe.any) {
+            if (xe.L) q[0] -= K.t[0] * vc[0];
+            if (xe.B) {
+#pragma unroll
+                for (int i = 0; i < V; ++i) {
+                    if (i == xe.posB) q[i] -= K.t[0] * vc[i];
+                    if (i > xe.posB) q[i] = T(0);                 // pad cells nx..px-1
+                }
+            }
+        }
+    } else {
+#pragma unroll
+        for (int i = 0; i < V; ++i) {
+            T w = (i == 0) ? xl : vc[i - 1];
+            T e = (i == V - 1) ? xr : vc[i + 1];
+            const uint32_t l = lk[i];
+            T acc = T(0);
+            if (l & 1u) acc += K.t[0] * (vc[i] - e);
+            if (l & 2u) acc += K.t[0] * (vc[i] - w);
+            if (l & 4u) acc += K.t[1] * (vc[i] - vn[i]);
+            if (l & 8u) acc += K.t[1] * (vc[i] - vs[i]);
+            if (l & 16u) acc += K.t[2] * (vc[i] - vp[i]);
+            if (l & 32u) acc += K.t[2] * (vc[i] - vm[i]);
+            q[i] = (l & LINK_VALID) ? acc : T(0);
+        }
+    }
+}
+
+// the operator a CG kernel applies: M (Alg. 1) or L (fixed-point solve); `code` holds stencil codes resp. link bytes
+template <bool LOP, typename T, int V>
+__device__ __forceinline__ void apply_op_chunk(T (&q)[V], const T (&vm)[V], const T (&vc)[V], const T (&vp)[V],
+                                               const T (&vn)[V], const T (&vs)[V], T xl, T xr, uint32_t fb,
+                                               const uint32_t (&code)[V], const Coef<T>& K,
+                                               const XEdge& xe, int ycls, int zcls)
+{
+    if constexpr (LOP) apply_L_chunk<T, V>(q, vm, vc, vp, vn, vs, xl, xr, fb, code, K, xe, ycls, zcls);
+    else apply_M_chunk<T, V>(q, vm, vc, vp, vn, vs, xl, xr, fb, code, K, xe, ycls, zcls);
+}
+
+// per-cell data of a flagged chunk: the V stencil codes (M) or the V link bytes (L), one per array element
+template <bool LOP, int V>
+__device__ __forceinline__ void load_cell_codes(const uint32_t* __restrict__ wcode, const uint8_t* __restrict__ link,
+                                                long long cell, uint32_t (&code)[V])
+{
+    if constexpr (!LOP) {
+        ld_chunk<uint32_t, V>(wcode + cell, code);
+    } else if constexpr (V == 4) {
+        const uint32_t w = *reinterpret_cast<const uint32_t*>(link + cell);
+#pragma unroll
+        for (int i = 0; i < 4; ++i) code[i] = (w >> (8 * i)) & 0xffu;
+    } else {
+        static_assert(V == 2, "chunks hold 4 fp32 or 2 fp64 cells");
+        const uint32_t w = *reinterpret_cast<const unsigned short*>(link + cell);
+        code[0] = w & 0xffu; code[1] = w >> 8;
+    }
+}
+
 // interior-flag bits of the V/4 groups starting at padded cell idx (one bit per 4 cells, global linear bit index)
 template <int V>
 __device__ __forceinline__ uint32_t flag_bits(const uint32_t* __restrict__ flags, long long idx)

@@ -185,7 +185,7 @@ struct RowTask {
     }
 };
 
-template <typename T, int NT>
+template <typename T, int NT, bool LOP>
 __global__ void __launch_bounds__(NT, 1)
 persist_kernel(const Geom g, const PersistArgs<T> a)
 {
@@ -334,7 +334,7 @@ persist_kernel(const Geom g, const PersistArgs<T> a)
                     for (int c = 0; c < V; ++c) code[c] = 0u;
                     if (tk.out) {
                         fb = flag_bits<V>(a.flags, tk.idx);
-                        if (fb) ld_chunk<uint32_t, V>(a.wcode + tk.idx, code);
+                        if (fb) load_cell_codes<LOP, V>(a.wcode, a.link, tk.idx, code);
                     }
                     T vm[V], vc[V], vp[V], vn[V], vs[V];
                     pn(tk.idx, tk.inb, vc);
@@ -350,7 +350,7 @@ persist_kernel(const Geom g, const PersistArgs<T> a)
                     st_chunk<T, V>(pnew + tk.idx, vc);
                     const XEdge xe = make_xedge<V>(g, tk.x);
                     T q[V];
-                    apply_M_chunk<T, V>(q, vm, vc, vp, vn, vs, xl, xr, fb, code, a.K, xe, face_class(tk.j, g.ny, g.fix[1]),
+                    apply_op_chunk<LOP, T, V>(q, vm, vc, vp, vn, vs, xl, xr, fb, code, a.K, xe, face_class(tk.j, g.ny, g.fix[1]),
                                         face_class(tk.k, g.nz, g.fix[2]));
 #pragma unroll
                     for (int c = 0; c < V; ++c) acc[0] += (double)vc[c] * (double)q[c];
@@ -379,7 +379,7 @@ persist_kernel(const Geom g, const PersistArgs<T> a)
                     zero_chunk<T, V>(er); zero_chunk<T, V>(ed);
                     if (tk.out) {
                         fb = flag_bits<V>(a.flags, tk.idx);
-                        if (fb) ld_chunk<uint32_t, V>(a.wcode + tk.idx, code);
+                        if (fb) load_cell_codes<LOP, V>(a.wcode, a.link, tk.idx, code);
                         ldcg_chunk<T, V>(a.r + tk.idx, er);
                         if (!first) ldcg_chunk<T, V>(a.delta + tk.idx, ed);
                     }
@@ -396,7 +396,7 @@ persist_kernel(const Geom g, const PersistArgs<T> a)
                     if (!tk.out) continue;
                     const XEdge xe = make_xedge<V>(g, tk.x);
                     T q[V];
-                    apply_M_chunk<T, V>(q, vm, vc, vp, vn, vs, xl, xr, fb, code, a.K, xe, face_class(tk.j, g.ny, g.fix[1]),
+                    apply_op_chunk<LOP, T, V>(q, vm, vc, vp, vn, vs, xl, xr, fb, code, a.K, xe, face_class(tk.j, g.ny, g.fix[1]),
                                         face_class(tk.k, g.nz, g.fix[2]));
                     T rn[V], dn[V];
 #pragma unroll

@@ -267,14 +267,14 @@ tma_kernel(const Geom g, const int zlen, const typename Op::Args a, const __grid
 // ------------------------------------------------------------------------------------------------ K3 (TMA)
 // p_new = r + beta p_old evaluated from the raw r / p_old tiles wherever the stencil needs it (centre, N, S, F, B
 // chunks and the two x-halo cells); store p_new; gamma = p_new . M p_new; last CTA: alpha = rho / gamma.
-template <typename T, int BY_, int D_, int MINB_>
+template <typename T, int BY_, int D_, int MINB_, bool LOP_ = false>
 struct OpT3 {
     using VT = T;
     using TG = TileGeom<T, BY_>;
     enum { V = TG::V, D = D_, MINB = MINB_, NACC = 1, TICKET = 0, STAGE_BYTES = 2 * TG::TILE_H,
            BOX_H = (BY_ + 2) * TG::PITCH_H };
     struct Args {
-        T* pbuf[2]; const uint32_t* wcode; const uint32_t* flags; const uint32_t* tflags;
+        T* pbuf[2]; const uint32_t* wcode; const uint8_t* link; const uint32_t* flags; const uint32_t* tflags;
         Coef<T> K; Scalars* sc; double* partial; CondHandles cond;
     };
     struct Ctx {
@@ -285,7 +285,7 @@ struct OpT3 {
     __device__ static TC thread_init(const Geom& g, int x) { return make_xedge<V>(g, x); }
     __device__ static bool active(const Args& a) { return a.sc->inner_go != 0; }
     __device__ static void idle(const Args& a) { set_cond(a.cond, -1, 0); }
-    __device__ static void load_codes(const Args& a, long long cell, uint32_t (&code)[V]) { ld_chunk<uint32_t, V>(a.wcode + cell, code); }
+    __device__ static void load_codes(const Args& a, long long cell, uint32_t (&code)[V]) { load_cell_codes<LOP_, V>(a.wcode, a.link, cell, code); }
     __device__ static void produce(const Args&, const Ctx& c, const TmaSet& m, uint32_t stage, uint32_t bar, int x0, int y0,
                                    int plane, bool)
     {
@@ -339,7 +339,7 @@ struct OpT3 {
         if (!out) return;
         st_chunk<T, V>(c.pnew + idx, vc);
         T q[V];
-        apply_M_chunk<T, V>(q, vm, vc, vp, vn, vs, xl, xr, CLEAN ? 0u : fb, code, a.K, xe, ycls, zcls);
+        apply_op_chunk<LOP_, T, V>(q, vm, vc, vp, vn, vs, xl, xr, CLEAN ? 0u : fb, code, a.K, xe, ycls, zcls);
 #pragma unroll
         for (int i = 0; i < V; ++i) acc += (double)vc[i] * (double)q[i];
     }
@@ -359,7 +359,7 @@ struct OpT3 {
 
 // ------------------------------------------------------------------------------------------------ K4 (TMA)
 // q = M p recomputed from the haloed p tile; delta += alpha p; r -= alpha q; rho' = r.r; beta, loop test.
-template <typename T, int BY_, int D_, int MINB_>
+template <typename T, int BY_, int D_, int MINB_, bool LOP_ = false>
 struct OpT4 {
     using VT = T;
     using TG = TileGeom<T, BY_>;
@@ -367,7 +367,7 @@ struct OpT4 {
            BOX_H = (BY_ + 2) * TG::PITCH_H };
     struct Args {
         T* r; T* delta; int p_fixed;      // p_fixed >= 0: read p from pbuf[p_fixed] (omni_apply_M), else by parity
-        const uint32_t* wcode; const uint32_t* flags; const uint32_t* tflags;
+        const uint32_t* wcode; const uint8_t* link; const uint32_t* flags; const uint32_t* tflags;
         Coef<T> K; Scalars* sc; double* partial; CondHandles cond;
         T* q_out;                         // only for omni_apply_M: store q, leave r / delta untouched
     };
@@ -384,7 +384,7 @@ struct OpT4 {
     __device__ static TC thread_init(const Geom& g, int x) { return make_xedge<V>(g, x); }
     __device__ static bool active(const Args& a) { return a.sc->inner_go != 0; }
     __device__ static void idle(const Args& a) { set_cond(a.cond, -1, 0); }
-    __device__ static void load_codes(const Args& a, long long cell, uint32_t (&code)[V]) { ld_chunk<uint32_t, V>(a.wcode + cell, code); }
+    __device__ static void load_codes(const Args& a, long long cell, uint32_t (&code)[V]) { load_cell_codes<LOP_, V>(a.wcode, a.link, cell, code); }
     __device__ static void produce(const Args& a, const Ctx& c, const TmaSet& m, uint32_t stage, uint32_t bar, int x0,
                                    int y0, int plane, bool inner)
     {
@@ -419,7 +419,7 @@ struct OpT4 {
         if (lane == 31) xr = hr;
         if (!out) return;
         T q[V];
-        apply_M_chunk<T, V>(q, vm, vc, vp, vn, vs, xl, xr, CLEAN ? 0u : fb, code, a.K, xe, ycls, zcls);
+        apply_op_chunk<LOP_, T, V>(q, vm, vc, vp, vn, vs, xl, xr, CLEAN ? 0u : fb, code, a.K, xe, ycls, zcls);
         if (a.q_out != nullptr) {
             st_chunk<T, V>(a.q_out + idx, q);
 #pragma unroll

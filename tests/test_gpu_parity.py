@@ -281,6 +281,68 @@ def test_graph_and_host_loops_are_bit_identical():
                 assert rel_l2_after_mean_removal(Pa.cpu().numpy(), res[0][0], valid) <= (1e-11 if dtype == "f64" else 1e-5)
 
 
+def _direct_both(oracle, f, dtype, tol, max_outer, max_cg, mask=None, loop=None):
+    g_dev, g_or, m_dev, m = _inputs(f, dtype, mask)
+    d = f["d"]
+    prev = omni.set_loop_mode(LOOPS[loop]) if loop else None
+    try:
+        P, info = omni.solve_direct(g_dev[0], g_dev[1], g_dev[2], m_dev, d, tol, max_outer, max_cg)
+        torch.cuda.synchronize()
+    finally:
+        if loop:
+            omni.set_loop_mode(prev)
+    Po, io = oracle.solve_direct(g_or[0], g_or[1], g_or[2], m, *d, tol=tol, max_outer=max_outer, max_cg=max_cg)
+    return P.cpu().numpy(), info, Po, io
+
+
+@pytest.mark.parametrize("loop", list(LOOPS))
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("kind,shape,frac", TRAJ + [("fourier3d", (5, 4, 9), 0.2), ("gaussians2d", (3, 70), None)])
+def test_direct_solve_trajectory_parity(oracle, dtype, kind, shape, frac, loop):
+    """omni_solve_direct (CG on L P = S, SURVEY 8(f) NEXT-2 iii) against oracle.solve_direct: tol = 0 and fixed caps,
+    both sides execute the same 2 x 25 CG steps (the second outer iteration restarts from the fp64 residual)."""
+    f = make_field(kind, shape, seed=7, noise=0.05, kmax=4.0)
+    mask = _random_mask(shape, 9, frac) if frac else None
+    P, info, Po, io = _direct_both(oracle, f, dtype, 0.0, 2, 25, mask, loop=loop)
+    valid = ~np.isnan(Po)
+    assert np.array_equal(np.isnan(P), ~valid)
+    assert info["outer_iters"] == io["outer_iters"] == 2
+    assert info["cg_iters_total"] == io["cg_iters_total"]
+    err = rel_l2_after_mean_removal(P, Po, valid)
+    assert err <= TOL_SOLVE[dtype], err
+    assert info["eps_R_final"] == pytest.approx(io["eps_R_final"], rel=5e-3 if dtype == "f32" else 1e-6)
+
+
+@pytest.mark.parametrize("dtype,tol", [("f64", 1e-8), ("f32", 1e-5)])
+def test_direct_solve_converged(oracle, dtype, tol):
+    """Converged: the direct solve meets Eq. 41 with the oracle's operators, agrees with the oracle's direct solve and
+    lands on the field Algorithm 1 converges to (configs[0], and masked stand-ins of configs 1 and 3)."""
+    for idx, n in ((0, None), (1, 96), (3, 32)):
+        f = make_config(idx, n) if n else make_config(idx)
+        P, info, Po, io = _direct_both(oracle, f, dtype, tol, 20, 3000)
+        assert info["status"] == 0 and io["converged"], (idx, info, io)
+        assert info["eps_R_final"] <= tol
+        if dtype == "f64":
+            assert abs(info["cg_iters_total"] - io["cg_iters_total"]) <= max(3, io["cg_iters_total"] // 50), (info, io)
+        else:   # fp32 CG: the recursive residual drifts from the true one, the fp64 outer check restarts it once or twice
+            assert info["cg_iters_total"] <= 1.5 * io["cg_iters_total"] + 10 and info["outer_iters"] <= io["outer_iters"] + 3, (info, io)
+        valid = ~np.isnan(Po)
+        assert rel_l2_after_mean_removal(P, Po, valid) <= TOL_SOLVE[dtype] * (100 if dtype == "f64" else 1)
+        # the residual of the GPU field, re-evaluated by the oracle's stored-weight operators in fp64 (r0 = W^n P + S - M P)
+        g_dev, g_or, m_dev, m = _inputs(f, dtype)
+        v = oracle.validity(g_or[0], g_or[1], g_or[2], m)
+        w1, w0, w0C = oracle.weights(v, *f["d"])
+        S = oracle.source(v, w1, w0, g_or[0], g_or[1], g_or[2], *f["d"])
+        Pz = np.nan_to_num(P.astype(np.float64))
+        r0 = oracle.apply_Wn(v, w0, w0C, Pz) + S - oracle.apply_M(v, w1, Pz)
+        assert np.linalg.norm(r0) / np.linalg.norm(S) <= (1.05 * tol if dtype == "f64" else 3 * tol)
+        # same fixed point as the two-level iteration
+        P2, i2 = omni.solve(g_dev[0], g_dev[1], g_dev[2], m_dev, f["d"], tol, 200000, 16)
+        assert i2["status"] == 0
+        assert info["cg_iters_total"] * 5 < i2["cg_iters_total"]
+        assert rel_l2_after_mean_removal(P2.cpu().numpy(), P, valid) <= (1e-4 if dtype == "f64" else 5e-3)
+
+
 @pytest.mark.parametrize("dtype", ["f64", "f32"])
 def test_persistent_loop_stress(dtype):
     """The persistent kernel's grid barrier under every mix of phases (max_cg = 0, 1, 2, 3, 16: the outer and the
