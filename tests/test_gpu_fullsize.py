@@ -97,3 +97,21 @@ def test_fullsize_config(oracle, idx, dtype):
         err = rel_l2_after_mean_removal(Pg.cpu().numpy(), Po, v == 1)
         assert err <= TOL_SOLVE[dtype], err
         assert ig["eps_R_final"] == pytest.approx(io["eps_R_final"], rel=1e-3 if dtype == "f32" else 1e-8)
+        # the fixed-point solve (omni_solve_direct) on the same footing
+        Pg, ig = omni.solve_direct(g_dev[0], g_dev[1], g_dev[2], m_dev, d, 0.0, mo, mc)
+        Po, io = oracle.solve_direct(g_or[0], g_or[1], g_or[2], mask, *d, tol=0.0, max_outer=mo, max_cg=mc)
+        assert ig["cg_iters_total"] == io["cg_iters_total"] == mo * mc
+        err = rel_l2_after_mean_removal(Pg.cpu().numpy(), Po, v == 1)
+        assert err <= TOL_SOLVE[dtype], err
+        assert ig["eps_R_final"] == pytest.approx(io["eps_R_final"], rel=1e-3 if dtype == "f32" else 1e-8)
+
+    # omni_solve_direct at full size: its eps_R against the residual kernel on the returned field, the residual at the
+    # sampled cells against the oracle
+    Pd, idd = omni.solve_direct(g_dev[0], g_dev[1], g_dev[2], m_dev, d, tol, 2, 60)
+    assert idd["status"] in (0, 1) and idd["cg_iters_total"] > 0
+    Pn = torch.nan_to_num(Pd.double(), nan=0.0)
+    r, eps = omni.residual(g_dev[0], g_dev[1], g_dev[2], m_dev, Pn, d)
+    assert idd["eps_R_final"] == pytest.approx(eps, rel=5e-2 if dtype == "f32" else 1e-6)
+    _, MP, WP = oracle.sample(v, None, None, None, Pn.cpu().numpy(), cells, *d)
+    r_s = r.flatten()[torch.from_numpy(cells).cuda()].cpu().numpy().astype(np.float64)
+    assert np.abs(r_s - (S_or + WP - MP)).max() <= TOL_STEP[dtype] * 16 * max(np.abs(MP).max(), np.abs(S_or).max())
