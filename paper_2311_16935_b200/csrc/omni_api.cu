@@ -366,9 +366,27 @@ int setup_codes(const Geom& g, const Workspace<T>& w, const T* gx, const T* gy, 
     validity_kernel<T><<<blocks_for(g.npad, 256), 256, 0, st>>>(g, gx, gy, gz, mask, vbyte);
     CK(cudaGetLastError());
     CK(cudaMemsetAsync(w.tflags, 0, (size_t)g.ntx * g.nty * g.twords * 4, st));
-    codes_kernel<<<blocks_for(g.npad / 4, 256), 256, 0, st>>>(g, vbyte, w.link, w.wcode, w.flags, w.tflags);
+    // work list of the groups that need the cell-by-cell decode: scratch in p1 (4 bytes per 4-cell group at most),
+    // its counter in the first word of the barrier slots (both are cleared again below / before their own use)
+    uint32_t* worklist = reinterpret_cast<uint32_t*>(w.p1);
+    unsigned int* work_count = reinterpret_cast<unsigned int*>(w.slots);
+    CK(cudaMemsetAsync(work_count, 0, sizeof(unsigned int), st));
+    codes_kernel<<<blocks_for(g.npad / 4, 256), 256, 0, st>>>(g, vbyte, w.link, w.wcode, w.flags, worklist, work_count);
     CK(cudaGetLastError());
-    g_launches.fetch_add(2, std::memory_order_relaxed);
+    {
+        static int nsm = 0;
+        if (nsm == 0) {
+            int dev = 0;
+            cudaGetDevice(&dev);
+            if (cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || nsm < 1) nsm = 148;
+        }
+        long long nb = (g.npad / 4 + 127) / 128;
+        if (nb > 16LL * nsm) nb = 16LL * nsm;
+        if (nb < 1) nb = 1;
+        codes_worklist_kernel<<<(unsigned)nb, 128, 0, st>>>(g, vbyte, w.link, w.wcode, w.flags, w.tflags, worklist, work_count);
+        CK(cudaGetLastError());
+    }
+    g_launches.fetch_add(3, std::memory_order_relaxed);
     const size_t n = (size_t)g.npad;
     CK(cudaMemsetAsync(w.p0, 0, n * sizeof(T), st));
     CK(cudaMemsetAsync(w.p1, 0, n * sizeof(T), st));

@@ -357,6 +357,19 @@ __device__ __forceinline__ uint32_t flag_bits(const uint32_t* __restrict__ flags
     return (flags[g >> 5] >> (unsigned)(g & 31)) & ((1u << (V >= 4 ? V / 4 : 1)) - 1u);
 }
 
+// padded linear index -> (i, row = j + ny*k); 32-bit arithmetic wherever the grid allows it
+__device__ __forceinline__ void split_pid(const Geom& g, long long pid, int& i, long long& row)
+{
+    if (g.npad < (1LL << 31)) {
+        const unsigned int r = (unsigned int)pid / (unsigned int)g.px;
+        i = (int)((unsigned int)pid - r * (unsigned int)g.px);
+        row = r;
+    } else {
+        i = (int)(pid % g.px);
+        row = pid / g.px;
+    }
+}
+
 // ------------------------------------------------------------------------------------------------ K0a validity
 template <typename T>
 __global__ void validity_kernel(Geom g, const T* __restrict__ gx, const T* __restrict__ gy, const T* __restrict__ gz,
@@ -364,8 +377,9 @@ __global__ void validity_kernel(Geom g, const T* __restrict__ gx, const T* __res
 {
     long long pid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (pid >= g.npad) return;
-    int i = (int)(pid % g.px);
-    long long row = pid / g.px;                   // j + ny*k
+    int i;
+    long long row;                                // j + ny*k
+    split_pid(g, pid, i, row);
     uint8_t ok = 0;
     if (i < g.nx) {
         long long u = row * g.nx + i;             // user-layout index
@@ -419,23 +433,76 @@ __device__ __forceinline__ uint32_t box_code(const Geom& g, int i, int j, int k)
     return code;
 }
 
-// one thread per 4-cell group; a warp's 32 groups fill exactly one flag word
+// decode one 4-cell group cell by cell (any position: faces, corners, mask surface); returns its flag
+__device__ __forceinline__ bool decode_group(const Geom& g, const uint8_t* __restrict__ vbyte, uint8_t* __restrict__ link,
+                                             uint32_t* __restrict__ wcode, long long base, int i0, int j, int k)
+{
+    const int naxes = g.naxes;
+    uint32_t codes[4];
+    uint32_t links = 0;
+    bool flagged = false;
+#pragma unroll
+    for (int c = 0; c < 4; ++c) {
+        const int i = i0 + c;
+        uint32_t code = 0, lk = 0;
+        if (vget(g, vbyte, i, j, k)) {
+            code = WCODE_VALID; lk = LINK_VALID;
+            for (int d = 0; d < 6; ++d) {
+                const int a = d >> 1, sg = (d & 1) ? -1 : 1;
+                int e[3] = { 0, 0, 0 };
+                e[a] = sg;
+                const int qi = i + e[0], qj = j + e[1], qk = k + e[2];
+                if (a >= naxes) continue;                       // 2D scheme: no F/B links at all
+                if (!vget(g, vbyte, qi, qj, qk)) continue;
+                lk |= 1u << d;
+                const int b = (a + 1) % 3, cc = (a + 2) % 3;
+                int eb[3] = { 0, 0, 0 }, ec[3] = { 0, 0, 0 };
+                eb[b] = 1; ec[cc] = 1;
+                uint32_t far = vget(g, vbyte, qi + e[0], qj + e[1], qk + e[2]);
+                uint32_t nb = (b < naxes) ? vget(g, vbyte, qi + eb[0], qj + eb[1], qk + eb[2]) +
+                                            vget(g, vbyte, qi - eb[0], qj - eb[1], qk - eb[2]) : 0u;
+                uint32_t nc = (cc < naxes) ? vget(g, vbyte, qi + ec[0], qj + ec[1], qk + ec[2]) +
+                                             vget(g, vbyte, qi - ec[0], qj - ec[1], qk - ec[2]) : 0u;
+                code |= (far | (nb << 1) | (nc << 3)) << (5 * d);
+            }
+        }
+        codes[c] = code;
+        links |= lk << (8 * c);
+        // two or more cells away from every face the mask-free box code is the interior code
+        const bool deep = (i >= 2 && i < g.nx - 2) && (j >= 2 && j < g.ny - 2) && (g.naxes == 2 || (k >= 2 && k < g.nz - 2));
+        const uint32_t expect = deep ? g.icode : box_code(g, i, j, k);
+        flagged |= (code != expect);
+    }
+    *reinterpret_cast<uint4*>(wcode + base) = make_uint4(codes[0], codes[1], codes[2], codes[3]);
+    *reinterpret_cast<uint32_t*>(link + base) = links;
+    return flagged;
+}
+
+// K0b pass 1: one thread per 4-cell group.  A group at least two cells away from every face whose 25-cell
+// neighbourhoods are all valid (23 aligned word loads instead of ~150 byte loads) is interior: nothing to decode,
+// nothing flagged.  Every other group (box faces, the neighbourhood of masked cells: a few per cent, but at least one
+// lane of half the warps of a 500-cell row) is appended to a work list with a warp-aggregated atomic and decoded by
+// pass 2 with all lanes busy, instead of stalling its whole warp on the cell-by-cell path here.
 __global__ void codes_kernel(Geom g, const uint8_t* __restrict__ vbyte, uint8_t* __restrict__ link,
-                             uint32_t* __restrict__ wcode, uint32_t* __restrict__ flags, uint32_t* __restrict__ tflags)
+                             uint32_t* __restrict__ wcode, uint32_t* __restrict__ flags, uint32_t* __restrict__ worklist,
+                             unsigned int* __restrict__ work_count)
 {
     const long long grp = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     const long long ngrp = g.npad >> 2;
-    bool flagged = false;
+    bool defer = false;
     if (grp < ngrp) {
         const long long base = grp << 2;
-        const int i0 = (int)(base % g.px);
-        const long long row = base / g.px;
-        const int j = (int)(row % g.ny), k = (int)(row / g.ny);
-        const int naxes = g.naxes;
-        uint32_t codes[4];
-        uint32_t links = 0;
-        // fast path: a group at least two cells away from every face whose 25-cell neighbourhoods are all valid (23
-        // aligned word loads instead of ~150 byte loads) is interior: nothing to decode, nothing flagged
+        int i0, j, k;
+        if (g.npad < (1LL << 31)) {                  // 32-bit index arithmetic wherever it fits
+            const unsigned int b32 = (unsigned int)base, row = b32 / (unsigned int)g.px;
+            i0 = (int)(b32 - row * (unsigned int)g.px);
+            k = (int)(row / (unsigned int)g.ny);
+            j = (int)(row - (unsigned int)k * (unsigned int)g.ny);
+        } else {
+            i0 = (int)(base % g.px);
+            const long long row = base / g.px;
+            j = (int)(row % g.ny); k = (int)(row / g.ny);
+        }
         const bool deep_grp = (i0 >= 4) && (i0 + 8 <= g.nx) && (j >= 2) && (j < g.ny - 2) &&
                               (g.naxes == 2 || (k >= 2 && k < g.nz - 2));
         bool all_valid = false;
@@ -454,48 +521,40 @@ __global__ void codes_kernel(Geom g, const uint8_t* __restrict__ vbyte, uint8_t*
             *reinterpret_cast<uint4*>(wcode + base) = make_uint4(g.icode, g.icode, g.icode, g.icode);
             *reinterpret_cast<uint32_t*>(link + base) = (g.naxes == 3) ? 0x7f7f7f7fu : 0x4f4f4f4fu;
         } else {
-#pragma unroll
-        for (int c = 0; c < 4; ++c) {
-            const int i = i0 + c;
-            uint32_t code = 0, lk = 0;
-            if (vget(g, vbyte, i, j, k)) {
-                code = WCODE_VALID; lk = LINK_VALID;
-                for (int d = 0; d < 6; ++d) {
-                    const int a = d >> 1, sg = (d & 1) ? -1 : 1;
-                    int e[3] = { 0, 0, 0 };
-                    e[a] = sg;
-                    const int qi = i + e[0], qj = j + e[1], qk = k + e[2];
-                    if (a >= naxes) continue;                       // 2D scheme: no F/B links at all
-                    if (!vget(g, vbyte, qi, qj, qk)) continue;
-                    lk |= 1u << d;
-                    const int b = (a + 1) % 3, cc = (a + 2) % 3;
-                    int eb[3] = { 0, 0, 0 }, ec[3] = { 0, 0, 0 };
-                    eb[b] = 1; ec[cc] = 1;
-                    uint32_t far = vget(g, vbyte, qi + e[0], qj + e[1], qk + e[2]);
-                    uint32_t nb = (b < naxes) ? vget(g, vbyte, qi + eb[0], qj + eb[1], qk + eb[2]) +
-                                                vget(g, vbyte, qi - eb[0], qj - eb[1], qk - eb[2]) : 0u;
-                    uint32_t nc = (cc < naxes) ? vget(g, vbyte, qi + ec[0], qj + ec[1], qk + ec[2]) +
-                                                 vget(g, vbyte, qi - ec[0], qj - ec[1], qk - ec[2]) : 0u;
-                    code |= (far | (nb << 1) | (nc << 3)) << (5 * d);
-                }
-            }
-            codes[c] = code;
-            links |= lk << (8 * c);
-            // two or more cells away from every face the mask-free box code is the interior code
-            const bool deep = (i >= 2 && i < g.nx - 2) && (j >= 2 && j < g.ny - 2) && (g.naxes == 2 || (k >= 2 && k < g.nz - 2));
-            const uint32_t expect = deep ? g.icode : box_code(g, i, j, k);
-            flagged |= (code != expect);
+            defer = true;
         }
-        *reinterpret_cast<uint4*>(wcode + base) = make_uint4(codes[0], codes[1], codes[2], codes[3]);
-        *reinterpret_cast<uint32_t*>(link + base) = links;
-        }
-        if (flagged) {
+    }
+    const unsigned int lane = threadIdx.x & 31u;
+    const uint32_t m = __ballot_sync(0xffffffffu, defer);
+    if (m) {
+        unsigned int at = 0;
+        const int leader = __ffs(m) - 1;
+        if ((int)lane == leader) at = atomicAdd(work_count, (unsigned int)__popc(m));
+        at = __shfl_sync(0xffffffffu, at, leader);
+        if (defer) worklist[at + __popc(m & ((1u << lane) - 1u))] = (uint32_t)grp;
+    }
+    if (lane == 0 && grp < ngrp) flags[grp >> 5] = 0u;       // pass 2 sets the bits of the flagged groups
+}
+
+// K0b pass 2: the deferred groups, one per thread (grid-stride over the work list)
+__global__ void codes_worklist_kernel(Geom g, const uint8_t* __restrict__ vbyte, uint8_t* __restrict__ link,
+                                      uint32_t* __restrict__ wcode, uint32_t* __restrict__ flags,
+                                      uint32_t* __restrict__ tflags, const uint32_t* __restrict__ worklist,
+                                      const unsigned int* __restrict__ work_count)
+{
+    const unsigned int n = *work_count;
+    for (unsigned int w = blockIdx.x * blockDim.x + threadIdx.x; w < n; w += gridDim.x * blockDim.x) {
+        const long long grp = worklist[w];
+        const long long base = grp << 2;
+        const int i0 = (int)(base % g.px);
+        const long long row = base / g.px;
+        const int j = (int)(row % g.ny), k = (int)(row / g.ny);
+        if (decode_group(g, vbyte, link, wcode, base, i0, j, k)) {
+            atomicOr(&flags[grp >> 5], 1u << (unsigned)(grp & 31));
             const int tile = (j / g.tby) * g.ntx + (i0 / g.tbx);
             atomicOr(&tflags[(size_t)tile * g.twords + (k >> 5)], 1u << (k & 31));
         }
     }
-    const uint32_t word = __ballot_sync(0xffffffffu, flagged);
-    if ((threadIdx.x & 31) == 0 && grp < ngrp) flags[grp >> 5] = word;
 }
 
 // ------------------------------------------------------------------------------------------------ K1 source
@@ -510,8 +569,9 @@ source_kernel(Geom g, const T* __restrict__ gx, const T* __restrict__ gy, const 
     const long long pid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     double sq = 0.0;
     if (pid < g.npad) {
-        const int i = (int)(pid % g.px);
-        const long long row = pid / g.px;
+        int i;
+        long long row;
+        split_pid(g, pid, i, row);
         T s = T(0);
         const uint32_t l = link[pid];
         if (l & LINK_VALID) {
@@ -574,8 +634,17 @@ __global__ void finalize_kernel(Geom g, const double* P0, const double* P1, cons
     long long u = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     long long nuser = (long long)g.nx * g.ny * g.nz;
     if (u >= nuser) return;
-    int i = (int)(u % g.nx);
-    long long pid = (u / g.nx) * g.px + i;
+    int i;
+    long long row;
+    if (nuser < (1LL << 31)) {
+        const unsigned int r = (unsigned int)u / (unsigned int)g.nx;
+        i = (int)((unsigned int)u - r * (unsigned int)g.nx);
+        row = r;
+    } else {
+        i = (int)(u % g.nx);
+        row = u / g.nx;
+    }
+    const long long pid = row * g.px + i;
     out[u] = (link[pid] & LINK_VALID) ? (T)P[pid] : (T)nan("");
 }
 
@@ -586,8 +655,10 @@ __global__ void pad_copy_kernel(Geom g, const TI* __restrict__ in, TO* __restric
 {
     long long pid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (pid >= g.npad) return;
-    int i = (int)(pid % g.px);
-    long long u = (pid / g.px) * g.nx + i;
+    int i;
+    long long row;
+    split_pid(g, pid, i, row);
+    long long u = row * g.nx + i;
     if (to_padded) out[pid] = (i < g.nx && (link[pid] & LINK_VALID)) ? (TO)in[u] : TO(0);
     else if (i < g.nx) out[u] = (TO)in[pid];
 }

@@ -97,6 +97,25 @@ __device__ __forceinline__ double lds_scalar(uint32_t addr, double)
     return v;
 }
 
+// a thread's contribution to a dot product: fp64 products for fp64 data; for fp32 data the V products of one 16-byte
+// chunk are summed in fp32 (fused multiply-adds) and enter the fp64 accumulator as one term -- one conversion per
+// chunk instead of two per cell, the fp32 sum of 4 terms adding 1e-7 relative to a term, like the data's own rounding
+template <typename T, int V>
+__device__ __forceinline__ double chunk_dot(const T (&a)[V], const T (&b)[V])
+{
+    if constexpr (sizeof(T) == 8) {
+        double s = 0.0;
+#pragma unroll
+        for (int i = 0; i < V; ++i) s += (double)a[i] * (double)b[i];
+        return s;
+    } else {
+        float s = 0.f;
+#pragma unroll
+        for (int i = 0; i < V; ++i) s = fmaf((float)a[i], (float)b[i], s);
+        return (double)s;
+    }
+}
+
 template <class Op>
 __global__ void __launch_bounds__(Op::TG::NTHR, Op::MINB)
 tma_kernel(const Geom g, const int zlen, const typename Op::Args a, const __grid_constant__ TmaSet maps)
@@ -340,8 +359,12 @@ struct OpT3 {
         st_chunk<T, V>(c.pnew + idx, vc);
         T q[V];
         apply_op_chunk<LOP_, T, V>(q, vm, vc, vp, vn, vs, xl, xr, CLEAN ? 0u : fb, code, a.K, xe, ycls, zcls);
+#if 0
 #pragma unroll
         for (int i = 0; i < V; ++i) acc += (double)vc[i] * (double)q[i];
+#else
+        acc += chunk_dot<T, V>(vc, q);
+#endif
     }
     __device__ static void finalize(const Args& a, const double (&tot)[1])
     {
@@ -434,8 +457,8 @@ struct OpT4 {
         for (int i = 0; i < V; ++i) {
             rn[i] = er[i] - c.alpha * q[i];
             dn[i] = ed[i] + c.alpha * vc[i];
-            acc += (double)rn[i] * (double)rn[i];
         }
+        acc += chunk_dot<T, V>(rn, rn);
         st_chunk<T, V>(a.r + idx, rn);
         st_chunk<T, V>(a.delta + idx, dn);
     }
