@@ -401,7 +401,9 @@ template <typename T>
 int launch_source(const Geom& g, const Workspace<T>& w, const Coef<T>& K, const T* gx, const T* gy, const T* gz,
                   cudaStream_t st)
 {
-    source_kernel<T><<<blocks_for(g.npad, 256), 256, 0, st>>>(g, gx, gy, gz, w.link, K, w.S, w.sc, w.partial);
+    unsigned nb = blocks_for(g.npad, 256);
+    if (nb > 4736u) nb = 4736u;                 // 148 SMs x 8 CTAs x 4: the kernel is grid-stride
+    source_kernel<T><<<nb, 256, 0, st>>>(g, gx, gy, gz, w.link, K, w.S, w.sc, w.partial);
     g_launches.fetch_add(1, std::memory_order_relaxed);
     CK(cudaGetLastError());
     return OMNI_OK;

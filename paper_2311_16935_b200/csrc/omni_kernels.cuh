@@ -566,9 +566,10 @@ source_kernel(Geom g, const T* __restrict__ gx, const T* __restrict__ gy, const 
 {
     __shared__ double red[8];
     __shared__ int is_last;
-    const long long pid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    // grid-stride: a few thousand CTAs (one ticket atomic each), every thread walks cells a whole grid apart
     double sq = 0.0;
-    if (pid < g.npad) {
+    for (long long pid = (long long)blockIdx.x * blockDim.x + threadIdx.x; pid < g.npad;
+         pid += (long long)gridDim.x * blockDim.x) {
         int i;
         long long row;
         split_pid(g, pid, i, row);
@@ -589,7 +590,7 @@ source_kernel(Geom g, const T* __restrict__ gx, const T* __restrict__ gy, const 
             }
         }
         S[pid] = s;
-        sq = (double)s * (double)s;
+        sq += (double)s * (double)s;
     }
     sq = warp_sum(sq);
     if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = sq;
