@@ -70,10 +70,10 @@ def converge(args, cfg, dtype):
         gx = torch.from_numpy(np.stack([x["g"][0] for x in fs])).to(tdt).cuda()
         gy = torch.from_numpy(np.stack([x["g"][1] for x in fs])).to(tdt).cuda()
         m = None if f["mask"] is None else torch.from_numpy(f["mask"]).cuda()
-        omni.solve_batch2d(gx, gy, m, f["d"], tol, 2, 2)
+        omni.solve_batch2d(gx, gy, m, f["d"], tol, 2, 2, direct=args.direct)
         torch.cuda.synchronize()
         e0.record()
-        P, info = omni.solve_batch2d(gx, gy, m, f["d"], tol, args.max_outer, args.max_cg)
+        P, info = omni.solve_batch2d(gx, gy, m, f["d"], tol, args.max_outer, args.max_cg, direct=args.direct)
         e1.record()
         torch.cuda.synchronize()
         Pn = P[0].double().cpu().numpy()

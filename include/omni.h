@@ -104,6 +104,14 @@ int omni_solve_direct_f32(int nx, int ny, int nz, double dx, double dy, double d
                           const float* d_gx, const float* d_gy, const float* d_gz, const unsigned char* d_mask,
                           float* d_P_out, double tol, int max_outer, int max_cg, void* stream, omni_info* info);
 
+/* The two combined: nb snapshots on one mask (arguments as omni_solve_batch2d_*), inner systems L P = S. */
+int omni_solve_direct_batch2d_f64(int nx, int ny, int nb, double dx, double dy, const double* d_gx, const double* d_gy,
+                                  const unsigned char* d_mask2d, const double* d_P_init, double* d_P_out, double tol,
+                                  int max_outer, int max_cg, void* stream, omni_info* info);
+int omni_solve_direct_batch2d_f32(int nx, int ny, int nb, double dx, double dy, const float* d_gx, const float* d_gy,
+                                  const unsigned char* d_mask2d, const float* d_P_init, float* d_P_out, double tol,
+                                  int max_outer, int max_cg, void* stream, omni_info* info);
+
 /* ---- batched 2D snapshots with an optional first guess (SURVEY.md 8(f) NEXT-1; time-resolved PIV: PAPER.md:365, :503) ----
  * nb independent 2D gradient fields [nb][ny][nx] on ONE mask [ny][nx] (NULL = all valid) are stacked and solved as one
  * block-diagonal system with the 2D scheme: stencil codes are built once, every stencil sweep serves all snapshots,

@@ -432,6 +432,17 @@ int oracle_solve_batch2d(int nx, int ny, int nb, double dx, double dy,
     return rc;
 }
 
+/* oracle_solve_batch2d with the inner systems of oracle_solve_direct: CG on the block-diagonal L P = S of the stack */
+int oracle_solve_direct_batch2d(int nx, int ny, int nb, double dx, double dy,
+                                const double *gx, const double *gy, const unsigned char *mask2d, const double *P_init,
+                                double *P_out, double tol, int max_outer, int max_cg, oracle_info *info)
+{
+    g_direct = 1;
+    int rc = oracle_solve_batch2d(nx, ny, nb, dx, dy, gx, gy, mask2d, P_init, P_out, tol, max_outer, max_cg, info);
+    g_direct = 0;
+    return rc;
+}
+
 static int solve_impl(int nx, int ny, int nz, double dx, double dy, double dz,
                       const double *gx, const double *gy, const double *gz, const unsigned char *mask,
                       const double *P_init, double *P_out, double tol, int max_outer, int max_cg, oracle_info *info,

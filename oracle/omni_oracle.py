@@ -193,15 +193,16 @@ def sample(v, gx, gy, gz, x, cells, dx, dy, dz=1.0):
     return S, Mx, Wx
 
 
-def solve_batch2d(gx, gy, mask2d, dx, dy, tol, max_outer, max_cg, P_init=None):
-    """nb stacked 2D snapshots (nb, ny, nx) on one mask (ny, nx), solved as one block-diagonal system."""
+def solve_batch2d(gx, gy, mask2d, dx, dy, tol, max_outer, max_cg, P_init=None, direct=False):
+    """nb stacked 2D snapshots (nb, ny, nx) on one mask (ny, nx), solved as one block-diagonal system
+    (direct: with the inner systems of solve_direct)."""
     gx, gy = _f64(gx), _f64(gy)
     nb, ny, nx = gx.shape
     m = None if mask2d is None else np.ascontiguousarray(mask2d, dtype=np.uint8)
     P0 = None if P_init is None else _f64(P_init)
     P = np.zeros(gx.shape)
     info = Info()
-    f = lib().oracle_solve_batch2d
+    f = lib().oracle_solve_direct_batch2d if direct else lib().oracle_solve_batch2d
     f.restype = C.c_int
     rc = f(C.c_int(nx), C.c_int(ny), C.c_int(nb), C.c_double(dx), C.c_double(dy), _p(gx), _p(gy), _p(m), _p(P0), _p(P),
            C.c_double(tol), C.c_int(max_outer), C.c_int(max_cg), C.byref(info))

@@ -17,7 +17,7 @@ STATUS_NAMES = {0: "OMNI_OK", 1: "OMNI_NOT_CONVERGED", -1: "OMNI_ERR_INVALID_ARG
                 -3: "OMNI_ERR_ALLOC", -4: "OMNI_ERR_BREAKDOWN"}
 # every symbol include/omni.h declares
 SYMBOLS = ["omni_solve_f64", "omni_solve_f32", "omni_workspace_bytes", "omni_solve_f64_ws", "omni_solve_f32_ws",
-           "omni_solve_host_f64", "omni_solve_host_f32", "omni_solve_batch2d_f64", "omni_solve_batch2d_f32", "omni_solve_direct_f64", "omni_solve_direct_f32", "omni_constants", "omni_source_f64", "omni_source_f32",
+           "omni_solve_host_f64", "omni_solve_host_f32", "omni_solve_batch2d_f64", "omni_solve_batch2d_f32", "omni_solve_direct_f64", "omni_solve_direct_f32", "omni_solve_direct_batch2d_f64", "omni_solve_direct_batch2d_f32", "omni_constants", "omni_source_f64", "omni_source_f32",
            "omni_apply_M_f64", "omni_apply_M_f32", "omni_residual_f64", "omni_residual_f32", "omni_launch_count",
            "omni_set_loop_mode", "omni_release_memory", "omni_profile_enable", "omni_profile_read", "omni_status_string", "omni_version"]
 
@@ -204,8 +204,9 @@ def solve_direct(gx, gy, gz, mask, d, tol, max_outer, max_cg, out=None):
     return P, info.as_dict()
 
 
-def solve_batch2d(gx, gy, mask2d, d, tol, max_outer, max_cg, P_init=None, out=None):
-    """omni_solve_batch2d_*: gx, gy (nb, ny, nx) CUDA tensors, mask2d (ny, nx) uint8 or None, d = (dx, dy)."""
+def solve_batch2d(gx, gy, mask2d, d, tol, max_outer, max_cg, P_init=None, out=None, direct=False):
+    """omni_solve_batch2d_* (direct=True: omni_solve_direct_batch2d_*): gx, gy (nb, ny, nx) CUDA tensors, mask2d
+    (ny, nx) uint8 or None, d = (dx, dy)."""
     import torch
     sfx = _suffix(gx)
     _check([gx, gy, mask2d, P_init, out], "cuda")
@@ -215,7 +216,7 @@ def solve_batch2d(gx, gy, mask2d, d, tol, max_outer, max_cg, P_init=None, out=No
     P = out if out is not None else torch.empty_like(gx)
     info = Info()
     with torch.cuda.device(gx.device):
-        fn = getattr(lib(), f"omni_solve_batch2d_{sfx}")
+        fn = getattr(lib(), f"omni_solve_direct_batch2d_{sfx}" if direct else f"omni_solve_batch2d_{sfx}")
         rc = fn(C.c_int(nx), C.c_int(ny), C.c_int(nb), C.c_double(float(d[0])), C.c_double(float(d[1])), _ptr(gx), _ptr(gy),
                 _ptr(mask2d), _ptr(P_init), _ptr(P), C.c_double(tol), C.c_int(max_outer), C.c_int(max_cg),
                 _stream(gx.device), C.byref(info))

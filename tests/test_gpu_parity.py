@@ -221,6 +221,36 @@ def test_batch2d_and_first_guess(oracle, dtype):
     assert torch.allclose(torch.nan_to_num(Pw), torch.nan_to_num(Pc), rtol=0, atol=1e-6 if dtype == "f32" else 1e-13)
 
 
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_direct_batch2d(oracle, dtype):
+    """omni_solve_direct_batch2d_*: the stacked snapshots with the inner systems L P = S, against the oracle's, with
+    and without a first guess; converged, every snapshot meets the tolerance of the joint system."""
+    fs = [make_field("lamb_oseen2d", (45, 140), seed=s, noise=0.05) for s in range(4)]
+    np_dt = np.float32 if dtype == "f32" else np.float64
+    gx = np.stack([f["g"][0] for f in fs]).astype(np_dt); gy = np.stack([f["g"][1] for f in fs]).astype(np_dt)
+    m, d = fs[0]["mask"], fs[0]["d"]
+    gxd, gyd, md = to_dev(gx), to_dev(gy), to_dev(m)
+    rng = np.random.default_rng(6)
+    P0 = (0.1 * rng.normal(size=gx.shape)).astype(np_dt)
+    for init in (None, P0):
+        P, info = omni.solve_batch2d(gxd, gyd, md, d, 0.0, 2, 30, P_init=None if init is None else to_dev(init), direct=True)
+        Po, io = oracle.solve_batch2d(gx.astype(np.float64), gy.astype(np.float64), m, d[0], d[1], 0.0, 2, 30,
+                                      P_init=None if init is None else init.astype(np.float64), direct=True)
+        assert info["cg_iters_total"] == io["cg_iters_total"] == 60
+        Pn = P.cpu().numpy()
+        assert np.array_equal(np.isnan(Pn), np.isnan(Po))
+        for b in range(4):
+            assert rel_l2_after_mean_removal(Pn[b], Po[b], ~np.isnan(Po[b])) <= TOL_SOLVE[dtype]
+    tol = 1e-5 if dtype == "f32" else 1e-8
+    Pc, ic = omni.solve_batch2d(gxd, gyd, md, d, tol, 20, 3000, direct=True)
+    assert ic["status"] == 0 and ic["eps_R_final"] <= tol
+    P2, i2 = omni.solve_batch2d(gxd, gyd, md, d, tol, 200000, 16)
+    assert i2["status"] == 0 and ic["cg_iters_total"] * 5 < i2["cg_iters_total"]
+    for b in range(4):
+        valid = ~torch.isnan(Pc[b]).cpu().numpy()
+        assert rel_l2_after_mean_removal(P2[b].cpu().numpy(), Pc[b].cpu().numpy(), valid) <= (1e-4 if dtype == "f64" else 5e-3)
+
+
 def test_converged_parity_config0(oracle):
     """BASELINE configs[0]: 64^2 fp64, tol 1e-8, converged on both sides with the same stopping rules; and the
     recovered field matches the analytic P up to a constant at the discretisation + noise level."""

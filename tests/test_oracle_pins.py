@@ -560,3 +560,25 @@ def test_batch2d_oracle_pins(oracle):
     for b in range(3):
         a, c = Pr[b][v[b]] - Pr[b][v[b]].mean(), Pb[b][v[b]] - Pb[b][v[b]].mean()
         assert np.linalg.norm(a - c) / np.linalg.norm(c) < 1e-7
+
+
+def test_direct_batch2d_oracle_pins(oracle):
+    """The stacked direct solve: nb = 1 is bit-identical to solve_direct on the 2D grid; converged, every snapshot equals
+    its own direct solve (pinned to pinv(L) S above); a first guess moves nothing but the per-component constant."""
+    fs = [make_field("lamb_oseen2d", (26, 30), seed=s, noise=0.05) for s in range(3)]
+    gx = np.stack([f["g"][0] for f in fs]); gy = np.stack([f["g"][1] for f in fs])
+    m, d = fs[0]["mask"], fs[0]["d"]
+    P1, i1 = oracle.solve_batch2d(gx[:1], gy[:1], m, d[0], d[1], 0.0, 2, 9, direct=True)
+    P2, i2 = oracle.solve_direct(gx[0], gy[0], None, m, d[0], d[1], 1.0, tol=0.0, max_outer=2, max_cg=9)
+    assert np.array_equal(P1[0], P2, equal_nan=True) and i1["eps_R_final"] == i2["eps_R_final"]
+    Pb, ib = oracle.solve_batch2d(gx, gy, m, d[0], d[1], 1e-11, 10, 2000, direct=True)
+    assert ib["converged"]
+    rng = np.random.default_rng(1)
+    Pr, ir = oracle.solve_batch2d(gx, gy, m, d[0], d[1], 1e-11, 10, 2000, P_init=rng.normal(size=gx.shape), direct=True)
+    assert ir["converged"]
+    for b in range(3):
+        Pi, ii = oracle.solve_direct(gx[b], gy[b], None, m, d[0], d[1], 1.0, tol=1e-11, max_outer=10, max_cg=2000)
+        v = ~np.isnan(Pi)
+        for other in (Pb, Pr):
+            a, c = other[b][v] - other[b][v].mean(), Pi[v] - Pi[v].mean()
+            assert np.linalg.norm(a - c) / np.linalg.norm(c) < 1e-8
