@@ -51,6 +51,44 @@ inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 std::mutex g_pool_mu;
 cudaMemPool_t g_pools[64] = {};
 
+// Executable graphs in flight: cudaGraphExecDestroy on a running conditional graph blocks the host until it has
+// finished (measured: the whole solve), so a launched graph is parked here with an event and destroyed by a later call
+// (or by omni_release_memory) once the event has completed -- omni_solve_* with info == NULL stays asynchronous.
+struct PendingGraph { cudaGraphExec_t exec; cudaEvent_t done; };
+std::mutex g_pend_mu;
+std::vector<PendingGraph> g_pending;
+
+void reap_graphs(bool wait)
+{
+    std::lock_guard<std::mutex> lk(g_pend_mu);
+    size_t keep = 0;
+    for (size_t i = 0; i < g_pending.size(); ++i) {
+        PendingGraph& pg = g_pending[i];
+        if (wait) cudaEventSynchronize(pg.done);
+        if (cudaEventQuery(pg.done) == cudaSuccess) {
+            cudaGraphExecDestroy(pg.exec);
+            cudaEventDestroy(pg.done);
+        } else {
+            g_pending[keep++] = pg;
+        }
+    }
+    g_pending.resize(keep);
+    cudaGetLastError();        // cudaErrorNotReady from the queries is not an error
+}
+
+void park_graph(cudaGraphExec_t exec, cudaStream_t st)
+{
+    cudaEvent_t ev = nullptr;
+    if (cudaEventCreateWithFlags(&ev, cudaEventDisableTiming) != cudaSuccess || cudaEventRecord(ev, st) != cudaSuccess) {
+        if (ev) cudaEventDestroy(ev);
+        cudaGetLastError();
+        cudaGraphExecDestroy(exec);            // falls back to the blocking destroy
+        return;
+    }
+    std::lock_guard<std::mutex> lk(g_pend_mu);
+    g_pending.push_back(PendingGraph{ exec, ev });
+}
+
 cudaMemPool_t device_pool()
 {
     int dev = 0;
@@ -534,6 +572,7 @@ int run_loop_graph(const Geom& g, const Workspace<T>& w, const HostConst& H, con
     cudaGraphExec_t exec = nullptr;
     cudaStream_t cap = nullptr;
     int rc = OMNI_ERR_CUDA;
+    reap_graphs(false);
     // occupancy queries happen here, outside any stream capture (results are cached per kernel)
     (void)tma_config<K2<T>>(g); (void)tma_config<K3<T, LOP>>(g); (void)tma_config<K4<T, LOP>>(g);
     TmaSet maps;
@@ -584,8 +623,9 @@ int run_loop_graph(const Geom& g, const Workspace<T>& w, const HostConst& H, con
         rc = OMNI_OK;
     } while (0);
     if (rc != OMNI_OK) cudaGetLastError();
-    // an executable graph in flight is freed asynchronously on completion
-    if (exec) cudaGraphExecDestroy(exec);
+    if (exec) {
+        if (rc == OMNI_OK) park_graph(exec, st); else cudaGraphExecDestroy(exec);
+    }
     if (G) cudaGraphDestroy(G);
     if (cap) cudaStreamDestroy(cap);
     return rc;
@@ -1071,6 +1111,7 @@ void omni_profile_read(double* h_ms3, long long* h_count3, int reset)
 
 void omni_release_memory(void)
 {
+    reap_graphs(true);
     std::lock_guard<std::mutex> lk(g_pool_mu);
     for (auto& p : g_pools)
         if (p) cudaMemPoolTrimTo(p, 0);

@@ -404,6 +404,33 @@ def test_persistent_loop_stress(dtype):
                 assert np.array_equal(P0, Pg, equal_nan=True)
 
 
+def test_solve_without_info_is_asynchronous():
+    """include/omni.h: with info == NULL the call returns after enqueueing.  The graph loop parks its executable graph
+    instead of destroying it in flight (that blocks the host for the whole solve); the persistent loop is one launch."""
+    import time
+    f = make_config(3, 160)
+    g_dev, _, m_dev, _ = _inputs(f, "f32")
+    for mode in (2, 3):
+        prev = omni.set_loop_mode(mode)
+        try:
+            for _ in range(2):
+                omni.solve(g_dev[0], g_dev[1], g_dev[2], m_dev, f["d"], 0.0, 6, 50)
+            torch.cuda.synchronize()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            t0 = time.perf_counter()
+            e0.record()
+            P, info = omni.solve(g_dev[0], g_dev[1], g_dev[2], m_dev, f["d"], 0.0, 6, 50, want_info=False)
+            host_ms = (time.perf_counter() - t0) * 1e3
+            e1.record()
+            torch.cuda.synchronize()
+            gpu_ms = e0.elapsed_time(e1)
+        finally:
+            omni.set_loop_mode(prev)
+        assert info is None
+        assert host_ms < 0.5 * gpu_ms, (mode, host_ms, gpu_ms)
+    omni.release_memory()
+
+
 def test_edge_cases(oracle):
     dev = "cuda"
     # zero gradient -> P = 0, no iterations
