@@ -47,6 +47,8 @@ def parse():
     ap.add_argument("--max-outer", type=int, default=200000, help="--converge: outer iteration cap")
     ap.add_argument("--direct", action="store_true",
                     help="--converge: omni_solve_direct (CG on the fixed-point system L P = S) instead of Algorithm 1")
+    ap.add_argument("--cascade", type=int, default=-1,
+                    help="--converge: omni_solve_cascade with this many coarse levels (implies the direct solve)")
     ap.add_argument("--batch", type=int, default=1,
                     help="--converge on a 2D config: solve this many snapshots (same mask, different noise seeds) in one "
                          "omni_solve_batch2d call")
@@ -83,6 +85,9 @@ def converge(args, cfg, dtype):
         g = [torch.from_numpy(c).to(tdt).cuda() for c in f["g"]] + [None] * (3 - len(f["g"]))
         m = None if f["mask"] is None else torch.from_numpy(f["mask"]).cuda()
         fn = omni.solve_direct if args.direct else omni.solve
+        if args.cascade >= 0:
+            def fn(gx, gy, gz, m, d, tol, mo, mc):
+                return omni.solve_cascade(gx, gy, gz, m, d, tol, mo, mc, levels=args.cascade)
         fn(g[0], g[1], g[2], m, f["d"], tol, 2, 2)                               # warm-up (module load, pool)
         torch.cuda.synchronize()
         e0.record()
@@ -95,7 +100,7 @@ def converge(args, cfg, dtype):
     valid = ~np.isnan(Pn)
     a, b = Pn[valid] - Pn[valid].mean(), f["P"][valid] - f["P"][valid].mean()
     print(json.dumps({"converge": True, "workload": f"configs[{args.config}] {cfg['kind']} {cfg['n']} {dtype}", "tol": tol,
-                      "max_cg": args.max_cg, "batch": args.batch, "direct": bool(args.direct), "outer_iters": info["outer_iters"], "cg_iters": info["cg_iters_total"],
+                      "max_cg": args.max_cg, "batch": args.batch, "direct": bool(args.direct or args.cascade >= 0), "cascade_levels": args.cascade, "outer_iters": info["outer_iters"], "cg_iters": info["cg_iters_total"],
                       "seconds": sec, "eps_R": info["eps_R_final"], "status": info["status"],
                       "updates_per_s": N * info["cg_iters_total"] / sec,
                       "rel_l2_vs_analytic_P": float(np.linalg.norm(a - b) / np.linalg.norm(b))}))

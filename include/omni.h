@@ -95,14 +95,31 @@ int omni_solve_host_f32(int nx, int ny, int nz, double dx, double dy, double dz,
  * applying L instead of M -- inside the same outer loop, which here is an fp64 iterative refinement (the true
  * residual S - L P is re-evaluated from the fp64 master pressure, eps_R of Eq. 41, and the CG restarted on it).
  * It returns the field Alg. 1 converges to (zero mean on every connected component) in O(n) instead of O(n^2) CG
- * iterations for an n-cell-wide domain.  Typical caps: max_outer 10, max_cg a few thousand.  Arguments, layout,
- * ownership, status codes and omni_info as omni_solve_*. */
+ * iterations for an n-cell-wide domain.  Typical caps: max_outer 10, max_cg a few thousand.  d_P_init (device,
+ * [nz][ny][nx], may be NULL = zeros) is the first guess; the returned field differs from the P_init = 0
+ * one by a constant per connected component.  Other arguments, layout, ownership, status codes and omni_info as
+ * omni_solve_*. */
 int omni_solve_direct_f64(int nx, int ny, int nz, double dx, double dy, double dz,
                           const double* d_gx, const double* d_gy, const double* d_gz, const unsigned char* d_mask,
-                          double* d_P_out, double tol, int max_outer, int max_cg, void* stream, omni_info* info);
+                          const double* d_P_init, double* d_P_out, double tol, int max_outer, int max_cg, void* stream,
+                          omni_info* info);
 int omni_solve_direct_f32(int nx, int ny, int nz, double dx, double dy, double dz,
                           const float* d_gx, const float* d_gy, const float* d_gz, const unsigned char* d_mask,
-                          float* d_P_out, double tol, int max_outer, int max_cg, void* stream, omni_info* info);
+                          const float* d_P_init, float* d_P_out, double tol, int max_outer, int max_cg, void* stream,
+                          omni_info* info);
+
+/* omni_solve_direct_* with a cascadic first guess: the same system is first solved on up to `levels` grids coarsened by
+ * 2 along every axis (a coarse cell is valid iff one of its children is; its gradient is the mean over the valid
+ * children; coarsening stops before an axis would drop below 8 cells), coarsest first, each level's pressure being the
+ * first guess of the next finer one.  The coarse levels only produce guesses: tol, max_outer, max_cg apply to every
+ * level, info and the returned status are those of the finest level, whose solve alone decides the answer (the same
+ * field as omni_solve_direct_* up to tol and a constant per connected component).  levels = 0 is omni_solve_direct_*. */
+int omni_solve_cascade_f64(int nx, int ny, int nz, double dx, double dy, double dz,
+                           const double* d_gx, const double* d_gy, const double* d_gz, const unsigned char* d_mask,
+                           double* d_P_out, double tol, int max_outer, int max_cg, int levels, void* stream, omni_info* info);
+int omni_solve_cascade_f32(int nx, int ny, int nz, double dx, double dy, double dz,
+                           const float* d_gx, const float* d_gy, const float* d_gz, const unsigned char* d_mask,
+                           float* d_P_out, double tol, int max_outer, int max_cg, int levels, void* stream, omni_info* info);
 
 /* The two combined: nb snapshots on one mask (arguments as omni_solve_batch2d_*), inner systems L P = S. */
 int omni_solve_direct_batch2d_f64(int nx, int ny, int nb, double dx, double dy, const double* d_gx, const double* d_gy,

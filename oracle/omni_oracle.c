@@ -401,13 +401,14 @@ int oracle_solve(int nx, int ny, int nz, double dx, double dy, double dz,
  * (M - W^n) P = S, i.e. L P = S with L the symmetric positive semi-definite weighted graph Laplacian of the valid
  * cells (constant null space per connected component; S sums to zero on each).  CG on it from P = 0 returns the
  * solution with zero mean on every component.  NOT the paper's algorithm (SURVEY 8(f) NEXT-2 iii): same converged
- * field, a different iteration.  Same arguments and stopping rules as oracle_solve. */
+ * field, a different iteration.  Same arguments and stopping rules as oracle_solve, plus an optional first guess
+ * P_init (NULL = 0; :82), which shifts the result by a constant per component. */
 int oracle_solve_direct(int nx, int ny, int nz, double dx, double dy, double dz,
                         const double *gx, const double *gy, const double *gz, const unsigned char *mask,
-                        double *P_out, double tol, int max_outer, int max_cg, oracle_info *info)
+                        const double *P_init, double *P_out, double tol, int max_outer, int max_cg, oracle_info *info)
 {
     g_direct = 1;
-    int rc = solve_impl(nx, ny, nz, dx, dy, dz, gx, gy, gz, mask, NULL, P_out, tol, max_outer, max_cg, info, NULL, 0);
+    int rc = solve_impl(nx, ny, nz, dx, dy, dz, gx, gy, gz, mask, P_init, P_out, tol, max_outer, max_cg, info, NULL, 0);
     g_direct = 0;
     return rc;
 }

@@ -17,7 +17,7 @@ STATUS_NAMES = {0: "OMNI_OK", 1: "OMNI_NOT_CONVERGED", -1: "OMNI_ERR_INVALID_ARG
                 -3: "OMNI_ERR_ALLOC", -4: "OMNI_ERR_BREAKDOWN"}
 # every symbol include/omni.h declares
 SYMBOLS = ["omni_solve_f64", "omni_solve_f32", "omni_workspace_bytes", "omni_solve_f64_ws", "omni_solve_f32_ws",
-           "omni_solve_host_f64", "omni_solve_host_f32", "omni_solve_batch2d_f64", "omni_solve_batch2d_f32", "omni_solve_direct_f64", "omni_solve_direct_f32", "omni_solve_direct_batch2d_f64", "omni_solve_direct_batch2d_f32", "omni_constants", "omni_source_f64", "omni_source_f32",
+           "omni_solve_host_f64", "omni_solve_host_f32", "omni_solve_batch2d_f64", "omni_solve_batch2d_f32", "omni_solve_direct_f64", "omni_solve_direct_f32", "omni_solve_direct_batch2d_f64", "omni_solve_direct_batch2d_f32", "omni_solve_cascade_f64", "omni_solve_cascade_f32", "omni_constants", "omni_source_f64", "omni_source_f32",
            "omni_apply_M_f64", "omni_apply_M_f32", "omni_residual_f64", "omni_residual_f32", "omni_launch_count",
            "omni_set_loop_mode", "omni_release_memory", "omni_profile_enable", "omni_profile_read", "omni_status_string", "omni_version"]
 
@@ -185,9 +185,29 @@ def solve(gx, gy, gz, mask, d, tol, max_outer, max_cg, out=None, workspace=None,
     return P, (info.as_dict() if (want_info or host) else None)
 
 
-def solve_direct(gx, gy, gz, mask, d, tol, max_outer, max_cg, out=None):
+def solve_direct(gx, gy, gz, mask, d, tol, max_outer, max_cg, out=None, P_init=None):
     """omni_solve_direct_*: the fixed point of Algorithm 1 by CG on L P = S (not the paper's iteration; include/omni.h).
     CUDA tensors; d = (dx, dy[, dz]).  Returns (P, info dict)."""
+    import torch
+    sfx = _suffix(gx)
+    _check([gx, gy, gz, mask, out, P_init], "cuda")
+    if mask is not None and mask.dtype != torch.uint8:
+        raise TypeError("mask must be uint8")
+    if P_init is not None and (P_init.dtype != gx.dtype or P_init.shape != gx.shape):
+        raise TypeError("P_init must match gx in dtype and shape")
+    P = out if out is not None else torch.empty_like(gx)
+    info = Info()
+    with torch.cuda.device(gx.device):
+        fn = getattr(lib(), f"omni_solve_direct_{sfx}")
+        rc = fn(*_geom(gx, d), _ptr(gx), _ptr(gy), _ptr(gz), _ptr(mask), _ptr(P_init), _ptr(P), C.c_double(tol), C.c_int(max_outer),
+                C.c_int(max_cg), _stream(gx.device), C.byref(info))
+    if rc < 0:
+        raise OmniError(rc, f"omni_solve_direct_{sfx}")
+    return P, info.as_dict()
+
+
+def solve_cascade(gx, gy, gz, mask, d, tol, max_outer, max_cg, levels=3, out=None):
+    """omni_solve_cascade_*: omni_solve_direct_* started from a guess computed on `levels` coarser grids."""
     import torch
     sfx = _suffix(gx)
     _check([gx, gy, gz, mask, out], "cuda")
@@ -196,11 +216,11 @@ def solve_direct(gx, gy, gz, mask, d, tol, max_outer, max_cg, out=None):
     P = out if out is not None else torch.empty_like(gx)
     info = Info()
     with torch.cuda.device(gx.device):
-        fn = getattr(lib(), f"omni_solve_direct_{sfx}")
+        fn = getattr(lib(), f"omni_solve_cascade_{sfx}")
         rc = fn(*_geom(gx, d), _ptr(gx), _ptr(gy), _ptr(gz), _ptr(mask), _ptr(P), C.c_double(tol), C.c_int(max_outer),
-                C.c_int(max_cg), _stream(gx.device), C.byref(info))
+                C.c_int(max_cg), C.c_int(levels), _stream(gx.device), C.byref(info))
     if rc < 0:
-        raise OmniError(rc, f"omni_solve_direct_{sfx}")
+        raise OmniError(rc, f"omni_solve_cascade_{sfx}")
     return P, info.as_dict()
 
 

@@ -780,6 +780,66 @@ int solve_alloc(int nx, int ny, int nz, double dx, double dy, double dz, const T
     return rc;
 }
 
+// Cascadic first guess for the fixed-point solve: solve L P = S on grids coarsened by 2 (restrict_kernel), coarsest
+// first, and hand each level's pressure to the next finer one as its first guess (prolong_kernel).  The coarse levels
+// only produce guesses: their status is not examined, and the answer is whatever the finest-level solve, with the
+// caller's tol and caps, converges to.
+template <typename T>
+int solve_cascade(int nx, int ny, int nz, double dx, double dy, double dz, const T* gx, const T* gy, const T* gz,
+                  const unsigned char* mask, T* P_out, double tol, int max_outer, int max_cg, int levels, void* stream,
+                  omni_info* info)
+{
+    Geom g0;
+    if (!valid_common(nx, ny, nz, dx, dy, dz, tol, max_outer, max_cg) || levels < 0 || !make_geom(nx, ny, nz, (int)sizeof(T), g0))
+        return OMNI_ERR_INVALID_ARG;
+    if (!gx || !gy || (nz > 1 && !gz) || !P_out) return OMNI_ERR_INVALID_ARG;
+    cudaStream_t st = (cudaStream_t)stream;
+    struct Level { int nx, ny, nz, fx, fy, fz; double dx, dy, dz; const T *gx, *gy, *gz; const unsigned char* mask; T* P; void* own; };
+    std::vector<Level> lv;
+    lv.push_back(Level{ nx, ny, nz, 1, 1, 1, dx, dy, dz, gx, gy, gz, mask, P_out, nullptr });
+    const int ncomp = (nz > 1) ? 3 : 2;
+    int rc = OMNI_OK;
+    for (int l = 1; l <= levels && rc == OMNI_OK; ++l) {
+        const Level f = lv.back();
+        const int fx = f.nx > 1 ? 2 : 1, fy = f.ny > 1 ? 2 : 1, fz = f.nz > 1 ? 2 : 1;
+        const int cx = (f.nx + fx - 1) / fx, cy = (f.ny + fy - 1) / fy, cz = (f.nz + fz - 1) / fz;
+        // stop where a coarser grid is too small to be worth a solve (or would lose an axis of a 3D problem)
+        if ((fx == 2 && cx < 8) || (fy == 2 && cy < 8) || (fz == 2 && cz < 8)) break;
+        const size_t n = (size_t)cx * cy * cz;
+        const size_t bytes = align_up((ncomp + 1) * n * sizeof(T), 256) + align_up(n, 256);
+        void* own = nullptr;
+        if (pool_alloc(&own, bytes, st) != cudaSuccess) { cudaGetLastError(); rc = OMNI_ERR_ALLOC; break; }
+        T* b = (T*)own;
+        unsigned char* cm = (unsigned char*)own + align_up((ncomp + 1) * n * sizeof(T), 256);
+        Level c{ cx, cy, cz, fx, fy, fz, f.dx * fx, f.dy * fy, f.dz * fz, b, b + n, ncomp == 3 ? b + 2 * n : nullptr, cm,
+                 b + (size_t)ncomp * n, own };
+        restrict_kernel<T><<<blocks_for((long long)n, 256), 256, 0, st>>>(f.nx, f.ny, f.nz, fx, fy, fz, cx, cy, cz, ncomp, f.gx, f.gy,
+                                                                         f.gz, f.mask, b, b + n, ncomp == 3 ? b + 2 * n : nullptr, cm);
+        g_launches.fetch_add(1, std::memory_order_relaxed);
+        lv.push_back(c);
+        if (cudaGetLastError() != cudaSuccess) rc = OMNI_ERR_CUDA;
+    }
+    for (int l = (int)lv.size() - 1; l >= 0 && rc >= 0; --l) {
+        const Level& L = lv[l];
+        T* pinit = nullptr;
+        if (l + 1 < (int)lv.size()) {
+            const Level& C = lv[l + 1];
+            const size_t n = (size_t)L.nx * L.ny * L.nz;
+            if (pool_alloc((void**)&pinit, n * sizeof(T), st) != cudaSuccess) { cudaGetLastError(); rc = OMNI_ERR_ALLOC; break; }
+            prolong_kernel<T><<<blocks_for((long long)n, 256), 256, 0, st>>>(L.nx, L.ny, L.nz, C.fx, C.fy, C.fz, C.nx, C.ny, C.P, pinit);
+            g_launches.fetch_add(1, std::memory_order_relaxed);
+            if (cudaGetLastError() != cudaSuccess) { cudaFreeAsync(pinit, st); rc = OMNI_ERR_CUDA; break; }
+        }
+        const int r = solve_alloc<T>(L.nx, L.ny, L.nz, L.dx, L.dy, L.dz, L.gx, L.gy, L.gz, L.mask, L.P, tol, max_outer, max_cg, stream,
+                                     l == 0 ? info : nullptr, 0, pinit, 1);
+        if (pinit) cudaFreeAsync(pinit, st);
+        if (l == 0 || r < 0) rc = r;
+    }
+    for (auto& L : lv)
+        if (L.own) cudaFreeAsync(L.own, st);
+    return rc;
+}
+
 template <typename T>
 int solve_host(int nx, int ny, int nz, double dx, double dy, double dz, const T* gx, const T* gy, const T* gz,
                const unsigned char* mask, T* P_out, double tol, int max_outer, int max_cg, void* stream, omni_info* info)
@@ -1028,19 +1088,33 @@ int omni_solve_direct_batch2d_f32(int nx, int ny, int nb, double dx, double dy, 
 }
 
 int omni_solve_direct_f64(int nx, int ny, int nz, double dx, double dy, double dz, const double* d_gx, const double* d_gy,
-                          const double* d_gz, const unsigned char* d_mask, double* d_P_out, double tol, int max_outer,
-                          int max_cg, void* stream, omni_info* info)
+                          const double* d_gz, const unsigned char* d_mask, const double* d_P_init, double* d_P_out,
+                          double tol, int max_outer, int max_cg, void* stream, omni_info* info)
 {
     return solve_alloc<double>(nx, ny, nz, dx, dy, dz, d_gx, d_gy, d_gz, d_mask, d_P_out, tol, max_outer, max_cg, stream, info,
-                               0, nullptr, 1);
+                               0, d_P_init, 1);
 }
 
 int omni_solve_direct_f32(int nx, int ny, int nz, double dx, double dy, double dz, const float* d_gx, const float* d_gy,
-                          const float* d_gz, const unsigned char* d_mask, float* d_P_out, double tol, int max_outer,
-                          int max_cg, void* stream, omni_info* info)
+                          const float* d_gz, const unsigned char* d_mask, const float* d_P_init, float* d_P_out,
+                          double tol, int max_outer, int max_cg, void* stream, omni_info* info)
 {
     return solve_alloc<float>(nx, ny, nz, dx, dy, dz, d_gx, d_gy, d_gz, d_mask, d_P_out, tol, max_outer, max_cg, stream, info,
-                              0, nullptr, 1);
+                              0, d_P_init, 1);
+}
+
+int omni_solve_cascade_f64(int nx, int ny, int nz, double dx, double dy, double dz, const double* d_gx, const double* d_gy,
+                           const double* d_gz, const unsigned char* d_mask, double* d_P_out, double tol, int max_outer,
+                           int max_cg, int levels, void* stream, omni_info* info)
+{
+    return solve_cascade<double>(nx, ny, nz, dx, dy, dz, d_gx, d_gy, d_gz, d_mask, d_P_out, tol, max_outer, max_cg, levels, stream, info);
+}
+
+int omni_solve_cascade_f32(int nx, int ny, int nz, double dx, double dy, double dz, const float* d_gx, const float* d_gy,
+                           const float* d_gz, const unsigned char* d_mask, float* d_P_out, double tol, int max_outer,
+                           int max_cg, int levels, void* stream, omni_info* info)
+{
+    return solve_cascade<float>(nx, ny, nz, dx, dy, dz, d_gx, d_gy, d_gz, d_mask, d_P_out, tol, max_outer, max_cg, levels, stream, info);
 }
 
 int omni_constants(int nx, int ny, int nz, double dx, double dy, double dz, double* h_out13)

@@ -664,4 +664,50 @@ __global__ void pad_copy_kernel(Geom g, const TI* __restrict__ in, TO* __restric
     else if (i < g.nx) out[u] = (TO)in[pid];
 }
 
+// ------------------------------------------------------------------------------------------------ cascade (first guess)
+// omni_solve_cascade: grids coarsened by 2 along every axis longer than one cell.  A coarse cell is valid iff one of
+// its children is (in the box, mask != 0, no NaN component); its gradient is the mean over the valid children.
+// Caller layout (unpadded) on both sides; one thread per coarse cell.
+template <typename T>
+__global__ void restrict_kernel(int nx, int ny, int nz, int fx, int fy, int fz, int cx, int cy, int cz, int ncomp,
+                                const T* __restrict__ gx, const T* __restrict__ gy, const T* __restrict__ gz,
+                                const uint8_t* __restrict__ mask, T* __restrict__ ox, T* __restrict__ oy,
+                                T* __restrict__ oz, uint8_t* __restrict__ omask)
+{
+    const long long c = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const long long nc = (long long)cx * cy * cz;
+    if (c >= nc) return;
+    const int ci = (int)(c % cx), cj = (int)((c / cx) % cy), ck = (int)(c / ((long long)cx * cy));
+    T sx = T(0), sy = T(0), sz = T(0);
+    int cnt = 0;
+    for (int dk = 0; dk < fz; ++dk)
+        for (int dj = 0; dj < fy; ++dj)
+            for (int di = 0; di < fx; ++di) {
+                const int i = ci * fx + di, j = cj * fy + dj, k = ck * fz + dk;
+                if (i >= nx || j >= ny || k >= nz) continue;
+                const long long u = i + (long long)nx * (j + (long long)ny * k);
+                if (mask != nullptr && mask[u] == 0) continue;
+                const T a = gx[u], b = gy[u], e = (ncomp == 3) ? gz[u] : T(0);
+                if (isnan(a) || isnan(b) || isnan(e)) continue;
+                sx += a; sy += b; sz += e; ++cnt;
+            }
+    const T inv = cnt ? T(1) / T(cnt) : T(0);
+    ox[c] = sx * inv; oy[c] = sy * inv;
+    if (ncomp == 3) oz[c] = sz * inv;
+    omask[c] = cnt ? 1 : 0;
+}
+
+// first guess of a level: the parent's pressure (0 where the parent is missing); one thread per fine cell
+template <typename T>
+__global__ void prolong_kernel(int nx, int ny, int nz, int fx, int fy, int fz, int cx, int cy,
+                               const T* __restrict__ Pc, T* __restrict__ Pf)
+{
+    const long long u = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const long long n = (long long)nx * ny * nz;
+    if (u >= n) return;
+    const int i = (int)(u % nx), j = (int)((u / nx) % ny), k = (int)(u / ((long long)nx * ny));
+    const T v = Pc[(i / fx) + (long long)cx * ((j / fy) + (long long)cy * (k / fz))];
+    Pf[u] = isnan(v) ? T(0) : v;
+}
+
 }  // namespace omni

@@ -373,6 +373,44 @@ def test_direct_solve_converged(oracle, dtype, tol):
         assert rel_l2_after_mean_removal(P2.cpu().numpy(), P, valid) <= (1e-4 if dtype == "f64" else 5e-3)
 
 
+@pytest.mark.parametrize("dtype,tol", [("f64", 1e-8), ("f32", 1e-5)])
+def test_cascade_first_guess(oracle, dtype, tol):
+    """omni_solve_cascade_*: the coarse levels only supply a first guess, so what is checked is what is unique -- the
+    returned field meets Eq. 41 with the oracle's operators and equals the direct solve's (hence the oracle's) to the
+    tolerance -- plus that the guess pays (fewer finest-level CG iterations at the fp32 tolerance).  levels = 0 is the direct solve, bitwise.
+    Odd sizes (ragged children), a masked 3D case, a 2D case."""
+    cases = [("sphere3d", (45, 51, 67), 3), ("lamb_oseen2d", (150, 131), 4), ("fourier3d", (33, 40, 38), 2)]
+    for kind, shape, levels in cases:
+        f = make_field(kind, shape, seed=4, noise=0.05, kmax=3.0)
+        g_dev, g_or, m_dev, m = _inputs(f, dtype)
+        d = f["d"]
+        Pd, idd = omni.solve_direct(g_dev[0], g_dev[1], g_dev[2], m_dev, d, tol, 20, 5000)
+        P0, i0 = omni.solve_cascade(g_dev[0], g_dev[1], g_dev[2], m_dev, d, tol, 20, 5000, levels=0)
+        assert i0 == idd and np.array_equal(P0.cpu().numpy(), Pd.cpu().numpy(), equal_nan=True)
+        Pc, ic = omni.solve_cascade(g_dev[0], g_dev[1], g_dev[2], m_dev, d, tol, 20, 5000, levels=levels)
+        assert ic["status"] == 0 and ic["eps_R_final"] <= tol
+        # the guess pays at the fp32 tolerance (the smooth part of the error is gone); at 1e-8 on these small noisy cases
+        # the finest level still has to resolve the noise and the count is about the same
+        if dtype == "f32":
+            assert ic["cg_iters_total"] < idd["cg_iters_total"], (kind, ic, idd)
+        else:
+            assert ic["cg_iters_total"] <= 1.15 * idd["cg_iters_total"] + 5, (kind, ic, idd)
+        Pn, Pdn = Pc.cpu().numpy().astype(np.float64), Pd.cpu().numpy().astype(np.float64)
+        valid = ~np.isnan(Pdn)
+        assert np.array_equal(np.isnan(Pn), ~valid)
+        v = oracle.validity(g_or[0], g_or[1], g_or[2], m)
+        assert np.array_equal(v == 1, valid)
+        w1, w0, w0C = oracle.weights(v, *d)
+        S = oracle.source(v, w1, w0, g_or[0], g_or[1], g_or[2], *d)
+        Pz = np.nan_to_num(Pn)
+        r0 = oracle.apply_Wn(v, w0, w0C, Pz) + S - oracle.apply_M(v, w1, Pz)
+        assert np.linalg.norm(r0) / np.linalg.norm(S) <= (1.05 * tol if dtype == "f64" else 3 * tol)
+        # same field as the direct solve (one connected component in these cases): tolerance-level agreement
+        assert rel_l2_after_mean_removal(Pn, Pdn, valid) <= (1e-5 if dtype == "f64" else 5e-3)
+        Po, io = oracle.solve_direct(g_or[0], g_or[1], g_or[2], m, *d, tol=tol, max_outer=20, max_cg=5000)
+        assert rel_l2_after_mean_removal(Pn, Po, valid) <= (1e-5 if dtype == "f64" else 5e-3)
+
+
 @pytest.mark.parametrize("dtype", ["f64", "f32"])
 def test_persistent_loop_stress(dtype):
     """The persistent kernel's grid barrier under every mix of phases (max_cg = 0, 1, 2, 3, 16: the outer and the
