@@ -444,7 +444,11 @@ def test_direct_solve_vs_dense_pseudo_inverse(oracle, shape, sp):
     from scipy.sparse import csr_matrix
     from scipy.sparse.csgraph import connected_components
     ncomp, lab = connected_components(csr_matrix(np.abs(Lk) > 0), directed=False)
-    for other, bound in ((P2, 1e-8), (Pr, 1e-6)):
+    # a first guess (:82) only moves the constant of each component
+    Pg, ig = oracle.solve_direct(g[0], g[1], g[2], mask, *sp, tol=1e-12, max_outer=5, max_cg=2000,
+                                 P_init=rng.normal(size=shape))
+    assert ig["converged"]
+    for other, bound in ((P2, 1e-8), (Pr, 1e-6), (Pg, 1e-8)):
         a, b = other.ravel()[keep].copy(), Pstar.copy()
         for cpt in range(ncomp):
             m = lab == cpt
