@@ -29,8 +29,17 @@ UNIT = "grid-point CG updates/s"
 CPU_SAMPLE_EDGE = 320                   # 3D: edge of the corner crop the oracle is timed on (2D: the whole grid);
                                         # with the step's own caps that is ~10 s of work on 16 host threads
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel (K4) from the ncu --set full capture
-# summarised in profiles/r1_ncu_k3_k4_500cube_f32.md; only valid for that workload.
-NCU_TRAFFIC_K4 = {(4, "f32"): 1.526446e9 + 0.955657e9}
+# summarised in profiles/r1_ncu_k3_k4_500cube_f32.md; only valid for that workload.  K4 streams different arrays by
+# CG-iteration parity (lazy delta): even k, the first odd k (delta not read yet), the other odd k.
+NCU_TRAFFIC_K4 = {(4, "f32"): {"even": 1.021704e9 + 0.461907e9, "odd_first": 1.530113e9 + 0.963922e9,
+                               "odd": 2.028161e9 + 0.963717e9}}
+
+
+def k4_traffic(t, n_even, n_odd):
+    """Average measured DRAM bytes per K4 launch over the step's mix of even / first-odd / odd CG iterations."""
+    if t is None:
+        return None
+    return (n_even * t["even"] + (t["odd_first"] if n_odd else 0.0) + max(n_odd - 1, 0) * t["odd"]) / (n_even + n_odd)
 
 
 def parse():
@@ -312,12 +321,16 @@ def main():
     k2_ms, k2_n = prof["K2"]
     t4 = k4_ms / max(k4_n, 1) * 1e-3
     t3 = k3_ms / max(k3_n, 1) * 1e-3
-    alg4, alg3 = 5 * esz * N, 3 * esz * N          # K4: R p,r,delta W r,delta ; K3: R r,p W p
+    # K3: R r,p W p.  K4 (lazy delta): even CG iterations R p,r W r (3 passes), odd ones
+    # R p,p_old,r,delta W r,delta (6 passes; the first odd one does not read delta): the average over the step's launches
+    n_even, n_odd = (STEP_MAX_CG + 1) // 2, STEP_MAX_CG // 2
+    k4_passes = (3 * n_even + 6 * n_odd - (1 if n_odd else 0)) / STEP_MAX_CG
+    alg4, alg3 = k4_passes * esz * N, 3 * esz * N
     ach = alg4 / t4 / 1e9 if t4 > 0 else 0.0
     roofline = {"bound": "hbm", "kernel": "K4 tma_kernel<OpT4> (operator recomputed + axpys + r.r)",
                 "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak, "peak_source": peak_src,
-                "traffic": NCU_TRAFFIC_K4.get((args.config, dtype)),
-                "algorithmic_bytes_per_launch": alg4, "us_per_launch": t4 * 1e6,
+                "traffic": k4_traffic(NCU_TRAFFIC_K4.get((args.config, dtype)), n_even, n_odd),
+                "algorithmic_bytes_per_launch": alg4, "k4_passes_avg": k4_passes, "us_per_launch": t4 * 1e6,
                 "k3": {"achieved": alg3 / t3 / 1e9 if t3 > 0 else 0.0, "us_per_launch": t3 * 1e6,
                        "algorithmic_bytes_per_launch": alg3},
                 "cg_iteration": {"us": (t3 + t4) * 1e6, "achieved": (alg3 + alg4) / (t3 + t4) / 1e9 if t3 + t4 > 0 else 0.0,

@@ -19,7 +19,7 @@ using namespace omni;
 #ifndef OMNI_BY
 #define OMNI_BY 8
 #define OMNI_D3 6
-#define OMNI_D4 5
+#define OMNI_D4 4      // K4 ring depth in its 4-array iterations ({p_h, r, p_old, delta}); 7 in the 2-array ones
 #define OMNI_MINB 3
 #define OMNI_PERSIST_MAX_CELLS 1500000LL   // automatic mode: grids up to this many padded cells take the persistent loop
 #define OMNI_PERSIST_SMALL_CELLS 65536LL   // persistent loop: 512-thread CTAs up to here, 1024-thread CTAs above
@@ -307,7 +307,8 @@ __global__ void init_scalars_kernel(Scalars* sc, double tol, int max_outer, int 
 struct MarchCfg { dim3 grid, block; int zlen; };
 
 // K2 / K3 / K4: TMA + mbarrier pipeline (omni_tma.cuh): 512-byte x 8-row tiles, 8 consumer warps + 1 producer warp,
-// several CTAs per SM (shared memory: K3 6 stages x 10.8 KB, K4 5 x 13.4 KB, K2 5 x 10.3 KB fp32 / 4 x 14.8 KB fp64).
+// several CTAs per SM (shared memory: K3 6 stages x 10.8 KB, K4 4 x 17.4 KB or 7 x 9.4 KB by iteration parity,
+// K2 5 x 10.3 KB fp32 / 4 x 14.8 KB fp64).
 template <typename T, bool LOP = false> using K3 = OpT3<T, OMNI_BY, OMNI_D3, OMNI_MINB, LOP>;
 template <typename T, bool LOP = false> using K4 = OpT4<T, OMNI_BY, OMNI_D4, (sizeof(T) == 8 ? 2 : OMNI_MINB), LOP>;   // fp64 K4: 72 registers spill
 template <typename T> using K2 = OpT2<T, OMNI_BY, (sizeof(T) == 8 ? 4 : 5), OMNI_MINB>;
@@ -317,7 +318,7 @@ template <class Op>
 MarchCfg tma_config(const Geom& g)
 {
     using TG = typename Op::TG;
-    constexpr int SMEM = Op::D * Op::STAGE_BYTES + 128;
+    constexpr int SMEM = Op::SMEM_BYTES + 128;
     static int slots_cache = 0;
     if (slots_cache == 0) {
         int dev = 0, sms = 148, occ = 1;
@@ -356,7 +357,7 @@ template <class Op>
 cudaError_t launch_tma(const Geom& g, const typename Op::Args& a, const TmaSet& maps, cudaStream_t st)
 {
     const MarchCfg c = tma_config<Op>(g);
-    tma_kernel<Op><<<c.grid, c.block, Op::D * Op::STAGE_BYTES + 128, st>>>(g, c.zlen, a, maps);
+    tma_kernel<Op><<<c.grid, c.block, Op::SMEM_BYTES + 128, st>>>(g, c.zlen, a, maps);
     g_launches.fetch_add(1, std::memory_order_relaxed);
     return cudaGetLastError();
 }
@@ -481,12 +482,32 @@ bool make_tma_set(const Geom& g, const Workspace<T>& w, TmaSet& m)
     return encode_map<T>(&m.r_h, g, w.r, hx, hy) && encode_map<T>(&m.p_h[0], g, w.p0, hx, hy) &&
            encode_map<T>(&m.p_h[1], g, w.p1, hx, hy) && encode_map<T>(&m.r_c, g, w.r, TG::BX, TG::BY) &&
            encode_map<T>(&m.d_c, g, w.delta, TG::BX, TG::BY) &&
+           encode_map<T>(&m.p_c[0], g, w.p0, TG::BX, TG::BY) && encode_map<T>(&m.p_c[1], g, w.p1, TG::BX, TG::BY) &&
            encode_map<double>(&m.P_h[0], g, w.P, 64 + 4, TG::BY + 2) && encode_map<double>(&m.P_h[1], g, w.P1, 64 + 4, TG::BY + 2) &&
            encode_map<T>(&m.d2_h, g, w.delta, 64 + 2 * (16 / (int)sizeof(T)), TG::BY + 2) &&
            encode_map<T>(&m.S_c, g, w.S, 64, TG::BY);
 }
 
 // ------------------------------------------------------------------------------------------------ loop drivers
+
+// delta += alpha p of a CG iteration K4 left pending (lazy delta); no-op kernel when nothing is pending
+template <typename T>
+cudaError_t launch_flush(const Geom& g, const Workspace<T>& w, cudaStream_t st)
+{
+    static int nsm = 0;
+    if (nsm == 0) {
+        int dev = 0;
+        cudaGetDevice(&dev);
+        if (cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || nsm < 1) nsm = 148;
+    }
+    constexpr int V = 16 / (int)sizeof(T);
+    long long nb = (g.npad / V + 255) / 256;
+    if (nb > 8LL * nsm) nb = 8LL * nsm;
+    if (nb < 1) nb = 1;
+    flush_delta_kernel<T><<<(unsigned)nb, 256, 0, st>>>(g.npad, w.delta, w.p0, w.p1, w.sc);
+    g_launches.fetch_add(1, std::memory_order_relaxed);
+    return cudaGetLastError();
+}
 
 // Host-driven loop (debug / profiling): one synchronisation per outer iteration (plus one per 16 CG iterations).
 template <typename T, bool LOP>
@@ -536,6 +557,7 @@ int run_loop_host(const Geom& g, const Workspace<T>& w, const HostConst& H, cons
             synced = true;
             if (!h.inner_go) break;
         }
+        if (rc == OMNI_OK && launch_flush<T>(g, w, st) != cudaSuccess) rc = OMNI_ERR_CUDA;
         if (rc == OMNI_OK && !synced) {
             if (cudaMemcpyAsync(&h, w.sc, sizeof(Scalars), cudaMemcpyDeviceToHost, st) != cudaSuccess ||
                 cudaStreamSynchronize(st) != cudaSuccess) rc = OMNI_ERR_CUDA;
@@ -616,7 +638,11 @@ int run_loop_graph(const Geom& g, const Workspace<T>& w, const HostConst& H, con
         cudaError_t e3 = launch_tma<K3<T, LOP>>(g, k3_args<T, LOP>(w, K, ch), maps, cap);
         cudaError_t e4 = launch_tma<K4<T, LOP>>(g, k4_args<T, LOP>(w, K, ch), maps, cap);
         if (cudaStreamEndCapture(cap, &tmp) != cudaSuccess || e3 != cudaSuccess || e4 != cudaSuccess) break;
-        g_launches.fetch_sub(3, std::memory_order_relaxed);     // captured, not launched; counted from the device state
+        // after the inner loop: the delta update an even last iteration left pending
+        if (cudaStreamBeginCaptureToGraph(cap, bodyOuter, &nInner, nullptr, 1, cudaStreamCaptureModeThreadLocal) != cudaSuccess) break;
+        cudaError_t ef = launch_flush<T>(g, w, cap);
+        if (cudaStreamEndCapture(cap, &tmp) != cudaSuccess || ef != cudaSuccess) break;
+        g_launches.fetch_sub(4, std::memory_order_relaxed);     // captured, not launched; counted from the device state
 
         if (cudaGraphInstantiate(&exec, G, 0) != cudaSuccess) break;
         if (cudaGraphLaunch(exec, st) != cudaSuccess) break;
@@ -757,7 +783,7 @@ int solve_ws(int nx, int ny, int nz, double dx, double dy, double dz, const T* g
         info->norm_S = std::sqrt(h.normS2);
         info->eps_R_final = (h.normS2 > 0.0) ? std::sqrt(h.epsR2 / h.normS2) : 0.0;
         info->status = h.status;
-        if (mode == 2) g_launches.fetch_add((long long)(h.normS2 > 0.0 ? h.n + 1 : 0) + 2 * h.cg_total, std::memory_order_relaxed);
+        if (mode == 2) g_launches.fetch_add((long long)(h.normS2 > 0.0 ? 2 * h.n + 1 : 0) + 2 * h.cg_total, std::memory_order_relaxed);
         return h.status;
     }
     return OMNI_OK;

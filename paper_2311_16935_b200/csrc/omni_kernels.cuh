@@ -70,6 +70,7 @@ __device__ __forceinline__ XEdge make_xedge(const Geom& g, int x)
 // device-resident loop state: no scalar ever visits the host inside the iteration
 struct Scalars {
     double rho, gamma, alpha, beta;
+    double alpha_prev; // alpha of the CG iteration whose delta update is pending (lazy delta, omni_tma.cuh K4)
     double normS2;     // ||S||^2
     double thresh2;    // (0.1 * tol)^2 * ||S||^2   inner stop (A3)
     double tol2S;      // tol^2 * ||S||^2           outer stop (Eq. 41)
@@ -79,6 +80,7 @@ struct Scalars {
     int k;             // CG iteration index inside the current outer iteration
     int n;             // outer iterations done
     int inner_go, outer_go;
+    int pend;          // 1: delta still lacks alpha_prev * p of the last (even) CG iteration
     int status;        // omni_status
     int max_cg, max_outer;
     unsigned int ticket[4];

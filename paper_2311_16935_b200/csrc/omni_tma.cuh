@@ -58,6 +58,7 @@ struct alignas(64) TmaSet {
     CUtensorMap r_h, p_h[2];     // boxes with halo: (BX + 2 HX) x (BY + 2) x 1
     CUtensorMap r_c, d_c;        // plain boxes: BX x BY x 1
     // K2 (64-cell tiles: the fp64 master pressure sets the 16-byte lane chunk)
+    CUtensorMap p_c[2];          // plain: both p buffers (K4's lazy delta update reads p_{k-1} without halo)
     CUtensorMap P_h[2], d2_h;    // haloed: P (fp64, both buffers), delta (T)
     CUtensorMap S_c;             // plain: S (T)
 };
@@ -122,11 +123,11 @@ tma_kernel(const Geom g, const int zlen, const typename Op::Args a, const __grid
 {
     using TG = typename Op::TG;
     using T = typename Op::VT;
-    constexpr int V = TG::V, BX = TG::BX, BY = TG::BY, D = Op::D, NACC = Op::NACC;
+    constexpr int V = TG::V, BX = TG::BX, BY = TG::BY, NACC = Op::NACC;
     extern __shared__ __align__(128) char smem_raw[];
     __shared__ double red[NACC][BY + 1];
     __shared__ int is_last;
-    __shared__ __align__(8) unsigned long long bars[2 * D];
+    __shared__ __align__(8) unsigned long long bars[2 * Op::DMAX];
 
     if (!Op::active(a)) {
         if (threadIdx.x == 0 && blockIdx.x == 0 && blockIdx.y == 0 && blockIdx.z == 0) Op::idle(a);
@@ -142,6 +143,9 @@ tma_kernel(const Geom g, const int zlen, const typename Op::Args a, const __grid
     const int k0 = blockIdx.z * zlen, k1 = min(g.nz, k0 + zlen);
     const int E = k1 - k0 + 2;                       // events: planes k0-1 .. k1
     const typename Op::Ctx ctx(a);
+    // ring depth and stage size may depend on what this launch streams (K4: DESIGN.md section 6, lazy delta)
+    const int D = Op::stages(ctx);
+    const uint32_t SB = (uint32_t)Op::stage_bytes(ctx);
 
     if (threadIdx.x == 0) {
         for (int s = 0; s < D; ++s) { mbar_init(bar_s + 8 * s, 1); mbar_init(bar_s + 8 * (D + s), BY); }
@@ -161,7 +165,7 @@ tma_kernel(const Geom g, const int zlen, const typename Op::Args a, const __grid
             for (int e = 0; e < E; ++e) {
                 if (e >= D) mbar_wait(bar_s + 8 * (D + s), phase);
                 const int c = k0 - 1 + e;
-                Op::produce(a, ctx, maps, smem_s + (uint32_t)(s * Op::STAGE_BYTES), bar_s + 8 * s, x0, y0, c,
+                Op::produce(a, ctx, maps, smem_s + (uint32_t)s * SB, bar_s + 8 * s, x0, y0, c,
                             (c >= k0) && (c < k1));
                 s = (s + 1 == D) ? 0 : s + 1;
                 phase ^= (s == 0);
@@ -234,7 +238,7 @@ tma_kernel(const Geom g, const int zlen, const typename Op::Args a, const __grid
                 aB = aC; aC = aF;
                 s = (s + 1 == D) ? 0 : s + 1;
                 phase ^= (s == 0);
-                aF = smem_s + (uint32_t)(s * Op::STAGE_BYTES);
+                aF = smem_s + (uint32_t)s * SB;
             }
         };
         if (anyf) run(std::false_type{}); else run(std::true_type{});
@@ -290,8 +294,8 @@ template <typename T, int BY_, int D_, int MINB_, bool LOP_ = false>
 struct OpT3 {
     using VT = T;
     using TG = TileGeom<T, BY_>;
-    enum { V = TG::V, D = D_, MINB = MINB_, NACC = 1, TICKET = 0, STAGE_BYTES = 2 * TG::TILE_H,
-           BOX_H = (BY_ + 2) * TG::PITCH_H };
+    enum { V = TG::V, D = D_, DMAX = D_, MINB = MINB_, NACC = 1, TICKET = 0, STAGE_BYTES = 2 * TG::TILE_H,
+           SMEM_BYTES = D_ * STAGE_BYTES, BOX_H = (BY_ + 2) * TG::PITCH_H };
     struct Args {
         T* pbuf[2]; const uint32_t* wcode; const uint8_t* link; const uint32_t* flags; const uint32_t* tflags;
         Coef<T> K; Scalars* sc; double* partial; CondHandles cond;
@@ -301,6 +305,8 @@ struct OpT3 {
         __device__ Ctx(const Args& a) { beta = (T)a.sc->beta; par = a.sc->k & 1; pnew = a.pbuf[par ^ 1]; }
     };
     using TC = XEdge;
+    __device__ static int stages(const Ctx&) { return D; }
+    __device__ static int stage_bytes(const Ctx&) { return STAGE_BYTES; }
     __device__ static TC thread_init(const Geom& g, int x) { return make_xedge<V>(g, x); }
     __device__ static bool active(const Args& a) { return a.sc->inner_go != 0; }
     __device__ static void idle(const Args& a) { set_cond(a.cond, -1, 0); }
@@ -381,12 +387,20 @@ struct OpT3 {
 };
 
 // ------------------------------------------------------------------------------------------------ K4 (TMA)
-// q = M p recomputed from the haloed p tile; delta += alpha p; r -= alpha q; rho' = r.r; beta, loop test.
-template <typename T, int BY_, int D_, int MINB_, bool LOP_ = false>
+// q = A p recomputed from the haloed p tile; r -= alpha q; rho' = r.r; beta, loop test.
+// Lazy delta: delta does not have to exist between CG iterations, only when K2 folds it into P.  Both p buffers are
+// alive in K4 -- p_k (haloed, for the stencil) and p_{k-1} (K3 overwrites it only in the next iteration) -- so delta
+// is touched every SECOND iteration: even k stream {p, r} and leave alpha_k p_k pending; odd k stream {p, p_old, r,
+// delta} and apply delta += alpha_{k-1} p_{k-1} + alpha_k p_k.  7.5 instead of 8 passes per CG iteration on average
+// (K4: 3 / 6 instead of 5 / 5).  A pending update at loop exit is applied by flush_delta_kernel before K2.
+// The ring is sized per parity: DO_ stages of {p_h, r, p_old, delta} or as many {p_h, r} stages as fit the same bytes.
+template <typename T, int BY_, int DO_, int MINB_, bool LOP_ = false>
 struct OpT4 {
     using VT = T;
     using TG = TileGeom<T, BY_>;
-    enum { V = TG::V, D = D_, MINB = MINB_, NACC = 1, TICKET = 1, STAGE_BYTES = TG::TILE_H + 2 * TG::TILE_C,
+    enum { V = TG::V, MINB = MINB_, NACC = 1, TICKET = 1,
+           STAGE_ODD = TG::TILE_H + 3 * TG::TILE_C, STAGE_EVEN = TG::TILE_H + TG::TILE_C,
+           D_ODD = DO_, D_EVEN = (DO_ * STAGE_ODD) / STAGE_EVEN, DMAX = D_EVEN, SMEM_BYTES = DO_ * STAGE_ODD,
            BOX_H = (BY_ + 2) * TG::PITCH_H };
     struct Args {
         T* r; T* delta; int p_fixed;      // p_fixed >= 0: read p from pbuf[p_fixed] (omni_apply_M), else by parity
@@ -395,28 +409,37 @@ struct OpT4 {
         T* q_out;                         // only for omni_apply_M: store q, leave r / delta untouched
     };
     struct Ctx {
-        T alpha; int pidx; bool first;
+        T alpha, alpha_prev; int pidx, pold; bool odd, first, step;
         __device__ Ctx(const Args& a)
         {
+            const int k = a.sc->k;
             alpha = (T)a.sc->alpha;
-            first = (a.sc->k == 0);
-            pidx = (a.p_fixed >= 0) ? a.p_fixed : ((a.sc->k & 1) ^ 1);
+            alpha_prev = (T)a.sc->alpha_prev;
+            step = (a.q_out != nullptr);
+            odd = (k & 1) != 0;
+            first = (k == 1);                        // first delta write of this inner solve: delta counts as zero
+            pidx = (a.p_fixed >= 0) ? a.p_fixed : ((k & 1) ^ 1);
+            pold = k & 1;
         }
     };
     using TC = XEdge;
+    __device__ static int stages(const Ctx& c) { return (c.odd || c.step) ? D_ODD : D_EVEN; }
+    __device__ static int stage_bytes(const Ctx& c) { return (c.odd || c.step) ? STAGE_ODD : STAGE_EVEN; }
     __device__ static TC thread_init(const Geom& g, int x) { return make_xedge<V>(g, x); }
     __device__ static bool active(const Args& a) { return a.sc->inner_go != 0; }
     __device__ static void idle(const Args& a) { set_cond(a.cond, -1, 0); }
     __device__ static void load_codes(const Args& a, long long cell, uint32_t (&code)[V]) { load_cell_codes<LOP_, V>(a.wcode, a.link, cell, code); }
-    __device__ static void produce(const Args& a, const Ctx& c, const TmaSet& m, uint32_t stage, uint32_t bar, int x0,
+    __device__ static void produce(const Args&, const Ctx& c, const TmaSet& m, uint32_t stage, uint32_t bar, int x0,
                                    int y0, int plane, bool inner)
     {
-        const bool ext = inner && (a.q_out == nullptr);
-        const bool dl = ext && !c.first;           // first CG iteration: delta counts as zero, never read
-        mbar_expect_tx(bar, BOX_H + (ext ? TG::TILE_C : 0) + (dl ? TG::TILE_C : 0));
+        const bool ext = inner && !c.step;
+        const bool upd = ext && c.odd;
+        const bool dl = upd && !c.first;
+        mbar_expect_tx(bar, BOX_H + (ext ? TG::TILE_C : 0) + (upd ? TG::TILE_C : 0) + (dl ? TG::TILE_C : 0));
         tma_load_3d(stage, &m.p_h[c.pidx], bar, x0 - TG::HX, y0 - 1, plane);
         if (ext) tma_load_3d(stage + TG::TILE_H, &m.r_c, bar, x0, y0, plane);
-        if (dl) tma_load_3d(stage + TG::TILE_H + TG::TILE_C, &m.d_c, bar, x0, y0, plane);
+        if (upd) tma_load_3d(stage + TG::TILE_H + TG::TILE_C, &m.p_c[c.pold], bar, x0, y0, plane);
+        if (dl) tma_load_3d(stage + TG::TILE_H + 2 * TG::TILE_C, &m.d_c, bar, x0, y0, plane);
     }
     struct State {};
     __device__ static void advance(State&, const Ctx&, uint32_t, int, int) {}
@@ -443,24 +466,26 @@ struct OpT4 {
         if (!out) return;
         T q[V];
         apply_op_chunk<LOP_, T, V>(q, vm, vc, vp, vn, vs, xl, xr, CLEAN ? 0u : fb, code, a.K, xe, ycls, zcls);
-        if (a.q_out != nullptr) {
+        if (c.step) {
             st_chunk<T, V>(a.q_out + idx, q);
-#pragma unroll
-            for (int i = 0; i < V; ++i) acc += (double)vc[i] * (double)q[i];
+            acc += chunk_dot<T, V>(vc, q);
             return;
         }
         const int eoff = TG::TILE_H + (warp * TG::BX + lane * V) * (int)sizeof(T);
-        T er[V], ed[V], rn[V], dn[V];
+        T er[V], rn[V];
         lds_chunk<T, V>(sC + eoff, er);
-        if (c.first) zero_chunk<T, V>(ed); else lds_chunk<T, V>(sC + eoff + TG::TILE_C, ed);
 #pragma unroll
-        for (int i = 0; i < V; ++i) {
-            rn[i] = er[i] - c.alpha * q[i];
-            dn[i] = ed[i] + c.alpha * vc[i];
-        }
+        for (int i = 0; i < V; ++i) rn[i] = er[i] - c.alpha * q[i];
         acc += chunk_dot<T, V>(rn, rn);
         st_chunk<T, V>(a.r + idx, rn);
-        st_chunk<T, V>(a.delta + idx, dn);
+        if (c.odd) {
+            T ep[V], ed[V], dn[V];
+            lds_chunk<T, V>(sC + eoff + TG::TILE_C, ep);
+            if (c.first) zero_chunk<T, V>(ed); else lds_chunk<T, V>(sC + eoff + 2 * TG::TILE_C, ed);
+#pragma unroll
+            for (int i = 0; i < V; ++i) dn[i] = (ed[i] + c.alpha_prev * ep[i]) + c.alpha * vc[i];
+            st_chunk<T, V>(a.delta + idx, dn);
+        }
     }
     __device__ static void finalize(const Args& a, const double (&tot)[1])
     {
@@ -472,6 +497,7 @@ struct OpT4 {
             set_cond(a.cond, 0, 0);
             return;
         }
+        if (s->k & 1) { s->pend = 0; } else { s->pend = 1; s->alpha_prev = s->alpha; }
         s->beta = rho1 / s->rho;
         s->rho = rho1;
         s->k += 1;
@@ -481,6 +507,28 @@ struct OpT4 {
         set_cond(a.cond, -1, go);
     }
 };
+
+// delta += alpha_prev * p_last for the update an even last CG iteration left pending (no-op otherwise); K2, which runs
+// next, clears the flag.  One 16-byte chunk per thread step, grid-stride.
+template <typename T>
+__global__ void flush_delta_kernel(long long npad, T* __restrict__ delta, const T* p0, const T* p1, const Scalars* sc)
+{
+    if (!sc->pend) return;
+    constexpr int V = 16 / (int)sizeof(T);
+    const int k = sc->k;                             // iterations done; the pending one is k - 1 (even)
+    const T* __restrict__ p = ((k - 1) & 1) ? p0 : p1;        // p_{k-1} lives in pbuf[((k-1) & 1) ^ 1]
+    const T al = (T)sc->alpha_prev;
+    const bool first = (k == 1);
+    for (long long c = ((long long)blockIdx.x * blockDim.x + threadIdx.x) * V; c < npad;
+         c += (long long)gridDim.x * blockDim.x * V) {
+        T pv[V], dv[V];
+        ld_chunk<T, V>(p + c, pv);
+        if (first) zero_chunk<T, V>(dv); else ld_chunk<T, V>(delta + c, dv);
+#pragma unroll
+        for (int i = 0; i < V; ++i) dv[i] += al * pv[i];
+        st_chunk<T, V>(delta + c, dv);
+    }
+}
 
 // ------------------------------------------------------------------------------------------------ K2 (TMA)
 // outer boundary update (Eq. 12 collapsed): P <- P + delta (into the other P buffer);
@@ -507,7 +555,8 @@ struct OpT2 {
         static constexpr int TILE_P = (BOX_P + 127) / 128 * 128, TILE_D = (BOX_D + 127) / 128 * 128;
         static constexpr int TILE_S = BY_ * BX * (int)sizeof(T);
     };
-    enum { V = 2, D = D_, MINB = MINB_, NACC = 2, TICKET = 2, STAGE_BYTES = TG::TILE_P + TG::TILE_D + TG::TILE_S };
+    enum { V = 2, D = D_, DMAX = D_, MINB = MINB_, NACC = 2, TICKET = 2, STAGE_BYTES = TG::TILE_P + TG::TILE_D + TG::TILE_S,
+           SMEM_BYTES = D_ * STAGE_BYTES };
     struct Args {
         double* Pbuf[2]; T* r; const uint8_t* link; const uint32_t* flags; const uint32_t* tflags;
         double t[3]; Scalars* sc; double* partial; CondHandles cond;
@@ -536,6 +585,8 @@ struct OpT2 {
         }
         return lk;
     }
+    __device__ static int stages(const Ctx&) { return D; }
+    __device__ static int stage_bytes(const Ctx&) { return STAGE_BYTES; }
     __device__ static bool active(const Args& a) { return a.sc->outer_go != 0; }
     __device__ static void idle(const Args& a) { set_cond(a.cond, 0, 0); }
     __device__ static void load_codes(const Args& a, long long cell, uint32_t (&code)[V])
@@ -630,6 +681,7 @@ struct OpT2 {
         }
         s->n += 1;
         s->k = 0;
+        s->pend = 0;
         s->beta = 0.0;
         s->rho = tot[1];
         const int go = (tot[1] > s->thresh2) && (tot[1] != 0.0) && (s->max_cg > 0);

@@ -65,7 +65,9 @@ def test_fullsize_config(oracle, idx, dtype):
     q_s = q.flatten()[torch.from_numpy(cells).cuda()].cpu().numpy().astype(np.float64)
     assert np.abs(q_s - Mx_or).max() <= TOL_STEP[dtype] * np.abs(Mx_or).max() * 8
     xv = x_dev.double() * torch.from_numpy(v).cuda()
-    assert pq == pytest.approx(float((xv * q.double()).sum()), rel=1e-10)
+    # fp32: the products of a 16-byte chunk are summed in fp32 before the fp64 accumulator (chunk_dot), 2e-7 relative
+    # per 4-term partial, averaging down over the 2.6e5+ chunks of a config
+    assert pq == pytest.approx(float((xv * q.double()).sum()), rel=1e-10 if dtype == "f64" else 1e-8)
     del q, xv
 
     # the whole path in bench.py's launch configuration (fixed caps, graph loop)
