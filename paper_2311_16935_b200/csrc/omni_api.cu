@@ -21,6 +21,9 @@ using namespace omni;
 #define OMNI_D3 6
 #define OMNI_D4 4      // K4 ring depth in its 4-array iterations ({p_h, r, p_old, delta}); 7 in the 2-array ones
 #define OMNI_MINB 3
+#ifndef OMNI_D4_F64
+#define OMNI_D4_F64 6   // fp64 K4 runs 2 CTAs per SM (registers): deeper ring from the same shared memory
+#endif
 #define OMNI_PERSIST_MAX_CELLS 1500000LL   // automatic mode: grids up to this many padded cells take the persistent loop
 #define OMNI_PERSIST_SMALL_CELLS 65536LL   // persistent loop: 512-thread CTAs up to here, 1024-thread CTAs above
 #endif
@@ -310,7 +313,7 @@ struct MarchCfg { dim3 grid, block; int zlen; };
 // several CTAs per SM (shared memory: K3 6 stages x 10.8 KB, K4 4 x 17.4 KB or 7 x 9.4 KB by iteration parity,
 // K2 5 x 10.3 KB fp32 / 4 x 14.8 KB fp64).
 template <typename T, bool LOP = false> using K3 = OpT3<T, OMNI_BY, OMNI_D3, OMNI_MINB, LOP>;
-template <typename T, bool LOP = false> using K4 = OpT4<T, OMNI_BY, OMNI_D4, (sizeof(T) == 8 ? 2 : OMNI_MINB), LOP>;   // fp64 K4: 72 registers spill
+template <typename T, bool LOP = false> using K4 = OpT4<T, OMNI_BY, (sizeof(T) == 8 ? OMNI_D4_F64 : OMNI_D4), (sizeof(T) == 8 ? 2 : OMNI_MINB), LOP>;   // fp64 K4: 72 registers spill
 template <typename T> using K2 = OpT2<T, OMNI_BY, (sizeof(T) == 8 ? 4 : 5), OMNI_MINB>;
 
 
@@ -532,14 +535,9 @@ int run_loop_host(const Geom& g, const Workspace<T>& w, const HostConst& H, cons
         recs.push_back(r);
         return e;
     };
-    auto flush = [&](const Scalars& h_before, const Scalars& h_after) {
-        (void)h_before; (void)h_after;
-    };
-    (void)flush;
     Scalars h;
     memset(&h, 0, sizeof(h));
     int rc = OMNI_OK;
-    long long executed_k34 = 0, seen_cg = 0;
     for (long long it = 0; it <= (long long)max_outer && rc == OMNI_OK; ++it) {
         if (timed(0, [&] { return launch_tma<K2<T>>(g, a2, maps, st); }) != cudaSuccess) { rc = OMNI_ERR_CUDA; break; }
         int done = 0;
@@ -564,7 +562,6 @@ int run_loop_host(const Geom& g, const Workspace<T>& w, const HostConst& H, cons
         }
         if (!h.outer_go) break;
     }
-    (void)executed_k34; (void)seen_cg;
     if (prof) {
         cudaStreamSynchronize(st);
         // launches that found the loop flag cleared return at once; keep only those that did the work:
