@@ -83,6 +83,14 @@ def test_source_and_operator_steps(oracle, dtype, shape, frac):
 LOOPS = {"graph": 2, "persistent": 3}       # omni_set_loop_mode; the default (0) picks one of the two by grid size
 
 
+@pytest.fixture(params=list(LOOPS))
+def forced_loop(request):
+    """Runs a test once per loop driver (the grids here are small enough that the default would always pick one)."""
+    prev = omni.set_loop_mode(LOOPS[request.param])
+    yield request.param
+    omni.set_loop_mode(prev)
+
+
 def _solve_both(oracle, f, dtype, tol, max_outer, max_cg, mask=None, nan_mask=False, loop=None):
     g_dev, g_or, m_dev, m = _inputs(f, dtype, mask)
     d = f["d"]
@@ -186,7 +194,7 @@ def test_fuzz_random_shapes_masks_spacings(oracle, seed, loop):
 
 
 @pytest.mark.parametrize("dtype", ["f64", "f32"])
-def test_batch2d_and_first_guess(oracle, dtype):
+def test_batch2d_and_first_guess(oracle, dtype, forced_loop):
     """omni_solve_batch2d_*: stacked 2D snapshots on one mask against the oracle's stacked solve (same joint CG scalars),
     with and without a first guess; nb = 1 is bit-identical to omni_solve_*; a converged first guess stops at once."""
     fs = [make_field("lamb_oseen2d", (45, 140), seed=s, noise=0.05) for s in range(5)]
@@ -222,7 +230,7 @@ def test_batch2d_and_first_guess(oracle, dtype):
 
 
 @pytest.mark.parametrize("dtype", ["f64", "f32"])
-def test_direct_batch2d(oracle, dtype):
+def test_direct_batch2d(oracle, dtype, forced_loop):
     """omni_solve_direct_batch2d_*: the stacked snapshots with the inner systems L P = S, against the oracle's, with
     and without a first guess; converged, every snapshot meets the tolerance of the joint system."""
     fs = [make_field("lamb_oseen2d", (45, 140), seed=s, noise=0.05) for s in range(4)]
@@ -350,7 +358,7 @@ def test_direct_solve_trajectory_parity(oracle, dtype, kind, shape, frac, loop):
 
 
 @pytest.mark.parametrize("dtype,tol", [("f64", 1e-8), ("f32", 1e-5)])
-def test_direct_solve_converged(oracle, dtype, tol):
+def test_direct_solve_converged(oracle, dtype, tol, forced_loop):
     """Converged: the direct solve meets Eq. 41 with the oracle's operators, agrees with the oracle's direct solve and
     lands on the field Algorithm 1 converges to (configs[0], and masked stand-ins of configs 1 and 3)."""
     for idx, n in ((0, None), (1, 96), (3, 32)):
@@ -380,7 +388,7 @@ def test_direct_solve_converged(oracle, dtype, tol):
 
 
 @pytest.mark.parametrize("dtype,tol", [("f64", 1e-8), ("f32", 1e-5)])
-def test_cascade_first_guess(oracle, dtype, tol):
+def test_cascade_first_guess(oracle, dtype, tol, forced_loop):
     """omni_solve_cascade_*: the coarse levels only supply a first guess, so what is checked is what is unique -- the
     returned field meets Eq. 41 with the oracle's operators and equals the direct solve's (hence the oracle's) to the
     tolerance -- plus that the guess pays (fewer finest-level CG iterations at the fp32 tolerance).  levels = 0 is the direct solve, bitwise.
