@@ -211,3 +211,44 @@ def solve_batch2d(gx, gy, mask2d, dx, dy, tol, max_outer, max_cg, P_init=None, d
         raise MemoryError("oracle_solve_batch2d: allocation failed")
     return P, {"outer_iters": info.outer_iters, "cg_iters_total": info.cg_iters_total, "eps_R_final": info.eps_R_final,
                "norm_S": info.norm_S, "converged": bool(info.converged)}
+
+
+def velocity_source(u, v, w, mask, dx, dy, dz=1.0, rho=1.0, mu=0.0, dudt=None):
+    """f(u) = grad P of Eq. 1: -rho (du/dt + (u . grad) u) + mu lap u, on the cell grid, written out with
+    second-order central differences (plain numpy slicing, fp64).  u, v(, w): (ny, nx) or (nz, ny, nx); w = None in 2D.
+    dudt: optional list of the local accelerations du_i/dt (same shapes; None = steady).  Reading R-V1:
+    the paper does not fix the discretisation; a cell whose central stencil touches a missing cell (outside the box,
+    mask == 0, NaN velocity) gets NaN in every component, which the solver treats as missing (Eq. 13 :176).
+    Returns [gx, gy(, gz)]."""
+    comps = [_f64(u), _f64(v)] + ([] if w is None else [_f64(w)])
+    nd = comps[0].ndim
+    assert nd == len(comps), "2D fields take (u, v), 3D fields (u, v, w)"
+    h = [dx, dy, dz][:nd]                     # spacing of axis a = 0 (x), 1 (y), 2 (z); numpy axis of a is nd - 1 - a
+    ok = np.ones(comps[0].shape, bool) if mask is None else (np.asarray(mask) != 0)
+    for c in comps:
+        ok &= ~np.isnan(c)
+    acc = [np.zeros(comps[0].shape) if dudt is None else _f64(dudt[i]).copy() for i in range(nd)]
+    lap = [np.zeros(comps[0].shape) for _ in range(nd)]
+    good = ok.copy()
+    for a in range(nd):
+        ax = nd - 1 - a
+        n = comps[0].shape[ax]
+        ctr = [slice(None)] * nd; lo = [slice(None)] * nd; hi = [slice(None)] * nd
+        ctr[ax] = slice(1, n - 1); lo[ax] = slice(0, n - 2); hi[ax] = slice(2, n)
+        ctr, lo, hi = tuple(ctr), tuple(lo), tuple(hi)
+        nb_ok = np.zeros_like(ok)
+        nb_ok[ctr] = ok[lo] & ok[hi]
+        good &= nb_ok
+        for i in range(nd):
+            d1 = np.zeros(comps[0].shape); d2 = np.zeros(comps[0].shape)
+            with np.errstate(invalid="ignore"):
+                d1[ctr] = (comps[i][hi] - comps[i][lo]) / (2.0 * h[a])
+                d2[ctr] = (comps[i][hi] - 2.0 * comps[i][ctr] + comps[i][lo]) / (h[a] * h[a])
+            acc[i] = acc[i] + np.nan_to_num(comps[a]) * np.nan_to_num(d1)
+            lap[i] = lap[i] + np.nan_to_num(d2)
+    out = []
+    for i in range(nd):
+        g = -rho * acc[i] + mu * lap[i]
+        g[~good] = np.nan
+        out.append(g)
+    return out

@@ -586,3 +586,54 @@ def test_direct_batch2d_oracle_pins(oracle):
         for other in (Pb, Pr):
             a, c = other[b][v] - other[b][v].mean(), Pi[v] - Pi[v].mean()
             assert np.linalg.norm(a - c) / np.linalg.norm(c) < 1e-8
+
+
+# ----------------------------------------------------------------------------- NEXT-4: f(u) of Eq. 1 (:23)
+
+def test_velocity_source_closed_forms(oracle):
+    """oracle.velocity_source against closed forms: (i) central differences are exact on quadratics, so for a quadratic
+    velocity field -rho (u . grad) u + mu lap u is reproduced to rounding at every cell with a full stencil; (ii) the 2D
+    Taylor-Green vortex (steady Euler solution, P = rho/4 (cos 2x + cos 2y)): f -> grad P at second order; with
+    viscosity and the matching decay rate du/dt = -2 nu u the viscous and unsteady terms cancel; (iii) missing cells
+    poison exactly their stencil neighbours."""
+    rng = np.random.default_rng(0)
+    nz, ny, nx = 7, 8, 9
+    d = (0.3, 0.5, 0.7)
+    z, y, x = np.meshgrid(np.arange(nz) * d[2], np.arange(ny) * d[1], np.arange(nx) * d[0], indexing="ij")
+    X = [x, y, z]
+    # u_i = a_i + b_ij X_j + X^T C_i X / 2   (C_i symmetric)
+    a = rng.normal(size=3); b = rng.normal(size=(3, 3)); Cq = rng.normal(size=(3, 3, 3)); Cq = Cq + Cq.transpose(0, 2, 1)
+    U = [a[i] + sum(b[i, j] * X[j] for j in range(3)) + 0.5 * sum(Cq[i, j, k] * X[j] * X[k] for j in range(3) for k in range(3))
+         for i in range(3)]
+    grad = [[b[i, j] + sum(Cq[i, j, k] * X[k] for k in range(3)) for j in range(3)] for i in range(3)]
+    rho, mu = 1.7, 0.05
+    acc = [rng.normal(size=x.shape) for _ in range(3)]
+    exact = [-rho * (acc[i] + sum(U[j] * grad[i][j] for j in range(3))) + mu * np.trace(Cq[i]) for i in range(3)]
+    g = oracle.velocity_source(U[0], U[1], U[2], None, *d, rho=rho, mu=mu, dudt=acc)
+    inner = (slice(1, -1),) * 3
+    for i in range(3):
+        assert np.allclose(g[i][inner], exact[i][inner], rtol=1e-12, atol=1e-12)
+        edge = np.ones(x.shape, bool); edge[inner] = False
+        assert np.isnan(g[i][edge]).all() and not np.isnan(g[i][inner]).any()
+    # (iii) one missing cell (NaN velocity) and one masked cell: exactly the cells whose 7-point stencil touches them
+    U2 = [c.copy() for c in U]; U2[1][3, 4, 4] = np.nan
+    mask = np.ones(x.shape, np.uint8); mask[2, 2, 6] = 0
+    g2 = oracle.velocity_source(U2[0], U2[1], U2[2], mask, *d, rho=rho, mu=mu, dudt=acc)
+    expect_nan = np.ones(x.shape, bool); expect_nan[inner] = False
+    for (k, j, i) in ((3, 4, 4), (2, 2, 6)):
+        for dk, dj, di in ((0, 0, 0), (1, 0, 0), (-1, 0, 0), (0, 1, 0), (0, -1, 0), (0, 0, 1), (0, 0, -1)):
+            expect_nan[k + dk, j + dj, i + di] = True
+    assert np.array_equal(np.isnan(g2[0]), expect_nan)
+    assert np.allclose(g2[2][~expect_nan], exact[2][~expect_nan], rtol=1e-12, atol=1e-12)
+    # (ii) Taylor-Green, 2D, two resolutions
+    errs = []
+    for n in (32, 64):
+        hh = 2 * np.pi / n
+        yy, xx = np.meshgrid(np.arange(n) * hh, np.arange(n) * hh, indexing="ij")
+        nu = 0.3
+        u, v = np.sin(xx) * np.cos(yy), -np.cos(xx) * np.sin(yy)
+        gP = [-0.5 * rho * np.sin(2 * xx), -0.5 * rho * np.sin(2 * yy)]
+        g = oracle.velocity_source(u, v, None, None, hh, hh, rho=rho, mu=rho * nu, dudt=[-2 * nu * u, -2 * nu * v])
+        inner2 = (slice(1, -1),) * 2
+        errs.append(max(np.abs(g[i][inner2] - gP[i][inner2]).max() for i in range(2)))
+    assert errs[0] < 2e-2 and 3.5 < errs[0] / errs[1] < 4.5
