@@ -144,6 +144,25 @@ int omni_solve_batch2d_f32(int nx, int ny, int nb, double dx, double dy, const f
                            const unsigned char* d_mask2d, const float* d_P_init, float* d_P_out, double tol,
                            int max_outer, int max_cg, void* stream, omni_info* info);
 
+/* ---- upstream of the path: the pressure gradient from a velocity field, Eq. 1 ----
+ *   g = f(u) = -rho (du/dt + (u . grad) u) + mu lap u
+ * with second-order central differences on the cell grid.  The paper does not fix the discretisation (reading R-V1,
+ * DESIGN.md 13): a cell whose 2*naxes-neighbour stencil touches a missing cell (outside the box, mask == 0, a NaN
+ * velocity component) gets NaN in every output component, which omni_solve_* treats as missing (Eq. 13 :176) -- so the
+ * outputs can be fed to the solver with the same mask.  d_u, d_v, d_w: device, [nz][ny][nx] (d_w NULL iff nz == 1);
+ * d_dudt, d_dvdt, d_dwdt: optional local accelerations (all NULL = steady flow); d_g*: device outputs (d_gz NULL iff
+ * nz == 1).  Asynchronous on `stream`; returns an omni_status. */
+int omni_velocity_source_f64(int nx, int ny, int nz, double dx, double dy, double dz,
+                             const double* d_u, const double* d_v, const double* d_w,
+                             const double* d_dudt, const double* d_dvdt, const double* d_dwdt,
+                             const unsigned char* d_mask, double rho, double mu,
+                             double* d_gx, double* d_gy, double* d_gz, void* stream);
+int omni_velocity_source_f32(int nx, int ny, int nz, double dx, double dy, double dz,
+                             const float* d_u, const float* d_v, const float* d_w,
+                             const float* d_dudt, const float* d_dvdt, const float* d_dwdt,
+                             const unsigned char* d_mask, double rho, double mu,
+                             float* d_gx, float* d_gy, float* d_gz, void* stream);
+
 /* ---- single steps of the path (each runs the same device code the solve runs; used by the parity tests) ----------
  * a0  geometry constants (host only, no device needed).  out[0..2] = face totals F_x,F_y,F_z (Eq. 5 :75 / Eq. 23 :258),
  *     out[3] = A_tot (Eq. 8 :94 / Eq. 24 :262), out[4..12] = c_jk row-major 3x3 (Eq. 17 :207 / Eq. 32-35 :314-326 /

@@ -17,7 +17,7 @@ STATUS_NAMES = {0: "OMNI_OK", 1: "OMNI_NOT_CONVERGED", -1: "OMNI_ERR_INVALID_ARG
                 -3: "OMNI_ERR_ALLOC", -4: "OMNI_ERR_BREAKDOWN"}
 # every symbol include/omni.h declares
 SYMBOLS = ["omni_solve_f64", "omni_solve_f32", "omni_workspace_bytes", "omni_solve_f64_ws", "omni_solve_f32_ws",
-           "omni_solve_host_f64", "omni_solve_host_f32", "omni_solve_batch2d_f64", "omni_solve_batch2d_f32", "omni_solve_direct_f64", "omni_solve_direct_f32", "omni_solve_direct_batch2d_f64", "omni_solve_direct_batch2d_f32", "omni_solve_cascade_f64", "omni_solve_cascade_f32", "omni_constants", "omni_source_f64", "omni_source_f32",
+           "omni_solve_host_f64", "omni_solve_host_f32", "omni_solve_batch2d_f64", "omni_solve_batch2d_f32", "omni_solve_direct_f64", "omni_solve_direct_f32", "omni_solve_direct_batch2d_f64", "omni_solve_direct_batch2d_f32", "omni_solve_cascade_f64", "omni_solve_cascade_f32", "omni_velocity_source_f64", "omni_velocity_source_f32", "omni_constants", "omni_source_f64", "omni_source_f32",
            "omni_apply_M_f64", "omni_apply_M_f32", "omni_residual_f64", "omni_residual_f32", "omni_launch_count",
            "omni_set_loop_mode", "omni_release_memory", "omni_profile_enable", "omni_profile_read", "omni_status_string", "omni_version"]
 
@@ -204,6 +204,26 @@ def solve_direct(gx, gy, gz, mask, d, tol, max_outer, max_cg, out=None, P_init=N
     if rc < 0:
         raise OmniError(rc, f"omni_solve_direct_{sfx}")
     return P, info.as_dict()
+
+
+def velocity_source(u, v, w, mask, d, rho=1.0, mu=0.0, dudt=None):
+    """omni_velocity_source_*: g = f(u) of Eq. 1 on CUDA tensors (w = None in 2D; dudt = optional list of local
+    accelerations).  Returns [gx, gy(, gz)]."""
+    import torch
+    sfx = _suffix(u)
+    acc = list(dudt) if dudt is not None else [None, None, None]
+    acc += [None] * (3 - len(acc))
+    _check([u, v, w, mask] + acc, "cuda")
+    if mask is not None and mask.dtype != torch.uint8:
+        raise TypeError("mask must be uint8")
+    g = [torch.empty_like(u), torch.empty_like(u), None if w is None else torch.empty_like(u)]
+    with torch.cuda.device(u.device):
+        fn = getattr(lib(), f"omni_velocity_source_{sfx}")
+        rc = fn(*_geom(u, d), _ptr(u), _ptr(v), _ptr(w), _ptr(acc[0]), _ptr(acc[1]), _ptr(acc[2]), _ptr(mask),
+                C.c_double(rho), C.c_double(mu), _ptr(g[0]), _ptr(g[1]), _ptr(g[2]), _stream(u.device))
+    if rc < 0:
+        raise OmniError(rc, f"omni_velocity_source_{sfx}")
+    return g[:2] if w is None else g
 
 
 def solve_cascade(gx, gy, gz, mask, d, tol, max_outer, max_cg, levels=3, out=None):

@@ -863,6 +863,27 @@ int solve_cascade(int nx, int ny, int nz, double dx, double dy, double dz, const
     return rc;
 }
 
+// NEXT-4: the upstream step g = f(u) (Eq. 1 :23) on device arrays in the caller's layout
+template <typename T>
+int velocity_source(int nx, int ny, int nz, double dx, double dy, double dz, const T* u, const T* v, const T* w,
+                    const T* atx, const T* aty, const T* atz, const unsigned char* mask, double rho, double mu,
+                    T* gx, T* gy, T* gz, void* stream)
+{
+    if (nx < 1 || ny < 1 || nz < 1 || !(dx > 0.0) || !(dy > 0.0) || (nz > 1 && !(dz > 0.0))) return OMNI_ERR_INVALID_ARG;
+    if (!std::isfinite(rho) || !std::isfinite(mu)) return OMNI_ERR_INVALID_ARG;
+    const int ncomp = (nz > 1) ? 3 : 2;
+    if (!u || !v || !gx || !gy || (ncomp == 3 && (!w || !gz))) return OMNI_ERR_INVALID_ARG;
+    if ((atx == nullptr) != (aty == nullptr) || (ncomp == 3 && (atx == nullptr) != (atz == nullptr))) return OMNI_ERR_INVALID_ARG;
+    cudaStream_t st = (cudaStream_t)stream;
+    const long long n = (long long)nx * ny * nz;
+    velocity_source_kernel<T><<<blocks_for(n, 256), 256, 0, st>>>(
+        nx, ny, nz, ncomp, (T)(1.0 / (dx * dx)), (T)(1.0 / (dy * dy)), (T)(ncomp == 3 ? 1.0 / (dz * dz) : 0.0),
+        (T)(0.5 / dx), (T)(0.5 / dy), (T)(ncomp == 3 ? 0.5 / dz : 0.0), (T)rho, (T)mu, u, v, w, atx, aty, atz, mask, gx, gy, gz);
+    g_launches.fetch_add(1, std::memory_order_relaxed);
+    CK(cudaGetLastError());
+    return OMNI_OK;
+}
+
 template <typename T>
 int solve_host(int nx, int ny, int nz, double dx, double dy, double dz, const T* gx, const T* gy, const T* gz,
                const unsigned char* mask, T* P_out, double tol, int max_outer, int max_cg, void* stream, omni_info* info)
@@ -1138,6 +1159,22 @@ int omni_solve_cascade_f32(int nx, int ny, int nz, double dx, double dy, double 
                            int max_cg, int levels, void* stream, omni_info* info)
 {
     return solve_cascade<float>(nx, ny, nz, dx, dy, dz, d_gx, d_gy, d_gz, d_mask, d_P_out, tol, max_outer, max_cg, levels, stream, info);
+}
+
+int omni_velocity_source_f64(int nx, int ny, int nz, double dx, double dy, double dz, const double* d_u, const double* d_v,
+                             const double* d_w, const double* d_dudt, const double* d_dvdt, const double* d_dwdt,
+                             const unsigned char* d_mask, double rho, double mu, double* d_gx, double* d_gy, double* d_gz,
+                             void* stream)
+{
+    return velocity_source<double>(nx, ny, nz, dx, dy, dz, d_u, d_v, d_w, d_dudt, d_dvdt, d_dwdt, d_mask, rho, mu, d_gx, d_gy, d_gz, stream);
+}
+
+int omni_velocity_source_f32(int nx, int ny, int nz, double dx, double dy, double dz, const float* d_u, const float* d_v,
+                             const float* d_w, const float* d_dudt, const float* d_dvdt, const float* d_dwdt,
+                             const unsigned char* d_mask, double rho, double mu, float* d_gx, float* d_gy, float* d_gz,
+                             void* stream)
+{
+    return velocity_source<float>(nx, ny, nz, dx, dy, dz, d_u, d_v, d_w, d_dudt, d_dvdt, d_dwdt, d_mask, rho, mu, d_gx, d_gy, d_gz, stream);
 }
 
 int omni_constants(int nx, int ny, int nz, double dx, double dy, double dz, double* h_out13)

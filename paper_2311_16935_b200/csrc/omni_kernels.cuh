@@ -712,4 +712,50 @@ __global__ void prolong_kernel(int nx, int ny, int nz, int fx, int fy, int fz, i
     Pf[u] = isnan(v) ? T(0) : v;
 }
 
+// ------------------------------------------------------------------------------------------------ NEXT-4: f(u), Eq. 1
+// g = -rho (du/dt + (u . grad) u) + mu lap u with second-order central differences; a cell whose
+// 2*naxes-neighbour stencil touches a missing cell (outside the box, mask == 0, NaN velocity) gets NaN in every
+// component (reading R-V1), which the solver treats as missing (Eq. 13 :176).  Caller layout
+// (unpadded, x fastest); one thread per cell; at* = optional local accelerations (nullptr = steady).
+template <typename T>
+__global__ void velocity_source_kernel(int nx, int ny, int nz, int ncomp, T idx2, T idy2, T idz2, T ihx, T ihy, T ihz,
+                                       T rho, T mu, const T* __restrict__ u, const T* __restrict__ v,
+                                       const T* __restrict__ w, const T* __restrict__ atx, const T* __restrict__ aty,
+                                       const T* __restrict__ atz, const uint8_t* __restrict__ mask,
+                                       T* __restrict__ gx, T* __restrict__ gy, T* __restrict__ gz)
+{
+    const long long c = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const long long n = (long long)nx * ny * nz;
+    if (c >= n) return;
+    const int i = (int)(c % nx), j = (int)((c / nx) % ny), k = (int)(c / ((long long)nx * ny));
+    const long long sy = nx, sz = (long long)nx * ny;
+    auto ok = [&](long long q) {
+        if (mask != nullptr && mask[q] == 0) return false;
+        if (isnan(u[q]) || isnan(v[q])) return false;
+        return !(ncomp == 3 && isnan(w[q]));
+    };
+    bool good = ok(c) && i > 0 && i < nx - 1 && j > 0 && j < ny - 1 && (ncomp == 2 || (k > 0 && k < nz - 1));
+    if (good) good = ok(c - 1) && ok(c + 1) && ok(c - sy) && ok(c + sy) && (ncomp == 2 || (ok(c - sz) && ok(c + sz)));
+    const T qnan = (T)nan("");
+    if (!good) {
+        gx[c] = qnan; gy[c] = qnan;
+        if (ncomp == 3) gz[c] = qnan;
+        return;
+    }
+    const T uc = u[c], vc = v[c], wc = (ncomp == 3) ? w[c] : T(0);
+    auto term = [&](const T* __restrict__ f, const T* __restrict__ at) {
+        const T fc = f[c];
+        T conv = uc * ((f[c + 1] - f[c - 1]) * ihx) + vc * ((f[c + sy] - f[c - sy]) * ihy);
+        T lap = (f[c + 1] - T(2) * fc + f[c - 1]) * idx2 + (f[c + sy] - T(2) * fc + f[c - sy]) * idy2;
+        if (ncomp == 3) {
+            conv += wc * ((f[c + sz] - f[c - sz]) * ihz);
+            lap += (f[c + sz] - T(2) * fc + f[c - sz]) * idz2;
+        }
+        return -rho * ((at != nullptr ? at[c] : T(0)) + conv) + mu * lap;
+    };
+    gx[c] = term(u, atx);
+    gy[c] = term(v, aty);
+    if (ncomp == 3) gz[c] = term(w, atz);
+}
+
 }  // namespace omni

@@ -456,6 +456,50 @@ def test_persistent_loop_stress(dtype):
                 assert np.array_equal(P0, Pg, equal_nan=True)
 
 
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_velocity_source_parity(oracle, dtype):
+    """omni_velocity_source_* (g = f(u), Eq. 1 :23) against oracle.velocity_source, entry by entry: 3D and 2D, ragged
+    sizes, random masks plus NaN velocities, steady and with local accelerations; the NaN pattern is identical.  Then
+    the whole chain on a Taylor-Green vortex: velocity -> g on the GPU -> omni_solve_direct -> the analytic pressure."""
+    rng = np.random.default_rng(12)
+    np_dt = np.float32 if dtype == "f32" else np.float64
+    for shape, frac, unsteady in (((13, 21, 70), 0.05, True), ((37, 150), 0.03, False), ((6, 5, 9), 0.0, True), ((3, 40), 0.0, False)):
+        nd = len(shape)
+        d = (0.4, 0.7, 1.1)
+        vel = [rng.normal(size=shape).astype(np_dt) for _ in range(nd)]
+        if frac > 0:
+            vel[0][rng.random(shape) < 0.01] = np.nan
+        mask = (rng.random(shape) > frac).astype(np.uint8) if frac > 0 else None
+        acc = [rng.normal(size=shape).astype(np_dt) for _ in range(nd)] if unsteady else None
+        vd = [to_dev(c) for c in vel] + [None] * (3 - nd)
+        g = omni.velocity_source(vd[0], vd[1], vd[2], None if mask is None else to_dev(mask), d, rho=1.3, mu=0.02,
+                                 dudt=None if acc is None else [to_dev(c) for c in acc])
+        v64 = [c.astype(np.float64) for c in vel] + [None] * (3 - nd)
+        go = oracle.velocity_source(v64[0], v64[1], v64[2], mask, *d[:nd], rho=1.3, mu=0.02,
+                                    dudt=None if acc is None else [c.astype(np.float64) for c in acc])
+        assert len(g) == nd
+        for i in range(nd):
+            gi = g[i].cpu().numpy().astype(np.float64)
+            assert np.array_equal(np.isnan(gi), np.isnan(go[i])), (shape, i)
+            scale = np.nanmax(np.abs(go[i])) if np.isfinite(go[i]).any() else 1.0
+            assert np.nanmax(np.abs(gi - go[i]), initial=0.0) <= (1e-12 if dtype == "f64" else 2e-5) * scale, (shape, i)
+    # chain: Taylor-Green (steady, inviscid): P = rho/4 (cos 2x + cos 2y)
+    n = 96
+    h = 2 * np.pi / n
+    yy, xx = np.meshgrid(np.arange(n) * h, np.arange(n) * h, indexing="ij")
+    rho = 1.2
+    u, v = (np.sin(xx) * np.cos(yy)).astype(np_dt), (-np.cos(xx) * np.sin(yy)).astype(np_dt)
+    gx, gy = omni.velocity_source(to_dev(u), to_dev(v), None, None, (h, h), rho=rho)
+    tol = 1e-8 if dtype == "f64" else 1e-5
+    P, info = omni.solve_direct(gx, gy, None, None, (h, h), tol, 20, 5000)
+    assert info["status"] == 0
+    Pa = 0.25 * rho * (np.cos(2 * xx) + np.cos(2 * yy))
+    Pn = P.cpu().numpy().astype(np.float64)
+    valid = ~np.isnan(Pn)
+    assert valid.sum() == (n - 2) ** 2                      # the one-cell rim has no central stencil
+    assert rel_l2_after_mean_removal(Pn, Pa, valid) < 5e-3
+
+
 def test_solve_without_info_is_asynchronous():
     """include/omni.h: with info == NULL the call returns after enqueueing.  The graph loop parks its executable graph
     instead of destroying it in flight (that blocks the host for the whole solve); the persistent loop is one launch."""
