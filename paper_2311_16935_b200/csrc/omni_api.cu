@@ -24,9 +24,13 @@ using namespace omni;
 #ifndef OMNI_D4_F64
 #define OMNI_D4_F64 6   // fp64 K4 runs 2 CTAs per SM (registers): deeper ring from the same shared memory
 #endif
+#endif
+#ifndef OMNI_TAPER_F
+#define OMNI_TAPER_F 0.5     // tapered z segments (tma_config): fraction of the remaining planes per slot; 0 = uniform segments
+#define OMNI_TAPER_MIN 24    // and the shortest segment
+#endif
 #define OMNI_PERSIST_MAX_CELLS 1500000LL   // automatic mode: grids up to this many padded cells take the persistent loop
 #define OMNI_PERSIST_SMALL_CELLS 65536LL   // persistent loop: 512-thread CTAs up to here, 1024-thread CTAs above
-#endif
 
 namespace {
 
@@ -307,7 +311,7 @@ __global__ void init_scalars_kernel(Scalars* sc, double tol, int max_outer, int 
 
 // ------------------------------------------------------------------------------------------------ launch configuration
 
-struct MarchCfg { dim3 grid, block; int zlen; };
+struct MarchCfg { dim3 grid, block; ZSeg zs; };
 
 // K2 / K3 / K4: TMA + mbarrier pipeline (omni_tma.cuh): 512-byte x 8-row tiles, 8 consumer warps + 1 producer warp,
 // several CTAs per SM (shared memory: K3 6 stages x 10.8 KB, K4 4 x 17.4 KB or 7 x 9.4 KB by iteration parity,
@@ -348,9 +352,38 @@ MarchCfg tma_config(const Geom& g)
         if (cost < best_cost) { best_cost = cost; best = nseg; }
         if (zlen <= 4) break;
     }
+#ifdef OMNI_TUNING   // tuning builds only: force the number of z segments from the environment
+    if (const char* ev = getenv("OMNI_NSEG")) { const int v = atoi(ev); if (v >= 1) best = v < g.nz ? v : g.nz; }
+#endif
     MarchCfg c;
-    c.zlen = (g.nz + best - 1) / best;
-    const int nseg = (g.nz + c.zlen - 1) / c.zlen;
+    c.zs.n = 0;
+    c.zs.zlen = (g.nz + best - 1) / best;
+    int nseg = (g.nz + c.zs.zlen - 1) / c.zs.zlen;
+    // Tapered z segments: CTAs are dispatched in blockIdx order, z slowest, so the segments of
+    // later z indices start later.  Long segments first (few halo planes, few pipeline fills), short ones last: the
+    // launch then drains in the time of a short CTA instead of about half a long one.  Each segment takes the
+    // fraction taper_f of the planes still to be assigned per CTA slot, but at least taper_min planes.
+    double taper_f = OMNI_TAPER_F;
+    int taper_min = OMNI_TAPER_MIN;
+#ifdef OMNI_TUNING
+    if (const char* ev = getenv("OMNI_TAPER_F")) taper_f = atof(ev);
+    if (const char* ev = getenv("OMNI_TAPER_MIN")) taper_min = atoi(ev) > 1 ? atoi(ev) : 1;
+#endif
+    if (taper_f > 0.0 && (double)tiles * g.nz / slots >= 2.0 * taper_min) {
+        int k = 0, n = 0;
+        bool ok = true;
+        c.zs.k[0] = 0;
+        while (k < g.nz) {
+            const double rem = (double)(g.nz - k) * (double)tiles / slots;     // planes left per CTA slot
+            int len = (int)(rem * taper_f + 0.5);
+            if (len < taper_min) len = taper_min;
+            if (g.nz - k - len < (taper_min + 1) / 2) len = g.nz - k;
+            if (n == ZSeg::MAXSEG) { ok = false; break; }
+            k += len;
+            c.zs.k[++n] = k;
+        }
+        if (ok) { c.zs.n = n; nseg = n; }
+    }
     c.grid = dim3(ntx, nty, nseg);
     c.block = dim3(TG::NTHR, 1, 1);
     return c;
@@ -360,7 +393,7 @@ template <class Op>
 cudaError_t launch_tma(const Geom& g, const typename Op::Args& a, const TmaSet& maps, cudaStream_t st)
 {
     const MarchCfg c = tma_config<Op>(g);
-    tma_kernel<Op><<<c.grid, c.block, Op::SMEM_BYTES + 128, st>>>(g, c.zlen, a, maps);
+    tma_kernel<Op><<<c.grid, c.block, Op::SMEM_BYTES + 128, st>>>(g, c.zs, a, maps);
     g_launches.fetch_add(1, std::memory_order_relaxed);
     return cudaGetLastError();
 }
@@ -1242,6 +1275,16 @@ void omni_profile_read(double* h_ms3, long long* h_count3, int reset)
         if (reset) { g_prof_ms[i] = 0.0; g_prof_n[i] = 0; }
     }
 }
+
+#ifdef OMNI_TUNING
+// tuning builds only: copy the per-CTA timeline of operator `which` (ticket index: 0 K3, 1 K4, 2 K2) to the host
+int omni_debug_cta_trace(int which, unsigned long long* h_out, int n_ctas)
+{
+    if (which < 0 || which > 2 || n_ctas > 8192) return -1;
+    cudaDeviceSynchronize();
+    return cudaMemcpyFromSymbol(h_out, omni::g_cta_trace, (size_t)n_ctas * 24, (size_t)which * 3 * 8192 * 8) == cudaSuccess ? 0 : -2;
+}
+#endif
 
 void omni_release_memory(void)
 {

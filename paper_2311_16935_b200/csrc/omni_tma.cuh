@@ -63,6 +63,14 @@ struct alignas(64) TmaSet {
     CUtensorMap S_c;             // plain: S (T)
 };
 
+// z segments of a launch: uniform (n == 0: segment b covers planes [b zlen, (b+1) zlen)) or a table of boundaries
+// (segment b covers [k[b], k[b+1]); tapered schedules, tma_config)
+struct ZSeg {
+    enum { MAXSEG = 48 };
+    int n, zlen;
+    int k[MAXSEG + 1];
+};
+
 template <typename T, int BY_>
 struct TileGeom {
     static constexpr int V = 16 / (int)sizeof(T);          // cells per lane (one 16-byte piece)
@@ -117,9 +125,19 @@ __device__ __forceinline__ double chunk_dot(const T (&a)[V], const T (&b)[V])
     }
 }
 
+#ifdef OMNI_TUNING   // tuning builds only: per-CTA timeline (start, end, SM) of the last launch of each operator
+__device__ unsigned long long g_cta_trace[3][3 * 8192];
+__device__ __forceinline__ unsigned long long dbg_timer()
+{
+    unsigned long long t;
+    asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t));
+    return t;
+}
+#endif
+
 template <class Op>
 __global__ void __launch_bounds__(Op::TG::NTHR, Op::MINB)
-tma_kernel(const Geom g, const int zlen, const typename Op::Args a, const __grid_constant__ TmaSet maps)
+tma_kernel(const Geom g, const ZSeg zs, const typename Op::Args a, const __grid_constant__ TmaSet maps)
 {
     using TG = typename Op::TG;
     using T = typename Op::VT;
@@ -133,6 +151,9 @@ tma_kernel(const Geom g, const int zlen, const typename Op::Args a, const __grid
         if (threadIdx.x == 0 && blockIdx.x == 0 && blockIdx.y == 0 && blockIdx.z == 0) Op::idle(a);
         return;
     }
+#ifdef OMNI_TUNING
+    const unsigned long long dbg_t0 = dbg_timer();
+#endif
     // dynamic shared memory is only guaranteed 16-byte aligned: round up to 128 for the TMA destinations
     char* smem = reinterpret_cast<char*>((reinterpret_cast<uintptr_t>(smem_raw) + 127) & ~uintptr_t(127));
     const uint32_t smem_s = (uint32_t)__cvta_generic_to_shared(smem);
@@ -140,7 +161,8 @@ tma_kernel(const Geom g, const int zlen, const typename Op::Args a, const __grid
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int x0 = blockIdx.x * BX, y0 = blockIdx.y * BY;
-    const int k0 = blockIdx.z * zlen, k1 = min(g.nz, k0 + zlen);
+    const int k0 = zs.n ? zs.k[blockIdx.z] : blockIdx.z * zs.zlen;
+    const int k1 = zs.n ? zs.k[blockIdx.z + 1] : min(g.nz, k0 + zs.zlen);
     const int E = k1 - k0 + 2;                       // events: planes k0-1 .. k1
     const typename Op::Ctx ctx(a);
     // ring depth and stage size may depend on what this launch streams (K4: DESIGN.md section 6, lazy delta)
@@ -265,6 +287,15 @@ tma_kernel(const Geom g, const int zlen, const typename Op::Args a, const __grid
         is_last = (t == nblk - 1);
     }
     __syncthreads();
+#ifdef OMNI_TUNING
+    if (threadIdx.x == 0 && bid < 8192) {
+        unsigned int smid;
+        asm volatile("mov.u32 %0, %smid;" : "=r"(smid));
+        g_cta_trace[Op::TICKET][3 * bid] = dbg_t0;
+        g_cta_trace[Op::TICKET][3 * bid + 1] = dbg_timer();
+        g_cta_trace[Op::TICKET][3 * bid + 2] = smid | ((unsigned long long)nblk << 32);
+    }
+#endif
     if (is_last) {
         __threadfence();
         double tot[NACC];
