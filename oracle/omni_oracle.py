@@ -2,8 +2,9 @@
 
 Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference leg may import
 this module.  It never imports paper_2311_16935_b200 and shares nothing with the CUDA path.
-Everything here is argument marshalling for the C functions; the arithmetic lives in omni_oracle.c,
-each function citing the PAPER.md passage it follows.
+The solver path (constants, weights, S, operators, CG, Algorithm 1) is argument marshalling for the C functions of
+omni_oracle.c, each citing the PAPER.md passage it follows.  The upstream source-field steps g = f(u) -- velocity_source
+(Eq. 1), rans_source (Eq. 42), compressible_rans_source (Eq. 43-44) -- are written out here in plain numpy (fp64).
 """
 import ctypes as C
 import os
@@ -251,4 +252,112 @@ def velocity_source(u, v, w, mask, dx, dy, dz=1.0, rho=1.0, mu=0.0, dudt=None):
         g = -rho * acc[i] + mu * lap[i]
         g[~good] = np.nan
         out.append(g)
+    return out
+
+
+def _central(f, a, h, nd):
+    """d f / d x_a by second-order central differences on the interior of axis a (zero on its two end planes, which
+    the callers mark missing); numpy axis of a is nd - 1 - a."""
+    ax = nd - 1 - a
+    n = f.shape[ax]
+    ctr = [slice(None)] * nd; lo = [slice(None)] * nd; hi = [slice(None)] * nd
+    ctr[ax] = slice(1, n - 1); lo[ax] = slice(0, n - 2); hi[ax] = slice(2, n)
+    d = np.zeros(f.shape)
+    with np.errstate(invalid="ignore"):
+        d[tuple(ctr)] = (f[tuple(hi)] - f[tuple(lo)]) / (2.0 * h)
+    return d
+
+
+def _full_stencil(ok, nd):
+    """cells whose 2 nd face neighbours are all inside the box and ok (and that are ok themselves)."""
+    good = ok.copy()
+    for a in range(nd):
+        ax = nd - 1 - a
+        n = ok.shape[ax]
+        ctr = [slice(None)] * nd; lo = [slice(None)] * nd; hi = [slice(None)] * nd
+        ctr[ax] = slice(1, n - 1); lo[ax] = slice(0, n - 2); hi[ax] = slice(2, n)
+        nb = np.zeros_like(ok)
+        nb[tuple(ctr)] = ok[tuple(lo)] & ok[tuple(hi)]
+        good &= nb
+    return good
+
+
+def _stress_index(nd):
+    """position of R_ij in the stress list: 2D [xx, yy, xy]; 3D [xx, yy, zz, xy, xz, yz]."""
+    if nd == 2:
+        return {(0, 0): 0, (1, 1): 1, (0, 1): 2, (1, 0): 2}
+    return {(0, 0): 0, (1, 1): 1, (2, 2): 2, (0, 1): 3, (1, 0): 3, (0, 2): 4, (2, 0): 4, (1, 2): 5, (2, 1): 5}
+
+
+def rans_source(u, v, w, stress, mask, dx, dy, dz=1.0, rho=1.0):
+    """Eq. 42: f_i = -rho ( ubar_j d ubar_i / d x_j + d (u'_i u'_j) / d x_j ), viscous terms dropped, written
+    out with second-order central differences (reading R-V1).  u, v(, w): mean velocity, (ny, nx) or
+    (nz, ny, nx), w = None in 2D; stress: Reynolds stresses [xx, yy, xy] (2D) or [xx, yy, zz, xy, xz, yz] (3D).
+    A cell whose stencil touches a missing cell (outside the box, mask == 0, NaN in any input) gets NaN in every component.
+    Returns [fx, fy(, fz)]."""
+    U = [_f64(u), _f64(v)] + ([] if w is None else [_f64(w)])
+    nd = U[0].ndim
+    R = [_f64(s) for s in stress]
+    idx = _stress_index(nd)
+    assert nd == len(U) and len(R) == (3 if nd == 2 else 6)
+    h = [dx, dy, dz][:nd]
+    ok = np.ones(U[0].shape, bool) if mask is None else (np.asarray(mask) != 0)
+    for c in U + R:
+        ok &= ~np.isnan(c)
+    good = _full_stencil(ok, nd)
+    out = []
+    for i in range(nd):
+        conv = np.zeros(U[0].shape)
+        div = np.zeros(U[0].shape)
+        for j in range(nd):
+            conv = conv + np.nan_to_num(U[j]) * np.nan_to_num(_central(U[i], j, h[j], nd))
+            div = div + np.nan_to_num(_central(R[idx[(i, j)]], j, h[j], nd))
+        f = -rho * (conv + div)
+        f[~good] = np.nan
+        out.append(f)
+    return out
+
+
+def compressible_rans_source(u, v, w, stress, mask, dx, dy, dz=1.0, gamma=1.4, mach_inf=2.0, v_inf=1.0, rgas_t_inf=1.0):
+    """Eq. 43-44: grad ln(P / P_inf) of the compressible RANS momentum equations for an adiabatic ideal
+    gas with negligible density fluctuations.  Step by step:
+      T / T_inf = 1 + (gamma - 1)/2 M_inf^2 (1 - V^2 / V_inf^2)                                   (Eq. 43)
+      uu_ij = ubar_i ubar_j + (u'_i u'_j)                                                          (:545)
+      (delta_ij + uu_ij / (R T)) g_j = -(1 / (R T)) ( d uu_ij / d x_j - (uu_ij / T) d T / d x_j )  (Eq. 44)
+    solved for g = grad ln(P / P_inf) cell by cell (numpy.linalg.solve on the 2x2 / 3x3 systems).  rgas_t_inf = R T_inf
+    (the only way R and T_inf enter); stress may be None (no Reynolds stresses).  Central differences and missing cells
+    as in rans_source.  Returns [gx, gy(, gz)]."""
+    U = [_f64(u), _f64(v)] + ([] if w is None else [_f64(w)])
+    nd = U[0].ndim
+    idx = _stress_index(nd)
+    R = None if stress is None else [_f64(s) for s in stress]
+    h = [dx, dy, dz][:nd]
+    ok = np.ones(U[0].shape, bool) if mask is None else (np.asarray(mask) != 0)
+    for c in U + ([] if R is None else R):
+        ok &= ~np.isnan(c)
+    good = _full_stencil(ok, nd)
+    V2 = sum(c * c for c in U)
+    theta = 1.0 + 0.5 * (gamma - 1.0) * mach_inf ** 2 * (1.0 - V2 / v_inf ** 2)         # T / T_inf
+    RT = rgas_t_inf * theta
+    uu = {}
+    for i in range(nd):
+        for j in range(i, nd):
+            uu[(i, j)] = U[i] * U[j] + (0.0 if R is None else R[idx[(i, j)]])
+            uu[(j, i)] = uu[(i, j)]
+    dth = [_central(theta, j, h[j], nd) for j in range(nd)]
+    A = np.zeros(U[0].shape + (nd, nd))
+    b = np.zeros(U[0].shape + (nd,))
+    with np.errstate(invalid="ignore", divide="ignore"):
+        for i in range(nd):
+            for j in range(nd):
+                A[..., i, j] = (1.0 if i == j else 0.0) + uu[(i, j)] / RT
+                b[..., i] += -(1.0 / RT) * (_central(uu[(i, j)], j, h[j], nd) - uu[(i, j)] / theta * dth[j])
+    A[~good] = np.eye(nd)
+    b[~good] = 0.0
+    g = np.linalg.solve(A, b[..., None])[..., 0]
+    out = []
+    for i in range(nd):
+        gi = g[..., i].copy()
+        gi[~good] = np.nan
+        out.append(gi)
     return out

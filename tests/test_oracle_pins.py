@@ -637,3 +637,129 @@ def test_velocity_source_closed_forms(oracle):
         inner2 = (slice(1, -1),) * 2
         errs.append(max(np.abs(g[i][inner2] - gP[i][inner2]).max() for i in range(2)))
     assert errs[0] < 2e-2 and 3.5 < errs[0] / errs[1] < 4.5
+
+
+def test_rans_source_closed_forms(oracle):
+    """oracle.rans_source (Eq. 42 :507) against closed forms: (i) with quadratic mean velocity and quadratic Reynolds
+    stresses every central difference is exact, so -rho (ubar . grad ubar_i + d_j R_ij) is reproduced to rounding, in 3D
+    and 2D, with anisotropic spacing -- a transposed stress index, a dropped term or a wrong sign fails it;
+    (ii) zero stresses reduce it to the steady inviscid velocity_source (pinned above); (iii) ubar = 0, R_xx = x^2:
+    f = (-2 rho x, 0, 0); (iv) a NaN in a stress component poisons exactly its stencil neighbours."""
+    rng = np.random.default_rng(1)
+    rho = 1.3
+    for nd, shape, d in ((3, (6, 7, 8), (0.3, 0.5, 0.7)), (2, (9, 8), (0.4, 0.25))):
+        coords = np.meshgrid(*[np.arange(n) * d[nd - 1 - ax] for ax, n in enumerate(shape)], indexing="ij")
+        X = coords[::-1]                                        # X[a] = coordinate along axis a (x fastest)
+        def quad():
+            a, b = rng.normal(), rng.normal(size=nd)
+            Cq = rng.normal(size=(nd, nd)); Cq = Cq + Cq.T
+            f = a + sum(b[j] * X[j] for j in range(nd)) + 0.5 * sum(Cq[j, k] * X[j] * X[k] for j in range(nd) for k in range(nd))
+            g = [b[j] + sum(Cq[j, k] * X[k] for k in range(nd)) for j in range(nd)]
+            return f, g
+        U, gU = zip(*[quad() for _ in range(nd)])
+        pairs = [(0, 0), (1, 1), (0, 1)] if nd == 2 else [(0, 0), (1, 1), (2, 2), (0, 1), (0, 2), (1, 2)]
+        R, gR = zip(*[quad() for _ in pairs])
+        Rij = {}
+        for (i, j), g in zip(pairs, gR):
+            Rij[(i, j)] = g; Rij[(j, i)] = g
+        exact = [-rho * (sum(U[j] * gU[i][j] for j in range(nd)) + sum(Rij[(i, j)][j] for j in range(nd))) for i in range(nd)]
+        f = oracle.rans_source(U[0], U[1], U[2] if nd == 3 else None, list(R), None, *d, rho=rho)
+        inner = (slice(1, -1),) * nd
+        for i in range(nd):
+            assert np.allclose(f[i][inner], exact[i][inner], rtol=1e-12, atol=1e-12)
+            edge = np.ones(shape, bool); edge[inner] = False
+            assert np.isnan(f[i][edge]).all()
+        # (ii) zero stresses: the steady, inviscid form of Eq. 1
+        f0 = oracle.rans_source(U[0], U[1], U[2] if nd == 3 else None, [np.zeros(shape)] * len(pairs), None, *d, rho=rho)
+        v0 = oracle.velocity_source(U[0], U[1], U[2] if nd == 3 else None, None, *d, rho=rho, mu=0.0)
+        for i in range(nd):
+            assert np.array_equal(np.isnan(f0[i]), np.isnan(v0[i]))
+            assert np.allclose(f0[i][inner], v0[i][inner], rtol=1e-13, atol=1e-13)
+    # (iii) a stress gradient alone
+    shape, d = (5, 6, 7), (0.5, 0.5, 0.5)
+    z, y, x = np.meshgrid(*[np.arange(n) * 0.5 for n in shape], indexing="ij")
+    Z = np.zeros(shape)
+    f = oracle.rans_source(Z, Z, Z, [x * x, Z, Z, Z, Z, Z], None, *d, rho=rho)
+    inner = (slice(1, -1),) * 3
+    assert np.allclose(f[0][inner], -2 * rho * x[inner]) and np.allclose(f[1][inner], 0) and np.allclose(f[2][inner], 0)
+    f = oracle.rans_source(Z, Z, Z, [Z, Z, Z, Z, Z, y * z], None, *d, rho=rho)       # R_yz = y z: f_y = -rho y, f_z = -rho z... by axis
+    assert np.allclose(f[1][inner], -rho * y[inner]) and np.allclose(f[2][inner], -rho * z[inner]) and np.allclose(f[0][inner], 0)
+    # (iv) NaN pattern
+    Rxy = Z.copy(); Rxy[2, 3, 3] = np.nan
+    f = oracle.rans_source(Z, Z, Z, [Z, Z, Z, Rxy, Z, Z], None, *d, rho=rho)
+    expect = np.ones(shape, bool); expect[inner] = False
+    for dk, dj, di in ((0, 0, 0), (1, 0, 0), (-1, 0, 0), (0, 1, 0), (0, -1, 0), (0, 0, 1), (0, 0, -1)):
+        expect[2 + dk, 3 + dj, 3 + di] = True
+    assert all(np.array_equal(np.isnan(c), expect) for c in f)
+
+
+def test_compressible_rans_source_closed_forms(oracle):
+    """oracle.compressible_rans_source (Eq. 43-44 :540-545).  (i) Textbook case: the compressible free vortex
+    u_theta = Gamma / (2 pi r) is a steady, irrotational, homentropic Euler solution, so P / P_inf = (T / T_inf)^(gamma/(gamma-1))
+    with T from the adiabatic energy equation (Eq. 43): the oracle's g must converge to gamma/(gamma-1) grad ln T at
+    second order (the core is masked).  (ii) Linear mean velocity, quadratic stresses: uu_ij and T are quadratic, every
+    central difference is exact, and g equals the cell-wise solve of Eq. 44 with ANALYTIC derivatives to rounding
+    (catches a transposed matrix, a wrong stress index, a sign).  (iii) Fluid at rest or in uniform motion: g = 0."""
+    gam = 1.4
+    errs = []
+    for n in (65, 129):
+        h = 2.0 / (n - 1)
+        y, x = np.meshgrid(-1 + np.arange(n) * h, -1 + np.arange(n) * h, indexing="ij")
+        r2 = x * x + y * y
+        mask = (r2 >= 0.5 ** 2).astype(np.uint8)
+        G, Minf = 0.5, 0.4
+        Vinf = G                                         # reference state: the streamline r = 1
+        RTinf = Vinf ** 2 / (gam * Minf ** 2)            # M_inf^2 = V_inf^2 / (gamma R T_inf)
+        with np.errstate(divide="ignore", invalid="ignore"):
+            u, v = -G * y / r2, G * x / r2
+        u[mask == 0] = np.nan; v[mask == 0] = np.nan
+        g = oracle.compressible_rans_source(u, v, None, None, mask, h, h, gamma=gam, mach_inf=Minf, v_inf=Vinf, rgas_t_inf=RTinf)
+        c = 0.5 * (gam - 1) * Minf ** 2 / Vinf ** 2
+        with np.errstate(invalid="ignore", divide="ignore"):
+            th = 1 + c * (Vinf ** 2 - G * G / r2)
+            ex = [gam / (gam - 1) * c * 2 * G * G * x / r2 ** 2 / th, gam / (gam - 1) * c * 2 * G * G * y / r2 ** 2 / th]
+        ok = ~np.isnan(g[0])
+        assert ok.sum() > 0.5 * n * n
+        errs.append(max(np.abs(g[i][ok] - ex[i][ok]).max() for i in range(2)) / max(np.abs(ex[i][ok]).max() for i in range(2)))
+    assert errs[0] < 2e-2 and 3.2 < errs[0] / errs[1] < 4.8, errs      # max norm; the staircase core edge moves with n
+    # (ii) exactness with analytic derivatives, 3D, anisotropic spacing, with Reynolds stresses
+    rng = np.random.default_rng(2)
+    shape, d = (6, 7, 8), (0.03, 0.05, 0.07)
+    z, y, x = np.meshgrid(*[np.arange(n) * d[2 - ax] for ax, n in enumerate(shape)], indexing="ij")
+    X = [x, y, z]
+    a = rng.normal(size=3); B = 0.5 * rng.normal(size=(3, 3))
+    U = [a[i] + sum(B[i, j] * X[j] for j in range(3)) for i in range(3)]
+    pairs = [(0, 0), (1, 1), (2, 2), (0, 1), (0, 2), (1, 2)]
+    Rq, gRq = {}, {}
+    stress = []
+    for (i, j) in pairs:
+        b = 0.1 * rng.normal(size=3); Cq = 0.1 * rng.normal(size=(3, 3)); Cq = Cq + Cq.T
+        f = 0.05 * rng.normal() + sum(b[k] * X[k] for k in range(3)) + 0.5 * sum(Cq[k, l] * X[k] * X[l] for k in range(3) for l in range(3))
+        gf = [b[k] + sum(Cq[k, l] * X[l] for l in range(3)) for k in range(3)]
+        Rq[(i, j)] = Rq[(j, i)] = f; gRq[(i, j)] = gRq[(j, i)] = gf
+        stress.append(f)
+    Minf, Vinf, RTinf = 1.5, 2.0, 3.0
+    g = oracle.compressible_rans_source(U[0], U[1], U[2], stress, None, *d, gamma=gam, mach_inf=Minf, v_inf=Vinf, rgas_t_inf=RTinf)
+    c = 0.5 * (gam - 1) * Minf ** 2
+    th = 1 + c * (1 - sum(Ui * Ui for Ui in U) / Vinf ** 2)
+    dth = [-c / Vinf ** 2 * 2 * sum(U[i] * B[i, k] for i in range(3)) for k in range(3)]
+    inner = (slice(1, -1),) * 3
+    for (kk, jj, ii) in ((1, 1, 1), (2, 3, 4), (4, 5, 6), (3, 2, 5)):
+        A = np.zeros((3, 3)); rhs = np.zeros(3)
+        for i in range(3):
+            for j in range(3):
+                uu = U[i][kk, jj, ii] * U[j][kk, jj, ii] + Rq[(i, j)][kk, jj, ii]
+                duu = B[i, j] * U[j][kk, jj, ii] + U[i][kk, jj, ii] * B[j, j] + gRq[(i, j)][j][kk, jj, ii]
+                RT = RTinf * th[kk, jj, ii]
+                A[i, j] = (i == j) + uu / RT
+                rhs[i] += -(duu - uu / th[kk, jj, ii] * dth[j][kk, jj, ii]) / RT
+        ref = np.linalg.solve(A, rhs)
+        got = np.array([g[i][kk, jj, ii] for i in range(3)])
+        assert np.allclose(got, ref, rtol=1e-10, atol=1e-12), (got, ref)
+    edge = np.ones(shape, bool); edge[inner] = False
+    assert all(np.isnan(c_[edge]).all() and not np.isnan(c_[inner]).any() for c_ in g)
+    # (iii) rest and uniform motion
+    Z = np.zeros(shape)
+    for Uc in ((Z, Z, Z), (Z + 0.7, Z - 0.2, Z + 0.1)):
+        g = oracle.compressible_rans_source(*Uc, None, None, *d, gamma=gam, mach_inf=Minf, v_inf=Vinf, rgas_t_inf=RTinf)
+        assert all(np.allclose(c_[inner], 0.0, atol=1e-13) for c_ in g)
