@@ -163,6 +163,39 @@ int omni_velocity_source_f32(int nx, int ny, int nz, double dx, double dy, doubl
                              const unsigned char* d_mask, double rho, double mu,
                              float* d_gx, float* d_gy, float* d_gz, void* stream);
 
+/* ---- upstream, time-averaged flows: RANS source fields --------------------------------------
+ * Incompressible RANS, viscous terms dropped, Eq. 42:
+ *   f_i = -rho ( ubar_j d ubar_i / d x_j + d (u'_i u'_j) / d x_j )
+ * d_u, d_v, d_w: mean velocity, device, [nz][ny][nx] (d_w NULL iff nz == 1).  h_stress: HOST array of 3 (nz == 1: xx,
+ * yy, xy) or 6 (xx, yy, zz, xy, xz, yz) DEVICE pointers to the Reynolds stresses u'_i u'_j, or NULL / all entries NULL
+ * for none.  d_f*: device outputs (d_fz NULL iff nz == 1).  Discretisation and missing cells as in
+ * omni_velocity_source_* (reading R-V1): second-order central differences; a cell whose stencil touches a missing cell
+ * (outside the box, mask == 0, NaN in any input) gets NaN in every component.  Asynchronous on `stream`; returns an
+ * omni_status; invalid sizes / spacings / a partly given stress list: OMNI_ERR_INVALID_ARG, nothing enqueued. */
+int omni_rans_source_f64(int nx, int ny, int nz, double dx, double dy, double dz,
+                         const double* d_u, const double* d_v, const double* d_w, const double* const* h_stress,
+                         const unsigned char* d_mask, double rho, double* d_fx, double* d_fy, double* d_fz, void* stream);
+int omni_rans_source_f32(int nx, int ny, int nz, double dx, double dy, double dz,
+                         const float* d_u, const float* d_v, const float* d_w, const float* const* h_stress,
+                         const unsigned char* d_mask, double rho, float* d_fx, float* d_fy, float* d_fz, void* stream);
+
+/* Compressible RANS for an adiabatic ideal gas with negligible density fluctuations, Eq. 43-44:
+ *   T / T_inf = 1 + (gamma - 1)/2 M_inf^2 (1 - V^2 / V_inf^2),      uu_ij = ubar_i ubar_j + u'_i u'_j,
+ *   (delta_ij + uu_ij / (R T)) g_j = -(1 / (R T)) ( d uu_ij / d x_j - (uu_ij / T) d T / d x_j ),
+ * solved cell by cell for g = grad ln(P / P_inf); integrating g with omni_solve_* gives ln(P / P_inf) (:547).
+ * rgas_t_inf = R T_inf (the only way the gas constant and T_inf enter); gamma > 1, v_inf > 0, rgas_t_inf > 0.
+ * Arrays, h_stress, discretisation, missing cells and error behaviour as for omni_rans_source_*. */
+int omni_compressible_rans_source_f64(int nx, int ny, int nz, double dx, double dy, double dz,
+                                      const double* d_u, const double* d_v, const double* d_w,
+                                      const double* const* h_stress, const unsigned char* d_mask,
+                                      double gamma, double mach_inf, double v_inf, double rgas_t_inf,
+                                      double* d_gx, double* d_gy, double* d_gz, void* stream);
+int omni_compressible_rans_source_f32(int nx, int ny, int nz, double dx, double dy, double dz,
+                                      const float* d_u, const float* d_v, const float* d_w,
+                                      const float* const* h_stress, const unsigned char* d_mask,
+                                      double gamma, double mach_inf, double v_inf, double rgas_t_inf,
+                                      float* d_gx, float* d_gy, float* d_gz, void* stream);
+
 /* ---- single steps of the path (each runs the same device code the solve runs; used by the parity tests) ----------
  * a0  geometry constants (host only, no device needed).  out[0..2] = face totals F_x,F_y,F_z (Eq. 5 :75 / Eq. 23 :258),
  *     out[3] = A_tot (Eq. 8 :94 / Eq. 24 :262), out[4..12] = c_jk row-major 3x3 (Eq. 17 :207 / Eq. 32-35 :314-326 /

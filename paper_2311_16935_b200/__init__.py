@@ -4,7 +4,8 @@ The product is the C-ABI library libomni.so (include/omni.h, csrc/); this packag
 Importing the package does not load the library; the first call does, and fails loudly when it is missing.
 """
 from .binding import (Info, OmniError, SYMBOLS, apply_M, constants, launch_count, lib, profile_enable,  # noqa: F401
-                      profile_read, release_memory, residual, set_loop_mode, solve, solve_batch2d, solve_cascade, solve_direct, source, status_string, velocity_source, version, workspace_bytes)
+                      profile_read, release_memory, residual, set_loop_mode, solve, solve_batch2d, solve_cascade, solve_direct, source, status_string, velocity_source, version, workspace_bytes,
+                      rans_source, compressible_rans_source)
 
 # the C names, for callers who think in terms of include/omni.h
 omni_solve = solve
@@ -13,6 +14,8 @@ omni_solve_direct = solve_direct
 omni_solve_cascade = solve_cascade
 omni_source = source
 omni_velocity_source = velocity_source
+omni_rans_source = rans_source
+omni_compressible_rans_source = compressible_rans_source
 omni_apply_M = apply_M
 omni_residual = residual
 omni_constants = constants

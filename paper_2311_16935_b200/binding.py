@@ -17,7 +17,8 @@ STATUS_NAMES = {0: "OMNI_OK", 1: "OMNI_NOT_CONVERGED", -1: "OMNI_ERR_INVALID_ARG
                 -3: "OMNI_ERR_ALLOC", -4: "OMNI_ERR_BREAKDOWN"}
 # every symbol include/omni.h declares
 SYMBOLS = ["omni_solve_f64", "omni_solve_f32", "omni_workspace_bytes", "omni_solve_f64_ws", "omni_solve_f32_ws",
-           "omni_solve_host_f64", "omni_solve_host_f32", "omni_solve_batch2d_f64", "omni_solve_batch2d_f32", "omni_solve_direct_f64", "omni_solve_direct_f32", "omni_solve_direct_batch2d_f64", "omni_solve_direct_batch2d_f32", "omni_solve_cascade_f64", "omni_solve_cascade_f32", "omni_velocity_source_f64", "omni_velocity_source_f32", "omni_constants", "omni_source_f64", "omni_source_f32",
+           "omni_solve_host_f64", "omni_solve_host_f32", "omni_solve_batch2d_f64", "omni_solve_batch2d_f32", "omni_solve_direct_f64", "omni_solve_direct_f32", "omni_solve_direct_batch2d_f64", "omni_solve_direct_batch2d_f32", "omni_solve_cascade_f64", "omni_solve_cascade_f32", "omni_velocity_source_f64", "omni_velocity_source_f32", "omni_rans_source_f64", "omni_rans_source_f32",
+           "omni_compressible_rans_source_f64", "omni_compressible_rans_source_f32", "omni_constants", "omni_source_f64", "omni_source_f32",
            "omni_apply_M_f64", "omni_apply_M_f32", "omni_residual_f64", "omni_residual_f32", "omni_launch_count",
            "omni_set_loop_mode", "omni_release_memory", "omni_profile_enable", "omni_profile_read", "omni_status_string", "omni_version"]
 
@@ -223,6 +224,51 @@ def velocity_source(u, v, w, mask, d, rho=1.0, mu=0.0, dudt=None):
                 C.c_double(rho), C.c_double(mu), _ptr(g[0]), _ptr(g[1]), _ptr(g[2]), _stream(u.device))
     if rc < 0:
         raise OmniError(rc, f"omni_velocity_source_{sfx}")
+    return g[:2] if w is None else g
+
+
+def _stress_array(stress, nd):
+    """HOST array of device pointers to the Reynolds stresses (2D: xx, yy, xy; 3D: xx, yy, zz, xy, xz, yz), or None."""
+    if stress is None:
+        return None
+    if len(stress) != (3 if nd == 2 else 6):
+        raise ValueError("stress: 3 components (xx, yy, xy) in 2D, 6 (xx, yy, zz, xy, xz, yz) in 3D")
+    return (C.c_void_p * len(stress))(*[_ptr(t) for t in stress])
+
+
+def rans_source(u, v, w, stress, mask, d, rho=1.0):
+    """omni_rans_source_*: f of Eq. 42 from the mean velocity and the Reynolds stresses (CUDA tensors; w = None in 2D;
+    stress = list of tensors or None).  Returns [fx, fy(, fz)]."""
+    import torch
+    sfx = _suffix(u)
+    _check([u, v, w, mask] + (list(stress) if stress is not None else []), "cuda")
+    if mask is not None and mask.dtype != torch.uint8:
+        raise TypeError("mask must be uint8")
+    g = [torch.empty_like(u), torch.empty_like(u), None if w is None else torch.empty_like(u)]
+    arr = _stress_array(stress, 2 if w is None else 3)
+    with torch.cuda.device(u.device):
+        rc = getattr(lib(), f"omni_rans_source_{sfx}")(*_geom(u, d), _ptr(u), _ptr(v), _ptr(w), arr, _ptr(mask), C.c_double(rho),
+                                                       _ptr(g[0]), _ptr(g[1]), _ptr(g[2]), _stream(u.device))
+    if rc < 0:
+        raise OmniError(rc, f"omni_rans_source_{sfx}")
+    return g[:2] if w is None else g
+
+
+def compressible_rans_source(u, v, w, stress, mask, d, gamma=1.4, mach_inf=2.0, v_inf=1.0, rgas_t_inf=1.0):
+    """omni_compressible_rans_source_*: g = grad ln(P / P_inf) of Eq. 43-44.  Returns [gx, gy(, gz)]."""
+    import torch
+    sfx = _suffix(u)
+    _check([u, v, w, mask] + (list(stress) if stress is not None else []), "cuda")
+    if mask is not None and mask.dtype != torch.uint8:
+        raise TypeError("mask must be uint8")
+    g = [torch.empty_like(u), torch.empty_like(u), None if w is None else torch.empty_like(u)]
+    arr = _stress_array(stress, 2 if w is None else 3)
+    with torch.cuda.device(u.device):
+        fn = getattr(lib(), f"omni_compressible_rans_source_{sfx}")
+        rc = fn(*_geom(u, d), _ptr(u), _ptr(v), _ptr(w), arr, _ptr(mask), C.c_double(gamma), C.c_double(mach_inf),
+                C.c_double(v_inf), C.c_double(rgas_t_inf), _ptr(g[0]), _ptr(g[1]), _ptr(g[2]), _stream(u.device))
+    if rc < 0:
+        raise OmniError(rc, f"omni_compressible_rans_source_{sfx}")
     return g[:2] if w is None else g
 
 

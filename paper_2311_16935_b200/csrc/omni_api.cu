@@ -917,6 +917,46 @@ int velocity_source(int nx, int ny, int nz, double dx, double dy, double dz, con
     return OMNI_OK;
 }
 
+// NEXT-4: RANS source fields (Eq. 42 :507; Eq. 43-44 :540-545) on device arrays in the caller's layout
+template <typename T>
+int rans_source(bool compressible, int nx, int ny, int nz, double dx, double dy, double dz, const T* u, const T* v, const T* w,
+                const T* const* stress, const unsigned char* mask, double rho, double gamma, double mach_inf, double v_inf,
+                double rgas_t_inf, T* gx, T* gy, T* gz, void* stream)
+{
+    if (nx < 1 || ny < 1 || nz < 1 || !(dx > 0.0) || !(dy > 0.0) || (nz > 1 && !(dz > 0.0))) return OMNI_ERR_INVALID_ARG;
+    const int nd = (nz > 1) ? 3 : 2, nR = (nd == 2) ? 3 : 6;
+    if (!u || !v || !gx || !gy || (nd == 3 && (!w || !gz))) return OMNI_ERR_INVALID_ARG;
+    int given = 0;
+    if (stress)
+        for (int m = 0; m < nR; ++m) given += (stress[m] != nullptr);
+    if (given != 0 && given != nR) return OMNI_ERR_INVALID_ARG;
+    if (compressible) {
+        if (!(gamma > 1.0) || !std::isfinite(gamma) || !std::isfinite(mach_inf) || !(v_inf > 0.0) || !std::isfinite(v_inf) ||
+            !(rgas_t_inf > 0.0) || !std::isfinite(rgas_t_inf))
+            return OMNI_ERR_INVALID_ARG;
+    } else if (!std::isfinite(rho)) {
+        return OMNI_ERR_INVALID_ARG;
+    }
+    RansArgs<T> a;
+    a.u[0] = u; a.u[1] = v; a.u[2] = (nd == 3) ? w : nullptr;
+    for (int m = 0; m < 6; ++m) a.R[m] = (given && m < nR) ? stress[m] : nullptr;
+    a.mask = mask;
+    a.g[0] = gx; a.g[1] = gy; a.g[2] = (nd == 3) ? gz : nullptr;
+    a.ih[0] = (T)(0.5 / dx); a.ih[1] = (T)(0.5 / dy); a.ih[2] = (T)(nd == 3 ? 0.5 / dz : 0.0);
+    a.rho = (T)rho;
+    a.cth = (T)(compressible ? 0.5 * (gamma - 1.0) * mach_inf * mach_inf : 0.0);
+    a.inv_v2 = (T)(compressible ? 1.0 / (v_inf * v_inf) : 0.0);
+    a.rt_inf = (T)rgas_t_inf;
+    a.has_R = given ? 1 : 0;
+    cudaStream_t st = (cudaStream_t)stream;
+    const long long n = (long long)nx * ny * nz;
+    if (compressible) rans_source_kernel<T, true><<<blocks_for(n, 256), 256, 0, st>>>(nx, ny, nz, nd, a);
+    else rans_source_kernel<T, false><<<blocks_for(n, 256), 256, 0, st>>>(nx, ny, nz, nd, a);
+    g_launches.fetch_add(1, std::memory_order_relaxed);
+    CK(cudaGetLastError());
+    return OMNI_OK;
+}
+
 template <typename T>
 int solve_host(int nx, int ny, int nz, double dx, double dy, double dz, const T* gx, const T* gy, const T* gz,
                const unsigned char* mask, T* P_out, double tol, int max_outer, int max_cg, void* stream, omni_info* info)
@@ -1208,6 +1248,38 @@ int omni_velocity_source_f32(int nx, int ny, int nz, double dx, double dy, doubl
                              void* stream)
 {
     return velocity_source<float>(nx, ny, nz, dx, dy, dz, d_u, d_v, d_w, d_dudt, d_dvdt, d_dwdt, d_mask, rho, mu, d_gx, d_gy, d_gz, stream);
+}
+
+int omni_rans_source_f64(int nx, int ny, int nz, double dx, double dy, double dz, const double* d_u, const double* d_v,
+                         const double* d_w, const double* const* d_stress, const unsigned char* d_mask, double rho,
+                         double* d_fx, double* d_fy, double* d_fz, void* stream)
+{
+    return rans_source<double>(false, nx, ny, nz, dx, dy, dz, d_u, d_v, d_w, d_stress, d_mask, rho, 0, 0, 0, 0, d_fx, d_fy, d_fz, stream);
+}
+
+int omni_rans_source_f32(int nx, int ny, int nz, double dx, double dy, double dz, const float* d_u, const float* d_v,
+                         const float* d_w, const float* const* d_stress, const unsigned char* d_mask, double rho,
+                         float* d_fx, float* d_fy, float* d_fz, void* stream)
+{
+    return rans_source<float>(false, nx, ny, nz, dx, dy, dz, d_u, d_v, d_w, d_stress, d_mask, rho, 0, 0, 0, 0, d_fx, d_fy, d_fz, stream);
+}
+
+int omni_compressible_rans_source_f64(int nx, int ny, int nz, double dx, double dy, double dz, const double* d_u,
+                                      const double* d_v, const double* d_w, const double* const* d_stress,
+                                      const unsigned char* d_mask, double gamma, double mach_inf, double v_inf,
+                                      double rgas_t_inf, double* d_gx, double* d_gy, double* d_gz, void* stream)
+{
+    return rans_source<double>(true, nx, ny, nz, dx, dy, dz, d_u, d_v, d_w, d_stress, d_mask, 0, gamma, mach_inf, v_inf, rgas_t_inf,
+                               d_gx, d_gy, d_gz, stream);
+}
+
+int omni_compressible_rans_source_f32(int nx, int ny, int nz, double dx, double dy, double dz, const float* d_u,
+                                      const float* d_v, const float* d_w, const float* const* d_stress,
+                                      const unsigned char* d_mask, double gamma, double mach_inf, double v_inf,
+                                      double rgas_t_inf, float* d_gx, float* d_gy, float* d_gz, void* stream)
+{
+    return rans_source<float>(true, nx, ny, nz, dx, dy, dz, d_u, d_v, d_w, d_stress, d_mask, 0, gamma, mach_inf, v_inf, rgas_t_inf,
+                              d_gx, d_gy, d_gz, stream);
 }
 
 int omni_constants(int nx, int ny, int nz, double dx, double dy, double dz, double* h_out13)

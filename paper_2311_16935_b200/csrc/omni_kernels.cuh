@@ -758,4 +758,120 @@ __global__ void velocity_source_kernel(int nx, int ny, int nz, int ncomp, T idx2
     if (ncomp == 3) gz[c] = term(w, atz);
 }
 
+// ------------------------------------------------------------------------------------------------ RANS source fields
+// Eq. 42: f_i = -rho (ubar_j d_j ubar_i + d_j R_ij)                                  (COMPRESSIBLE = false)
+// Eq. 43-44 (:540-545):  theta = T/T_inf = 1 + (gamma-1)/2 M_inf^2 (1 - V^2/V_inf^2), uu_ij = ubar_i ubar_j + R_ij,
+//                        (delta_ij + uu_ij/(R T)) g_j = -(1/(R T)) (d_j uu_ij - uu_ij/T d_j T)       (COMPRESSIBLE = true)
+// solved cell by cell for g = grad ln(P/P_inf) (Gaussian elimination with partial pivoting, 2x2 / 3x3).
+// Second-order central differences, caller layout, one thread per cell; a cell whose stencil touches a missing cell
+// (outside the box, mask == 0, NaN in any input) gets NaN in every component (reading R-V1).
+template <typename T>
+struct RansArgs {
+    const T* u[3];            // mean velocity (u[2] null in 2D)
+    const T* R[6];            // Reynolds stresses: 2D xx, yy, xy; 3D xx, yy, zz, xy, xz, yz (all null: none)
+    const uint8_t* mask;
+    T* g[3];
+    T ih[3];                  // 1 / (2 h_a)
+    T rho;                    // Eq. 42
+    T cth, inv_v2, rt_inf;    // Eq. 43-44: (gamma-1)/2 M_inf^2, 1 / V_inf^2, R T_inf
+    int has_R;
+};
+
+__host__ __device__ __forceinline__ int stress_slot(int nd, int i, int j)
+{
+    if (i == j) return i;
+    if (nd == 2) return 2;
+    return i + j + 2;         // (0,1) -> 3, (0,2) -> 4, (1,2) -> 5
+}
+
+template <typename T, bool COMPRESSIBLE>
+__global__ void rans_source_kernel(int nx, int ny, int nz, int nd, const RansArgs<T> a)
+{
+    const long long c = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const long long n = (long long)nx * ny * nz;
+    if (c >= n) return;
+    const int i = (int)(c % nx), j = (int)((c / nx) % ny), k = (int)(c / ((long long)nx * ny));
+    const long long st[3] = { 1, nx, (long long)nx * ny };
+    const int nR = (nd == 2) ? 3 : 6;
+    auto ok = [&](long long q) {
+        if (a.mask != nullptr && a.mask[q] == 0) return false;
+        for (int m = 0; m < nd; ++m)
+            if (isnan(a.u[m][q])) return false;
+        if (a.has_R)
+            for (int m = 0; m < nR; ++m)
+                if (isnan(a.R[m][q])) return false;
+        return true;
+    };
+    bool good = ok(c) && i > 0 && i < nx - 1 && j > 0 && j < ny - 1 && (nd == 2 || (k > 0 && k < nz - 1));
+    if (good)
+        for (int m = 0; m < nd; ++m) good = good && ok(c - st[m]) && ok(c + st[m]);
+    if (!good) {
+        const T qnan = (T)nan("");
+        for (int m = 0; m < nd; ++m) a.g[m][c] = qnan;
+        return;
+    }
+    T uc[3] = { T(0), T(0), T(0) };
+    for (int m = 0; m < nd; ++m) uc[m] = a.u[m][c];
+    if constexpr (!COMPRESSIBLE) {
+        for (int p = 0; p < nd; ++p) {
+            T conv = T(0), div = T(0);
+            for (int q = 0; q < nd; ++q) {
+                conv += uc[q] * ((a.u[p][c + st[q]] - a.u[p][c - st[q]]) * a.ih[q]);
+                if (a.has_R) {
+                    const T* __restrict__ Rpq = a.R[stress_slot(nd, p < q ? p : q, p < q ? q : p)];
+                    div += (Rpq[c + st[q]] - Rpq[c - st[q]]) * a.ih[q];
+                }
+            }
+            a.g[p][c] = -a.rho * (conv + div);
+        }
+    } else {
+        auto theta_at = [&](long long q) {
+            T v2 = T(0);
+            for (int m = 0; m < nd; ++m) v2 += a.u[m][q] * a.u[m][q];
+            return T(1) + a.cth * (T(1) - v2 * a.inv_v2);
+        };
+        auto uu_at = [&](int p, int q, long long cell) {
+            T v = a.u[p][cell] * a.u[q][cell];
+            if (a.has_R) v += a.R[stress_slot(nd, p < q ? p : q, p < q ? q : p)][cell];
+            return v;
+        };
+        const T th = theta_at(c);
+        const T rt = a.rt_inf * th;
+        T dth[3] = { T(0), T(0), T(0) };
+        for (int q = 0; q < nd; ++q) dth[q] = (theta_at(c + st[q]) - theta_at(c - st[q])) * a.ih[q];
+        T A[3][4];
+        for (int p = 0; p < 3; ++p)
+            for (int q = 0; q < 4; ++q) A[p][q] = (p == q) ? T(1) : T(0);
+        for (int p = 0; p < nd; ++p) {
+            T b = T(0);
+            for (int q = 0; q < nd; ++q) {
+                const T uu = uu_at(p, q, c);
+                A[p][q] = ((p == q) ? T(1) : T(0)) + uu / rt;
+                const T duu = (uu_at(p, q, c + st[q]) - uu_at(p, q, c - st[q])) * a.ih[q];
+                b += -(T(1) / rt) * (duu - uu / th * dth[q]);
+            }
+            A[p][3] = b;
+        }
+        // Gaussian elimination with partial pivoting on the nd x nd system (rows beyond nd are identity)
+#pragma unroll
+        for (int col = 0; col < 3; ++col) {
+            int piv = col;
+            for (int r = col + 1; r < 3; ++r)
+                if (fabs(A[r][col]) > fabs(A[piv][col])) piv = r;
+            for (int q = 0; q < 4; ++q) { const T t = A[col][q]; A[col][q] = A[piv][q]; A[piv][q] = t; }
+            for (int r = col + 1; r < 3; ++r) {
+                const T f = A[r][col] / A[col][col];
+                for (int q = col; q < 4; ++q) A[r][q] -= f * A[col][q];
+            }
+        }
+        T x[3];
+        for (int r = 2; r >= 0; --r) {
+            T s = A[r][3];
+            for (int q = r + 1; q < 3; ++q) s -= A[r][q] * x[q];
+            x[r] = s / A[r][r];
+        }
+        for (int m = 0; m < nd; ++m) a.g[m][c] = x[m];
+    }
+}
+
 }  // namespace omni
