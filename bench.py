@@ -31,8 +31,8 @@ CPU_SAMPLE_EDGE = 320                   # 3D: edge of the corner crop the oracle
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel (K4) from the ncu --set full capture
 # summarised in profiles/r1_ncu_k3_k4_500cube_f32.md; only valid for that workload.  K4 streams different arrays by
 # CG-iteration parity (lazy delta): even k, the first odd k (delta not read yet), the other odd k.
-NCU_TRAFFIC_K4 = {(4, "f32"): {"even": 1.021704e9 + 0.461907e9, "odd_first": 1.530113e9 + 0.963922e9,
-                               "odd": 2.028161e9 + 0.963717e9}}
+NCU_TRAFFIC_K4 = {(4, "f32"): {"even": 1.032482e9 + 0.462397e9, "odd_first": 1.544273e9 + 0.962295e9,
+                               "odd": 2.042280e9 + 0.962293e9}}
 
 
 def k4_traffic(t, n_even, n_odd):
