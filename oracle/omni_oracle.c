@@ -397,6 +397,16 @@ int oracle_solve(int nx, int ny, int nz, double dx, double dy, double dz,
     return solve_impl(nx, ny, nz, dx, dy, dz, gx, gy, gz, mask, NULL, P_out, tol, max_outer, max_cg, info, hist, hist_cap);
 }
 
+/* Algorithm 1 started from a first guess instead of P^0 = 0 ("initializing with a first guess for the pressure field",
+ * PAPER.md:82; a volume of a time series starts from the previous one's pressure).  Same iteration, same stopping
+ * rules; P_init at missing cells is ignored. */
+int oracle_solve_guess(int nx, int ny, int nz, double dx, double dy, double dz,
+                       const double *gx, const double *gy, const double *gz, const unsigned char *mask,
+                       const double *P_init, double *P_out, double tol, int max_outer, int max_cg, oracle_info *info)
+{
+    return solve_impl(nx, ny, nz, dx, dy, dz, gx, gy, gz, mask, P_init, P_out, tol, max_outer, max_cg, info, NULL, 0);
+}
+
 /* The fixed point of Alg. 1 computed without the boundary iteration: at convergence P^{n+1} = P^n, so Eq. 12 reads
  * (M - W^n) P = S, i.e. L P = S with L the symmetric positive semi-definite weighted graph Laplacian of the valid
  * cells (constant null space per connected component; S sums to zero on each).  CG on it from P = 0 returns the

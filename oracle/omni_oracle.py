@@ -159,6 +159,28 @@ def solve(gx, gy, gz, mask, dx, dy, dz, tol, max_outer, max_cg, hist_cap=0):
     return (P, d, hist) if hist_cap else (P, d)
 
 
+def solve_guess(gx, gy, gz, mask, dx, dy, dz, tol, max_outer, max_cg, P_init):
+    """Algorithm 1 started from the first guess P_init (oracle_solve_guess).  Returns (P, info)."""
+    gx, gy = _f64(gx), _f64(gy)
+    nx, ny, nz = _dims(gx.shape)
+    gz = _f64(gz) if gz is not None else None
+    if nz > 1 and gz is None:
+        raise ValueError("gz required in 3D")
+    m = None if mask is None else np.ascontiguousarray(mask, dtype=np.uint8)
+    P = np.zeros(gx.shape)
+    info = Info()
+    P0 = None if P_init is None else _f64(P_init)
+    f = lib().oracle_solve_guess
+    f.restype = C.c_int
+    rc = f(C.c_int(nx), C.c_int(ny), C.c_int(nz), C.c_double(dx), C.c_double(dy), C.c_double(dz),
+           _p(gx), _p(gy), _p(gz if gz is not None else gx), _p(m), _p(P0), _p(P), C.c_double(tol), C.c_int(max_outer),
+           C.c_int(max_cg), C.byref(info))
+    if rc != 0:
+        raise MemoryError("oracle_solve_guess: allocation failed")
+    return P, {"outer_iters": info.outer_iters, "cg_iters_total": info.cg_iters_total, "eps_R_final": info.eps_R_final,
+               "norm_S": info.norm_S, "converged": bool(info.converged)}
+
+
 def solve_direct(gx, gy, gz, mask, dx, dy, dz, tol, max_outer, max_cg, P_init=None):
     """Fixed point of Algorithm 1 by CG on L P = S (oracle_solve_direct; not the paper's iteration).  Returns (P, info)."""
     gx, gy = _f64(gx), _f64(gy)

@@ -763,3 +763,39 @@ def test_compressible_rans_source_closed_forms(oracle):
     for Uc in ((Z, Z, Z), (Z + 0.7, Z - 0.2, Z + 0.1)):
         g = oracle.compressible_rans_source(*Uc, None, None, *d, gamma=gam, mach_inf=Minf, v_inf=Vinf, rgas_t_inf=RTinf)
         assert all(np.allclose(c_[inner], 0.0, atol=1e-13) for c_ in g)
+
+
+def test_solve_guess_pins(oracle):
+    """oracle.solve_guess (Alg. 1 from a first guess): (i) P_init = 0 / None is oracle.solve; (ii) started from
+    its own converged field it stops at the first residual check (0 outer iterations) and returns the field; (iii) every
+    row of M - W^n sums to zero (:631), so a guess shifted by a constant per connected component shifts every iterate by
+    the same constants: after a fixed number of steps P(guess + c) - P(guess) = c exactly up to rounding; (iv) the fixed
+    point does not depend on the guess up to that constant (compared with the dense pseudo-inverse pin via oracle.solve);
+    (v) the guess at missing cells is ignored."""
+    from workloads import make_field
+    f = make_field("sphere3d", (10, 11, 12), seed=5, noise=0.05)
+    g, m, d = f["g"], f["mask"], f["d"]
+    P0, i0 = oracle.solve(*g, m, *d, tol=0.0, max_outer=4, max_cg=10)
+    Pz, iz = oracle.solve_guess(*g, m, *d, tol=0.0, max_outer=4, max_cg=10, P_init=np.zeros(g[0].shape))
+    assert np.array_equal(P0, Pz, equal_nan=True) and i0 == iz
+    Pn, i_n = oracle.solve_guess(*g, m, *d, tol=0.0, max_outer=4, max_cg=10, P_init=None)
+    assert np.array_equal(P0, Pn, equal_nan=True)
+    # (ii)
+    Pc, ic = oracle.solve(*g, m, *d, tol=1e-9, max_outer=100000, max_cg=200)
+    assert ic["converged"]
+    guess = np.where(np.isnan(Pc), 123.0, Pc)                   # (v): garbage at the missing cells
+    Pr, ir = oracle.solve_guess(*g, m, *d, tol=1.0001e-9, max_outer=100000, max_cg=200, P_init=guess)
+    assert ir["outer_iters"] == 0 and ir["cg_iters_total"] == 0
+    assert np.array_equal(Pr, Pc, equal_nan=True)
+    # (iii)
+    rng = np.random.default_rng(3)
+    base = rng.normal(size=g[0].shape)
+    Pa, _ = oracle.solve_guess(*g, m, *d, tol=0.0, max_outer=3, max_cg=8, P_init=base)
+    Pb, _ = oracle.solve_guess(*g, m, *d, tol=0.0, max_outer=3, max_cg=8, P_init=base + 2.5)
+    v = ~np.isnan(Pa)
+    assert np.allclose(Pb[v] - Pa[v], 2.5, rtol=0, atol=1e-11)
+    # (iv)
+    Pg, ig = oracle.solve_guess(*g, m, *d, tol=1e-9, max_outer=100000, max_cg=200, P_init=base)
+    assert ig["converged"]
+    a, b = Pg[v] - Pg[v].mean(), Pc[v] - Pc[v].mean()
+    assert np.linalg.norm(a - b) / np.linalg.norm(b) < 1e-6
