@@ -87,6 +87,21 @@ int omni_solve_host_f32(int nx, int ny, int nz, double dx, double dy, double dz,
                         const float* h_gx, const float* h_gy, const float* h_gz, const unsigned char* h_mask,
                         float* h_P_out, double tol, int max_outer, int max_cg, void* stream, omni_info* info);
 
+/* ---- Algorithm 1 from a first guess ("initializing with a first guess for the pressure field") -------------
+ * omni_solve_* with P^0 = d_P_init (device, [nz][ny][nx]; values at missing cells are ignored; NULL = zeros, i.e.
+ * omni_solve_*) instead of P^0 = 0 (:139): the next volume of a time series starts from the previous one's pressure.
+ * Same iteration, kernels, stopping rules, status codes and omni_info; the first residual check already counts, so a
+ * guess that satisfies eps_R <= tol returns after zero outer iterations.  A constant added to the guess on a connected
+ * component is added to the result on it (every row of M - W^n sums to zero, :631). */
+int omni_solve_guess_f64(int nx, int ny, int nz, double dx, double dy, double dz,
+                         const double* d_gx, const double* d_gy, const double* d_gz, const unsigned char* d_mask,
+                         const double* d_P_init, double* d_P_out, double tol, int max_outer, int max_cg, void* stream,
+                         omni_info* info);
+int omni_solve_guess_f32(int nx, int ny, int nz, double dx, double dy, double dz,
+                         const float* d_gx, const float* d_gy, const float* d_gz, const unsigned char* d_mask,
+                         const float* d_P_init, float* d_P_out, double tol, int max_outer, int max_cg, void* stream,
+                         omni_info* info);
+
 /* ---- fixed point of Algorithm 1 without the boundary iteration (SURVEY.md 8(f) NEXT-2 iii) -----------------------------
  * NOT the paper's iteration: at a fixed point P^{n+1} = P^n of Alg. 1, Eq. 12 reads (M - W^n) P = S,
  * i.e. L P = S with L the symmetric positive semi-definite weighted graph Laplacian of the valid cells

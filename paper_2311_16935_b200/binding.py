@@ -17,7 +17,7 @@ STATUS_NAMES = {0: "OMNI_OK", 1: "OMNI_NOT_CONVERGED", -1: "OMNI_ERR_INVALID_ARG
                 -3: "OMNI_ERR_ALLOC", -4: "OMNI_ERR_BREAKDOWN"}
 # every symbol include/omni.h declares
 SYMBOLS = ["omni_solve_f64", "omni_solve_f32", "omni_workspace_bytes", "omni_solve_f64_ws", "omni_solve_f32_ws",
-           "omni_solve_host_f64", "omni_solve_host_f32", "omni_solve_batch2d_f64", "omni_solve_batch2d_f32", "omni_solve_direct_f64", "omni_solve_direct_f32", "omni_solve_direct_batch2d_f64", "omni_solve_direct_batch2d_f32", "omni_solve_cascade_f64", "omni_solve_cascade_f32", "omni_velocity_source_f64", "omni_velocity_source_f32", "omni_rans_source_f64", "omni_rans_source_f32",
+           "omni_solve_host_f64", "omni_solve_host_f32", "omni_solve_batch2d_f64", "omni_solve_batch2d_f32", "omni_solve_guess_f64", "omni_solve_guess_f32", "omni_solve_direct_f64", "omni_solve_direct_f32", "omni_solve_direct_batch2d_f64", "omni_solve_direct_batch2d_f32", "omni_solve_cascade_f64", "omni_solve_cascade_f32", "omni_velocity_source_f64", "omni_velocity_source_f32", "omni_rans_source_f64", "omni_rans_source_f32",
            "omni_compressible_rans_source_f64", "omni_compressible_rans_source_f32", "omni_constants", "omni_source_f64", "omni_source_f32",
            "omni_apply_M_f64", "omni_apply_M_f32", "omni_residual_f64", "omni_residual_f32", "omni_launch_count",
            "omni_set_loop_mode", "omni_release_memory", "omni_profile_enable", "omni_profile_read", "omni_status_string", "omni_version"]
@@ -186,9 +186,15 @@ def solve(gx, gy, gz, mask, d, tol, max_outer, max_cg, out=None, workspace=None,
     return P, (info.as_dict() if (want_info or host) else None)
 
 
-def solve_direct(gx, gy, gz, mask, d, tol, max_outer, max_cg, out=None, P_init=None):
+def solve_guess(gx, gy, gz, mask, d, tol, max_outer, max_cg, P_init, out=None):
+    """omni_solve_guess_*: Algorithm 1 started from the first guess P_init.  Returns (P, info dict)."""
+    return solve_direct(gx, gy, gz, mask, d, tol, max_outer, max_cg, out=out, P_init=P_init, _entry="omni_solve_guess")
+
+
+def solve_direct(gx, gy, gz, mask, d, tol, max_outer, max_cg, out=None, P_init=None, _entry="omni_solve_direct"):
     """omni_solve_direct_*: the fixed point of Algorithm 1 by CG on L P = S (not the paper's iteration; include/omni.h).
-    CUDA tensors; d = (dx, dy[, dz]).  Returns (P, info dict)."""
+    CUDA tensors; d = (dx, dy[, dz]).  Returns (P, info dict).  (`_entry` selects the C entry point with the same
+    argument list: omni_solve_guess_* shares the marshalling.)"""
     import torch
     sfx = _suffix(gx)
     _check([gx, gy, gz, mask, out, P_init], "cuda")
@@ -199,11 +205,11 @@ def solve_direct(gx, gy, gz, mask, d, tol, max_outer, max_cg, out=None, P_init=N
     P = out if out is not None else torch.empty_like(gx)
     info = Info()
     with torch.cuda.device(gx.device):
-        fn = getattr(lib(), f"omni_solve_direct_{sfx}")
+        fn = getattr(lib(), f"{_entry}_{sfx}")
         rc = fn(*_geom(gx, d), _ptr(gx), _ptr(gy), _ptr(gz), _ptr(mask), _ptr(P_init), _ptr(P), C.c_double(tol), C.c_int(max_outer),
                 C.c_int(max_cg), _stream(gx.device), C.byref(info))
     if rc < 0:
-        raise OmniError(rc, f"omni_solve_direct_{sfx}")
+        raise OmniError(rc, f"{_entry}_{sfx}")
     return P, info.as_dict()
 
 

@@ -1204,6 +1204,22 @@ int omni_solve_direct_batch2d_f32(int nx, int ny, int nb, double dx, double dy, 
                               info, 1, d_P_init, 1);
 }
 
+int omni_solve_guess_f64(int nx, int ny, int nz, double dx, double dy, double dz, const double* d_gx, const double* d_gy,
+                         const double* d_gz, const unsigned char* d_mask, const double* d_P_init, double* d_P_out,
+                         double tol, int max_outer, int max_cg, void* stream, omni_info* info)
+{
+    return solve_alloc<double>(nx, ny, nz, dx, dy, dz, d_gx, d_gy, d_gz, d_mask, d_P_out, tol, max_outer, max_cg, stream, info,
+                               0, d_P_init, 0);
+}
+
+int omni_solve_guess_f32(int nx, int ny, int nz, double dx, double dy, double dz, const float* d_gx, const float* d_gy,
+                         const float* d_gz, const unsigned char* d_mask, const float* d_P_init, float* d_P_out,
+                         double tol, int max_outer, int max_cg, void* stream, omni_info* info)
+{
+    return solve_alloc<float>(nx, ny, nz, dx, dy, dz, d_gx, d_gy, d_gz, d_mask, d_P_out, tol, max_outer, max_cg, stream, info,
+                              0, d_P_init, 0);
+}
+
 int omni_solve_direct_f64(int nx, int ny, int nz, double dx, double dy, double dz, const double* d_gx, const double* d_gy,
                           const double* d_gz, const unsigned char* d_mask, const double* d_P_init, double* d_P_out,
                           double tol, int max_outer, int max_cg, void* stream, omni_info* info)

@@ -645,3 +645,41 @@ def test_rans_source_parity(oracle, dtype):
     valid = ~np.isnan(Pn)
     assert valid.sum() > 0.6 * n * n
     assert rel_l2_after_mean_removal(Pn, lnP, valid) < 5e-3
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_solve_guess_parity(oracle, dtype, forced_loop):
+    """omni_solve_guess_* (Alg. 1 from a first guess) against oracle.solve_guess: trajectory parity from a
+    random guess in 3D (masked) and 2D, garbage at the missing cells ignored; a NULL guess is bit-identical to omni_solve;
+    a restart from the converged field of omni_solve stops at the first residual check."""
+    rng = np.random.default_rng(31)
+    np_dt = np.float32 if dtype == "f32" else np.float64
+    bound = 1e-9 if dtype == "f64" else 2e-4
+    for kind, shape in (("sphere3d", (20, 26, 70)), ("lamb_oseen2d", (40, 150))):
+        f = make_field(kind, shape, seed=8, noise=0.05)
+        gh = [c.astype(np_dt) for c in f["g"]]
+        g = [to_dev(c) for c in gh] + [None] * (3 - len(gh))
+        g64 = [c.astype(np.float64) for c in gh] + [None] * (3 - len(gh))
+        m = None if f["mask"] is None else to_dev(f["mask"])
+        guess = rng.normal(size=shape).astype(np_dt)
+        if f["mask"] is not None:
+            guess[f["mask"] == 0] = 1e30
+        P, info = omni.solve_guess(g[0], g[1], g[2], m, f["d"], 0.0, 5, 20, to_dev(guess))
+        Po, io = oracle.solve_guess(g64[0], g64[1], g64[2], f["mask"], *f["d"], tol=0.0, max_outer=5, max_cg=20,
+                                    P_init=guess.astype(np.float64))
+        assert info["cg_iters_total"] == io["cg_iters_total"] == 100
+        assert rel_l2_after_mean_removal(P.cpu().numpy(), Po, ~np.isnan(Po)) <= bound
+        # raw values too: the guess fixes the additive constant (no mean removal), up to the trajectory bound
+        v = ~np.isnan(Po)
+        assert np.abs(P.cpu().numpy()[v] - Po[v]).max() <= (1e-9 if dtype == "f64" else 5e-4) * max(1.0, np.abs(Po[v]).max())
+        P0, i0 = omni.solve(g[0], g[1], g[2], m, f["d"], 0.0, 3, 10)
+        Pn, i_n = omni.solve_guess(g[0], g[1], g[2], m, f["d"], 0.0, 3, 10, None)
+        assert torch.equal(torch.nan_to_num(P0), torch.nan_to_num(Pn)) and i0 == i_n
+    tol = 1e-8 if dtype == "f64" else 1e-5
+    Pc, ic = omni.solve(g[0], g[1], g[2], m, f["d"], tol, 200000, 16)
+    assert ic["status"] == 0
+    # fp32: the returned field is the fp64 master pressure rounded to fp32, which perturbs eps_R at the 1e-6 level
+    Pr, ir = omni.solve_guess(g[0], g[1], g[2], m, f["d"], tol * (1.01 if dtype == "f64" else 3.0), 200000, 16, torch.nan_to_num(Pc))
+    assert ir["status"] == 0 and ir["outer_iters"] == 0 and ir["cg_iters_total"] == 0
+    vv = ~torch.isnan(Pc)
+    assert torch.allclose(Pr[vv], Pc[vv], rtol=0, atol=(1e-12 if dtype == "f64" else 1e-6) * float(Pc[vv].abs().max()))
