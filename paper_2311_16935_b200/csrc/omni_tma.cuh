@@ -233,6 +233,9 @@ tma_kernel(const Geom g, const ZSeg zs, const typename Op::Args a, const __grid_
                 if (k0 + 1 < k1) fwB = flag_word(c0 + g.pplane);
                 if (flag_bit(fwA, c0)) Op::load_codes(a, c0, codeA);
             }
+            // two events per trip: half of the ring / window rotation becomes register renaming (+2 % on the fp64
+            // kernels at 256^3, +0.5 % at 500^3 fp32; three per trip is slower: profiles/r1_tile_variants.md)
+#pragma unroll 2
             for (int e = 0; e < E; ++e) {
                 mbar_wait(bar_s + 8 * s, phase);
                 Op::advance(st, ctx, aF, warp, lane);
