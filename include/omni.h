@@ -256,6 +256,14 @@ long long omni_launch_count(int reset);
  * The environment variable OMNI_PERSIST_MAX_CELLS overrides the automatic threshold.  Modes 1 and 2 give bit-identical
  * results; mode 3 sums its reductions in a different (fixed) order.  Returns the previous mode; other values are ignored. */
 int omni_set_loop_mode(int mode);
+/* Convergence history (the momentum residual of Eq. 41, plotted in Fig. 10-13): registers a caller-owned
+ * DEVICE buffer of `capacity` doubles that every solve enqueued afterwards fills on the device -- entry i = eps_R =
+ * ||S - L P^i|| / ||S|| at the i-th outer residual check (i = 0: the first guess), written by the kernel that evaluates the
+ * check; info.outer_iters + 1 entries for a completed solve, the first `capacity` of them if there are more.  No host
+ * synchronisation is added.  (NULL, 0) switches it off.  Process-wide setting (like omni_set_loop_mode); a cascade solve
+ * leaves the history of its finest level.  Returns OMNI_OK, or OMNI_ERR_INVALID_ARG for capacity < 0 or NULL with
+ * capacity > 0. */
+int omni_set_history(double* d_hist, int capacity);
 /* Workspace of the non-_ws entry points comes from a library-owned stream-ordered memory pool (one per device) that
  * keeps freed blocks mapped between calls; this returns the unused memory to the driver. */
 void omni_release_memory(void);

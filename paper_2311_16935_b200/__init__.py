@@ -5,7 +5,7 @@ Importing the package does not load the library; the first call does, and fails 
 """
 from .binding import (Info, OmniError, SYMBOLS, apply_M, constants, launch_count, lib, profile_enable,  # noqa: F401
                       profile_read, release_memory, residual, set_loop_mode, solve, solve_batch2d, solve_cascade, solve_direct, source, status_string, velocity_source, version, workspace_bytes,
-                      rans_source, compressible_rans_source, solve_guess)
+                      rans_source, compressible_rans_source, solve_guess, set_history)
 
 # the C names, for callers who think in terms of include/omni.h
 omni_solve = solve
@@ -23,6 +23,7 @@ omni_constants = constants
 omni_workspace_bytes = workspace_bytes
 omni_launch_count = launch_count
 omni_set_loop_mode = set_loop_mode
+omni_set_history = set_history
 omni_release_memory = release_memory
 omni_profile_enable = profile_enable
 omni_profile_read = profile_read

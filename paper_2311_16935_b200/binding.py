@@ -20,7 +20,7 @@ SYMBOLS = ["omni_solve_f64", "omni_solve_f32", "omni_workspace_bytes", "omni_sol
            "omni_solve_host_f64", "omni_solve_host_f32", "omni_solve_batch2d_f64", "omni_solve_batch2d_f32", "omni_solve_guess_f64", "omni_solve_guess_f32", "omni_solve_direct_f64", "omni_solve_direct_f32", "omni_solve_direct_batch2d_f64", "omni_solve_direct_batch2d_f32", "omni_solve_cascade_f64", "omni_solve_cascade_f32", "omni_velocity_source_f64", "omni_velocity_source_f32", "omni_rans_source_f64", "omni_rans_source_f32",
            "omni_compressible_rans_source_f64", "omni_compressible_rans_source_f32", "omni_constants", "omni_source_f64", "omni_source_f32",
            "omni_apply_M_f64", "omni_apply_M_f32", "omni_residual_f64", "omni_residual_f32", "omni_launch_count",
-           "omni_set_loop_mode", "omni_release_memory", "omni_profile_enable", "omni_profile_read", "omni_status_string", "omni_version"]
+           "omni_set_loop_mode", "omni_set_history", "omni_release_memory", "omni_profile_enable", "omni_profile_read", "omni_status_string", "omni_version"]
 
 
 class OmniError(RuntimeError):
@@ -74,6 +74,20 @@ def set_loop_mode(mode):
     """0 = automatic (default), 1 = host-driven debug loop, 2 = CUDA-graph loop, 3 = persistent cooperative kernel
     (include/omni.h).  Returns the previous mode."""
     return int(lib().omni_set_loop_mode(C.c_int(mode)))
+
+
+def set_history(buf):
+    """omni_set_history: buf = CUDA float64 tensor that the next solves fill with eps_R of every outer residual check
+    (None switches it off).  The caller keeps the tensor alive while it is registered."""
+    if buf is None:
+        rc = lib().omni_set_history(C.c_void_p(0), C.c_int(0))
+    else:
+        import torch
+        if buf.dtype != torch.float64 or not buf.is_cuda or not buf.is_contiguous():
+            raise TypeError("history buffer must be a contiguous CUDA float64 tensor")
+        rc = lib().omni_set_history(_ptr(buf), C.c_int(buf.numel()))
+    if rc < 0:
+        raise OmniError(rc, "omni_set_history")
 
 
 def release_memory():

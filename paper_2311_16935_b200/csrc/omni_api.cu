@@ -36,6 +36,8 @@ namespace {
 
 std::atomic<long long> g_launches{0};
 std::atomic<int> g_loop_mode{0};
+std::atomic<double*> g_hist{nullptr};     // omni_set_history: device buffer for the eps_R history of the next solves
+std::atomic<int> g_hist_cap{0};
 
 // optional per-kernel timing of the host-driven loop (omni_profile_*): CUDA events around every K2/K3/K4 launch
 std::atomic<int> g_profile{0};
@@ -300,11 +302,12 @@ size_t carve(const Geom& g, char* base, Workspace<T>* w)
     return off;
 }
 
-__global__ void init_scalars_kernel(Scalars* sc, double tol, int max_outer, int max_cg)
+__global__ void init_scalars_kernel(Scalars* sc, double tol, int max_outer, int max_cg, double* hist = nullptr, int hist_cap = 0)
 {
     Scalars s;
     memset(&s, 0, sizeof(s));
     s.tol = tol; s.max_outer = max_outer; s.max_cg = max_cg;
+    s.hist = hist; s.hist_cap = hist_cap; s.hist_n = 0;
     s.inner_go = 0; s.outer_go = 1; s.status = ST_OK;
     *sc = s;
 }
@@ -774,7 +777,7 @@ int solve_ws(int nx, int ny, int nz, double dx, double dy, double dz, const T* g
     host_constants(g.naxes, dx, dy, dz, H);
     const Coef<T> K = make_coef<T>(H, dx, dy, dz, g);
 
-    init_scalars_kernel<<<1, 1, 0, st>>>(w.sc, tol, max_outer, max_cg);
+    init_scalars_kernel<<<1, 1, 0, st>>>(w.sc, tol, max_outer, max_cg, g_hist.load(), g_hist_cap.load());
     CK(cudaGetLastError());
     g_launches.fetch_add(1, std::memory_order_relaxed);
     int rc = setup_codes<T>(g, w, gx, gy, gz, mask, st);
@@ -1373,6 +1376,14 @@ int omni_debug_cta_trace(int which, unsigned long long* h_out, int n_ctas)
     return cudaMemcpyFromSymbol(h_out, omni::g_cta_trace, (size_t)n_ctas * 24, (size_t)which * 3 * 8192 * 8) == cudaSuccess ? 0 : -2;
 }
 #endif
+
+int omni_set_history(double* d_hist, int capacity)
+{
+    if (capacity < 0 || (d_hist == nullptr && capacity > 0)) return OMNI_ERR_INVALID_ARG;
+    g_hist.store(capacity > 0 ? d_hist : nullptr);
+    g_hist_cap.store(capacity > 0 ? capacity : 0);
+    return OMNI_OK;
+}
 
 void omni_release_memory(void)
 {

@@ -84,7 +84,16 @@ struct Scalars {
     int status;        // omni_status
     int max_cg, max_outer;
     unsigned int ticket[4];
+    // optional residual history (omni_set_history): eps_R (Eq. 41) of every outer residual check, entry i = check i
+    double* hist;
+    int hist_cap, hist_n;
 };
+
+__device__ __forceinline__ void record_history(Scalars* s, double epsR2)
+{
+    if (s->hist != nullptr && s->hist_n < s->hist_cap) s->hist[s->hist_n] = (s->normS2 > 0.0) ? sqrt(epsR2 / s->normS2) : 0.0;
+    s->hist_n += 1;
+}
 
 struct CondHandles {
     unsigned long long h_outer, h_inner;   // cudaGraphConditionalHandle

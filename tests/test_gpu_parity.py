@@ -683,3 +683,47 @@ def test_solve_guess_parity(oracle, dtype, forced_loop):
     assert ir["status"] == 0 and ir["outer_iters"] == 0 and ir["cg_iters_total"] == 0
     vv = ~torch.isnan(Pc)
     assert torch.allclose(Pr[vv], Pc[vv], rtol=0, atol=(1e-12 if dtype == "f64" else 1e-6) * float(Pc[vv].abs().max()))
+
+
+@pytest.mark.parametrize("loop", list(LOOPS))
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_residual_history_parity(oracle, dtype, loop):
+    """omni_set_history: eps_R (Eq. 41 :442) of every outer residual check against the oracle's history of the same run
+    (fixed caps, both loop drivers, Alg. 1 and the direct solve): outer_iters + 1 entries, each within the trajectory
+    bound relative to its value; entries beyond stay untouched; a short buffer keeps the first entries only."""
+    f = make_field("sphere3d", (18, 22, 40), seed=4, noise=0.05)
+    np_dt = np.float32 if dtype == "f32" else np.float64
+    gh = [c.astype(np_dt) for c in f["g"]]
+    g = [to_dev(c) for c in gh]
+    g64 = [c.astype(np.float64) for c in gh]
+    m = to_dev(f["mask"])
+    rel = 1e-9 if dtype == "f64" else 2e-4
+    prev = omni.set_loop_mode(LOOPS[loop])
+    try:
+        hist = torch.full((16,), -1.0, dtype=torch.float64, device="cuda")
+        omni.set_history(hist)
+        P, info = omni.solve(g[0], g[1], g[2], m, f["d"], 0.0, 6, 15)
+        h = hist.cpu().numpy()
+        _, io, ho = oracle.solve(*g64, f["mask"], *f["d"], tol=0.0, max_outer=6, max_cg=15, hist_cap=16)
+        n = info["outer_iters"] + 1
+        assert n == 7 and np.all(h[n:] == -1.0) and np.all(np.isnan(ho[n:]))
+        assert h[0] == pytest.approx(1.0, abs=1e-6)                 # P^0 = 0: r_0 = S
+        assert np.all(np.abs(h[:n] - ho[:n]) <= rel * np.maximum(ho[:n], 1e-3)), (h[:n], ho[:n])
+        assert h[n - 1] == pytest.approx(info["eps_R_final"], rel=1e-12)
+        short = torch.full((3,), -1.0, dtype=torch.float64, device="cuda")
+        omni.set_history(short)
+        omni.solve(g[0], g[1], g[2], m, f["d"], 0.0, 6, 15)
+        assert np.array_equal(short.cpu().numpy(), h[:3])
+        # the direct solve records its refinement checks the same way
+        omni.set_history(hist.fill_(-1.0))
+        Pd, idd = omni.solve_direct(g[0], g[1], g[2], m, f["d"], 0.0, 2, 40)
+        hd = hist.cpu().numpy()
+        assert np.all(hd[:3] > 0) and np.all(hd[3:] == -1.0) and hd[2] == pytest.approx(idd["eps_R_final"], rel=1e-12)
+        assert hd[1] < 1e-2 * hd[0]
+        omni.set_history(None)
+        hist.fill_(-1.0)
+        omni.solve(g[0], g[1], g[2], m, f["d"], 0.0, 2, 5)
+        assert float(hist.max()) == -1.0                           # switched off: nothing written
+    finally:
+        omni.set_history(None)
+        omni.set_loop_mode(prev)
