@@ -727,3 +727,40 @@ def test_residual_history_parity(oracle, dtype, loop):
     finally:
         omni.set_history(None)
         omni.set_loop_mode(prev)
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_disconnected_components_and_isolated_cells(oracle, dtype, forced_loop):
+    """Reading A12: P is fixed up to one constant PER connected component of the valid set.  A masked wall splits the box
+    in two, one valid cell is walled in on its own.  Both sides start from P^0 = 0 and take identical steps, so the RAW
+    values agree (no mean removal at all); the isolated cell has no link and stays 0; the direct solve returns zero mean
+    on each component separately."""
+    f = make_field("fourier3d", (14, 18, 40), seed=9, noise=0.05, kmax=3.0)
+    mask = np.ones((14, 18, 40), np.uint8)
+    mask[:, :, 19:21] = 0                       # wall normal to x: two components
+    mask[6:9, 8:11, 4:7] = 0
+    mask[7, 9, 5] = 1                           # a valid cell with six missing neighbours
+    np_dt = np.float32 if dtype == "f32" else np.float64
+    gh = [c.astype(np_dt) for c in f["g"]]
+    g = [to_dev(c) for c in gh]
+    g64 = [c.astype(np.float64) for c in gh]
+    P, info = omni.solve(g[0], g[1], g[2], to_dev(mask), f["d"], 0.0, 5, 20)
+    Po, io = oracle.solve(*g64, mask, *f["d"], tol=0.0, max_outer=5, max_cg=20)
+    Pn = P.cpu().numpy().astype(np.float64)
+    v = mask == 1
+    assert np.array_equal(np.isnan(Pn), ~v) and np.array_equal(np.isnan(Po), ~v)
+    assert Pn[7, 9, 5] == 0.0 and Po[7, 9, 5] == 0.0
+    bound = 1e-9 if dtype == "f64" else 2e-4
+    assert np.abs(Pn[v] - Po[v]).max() <= bound * np.abs(Po[v]).max()
+    left, right = v.copy(), v.copy()
+    left[:, :, 19:] = False; left[7, 9, 5] = False
+    right[:, :, :21] = False
+    for comp in (left, right):
+        assert rel_l2_after_mean_removal(Pn, Po, comp) <= bound
+    Pd, idd = omni.solve_direct(g[0], g[1], g[2], to_dev(mask), f["d"], 1e-8 if dtype == "f64" else 1e-5, 10, 3000)
+    assert idd["status"] == 0
+    Pdn = Pd.cpu().numpy().astype(np.float64)
+    scale = np.abs(Pdn[v]).max()
+    for comp in (left, right):
+        assert abs(Pdn[comp].mean()) <= (1e-9 if dtype == "f64" else 1e-4) * scale
+    assert Pdn[7, 9, 5] == 0.0
