@@ -259,11 +259,13 @@ int omni_set_loop_mode(int mode);
 /* Convergence history (the momentum residual of Eq. 41, plotted in Fig. 10-13): registers a caller-owned
  * DEVICE buffer of `capacity` doubles that every solve enqueued afterwards fills on the device -- entry i = eps_R =
  * ||S - L P^i|| / ||S|| at the i-th outer residual check (i = 0: the first guess), written by the kernel that evaluates the
- * check; info.outer_iters + 1 entries for a completed solve, the first `capacity` of them if there are more.  No host
- * synchronisation is added.  (NULL, 0) switches it off.  Process-wide setting (like omni_set_loop_mode); a cascade solve
- * leaves the history of its finest level.  Returns OMNI_OK, or OMNI_ERR_INVALID_ARG for capacity < 0 or NULL with
- * capacity > 0. */
-int omni_set_history(double* d_hist, int capacity);
+ * check; info.outer_iters + 1 entries for a completed solve, the first `capacity` of them if there are more.  d_cg_iters
+ * (device, `capacity` ints, may be NULL) receives next to it the CG iterations of the outer iteration that led to the
+ * check (0 for i = 0) -- the quantity behind the falling cost per iteration of Fig. 13 (:489).  No host
+ * synchronisation is added.  (NULL, NULL, 0) switches it off.  Process-wide setting (like omni_set_loop_mode); a cascade solve
+ * leaves the history of its finest level.  Returns OMNI_OK, or OMNI_ERR_INVALID_ARG for capacity < 0 or a NULL d_hist
+ * with capacity > 0 or with d_cg_iters given. */
+int omni_set_history(double* d_hist, int* d_cg_iters, int capacity);
 /* Workspace of the non-_ws entry points comes from a library-owned stream-ordered memory pool (one per device) that
  * keeps freed blocks mapped between calls; this returns the unused memory to the driver. */
 void omni_release_memory(void);

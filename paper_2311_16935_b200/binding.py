@@ -76,16 +76,20 @@ def set_loop_mode(mode):
     return int(lib().omni_set_loop_mode(C.c_int(mode)))
 
 
-def set_history(buf):
-    """omni_set_history: buf = CUDA float64 tensor that the next solves fill with eps_R of every outer residual check
-    (None switches it off).  The caller keeps the tensor alive while it is registered."""
+def set_history(buf, cg_iters=None):
+    """omni_set_history: buf = CUDA float64 tensor that the next solves fill with eps_R of every outer residual check,
+    cg_iters = optional CUDA int32 tensor of the same length for the CG iterations per outer iteration (None switches it
+    off).  The caller keeps the tensors alive while they are registered."""
     if buf is None:
-        rc = lib().omni_set_history(C.c_void_p(0), C.c_int(0))
+        rc = lib().omni_set_history(C.c_void_p(0), C.c_void_p(0), C.c_int(0))
     else:
         import torch
         if buf.dtype != torch.float64 or not buf.is_cuda or not buf.is_contiguous():
             raise TypeError("history buffer must be a contiguous CUDA float64 tensor")
-        rc = lib().omni_set_history(_ptr(buf), C.c_int(buf.numel()))
+        if cg_iters is not None and (cg_iters.dtype != torch.int32 or not cg_iters.is_cuda or not cg_iters.is_contiguous()
+                                     or cg_iters.numel() != buf.numel()):
+            raise TypeError("cg_iters must be a contiguous CUDA int32 tensor as long as the history buffer")
+        rc = lib().omni_set_history(_ptr(buf), _ptr(cg_iters), C.c_int(buf.numel()))
     if rc < 0:
         raise OmniError(rc, "omni_set_history")
 

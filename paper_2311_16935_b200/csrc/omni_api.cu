@@ -38,6 +38,7 @@ std::atomic<long long> g_launches{0};
 std::atomic<int> g_loop_mode{0};
 std::atomic<double*> g_hist{nullptr};     // omni_set_history: device buffer for the eps_R history of the next solves
 std::atomic<int> g_hist_cap{0};
+std::atomic<int*> g_hist_k{nullptr};
 
 // optional per-kernel timing of the host-driven loop (omni_profile_*): CUDA events around every K2/K3/K4 launch
 std::atomic<int> g_profile{0};
@@ -302,12 +303,13 @@ size_t carve(const Geom& g, char* base, Workspace<T>* w)
     return off;
 }
 
-__global__ void init_scalars_kernel(Scalars* sc, double tol, int max_outer, int max_cg, double* hist = nullptr, int hist_cap = 0)
+__global__ void init_scalars_kernel(Scalars* sc, double tol, int max_outer, int max_cg, double* hist = nullptr, int hist_cap = 0,
+                                    int* hist_k = nullptr)
 {
     Scalars s;
     memset(&s, 0, sizeof(s));
     s.tol = tol; s.max_outer = max_outer; s.max_cg = max_cg;
-    s.hist = hist; s.hist_cap = hist_cap; s.hist_n = 0;
+    s.hist = hist; s.hist_k = hist_k; s.hist_cap = hist_cap; s.hist_n = 0;
     s.inner_go = 0; s.outer_go = 1; s.status = ST_OK;
     *sc = s;
 }
@@ -777,7 +779,7 @@ int solve_ws(int nx, int ny, int nz, double dx, double dy, double dz, const T* g
     host_constants(g.naxes, dx, dy, dz, H);
     const Coef<T> K = make_coef<T>(H, dx, dy, dz, g);
 
-    init_scalars_kernel<<<1, 1, 0, st>>>(w.sc, tol, max_outer, max_cg, g_hist.load(), g_hist_cap.load());
+    init_scalars_kernel<<<1, 1, 0, st>>>(w.sc, tol, max_outer, max_cg, g_hist.load(), g_hist_cap.load(), g_hist_k.load());
     CK(cudaGetLastError());
     g_launches.fetch_add(1, std::memory_order_relaxed);
     int rc = setup_codes<T>(g, w, gx, gy, gz, mask, st);
@@ -1377,10 +1379,11 @@ int omni_debug_cta_trace(int which, unsigned long long* h_out, int n_ctas)
 }
 #endif
 
-int omni_set_history(double* d_hist, int capacity)
+int omni_set_history(double* d_hist, int* d_cg_iters, int capacity)
 {
-    if (capacity < 0 || (d_hist == nullptr && capacity > 0)) return OMNI_ERR_INVALID_ARG;
+    if (capacity < 0 || (d_hist == nullptr && (capacity > 0 || d_cg_iters != nullptr))) return OMNI_ERR_INVALID_ARG;
     g_hist.store(capacity > 0 ? d_hist : nullptr);
+    g_hist_k.store(capacity > 0 ? d_cg_iters : nullptr);
     g_hist_cap.store(capacity > 0 ? capacity : 0);
     return OMNI_OK;
 }

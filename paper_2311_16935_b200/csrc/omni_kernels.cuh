@@ -85,13 +85,18 @@ struct Scalars {
     int max_cg, max_outer;
     unsigned int ticket[4];
     // optional residual history (omni_set_history): eps_R (Eq. 41) of every outer residual check, entry i = check i
+    // and, optionally, the CG iterations the outer iteration before the check took (0 for the first check)
     double* hist;
+    int* hist_k;
     int hist_cap, hist_n;
 };
 
-__device__ __forceinline__ void record_history(Scalars* s, double epsR2)
+__device__ __forceinline__ void record_history(Scalars* s, double epsR2, int k_prev)
 {
-    if (s->hist != nullptr && s->hist_n < s->hist_cap) s->hist[s->hist_n] = (s->normS2 > 0.0) ? sqrt(epsR2 / s->normS2) : 0.0;
+    if (s->hist != nullptr && s->hist_n < s->hist_cap) {
+        s->hist[s->hist_n] = (s->normS2 > 0.0) ? sqrt(epsR2 / s->normS2) : 0.0;
+        if (s->hist_k != nullptr) s->hist_k[s->hist_n] = k_prev;
+    }
     s->hist_n += 1;
 }
 

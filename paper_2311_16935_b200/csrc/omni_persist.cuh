@@ -298,7 +298,7 @@ persist_kernel(const Geom g, const PersistArgs<T> a)
             double tot[2];
             if (!grid_allreduce<2, NT>(gs, a.slots, acc, tot)) { status = ST_BARRIER_TIMEOUT; break; }
             epsR2 = tot[0];
-            if (blockIdx.x == 0 && threadIdx.x == 0) record_history(sc, tot[0]);
+            if (blockIdx.x == 0 && threadIdx.x == 0) record_history(sc, tot[0], k);
             if (!isfinite(tot[0])) { status = ST_BREAKDOWN; break; }
             if (tot[0] <= tol2S || n >= max_outer) { status = (tot[0] <= tol2S) ? ST_OK : ST_NOT_CONVERGED; break; }
             n += 1;

@@ -702,7 +702,7 @@ struct OpT2 {
         Scalars* s = a.sc;
         s->epsR2 = tot[0];
         if (!a.fold_delta) return;
-        record_history(s, tot[0]);
+        record_history(s, tot[0], s->k);
         if (!isfinite(tot[0])) {
             s->status = ST_BREAKDOWN; s->inner_go = 0; s->outer_go = 0;
             set_cond(a.cond, 0, 0);

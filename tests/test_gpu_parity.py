@@ -701,9 +701,11 @@ def test_residual_history_parity(oracle, dtype, loop):
     prev = omni.set_loop_mode(LOOPS[loop])
     try:
         hist = torch.full((16,), -1.0, dtype=torch.float64, device="cuda")
-        omni.set_history(hist)
+        its = torch.full((16,), -1, dtype=torch.int32, device="cuda")
+        omni.set_history(hist, its)
         P, info = omni.solve(g[0], g[1], g[2], m, f["d"], 0.0, 6, 15)
         h = hist.cpu().numpy()
+        assert its.cpu().tolist() == [0] + [15] * 6 + [-1] * 9           # CG iterations per outer iteration (fixed caps)
         _, io, ho = oracle.solve(*g64, f["mask"], *f["d"], tol=0.0, max_outer=6, max_cg=15, hist_cap=16)
         n = info["outer_iters"] + 1
         assert n == 7 and np.all(h[n:] == -1.0) and np.all(np.isnan(ho[n:]))
