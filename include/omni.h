@@ -276,7 +276,7 @@ void omni_release_memory(void);
 int omni_profile_enable(int on);          /* returns the previous setting */
 void omni_profile_read(double* h_ms3, long long* h_count3, int reset);
 const char* omni_status_string(int status);
-int omni_version(void);
+int omni_version(void);                  /* 100 * major + minor; 101 added the _guess, _rans_source and history entry points */
 
 #ifdef __cplusplus
 }

@@ -1415,6 +1415,6 @@ const char* omni_status_string(int status)
     }
 }
 
-int omni_version(void) { return 100; }
+int omni_version(void) { return 101; }   // 101: omni_solve_guess_*, omni_set_history, omni_rans_source_*, omni_compressible_rans_source_*
 
 }  // extern "C"
