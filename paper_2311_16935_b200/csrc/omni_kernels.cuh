@@ -212,12 +212,13 @@ __device__ __forceinline__ void xfix_zero_after(T (&q)[V])
 // face class of position i on an axis of length n: 0, 1 (cells 0, 1), 2, 3 (cells n-2, n-1), -1 otherwise / axis off
 __device__ __forceinline__ int face_class(int i, int n, int on)
 {
-    if (!on) return -1;
-    if (i == 0) return 0;
-    if (i == 1) return 1;
-    if (i == n - 2) return 2;
-    if (i == n - 1) return 3;
-    return -1;
+    // selects, not branches: evaluated per emitted plane in the tile kernels
+    int c = -1;
+    c = (i == n - 1) ? 3 : c;
+    c = (i == n - 2) ? 2 : c;
+    c = (i == 1) ? 1 : c;
+    c = (i == 0) ? 0 : c;
+    return on ? c : -1;
 }
 
 // whole-chunk correction for a row (y class) or plane (z class) next to a box face: uniform over the warp
