@@ -148,8 +148,11 @@ int omni_solve_direct_batch2d_f32(int nx, int ny, int nb, double dx, double dy, 
  * nb independent 2D gradient fields [nb][ny][nx] on ONE mask [ny][nx] (NULL = all valid) are stacked and solved as one
  * block-diagonal system with the 2D scheme: stencil codes are built once, every stencil sweep serves all snapshots,
  * and the tile pipeline marches through the snapshots like through the planes of a volume.  The CG scalars and eps_R
- * (Eq. 41) are those of the stacked system: on return EVERY snapshot satisfies Eq. 12 to the joint tolerance, and each
- * converged P_b equals the single-snapshot result within tol.  d_P_init [nb][ny][nx] (may be NULL = zeros) is the
+ * (Eq. 41) are those of the stacked system: on return ||r|| <= tol ||S|| holds for the STACK, which bounds every
+ * snapshot's own residual by ||r_b|| <= tol ||S||, i.e. eps_R,b <= tol ||S|| / ||S_b|| -- about tol sqrt(nb) for
+ * snapshots of similar strength, but a snapshot whose source is much weaker than the others' can sit above tol by that
+ * ratio (solve such a series one by one, or tighten tol).  Each converged P_b equals the single-snapshot result to
+ * that accuracy.  d_P_init [nb][ny][nx] (may be NULL = zeros) is the
  * first guess P^0, e.g. the previous time step's pressure ("zero ... or any other arbitrary value");
  * its values at missing cells are ignored.  Everything else as omni_solve_*. */
 int omni_solve_batch2d_f64(int nx, int ny, int nb, double dx, double dy, const double* d_gx, const double* d_gy,

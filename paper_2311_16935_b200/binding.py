@@ -156,6 +156,21 @@ def _check(ts, device_type):
             raise ValueError(f"tensor on {t.device}, expected {device_type}")
 
 
+def _check_like(ref, fields, mask=None, mask_shape=None, what="gx"):
+    """Every field tensor must match `ref` in shape and dtype (the C entry points take one nx, ny, nz and one element
+    type for all of them); the mask is uint8 with the grid's shape (`mask_shape` for the batched entry points)."""
+    import torch
+    for name, t in fields:
+        if t is None:
+            continue
+        if t.dtype != ref.dtype or tuple(t.shape) != tuple(ref.shape):
+            raise TypeError(f"{name}: shape {tuple(t.shape)} / {t.dtype} does not match {what} {tuple(ref.shape)} / {ref.dtype}")
+    if mask is not None:
+        want = tuple(ref.shape) if mask_shape is None else tuple(mask_shape)
+        if mask.dtype != torch.uint8 or tuple(mask.shape) != want:
+            raise TypeError(f"mask must be uint8 with shape {want}, got {mask.dtype} {tuple(mask.shape)}")
+
+
 def _stream(dev):
     import torch
     if not torch.cuda.is_available():
@@ -178,8 +193,9 @@ def solve(gx, gy, gz, mask, d, tol, max_outer, max_cg, out=None, workspace=None,
     sfx = _suffix(gx)
     host = gx.device.type == "cpu"
     _check([gx, gy, gz, mask, out], "cpu" if host else "cuda")
-    if mask is not None and mask.dtype != torch.uint8:
-        raise TypeError("mask must be uint8")
+    _check_like(gx, [("gy", gy), ("gz", gz), ("out", out)], mask)
+    if workspace is not None and (not workspace.is_cuda or not workspace.is_contiguous() or workspace.data_ptr() % 256):
+        raise ValueError("workspace must be a contiguous CUDA tensor aligned to 256 bytes")
     P = out if out is not None else torch.empty_like(gx)
     info = Info()
     geom = _geom(gx, d)
@@ -216,10 +232,7 @@ def solve_direct(gx, gy, gz, mask, d, tol, max_outer, max_cg, out=None, P_init=N
     import torch
     sfx = _suffix(gx)
     _check([gx, gy, gz, mask, out, P_init], "cuda")
-    if mask is not None and mask.dtype != torch.uint8:
-        raise TypeError("mask must be uint8")
-    if P_init is not None and (P_init.dtype != gx.dtype or P_init.shape != gx.shape):
-        raise TypeError("P_init must match gx in dtype and shape")
+    _check_like(gx, [("gy", gy), ("gz", gz), ("out", out), ("P_init", P_init)], mask)
     P = out if out is not None else torch.empty_like(gx)
     info = Info()
     with torch.cuda.device(gx.device):
@@ -239,8 +252,7 @@ def velocity_source(u, v, w, mask, d, rho=1.0, mu=0.0, dudt=None):
     acc = list(dudt) if dudt is not None else [None, None, None]
     acc += [None] * (3 - len(acc))
     _check([u, v, w, mask] + acc, "cuda")
-    if mask is not None and mask.dtype != torch.uint8:
-        raise TypeError("mask must be uint8")
+    _check_like(u, [("v", v), ("w", w)] + [("dudt", t) for t in acc], mask, what="u")
     g = [torch.empty_like(u), torch.empty_like(u), None if w is None else torch.empty_like(u)]
     with torch.cuda.device(u.device):
         fn = getattr(lib(), f"omni_velocity_source_{sfx}")
@@ -266,8 +278,7 @@ def rans_source(u, v, w, stress, mask, d, rho=1.0):
     import torch
     sfx = _suffix(u)
     _check([u, v, w, mask] + (list(stress) if stress is not None else []), "cuda")
-    if mask is not None and mask.dtype != torch.uint8:
-        raise TypeError("mask must be uint8")
+    _check_like(u, [("v", v), ("w", w)] + [("stress", t) for t in (stress or [])], mask, what="u")
     g = [torch.empty_like(u), torch.empty_like(u), None if w is None else torch.empty_like(u)]
     arr = _stress_array(stress, 2 if w is None else 3)
     with torch.cuda.device(u.device):
@@ -283,8 +294,7 @@ def compressible_rans_source(u, v, w, stress, mask, d, gamma=1.4, mach_inf=2.0, 
     import torch
     sfx = _suffix(u)
     _check([u, v, w, mask] + (list(stress) if stress is not None else []), "cuda")
-    if mask is not None and mask.dtype != torch.uint8:
-        raise TypeError("mask must be uint8")
+    _check_like(u, [("v", v), ("w", w)] + [("stress", t) for t in (stress or [])], mask, what="u")
     g = [torch.empty_like(u), torch.empty_like(u), None if w is None else torch.empty_like(u)]
     arr = _stress_array(stress, 2 if w is None else 3)
     with torch.cuda.device(u.device):
@@ -301,8 +311,7 @@ def solve_cascade(gx, gy, gz, mask, d, tol, max_outer, max_cg, levels=3, out=Non
     import torch
     sfx = _suffix(gx)
     _check([gx, gy, gz, mask, out], "cuda")
-    if mask is not None and mask.dtype != torch.uint8:
-        raise TypeError("mask must be uint8")
+    _check_like(gx, [("gy", gy), ("gz", gz), ("out", out)], mask)
     P = out if out is not None else torch.empty_like(gx)
     info = Info()
     with torch.cuda.device(gx.device):
@@ -323,6 +332,7 @@ def solve_batch2d(gx, gy, mask2d, d, tol, max_outer, max_cg, P_init=None, out=No
     if gx.dim() != 3:
         raise ValueError("expected (nb, ny, nx) tensors")
     nb, ny, nx = gx.shape
+    _check_like(gx, [("gy", gy), ("P_init", P_init), ("out", out)], mask2d, mask_shape=(ny, nx))
     P = out if out is not None else torch.empty_like(gx)
     info = Info()
     with torch.cuda.device(gx.device):
@@ -340,6 +350,7 @@ def source(gx, gy, gz, mask, d):
     import torch
     sfx = _suffix(gx)
     _check([gx, gy, gz, mask], "cuda")
+    _check_like(gx, [("gy", gy), ("gz", gz)], mask)
     S = torch.empty_like(gx)
     nrm = C.c_double(0.0)
     with torch.cuda.device(gx.device):
@@ -354,6 +365,7 @@ def apply_M(p, mask, d):
     """q = M p (omni_apply_M_*).  Returns (q, p.Mp)."""
     sfx = _suffix(p)
     _check([p, mask], "cuda")
+    _check_like(p, [], mask, what="p")
     import torch
     q = torch.empty_like(p)
     pq = C.c_double(0.0)
@@ -370,8 +382,9 @@ def residual(gx, gy, gz, mask, P, d):
     import torch
     sfx = _suffix(gx)
     _check([gx, gy, gz, mask, P], "cuda")
-    if P.dtype != torch.float64:
-        raise TypeError("P must be fp64")
+    _check_like(gx, [("gy", gy), ("gz", gz)], mask)
+    if P.dtype != torch.float64 or tuple(P.shape) != tuple(gx.shape):
+        raise TypeError("P must be fp64 with the shape of gx")
     r = torch.empty_like(gx)
     eps = C.c_double(0.0)
     with torch.cuda.device(gx.device):

@@ -102,7 +102,7 @@ void park_graph(cudaGraphExec_t exec, cudaStream_t st)
 cudaMemPool_t device_pool()
 {
     int dev = 0;
-    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) return nullptr;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) { cudaGetLastError(); return nullptr; }
     std::lock_guard<std::mutex> lk(g_pool_mu);
     if (!g_pools[dev]) {
         cudaMemPoolProps props = {};
@@ -125,6 +125,27 @@ cudaError_t pool_alloc(P** ptr, size_t bytes, cudaStream_t st)
     cudaMemPool_t pool = device_pool();
     if (!pool) return cudaMallocAsync((void**)ptr, bytes, st);
     return cudaMallocFromPoolAsync((void**)ptr, bytes, pool, st);
+}
+
+// Per-device facts, looked up once per device (the library serves any device of the process: pools, occupancy and
+// kernel attributes are all per device).
+constexpr int MAX_DEVICES = 64;
+struct DevInfo { int dev, sms, coop; };
+DevInfo device_info()
+{
+    static std::mutex mu;
+    static DevInfo cache[MAX_DEVICES];
+    static bool have[MAX_DEVICES] = {};
+    DevInfo d{ 0, 148, 0 };
+    if (cudaGetDevice(&d.dev) != cudaSuccess) { cudaGetLastError(); d.dev = 0; return d; }
+    const bool cached = d.dev >= 0 && d.dev < MAX_DEVICES;
+    std::lock_guard<std::mutex> lk(mu);
+    if (cached && have[d.dev]) return cache[d.dev];
+    if (cudaDeviceGetAttribute(&d.sms, cudaDevAttrMultiProcessorCount, d.dev) != cudaSuccess || d.sms < 1) d.sms = 148;
+    if (cudaDeviceGetAttribute(&d.coop, cudaDevAttrCooperativeLaunch, d.dev) != cudaSuccess) d.coop = 0;
+    cudaGetLastError();
+    if (cached) { cache[d.dev] = d; have[d.dev] = true; }
+    return d;
 }
 
 // ------------------------------------------------------------------------------------------------ a0 constants
@@ -266,8 +287,12 @@ struct Workspace {
 
 size_t partial_slots(const Geom& g)
 {
-    // 1D kernels: ceil(npad / 256) blocks; march kernels never exceed that
-    return (size_t)((g.npad + 255) / 256) * 2 + 64;
+    // one fp64 slot per CTA and accumulator.  1D kernels: at most ceil(npad / 256) blocks.  Tile kernels: NACC x
+    // (x tiles) x (y tiles) x (z segments) with at most nz segments; the finest tiling is K2's (64 cells x 8 rows,
+    // NACC = 2).  A thin cross-section with a long z axis has far more tile CTAs than npad / 256 (launch_tma checks).
+    const size_t lin = (size_t)((g.npad + 255) / 256) * 2 + 64;
+    const size_t tile = (size_t)2 * (size_t)((g.px + 63) / 64) * (size_t)((g.ny + OMNI_BY - 1) / OMNI_BY) * (size_t)g.nz + 64;
+    return std::max(lin, tile);
 }
 
 template <typename T>
@@ -311,6 +336,7 @@ __global__ void init_scalars_kernel(Scalars* sc, double tol, int max_outer, int 
     s.tol = tol; s.max_outer = max_outer; s.max_cg = max_cg;
     s.hist = hist; s.hist_k = hist_k; s.hist_cap = hist_cap; s.hist_n = 0;
     s.inner_go = 0; s.outer_go = 1; s.status = ST_OK;
+    s.dzero = 1;                     // no CG iteration has run yet: the first K2 takes delta as zero
     *sc = s;
 }
 
@@ -331,17 +357,24 @@ MarchCfg tma_config(const Geom& g)
 {
     using TG = typename Op::TG;
     constexpr int SMEM = Op::SMEM_BYTES + 128;
-    static int slots_cache = 0;
-    if (slots_cache == 0) {
-        int dev = 0, sms = 148, occ = 1;
-        cudaGetDevice(&dev);
-        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-        cudaFuncSetAttribute(tma_kernel<Op>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM);
-        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, tma_kernel<Op>, TG::NTHR, SMEM);
-        if (occ < 1) occ = 1;
-        slots_cache = sms * occ;
+    // CTA slots of the current device (SMs x resident CTAs); the shared-memory opt-in is a per-device attribute too
+    static std::mutex mu;
+    static int slots_cache[MAX_DEVICES] = {};
+    const DevInfo di = device_info();
+    int slots = 0;
+    {
+        std::lock_guard<std::mutex> lk(mu);
+        const bool cached = di.dev >= 0 && di.dev < MAX_DEVICES;
+        if (cached) slots = slots_cache[di.dev];
+        if (slots == 0) {
+            int occ = 1;
+            cudaFuncSetAttribute(tma_kernel<Op>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM);
+            cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, tma_kernel<Op>, TG::NTHR, SMEM);
+            if (occ < 1) occ = 1;
+            slots = di.sms * occ;
+            if (cached) slots_cache[di.dev] = slots;
+        }
     }
-    const int slots = slots_cache;
     const int ntx = (g.px + TG::BX - 1) / TG::BX, nty = (g.ny + TG::BY - 1) / TG::BY;
     const long long tiles = (long long)ntx * nty;
     int best = 1;
@@ -398,6 +431,8 @@ template <class Op>
 cudaError_t launch_tma(const Geom& g, const typename Op::Args& a, const TmaSet& maps, cudaStream_t st)
 {
     const MarchCfg c = tma_config<Op>(g);
+    // every CTA owns Op::NACC slots of the partial buffer (carve / partial_slots)
+    if ((size_t)Op::NACC * c.grid.x * c.grid.y * c.grid.z > partial_slots(g)) return cudaErrorInvalidConfiguration;
     tma_kernel<Op><<<c.grid, c.block, Op::SMEM_BYTES + 128, st>>>(g, c.zs, a, maps);
     g_launches.fetch_add(1, std::memory_order_relaxed);
     return cudaGetLastError();
@@ -454,12 +489,7 @@ int setup_codes(const Geom& g, const Workspace<T>& w, const T* gx, const T* gy, 
     codes_kernel<<<blocks_for(g.npad / 4, 256), 256, 0, st>>>(g, vbyte, w.link, w.wcode, w.flags, worklist, work_count);
     CK(cudaGetLastError());
     {
-        static int nsm = 0;
-        if (nsm == 0) {
-            int dev = 0;
-            cudaGetDevice(&dev);
-            if (cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || nsm < 1) nsm = 148;
-        }
+        const int nsm = device_info().sms;
         long long nb = (g.npad / 4 + 127) / 128;
         if (nb > 16LL * nsm) nb = 16LL * nsm;
         if (nb < 1) nb = 1;
@@ -535,12 +565,7 @@ bool make_tma_set(const Geom& g, const Workspace<T>& w, TmaSet& m)
 template <typename T>
 cudaError_t launch_flush(const Geom& g, const Workspace<T>& w, cudaStream_t st)
 {
-    static int nsm = 0;
-    if (nsm == 0) {
-        int dev = 0;
-        cudaGetDevice(&dev);
-        if (cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || nsm < 1) nsm = 148;
-    }
+    const int nsm = device_info().sms;
     constexpr int V = 16 / (int)sizeof(T);
     long long nb = (g.npad / V + 255) / 256;
     if (nb > 8LL * nsm) nb = 8LL * nsm;
@@ -692,6 +717,19 @@ int run_loop_graph(const Geom& g, const Workspace<T>& w, const HostConst& H, con
     return rc;
 }
 
+// longest wait at a grid barrier of the persistent loop: 30 s by default (a healthy grid that is merely descheduled
+// on a time-shared GPU must not be reported as an error), OMNI_BARRIER_TIMEOUT_S overrides
+unsigned long long barrier_timeout_ns()
+{
+    static unsigned long long v = 0;
+    if (v == 0) {
+        const char* e = getenv("OMNI_BARRIER_TIMEOUT_S");
+        const double s = e ? atof(e) : 30.0;
+        v = (unsigned long long)((s > 0.001 ? s : 30.0) * 1e9);
+    }
+    return v;
+}
+
 // Persistent loop: the whole iteration in one cooperative launch (omni_persist.cuh).  Returns -100 if the device cannot
 // co-schedule the grid (the caller then falls back to the graph loop).  NT = threads per CTA: 512 (up to 128 registers)
 // for the smallest grids, where one row segment per warp is all there is; 1024 where a warp has several segments and
@@ -709,6 +747,7 @@ int launch_persist(const Geom& g, const Workspace<T>& w, const HostConst& H, con
     a.link = w.link; a.wcode = w.wcode; a.flags = w.flags; a.K = K;
     for (int i = 0; i < 3; ++i) a.t[i] = H.F[i] / H.Atot;
     a.sc = w.sc; a.slots = w.slots;
+    a.timeout_ns = barrier_timeout_ns();
     // one warp per 64-cell row segment of K2 (the finest phase), at most one CTA per SM, at most PERSIST_MAX_CTAS slots
     const long long tasks = (long long)g.ny * g.nz * ((g.nx + 63) / 64);
     const int nw = NT / 32;
@@ -719,7 +758,12 @@ int launch_persist(const Geom& g, const Workspace<T>& w, const HostConst& H, con
     CK(cudaMemsetAsync(w.slots, 0, (size_t)8 * G * sizeof(double), st));
     Geom gg = g;
     void* params[2] = { (void*)&gg, (void*)&a };
-    CK(cudaLaunchCooperativeKernel((const void*)persist_kernel<T, NT, LOP>, dim3((unsigned)G), dim3(NT), params, 0, st));
+    // a grid the context cannot co-schedule (fewer usable SMs than the device reports: MPS, green contexts) is not an
+    // error of the solve: report "cannot" and let the caller take the graph loop
+    if (cudaLaunchCooperativeKernel((const void*)persist_kernel<T, NT, LOP>, dim3((unsigned)G), dim3(NT), params, 0, st) != cudaSuccess) {
+        cudaGetLastError();
+        return -100;
+    }
     g_launches.fetch_add(1, std::memory_order_relaxed);
     return OMNI_OK;
 }
@@ -727,13 +771,8 @@ int launch_persist(const Geom& g, const Workspace<T>& w, const HostConst& H, con
 template <typename T, bool LOP>
 int run_loop_persist(const Geom& g, const Workspace<T>& w, const HostConst& H, const Coef<T>& K, cudaStream_t st)
 {
-    static int nsm = 0, coop = 0;
-    if (nsm == 0) {
-        int dev = 0;
-        if (cudaGetDevice(&dev) != cudaSuccess) return OMNI_ERR_CUDA;
-        cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev);
-        cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
-    }
+    const DevInfo di = device_info();
+    const int nsm = di.sms, coop = di.coop;
     if (!coop || nsm < 1) return -100;
     if ((long long)g.ny * g.nz * ((g.nx + 63) / 64) >= (1LL << 31)) return -100;      // 32-bit task indices
     return (g.npad <= OMNI_PERSIST_SMALL_CELLS) ? launch_persist<T, 512, LOP>(g, w, H, K, nsm, st)

@@ -81,6 +81,8 @@ struct Scalars {
     int n;             // outer iterations done
     int inner_go, outer_go;
     int pend;          // 1: delta still lacks alpha_prev * p of the last (even) CG iteration
+    int dzero;         // 1: delta counts as zero in the next K2 (no CG iteration has run since the last fold: the first
+                       //    outer check, or an outer iteration whose inner loop did not start) -- K2 must not fold a stale delta
     int status;        // omni_status
     int max_cg, max_outer;
     unsigned int ticket[4];

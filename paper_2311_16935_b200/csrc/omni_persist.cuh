@@ -18,12 +18,13 @@ struct PersistArgs {
     const uint8_t* link; const uint32_t* wcode; const uint32_t* flags;
     Coef<T> K; double t[3];
     Scalars* sc; double* slots;             // slots[2][2][2][gridDim.x]: [region][set][accumulator][CTA], tagged values; zero at launch
+    unsigned long long timeout_ns;          // longest wait at a grid barrier before the kernel gives up (status OMNI_ERR_CUDA)
 };
 
 
 constexpr int PERSIST_MAX_CTAS = 1024;
 constexpr size_t PERSIST_SLOT_BYTES = (size_t)2 * 2 * 2 * PERSIST_MAX_CTAS * 8;
-constexpr int ST_BARRIER_TIMEOUT = -2;      // = OMNI_ERR_CUDA: a CTA waited > 4 s at a grid barrier
+constexpr int ST_BARRIER_TIMEOUT = -2;      // = OMNI_ERR_CUDA: a CTA waited longer than PersistArgs::timeout_ns at a grid barrier
 
 #ifndef OMNI_PERSIST_LDCG
 #define OMNI_PERSIST_LDCG 0
@@ -64,7 +65,8 @@ __device__ __forceinline__ unsigned long long global_timer_ns()
 // (a CTA can be at most one barrier ahead of the slowest reader), each set flips its tag on every use.
 // Release: the publishing lane's st.release follows the CTA-wide barrier that follows the phase's stores (cumulative);
 // acquire: warp 0's ld.acquire precede the CTA-wide barrier that releases the other warps to their loads.
-// Returns false if a slot did not arrive within 4 s (a CTA is not resident or died): every CTA then leaves the kernel.
+// Returns false if a slot did not arrive within gs.timeout_ns (a CTA is not resident or died): every CTA then leaves
+// the kernel.
 struct GridSync {
     // Two slot regions with their own use counts: [0] the CG barriers (K3, K4: one accumulator), [1] the outer barrier
     // (K2: two accumulators) -- a slot's tag must flip on each of ITS uses, so barriers that publish different numbers
@@ -73,6 +75,7 @@ struct GridSync {
     unsigned int count[2];
     double* red;                     // shared: [2][NW + 1]
     int* flag;                       // shared
+    unsigned long long timeout_ns;
 };
 
 __device__ __forceinline__ void slot_publish(double* slot, double v, unsigned int tag)
@@ -129,7 +132,7 @@ __device__ __forceinline__ bool grid_allreduce(GridSync& gs, double* slots, cons
                         const double* sl = my + (size_t)i * G + b0 + 32 * u;
                         const unsigned long long t0 = global_timer_ns();
                         while (!slot_poll(sl, tag, v[u])) {
-                            if (global_timer_ns() - t0 > 4000000000ULL) { ok = 0; break; }
+                            if (global_timer_ns() - t0 > gs.timeout_ns) { ok = 0; break; }
                         }
                     }
                     s += v[u];                                     // fixed order: b0, b0 + 32, ...
@@ -207,7 +210,7 @@ persist_kernel(const Geom g, const PersistArgs<T> a)
     const bool three = g.naxes == 3;
     const long long pp = g.pplane;
 
-    GridSync gs{ { 2u, 2u }, red, &flag };
+    GridSync gs{ { 2u, 2u }, red, &flag, a.timeout_ns };
 
     // loop state, identical in every thread of the grid
     const double thresh2 = sc->thresh2, tol2S = sc->tol2S;
@@ -215,6 +218,7 @@ persist_kernel(const Geom g, const PersistArgs<T> a)
     int n = sc->n, k = 0, status = ST_OK;
     long long cg_total = 0;
     double rho = 0.0, beta = 0.0, alpha = 0.0, gamma = 0.0, epsR2 = 0.0;
+    bool dzero = sc->dzero != 0;                 // delta counts as zero in the next K2 (Scalars::dzero)
 
     for (;;) {
         // ------------------------------------------------------------------------------ K2: P += delta, r = S - L P
@@ -228,14 +232,14 @@ persist_kernel(const Geom g, const PersistArgs<T> a)
                 auto val = [&](long long i, bool ok, double (&v)[2]) {
                     v[0] = v[1] = 0.0;
                     if (ok) {
-                        double P[2]; T d[2];
+                        double P[2]; T d[2] = { T(0), T(0) };
                         ldcg_chunk<double, 2>(Pin + i, P);
-                        ldcg_chunk<T, 2>(a.delta + i, d);
+                        if (!dzero) ldcg_chunk<T, 2>(a.delta + i, d);
                         v[0] = P[0] + (double)d[0];
                         v[1] = P[1] + (double)d[1];
                     }
                 };
-                auto val1 = [&](long long i) { return ldd(Pin + i) + (double)ldd(a.delta + i); };
+                auto val1 = [&](long long i) { return ldd(Pin + i) + (dzero ? 0.0 : (double)ldd(a.delta + i)); };
                 // every load of the task is issued before the first use
                 uint32_t fw = 0, lkb = 0;
                 T S[2] = { T(0), T(0) };
@@ -305,7 +309,9 @@ persist_kernel(const Geom g, const PersistArgs<T> a)
             k = 0;
             beta = 0.0;
             rho = tot[1];
-            if (!((tot[1] > thresh2) && (tot[1] != 0.0) && (max_cg > 0))) continue;
+            // an inner loop that does not start leaves the old delta behind: the next K2 must not fold it again
+            dzero = !((tot[1] > thresh2) && (tot[1] != 0.0) && (max_cg > 0));
+            if (dzero) continue;
         }
         // ------------------------------------------------------------------------------ inner CG on M delta = r0
         bool stop_all = false;

@@ -399,12 +399,7 @@ struct OpT3 {
         st_chunk<T, V>(c.pnew + idx, vc);
         T q[V];
         apply_op_chunk<LOP_, T, V>(q, vm, vc, vp, vn, vs, xl, xr, CLEAN ? 0u : fb, code, a.K, xe, ycls, zcls);
-#if 0
-#pragma unroll
-        for (int i = 0; i < V; ++i) acc += (double)vc[i] * (double)q[i];
-#else
         acc += chunk_dot<T, V>(vc, q);
-#endif
     }
     __device__ static void finalize(const Args& a, const double (&tot)[1])
     {
@@ -597,8 +592,12 @@ struct OpT2 {
         int fold_delta;   // 0: residual of P as given (omni_residual); 1: inside the solve
     };
     struct Ctx {
-        int par; double* Pout;
-        __device__ Ctx(const Args& a) { par = a.fold_delta ? (a.sc->n & 1) : 0; Pout = a.Pbuf[par ^ 1]; }
+        int par; double* Pout; bool dz;
+        __device__ Ctx(const Args& a)
+        {
+            par = a.fold_delta ? (a.sc->n & 1) : 0; Pout = a.Pbuf[par ^ 1];
+            dz = !a.fold_delta || a.sc->dzero != 0;       // delta counts as zero: neither loaded nor added
+        }
     };
     // thread constant: link bytes of an unflagged chunk as far as x decides (box faces normal to x, pad cells)
     using TC = uint32_t;
@@ -631,18 +630,18 @@ struct OpT2 {
     __device__ static void produce(const Args&, const Ctx& c, const TmaSet& m, uint32_t stage, uint32_t bar, int x0, int y0,
                                    int plane, bool inner)
     {
-        mbar_expect_tx(bar, TG::BOX_P + TG::BOX_D + (inner ? TG::TILE_S : 0));
+        mbar_expect_tx(bar, TG::BOX_P + (c.dz ? 0 : TG::BOX_D) + (inner ? TG::TILE_S : 0));
         tma_load_3d(stage, &m.P_h[c.par], bar, x0 - TG::HXP, y0 - 1, plane);
-        tma_load_3d(stage + TG::TILE_P, &m.d2_h, bar, x0 - TG::HXD, y0 - 1, plane);
+        if (!c.dz) tma_load_3d(stage + TG::TILE_P, &m.d2_h, bar, x0 - TG::HXD, y0 - 1, plane);
         if (inner) tma_load_3d(stage + TG::TILE_P + TG::TILE_D, &m.S_c, bar, x0, y0, plane);
     }
     struct State {};
     __device__ static void advance(State&, const Ctx&, uint32_t, int, int) {}
-    __device__ static void value(uint32_t st, int offP, int offD, double (&v)[V])
+    __device__ static void value(uint32_t st, int offP, int offD, bool dz, double (&v)[V])
     {
-        double P[2]; T d[2];
+        double P[2]; T d[2] = { T(0), T(0) };
         lds_pair(st + offP, P);
-        lds_pair(st + TG::TILE_P + offD, d);
+        if (!dz) lds_pair(st + TG::TILE_P + offD, d);
         v[0] = P[0] + (double)d[0];
         v[1] = P[1] + (double)d[1];
     }
@@ -654,15 +653,17 @@ struct OpT2 {
         const int rowP = (warp + 1) * TG::PITCH_P, rowD = (warp + 1) * TG::PITCH_D;
         const int offP = rowP + (TG::HXP + lane * V) * 8, offD = rowD + (TG::HXD + lane * V) * (int)sizeof(T);
         double vm[V], vc[V], vp[V], vn[V], vs[V];
-        value(sC, offP, offD, vc);
-        value(sC, offP + TG::PITCH_P, offD + TG::PITCH_D, vn);
-        value(sC, offP - TG::PITCH_P, offD - TG::PITCH_D, vs);
-        value(sF, offP, offD, vp);
-        value(sB, offP, offD, vm);
-        const double hl = lds_scalar(sC + rowP + (TG::HXP - 1) * 8, double()) +
-                          (double)lds_scalar(sC + TG::TILE_P + rowD + (TG::HXD - 1) * (int)sizeof(T), T());
-        const double hr = lds_scalar(sC + rowP + (TG::HXP + TG::BX) * 8, double()) +
-                          (double)lds_scalar(sC + TG::TILE_P + rowD + (TG::HXD + TG::BX) * (int)sizeof(T), T());
+        value(sC, offP, offD, c.dz, vc);
+        value(sC, offP + TG::PITCH_P, offD + TG::PITCH_D, c.dz, vn);
+        value(sC, offP - TG::PITCH_P, offD - TG::PITCH_D, c.dz, vs);
+        value(sF, offP, offD, c.dz, vp);
+        value(sB, offP, offD, c.dz, vm);
+        double hl = lds_scalar(sC + rowP + (TG::HXP - 1) * 8, double());
+        double hr = lds_scalar(sC + rowP + (TG::HXP + TG::BX) * 8, double());
+        if (!c.dz) {
+            hl += (double)lds_scalar(sC + TG::TILE_P + rowD + (TG::HXD - 1) * (int)sizeof(T), T());
+            hr += (double)lds_scalar(sC + TG::TILE_P + rowD + (TG::HXD + TG::BX) * (int)sizeof(T), T());
+        }
         double xl = __shfl_up_sync(0xffffffffu, vc[V - 1], 1);
         double xr = __shfl_down_sync(0xffffffffu, vc[0], 1);
         if (lane == 0) xl = hl;
@@ -721,6 +722,7 @@ struct OpT2 {
         s->rho = tot[1];
         const int go = (tot[1] > s->thresh2) && (tot[1] != 0.0) && (s->max_cg > 0);
         s->inner_go = go;
+        s->dzero = !go;      // an inner loop that does not start leaves the old delta behind: the next K2 must not fold it again
         set_cond(a.cond, 1, go);
     }
 };

@@ -224,6 +224,22 @@ def test_batch2d_and_first_guess(oracle, dtype, forced_loop):
     tol = 1e-5 if dtype == "f32" else 1e-8
     Pc, ic = omni.solve_batch2d(gxd, gyd, md, d, tol, 100000, 32)
     assert ic["status"] == 0
+    # what the joint stopping rule guarantees per snapshot (include/omni.h): ||r_b|| <= tol ||S|| of the STACK, i.e.
+    # eps_R,b <= tol ||S|| / ||S_b||, with eps_R,b (Eq. 41) evaluated by the oracle's stored-weight operators
+    v2 = oracle.validity(gx[0].astype(np.float64), gy[0].astype(np.float64), None, m)
+    w1, w0, w0C = oracle.weights(v2, d[0], d[1])
+    rb, Sb = [], []
+    for b in range(5):
+        S_b = oracle.source(v2, w1, w0, gx[b].astype(np.float64), gy[b].astype(np.float64), None, d[0], d[1])
+        P_b = np.nan_to_num(Pc[b].cpu().numpy().astype(np.float64))
+        r_b = S_b + oracle.apply_Wn(v2, w0, w0C, P_b) - oracle.apply_M(v2, w1, P_b)
+        rb.append(np.linalg.norm(r_b)); Sb.append(np.linalg.norm(S_b))
+    normS = float(np.sqrt(np.sum(np.square(Sb))))
+    assert ic["norm_S"] == pytest.approx(normS, rel=1e-5 if dtype == "f32" else 1e-12)
+    slack = 3.0 if dtype == "f32" else 1.05           # fp32: P_out is the fp64 master pressure rounded to fp32
+    for b in range(5):
+        assert rb[b] <= slack * tol * normS, (b, rb[b] / Sb[b])          # eps_R,b <= tol ||S|| / ||S_b||
+    assert np.sqrt(np.sum(np.square(rb))) / normS <= slack * tol
     Pw, iw = omni.solve_batch2d(gxd, gyd, md, d, 2 * tol, 100, 32, P_init=torch.nan_to_num(Pc))
     assert iw["outer_iters"] == 0 and iw["cg_iters_total"] == 0
     assert torch.allclose(torch.nan_to_num(Pw), torch.nan_to_num(Pc), rtol=0, atol=1e-6 if dtype == "f32" else 1e-13)
@@ -766,3 +782,83 @@ def test_disconnected_components_and_isolated_cells(oracle, dtype, forced_loop):
     for comp in (left, right):
         assert abs(Pdn[comp].mean()) <= (1e-9 if dtype == "f64" else 1e-4) * scale
     assert Pdn[7, 9, 5] == 0.0
+
+
+PENCILS = [(2000, 1, 4), (500, 1, 1), (4000, 4, 4), (2000, 1, 8), (1200, 9, 3)]
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("shape", PENCILS)
+def test_pencil_shapes_long_z_axis(oracle, dtype, shape):
+    """Thin cross-sections with a long z axis: the tile kernels launch (x tiles) x (y tiles) x (z segments) CTAs with
+    z segments as short as ~4 planes, many more reduction slots than npad / 256 (the per-CTA partial buffer
+    must be sized from the launch geometry).  Through apply_M and residual (always the tile kernels) and through the
+    host-driven and graph loops."""
+    rng = np.random.default_rng(sum(shape))
+    g = [rng.normal(size=shape) for _ in range(3)]
+    mask = (rng.random(shape) > 0.03).astype(np.uint8)
+    f = dict(g=g, mask=mask, d=(0.7, 1.1, 0.4))
+    g_dev, g_or, m_dev, m = _inputs(f, dtype, mask)
+    d = f["d"]
+    v = oracle.validity(g_or[0], g_or[1], g_or[2], m)
+    w1, w0, w0C = oracle.weights(v, *d)
+    S_or = oracle.source(v, w1, w0, g_or[0], g_or[1], g_or[2], *d)
+    p = rng.normal(size=shape)
+    p_dev = to_dev(p, TDT[dtype])
+    p_or = p_dev.cpu().numpy().astype(np.float64) * v
+    q, pq = omni.apply_M(p_dev, m_dev, d)
+    q_or = oracle.apply_M(v, w1, p_or)
+    assert np.abs(q.cpu().numpy() - q_or).max() <= TOL_STEP[dtype] * 8 * np.abs(q_or).max()
+    assert pq == pytest.approx(float(np.sum(p_or * q_or)), rel=1e-5 if dtype == "f32" else 1e-11)
+    P = rng.normal(size=shape)
+    r, eps = omni.residual(g_dev[0], g_dev[1], g_dev[2], m_dev, to_dev(P), d)
+    Pv = P * v
+    r_or = S_or + oracle.apply_Wn(v, w0, w0C, Pv) - oracle.apply_M(v, w1, Pv)
+    assert np.abs(r.cpu().numpy() - r_or).max() <= TOL_STEP[dtype] * 8 * max(np.abs(r_or).max(), np.abs(Pv).max())
+    assert eps == pytest.approx(np.linalg.norm(r_or) / np.linalg.norm(S_or), rel=1e-5 if dtype == "f32" else 1e-10)
+    Po, io = oracle.solve(g_or[0], g_or[1], g_or[2], m, *d, tol=0.0, max_outer=3, max_cg=7)
+    for mode in (1, 2):
+        prev = omni.set_loop_mode(mode)
+        try:
+            Pg, ig = omni.solve(g_dev[0], g_dev[1], g_dev[2], m_dev, d, 0.0, 3, 7)
+        finally:
+            omni.set_loop_mode(prev)
+        assert ig["cg_iters_total"] == io["cg_iters_total"] == 21 and ig["outer_iters"] == io["outer_iters"]
+        assert np.array_equal(np.isnan(Pg.cpu().numpy()), np.isnan(Po))
+        assert rel_l2_after_mean_removal(Pg.cpu().numpy(), Po, ~np.isnan(Po)) <= TOL_SOLVE[dtype]
+        assert ig["eps_R_final"] == pytest.approx(io["eps_R_final"], rel=2e-3 if dtype == "f32" else 1e-7)
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_outer_iterations_whose_inner_loop_does_not_start(oracle, dtype, forced_loop):
+    """When an outer iteration's CG does not start (max_cg = 0; or an fp32-rounded r0 that underflows below the inner
+    threshold while the fp64 residual is still above tol) no new correction exists, and K2 must not fold whatever the
+    delta array holds into P (Scalars::dzero).  The oracle then repeats the same residual check until max_outer
+    (P unchanged, no CG iterations).  Reachable here through max_cg = 0, from zero and from a first guess."""
+    f = make_field("sphere3d", (20, 24, 36), seed=4, noise=0.05)
+    g_dev, g_or, m_dev, m = _inputs(f, dtype)
+    d = f["d"]
+    # (1) max_cg = 0: nothing may move
+    P, info = omni.solve(g_dev[0], g_dev[1], g_dev[2], m_dev, d, 1e-12, 5, 0)
+    Po, io = oracle.solve(g_or[0], g_or[1], g_or[2], m, *d, tol=1e-12, max_outer=5, max_cg=0)
+    assert info["outer_iters"] == io["outer_iters"] == 5 and info["cg_iters_total"] == io["cg_iters_total"] == 0
+    assert info["status"] == omni.binding.OMNI_NOT_CONVERGED
+    assert np.array_equal(np.nan_to_num(P.cpu().numpy()), np.nan_to_num(Po)) and not np.nan_to_num(Po).any()
+    assert info["eps_R_final"] == pytest.approx(1.0, rel=1e-6) and io["eps_R_final"] == pytest.approx(1.0, rel=1e-12)
+    # (2) a first guess plus max_cg = 0 comes back unchanged after several outer iterations, every check seeing the
+    # same residual
+    P1, i1 = omni.solve(g_dev[0], g_dev[1], g_dev[2], m_dev, d, 0.0, 2, 9)
+    guess = torch.nan_to_num(P1)
+    hist = torch.zeros(8, dtype=torch.float64, device="cuda")
+    omni.set_history(hist)
+    try:
+        P2, i2 = omni.solve_guess(g_dev[0], g_dev[1], g_dev[2], m_dev, d, 1e-12, 4, 0, guess)
+    finally:
+        omni.set_history(None)
+    assert i2["outer_iters"] == 4 and i2["cg_iters_total"] == 0
+    assert torch.equal(torch.nan_to_num(P2), guess)
+    h = hist.cpu().numpy()
+    assert np.all(h[:5] == h[0]) and h[0] > 0          # the same residual at every check
+    Po2, io2 = oracle.solve_guess(g_or[0], g_or[1], g_or[2], m, *d, tol=1e-12, max_outer=4, max_cg=0,
+                                  P_init=guess.cpu().numpy().astype(np.float64))
+    assert io2["outer_iters"] == 4 and h[0] == pytest.approx(io2["eps_R_final"], rel=1e-4 if dtype == "f32" else 1e-9)

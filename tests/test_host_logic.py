@@ -64,3 +64,34 @@ def test_no_cpu_fallback():
     g = torch.zeros(8, 8, dtype=torch.float64)
     with pytest.raises(RuntimeError):
         omni.solve(g, g, None, None, (1.0, 1.0), 1e-8, 1, 1)
+
+
+def test_binding_rejects_mismatched_tensors_before_the_call():
+    """A gy / gz / mask / out tensor whose shape or dtype differs from gx would make the kernels index out of bounds:
+    the binding raises before anything reaches the library (no device needed)."""
+    import torch
+    g = torch.zeros(6, 8, dtype=torch.float64)
+    for bad in (dict(gy=torch.zeros(6, 8, dtype=torch.float32)), dict(gy=torch.zeros(6, 9, dtype=torch.float64)),
+                dict(mask=torch.ones(8, 6, dtype=torch.uint8)), dict(mask=torch.ones(6, 8, dtype=torch.bool)),
+                dict(out=torch.zeros(6, 8, dtype=torch.float32))):
+        a = dict(gy=g, mask=None, out=None)
+        a.update(bad)
+        with pytest.raises(TypeError):
+            omni.solve(g, a["gy"], None, a["mask"], (1.0, 1.0), 1e-8, 1, 1, out=a["out"])
+    g3 = torch.zeros(4, 6, 8, dtype=torch.float32)
+    with pytest.raises(TypeError):
+        omni.solve(g3, g3, g3, torch.ones(6, 8, dtype=torch.uint8), (1.0, 1.0, 1.0), 1e-5, 1, 1)
+
+
+@pytest.mark.parametrize("dims", [(4, 1, 2000), (1, 1, 500), (4, 4, 4000), (8, 1, 2000), (500, 500, 500), (1024, 1024, 1)])
+def test_workspace_holds_one_reduction_slot_per_tile_cta(dims):
+    """thin cross-sections with a long z axis launch far more tile CTAs (x tiles * y tiles * z segments, two
+    accumulators in K2) than npad / 256; the workspace must grow with that bound, whatever segment count the device
+    picks (at most nz)."""
+    nx, ny, nz = dims
+    for dt, cell, pad in (("f32", 4, 8), ("f64", 8, 4)):
+        px = (nx + pad - 1) // pad * pad
+        npad = px * ny * nz
+        vectors = 5 * npad * cell + 2 * npad * 8 + npad * 5          # S r p0 p1 delta, P P1, link + wcode
+        worst_ctas = 2 * ((px + 63) // 64) * ((ny + 7) // 8) * nz
+        assert omni.workspace_bytes(nx, ny, nz, dt) >= vectors + 8 * worst_ctas

@@ -75,6 +75,106 @@ def test_3d_general_constants_symmetry_and_sum_rule(oracle):
     assert np.allclose(Kn["c"], Ki["c"], rtol=1e-8)
 
 
+# ----------------------------------------------------------------------------- general-spacing constants, pinned
+# without the oracle's own quadrature and without the CUDA library.  Everything below is derived
+# here from the geometric definition (Fig. 5b): the measure of the rays crossing two surface
+# elements dA1, dA2 a distance r apart is cos(th1) cos(th2) / r^2 dA1 dA2 (projected area x solid angle, Eq. 22 :253;
+# a whole face collects pi * area, Eq. 23 :258).
+
+def _far_face_adaptive(da, db, dc):
+    """c_aa: face a of C (db x dc) and the far face of Q = C + e_a, parallel at distance da: cos th1 = cos th2 = da / r.
+    The two area integrals reduce to differences u, v (int_0^L int_0^L f(|x1 - x2|) = 2 int_0^L (L - u) f(u) du):
+    c_aa = 4 int_0^db int_0^dc (db - u)(dc - v) da^2 / (u^2 + v^2 + da^2)^2 dv du.  Adaptive QUADPACK, not the
+    oracle's fixed Gauss-Legendre panels."""
+    from scipy import integrate
+    val, err = integrate.dblquad(lambda v, u: (db - u) * (dc - v) * da * da / (u * u + v * v + da * da) ** 2,
+                                 0.0, db, 0.0, dc, epsabs=1e-15, epsrel=1e-13)
+    return 4.0 * val, 4.0 * err
+
+
+def _far_face_mpmath(da, db, dc):
+    """The same integral with mpmath's tanh-sinh quadrature at 30 digits (a second, unrelated integrator)."""
+    import mpmath as mp
+    mp.mp.dps = 30
+    f = lambda u, v: (db - u) * (dc - v) * da * da / (u * u + v * v + da * da) ** 2
+    return float(4 * mp.quad(f, [0, db], [0, dc]))
+
+
+def _side_wall_1d(da, db, dc):
+    """c_ab by DIRECT integration of the side-wall measure (not through the sum rule): face a of C at a = 0,
+    (b, c) in [0, db] x [0, dc], normal e_a; the side wall of Q at b = db, (a, c) in [0, da] x [0, dc], normal e_b.
+    With s = db - b1 and v = |c2 - c1|: cos th1 = a / r, cos th2 = s / r, r^2 = a^2 + s^2 + v^2,
+      c_ab = 2 int_0^da int_0^db int_0^dc (dc - v) a s / r^4 dv ds da.
+    The a and s integrals are elementary (int a / (a^2 + k)^2 = -1 / (2 (a^2 + k)), int s / (s^2 + m) = ln(s^2 + m) / 2):
+      c_ab = 1/2 int_0^dc (dc - v) [ ln((db^2 + v^2) / v^2) - ln((da^2 + db^2 + v^2) / (da^2 + v^2)) ] dv,
+    a 1D integral with an integrable log singularity at v = 0."""
+    import mpmath as mp
+    mp.mp.dps = 30
+    f = lambda v: (dc - v) * (mp.log((db * db + v * v) / (v * v)) - mp.log((da * da + db * db + v * v) / (da * da + v * v)))
+    return float(mp.quad(f, [0, dc / 64, dc]) / 2)
+
+
+def _side_wall_3d_bruteforce(da, db, dc):
+    """The unreduced kernel a s / r^4 over (a, s, c1, c2) by plain nested adaptive quadrature in the three variables
+    (a, s, v) -- checks the reductions above at a looser tolerance."""
+    import warnings
+    from scipy import integrate
+    with warnings.catch_warnings():
+        warnings.simplefilter("ignore", integrate.IntegrationWarning)      # the kernel peaks along the shared edge
+        val, err = integrate.tplquad(lambda v, s, a: (dc - v) * a * s / (a * a + s * s + v * v) ** 2,
+                                     0.0, da, 0.0, db, 0.0, dc, epsabs=1e-9, epsrel=1e-9)
+    return 2.0 * val
+
+
+ANISO = [(1.0, 0.7, 1.9), (1.0 / 263, 1.0 / 15, 1.0 / 4), (0.25, 1.0 / 15, 1.0 / 263), (1.0, 1.0, 1.0)]
+
+
+@pytest.mark.parametrize("sp", ANISO)
+def test_far_face_constant_vs_adaptive_quadrature(oracle, sp):
+    """oracle.far_face_constant (fixed Gauss-Legendre on dyadic panels) against two adaptive integrators of the defining
+    integral written out in this file, for every axis ordering, at strongly anisotropic spacing (66:1).  A wrong panel
+    count, a swapped db / dc or a dropped factor fails here without the CUDA library being imported."""
+    for a in range(3):
+        da, db, dc = sp[a], sp[(a + 1) % 3], sp[(a + 2) % 3]
+        got = oracle.far_face_constant(da, db, dc)
+        F = math.pi * db * dc
+        ref_mp = _far_face_mpmath(da, db, dc)
+        ref_qp, err = _far_face_adaptive(da, db, dc)
+        assert ref_qp == pytest.approx(ref_mp, rel=1e-10, abs=1e-13 * F)          # the two integrators agree
+        # what enters the stencil is c / A_tot; relative to the face total F_a the pin is 1e-11
+        assert abs(got - ref_mp) <= 1e-11 * F, (a, got, ref_mp)
+        assert got == pytest.approx(ref_mp, rel=1e-9)                               # and relative to c_aa itself
+        # the integral is symmetric in (db, dc) but NOT in (da, db): a swapped argument is visible at these spacings
+        if abs(da - db) > 1e-12:
+            assert abs(oracle.far_face_constant(db, da, dc) - ref_mp) > 1e-6 * F
+
+
+@pytest.mark.parametrize("sp", ANISO)
+def test_cross_constants_vs_direct_side_wall_quadrature(oracle, sp):
+    """The oracle obtains c_ab from the sum rules c_aa + 2 c_ab + 2 c_ac = F_a and c_ab = c_ba (:304).  Here each c_ab is
+    integrated DIRECTLY over the side wall (survey probe A7 re-established): agreement to 1e-11 F_a pins the sum-rule
+    construction -- and with it far_face_constant -- from a second, independent side."""
+    dx, dy, dz = sp
+    K = oracle.constants(4, 4, 4, dx, dy, dz)
+    c, F = K["c"], K["F"]
+    for a in range(3):
+        for b in range(3):
+            if a == b:
+                continue
+            cc = 3 - a - b
+            direct = _side_wall_1d(sp[a], sp[b], sp[cc])
+            assert abs(c[a, b] - direct) <= 1e-11 * F[a], (a, b, c[a, b], direct)
+            assert c[a, b] == pytest.approx(direct, rel=1e-8)
+    # the reduction to one dimension itself, against the unreduced 3D kernel (looser: nested QUADPACK near the edge)
+    a, b, cc = 0, 1, 2
+    assert _side_wall_1d(sp[a], sp[b], sp[cc]) == pytest.approx(_side_wall_3d_bruteforce(sp[a], sp[b], sp[cc]), rel=2e-6)
+    # every ray through face a leaves Q through exactly one of its five other faces (Eq. 23 :258)
+    for a in range(3):
+        b, cc = (a + 1) % 3, (a + 2) % 3
+        tot = _far_face_mpmath(sp[a], sp[b], sp[cc]) + 2 * _side_wall_1d(sp[a], sp[b], sp[cc]) + 2 * _side_wall_1d(sp[a], sp[cc], sp[b])
+        assert tot == pytest.approx(math.pi * sp[b] * sp[cc], rel=1e-11)
+
+
 # ----------------------------------------------------------------------------- brute-force ray counts (P11)
 
 def _mc_fractions(da, db, dc, n, rng, three_d):
