@@ -217,6 +217,24 @@ def sample(v, gx, gy, gz, x, cells, dx, dy, dz=1.0):
     return S, Mx, Wx
 
 
+def eps_R_of_field(gx, gy, gz, mask, P, dx, dy, dz=1.0, chunk=4_000_000):
+    """Momentum residual of a GIVEN field (Eq. 41): eps_R = ||S + W^n P - M P||_2 / ||S||_2, evaluated cell by
+    cell through oracle_sample in chunks of `chunk` cells, so that a full-size field (500^3) needs no stored weight
+    arrays.  NaN / missing cells of P count as 0 (they carry zero weights).  Returns (eps_R, ||r||, ||S||).
+    SURVEY 8(c) parity protocol iii: certifies a converged field the oracle itself cannot afford to compute."""
+    v = validity(gx, gy, gz, mask)
+    x = np.nan_to_num(_f64(P), nan=0.0) * v
+    n = v.size
+    rr = ss = 0.0
+    for c0 in range(0, n, chunk):
+        cells = np.arange(c0, min(n, c0 + chunk), dtype=np.int64)
+        S, Mx, Wx = sample(v, gx, gy, gz, x, cells, dx, dy, dz)
+        r = S + Wx - Mx
+        rr += float(np.dot(r, r))
+        ss += float(np.dot(S, S))
+    return (float(np.sqrt(rr / ss)) if ss > 0 else 0.0), float(np.sqrt(rr)), float(np.sqrt(ss))
+
+
 def solve_batch2d(gx, gy, mask2d, dx, dy, tol, max_outer, max_cg, P_init=None, direct=False):
     """nb stacked 2D snapshots (nb, ny, nx) on one mask (ny, nx), solved as one block-diagonal system
     (direct: with the inner systems of solve_direct)."""

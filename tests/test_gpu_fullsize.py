@@ -1,7 +1,14 @@
 """BASELINE.json's full-size configs, in the launch configuration bench.py times, against the oracle:
-step outputs at sampled cells (the oracle evaluates S_C, (M x)_C, (W^n x)_C one cell at a time), the device
-reductions against fp64 sums of the full device arrays, and a short fixed-count trajectory against a full oracle
-solve where host memory allows it."""
+* test_fullsize_config: step outputs at sampled cells (the oracle evaluates S_C, (M x)_C, (W^n x)_C one cell at a
+  time) and the device reductions against fp64 sums of the full device arrays;
+* test_fullsize_trajectory_vs_oracle: a short fixed-count trajectory against a FULL oracle solve (SURVEY 8(c) parity
+  protocol i); skipped BY NAME, with the reason, only if the host cannot hold the oracle's 19 fp64 fields;
+* test_converged_parity_fullsize: converged on both sides with the same stopping rules (protocol ii) where the oracle
+  finishes in minutes -- configs[2] always, configs[1] / configs[3] fp32 with OMNI_TEST_LONG=1;
+* test_converged_field_certified_by_oracle: every config converged on the GPU (Alg. 1 and the cascade solve), then
+  eps_R of Eq. 41 re-evaluated by the oracle's per-cell operators over ALL cells (protocol iii)."""
+import os
+
 import numpy as np
 import pytest
 
@@ -24,20 +31,35 @@ def _host_mem_gb():
         import psutil
         return psutil.virtual_memory().available / 2**30
     except Exception:
-        return 0.0
+        pass
+    try:
+        with open("/proc/meminfo") as fh:
+            for line in fh:
+                if line.startswith("MemAvailable:"):
+                    return int(line.split()[1]) / 2**20
+    except Exception:
+        pass
+    return float("nan")                   # unknown: the callers then try, they do not skip silently
 
 
-@pytest.mark.parametrize("idx,dtype", CASES)
-def test_fullsize_config(oracle, idx, dtype):
+def _load(idx, dtype):
+    """Device tensors of configs[idx] in `dtype` and the values the oracle must consume (what the device consumed)."""
     f = make_config(idx, device="cuda")
-    d = f["d"]
     tdt = torch.float32 if dtype == "f32" else torch.float64
     g_dev = [torch.from_numpy(c).to(tdt).cuda() for c in f["g"]]
-    g_or = [c.cpu().numpy().astype(np.float64) for c in g_dev]           # the values the device consumed
+    g_or = [c.cpu().numpy().astype(np.float64) for c in g_dev]
     g_dev += [None] * (3 - len(g_dev))
     g_or += [None] * (3 - len(g_or))
     mask = f["mask"]
     m_dev = None if mask is None else torch.from_numpy(mask).cuda()
+    return f, g_dev, g_or, mask, m_dev
+
+
+@pytest.mark.parametrize("idx,dtype", CASES)
+def test_fullsize_config(oracle, idx, dtype):
+    f, g_dev, g_or, mask, m_dev = _load(idx, dtype)
+    d = f["d"]
+    tdt = torch.float32 if dtype == "f32" else torch.float64
     shape = f["g"][0].shape
     N = int(np.prod(shape))
     v = oracle.validity(g_or[0], g_or[1], g_or[2], mask)
@@ -90,23 +112,6 @@ def test_fullsize_config(oracle, idx, dtype):
     assert scale > 0
     del r, Pn, S, x_dev
 
-    # short fixed-count trajectory against a full oracle solve (needs ~18 fp64 fields on the host)
-    if N * 8 * 20 / 2**30 < 0.6 * _host_mem_gb():
-        mo, mc = (2, 5) if N > 5e7 else (3, 8)
-        Pg, ig = omni.solve(g_dev[0], g_dev[1], g_dev[2], m_dev, d, 0.0, mo, mc)
-        Po, io = oracle.solve(g_or[0], g_or[1], g_or[2], mask, *d, tol=0.0, max_outer=mo, max_cg=mc)
-        assert ig["cg_iters_total"] == io["cg_iters_total"] == mo * mc
-        err = rel_l2_after_mean_removal(Pg.cpu().numpy(), Po, v == 1)
-        assert err <= TOL_SOLVE[dtype], err
-        assert ig["eps_R_final"] == pytest.approx(io["eps_R_final"], rel=1e-3 if dtype == "f32" else 1e-8)
-        # the fixed-point solve (omni_solve_direct) on the same footing
-        Pg, ig = omni.solve_direct(g_dev[0], g_dev[1], g_dev[2], m_dev, d, 0.0, mo, mc)
-        Po, io = oracle.solve_direct(g_or[0], g_or[1], g_or[2], mask, *d, tol=0.0, max_outer=mo, max_cg=mc)
-        assert ig["cg_iters_total"] == io["cg_iters_total"] == mo * mc
-        err = rel_l2_after_mean_removal(Pg.cpu().numpy(), Po, v == 1)
-        assert err <= TOL_SOLVE[dtype], err
-        assert ig["eps_R_final"] == pytest.approx(io["eps_R_final"], rel=1e-3 if dtype == "f32" else 1e-8)
-
     # omni_solve_direct at full size: its eps_R against the residual kernel on the returned field, the residual at the
     # sampled cells against the oracle
     Pd, idd = omni.solve_direct(g_dev[0], g_dev[1], g_dev[2], m_dev, d, tol, 2, 60)
@@ -117,6 +122,100 @@ def test_fullsize_config(oracle, idx, dtype):
     _, MP, WP = oracle.sample(v, None, None, None, Pn.cpu().numpy(), cells, *d)
     r_s = r.flatten()[torch.from_numpy(cells).cuda()].cpu().numpy().astype(np.float64)
     assert np.abs(r_s - (S_or + WP - MP)).max() <= TOL_STEP[dtype] * 16 * max(np.abs(MP).max(), np.abs(S_or).max())
+
+
+@pytest.mark.parametrize("idx,dtype", CASES)
+def test_fullsize_trajectory_vs_oracle(oracle, idx, dtype):
+    """Short fixed-count trajectory (tol = 0: identical steps on both sides) of Alg. 1 and of the fixed-point solve at the
+    FULL size of every config, against a full oracle solve.  The oracle holds 19 fp64 fields plus inputs and outputs
+    (24 x 8 x N bytes: 24 GB at 500^3)."""
+    f, g_dev, g_or, mask, m_dev = _load(idx, dtype)
+    d = f["d"]
+    N = int(np.prod(f["g"][0].shape))
+    need, have = N * 8 * 24 / 2**30, _host_mem_gb()
+    if have == have and have < 1.2 * need:
+        pytest.skip(f"host memory: the oracle needs {need:.1f} GiB for configs[{idx}], {have:.1f} GiB available")
+    v = oracle.validity(g_or[0], g_or[1], g_or[2], mask)
+    mo, mc = (2, 5) if N > 5e7 else (3, 8)
+    Pg, ig = omni.solve(g_dev[0], g_dev[1], g_dev[2], m_dev, d, 0.0, mo, mc)
+    Po, io = oracle.solve(g_or[0], g_or[1], g_or[2], mask, *d, tol=0.0, max_outer=mo, max_cg=mc)
+    assert ig["cg_iters_total"] == io["cg_iters_total"] == mo * mc
+    err = rel_l2_after_mean_removal(Pg.cpu().numpy(), Po, v == 1)
+    assert err <= TOL_SOLVE[dtype], err
+    assert ig["eps_R_final"] == pytest.approx(io["eps_R_final"], rel=1e-3 if dtype == "f32" else 1e-8)
+    # the fixed-point solve (omni_solve_direct) on the same footing
+    Pg, ig = omni.solve_direct(g_dev[0], g_dev[1], g_dev[2], m_dev, d, 0.0, mo, mc)
+    Po, io = oracle.solve_direct(g_or[0], g_or[1], g_or[2], mask, *d, tol=0.0, max_outer=mo, max_cg=mc)
+    assert ig["cg_iters_total"] == io["cg_iters_total"] == mo * mc
+    err = rel_l2_after_mean_removal(Pg.cpu().numpy(), Po, v == 1)
+    assert err <= TOL_SOLVE[dtype], err
+    assert ig["eps_R_final"] == pytest.approx(io["eps_R_final"], rel=1e-3 if dtype == "f32" else 1e-8)
+
+
+LONG = os.environ.get("OMNI_TEST_LONG") == "1"
+TOL_CONV = {"f64": 1e-8, "f32": 1e-5}
+
+
+@pytest.mark.parametrize("idx,dtype,always", [(2, "f64", True), (1, "f32", False), (3, "f32", False)])
+def test_converged_parity_fullsize(oracle, idx, dtype, always):
+    """SURVEY 8(c) parity protocol ii at full size: BASELINE's tolerance, max_cg = 16 (the tuned cap of BASELINE.md 5a:
+    the same converged field), the same stopping rules on both sides; rel-L2 after mean removal <= 1e-9 / 2e-4 and the
+    outer-iteration counts within 2 (eps_R carries ~10 % of tol of inner-solve noise near the end).
+    The oracle needs about 3 min (configs[2]) / 5 min (configs[1] fp32) / 10 min (configs[3] fp32) on 16 host threads."""
+    if not always and not LONG:
+        pytest.skip(f"configs[{idx}] {dtype}: the oracle needs 5-10 min to converge; set OMNI_TEST_LONG=1 to run")
+    f, g_dev, g_or, mask, m_dev = _load(idx, dtype)
+    d, tol = f["d"], TOL_CONV[dtype]
+    P, info = omni.solve(g_dev[0], g_dev[1], g_dev[2], m_dev, d, tol, 200000, 16)
+    assert info["status"] == 0 and info["eps_R_final"] <= tol
+    Po, io = oracle.solve(g_or[0], g_or[1], g_or[2], mask, *d, tol=tol, max_outer=200000, max_cg=16)
+    assert io["converged"]
+    valid = ~np.isnan(Po)
+    assert np.array_equal(np.isnan(P.cpu().numpy()), ~valid)
+    err = rel_l2_after_mean_removal(P.cpu().numpy(), Po, valid)
+    print(f"configs[{idx}] {dtype}: GPU {info['outer_iters']} outer / {info['cg_iters_total']} CG, oracle "
+          f"{io['outer_iters']} / {io['cg_iters_total']}, rel-L2 {err:.3e}")
+    assert err <= TOL_SOLVE[dtype], err
+    assert abs(info["outer_iters"] - io["outer_iters"]) <= 2, (info, io)
+    Pa = f["P"]
+    assert rel_l2_after_mean_removal(P.cpu().numpy(), Pa, valid) == pytest.approx(rel_l2_after_mean_removal(Po, Pa, valid), rel=1e-3)
+
+
+@pytest.mark.parametrize("idx,dtype", [(0, "f64")] + CASES)
+def test_converged_field_certified_by_oracle(oracle, idx, dtype):
+    """SURVEY 8(c) parity protocol iii (north_star "Target"): the CONVERGED GPU field of every config -- by Alg. 1
+    (max_cg 16) and by omni_solve_cascade -- has its eps_R (Eq. 41 :442) re-evaluated by the oracle's per-cell operators
+    over all cells (oracle.eps_R_of_field).  fp64: the oracle must see eps_R <= 1.05 tol.  fp32: the returned field is
+    the fp64 master pressure rounded to fp32, and that rounding alone leaves a residual u |L||P| that grows with the
+    grid (SURVEY 7 hard part 3), so the oracle's figure is bounded by tol plus that floor, the floor being evaluated by
+    the oracle on the same field (the residual change under one more fp32 rounding of P_out has the same statistics).
+    configs[4] by Alg. 1 takes about two minutes of GPU time (10 500 outer iterations)."""
+    f, g_dev, g_or, mask, m_dev = _load(idx, dtype)
+    d, tol = f["d"], TOL_CONV[dtype]
+    runs = [("alg1", lambda: omni.solve(g_dev[0], g_dev[1], g_dev[2], m_dev, d, tol, 400000, 16)),
+            ("cascade", lambda: omni.solve_cascade(g_dev[0], g_dev[1], g_dev[2], m_dev, d, tol, 20, 30000, levels=4))]
+    for name, fn in runs:
+        P, info = fn()
+        assert info["status"] == 0 and info["eps_R_final"] <= tol, (name, info)
+        Pn = P.cpu().numpy()
+        eps, nr, nS = oracle.eps_R_of_field(g_or[0], g_or[1], g_or[2], mask, Pn, *d)
+        assert nS == pytest.approx(info["norm_S"], rel=1e-5 if dtype == "f32" else 1e-11)
+        if dtype == "f64":
+            bound = 1.05 * tol
+        else:
+            # floor of an fp32 field: perturb P_out by a relative 2^-24 per cell with alternating sign pattern drawn
+            # once (seeded), and let the oracle measure the residual change
+            rng = np.random.default_rng(5)
+            Pp = Pn.astype(np.float64) * (1.0 + 2.0 ** -24 * rng.uniform(-1.0, 1.0, size=Pn.shape))
+            eps_p, _, _ = oracle.eps_R_of_field(g_or[0], g_or[1], g_or[2], mask, Pp, *d)
+            floor = abs(eps_p ** 2 - eps ** 2) ** 0.5
+            bound = 1.05 * tol + 2.0 * floor
+            print(f"  fp32 rounding floor of eps_R on this field: {floor:.3e}")
+        print(f"configs[{idx}] {dtype} {name}: GPU eps_R {info['eps_R_final']:.3e} ({info['outer_iters']} outer, "
+              f"{info['cg_iters_total']} CG), oracle eps_R of P_out {eps:.3e} (bound {bound:.3e})")
+        assert eps <= bound, (name, eps, bound)
+        valid = ~np.isnan(Pn)
+        assert rel_l2_after_mean_removal(Pn, f["P"], valid) < 0.05
 
 
 def _quadratic_case(nx, ny, nz, dev):

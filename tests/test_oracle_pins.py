@@ -638,6 +638,30 @@ def test_sample_matches_stored_weight_path(oracle):
 
 # ----------------------------------------------------------------------------- batched snapshots / first guess (NEXT-1)
 
+def test_eps_R_of_field_matches_the_solver_and_the_stored_weight_path(oracle):
+    """eps_R_of_field (chunked per-cell evaluation, used to certify full-size GPU fields) against (i) the eps_R the
+    oracle's own solve reports for the field it returns and (ii) S + W^n P - M P through the stored-weight operators,
+    on a masked anisotropic 3D grid with NaN-marked cells; chunk boundaries must not matter."""
+    rng = np.random.default_rng(17)
+    shape = (7, 9, 11)
+    g = [rng.normal(size=shape) for _ in range(3)]
+    mask = (rng.random(shape) > 0.15).astype(np.uint8)
+    g[1][2, 3, 4] = np.nan
+    d = (0.4, 1.1, 0.7)
+    P, info = oracle.solve(g[0], g[1], g[2], mask, *d, tol=1e-6, max_outer=60, max_cg=50)     # any returned field will do
+    assert 0 < info["eps_R_final"] < 1
+    for chunk in (10_000_000, 97):
+        eps, nr, nS = oracle.eps_R_of_field(g[0], g[1], g[2], mask, P, *d, chunk=chunk)
+        assert eps == pytest.approx(info["eps_R_final"], rel=1e-9) and nS == pytest.approx(info["norm_S"], rel=1e-12)
+    v = oracle.validity(g[0], g[1], g[2], mask)
+    w1, w0, w0C = oracle.weights(v, *d)
+    S = oracle.source(v, w1, w0, np.nan_to_num(g[0]), np.nan_to_num(g[1]), np.nan_to_num(g[2]), *d)
+    Q = rng.normal(size=shape) * v
+    r = S + oracle.apply_Wn(v, w0, w0C, Q) - oracle.apply_M(v, w1, Q)
+    eps, nr, nS = oracle.eps_R_of_field(g[0], g[1], g[2], mask, np.where(v == 1, Q, np.nan), *d, chunk=1000)
+    assert nr == pytest.approx(np.linalg.norm(r), rel=1e-12) and eps == pytest.approx(np.linalg.norm(r) / np.linalg.norm(S), rel=1e-12)
+
+
 def test_batch2d_oracle_pins(oracle):
     """Stacked 2D snapshots solved as one block-diagonal system (2D constants, no coupling across planes):
     nb = 1 is bit-identical to the plain 2D solve; converged, every snapshot equals its own single solve (pinned above)
