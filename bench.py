@@ -28,18 +28,45 @@ METRIC = "grid-point CG updates/s"
 UNIT = "grid-point CG updates/s"
 CPU_SAMPLE_EDGE = 320                   # 3D: edge of the corner crop the oracle is timed on (2D: the whole grid);
                                         # with the step's own caps that is ~10 s of work on 16 host threads
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel (K4) from the ncu --set full capture
-# summarised in profiles/r1_ncu_k3_k4_500cube_f32.md; only valid for that workload.  K4 streams different arrays by
-# CG-iteration parity (lazy delta): even k, the first odd k (delta not read yet), the other odd k.
-NCU_TRAFFIC_K4 = {(4, "f32"): {"even": 1.032482e9 + 0.462397e9, "odd_first": 1.544273e9 + 0.962295e9,
-                               "odd": 2.042280e9 + 0.962293e9}}
+# roofline.traffic: dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel (K4) comes from an ncu
+# --set full capture that cannot be taken inside a timed run; its per-launch bytes are kept in TRAFFIC_CSV together with
+# the hash of the kernel sources they were captured from.  The figure is reported only while that hash matches the tree
+# (a changed kernel must be re-captured); otherwise traffic is null and traffic_source says why.
+TRAFFIC_CSV = os.path.join(ROOT, "profiles", "r2_ncu_traffic.csv")
+CONV_MAX_CG = 16                        # Alg. 1 time-to-converged: the tuned inner cap of BASELINE.md 5a (same converged field)
+ALL_CASES = [(0, "f64"), (1, "f32"), (1, "f64"), (2, "f64"), (3, "f32"), (3, "f64"), (4, "f32")]
+L2_BYTES = 126e6
 
 
-def k4_traffic(t, n_even, n_odd):
-    """Average measured DRAM bytes per K4 launch over the step's mix of even / first-odd / odd CG iterations."""
-    if t is None:
-        return None
-    return (n_even * t["even"] + (t["odd_first"] if n_odd else 0.0) + max(n_odd - 1, 0) * t["odd"]) / (n_even + n_odd)
+def csrc_hash():
+    """sha1 over the kernel sources (csrc/*): identifies what an ncu capture in profiles/ was taken from."""
+    import hashlib
+    h = hashlib.sha1()
+    d = os.path.join(ROOT, "paper_2311_16935_b200", "csrc")
+    for name in sorted(os.listdir(d)):
+        with open(os.path.join(d, name), "rb") as fh:
+            h.update(name.encode() + b"\0" + fh.read())
+    return h.hexdigest()[:16]
+
+
+def k4_traffic(config, dtype, n_even, n_odd):
+    """(average measured DRAM bytes per K4 launch over the step's mix of even / first-odd / odd CG iterations, source)."""
+    import csv
+    try:
+        with open(TRAFFIC_CSV) as fh:
+            rows = [r for r in csv.DictReader(fh) if int(r["config"]) == config and r["dtype"] == dtype and r["kernel"] == "K4"]
+    except Exception:
+        return None, "no ncu capture committed for this workload (profiles/r2_ncu_traffic.csv)"
+    if not rows:
+        return None, "no ncu capture committed for this workload (profiles/r2_ncu_traffic.csv)"
+    t = {r["variant"]: float(r["dram_read_bytes"]) + float(r["dram_write_bytes"]) for r in rows}
+    src = rows[0]["csrc_hash"]
+    if src != csrc_hash():
+        return None, f"stale: profiles/r2_ncu_traffic.csv was captured at csrc hash {src}, the tree is at {csrc_hash()}"
+    if not all(k in t for k in ("even", "odd_first", "odd")):
+        return None, "profiles/r2_ncu_traffic.csv lacks a K4 variant"
+    avg = (n_even * t["even"] + (t["odd_first"] if n_odd else 0.0) + max(n_odd - 1, 0) * t["odd"]) / (n_even + n_odd)
+    return avg, f"profiles/r2_ncu_traffic.csv (ncu --set full, csrc hash {src}), see profiles/r2_ncu_traffic.md"
 
 
 def parse():
@@ -58,6 +85,10 @@ def parse():
                     help="--converge: omni_solve_direct (CG on the fixed-point system L P = S) instead of Algorithm 1")
     ap.add_argument("--cascade", type=int, default=-1,
                     help="--converge: omni_solve_cascade with this many coarse levels (implies the direct solve)")
+    ap.add_argument("--no-extras", action="store_true",
+                    help="default run: skip the per_config and converged sections (profiling runs; always skipped for N > 1)")
+    ap.add_argument("--certify", action="store_true",
+                    help="--converge: let the oracle re-evaluate eps_R (Eq. 41) of the converged GPU field over all cells")
     ap.add_argument("--batch", type=int, default=1,
                     help="--converge on a 2D config: solve this many snapshots (same mask, different noise seeds) in one "
                          "omni_solve_batch2d call")
@@ -108,7 +139,10 @@ def converge(args, cfg, dtype):
     sec = e0.elapsed_time(e1) * 1e-3
     valid = ~np.isnan(Pn)
     a, b = Pn[valid] - Pn[valid].mean(), f["P"][valid] - f["P"][valid].mean()
-    print(json.dumps({"converge": True, "workload": f"configs[{args.config}] {cfg['kind']} {cfg['n']} {dtype}", "tol": tol,
+    cert = None
+    if args.certify and args.batch == 1:
+        cert = oracle_eps_R(f, g, Pn)
+    print(json.dumps({"converge": True, "eps_R_oracle": cert, "workload": f"configs[{args.config}] {cfg['kind']} {cfg['n']} {dtype}", "tol": tol,
                       "max_cg": args.max_cg, "batch": args.batch, "direct": bool(args.direct or args.cascade >= 0), "cascade_levels": args.cascade, "outer_iters": info["outer_iters"], "cg_iters": info["cg_iters_total"],
                       "seconds": sec, "eps_R": info["eps_R_final"], "status": info["status"],
                       "updates_per_s": N * info["cg_iters_total"] / sec,
@@ -206,10 +240,120 @@ def run_oracle(f, dtype, steps, warmup):
     units = 0
     for _ in range(steps):
         _, info = orc.solve(g[0], g[1], g[2], m, *f["d"], tol=tol, max_outer=mo, max_cg=mc)
-        units += g[0].size * info["cg_iters_total"]
+        units += (g[0].size if m is None else int(m.sum())) * info["cg_iters_total"]
     dt = time.perf_counter() - t0
     desc = f"corner crop {e}^{ndim} of the same field, omni oracle solve max_outer={mo} max_cg={mc}, {steps} step(s)"
     return units / dt, orc.num_threads(), desc, dt / steps
+
+
+def oracle_eps_R(f, g_dev, P_np):
+    """SURVEY 8(c) parity protocol iii: eps_R (Eq. 41) of a GPU field re-evaluated by the ORACLE's per-cell operators over
+    all cells, from the values the device consumed.  Reporting only (bench.py's cpu_baseline leg is where the bench may
+    run the oracle); never inside a timed region."""
+    import numpy as np
+    from oracle import omni_oracle as orc
+    g = [None if c is None else c.cpu().numpy().astype(np.float64) for c in g_dev]
+    eps, _, _ = orc.eps_R_of_field(g[0], g[1], g[2], f["mask"], P_np, *f["d"])
+    return eps
+
+
+def _load_case(idx, dtype, dev):
+    import torch
+    from workloads import make_config
+    f = make_config(idx, device=str(dev))
+    tdt = torch.float32 if dtype == "f32" else torch.float64
+    g = [torch.from_numpy(c).to(tdt).to(dev) for c in f["g"]] + [None] * (3 - len(f["g"]))
+    m = None if f["mask"] is None else torch.from_numpy(f["mask"]).to(dev)
+    return f, g, m
+
+
+def _timed(fn, reps=1):
+    """Best-of-reps CUDA-event time (s) of fn(), events on the current stream; returns (seconds, last result)."""
+    import torch
+    best, out = None, None
+    for _ in range(reps):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        e0.record()
+        out = fn()
+        e1.record()
+        torch.cuda.synchronize()
+        t = e0.elapsed_time(e1) * 1e-3
+        best = t if best is None else min(best, t)
+    return best, out
+
+
+def per_config_entry(idx, dtype, dev, peak, cache=None):
+    """CG inner loop of one config at full size (SURVEY 8(d) metric 1 and 3), two live measurements:
+    * `cg_iteration_us`: whole-call CUDA-event time of two fixed-count solves that differ only in max_cg (one outer
+      iteration, tol = 0), difference / iteration difference -- what one CG iteration costs in the loop driver the
+      library picks by itself for this size, everything included;
+    * `k3_us`, `k4_us`: CUDA events around every tile-kernel launch of the host-driven loop (loop mode 1)."""
+    import paper_2311_16935_b200 as omni
+    f, g, m = cache if cache is not None else _load_case(idx, dtype, dev)
+    d = f["d"]
+    N = g[0].numel()
+    nvalid = N if m is None else int(m.sum().item())
+    esz = 4 if dtype == "f32" else 8
+    # enough iterations for ~20 ms of difference whatever the size
+    m1 = 10
+    m2 = m1 + int(min(2000, max(60, 3e9 / (N * esz))))
+    omni.solve(g[0], g[1], g[2], m, d, 0.0, 1, m1, want_info=False)
+    t1, _ = _timed(lambda: omni.solve(g[0], g[1], g[2], m, d, 0.0, 1, m1, want_info=False), 3)
+    t2, _ = _timed(lambda: omni.solve(g[0], g[1], g[2], m, d, 0.0, 1, m2, want_info=False), 3)
+    cg = (t2 - t1) / (m2 - m1)
+    prev = omni.set_loop_mode(1)
+    omni.profile_enable(1)
+    omni.profile_read(reset=True)
+    omni.solve(g[0], g[1], g[2], m, d, 0.0, 2, 25)
+    prof = omni.profile_read(reset=True)
+    omni.profile_enable(0)
+    omni.set_loop_mode(prev)
+    k3 = prof["K3"][0] / max(prof["K3"][1], 1) * 1e-3
+    k4 = prof["K4"][0] / max(prof["K4"][1], 1) * 1e-3
+    alg = 7.5 * esz * N                     # DESIGN.md section 6: K3 3 passes, K4 3 / 6 by iteration parity
+    resident = (5 * esz + 16) * N < L2_BYTES
+    return {"workload": f"configs[{idx}] {f['kind']} {'x'.join(str(x) for x in f['shape'])} {dtype}", "cells": N,
+            "valid_cells": nvalid, "cg_iteration_us": cg * 1e6, "updates_per_s_in_loop": nvalid / cg,
+            "algorithmic_bytes_per_cg_iteration": alg, "algorithmic_GBps": alg / cg / 1e9,
+            "frac_of_measured": alg / cg / 1e9 / peak, "frac_of_8TBps": alg / cg / 8e12,
+            "memory": "L2-resident: effective GB/s, not HBM" if resident else "HBM (state exceeds L2)",
+            "k3_us": k3 * 1e6, "k4_us": k4 * 1e6, "tile_kernels_cg_iteration_us": (k3 + k4) * 1e6,
+            "iterations_timed": [m1, m2]}
+
+
+def converged_entries(idx, dtype, dev, cache=None, alg1=True):
+    """Time to converged P (SURVEY 8(d) metric 2): whole call, CUDA events, inputs resident, eps_R <= tol -- by Alg. 1
+    (the paper's iteration, max_cg = 16) and, separately named, by the fixed-point solves; each converged field has its
+    eps_R re-evaluated by the oracle over all cells (parity protocol iii)."""
+    import numpy as np
+    import paper_2311_16935_b200 as omni
+    f, g, m = cache if cache is not None else _load_case(idx, dtype, dev)
+    d = f["d"]
+    tol = 1e-5 if dtype == "f32" else 1e-8
+    N = g[0].numel()
+    nvalid = N if m is None else int(m.sum().item())
+    methods = []
+    if alg1:
+        methods.append((f"alg1 max_cg={CONV_MAX_CG}", lambda: omni.solve(g[0], g[1], g[2], m, d, tol, 400000, CONV_MAX_CG)))
+    methods.append(("direct (CG on L P = S)", lambda: omni.solve_direct(g[0], g[1], g[2], m, d, tol, 20, 30000)))
+    methods.append(("cascade levels=4", lambda: omni.solve_cascade(g[0], g[1], g[2], m, d, tol, 20, 30000, levels=4)))
+    if hasattr(omni, "solve_pcg"):
+        methods.append(("pcg (multigrid-preconditioned CG on L P = S)", lambda: omni.solve_pcg(g[0], g[1], g[2], m, d, tol, 20, 2000)))
+    out = []
+    omni.solve(g[0], g[1], g[2], m, d, tol, 1, 2)          # pool / module warm-up
+    for name, fn in methods:
+        sec, (P, info) = _timed(fn)
+        Pn = P.double().cpu().numpy()
+        valid = ~np.isnan(Pn)
+        a, b = Pn[valid] - Pn[valid].mean(), f["P"][valid] - f["P"][valid].mean()
+        out.append({"workload": f"configs[{idx}] {f['kind']} {'x'.join(str(x) for x in f['shape'])} {dtype}", "method": name,
+                    "tol": tol, "seconds": sec, "outer_iters": info["outer_iters"], "cg_iters": info["cg_iters_total"],
+                    "status": info["status"], "eps_R_gpu": info["eps_R_final"],
+                    "eps_R_oracle": oracle_eps_R(f, g, P.cpu().numpy()),
+                    "updates_per_s_whole_call": nvalid * info["cg_iters_total"] / sec,
+                    "rel_l2_vs_analytic_P": float(np.linalg.norm(a - b) / np.linalg.norm(b))})
+    return out
 
 
 def main():
@@ -225,6 +369,7 @@ def main():
     workload = f"configs[{args.config}] {cfg['kind']} {n}^{ndim} {dtype} noise={cfg['noise']}"
     config = {"workload": workload, "step": f"omni_solve tol={'1e-5' if dtype == 'f32' else '1e-8'} "
               f"max_outer={STEP_MAX_OUTER} max_cg={STEP_MAX_CG} (fixed caps)", "parallelism": f"replicas x{world}",
+              "units": "valid grid points x CG iterations",
               "l2": "inputs larger than L2 (no flush)" if n ** ndim * (4 if dtype == "f32" else 8) > 126e6
               else "CG state fits L2: numbers are L2-resident, flushed between steps by the solve's own setup passes"}
 
@@ -265,6 +410,7 @@ def main():
     d = f["d"]
     tol = 1e-5 if dtype == "f32" else 1e-8
     N = g[0].numel()
+    nvalid = N if m is None else int(m.sum().item())      # grid-point updates count VALID cells (masked cells do no work)
     esz = 4 if dtype == "f32" else 8
     P = torch.empty_like(g[0])
 
@@ -278,7 +424,7 @@ def main():
     for _ in range(max(args.warmup - 1, 0)):
         step()
     torch.cuda.synchronize()
-    units_per_step = N * info["cg_iters_total"]
+    units_per_step = nvalid * info["cg_iters_total"]
 
     def barrier():
         if world > 1:
@@ -327,15 +473,16 @@ def main():
     k4_passes = (3 * n_even + 6 * n_odd - (1 if n_odd else 0)) / STEP_MAX_CG
     alg4, alg3 = k4_passes * esz * N, 3 * esz * N
     ach = alg4 / t4 / 1e9 if t4 > 0 else 0.0
+    traffic, traffic_src = k4_traffic(args.config, dtype, n_even, n_odd)
     roofline = {"bound": "hbm", "kernel": "K4 tma_kernel<OpT4> (operator recomputed + axpys + r.r)",
                 "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak, "peak_source": peak_src,
-                "traffic": k4_traffic(NCU_TRAFFIC_K4.get((args.config, dtype)), n_even, n_odd),
+                "traffic": traffic, "traffic_source": traffic_src,
                 "algorithmic_bytes_per_launch": alg4, "k4_passes_avg": k4_passes, "us_per_launch": t4 * 1e6,
                 "k3": {"achieved": alg3 / t3 / 1e9 if t3 > 0 else 0.0, "us_per_launch": t3 * 1e6,
                        "algorithmic_bytes_per_launch": alg3},
                 "cg_iteration": {"us": (t3 + t4) * 1e6, "achieved": (alg3 + alg4) / (t3 + t4) / 1e9 if t3 + t4 > 0 else 0.0,
                                  "frac": (alg3 + alg4) / (t3 + t4) / 1e9 / peak if t3 + t4 > 0 else 0.0,
-                                 "updates_per_s_in_loop": N / (t3 + t4) if t3 + t4 > 0 else 0.0},
+                                 "updates_per_s_in_loop": nvalid / (t3 + t4) if t3 + t4 > 0 else 0.0},
                 "k2_us_per_launch": k2_ms / max(k2_n, 1) * 1e3,
                 "share_of_step": {"K2": k2_ms, "K3": k3_ms, "K4": k4_ms}}
 
@@ -353,6 +500,17 @@ def main():
                          "eps_R": info["eps_R_final"], "status": info["status"]},
            "roofline": roofline}
     if world == 1:
+        if not args.no_extras:
+            # the rest of BASELINE.json's metric, same run: the CG loop of the other 3D configs and the time to a
+            # converged P of every config x dtype (sections per_config / converged)
+            out["per_config"], out["converged"] = [], []
+            for (ci, cd) in ALL_CASES:
+                cache = (f, g, m) if (ci, cd) == (args.config, dtype) else _load_case(ci, cd, dev)
+                if ci >= 1:
+                    out["per_config"].append(per_config_entry(ci, cd, dev, peak, cache))
+                out["converged"] += converged_entries(ci, cd, dev, cache)
+                del cache
+                torch.cuda.empty_cache()
         del g, P
         torch.cuda.empty_cache()
         v, cores, desc, _ = run_oracle(f, dtype, 1, 0)

@@ -3,6 +3,7 @@
 // loop driver (CUDA graph with device-side conditional WHILE nodes, or a host-driven debug loop).
 #include "omni_tma.cuh"
 #include "omni_persist.cuh"
+#include "omni_loop.cuh"
 #include "../../include/omni.h"
 
 #include <algorithm>
@@ -30,6 +31,9 @@ using namespace omni;
 #define OMNI_TAPER_MIN 24    // and the shortest segment
 #endif
 #define OMNI_PERSIST_MAX_CELLS 1500000LL   // automatic mode: grids up to this many padded cells take the persistent loop
+#ifndef OMNI_LOOPK_MAX_CELLS
+#define OMNI_LOOPK_MAX_CELLS 0LL           // ... and up to this many the cooperative tile-loop kernel (omni_loop.cuh, loop mode 4), if its grid fits one wave; 0: only on request
+#endif
 #define OMNI_PERSIST_SMALL_CELLS 65536LL   // persistent loop: 512-thread CTAs up to here, 1024-thread CTAs above
 
 namespace {
@@ -337,6 +341,7 @@ __global__ void init_scalars_kernel(Scalars* sc, double tol, int max_outer, int 
     s.hist = hist; s.hist_k = hist_k; s.hist_cap = hist_cap; s.hist_n = 0;
     s.inner_go = 0; s.outer_go = 1; s.status = ST_OK;
     s.dzero = 1;                     // no CG iteration has run yet: the first K2 takes delta as zero
+    s.bar_count = 2;                 // grid barrier of the loop kernel: set 0, tag 1 against zeroed slots (omni_persist.cuh)
     *sc = s;
 }
 
@@ -575,6 +580,108 @@ cudaError_t launch_flush(const Geom& g, const Workspace<T>& w, cudaStream_t st)
     return cudaGetLastError();
 }
 
+// longest wait at a grid barrier of the persistent loop: 30 s by default (a healthy grid that is merely descheduled
+// on a time-shared GPU must not be reported as an error), OMNI_BARRIER_TIMEOUT_S overrides
+unsigned long long barrier_timeout_ns()
+{
+    static unsigned long long v = 0;
+    if (v == 0) {
+        const char* e = getenv("OMNI_BARRIER_TIMEOUT_S");
+        const double s = e ? atof(e) : 30.0;
+        v = (unsigned long long)((s > 0.001 ? s : 30.0) * 1e9);
+    }
+    return v;
+}
+
+// ---- cooperative tile-loop kernel (omni_loop.cuh): the whole of Alg. 1 in one launch of the TMA pipeline
+template <typename T, bool LOP> struct LoopK {
+    using A2 = K2<T>;
+    using A = K3<T, LOP>;
+    using B = K4<T, LOP>;
+    static constexpr int MINB = (sizeof(T) == 8) ? 2 : OMNI_MINB;            // fp64: K4's registers allow 2 CTAs per SM
+    static constexpr int S34 = ((int)A::SMEM_BYTES > (int)B::SMEM_BYTES ? (int)A::SMEM_BYTES : (int)B::SMEM_BYTES);
+    static constexpr int SMEM = (S34 > (int)A2::SMEM_BYTES ? S34 : (int)A2::SMEM_BYTES) + 128;
+    static auto kernel() { return tma_loop_kernel<A2, A, B, MINB>; }
+};
+
+// one column (tile x z segment) per CTA, all CTAs resident at once: segments = resident slots / tiles, at least
+// OMNI_LOOPK_MINZ planes each.  Returns false if the tiles alone exceed the slots (the caller takes the graph loop).
+#ifndef OMNI_LOOPK_MINZ
+#define OMNI_LOOPK_MINZ 6
+#endif
+template <typename T, bool LOP>
+bool loop_config(const Geom& g, MarchCfg& c)
+{
+    using L = LoopK<T, LOP>;
+    using TG = typename L::A::TG;
+    static std::mutex mu;
+    static int slots_cache[MAX_DEVICES] = {};
+    const DevInfo di = device_info();
+    if (!di.coop) return false;
+    int slots = 0;
+    {
+        std::lock_guard<std::mutex> lk(mu);
+        const bool cached = di.dev >= 0 && di.dev < MAX_DEVICES;
+        if (cached) slots = slots_cache[di.dev];
+        if (slots == 0) {
+            int occ = 0;
+            cudaFuncSetAttribute(L::kernel(), cudaFuncAttributeMaxDynamicSharedMemorySize, L::SMEM);
+            cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, L::kernel(), TG::NTHR, L::SMEM);
+            cudaGetLastError();
+            slots = occ < 1 ? -1 : di.sms * occ;
+            if (cached) slots_cache[di.dev] = slots;
+        }
+    }
+    const int ntx = (g.px + TG::BX - 1) / TG::BX, nty = (g.ny + TG::BY - 1) / TG::BY;
+    const long long tiles = (long long)ntx * nty;
+    if (slots < 1 || tiles > slots || tiles > PERSIST_MAX_CTAS) return false;
+    int nseg = (int)(slots / tiles);
+#ifdef OMNI_TUNING
+    if (const char* ev = getenv("OMNI_LOOPK_NSEG")) { const int v = atoi(ev); if (v >= 1 && v < nseg) nseg = v; }
+#endif
+    if (nseg > g.nz / OMNI_LOOPK_MINZ) nseg = g.nz / OMNI_LOOPK_MINZ;
+    if (nseg < 1) nseg = 1;
+    if (tiles * nseg > PERSIST_MAX_CTAS) nseg = (int)(PERSIST_MAX_CTAS / tiles);
+    c.zs.n = 0;
+    c.zs.zlen = (g.nz + nseg - 1) / nseg;
+    nseg = (g.nz + c.zs.zlen - 1) / c.zs.zlen;
+    c.grid = dim3((unsigned)(tiles * nseg), 1, 1);
+    c.block = dim3(TG::NTHR, 1, 1);
+    return true;
+}
+
+// Returns -100 if the grid does not fit one wave on this device or cannot be launched cooperatively (the caller then
+// takes the graph loop).
+template <typename T, bool LOP>
+int run_loop_loopk(const Geom& g, const Workspace<T>& w, const HostConst& H, const Coef<T>& K, cudaStream_t st)
+{
+    using L = LoopK<T, LOP>;
+    MarchCfg c;
+    if (!loop_config<T, LOP>(g, c)) return -100;
+    TmaSet maps;
+    if (!make_tma_set<T>(g, w, maps)) return OMNI_ERR_CUDA;
+    CondHandles ch{ 0, 0, 0 };
+    LoopArgs<typename L::A2, typename L::A, typename L::B> a;
+    a.a2 = k2_args<T>(g, w, H, ch, 1);
+    a.a3 = k3_args<T, LOP>(w, K, ch);
+    a.a4 = k4_args<T, LOP>(w, K, ch);
+    a.slots = w.slots;
+    a.timeout_ns = barrier_timeout_ns();
+    CK(cudaMemsetAsync(w.slots, 0, (size_t)8 * c.grid.x * sizeof(double), st));
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = c.grid; cfg.blockDim = c.block; cfg.dynamicSmemBytes = L::SMEM; cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeCooperative;
+    attr[0].val.cooperative = 1;
+    cfg.attrs = attr; cfg.numAttrs = 1;
+    if (cudaLaunchKernelEx(&cfg, L::kernel(), g, c.zs, a, maps) != cudaSuccess) {
+        cudaGetLastError();
+        return -100;
+    }
+    g_launches.fetch_add(1, std::memory_order_relaxed);
+    return OMNI_OK;
+}
+
 // Host-driven loop (debug / profiling): one synchronisation per outer iteration (plus one per 16 CG iterations).
 template <typename T, bool LOP>
 int run_loop_host(const Geom& g, const Workspace<T>& w, const HostConst& H, const Coef<T>& K, int max_outer, int max_cg,
@@ -664,7 +771,7 @@ int run_loop_graph(const Geom& g, const Workspace<T>& w, const HostConst& H, con
         cudaGraphConditionalHandle hOuter, hInner;
         if (cudaGraphConditionalHandleCreate(&hOuter, G, 1, cudaGraphCondAssignDefault) != cudaSuccess) break;
         if (cudaGraphConditionalHandleCreate(&hInner, G, 0, cudaGraphCondAssignDefault) != cudaSuccess) break;
-        CondHandles ch{ (unsigned long long)hOuter, (unsigned long long)hInner, 1 };
+        CondHandles ch{ (unsigned long long)hOuter, (unsigned long long)hInner, 3 };
 
         cudaGraphNodeParams po = {};
         po.type = cudaGraphNodeTypeConditional;
@@ -715,19 +822,6 @@ int run_loop_graph(const Geom& g, const Workspace<T>& w, const HostConst& H, con
     if (G) cudaGraphDestroy(G);
     if (cap) cudaStreamDestroy(cap);
     return rc;
-}
-
-// longest wait at a grid barrier of the persistent loop: 30 s by default (a healthy grid that is merely descheduled
-// on a time-shared GPU must not be reported as an error), OMNI_BARRIER_TIMEOUT_S overrides
-unsigned long long barrier_timeout_ns()
-{
-    static unsigned long long v = 0;
-    if (v == 0) {
-        const char* e = getenv("OMNI_BARRIER_TIMEOUT_S");
-        const double s = e ? atof(e) : 30.0;
-        v = (unsigned long long)((s > 0.001 ? s : 30.0) * 1e9);
-    }
-    return v;
 }
 
 // Persistent loop: the whole iteration in one cooperative launch (omni_persist.cuh).  Returns -100 if the device cannot
@@ -792,6 +886,17 @@ long long persist_max_cells()
     return v;
 }
 
+long long loopk_max_cells()
+{
+    static long long v = -1;
+    if (v < 0) {
+        const char* e = getenv("OMNI_LOOPK_MAX_CELLS");
+        v = e ? atoll(e) : OMNI_LOOPK_MAX_CELLS;
+        if (v < 0) v = 0;
+    }
+    return v;
+}
+
 bool valid_common(int nx, int ny, int nz, double dx, double dy, double dz, double tol, int max_outer, int max_cg)
 {
     if (nx < 1 || ny < 1 || nz < 1) return false;
@@ -834,10 +939,14 @@ int solve_ws(int nx, int ny, int nz, double dx, double dy, double dz, const T* g
     }
 
     int mode = g_loop_mode.load();
-    if (mode == 0) mode = (g.npad <= persist_max_cells()) ? 3 : 2;
+    if (mode == 0) mode = (g.npad <= persist_max_cells()) ? 3 : (g.npad <= loopk_max_cells()) ? 4 : 2;
     // lop: the CG kernels apply L instead of M (omni_solve_direct); everything else -- K2, scalars, loop control -- is shared
     if (mode == 3) {
         rc = lop ? run_loop_persist<T, true>(g, w, H, K, st) : run_loop_persist<T, false>(g, w, H, K, st);
+        if (rc == -100) mode = 2;
+    }
+    if (mode == 4) {
+        rc = lop ? run_loop_loopk<T, true>(g, w, H, K, st) : run_loop_loopk<T, false>(g, w, H, K, st);
         if (rc == -100) mode = 2;
     }
     if (mode == 1) rc = lop ? run_loop_host<T, true>(g, w, H, K, max_outer, max_cg, st) : run_loop_host<T, false>(g, w, H, K, max_outer, max_cg, st);
@@ -857,6 +966,8 @@ int solve_ws(int nx, int ny, int nz, double dx, double dy, double dz, const T* g
         info->norm_S = std::sqrt(h.normS2);
         info->eps_R_final = (h.normS2 > 0.0) ? std::sqrt(h.epsR2 / h.normS2) : 0.0;
         info->status = h.status;
+        // kernels launched by the device-side loop of the graph, from its own counters: K2 + flush per outer check,
+        // K3 + K4 per CG iteration
         if (mode == 2) g_launches.fetch_add((long long)(h.normS2 > 0.0 ? 2 * h.n + 1 : 0) + 2 * h.cg_total, std::memory_order_relaxed);
         return h.status;
     }
@@ -1418,6 +1529,19 @@ int omni_debug_cta_trace(int which, unsigned long long* h_out, int n_ctas)
 }
 #endif
 
+#ifdef OMNI_TUNING
+// tuning builds only: per-CTA timeline of the loop kernel's first phases: h_out[phase][cta][3], returns the phase count
+int omni_debug_loop_trace(unsigned long long* h_out, int max_phases)
+{
+    cudaDeviceSynchronize();
+    int n = 0;
+    if (cudaMemcpyFromSymbol(&n, omni::g_loop_trace_n, sizeof(int)) != cudaSuccess) return -1;
+    if (n > max_phases) n = max_phases;
+    if (cudaMemcpyFromSymbol(h_out, omni::g_loop_trace, (size_t)n * 1024 * 3 * 8) != cudaSuccess) return -2;
+    return n;
+}
+#endif
+
 int omni_set_history(double* d_hist, int* d_cg_iters, int capacity)
 {
     if (capacity < 0 || (d_hist == nullptr && (capacity > 0 || d_cg_iters != nullptr))) return OMNI_ERR_INVALID_ARG;
@@ -1437,7 +1561,7 @@ void omni_release_memory(void)
 
 int omni_set_loop_mode(int mode)
 {
-    if (mode < 0 || mode > 3) return g_loop_mode.load();
+    if (mode < 0 || mode > 4) return g_loop_mode.load();
     return g_loop_mode.exchange(mode);
 }
 

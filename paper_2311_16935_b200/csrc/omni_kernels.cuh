@@ -86,6 +86,7 @@ struct Scalars {
     int status;        // omni_status
     int max_cg, max_outer;
     unsigned int ticket[4];
+    unsigned int bar_count;  // use count of the loop kernel's grid barrier, carried from one launch to the next (omni_loop.cuh)
     // optional residual history (omni_set_history): eps_R (Eq. 41) of every outer residual check, entry i = check i
     // and, optionally, the CG iterations the outer iteration before the check took (0 for the first check)
     double* hist;
@@ -104,7 +105,7 @@ __device__ __forceinline__ void record_history(Scalars* s, double epsR2, int k_p
 
 struct CondHandles {
     unsigned long long h_outer, h_inner;   // cudaGraphConditionalHandle
-    int use;                               // 1 inside the conditional-node graph
+    int use;                               // bit 0: h_outer is live (inside the conditional-node graph), bit 1: h_inner is
 };
 
 enum { ST_OK = 0, ST_NOT_CONVERGED = 1, ST_BREAKDOWN = -4 };

@@ -15,16 +15,18 @@
 #include <type_traits>
 #include "omni_kernels.cuh"
 
+#ifndef OMNI_ZIGZAG
+#define OMNI_ZIGZAG 1      // K4 marches z downwards (0: every kernel marches upwards)
+#endif
+
 namespace omni {
 
 // loop conditions of the CUDA-graph WHILE nodes, written by a kernel's last CTA (no-op outside the graph)
 __device__ __forceinline__ void set_cond(const CondHandles& h, int outer, int inner)
 {
 #if defined(__CUDA_ARCH__)
-    if (h.use) {
-        if (outer >= 0) cudaGraphSetConditional((cudaGraphConditionalHandle)h.h_outer, (unsigned)outer);
-        if (inner >= 0) cudaGraphSetConditional((cudaGraphConditionalHandle)h.h_inner, (unsigned)inner);
-    }
+    if ((h.use & 1) && outer >= 0) cudaGraphSetConditional((cudaGraphConditionalHandle)h.h_outer, (unsigned)outer);
+    if ((h.use & 2) && inner >= 0) cudaGraphSetConditional((cudaGraphConditionalHandle)h.h_inner, (unsigned)inner);
 #endif
 }
 
@@ -135,13 +137,158 @@ __device__ __forceinline__ unsigned long long dbg_timer()
 }
 #endif
 
+// (re)initialise the ring of a pass: D "full" barriers (one arrival: the producer's expect_tx) and D "empty" barriers
+// (BY arrivals: one per consumer warp).  again = the same words held the ring of an earlier pass (loop kernel); every
+// thread of the CTA has left that pass (the caller synchronises before and after).
+__device__ __forceinline__ void ring_init(uint32_t bar_s, int D, int nmax, int consumers, bool again)
+{
+    if (again)
+        for (int s = 0; s < 2 * nmax; ++s) asm volatile("mbarrier.inval.shared::cta.b64 [%0];" ::"r"(bar_s + 8 * s) : "memory");
+    for (int s = 0; s < D; ++s) { mbar_init(bar_s + 8 * s, 1); mbar_init(bar_s + 8 * (D + s), consumers); }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+}
+
+// One pass of a column -- planes [k0, k1) of tile (x0, y0) -- through the TMA ring.  Event e = 0 .. k1-k0+1 loads one
+// plane; the march runs up (plane k0-1+e) or, for Op::REV, down (plane k1-e), so that a kernel that follows another can
+// start where the other ended and find those planes still in L2 ("zig-zag").  At event e >= 2 the
+// plane of event e-1 is emitted from the three resident stages.  Called by every thread of the CTA after ring_init +
+// __syncthreads; warps only wait for data, never for each other.  acc: per-thread fp64 partials (producer warp: 0).
+template <class Op>
+__device__ __forceinline__ void run_column(const Geom& g, const typename Op::Args& a, const typename Op::Ctx& ctx,
+                                           const TmaSet& maps, uint32_t smem_s, uint32_t bar_s, int tx, int ty,
+                                           int k0, int k1, double (&acc)[Op::NACC])
+{
+    using TG = typename Op::TG;
+    constexpr int V = TG::V, BX = TG::BX, BY = TG::BY;
+    constexpr bool REV = Op::REV;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int x0 = tx * BX, y0 = ty * BY;
+    const int n = k1 - k0, E = n + 2;                 // emitted planes; events
+    const int pl0 = REV ? k1 : k0 - 1;                // plane of event 0
+    // ring depth and stage size may depend on what this launch streams (K4: DESIGN.md section 6, lazy delta)
+    const int D = Op::stages(ctx);
+    const uint32_t SB = (uint32_t)Op::stage_bytes(ctx);
+
+    if (warp == BY) {
+        // ---------------------------------------------------------------- producer warp (one elected lane)
+        if (lane == 0) {
+            int s = 0;
+            uint32_t phase = 1;                     // parity of the previous use of slot s (first pass: no wait)
+            for (int e = 0; e < E; ++e) {
+                if (e >= D) mbar_wait(bar_s + 8 * (D + s), phase);
+                const int c = REV ? pl0 - e : pl0 + e;
+                Op::produce(a, ctx, maps, smem_s + (uint32_t)s * SB, bar_s + 8 * s, x0, y0, c,
+                            (c >= k0) && (c < k1));
+                s = (s + 1 == D) ? 0 : s + 1;
+                phase ^= (s == 0);
+            }
+        }
+        return;
+    }
+    // ---------------------------------------------------------------- consumer warps: row = y0 + warp
+    const int x = x0 + lane * V, j = y0 + warp;
+    const bool out = (x < g.nx) && (j < g.ny);      // chunks made only of pad cells (x >= nx) stay zero
+    const typename Op::TC tc = Op::thread_init(g, x);
+    const int ycls = face_class(j, g.ny, g.fix[1]);  // rows next to the box faces normal to y (uniform per warp)
+    const long long rowbase = (long long)j * g.px + x;
+    const long long step = REV ? -g.pplane : g.pplane;
+    // tile-plane flag bits (a group of this tile is flagged in plane k): a CTA whose planes are all clear -- every
+    // CTA of a mask-free box -- runs the CLEAN loop, compiled without the coded path, the flag words and their
+    // branches; only CTAs next to masked cells run the general loop
+    const uint32_t* tf = a.tflags + (size_t)(ty * g.ntx + x0 / g.tbx) * g.twords;
+    uint32_t anyf = 0;
+    for (int w = k0 >> 5; w <= (k1 - 1) >> 5; ++w) {
+        uint32_t m = tf[w];
+        if (w == (k0 >> 5)) m &= ~0u << (k0 & 31);
+        if (w == ((k1 - 1) >> 5)) m &= (2u << ((k1 - 1) & 31)) - 1u;
+        anyf |= m;
+    }
+    auto run = [&](auto clean_tag) {
+        constexpr bool CLEAN = decltype(clean_tag)::value;
+        // running state instead of per-event div/mod: slot of event e, its phase bit, the shared addresses of
+        // the stages of events e-2 / e-1 / e, the cell offset of the plane of event e
+        int s = 0, sB = 0;
+        uint32_t phase = 0;
+        uint32_t a2 = smem_s, a1 = smem_s, a0 = smem_s;
+        long long off = rowbase + (long long)pl0 * g.pplane;
+        typename Op::State st;
+        // general loop only: the row's flag words of the emitted plane, the next one (and the one after, fetched now)
+        // and the chunk's stencil codes of the emitted and the next plane -- every global load is issued at least one
+        // plane before its use
+        uint32_t fwA = 0, fwB = 0, codeA[V], codeB[V];
+#pragma unroll
+        for (int i = 0; i < V; ++i) codeA[i] = codeB[i] = 0u;
+        auto flag_word = [&](long long cell) { return a.flags[(cell >> 2) >> 5]; };
+        auto flag_bit = [&](uint32_t w, long long cell) { return (w >> (unsigned)((cell >> 2) & 31)) & 1u; };
+        if (!CLEAN && out) {
+            const long long c0 = off + step;          // first emitted plane
+            fwA = flag_word(c0);
+            if (n > 1) fwB = flag_word(c0 + step);
+            if (flag_bit(fwA, c0)) Op::load_codes(a, c0, codeA);
+        }
+        // two events per trip: half of the ring / window rotation becomes register renaming (+2 % on the fp64
+        // kernels at 256^3, +0.5 % at 500^3 fp32; three per trip is slower: profiles/r1_tile_variants.md)
+#pragma unroll 2
+        for (int e = 0; e < E; ++e) {
+            mbar_wait(bar_s + 8 * s, phase);
+            Op::advance(st, ctx, a0, warp, lane);
+            if (e >= 2) {                        // emit the plane of event e-1 from the stages of events e-2, e-1, e
+                const int i = e - 2;             // index of the emitted plane in march order
+                const int kp = REV ? k1 - 1 - i : k0 + i;
+                const int zcls = face_class(kp, g.nz, g.fix[2]);
+                const long long idx = off - step;
+                uint32_t fb = 0, fwC = 0;
+                if (!CLEAN && out) {
+                    fb = flag_bit(fwA, idx);
+                    if (i + 2 < n) fwC = flag_word(idx + 2 * step);
+                    if (i + 1 < n && flag_bit(fwB, off)) Op::load_codes(a, off, codeB);
+                }
+                // stage of plane kp-1 (B), of plane kp, of plane kp+1 (F)
+                Op::template emit<CLEAN>(a, ctx, st, idx, REV ? a0 : a2, a1, REV ? a2 : a0, warp, lane, out, fb, codeA, tc,
+                                         ycls, zcls, acc);
+                if (!CLEAN) {
+                    fwA = fwB; fwB = fwC;
+#pragma unroll
+                    for (int q = 0; q < V; ++q) codeA[q] = codeB[q];
+                }
+                __syncwarp();
+                if (lane == 0) mbar_arrive(bar_s + 8 * (D + sB));
+                sB = (sB + 1 == D) ? 0 : sB + 1;
+            }
+            off += step;
+            a2 = a1; a1 = a0;
+            s = (s + 1 == D) ? 0 : s + 1;
+            phase ^= (s == 0);
+            a0 = smem_s + (uint32_t)s * SB;
+        }
+    };
+    if (anyf) run(std::false_type{}); else run(std::true_type{});
+}
+
+// tile and z segment of a CTA; Op::REV kernels take their CTAs in the opposite order (high z first, z table mirrored:
+// the long segments of a tapered schedule still come first)
+template <bool REV>
+__device__ __forceinline__ void cta_column(const Geom& g, const ZSeg& zs, int& tx, int& ty, int& k0, int& k1)
+{
+    const int bz = blockIdx.z;
+    int lo = zs.n ? zs.k[bz] : bz * zs.zlen;
+    int hi = zs.n ? zs.k[bz + 1] : min(g.nz, lo + zs.zlen);
+    if (REV) {
+        tx = gridDim.x - 1 - blockIdx.x; ty = gridDim.y - 1 - blockIdx.y;
+        k0 = g.nz - hi; k1 = g.nz - lo;
+    } else {
+        tx = blockIdx.x; ty = blockIdx.y;
+        k0 = lo; k1 = hi;
+    }
+}
+
 template <class Op>
 __global__ void __launch_bounds__(Op::TG::NTHR, Op::MINB)
 tma_kernel(const Geom g, const ZSeg zs, const typename Op::Args a, const __grid_constant__ TmaSet maps)
 {
     using TG = typename Op::TG;
-    using T = typename Op::VT;
-    constexpr int V = TG::V, BX = TG::BX, BY = TG::BY, NACC = Op::NACC;
+    constexpr int BY = TG::BY, NACC = Op::NACC;
     extern __shared__ __align__(128) char smem_raw[];
     __shared__ double red[NACC][BY + 1];
     __shared__ int is_last;
@@ -158,116 +305,17 @@ tma_kernel(const Geom g, const ZSeg zs, const typename Op::Args a, const __grid_
     char* smem = reinterpret_cast<char*>((reinterpret_cast<uintptr_t>(smem_raw) + 127) & ~uintptr_t(127));
     const uint32_t smem_s = (uint32_t)__cvta_generic_to_shared(smem);
     const uint32_t bar_s = (uint32_t)__cvta_generic_to_shared(bars);
-
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int x0 = blockIdx.x * BX, y0 = blockIdx.y * BY;
-    const int k0 = zs.n ? zs.k[blockIdx.z] : blockIdx.z * zs.zlen;
-    const int k1 = zs.n ? zs.k[blockIdx.z + 1] : min(g.nz, k0 + zs.zlen);
-    const int E = k1 - k0 + 2;                       // events: planes k0-1 .. k1
+    int tx, ty, k0, k1;
+    cta_column<Op::REV>(g, zs, tx, ty, k0, k1);
     const typename Op::Ctx ctx(a);
-    // ring depth and stage size may depend on what this launch streams (K4: DESIGN.md section 6, lazy delta)
-    const int D = Op::stages(ctx);
-    const uint32_t SB = (uint32_t)Op::stage_bytes(ctx);
-
-    if (threadIdx.x == 0) {
-        for (int s = 0; s < D; ++s) { mbar_init(bar_s + 8 * s, 1); mbar_init(bar_s + 8 * (D + s), BY); }
-        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-    }
+    if (threadIdx.x == 0) ring_init(bar_s, Op::stages(ctx), Op::DMAX, BY, false);
     __syncthreads();
 
     double acc[NACC];
 #pragma unroll
     for (int i = 0; i < NACC; ++i) acc[i] = 0.0;
-    if (warp == BY) {
-        // ---------------------------------------------------------------- producer warp (one elected lane)
-        if (lane == 0) {
-            int s = 0;
-            uint32_t phase = 1;                     // parity of the previous use of slot s (first pass: no wait)
-            for (int e = 0; e < E; ++e) {
-                if (e >= D) mbar_wait(bar_s + 8 * (D + s), phase);
-                const int c = k0 - 1 + e;
-                Op::produce(a, ctx, maps, smem_s + (uint32_t)s * SB, bar_s + 8 * s, x0, y0, c,
-                            (c >= k0) && (c < k1));
-                s = (s + 1 == D) ? 0 : s + 1;
-                phase ^= (s == 0);
-            }
-        }
-    } else {
-        // ---------------------------------------------------------------- consumer warps: row = y0 + warp
-        const int x = x0 + lane * V, j = y0 + warp;
-        const bool out = (x < g.nx) && (j < g.ny);      // chunks made only of pad cells (x >= nx) stay zero
-        const typename Op::TC tc = Op::thread_init(g, x);
-        const int ycls = face_class(j, g.ny, g.fix[1]);  // rows next to the box faces normal to y (uniform per warp)
-        const long long rowbase = (long long)j * g.px + x;
-        // tile-plane flag bits (a group of this tile is flagged in plane k): a CTA whose planes are all clear -- every
-        // CTA of a mask-free box -- runs the CLEAN loop, compiled without the coded path, the flag words and their
-        // branches; only CTAs next to masked cells run the general loop
-        const uint32_t* tf = a.tflags + (size_t)(blockIdx.y * g.ntx + x0 / g.tbx) * g.twords;
-        uint32_t anyf = 0;
-        for (int w = k0 >> 5; w <= (k1 - 1) >> 5; ++w) {
-            uint32_t m = tf[w];
-            if (w == (k0 >> 5)) m &= ~0u << (k0 & 31);
-            if (w == ((k1 - 1) >> 5)) m &= (2u << ((k1 - 1) & 31)) - 1u;
-            anyf |= m;
-        }
-        auto run = [&](auto clean_tag) {
-            constexpr bool CLEAN = decltype(clean_tag)::value;
-            // running state instead of per-event div/mod: slot of event e, its phase bit, the shared addresses of
-            // the stages of events e-2 / e-1 / e, the cell offset of plane c
-            int s = 0, sB = 0;
-            uint32_t phase = 0;
-            uint32_t aB = smem_s, aC = smem_s, aF = smem_s;
-            long long off = rowbase + (long long)(k0 - 1) * g.pplane;
-            typename Op::State st;
-            // general loop only: the row's flag words of the planes kp, kp+1 (and kp+2, fetched now) and the chunk's
-            // stencil codes of planes kp and kp+1 -- every global load is issued at least one plane before its use
-            uint32_t fwA = 0, fwB = 0, codeA[V], codeB[V];
-#pragma unroll
-            for (int i = 0; i < V; ++i) codeA[i] = codeB[i] = 0u;
-            auto flag_word = [&](long long cell) { return a.flags[(cell >> 2) >> 5]; };
-            auto flag_bit = [&](uint32_t w, long long cell) { return (w >> (unsigned)((cell >> 2) & 31)) & 1u; };
-            if (!CLEAN && out) {
-                const long long c0 = rowbase + (long long)k0 * g.pplane;
-                fwA = flag_word(c0);
-                if (k0 + 1 < k1) fwB = flag_word(c0 + g.pplane);
-                if (flag_bit(fwA, c0)) Op::load_codes(a, c0, codeA);
-            }
-            // two events per trip: half of the ring / window rotation becomes register renaming (+2 % on the fp64
-            // kernels at 256^3, +0.5 % at 500^3 fp32; three per trip is slower: profiles/r1_tile_variants.md)
-#pragma unroll 2
-            for (int e = 0; e < E; ++e) {
-                mbar_wait(bar_s + 8 * s, phase);
-                Op::advance(st, ctx, aF, warp, lane);
-                if (e >= 2) {                        // emit plane c-1 from stages e-2 (B), e-1 (centre), e (F)
-                    const int kp = k0 + e - 2;       // the plane being emitted
-                    const int zcls = face_class(kp, g.nz, g.fix[2]);
-                    const long long idx = off - g.pplane;
-                    uint32_t fb = 0, fwC = 0;
-                    if (!CLEAN && out) {
-                        fb = flag_bit(fwA, idx);
-                        if (kp + 2 < k1) fwC = flag_word(idx + 2 * g.pplane);
-                        if (kp + 1 < k1 && flag_bit(fwB, off)) Op::load_codes(a, off, codeB);
-                    }
-                    Op::template emit<CLEAN>(a, ctx, st, idx, aB, aC, aF, warp, lane, out, fb, codeA, tc, ycls, zcls, acc);
-                    if (!CLEAN) {
-                        fwA = fwB; fwB = fwC;
-#pragma unroll
-                        for (int i = 0; i < V; ++i) codeA[i] = codeB[i];
-                    }
-                    __syncwarp();
-                    if (lane == 0) mbar_arrive(bar_s + 8 * (D + sB));
-                    sB = (sB + 1 == D) ? 0 : sB + 1;
-                }
-                off += g.pplane;
-                aB = aC; aC = aF;
-                s = (s + 1 == D) ? 0 : s + 1;
-                phase ^= (s == 0);
-                aF = smem_s + (uint32_t)s * SB;
-            }
-        };
-        if (anyf) run(std::false_type{}); else run(std::true_type{});
-    }
+    run_column<Op>(g, a, ctx, maps, smem_s, bar_s, tx, ty, k0, k1, acc);
 
     // deterministic grid reduction (all warps, the producer contributes 0)
     const unsigned int nblk = gridDim.x * gridDim.y * gridDim.z;
@@ -330,13 +378,15 @@ struct OpT3 {
     using TG = TileGeom<T, BY_>;
     enum { V = TG::V, D = D_, DMAX = D_, MINB = MINB_, NACC = 1, TICKET = 0, STAGE_BYTES = 2 * TG::TILE_H,
            SMEM_BYTES = D_ * STAGE_BYTES, BOX_H = (BY_ + 2) * TG::PITCH_H };
+    static constexpr bool REV = false;       // marches z upwards
     struct Args {
         T* pbuf[2]; const uint32_t* wcode; const uint8_t* link; const uint32_t* flags; const uint32_t* tflags;
         Coef<T> K; Scalars* sc; double* partial; CondHandles cond;
     };
     struct Ctx {
         T beta; int par; T* pnew;
-        __device__ Ctx(const Args& a) { beta = (T)a.sc->beta; par = a.sc->k & 1; pnew = a.pbuf[par ^ 1]; }
+        __device__ Ctx(const Args& a) : Ctx(a, a.sc->beta, a.sc->k) {}
+        __device__ Ctx(const Args& a, double beta_, int k) { beta = (T)beta_; par = k & 1; pnew = a.pbuf[par ^ 1]; }
     };
     using TC = XEdge;
     __device__ static int stages(const Ctx&) { return D; }
@@ -431,6 +481,9 @@ struct OpT4 {
            STAGE_ODD = TG::TILE_H + 3 * TG::TILE_C, STAGE_EVEN = TG::TILE_H + TG::TILE_C,
            D_ODD = DO_, D_EVEN = (DO_ * STAGE_ODD) / STAGE_EVEN, DMAX = D_EVEN, SMEM_BYTES = DO_ * STAGE_ODD,
            BOX_H = (BY_ + 2) * TG::PITCH_H };
+    // marches z downwards, CTAs in the opposite order: K4 starts on the planes K3 has just written (p_new) and read (r),
+    // the next K3 on the planes K4 has just written (r) -- what the L2 still holds of them is not fetched from DRAM
+    static constexpr bool REV = OMNI_ZIGZAG != 0;
     struct Args {
         T* r; T* delta; int p_fixed;      // p_fixed >= 0: read p from pbuf[p_fixed] (omni_apply_M), else by parity
         const uint32_t* wcode; const uint8_t* link; const uint32_t* flags; const uint32_t* tflags;
@@ -439,11 +492,11 @@ struct OpT4 {
     };
     struct Ctx {
         T alpha, alpha_prev; int pidx, pold; bool odd, first, step;
-        __device__ Ctx(const Args& a)
+        __device__ Ctx(const Args& a) : Ctx(a, a.sc->alpha, a.sc->alpha_prev, a.sc->k) {}
+        __device__ Ctx(const Args& a, double alpha_, double alpha_prev_, int k)
         {
-            const int k = a.sc->k;
-            alpha = (T)a.sc->alpha;
-            alpha_prev = (T)a.sc->alpha_prev;
+            alpha = (T)alpha_;
+            alpha_prev = (T)alpha_prev_;
             step = (a.q_out != nullptr);
             odd = (k & 1) != 0;
             first = (k == 1);                        // first delta write of this inner solve: delta counts as zero
@@ -586,6 +639,7 @@ struct OpT2 {
     };
     enum { V = 2, D = D_, DMAX = D_, MINB = MINB_, NACC = 2, TICKET = 2, STAGE_BYTES = TG::TILE_P + TG::TILE_D + TG::TILE_S,
            SMEM_BYTES = D_ * STAGE_BYTES };
+    static constexpr bool REV = false;
     struct Args {
         double* Pbuf[2]; T* r; const uint8_t* link; const uint32_t* flags; const uint32_t* tflags;
         double t[3]; Scalars* sc; double* partial; CondHandles cond;
@@ -593,10 +647,11 @@ struct OpT2 {
     };
     struct Ctx {
         int par; double* Pout; bool dz;
-        __device__ Ctx(const Args& a)
+        __device__ Ctx(const Args& a) : Ctx(a, a.sc->n, a.sc->dzero) {}
+        __device__ Ctx(const Args& a, int n, int dzero)
         {
-            par = a.fold_delta ? (a.sc->n & 1) : 0; Pout = a.Pbuf[par ^ 1];
-            dz = !a.fold_delta || a.sc->dzero != 0;       // delta counts as zero: neither loaded nor added
+            par = a.fold_delta ? (n & 1) : 0; Pout = a.Pbuf[par ^ 1];
+            dz = !a.fold_delta || dzero != 0;             // delta counts as zero: neither loaded nor added
         }
     };
     // thread constant: link bytes of an unflagged chunk as far as x decides (box faces normal to x, pad cells)

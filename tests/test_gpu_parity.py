@@ -80,7 +80,8 @@ def test_source_and_operator_steps(oracle, dtype, shape, frac):
     assert eps == pytest.approx(np.linalg.norm(r_or) / np.linalg.norm(S_or), rel=1e-5 if dtype == "f32" else 1e-10)
 
 
-LOOPS = {"graph": 2, "persistent": 3}       # omni_set_loop_mode; the default (0) picks one of the two by grid size
+# omni_set_loop_mode; the default (0) picks one of the three by grid size
+LOOPS = {"graph": 2, "persistent": 3, "loopk": 4}
 
 
 @pytest.fixture(params=list(LOOPS))
@@ -317,9 +318,9 @@ def test_graph_and_host_loops_are_bit_identical():
             res.append((P.cpu().numpy(), info))
         assert res[0][1] == res[1][1]
         assert np.array_equal(res[0][0], res[1][0], equal_nan=True)
-        # determinism: same call twice, same bits -- in the graph loop and in the persistent kernel, whose reductions
-        # run in another (fixed) order: same iteration counts, fields equal to rounding
-        for mode in (2, 3):
+        # determinism: same call twice, same bits -- in the graph loop, in the persistent kernel and in the cooperative
+        # tile-loop kernel, whose reductions run in another (fixed) order: same iteration counts, fields equal to rounding
+        for mode in (2, 3, 4):
             prev = omni.set_loop_mode(mode)
             try:
                 Pa, ia = omni.solve(g_dev[0], g_dev[1], g_dev[2], m_dev, f["d"], 1e-4, 50, 12)
