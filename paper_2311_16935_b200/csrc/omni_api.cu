@@ -17,14 +17,24 @@
 
 using namespace omni;
 
+// tile shape and pipeline depths of K2 / K3 / K4 (each can be overridden at build time for sweeps)
 #ifndef OMNI_BY
-#define OMNI_BY 8
-#define OMNI_D3 6
-#define OMNI_D4 4      // K4 ring depth in its 4-array iterations ({p_h, r, p_old, delta}); 7 in the 2-array ones
-#define OMNI_MINB 3
-#ifndef OMNI_D4_F64
-#define OMNI_D4_F64 6   // fp64 K4 runs 2 CTAs per SM (registers): deeper ring from the same shared memory
+#define OMNI_BY 8          // rows of a tile
 #endif
+#ifndef OMNI_R
+#define OMNI_R 1           // rows of a tile per consumer warp (2 and 4 share N / S values in registers and halve the control overhead, but the halved warp count costs more: profiles/r2_loop_and_rows.md)
+#endif
+#ifndef OMNI_D3
+#define OMNI_D3 6          // K3 ring depth
+#endif
+#ifndef OMNI_D4
+#define OMNI_D4 4          // K4 ring depth in its 4-array iterations ({p_h, r, p_old, delta}); more in the 2-array ones
+#endif
+#ifndef OMNI_MINB
+#define OMNI_MINB 3        // CTAs per SM the kernels are compiled for
+#endif
+#ifndef OMNI_D4_F64
+#define OMNI_D4_F64 6      // fp64 K4 runs fewer CTAs per SM (registers): deeper ring from the same shared memory
 #endif
 #ifndef OMNI_TAPER_F
 #define OMNI_TAPER_F 0.5     // tapered z segments (tma_config): fraction of the remaining planes per slot; 0 = uniform segments
@@ -352,9 +362,12 @@ struct MarchCfg { dim3 grid, block; ZSeg zs; };
 // K2 / K3 / K4: TMA + mbarrier pipeline (omni_tma.cuh): 512-byte x 8-row tiles, 8 consumer warps + 1 producer warp,
 // several CTAs per SM (shared memory: K3 6 stages x 10.8 KB, K4 4 x 17.4 KB or 7 x 9.4 KB by iteration parity,
 // K2 5 x 10.3 KB fp32 / 4 x 14.8 KB fp64).
-template <typename T, bool LOP = false> using K3 = OpT3<T, OMNI_BY, OMNI_D3, OMNI_MINB, LOP>;
-template <typename T, bool LOP = false> using K4 = OpT4<T, OMNI_BY, (sizeof(T) == 8 ? OMNI_D4_F64 : OMNI_D4), (sizeof(T) == 8 ? 2 : OMNI_MINB), LOP>;   // fp64 K4: 72 registers spill
-template <typename T> using K2 = OpT2<T, OMNI_BY, (sizeof(T) == 8 ? 4 : 5), OMNI_MINB>;
+#ifndef OMNI_MINB_F64
+#define OMNI_MINB_F64 2    // CTAs per SM the fp64 K4 is compiled for (registers)
+#endif
+template <typename T, bool LOP = false> using K3 = OpT3<T, OMNI_BY, OMNI_R, OMNI_D3, OMNI_MINB, LOP>;
+template <typename T, bool LOP = false> using K4 = OpT4<T, OMNI_BY, OMNI_R, (sizeof(T) == 8 ? OMNI_D4_F64 : OMNI_D4), (sizeof(T) == 8 ? OMNI_MINB_F64 : OMNI_MINB), LOP>;
+template <typename T> using K2 = OpT2<T, OMNI_BY, OMNI_R, (sizeof(T) == 8 ? 4 : 5), OMNI_MINB>;
 
 
 template <class Op>
@@ -598,7 +611,7 @@ template <typename T, bool LOP> struct LoopK {
     using A2 = K2<T>;
     using A = K3<T, LOP>;
     using B = K4<T, LOP>;
-    static constexpr int MINB = (sizeof(T) == 8) ? 2 : OMNI_MINB;            // fp64: K4's registers allow 2 CTAs per SM
+    static constexpr int MINB = (sizeof(T) == 8) ? OMNI_MINB_F64 : OMNI_MINB;
     static constexpr int S34 = ((int)A::SMEM_BYTES > (int)B::SMEM_BYTES ? (int)A::SMEM_BYTES : (int)B::SMEM_BYTES);
     static constexpr int SMEM = (S34 > (int)A2::SMEM_BYTES ? S34 : (int)A2::SMEM_BYTES) + 128;
     static auto kernel() { return tma_loop_kernel<A2, A, B, MINB>; }

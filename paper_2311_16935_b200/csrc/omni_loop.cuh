@@ -35,7 +35,7 @@ __device__ int g_loop_trace_n;
 #define LOOP_TRACE_BEGIN() const unsigned long long tr0__ = dbg_timer();
 #define LOOP_TRACE_MID() const unsigned long long tr1__ = dbg_timer();
 #define LOOP_TRACE_END(ph) do { if (threadIdx.x == 0 && (ph) < 64 && blockIdx.x < 1024) { g_loop_trace[ph][blockIdx.x][0] = tr0__; \
-    g_loop_trace[ph][blockIdx.x][1] = tr1__; g_loop_trace[ph][blockIdx.x][2] = dbg_timer(); if (blockIdx.x == 0) g_loop_trace_n = (ph) + 1; } } while (0)
+    g_loop_trace[ph][blockIdx.x][1] = tr1__; g_loop_trace[ph][blockIdx.x][2] = dbg_timer(); if (blockIdx.x == 0) g_loop_trace_n = (ph) + 1; } (ph)++; } while (0)
 #else
 #define LOOP_TRACE_BEGIN()
 #define LOOP_TRACE_MID()
@@ -54,8 +54,8 @@ tma_loop_kernel(const Geom g, const ZSeg zs, const LoopArgs<K2, K3, K4> a, const
     using TG = typename K3::TG;
     using T = typename K3::VT;
     static_assert(TG::NTHR == K4::TG::NTHR && TG::BX == K4::TG::BX && TG::BY == K4::TG::BY, "K3 and K4 share the tile");
-    static_assert(K2::TG::NTHR == TG::NTHR && K2::TG::BY == TG::BY && TG::BX % K2::TG::BX == 0, "K2 tiles subdivide it in x");
-    constexpr int NT = TG::NTHR, BY = TG::BY, NW = NT / 32, V = TG::V;
+    static_assert(K2::TG::NTHR == TG::NTHR && K2::TG::BY == TG::BY && K2::TG::R == TG::R && TG::BX % K2::TG::BX == 0, "K2 tiles subdivide it in x");
+    constexpr int NT = TG::NTHR, BY = TG::BY, NCW = TG::NCW, R = TG::R, NW = NT / 32, V = TG::V;
     constexpr int XR = TG::BX / K2::TG::BX;          // K2 columns per K3 column (fp32: 2, the fp64 master pressure halves the tile)
     constexpr int NB34 = (K3::DMAX > K4::DMAX) ? K3::DMAX : K4::DMAX;
     constexpr int NBAR = (NB34 > K2::DMAX) ? NB34 : K2::DMAX;
@@ -102,7 +102,7 @@ tma_loop_kernel(const Geom g, const ZSeg zs, const LoopArgs<K2, K3, K4> a, const
             for (int h = 0; h < XR; ++h) {
                 const int tx2 = tx * XR + h;
                 if (tx2 >= ntx2) break;                                    // CTA-uniform
-                if (threadIdx.x == 0) ring_init(bar_s, K2::stages(c2), NBAR, BY, again);
+                if (threadIdx.x == 0) ring_init(bar_s, K2::stages(c2), NBAR, NCW, again);
                 again = true;
                 fence_proxy_async_global();          // the producer's TMA loads follow the acquire of the last barrier
                 __syncthreads();
@@ -112,7 +112,7 @@ tma_loop_kernel(const Geom g, const ZSeg zs, const LoopArgs<K2, K3, K4> a, const
             fence_proxy_async_global();              // this phase's stores, before the release in the barrier
             LOOP_TRACE_MID()
             if (!grid_allreduce<2, NT>(gs, a.slots, acc, tot)) { status = ST_BARRIER_TIMEOUT; break; }
-            LOOP_TRACE_END(trace_ph); trace_ph++;
+            LOOP_TRACE_END(trace_ph);
             epsR2 = tot[0];
             if (blockIdx.x == 0 && threadIdx.x == 0) record_history(sc, tot[0], k);
             if (!isfinite(tot[0])) { status = ST_BREAKDOWN; break; }
@@ -133,7 +133,7 @@ tma_loop_kernel(const Geom g, const ZSeg zs, const LoopArgs<K2, K3, K4> a, const
             {
                 const typename K3::Ctx c3(a.a3, beta, k);
                 LOOP_TRACE_BEGIN()
-                if (threadIdx.x == 0) ring_init(bar_s, K3::stages(c3), NBAR, BY, true);
+                if (threadIdx.x == 0) ring_init(bar_s, K3::stages(c3), NBAR, NCW, true);
                 fence_proxy_async_global();
                 __syncthreads();
                 double acc[1] = { 0.0 }, tot[1];
@@ -141,7 +141,7 @@ tma_loop_kernel(const Geom g, const ZSeg zs, const LoopArgs<K2, K3, K4> a, const
                 fence_proxy_async_global();
                 LOOP_TRACE_MID()
                 if (!grid_allreduce<1, NT>(gs, a.slots, acc, tot)) { status = ST_BARRIER_TIMEOUT; stop_all = true; break; }
-                LOOP_TRACE_END(trace_ph); trace_ph++;
+                LOOP_TRACE_END(trace_ph);
                 gamma = tot[0];
                 if (!(gamma > 0.0) || !isfinite(gamma)) { status = ST_BREAKDOWN; stop_all = true; break; }
                 alpha = rho / gamma;
@@ -150,7 +150,7 @@ tma_loop_kernel(const Geom g, const ZSeg zs, const LoopArgs<K2, K3, K4> a, const
             {
                 const typename K4::Ctx c4(a.a4, alpha, alpha_prev, k);
                 LOOP_TRACE_BEGIN()
-                if (threadIdx.x == 0) ring_init(bar_s, K4::stages(c4), NBAR, BY, true);
+                if (threadIdx.x == 0) ring_init(bar_s, K4::stages(c4), NBAR, NCW, true);
                 fence_proxy_async_global();
                 __syncthreads();
                 double acc[1] = { 0.0 }, tot[1];
@@ -158,7 +158,7 @@ tma_loop_kernel(const Geom g, const ZSeg zs, const LoopArgs<K2, K3, K4> a, const
                 fence_proxy_async_global();
                 LOOP_TRACE_MID()
                 if (!grid_allreduce<1, NT>(gs, a.slots, acc, tot)) { status = ST_BARRIER_TIMEOUT; stop_all = true; break; }
-                LOOP_TRACE_END(trace_ph); trace_ph++;
+                LOOP_TRACE_END(trace_ph);
                 const double rho1 = tot[0];
                 if (!isfinite(rho1)) { status = ST_BREAKDOWN; stop_all = true; break; }
                 if (k & 1) { pend = 0; } else { pend = 1; alpha_prev = alpha; }
@@ -174,19 +174,23 @@ tma_loop_kernel(const Geom g, const ZSeg zs, const LoopArgs<K2, K3, K4> a, const
         // (an even last CG iteration): delta += alpha_prev p_{k-1} on the own column -- every thread touches the chunks
         // it wrote itself in K3 / K4 -- then a barrier, because K2 reads delta with its halo through TMA
         if (pend) {
-            if (warp < BY) {
-                const int x = tx * TG::BX + lane * V, j = ty * BY + warp;
-                if (x < g.nx && j < g.ny) {
-                    const T* __restrict__ p = a.a3.pbuf[((k - 1) & 1) ^ 1];
-                    const T al = (T)alpha_prev;
-                    long long c = (long long)j * g.px + x + (long long)k0 * g.pplane;
-                    for (int kk = k0; kk < k1; ++kk, c += g.pplane) {
-                        T pv[V], dv[V];
-                        ld_chunk<T, V>(p + c, pv);
-                        if (k == 1) zero_chunk<T, V>(dv); else ld_chunk<T, V>(a.a4.delta + c, dv);
+            if (warp < NCW) {
+                const int x = tx * TG::BX + lane * V;
+                const T* __restrict__ p = a.a3.pbuf[((k - 1) & 1) ^ 1];
+                const T al = (T)alpha_prev;
 #pragma unroll
-                        for (int i = 0; i < V; ++i) dv[i] += al * pv[i];
-                        st_chunk<T, V>(a.a4.delta + c, dv);
+                for (int r = 0; r < R; ++r) {
+                    const int j = ty * BY + warp * R + r;
+                    if (x < g.nx && j < g.ny) {
+                        long long c = (long long)j * g.px + x + (long long)k0 * g.pplane;
+                        for (int kk = k0; kk < k1; ++kk, c += g.pplane) {
+                            T pv[V], dv[V];
+                            ld_chunk<T, V>(p + c, pv);
+                            if (k == 1) zero_chunk<T, V>(dv); else ld_chunk<T, V>(a.a4.delta + c, dv);
+#pragma unroll
+                            for (int i = 0; i < V; ++i) dv[i] += al * pv[i];
+                            st_chunk<T, V>(a.a4.delta + c, dv);
+                        }
                     }
                 }
             }

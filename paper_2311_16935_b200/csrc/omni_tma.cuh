@@ -73,16 +73,19 @@ struct ZSeg {
     int k[MAXSEG + 1];
 };
 
-template <typename T, int BY_>
+template <typename T, int BY_, int R_>
 struct TileGeom {
+    static_assert(BY_ % R_ == 0, "a tile's rows are shared out evenly among its consumer warps");
     static constexpr int V = 16 / (int)sizeof(T);          // cells per lane (one 16-byte piece)
     static constexpr int BX = 32 * V;                      // 512 bytes per row
     static constexpr int BY = BY_;
+    static constexpr int R = R_;                           // rows per consumer warp (neighbouring rows: N / S values are shared in registers)
+    static constexpr int NCW = BY_ / R_;                   // consumer warps
     static constexpr int HX = 16 / (int)sizeof(T);         // x halo in cells (16 bytes: TMA box rows are 16 B multiples)
     static constexpr int PITCH_H = (BX + 2 * HX) * (int)sizeof(T);       // 544 bytes
     static constexpr int TILE_H = ((BY + 2) * PITCH_H + 127) / 128 * 128;
     static constexpr int TILE_C = BY * BX * (int)sizeof(T);              // multiple of 512
-    static constexpr int NTHR = 32 * (BY + 1);             // BY consumer warps + 1 producer warp
+    static constexpr int NTHR = 32 * (NCW + 1);            // NCW consumer warps + 1 producer warp
 };
 
 // explicit shared-space loads (generic LD through a computed pointer costs an address-space check and a longer
@@ -160,7 +163,7 @@ __device__ __forceinline__ void run_column(const Geom& g, const typename Op::Arg
                                            int k0, int k1, double (&acc)[Op::NACC])
 {
     using TG = typename Op::TG;
-    constexpr int V = TG::V, BX = TG::BX, BY = TG::BY;
+    constexpr int V = TG::V, BX = TG::BX, BY = TG::BY, R = TG::R, NCW = TG::NCW;
     constexpr bool REV = Op::REV;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int x0 = tx * BX, y0 = ty * BY;
@@ -170,7 +173,7 @@ __device__ __forceinline__ void run_column(const Geom& g, const typename Op::Arg
     const int D = Op::stages(ctx);
     const uint32_t SB = (uint32_t)Op::stage_bytes(ctx);
 
-    if (warp == BY) {
+    if (warp == NCW) {
         // ---------------------------------------------------------------- producer warp (one elected lane)
         if (lane == 0) {
             int s = 0;
@@ -186,12 +189,17 @@ __device__ __forceinline__ void run_column(const Geom& g, const typename Op::Arg
         }
         return;
     }
-    // ---------------------------------------------------------------- consumer warps: row = y0 + warp
-    const int x = x0 + lane * V, j = y0 + warp;
-    const bool out = (x < g.nx) && (j < g.ny);      // chunks made only of pad cells (x >= nx) stay zero
+    // ---------------------------------------------------------------- consumer warps: rows y0 + warp R .. + R - 1
+    const int x = x0 + lane * V, j0 = y0 + warp * R;
+    bool out[R];                                    // chunks made only of pad cells (x >= nx) stay zero
+    int ycls[R];                                    // rows next to the box faces normal to y (uniform per warp)
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+        out[r] = (x < g.nx) && (j0 + r < g.ny);
+        ycls[r] = face_class(j0 + r, g.ny, g.fix[1]);
+    }
     const typename Op::TC tc = Op::thread_init(g, x);
-    const int ycls = face_class(j, g.ny, g.fix[1]);  // rows next to the box faces normal to y (uniform per warp)
-    const long long rowbase = (long long)j * g.px + x;
+    const long long rowbase = (long long)j0 * g.px + x;
     const long long step = REV ? -g.pplane : g.pplane;
     // tile-plane flag bits (a group of this tile is flagged in plane k): a CTA whose planes are all clear -- every
     // CTA of a mask-free box -- runs the CLEAN loop, compiled without the coded path, the flag words and their
@@ -213,19 +221,27 @@ __device__ __forceinline__ void run_column(const Geom& g, const typename Op::Arg
         uint32_t a2 = smem_s, a1 = smem_s, a0 = smem_s;
         long long off = rowbase + (long long)pl0 * g.pplane;
         typename Op::State st;
-        // general loop only: the row's flag words of the emitted plane, the next one (and the one after, fetched now)
-        // and the chunk's stencil codes of the emitted and the next plane -- every global load is issued at least one
-        // plane before its use
-        uint32_t fwA = 0, fwB = 0, codeA[V], codeB[V];
+        // general loop only, per row: the flag words of the emitted plane, the next one (and the one after, fetched
+        // now) and the chunk's stencil codes of the emitted and the next plane -- every global load is issued at least
+        // one plane before its use
+        uint32_t fwA[R], fwB[R], fb[R], codeA[R][V], codeB[R][V];
 #pragma unroll
-        for (int i = 0; i < V; ++i) codeA[i] = codeB[i] = 0u;
+        for (int r = 0; r < R; ++r) {
+            fwA[r] = fwB[r] = fb[r] = 0u;
+#pragma unroll
+            for (int i = 0; i < V; ++i) codeA[r][i] = codeB[r][i] = 0u;
+        }
         auto flag_word = [&](long long cell) { return a.flags[(cell >> 2) >> 5]; };
         auto flag_bit = [&](uint32_t w, long long cell) { return (w >> (unsigned)((cell >> 2) & 31)) & 1u; };
-        if (!CLEAN && out) {
-            const long long c0 = off + step;          // first emitted plane
-            fwA = flag_word(c0);
-            if (n > 1) fwB = flag_word(c0 + step);
-            if (flag_bit(fwA, c0)) Op::load_codes(a, c0, codeA);
+        if (!CLEAN) {
+#pragma unroll
+            for (int r = 0; r < R; ++r)
+                if (out[r]) {
+                    const long long c0 = off + step + (long long)r * g.px;          // first emitted plane
+                    fwA[r] = flag_word(c0);
+                    if (n > 1) fwB[r] = flag_word(c0 + step);
+                    if (flag_bit(fwA[r], c0)) Op::load_codes(a, c0, codeA[r]);
+                }
         }
         // two events per trip: half of the ring / window rotation becomes register renaming (+2 % on the fp64
         // kernels at 256^3, +0.5 % at 500^3 fp32; three per trip is slower: profiles/r1_tile_variants.md)
@@ -238,19 +254,28 @@ __device__ __forceinline__ void run_column(const Geom& g, const typename Op::Arg
                 const int kp = REV ? k1 - 1 - i : k0 + i;
                 const int zcls = face_class(kp, g.nz, g.fix[2]);
                 const long long idx = off - step;
-                uint32_t fb = 0, fwC = 0;
-                if (!CLEAN && out) {
-                    fb = flag_bit(fwA, idx);
-                    if (i + 2 < n) fwC = flag_word(idx + 2 * step);
-                    if (i + 1 < n && flag_bit(fwB, off)) Op::load_codes(a, off, codeB);
+                if (!CLEAN) {
+#pragma unroll
+                    for (int r = 0; r < R; ++r) {
+                        uint32_t fwC = 0;
+                        fb[r] = 0;
+                        if (out[r]) {
+                            const long long cr = idx + (long long)r * g.px;
+                            fb[r] = flag_bit(fwA[r], cr);
+                            if (i + 2 < n) fwC = flag_word(cr + 2 * step);
+                            if (i + 1 < n && flag_bit(fwB[r], cr + step)) Op::load_codes(a, cr + step, codeB[r]);
+                        }
+                        fwA[r] = fwB[r]; fwB[r] = fwC;
+                    }
                 }
                 // stage of plane kp-1 (B), of plane kp, of plane kp+1 (F)
-                Op::template emit<CLEAN>(a, ctx, st, idx, REV ? a0 : a2, a1, REV ? a2 : a0, warp, lane, out, fb, codeA, tc,
-                                         ycls, zcls, acc);
+                Op::template emit<CLEAN>(a, ctx, st, idx, g.px, REV ? a0 : a2, a1, REV ? a2 : a0, warp, lane, out, fb, codeA,
+                                         tc, ycls, zcls, acc);
                 if (!CLEAN) {
-                    fwA = fwB; fwB = fwC;
 #pragma unroll
-                    for (int q = 0; q < V; ++q) codeA[q] = codeB[q];
+                    for (int r = 0; r < R; ++r)
+#pragma unroll
+                        for (int q = 0; q < V; ++q) codeA[r][q] = codeB[r][q];
                 }
                 __syncwarp();
                 if (lane == 0) mbar_arrive(bar_s + 8 * (D + sB));
@@ -288,9 +313,9 @@ __global__ void __launch_bounds__(Op::TG::NTHR, Op::MINB)
 tma_kernel(const Geom g, const ZSeg zs, const typename Op::Args a, const __grid_constant__ TmaSet maps)
 {
     using TG = typename Op::TG;
-    constexpr int BY = TG::BY, NACC = Op::NACC;
+    constexpr int NCW = TG::NCW, NACC = Op::NACC;
     extern __shared__ __align__(128) char smem_raw[];
-    __shared__ double red[NACC][BY + 1];
+    __shared__ double red[NACC][NCW + 1];
     __shared__ int is_last;
     __shared__ __align__(8) unsigned long long bars[2 * Op::DMAX];
 
@@ -309,7 +334,7 @@ tma_kernel(const Geom g, const ZSeg zs, const typename Op::Args a, const __grid_
     int tx, ty, k0, k1;
     cta_column<Op::REV>(g, zs, tx, ty, k0, k1);
     const typename Op::Ctx ctx(a);
-    if (threadIdx.x == 0) ring_init(bar_s, Op::stages(ctx), Op::DMAX, BY, false);
+    if (threadIdx.x == 0) ring_init(bar_s, Op::stages(ctx), Op::DMAX, NCW, false);
     __syncthreads();
 
     double acc[NACC];
@@ -330,7 +355,7 @@ tma_kernel(const Geom g, const ZSeg zs, const typename Op::Args a, const __grid_
 #pragma unroll
         for (int i = 0; i < NACC; ++i) {
             double s = 0.0;
-            for (int w = 0; w < BY; ++w) s += red[i][w];
+            for (int w = 0; w < NCW; ++w) s += red[i][w];
             a.partial[(size_t)i * nblk + bid] = s;
         }
         __threadfence();
@@ -359,7 +384,7 @@ tma_kernel(const Geom g, const ZSeg zs, const typename Op::Args a, const __grid_
             if (lane == 0) red[i][warp] = s;
             __syncthreads();
             s = 0.0;
-            for (int w = 0; w <= BY; ++w) s += red[i][w];
+            for (int w = 0; w <= NCW; ++w) s += red[i][w];
             tot[i] = s;
         }
         if (threadIdx.x == 0) {
@@ -372,11 +397,11 @@ tma_kernel(const Geom g, const ZSeg zs, const typename Op::Args a, const __grid_
 // ------------------------------------------------------------------------------------------------ K3 (TMA)
 // p_new = r + beta p_old evaluated from the raw r / p_old tiles wherever the stencil needs it (centre, N, S, F, B
 // chunks and the two x-halo cells); store p_new; gamma = p_new . M p_new; last CTA: alpha = rho / gamma.
-template <typename T, int BY_, int D_, int MINB_, bool LOP_ = false>
+template <typename T, int BY_, int R_, int D_, int MINB_, bool LOP_ = false>
 struct OpT3 {
     using VT = T;
-    using TG = TileGeom<T, BY_>;
-    enum { V = TG::V, D = D_, DMAX = D_, MINB = MINB_, NACC = 1, TICKET = 0, STAGE_BYTES = 2 * TG::TILE_H,
+    using TG = TileGeom<T, BY_, R_>;
+    enum { V = TG::V, R = R_, D = D_, DMAX = D_, MINB = MINB_, NACC = 1, TICKET = 0, STAGE_BYTES = 2 * TG::TILE_H,
            SMEM_BYTES = D_ * STAGE_BYTES, BOX_H = (BY_ + 2) * TG::PITCH_H };
     static constexpr bool REV = false;       // marches z upwards
     struct Args {
@@ -410,46 +435,63 @@ struct OpT3 {
 #pragma unroll
         for (int i = 0; i < V; ++i) v[i] = r[i] + beta * p[i];
     }
-    // own-chunk p_new of the last three planes: each plane's chunk is formed once (when its stage arrives) and reused
-    // as F, centre and B neighbour of three consecutive emissions
+    // own-chunk p_new of the last three planes, for each of the warp's R rows: a plane's chunks are formed once (when its
+    // stage arrives) and reused as F, centre and B neighbour of three consecutive emissions -- and, within a plane, as
+    // N / S neighbour of the rows next to them
     struct State {
-        T m[V], c[V], f[V];
-        __device__ State() { zero_chunk<T, V>(m); zero_chunk<T, V>(c); zero_chunk<T, V>(f); }
-    };
-    __device__ static void advance(State& st, const Ctx& c, uint32_t sF, int warp, int lane)
-    {
-        const int off = (warp + 1) * TG::PITCH_H + (TG::HX + lane * V) * (int)sizeof(T);
+        T m[R][V], c[R][V], f[R][V];
+        __device__ State()
+        {
 #pragma unroll
-        for (int i = 0; i < V; ++i) { st.m[i] = st.c[i]; st.c[i] = st.f[i]; }
-        pnew_chunk(sF, off, c.beta, st.f);
+            for (int r = 0; r < R; ++r) { zero_chunk<T, V>(m[r]); zero_chunk<T, V>(c[r]); zero_chunk<T, V>(f[r]); }
+        }
+    };
+    __device__ static void advance(State& st, const Ctx& c, uint32_t sNew, int warp, int lane)
+    {
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            const int off = (warp * R + r + 1) * TG::PITCH_H + (TG::HX + lane * V) * (int)sizeof(T);
+#pragma unroll
+            for (int i = 0; i < V; ++i) { st.m[r][i] = st.c[r][i]; st.c[r][i] = st.f[r][i]; }
+            pnew_chunk(sNew, off, c.beta, st.f[r]);
+        }
     }
     template <bool CLEAN>
-    __device__ static void emit(const Args& a, const Ctx& c, const State& st, long long idx, uint32_t, uint32_t sC, uint32_t,
-                                int warp, int lane, bool out, uint32_t fb, const uint32_t (&code)[V], const TC& xe, int ycls, int zcls,
-                                double (&accs)[1])
+    __device__ static void emit(const Args& a, const Ctx& c, const State& st, long long idx, int px, uint32_t, uint32_t sC, uint32_t,
+                                int warp, int lane, const bool (&out)[R], const uint32_t (&fb)[R], const uint32_t (&code)[R][V],
+                                const TC& xe, const int (&ycls)[R], int zcls, double (&accs)[1])
     {
         double& acc = accs[0];
-        const int row = (warp + 1) * TG::PITCH_H;
-        const int off = row + (TG::HX + lane * V) * (int)sizeof(T);
-        T vn[V], vs[V];
-        const T (&vm)[V] = st.m;
-        const T (&vc)[V] = st.c;
-        const T (&vp)[V] = st.f;
-        pnew_chunk(sC, off + TG::PITCH_H, c.beta, vn);
-        pnew_chunk(sC, off - TG::PITCH_H, c.beta, vs);
-        // x neighbours: shuffles inside the warp, the row's two halo cells (same address for all lanes) at its ends
-        const int hl_off = row + (TG::HX - 1) * (int)sizeof(T), hr_off = row + (TG::HX + TG::BX) * (int)sizeof(T);
-        const T hl = lds_scalar(sC + hl_off, T()) + c.beta * lds_scalar(sC + TG::TILE_H + hl_off, T());
-        const T hr = lds_scalar(sC + hr_off, T()) + c.beta * lds_scalar(sC + TG::TILE_H + hr_off, T());
-        T xl = __shfl_up_sync(0xffffffffu, vc[V - 1], 1);
-        T xr = __shfl_down_sync(0xffffffffu, vc[0], 1);
-        if (lane == 0) xl = hl;
-        if (lane == 31) xr = hr;
-        if (!out) return;
-        st_chunk<T, V>(c.pnew + idx, vc);
-        T q[V];
-        apply_op_chunk<LOP_, T, V>(q, vm, vc, vp, vn, vs, xl, xr, CLEAN ? 0u : fb, code, a.K, xe, ycls, zcls);
-        acc += chunk_dot<T, V>(vc, q);
+        const int row0 = (warp * R + 1) * TG::PITCH_H;                     // shared-memory row of the warp's first row
+        const int xoff = (TG::HX + lane * V) * (int)sizeof(T);
+        // rows j0-1 .. j0+R of the emitted plane: the two outer ones from the stage, the warp's own from the window
+        T rows[R + 2][V];
+        pnew_chunk(sC, row0 - TG::PITCH_H + xoff, c.beta, rows[0]);
+        pnew_chunk(sC, row0 + R * TG::PITCH_H + xoff, c.beta, rows[R + 1]);
+#pragma unroll
+        for (int r = 0; r < R; ++r)
+#pragma unroll
+            for (int i = 0; i < V; ++i) rows[r + 1][i] = st.c[r][i];
+        const int hl_off = (TG::HX - 1) * (int)sizeof(T), hr_off = (TG::HX + TG::BX) * (int)sizeof(T);
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            const T (&vc)[V] = rows[r + 1];
+            // x neighbours: shuffles inside the warp, the row's two halo cells (same address for all lanes) at its ends
+            const int row = row0 + r * TG::PITCH_H;
+            const T hl = lds_scalar(sC + row + hl_off, T()) + c.beta * lds_scalar(sC + TG::TILE_H + row + hl_off, T());
+            const T hr = lds_scalar(sC + row + hr_off, T()) + c.beta * lds_scalar(sC + TG::TILE_H + row + hr_off, T());
+            T xl = __shfl_up_sync(0xffffffffu, vc[V - 1], 1);
+            T xr = __shfl_down_sync(0xffffffffu, vc[0], 1);
+            if (lane == 0) xl = hl;
+            if (lane == 31) xr = hr;
+            if (out[r]) {
+                st_chunk<T, V>(c.pnew + idx + (long long)r * px, vc);
+                T q[V];
+                apply_op_chunk<LOP_, T, V>(q, REV ? st.f[r] : st.m[r], vc, REV ? st.m[r] : st.f[r], rows[r + 2], rows[r], xl, xr,
+                                           CLEAN ? 0u : fb[r], code[r], a.K, xe, ycls[r], zcls);
+                acc += chunk_dot<T, V>(vc, q);
+            }
+        }
     }
     __device__ static void finalize(const Args& a, const double (&tot)[1])
     {
@@ -473,11 +515,11 @@ struct OpT3 {
 // delta} and apply delta += alpha_{k-1} p_{k-1} + alpha_k p_k.  7.5 instead of 8 passes per CG iteration on average
 // (K4: 3 / 6 instead of 5 / 5).  A pending update at loop exit is applied by flush_delta_kernel before K2.
 // The ring is sized per parity: DO_ stages of {p_h, r, p_old, delta} or as many {p_h, r} stages as fit the same bytes.
-template <typename T, int BY_, int DO_, int MINB_, bool LOP_ = false>
+template <typename T, int BY_, int R_, int DO_, int MINB_, bool LOP_ = false>
 struct OpT4 {
     using VT = T;
-    using TG = TileGeom<T, BY_>;
-    enum { V = TG::V, MINB = MINB_, NACC = 1, TICKET = 1,
+    using TG = TileGeom<T, BY_, R_>;
+    enum { V = TG::V, R = R_, MINB = MINB_, NACC = 1, TICKET = 1,
            STAGE_ODD = TG::TILE_H + 3 * TG::TILE_C, STAGE_EVEN = TG::TILE_H + TG::TILE_C,
            D_ODD = DO_, D_EVEN = (DO_ * STAGE_ODD) / STAGE_EVEN, DMAX = D_EVEN, SMEM_BYTES = DO_ * STAGE_ODD,
            BOX_H = (BY_ + 2) * TG::PITCH_H };
@@ -526,47 +568,54 @@ struct OpT4 {
     struct State {};
     __device__ static void advance(State&, const Ctx&, uint32_t, int, int) {}
     template <bool CLEAN>
-    __device__ static void emit(const Args& a, const Ctx& c, const State&, long long idx, uint32_t sB, uint32_t sC, uint32_t sF,
-                                int warp, int lane, bool out, uint32_t fb, const uint32_t (&code)[V], const TC& xe, int ycls, int zcls,
-                                double (&accs)[1])
+    __device__ static void emit(const Args& a, const Ctx& c, const State&, long long idx, int px, uint32_t sB, uint32_t sC, uint32_t sF,
+                                int warp, int lane, const bool (&out)[R], const uint32_t (&fb)[R], const uint32_t (&code)[R][V],
+                                const TC& xe, const int (&ycls)[R], int zcls, double (&accs)[1])
     {
         double& acc = accs[0];
-        const int row = (warp + 1) * TG::PITCH_H;
-        const int off = row + (TG::HX + lane * V) * (int)sizeof(T);
-        T vm[V], vc[V], vp[V], vn[V], vs[V];
-        lds_chunk<T, V>(sC + off, vc);
-        lds_chunk<T, V>(sC + off + TG::PITCH_H, vn);
-        lds_chunk<T, V>(sC + off - TG::PITCH_H, vs);
-        lds_chunk<T, V>(sF + off, vp);
-        lds_chunk<T, V>(sB + off, vm);
-        const T hl = lds_scalar(sC + row + (TG::HX - 1) * (int)sizeof(T), T());
-        const T hr = lds_scalar(sC + row + (TG::HX + TG::BX) * (int)sizeof(T), T());
-        T xl = __shfl_up_sync(0xffffffffu, vc[V - 1], 1);
-        T xr = __shfl_down_sync(0xffffffffu, vc[0], 1);
-        if (lane == 0) xl = hl;
-        if (lane == 31) xr = hr;
-        if (!out) return;
-        T q[V];
-        apply_op_chunk<LOP_, T, V>(q, vm, vc, vp, vn, vs, xl, xr, CLEAN ? 0u : fb, code, a.K, xe, ycls, zcls);
-        if (c.step) {
-            st_chunk<T, V>(a.q_out + idx, q);
-            acc += chunk_dot<T, V>(vc, q);
-            return;
-        }
-        const int eoff = TG::TILE_H + (warp * TG::BX + lane * V) * (int)sizeof(T);
-        T er[V], rn[V];
-        lds_chunk<T, V>(sC + eoff, er);
+        const int row0 = (warp * R + 1) * TG::PITCH_H;
+        const int xoff = (TG::HX + lane * V) * (int)sizeof(T);
+        // rows j0-1 .. j0+R of the emitted plane: each is the N / S neighbour of the rows next to it
+        T rows[R + 2][V];
 #pragma unroll
-        for (int i = 0; i < V; ++i) rn[i] = er[i] - c.alpha * q[i];
-        acc += chunk_dot<T, V>(rn, rn);
-        st_chunk<T, V>(a.r + idx, rn);
-        if (c.odd) {
-            T ep[V], ed[V], dn[V];
-            lds_chunk<T, V>(sC + eoff + TG::TILE_C, ep);
-            if (c.first) zero_chunk<T, V>(ed); else lds_chunk<T, V>(sC + eoff + 2 * TG::TILE_C, ed);
+        for (int q = 0; q < R + 2; ++q) lds_chunk<T, V>(sC + row0 + (q - 1) * TG::PITCH_H + xoff, rows[q]);
 #pragma unroll
-            for (int i = 0; i < V; ++i) dn[i] = (ed[i] + c.alpha_prev * ep[i]) + c.alpha * vc[i];
-            st_chunk<T, V>(a.delta + idx, dn);
+        for (int r = 0; r < R; ++r) {
+            const T (&vc)[V] = rows[r + 1];
+            const int row = row0 + r * TG::PITCH_H;
+            T vp[V], vm[V];
+            lds_chunk<T, V>(sF + row + xoff, vp);
+            lds_chunk<T, V>(sB + row + xoff, vm);
+            const T hl = lds_scalar(sC + row + (TG::HX - 1) * (int)sizeof(T), T());
+            const T hr = lds_scalar(sC + row + (TG::HX + TG::BX) * (int)sizeof(T), T());
+            T xl = __shfl_up_sync(0xffffffffu, vc[V - 1], 1);
+            T xr = __shfl_down_sync(0xffffffffu, vc[0], 1);
+            if (lane == 0) xl = hl;
+            if (lane == 31) xr = hr;
+            if (!out[r]) continue;
+            const long long cell = idx + (long long)r * px;
+            T q[V];
+            apply_op_chunk<LOP_, T, V>(q, vm, vc, vp, rows[r + 2], rows[r], xl, xr, CLEAN ? 0u : fb[r], code[r], a.K, xe, ycls[r], zcls);
+            if (c.step) {
+                st_chunk<T, V>(a.q_out + cell, q);
+                acc += chunk_dot<T, V>(vc, q);
+                continue;
+            }
+            const int eoff = TG::TILE_H + ((warp * R + r) * TG::BX + lane * V) * (int)sizeof(T);
+            T er[V], rn[V];
+            lds_chunk<T, V>(sC + eoff, er);
+#pragma unroll
+            for (int i = 0; i < V; ++i) rn[i] = er[i] - c.alpha * q[i];
+            acc += chunk_dot<T, V>(rn, rn);
+            st_chunk<T, V>(a.r + cell, rn);
+            if (c.odd) {
+                T ep[V], ed[V], dn[V];
+                lds_chunk<T, V>(sC + eoff + TG::TILE_C, ep);
+                if (c.first) zero_chunk<T, V>(ed); else lds_chunk<T, V>(sC + eoff + 2 * TG::TILE_C, ed);
+#pragma unroll
+                for (int i = 0; i < V; ++i) dn[i] = (ed[i] + c.alpha_prev * ep[i]) + c.alpha * vc[i];
+                st_chunk<T, V>(a.delta + cell, dn);
+            }
         }
     }
     __device__ static void finalize(const Args& a, const double (&tot)[1])
@@ -626,18 +675,18 @@ __device__ __forceinline__ void lds_pair(uint32_t addr, double (&v)[2])
     asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(v[0]), "=d"(v[1]) : "r"(addr));
 }
 
-template <typename T, int BY_, int D_, int MINB_>
+template <typename T, int BY_, int R_, int D_, int MINB_>
 struct OpT2 {
     using VT = double;
     struct TG {
-        static constexpr int V = 2, BX = 64, BY = BY_, NTHR = 32 * (BY_ + 1);
+        static constexpr int V = 2, BX = 64, BY = BY_, R = R_, NCW = BY_ / R_, NTHR = 32 * (NCW + 1);
         static constexpr int HXP = 2, PITCH_P = (BX + 2 * HXP) * 8;                      // 544 bytes
         static constexpr int HXD = 16 / (int)sizeof(T), PITCH_D = (BX + 2 * HXD) * (int)sizeof(T);
         static constexpr int BOX_P = (BY_ + 2) * PITCH_P, BOX_D = (BY_ + 2) * PITCH_D;
         static constexpr int TILE_P = (BOX_P + 127) / 128 * 128, TILE_D = (BOX_D + 127) / 128 * 128;
         static constexpr int TILE_S = BY_ * BX * (int)sizeof(T);
     };
-    enum { V = 2, D = D_, DMAX = D_, MINB = MINB_, NACC = 2, TICKET = 2, STAGE_BYTES = TG::TILE_P + TG::TILE_D + TG::TILE_S,
+    enum { V = 2, R = R_, D = D_, DMAX = D_, MINB = MINB_, NACC = 2, TICKET = 2, STAGE_BYTES = TG::TILE_P + TG::TILE_D + TG::TILE_S,
            SMEM_BYTES = D_ * STAGE_BYTES };
     static constexpr bool REV = false;
     struct Args {
@@ -701,57 +750,66 @@ struct OpT2 {
         v[1] = P[1] + (double)d[1];
     }
     template <bool CLEAN>
-    __device__ static void emit(const Args& a, const Ctx& c, const State&, long long idx, uint32_t sB, uint32_t sC, uint32_t sF,
-                                int warp, int lane, bool out, uint32_t fb, const uint32_t (&code)[V], const TC& lk_x, int ycls,
-                                int zcls, double (&acc)[2])
+    __device__ static void emit(const Args& a, const Ctx& c, const State&, long long idx, int px, uint32_t sB, uint32_t sC, uint32_t sF,
+                                int warp, int lane, const bool (&out)[R], const uint32_t (&fb)[R], const uint32_t (&code)[R][V],
+                                const TC& lk_x, const int (&ycls)[R], int zcls, double (&acc)[2])
     {
-        const int rowP = (warp + 1) * TG::PITCH_P, rowD = (warp + 1) * TG::PITCH_D;
-        const int offP = rowP + (TG::HXP + lane * V) * 8, offD = rowD + (TG::HXD + lane * V) * (int)sizeof(T);
-        double vm[V], vc[V], vp[V], vn[V], vs[V];
-        value(sC, offP, offD, c.dz, vc);
-        value(sC, offP + TG::PITCH_P, offD + TG::PITCH_D, c.dz, vn);
-        value(sC, offP - TG::PITCH_P, offD - TG::PITCH_D, c.dz, vs);
-        value(sF, offP, offD, c.dz, vp);
-        value(sB, offP, offD, c.dz, vm);
-        double hl = lds_scalar(sC + rowP + (TG::HXP - 1) * 8, double());
-        double hr = lds_scalar(sC + rowP + (TG::HXP + TG::BX) * 8, double());
-        if (!c.dz) {
-            hl += (double)lds_scalar(sC + TG::TILE_P + rowD + (TG::HXD - 1) * (int)sizeof(T), T());
-            hr += (double)lds_scalar(sC + TG::TILE_P + rowD + (TG::HXD + TG::BX) * (int)sizeof(T), T());
-        }
-        double xl = __shfl_up_sync(0xffffffffu, vc[V - 1], 1);
-        double xr = __shfl_down_sync(0xffffffffu, vc[0], 1);
-        if (lane == 0) xl = hl;
-        if (lane == 31) xr = hr;
-        if (!out) return;
-        if (a.fold_delta) st_chunk<double, V>(c.Pout + idx, vc);
-        uint32_t lk = lk_x;
-        if (ycls == 0) lk &= ~0x0808u;          // row 0: no S link; last row: no N link (faces normal to y)
-        if (ycls == 3) lk &= ~0x0404u;
-        if (zcls == 0) lk &= ~0x2020u;          // first plane: no B link; last plane: no F link
-        if (zcls == 3) lk &= ~0x1010u;
-        if (!CLEAN && fb) lk = code[0];
-        T S[2];
-        lds_pair(sC + TG::TILE_P + TG::TILE_D + (warp * TG::BX + lane * V) * (int)sizeof(T), S);
-        T rn[V];
+        const int rowP0 = (warp * R + 1) * TG::PITCH_P, rowD0 = (warp * R + 1) * TG::PITCH_D;
+        const int xP = (TG::HXP + lane * V) * 8, xD = (TG::HXD + lane * V) * (int)sizeof(T);
+        // P + delta of rows j0-1 .. j0+R of the emitted plane
+        double rows[R + 2][V];
 #pragma unroll
-        for (int i = 0; i < V; ++i) {
-            const double w = (i == 0) ? xl : vc[0];
-            const double ee = (i == V - 1) ? xr : vc[1];
-            const uint32_t l = (lk >> (8 * i)) & 0xffu;
-            double LP = 0.0;
-            if (l & 1u) LP += a.t[0] * (vc[i] - ee);
-            if (l & 2u) LP += a.t[0] * (vc[i] - w);
-            if (l & 4u) LP += a.t[1] * (vc[i] - vn[i]);
-            if (l & 8u) LP += a.t[1] * (vc[i] - vs[i]);
-            if (l & 16u) LP += a.t[2] * (vc[i] - vp[i]);
-            if (l & 32u) LP += a.t[2] * (vc[i] - vm[i]);
-            const double rr = (l & LINK_VALID) ? ((double)S[i] - LP) : 0.0;
-            rn[i] = (T)rr;
-            acc[0] += rr * rr;
-            acc[1] += (double)rn[i] * (double)rn[i];
+        for (int q = 0; q < R + 2; ++q) value(sC, rowP0 + (q - 1) * TG::PITCH_P + xP, rowD0 + (q - 1) * TG::PITCH_D + xD, c.dz, rows[q]);
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            const double (&vc)[V] = rows[r + 1];
+            const double (&vn)[V] = rows[r + 2];
+            const double (&vs)[V] = rows[r];
+            const int rowP = rowP0 + r * TG::PITCH_P, rowD = rowD0 + r * TG::PITCH_D;
+            double vm[V], vp[V];
+            value(sF, rowP + xP, rowD + xD, c.dz, vp);
+            value(sB, rowP + xP, rowD + xD, c.dz, vm);
+            double hl = lds_scalar(sC + rowP + (TG::HXP - 1) * 8, double());
+            double hr = lds_scalar(sC + rowP + (TG::HXP + TG::BX) * 8, double());
+            if (!c.dz) {
+                hl += (double)lds_scalar(sC + TG::TILE_P + rowD + (TG::HXD - 1) * (int)sizeof(T), T());
+                hr += (double)lds_scalar(sC + TG::TILE_P + rowD + (TG::HXD + TG::BX) * (int)sizeof(T), T());
+            }
+            double xl = __shfl_up_sync(0xffffffffu, vc[V - 1], 1);
+            double xr = __shfl_down_sync(0xffffffffu, vc[0], 1);
+            if (lane == 0) xl = hl;
+            if (lane == 31) xr = hr;
+            if (!out[r]) continue;
+            const long long cell = idx + (long long)r * px;
+            if (a.fold_delta) st_chunk<double, V>(c.Pout + cell, vc);
+            uint32_t lk = lk_x;
+            if (ycls[r] == 0) lk &= ~0x0808u;       // row 0: no S link; last row: no N link (faces normal to y)
+            if (ycls[r] == 3) lk &= ~0x0404u;
+            if (zcls == 0) lk &= ~0x2020u;          // first plane: no B link; last plane: no F link
+            if (zcls == 3) lk &= ~0x1010u;
+            if (!CLEAN && fb[r]) lk = code[r][0];
+            T S[2];
+            lds_pair(sC + TG::TILE_P + TG::TILE_D + ((warp * R + r) * TG::BX + lane * V) * (int)sizeof(T), S);
+            T rn[V];
+#pragma unroll
+            for (int i = 0; i < V; ++i) {
+                const double w = (i == 0) ? xl : vc[0];
+                const double ee = (i == V - 1) ? xr : vc[1];
+                const uint32_t l = (lk >> (8 * i)) & 0xffu;
+                double LP = 0.0;
+                if (l & 1u) LP += a.t[0] * (vc[i] - ee);
+                if (l & 2u) LP += a.t[0] * (vc[i] - w);
+                if (l & 4u) LP += a.t[1] * (vc[i] - vn[i]);
+                if (l & 8u) LP += a.t[1] * (vc[i] - vs[i]);
+                if (l & 16u) LP += a.t[2] * (vc[i] - vp[i]);
+                if (l & 32u) LP += a.t[2] * (vc[i] - vm[i]);
+                const double rr = (l & LINK_VALID) ? ((double)S[i] - LP) : 0.0;
+                rn[i] = (T)rr;
+                acc[0] += rr * rr;
+                acc[1] += (double)rn[i] * (double)rn[i];
+            }
+            st_chunk<T, V>(a.r + cell, rn);
         }
-        st_chunk<T, V>(a.r + idx, rn);
     }
     __device__ static void finalize(const Args& a, const double (&tot)[2])
     {
