@@ -923,3 +923,109 @@ def test_solve_guess_pins(oracle):
     assert ig["converged"]
     a, b = Pg[v] - Pg[v].mean(), Pc[v] - Pc[v].mean()
     assert np.linalg.norm(a - b) / np.linalg.norm(b) < 1e-6
+
+
+# ----------------------------------------------------------------------------- omni_pcg oracle (NEXT-2 ii)
+
+def _pcg_case(oracle, shape, sp, seed=9, frac=0.12):
+    rng = np.random.default_rng(seed)
+    f = make_field("gaussians2d" if len(shape) == 2 else "fourier3d", shape, seed=2, noise=0.05, kmax=2.0)
+    mask = (rng.random(shape) > frac).astype(np.uint8)
+    g = f["g"] + [None] * (3 - len(f["g"]))
+    v = oracle.validity(g[0], g[1], g[2], mask)
+    w1, w0, w0C = oracle.weights(v, *sp)
+    S = oracle.source(v, w1, w0, g[0], g[1], g[2], *sp)
+    K = oracle.constants(shape[-1], shape[-2], shape[0] if len(shape) == 3 else 1, *sp)
+    return g, mask, v, (w1, w0, w0C), S, K["F"] / K["A_tot"]
+
+
+@pytest.mark.parametrize("shape,sp", [((18, 21), (1.0, 0.6, 1.0)), ((9, 10, 17), (1.0, 1.3, 0.8)), ((5, 6), (0.7, 1.0, 1.0))])
+def test_pcg_oracle_vs_dense_algebra(oracle, shape, sp):
+    """oracle.omni_pcg.solve_pcg (multigrid-preconditioned CG on L P = S, reading R-P1) against dense linear algebra
+    written here: (a) its level-0 operator is M - W^n of the stored-weight oracle and the dense L assembled from the
+    definition; (b) the V-cycle, applied to unit vectors, is a SYMMETRIC positive semi-definite matrix B (PCG needs
+    that), positive on the range of L; (c) the truncated iterates are those of a dense textbook PCG with that B;
+    (d) converged, the result is pinv(L) S up to a constant per component; (e) far fewer iterations than plain CG."""
+    from oracle import omni_pcg as pcg
+    g, mask, v, (w1, w0, w0C), S, t = _pcg_case(oracle, shape, sp)
+    nd = len(shape)
+    levels, plans = pcg.build_levels(v.astype(bool), pcg.face_weights(nd, *sp))
+    assert np.allclose(levels[0].w, t[:nd], rtol=1e-15)
+    assert len(levels) == (1 if max(shape) < 8 else len(levels)) and (max(shape) < 8 or len(levels) >= 2)
+    L = _dense_laplacian(v, t)
+    rng = np.random.default_rng(4)
+    x = rng.normal(size=shape) * v
+    Lx = oracle.apply_M(v, w1, x) - oracle.apply_Wn(v, w0, w0C, x)
+    assert np.abs(levels[0].apply(x) - Lx).max() < 1e-14 and np.abs(levels[0].apply(x).ravel() - L @ x.ravel()).max() < 1e-14
+    N = v.size
+    B = np.zeros((N, N))
+    for c in range(N):
+        e = np.zeros(N); e[c] = 1.0
+        B[:, c] = pcg.vcycle(levels, plans, 0, e.reshape(shape)).ravel()
+    keep = v.ravel() == 1
+    assert np.abs(B[~keep]).max() == 0 and np.abs(B[:, ~keep]).max() == 0
+    Bk, Lk, Sk = B[np.ix_(keep, keep)], L[np.ix_(keep, keep)], S.ravel()[keep]
+    assert np.abs(Bk - Bk.T).max() <= 1e-13 * np.abs(Bk).max()
+    ev = np.linalg.eigvalsh(0.5 * (Bk + Bk.T))
+    assert ev.min() > -1e-12 * ev.max()
+    # preconditioned spectrum on the range of L: the nonzero eigenvalues of B L cluster (a usable preconditioner)
+    lam = np.sort(np.linalg.eigvals(Bk @ Lk).real)
+    nz = lam[lam > 1e-9]
+    assert nz.max() / nz.min() < 25.0, nz.max() / nz.min()
+    # dense textbook PCG with the matrix B
+    for k in (1, 2, 5):
+        xk = np.zeros_like(Sk); r = Sk.copy(); p = np.zeros_like(Sk); rho_old = 1.0
+        for it in range(k):
+            z = Bk @ r
+            rho = r @ z
+            p = z + ((rho / rho_old) if it else 0.0) * p
+            q = Lk @ p
+            al = rho / (p @ q)
+            xk += al * p; r -= al * q
+            rho_old = rho
+        Pk, ik = pcg.solve_pcg(g[0], g[1], g[2], mask, *sp, tol=0.0, max_outer=1, max_cg=k)
+        assert ik["cg_iters_total"] == k and np.all(np.isnan(Pk.ravel()[~keep]))
+        assert np.linalg.norm(Pk.ravel()[keep] - xk) / np.linalg.norm(xk) < 1e-10
+    Pc, ic = pcg.solve_pcg(g[0], g[1], g[2], mask, *sp, tol=1e-11, max_outer=5, max_cg=400)
+    assert ic["converged"] and ic["outer_iters"] <= 2
+    Pstar = np.linalg.pinv(Lk, rcond=1e-12) @ Sk
+    from scipy.sparse import csr_matrix
+    from scipy.sparse.csgraph import connected_components
+    ncomp, lab = connected_components(csr_matrix(np.abs(Lk) > 0), directed=False)
+    a, b = Pc.ravel()[keep].copy(), Pstar.copy()
+    for cpt in range(ncomp):
+        m = lab == cpt
+        a[m] -= a[m].mean(); b[m] -= b[m].mean()
+    assert np.linalg.norm(a - b) / np.linalg.norm(b) < 1e-8
+    Pd, idd = oracle.solve_direct(g[0], g[1], g[2], mask, *sp, tol=1e-11, max_outer=5, max_cg=4000)
+    assert idd["converged"] and (max(shape) < 8 or ic["cg_iters_total"] * 2 < idd["cg_iters_total"])
+
+
+def test_pcg_oracle_pieces():
+    """The pieces of the V-cycle against closed forms: restriction and prolongation are transposes (any halving plan,
+    odd sizes); on a grid too small to coarsen the preconditioner is the damped-Jacobi polynomial
+    sum_{j<8} (I - w D^-1 L)^j w D^-1; the coarse weights follow w * 2^m / 4 on halved axes, w * 2^m on the others."""
+    from oracle import omni_pcg as pcg
+    rng = np.random.default_rng(1)
+    for shape, halve in (((9, 8), [True, True]), ((5, 11, 8), [False, True, True]), ((7,), [True])):
+        cshape = tuple((s + 1) // 2 if h else s for s, h in zip(shape, halve))
+        r, e = rng.normal(size=shape), rng.normal(size=cshape)
+        assert pcg.restrict(r, halve).shape == cshape
+        assert np.sum(pcg.restrict(r, halve) * e) == pytest.approx(np.sum(r * pcg.prolong(e, halve, shape)), rel=1e-13)
+    assert pcg.coarsen_plan((5, 8, 17)) == [False, True, True]
+    v = rng.random((6, 7)) > 0.1
+    levels, plans = pcg.build_levels(v, [0.3, 0.2])
+    assert len(levels) == 1 and plans == []
+    L = _dense_laplacian(v, [0.3, 0.2])
+    D = np.diag(L).copy()
+    Dinv = np.where(D > 0, 1.0 / np.where(D > 0, D, 1.0), 0.0)
+    b = rng.normal(size=v.shape) * v
+    G = np.eye(v.size) - pcg.OMEGA * Dinv[:, None] * L
+    z, term = np.zeros(v.size), pcg.OMEGA * Dinv * b.ravel()
+    for _ in range(pcg.NU_COARSEST):
+        z, term = z + term, G @ term
+    assert np.abs(pcg.vcycle(levels, plans, 0, b).ravel() - z).max() < 1e-13
+    levels, plans = pcg.build_levels(np.ones((5, 16, 24), bool), [0.1, 0.2, 0.3])     # w[0] is x (24), w[2] is z (5)
+    assert plans[0] == [False, True, True] and np.allclose(levels[1].w, [0.1 * 4 / 4, 0.2 * 4 / 4, 0.3 * 4])
+    assert levels[1].v.shape == (5, 8, 12) and plans[1] == [False, True, True] and levels[2].v.shape == (5, 4, 6)
+    assert len(levels) == 3
