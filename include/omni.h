@@ -136,6 +136,28 @@ int omni_solve_cascade_f32(int nx, int ny, int nz, double dx, double dy, double 
                            const float* d_gx, const float* d_gy, const float* d_gz, const unsigned char* d_mask,
                            float* d_P_out, double tol, int max_outer, int max_cg, int levels, void* stream, omni_info* info);
 
+/* omni_solve_direct_* with the CG PRECONDITIONED by one geometric-multigrid V-cycle (SURVEY.md 8(f) NEXT-2 ii; reading
+ * R-P1 of DESIGN.md; not the paper's iteration, which names only "CG").  Same system L P = S, same outer
+ * loop (fp64 refinement: eps_R of Eq. 41 :442 re-evaluated from the fp64 master pressure, CG restarted on it), same
+ * stopping rules, status codes and omni_info; cg_iters_total counts preconditioned iterations.  The V-cycle: levels
+ * halving every axis that still has >= 8 cells (a coarse cell is valid iff one of its children is), link weights
+ * w_{l+1}[a] = w_l[a] 2^m (1/4 along halved axes), restriction = sum over the children, prolongation = its transpose,
+ * damped Jacobi (omega = 0.8), 2 sweeps before and after the coarse-grid correction, 8 on the coarsest level.  The
+ * iteration count is nearly independent of the grid size (about 10 to eps_R <= 1e-5, 15 to 1e-8) at about 4 times the
+ * memory traffic of a plain CG iteration.  _f32: an inner solve also returns to the fp64 refinement once ||r|| <= 1e-2
+ * ||r0|| (fp32 vectors cannot resolve more digits of one correction on 1000-cell-wide grids; 3 outer iterations of 3-5
+ * preconditioned iterations reach 1e-5).  Typical caps: max_outer 10-20, max_cg 200.  Always runs under the CUDA graph
+ * (omni_set_loop_mode does not apply).  Extra device memory: about 2.5 vectors, from the library's pool.
+ * d_P_init: first guess or NULL.  The returned field has zero mean per connected component when d_P_init is NULL. */
+int omni_solve_pcg_f64(int nx, int ny, int nz, double dx, double dy, double dz,
+                       const double* d_gx, const double* d_gy, const double* d_gz, const unsigned char* d_mask,
+                       const double* d_P_init, double* d_P_out, double tol, int max_outer, int max_cg, void* stream,
+                       omni_info* info);
+int omni_solve_pcg_f32(int nx, int ny, int nz, double dx, double dy, double dz,
+                       const float* d_gx, const float* d_gy, const float* d_gz, const unsigned char* d_mask,
+                       const float* d_P_init, float* d_P_out, double tol, int max_outer, int max_cg, void* stream,
+                       omni_info* info);
+
 /* The two combined: nb snapshots on one mask (arguments as omni_solve_batch2d_*), inner systems L P = S. */
 int omni_solve_direct_batch2d_f64(int nx, int ny, int nb, double dx, double dy, const double* d_gx, const double* d_gy,
                                   const unsigned char* d_mask2d, const double* d_P_init, double* d_P_out, double tol,
@@ -279,7 +301,7 @@ void omni_release_memory(void);
 int omni_profile_enable(int on);          /* returns the previous setting */
 void omni_profile_read(double* h_ms3, long long* h_count3, int reset);
 const char* omni_status_string(int status);
-int omni_version(void);                  /* 100 * major + minor; 101 added the _guess, _rans_source and history entry points */
+int omni_version(void);                  /* 100 * major + minor; 101 added the _guess, _rans_source and history entry points, 102 omni_solve_pcg_* */
 
 #ifdef __cplusplus
 }

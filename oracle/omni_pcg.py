@@ -18,7 +18,9 @@ Reading R-P1 (the algorithm, in the order executed):
   V-cycle  B_l(b): x = 2 sweeps from x = 0; b_c = restrict(b - L x); x += prolong(B_{l+1}(b_c)); 2 sweeps; return x.
            Coarsest level: 8 sweeps from 0.  Linear, symmetric (same smoother before and after, R = P^T), positive.
   PCG      on L delta = r0 from delta = 0:  z = B_0(r); rho = r.z; p = z + (rho/rho_old) p (p = z at first); q = L p;
-           alpha = rho / p.q; delta += alpha p; r -= alpha q;  until sqrt(r.r) <= 0.1 tol ||S||, r.r = 0 or max_cg.
+           alpha = rho / p.q; delta += alpha p; r -= alpha q;  until sqrt(r.r) <= 0.1 tol ||S||, r.r = 0 or max_cg
+           (fp32 library variant: also until sqrt(r.r) <= 1e-2 ||r0||, argument inner_rel -- fp32 vectors cannot
+           resolve more digits of one correction on large grids; the fp64 outer loop restarts on the true residual).
   outer    as oracle_solve_direct: r0 = S - L P, eps_R = ||r0|| / ||S|| (Eq. 41 :442); stop at eps_R <= tol or
            max_outer; P += delta.  P_init (optional) is the first guess.
 
@@ -145,8 +147,10 @@ def face_weights(nd, dx, dy, dz):
     return [K["F"][a] / K["A_tot"] for a in range(nd)]
 
 
-def solve_pcg(gx, gy, gz, mask, dx, dy, dz, tol, max_outer, max_cg, P_init=None, return_iterates=False):
-    """Returns (P with NaN at missing cells, info dict) -- same conventions as omni_oracle.solve_direct."""
+def solve_pcg(gx, gy, gz, mask, dx, dy, dz, tol, max_outer, max_cg, P_init=None, return_iterates=False, inner_rel=0.0):
+    """Returns (P with NaN at missing cells, info dict) -- same conventions as omni_oracle.solve_direct.
+    inner_rel: an inner solve also stops once ||r|| <= inner_rel ||r0|| (0 = off; the fp32 library variant uses 1e-2,
+    because fp32 vectors cannot resolve more digits of one correction on large grids -- the outer refinement restarts)."""
     gx = np.asarray(gx, dtype=np.float64)
     nd = gx.ndim
     v8 = _o.validity(gx, gy, gz, mask)
@@ -167,7 +171,8 @@ def solve_pcg(gx, gy, gz, mask, dx, dy, dz, tol, max_outer, max_cg, P_init=None,
                 break
             delta, p, rho_old, k = np.zeros_like(P), np.zeros_like(P), 1.0, 0
             rr = float(np.sum(r * r))
-            while np.sqrt(rr) > 0.1 * tol * normS and rr != 0.0 and k < max_cg:
+            thresh = max(0.1 * tol * normS, inner_rel * np.sqrt(rr))
+            while np.sqrt(rr) > thresh and rr != 0.0 and k < max_cg:
                 z = vcycle(levels, plans, 0, r)
                 rho = float(np.sum(r * z))
                 p = z + ((rho / rho_old) if k > 0 else 0.0) * p

@@ -17,7 +17,7 @@ STATUS_NAMES = {0: "OMNI_OK", 1: "OMNI_NOT_CONVERGED", -1: "OMNI_ERR_INVALID_ARG
                 -3: "OMNI_ERR_ALLOC", -4: "OMNI_ERR_BREAKDOWN"}
 # every symbol include/omni.h declares
 SYMBOLS = ["omni_solve_f64", "omni_solve_f32", "omni_workspace_bytes", "omni_solve_f64_ws", "omni_solve_f32_ws",
-           "omni_solve_host_f64", "omni_solve_host_f32", "omni_solve_batch2d_f64", "omni_solve_batch2d_f32", "omni_solve_guess_f64", "omni_solve_guess_f32", "omni_solve_direct_f64", "omni_solve_direct_f32", "omni_solve_direct_batch2d_f64", "omni_solve_direct_batch2d_f32", "omni_solve_cascade_f64", "omni_solve_cascade_f32", "omni_velocity_source_f64", "omni_velocity_source_f32", "omni_rans_source_f64", "omni_rans_source_f32",
+           "omni_solve_host_f64", "omni_solve_host_f32", "omni_solve_batch2d_f64", "omni_solve_batch2d_f32", "omni_solve_guess_f64", "omni_solve_guess_f32", "omni_solve_direct_f64", "omni_solve_direct_f32", "omni_solve_pcg_f64", "omni_solve_pcg_f32", "omni_solve_direct_batch2d_f64", "omni_solve_direct_batch2d_f32", "omni_solve_cascade_f64", "omni_solve_cascade_f32", "omni_velocity_source_f64", "omni_velocity_source_f32", "omni_rans_source_f64", "omni_rans_source_f32",
            "omni_compressible_rans_source_f64", "omni_compressible_rans_source_f32", "omni_constants", "omni_source_f64", "omni_source_f32",
            "omni_apply_M_f64", "omni_apply_M_f32", "omni_residual_f64", "omni_residual_f32", "omni_launch_count",
            "omni_set_loop_mode", "omni_set_history", "omni_release_memory", "omni_profile_enable", "omni_profile_read", "omni_status_string", "omni_version"]
@@ -242,6 +242,11 @@ def solve_direct(gx, gy, gz, mask, d, tol, max_outer, max_cg, out=None, P_init=N
     if rc < 0:
         raise OmniError(rc, f"{_entry}_{sfx}")
     return P, info.as_dict()
+
+
+def solve_pcg(gx, gy, gz, mask, d, tol, max_outer, max_cg, out=None, P_init=None):
+    """omni_solve_pcg_*: the fixed point L P = S by multigrid-preconditioned CG (include/omni.h).  Returns (P, info dict)."""
+    return solve_direct(gx, gy, gz, mask, d, tol, max_outer, max_cg, out=out, P_init=P_init, _entry="omni_solve_pcg")
 
 
 def velocity_source(u, v, w, mask, d, rho=1.0, mu=0.0, dudt=None):

@@ -4,6 +4,7 @@
 #include "omni_tma.cuh"
 #include "omni_persist.cuh"
 #include "omni_loop.cuh"
+#include "omni_mg.cuh"
 #include "../../include/omni.h"
 
 #include <algorithm>
@@ -40,6 +41,7 @@ using namespace omni;
 #define OMNI_TAPER_F 0.5     // tapered z segments (tma_config): fraction of the remaining planes per slot; 0 = uniform segments
 #define OMNI_TAPER_MIN 24    // and the shortest segment
 #endif
+#define OMNI_PCG_INNER_REL_F32 1e-2         // omni_solve_pcg_f32: relative reduction after which an inner solve returns to the fp64 refinement
 #define OMNI_PERSIST_MAX_CELLS 1500000LL   // automatic mode: grids up to this many padded cells take the persistent loop
 #ifndef OMNI_LOOPK_MAX_CELLS
 #define OMNI_LOOPK_MAX_CELLS 0LL           // ... and up to this many the cooperative tile-loop kernel (omni_loop.cuh, loop mode 4), if its grid fits one wave; 0: only on request
@@ -343,11 +345,12 @@ size_t carve(const Geom& g, char* base, Workspace<T>* w)
 }
 
 __global__ void init_scalars_kernel(Scalars* sc, double tol, int max_outer, int max_cg, double* hist = nullptr, int hist_cap = 0,
-                                    int* hist_k = nullptr)
+                                    int* hist_k = nullptr, double inner_rel = 0.0)
 {
     Scalars s;
     memset(&s, 0, sizeof(s));
     s.tol = tol; s.max_outer = max_outer; s.max_cg = max_cg;
+    s.inner_rel2 = inner_rel * inner_rel;
     s.hist = hist; s.hist_k = hist_k; s.hist_cap = hist_cap; s.hist_n = 0;
     s.inner_go = 0; s.outer_go = 1; s.status = ST_OK;
     s.dzero = 1;                     // no CG iteration has run yet: the first K2 takes delta as zero
@@ -560,7 +563,7 @@ typename K4<T, LOP>::Args k4_args(const Workspace<T>& w, const Coef<T>& K, CondH
 {
     typename K4<T, LOP>::Args a;
     a.r = w.r; a.delta = w.delta; a.p_fixed = -1; a.wcode = w.wcode; a.link = w.link; a.flags = w.flags; a.tflags = w.tflags;
-    a.K = K; a.sc = w.sc; a.partial = w.partial; a.cond = ch; a.q_out = nullptr;
+    a.K = K; a.sc = w.sc; a.partial = w.partial; a.cond = ch; a.q_out = nullptr; a.pcg = 0;
     return a;
 }
 template <typename T>
@@ -766,9 +769,105 @@ int run_loop_host(const Geom& g, const Workspace<T>& w, const HostConst& H, cons
     return rc;
 }
 
+// ------------------------------------------------------------------------------------------------ multigrid preconditioner (omni_mg.cuh)
+template <typename T>
+struct MgHier {
+    int nlev;
+    MgLevel<T> L[MG_MAX_LEVELS];
+    void* mem;                       // one pool block: level-0 iterates, coarse links / iterates / right-hand sides
+    long long launches_per_cycle;    // kernels one V-cycle enqueues (launch accounting)
+};
+
+// Level sizes and weights (reading R-P1), one pool block for all levels, link bytes of the coarse levels.
+// Level 0 aliases the solver's arrays: link bytes and right-hand side r in the padded layout.
+template <typename T>
+int mg_build(const Geom& g, const Workspace<T>& w, const HostConst& H, MgHier<T>& M, cudaStream_t st)
+{
+    M.nlev = 0; M.mem = nullptr; M.launches_per_cycle = 0;
+    MgLevel<T> L0 = {};
+    L0.nx = g.nx; L0.ny = g.ny; L0.nz = g.nz; L0.px = g.px; L0.pplane = g.pplane; L0.n = g.npad;
+    for (int a = 0; a < 3; ++a) L0.w[a] = (T)(a < g.naxes ? H.F[a] / H.Atot : 0.0);
+    double wd[3] = { H.F[0] / H.Atot, H.F[1] / H.Atot, g.naxes == 3 ? H.F[2] / H.Atot : 0.0 };
+    L0.link = w.link; L0.b = w.r;
+    M.L[M.nlev++] = L0;
+    while (M.nlev < MG_MAX_LEVELS) {
+        MgLevel<T>& F = M.L[M.nlev - 1];
+        F.hx = F.nx >= MG_MIN_COARSEN; F.hy = F.ny >= MG_MIN_COARSEN; F.hz = (g.naxes == 3 && F.nz >= MG_MIN_COARSEN);
+        const int m = F.hx + F.hy + F.hz;
+        if (m == 0) break;
+        MgLevel<T> C = {};
+        C.nx = F.hx ? (F.nx + 1) / 2 : F.nx; C.ny = F.hy ? (F.ny + 1) / 2 : F.ny; C.nz = F.hz ? (F.nz + 1) / 2 : F.nz;
+        C.px = C.nx; C.pplane = (long long)C.px * C.ny; C.n = C.pplane * C.nz;
+        const int h[3] = { F.hx, F.hy, F.hz };
+        for (int a = 0; a < 3; ++a) {
+            wd[a] = wd[a] * (double)(1 << m) * (h[a] ? 0.25 : 1.0);
+            C.w[a] = (T)wd[a];
+        }
+        M.L[M.nlev++] = C;
+    }
+    M.L[M.nlev - 1].hx = M.L[M.nlev - 1].hy = M.L[M.nlev - 1].hz = 0;
+    // carve
+    size_t off = 0;
+    auto take = [&](size_t bytes) { const size_t o = off; off += align_up(bytes, 256); return o; };
+    size_t o_x[MG_MAX_LEVELS], o_xt[MG_MAX_LEVELS], o_b[MG_MAX_LEVELS], o_link[MG_MAX_LEVELS];
+    for (int l = 0; l < M.nlev; ++l) {
+        const size_t n = (size_t)M.L[l].n;
+        o_x[l] = take(n * sizeof(T)); o_xt[l] = take(n * sizeof(T));
+        o_b[l] = l ? take(n * sizeof(T)) : 0; o_link[l] = l ? take(n) : 0;
+    }
+    const size_t o_vc = take(M.nlev > 1 ? (size_t)M.L[1].n : 1);
+    if (pool_alloc(&M.mem, off, st) != cudaSuccess) { cudaGetLastError(); M.mem = nullptr; return OMNI_ERR_ALLOC; }
+    char* base = (char*)M.mem;
+    for (int l = 0; l < M.nlev; ++l) {
+        M.L[l].x = (T*)(base + o_x[l]); M.L[l].xt = (T*)(base + o_xt[l]);
+        if (l) { M.L[l].b = (T*)(base + o_b[l]); M.L[l].link = (const uint8_t*)(base + o_link[l]); }
+    }
+    uint8_t* vc = (uint8_t*)(base + o_vc);
+    for (int l = 1; l < M.nlev; ++l) {
+        const unsigned nb = blocks_for(M.L[l].n, 256);
+        mg_coarse_valid_kernel<T><<<nb, 256, 0, st>>>(M.L[l - 1], M.L[l], vc);
+        mg_link_kernel<T><<<nb, 256, 0, st>>>(M.L[l], vc, (uint8_t*)(base + o_link[l]), g.naxes);
+        g_launches.fetch_add(2, std::memory_order_relaxed);
+    }
+    CK(cudaGetLastError());
+    return OMNI_OK;
+}
+
+// enqueue B_l(b_l) (V-cycle from level l down and up again); returns the array that holds the result
+template <typename T>
+T* mg_vcycle(MgHier<T>& M, int l, cudaStream_t st)
+{
+    const MgLevel<T>& L = M.L[l];
+    const bool last = (l + 1 == M.nlev);
+    const unsigned nb = blocks_for(L.n, 256);
+    T *cur = L.x, *oth = L.xt;
+    mg_jacobi_kernel<T, true><<<nb, 256, 0, st>>>(L, nullptr, cur);
+    M.launches_per_cycle += 1;
+    for (int sw = 1; sw < (last ? MG_NU_COARSEST : MG_NU); ++sw) {
+        mg_jacobi_kernel<T, false><<<nb, 256, 0, st>>>(L, cur, oth);
+        std::swap(cur, oth);
+        M.launches_per_cycle += 1;
+    }
+    if (last) return cur;
+    const MgLevel<T>& C = M.L[l + 1];
+    mg_residual_restrict_kernel<T><<<blocks_for(C.n, 256), 256, 0, st>>>(L, C, cur);
+    T* e = mg_vcycle<T>(M, l + 1, st);
+    mg_prolong_add_kernel<T><<<nb, 256, 0, st>>>(L, C, cur, e);
+    M.launches_per_cycle += 2;
+    for (int sw = 0; sw < MG_NU; ++sw) {
+        mg_jacobi_kernel<T, false><<<nb, 256, 0, st>>>(L, cur, oth);
+        std::swap(cur, oth);
+        M.launches_per_cycle += 1;
+    }
+    return cur;
+}
+
 // CUDA-graph loop: outer WHILE { K2 ; inner WHILE { K3 ; K4 } }, conditions written by the kernels' last CTAs.
+// mg != nullptr (omni_solve_pcg): the inner body is one PRECONDITIONED CG iteration -- V-cycle z = B r, rho = r.z and
+// beta (mg_dot_kernel), K3 with z in the place of r (p = z + beta p), K4 testing ||r|| only.
 template <typename T, bool LOP>
-int run_loop_graph(const Geom& g, const Workspace<T>& w, const HostConst& H, const Coef<T>& K, cudaStream_t st)
+int run_loop_graph(const Geom& g, const Workspace<T>& w, const HostConst& H, const Coef<T>& K, cudaStream_t st,
+                   MgHier<T>* mg = nullptr)
 {
     cudaGraph_t G = nullptr;
     cudaGraphExec_t exec = nullptr;
@@ -815,9 +914,23 @@ int run_loop_graph(const Geom& g, const Workspace<T>& w, const HostConst& H, con
         cudaGraph_t bodyInner = pi.conditional.phGraph_out[0];
 
         if (cudaStreamBeginCaptureToGraph(cap, bodyInner, nullptr, nullptr, 0, cudaStreamCaptureModeThreadLocal) != cudaSuccess) break;
-        cudaError_t e3 = launch_tma<K3<T, LOP>>(g, k3_args<T, LOP>(w, K, ch), maps, cap);
-        cudaError_t e4 = launch_tma<K4<T, LOP>>(g, k4_args<T, LOP>(w, K, ch), maps, cap);
-        if (cudaStreamEndCapture(cap, &tmp) != cudaSuccess || e3 != cudaSuccess || e4 != cudaSuccess) break;
+        auto a4 = k4_args<T, LOP>(w, K, ch);
+        TmaSet maps3 = maps;
+        bool okm = true;
+        if (mg) {
+            mg->launches_per_cycle = 0;
+            T* z = mg_vcycle<T>(*mg, 0, cap);
+            unsigned nbd = blocks_for(g.npad, 256);
+            if (nbd > 4736u) nbd = 4736u;
+            mg_dot_kernel<T><<<nbd, 256, 0, cap>>>(g.npad, w.r, z, w.sc, w.partial, ch);
+            mg->launches_per_cycle += 1;
+            using TG = typename K3<T>::TG;
+            okm = encode_map<T>(&maps3.r_h, g, z, TG::BX + 2 * TG::HX, TG::BY + 2);     // K3 forms p = z + beta p
+            a4.pcg = 1;
+        }
+        cudaError_t e3 = launch_tma<K3<T, LOP>>(g, k3_args<T, LOP>(w, K, ch), maps3, cap);
+        cudaError_t e4 = launch_tma<K4<T, LOP>>(g, a4, maps, cap);
+        if (cudaStreamEndCapture(cap, &tmp) != cudaSuccess || e3 != cudaSuccess || e4 != cudaSuccess || !okm || cudaGetLastError() != cudaSuccess) break;
         // after the inner loop: the delta update an even last iteration left pending
         if (cudaStreamBeginCaptureToGraph(cap, bodyOuter, &nInner, nullptr, 1, cudaStreamCaptureModeThreadLocal) != cudaSuccess) break;
         cudaError_t ef = launch_flush<T>(g, w, cap);
@@ -922,7 +1035,7 @@ bool valid_common(int nx, int ny, int nz, double dx, double dy, double dz, doubl
 template <typename T>
 int solve_ws(int nx, int ny, int nz, double dx, double dy, double dz, const T* gx, const T* gy, const T* gz,
              const unsigned char* mask, T* P_out, double tol, int max_outer, int max_cg, void* ws, size_t ws_bytes,
-             void* stream, omni_info* info, int batch = 0, const T* P_init = nullptr, int lop = 0)
+             void* stream, omni_info* info, int batch = 0, const T* P_init = nullptr, int lop = 0, int pcg = 0)
 {
     Geom g;
     if (!valid_common(nx, ny, batch ? 1 : nz, dx, dy, dz, tol, max_outer, max_cg) || !make_geom(nx, ny, nz, (int)sizeof(T), g, batch)) return OMNI_ERR_INVALID_ARG;
@@ -936,7 +1049,11 @@ int solve_ws(int nx, int ny, int nz, double dx, double dy, double dz, const T* g
     host_constants(g.naxes, dx, dy, dz, H);
     const Coef<T> K = make_coef<T>(H, dx, dy, dz, g);
 
-    init_scalars_kernel<<<1, 1, 0, st>>>(w.sc, tol, max_outer, max_cg, g_hist.load(), g_hist_cap.load(), g_hist_k.load());
+    // omni_solve_pcg in fp32: an inner solve cannot resolve more than a few digits of its correction (the fp32 vectors
+    // floor the recursive residual at ~1e-4 ||r0|| on 1000-cell-wide grids), so it hands back to the fp64 refinement
+    // after two digits (reading R-P1)
+    const double inner_rel = (pcg && sizeof(T) == 4) ? OMNI_PCG_INNER_REL_F32 : 0.0;
+    init_scalars_kernel<<<1, 1, 0, st>>>(w.sc, tol, max_outer, max_cg, g_hist.load(), g_hist_cap.load(), g_hist_k.load(), inner_rel);
     CK(cudaGetLastError());
     g_launches.fetch_add(1, std::memory_order_relaxed);
     int rc = setup_codes<T>(g, w, gx, gy, gz, mask, st);
@@ -953,6 +1070,17 @@ int solve_ws(int nx, int ny, int nz, double dx, double dy, double dz, const T* g
 
     int mode = g_loop_mode.load();
     if (mode == 0) mode = (g.npad <= persist_max_cells()) ? 3 : (g.npad <= loopk_max_cells()) ? 4 : 2;
+    MgHier<T> mg;
+    mg.mem = nullptr; mg.launches_per_cycle = 0;
+    if (pcg) {
+        // multigrid-preconditioned CG on L P = S: always the graph loop (its body holds the V-cycle's kernels)
+        rc = mg_build<T>(g, w, H, mg, st);
+        if (rc != OMNI_OK) return rc;
+        rc = run_loop_graph<T, true>(g, w, H, K, st, &mg);
+        cudaFreeAsync(mg.mem, st);                        // stream-ordered: after the graph has run
+        if (rc != OMNI_OK) return rc;
+        mode = -2;
+    }
     // lop: the CG kernels apply L instead of M (omni_solve_direct); everything else -- K2, scalars, loop control -- is shared
     if (mode == 3) {
         rc = lop ? run_loop_persist<T, true>(g, w, H, K, st) : run_loop_persist<T, false>(g, w, H, K, st);
@@ -982,6 +1110,7 @@ int solve_ws(int nx, int ny, int nz, double dx, double dy, double dz, const T* g
         // kernels launched by the device-side loop of the graph, from its own counters: K2 + flush per outer check,
         // K3 + K4 per CG iteration
         if (mode == 2) g_launches.fetch_add((long long)(h.normS2 > 0.0 ? 2 * h.n + 1 : 0) + 2 * h.cg_total, std::memory_order_relaxed);
+        if (mode == -2) g_launches.fetch_add((long long)(h.normS2 > 0.0 ? 2 * h.n + 1 : 0) + (2 + mg.launches_per_cycle) * h.cg_total, std::memory_order_relaxed);
         return h.status;
     }
     return OMNI_OK;
@@ -990,7 +1119,7 @@ int solve_ws(int nx, int ny, int nz, double dx, double dy, double dz, const T* g
 template <typename T>
 int solve_alloc(int nx, int ny, int nz, double dx, double dy, double dz, const T* gx, const T* gy, const T* gz,
                 const unsigned char* mask, T* P_out, double tol, int max_outer, int max_cg, void* stream, omni_info* info,
-                int batch = 0, const T* P_init = nullptr, int lop = 0)
+                int batch = 0, const T* P_init = nullptr, int lop = 0, int pcg = 0)
 {
     Geom g;
     if (!valid_common(nx, ny, batch ? 1 : nz, dx, dy, dz, tol, max_outer, max_cg) || !make_geom(nx, ny, nz, (int)sizeof(T), g, batch)) return OMNI_ERR_INVALID_ARG;
@@ -999,7 +1128,7 @@ int solve_alloc(int nx, int ny, int nz, double dx, double dy, double dz, const T
     void* ws = nullptr;
     if (pool_alloc(&ws, bytes, st) != cudaSuccess) { cudaGetLastError(); return OMNI_ERR_ALLOC; }
     int rc = solve_ws<T>(nx, ny, nz, dx, dy, dz, gx, gy, gz, mask, P_out, tol, max_outer, max_cg, ws, bytes, stream, info,
-                         batch, P_init, lop);
+                         batch, P_init, lop, pcg);
     cudaFreeAsync(ws, st);
     return rc;
 }
@@ -1404,6 +1533,22 @@ int omni_solve_direct_f32(int nx, int ny, int nz, double dx, double dy, double d
                               0, d_P_init, 1);
 }
 
+int omni_solve_pcg_f64(int nx, int ny, int nz, double dx, double dy, double dz, const double* d_gx, const double* d_gy,
+                       const double* d_gz, const unsigned char* d_mask, const double* d_P_init, double* d_P_out,
+                       double tol, int max_outer, int max_cg, void* stream, omni_info* info)
+{
+    return solve_alloc<double>(nx, ny, nz, dx, dy, dz, d_gx, d_gy, d_gz, d_mask, d_P_out, tol, max_outer, max_cg, stream, info,
+                               0, d_P_init, 1, 1);
+}
+
+int omni_solve_pcg_f32(int nx, int ny, int nz, double dx, double dy, double dz, const float* d_gx, const float* d_gy,
+                       const float* d_gz, const unsigned char* d_mask, const float* d_P_init, float* d_P_out,
+                       double tol, int max_outer, int max_cg, void* stream, omni_info* info)
+{
+    return solve_alloc<float>(nx, ny, nz, dx, dy, dz, d_gx, d_gy, d_gz, d_mask, d_P_out, tol, max_outer, max_cg, stream, info,
+                              0, d_P_init, 1, 1);
+}
+
 int omni_solve_cascade_f64(int nx, int ny, int nz, double dx, double dy, double dz, const double* d_gx, const double* d_gy,
                            const double* d_gz, const unsigned char* d_mask, double* d_P_out, double tol, int max_outer,
                            int max_cg, int levels, void* stream, omni_info* info)
@@ -1591,6 +1736,6 @@ const char* omni_status_string(int status)
     }
 }
 
-int omni_version(void) { return 101; }   // 101: omni_solve_guess_*, omni_set_history, omni_rans_source_*, omni_compressible_rans_source_*
+int omni_version(void) { return 102; }   // 101: omni_solve_guess_*, omni_set_history, omni_rans_source_*, omni_compressible_rans_source_*
 
 }  // extern "C"

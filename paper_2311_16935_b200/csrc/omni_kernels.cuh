@@ -73,6 +73,8 @@ struct Scalars {
     double alpha_prev; // alpha of the CG iteration whose delta update is pending (lazy delta, omni_tma.cuh K4)
     double normS2;     // ||S||^2
     double thresh2;    // (0.1 * tol)^2 * ||S||^2   inner stop (A3)
+    double inner_rel2; // omni_solve_pcg fp32 only (0 elsewhere): an inner solve also stops at ||r||^2 <= inner_rel2 ||r0||^2
+    double thresh2_in; // the inner threshold of the current outer iteration: max(thresh2, inner_rel2 ||r0||^2), set by K2
     double tol2S;      // tol^2 * ||S||^2           outer stop (Eq. 41)
     double epsR2;      // ||r0||^2 of the last outer check
     double tol;

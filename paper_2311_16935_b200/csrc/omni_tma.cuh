@@ -531,6 +531,8 @@ struct OpT4 {
         const uint32_t* wcode; const uint8_t* link; const uint32_t* flags; const uint32_t* tflags;
         Coef<T> K; Scalars* sc; double* partial; CondHandles cond;
         T* q_out;                         // only for omni_apply_M: store q, leave r / delta untouched
+        int pcg;                          // 1: preconditioned recurrence (omni_solve_pcg): rho = r.z and beta come from
+                                          //    mg_dot_kernel after the V-cycle; this kernel only tests ||r||
     };
     struct Ctx {
         T alpha, alpha_prev; int pidx, pold; bool odd, first, step;
@@ -629,11 +631,13 @@ struct OpT4 {
             return;
         }
         if (s->k & 1) { s->pend = 0; } else { s->pend = 1; s->alpha_prev = s->alpha; }
-        s->beta = rho1 / s->rho;
-        s->rho = rho1;
+        if (!a.pcg) {
+            s->beta = rho1 / s->rho;
+            s->rho = rho1;
+        }
         s->k += 1;
         s->cg_total += 1;
-        const int go = (rho1 > s->thresh2) && (rho1 != 0.0) && (s->k < s->max_cg);
+        const int go = (rho1 > s->thresh2_in) && (rho1 != 0.0) && (s->k < s->max_cg);
         s->inner_go = go;
         set_cond(a.cond, -1, go);
     }
@@ -833,7 +837,8 @@ struct OpT2 {
         s->pend = 0;
         s->beta = 0.0;
         s->rho = tot[1];
-        const int go = (tot[1] > s->thresh2) && (tot[1] != 0.0) && (s->max_cg > 0);
+        s->thresh2_in = fmax(s->thresh2, s->inner_rel2 * tot[1]);
+        const int go = (tot[1] > s->thresh2_in) && (tot[1] != 0.0) && (s->max_cg > 0);
         s->inner_go = go;
         s->dzero = !go;      // an inner loop that does not start leaves the old delta behind: the next K2 must not fold it again
         set_cond(a.cond, 1, go);

@@ -184,7 +184,7 @@ def test_converged_parity_fullsize(oracle, idx, dtype, always):
 @pytest.mark.parametrize("idx,dtype", [(0, "f64")] + CASES)
 def test_converged_field_certified_by_oracle(oracle, idx, dtype):
     """SURVEY 8(c) parity protocol iii (north_star "Target"): the CONVERGED GPU field of every config -- by Alg. 1
-    (max_cg 16) and by omni_solve_cascade -- has its eps_R (Eq. 41 :442) re-evaluated by the oracle's per-cell operators
+    (max_cg 16), by omni_solve_cascade and by omni_solve_pcg -- has its eps_R (Eq. 41 :442) re-evaluated by the oracle's per-cell operators
     over all cells (oracle.eps_R_of_field).  fp64: the oracle must see eps_R <= 1.05 tol.  fp32: the returned field is
     the fp64 master pressure rounded to fp32, and that rounding alone leaves a residual u |L||P| that grows with the
     grid (SURVEY 7 hard part 3), so the oracle's figure is bounded by tol plus that floor, the floor being evaluated by
@@ -193,7 +193,8 @@ def test_converged_field_certified_by_oracle(oracle, idx, dtype):
     f, g_dev, g_or, mask, m_dev = _load(idx, dtype)
     d, tol = f["d"], TOL_CONV[dtype]
     runs = [("alg1", lambda: omni.solve(g_dev[0], g_dev[1], g_dev[2], m_dev, d, tol, 400000, 16)),
-            ("cascade", lambda: omni.solve_cascade(g_dev[0], g_dev[1], g_dev[2], m_dev, d, tol, 20, 30000, levels=4))]
+            ("cascade", lambda: omni.solve_cascade(g_dev[0], g_dev[1], g_dev[2], m_dev, d, tol, 20, 30000, levels=4)),
+            ("pcg", lambda: omni.solve_pcg(g_dev[0], g_dev[1], g_dev[2], m_dev, d, tol, 20, 300))]
     for name, fn in runs:
         P, info = fn()
         assert info["status"] == 0 and info["eps_R_final"] <= tol, (name, info)

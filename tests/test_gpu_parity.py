@@ -863,3 +863,71 @@ def test_outer_iterations_whose_inner_loop_does_not_start(oracle, dtype, forced_
     Po2, io2 = oracle.solve_guess(g_or[0], g_or[1], g_or[2], m, *d, tol=1e-12, max_outer=4, max_cg=0,
                                   P_init=guess.cpu().numpy().astype(np.float64))
     assert io2["outer_iters"] == 4 and h[0] == pytest.approx(io2["eps_R_final"], rel=1e-4 if dtype == "f32" else 1e-9)
+
+
+PCG_CASES = [("gaussians2d", (64, 64), None), ("lamb_oseen2d", (150, 130), None), ("fourier3d", (20, 33, 140), None),
+             ("sphere3d", (40, 36, 44), None), ("fourier3d", (12, 30, 270), 0.15), ("gaussians2d", (21, 132), None),
+             ("fourier3d", (9, 19, 66), None), ("fourier3d", (5, 4, 9), 0.2), ("gaussians2d", (3, 70), None), ("gaussians2d", (6, 7), None)]
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("kind,shape,frac", PCG_CASES)
+def test_pcg_trajectory_parity(oracle, dtype, kind, shape, frac):
+    """omni_solve_pcg_* (multigrid-preconditioned CG on L P = S, reading R-P1) against oracle/omni_pcg.py with fixed
+    iteration counts (tol = 0): identical steps on both sides -- level plan (odd sizes, axes that stop coarsening, grids
+    too small to coarsen at all), coarse validity and link weights, transfers, Jacobi sweeps, the preconditioned
+    recurrence, the fp64 outer refinement."""
+    from oracle import omni_pcg
+    f = make_field(kind, shape, seed=7, noise=0.05, kmax=4.0)
+    mask = _random_mask(shape, 9, frac) if frac else None
+    g_dev, g_or, m_dev, m = _inputs(f, dtype, mask)
+    d = f["d"]
+    # fp32: an inner solve returns to the fp64 refinement after two digits (inner_rel = 1e-2), which 2 iterations do not
+    # reach: 4 x 2 iterations there, 2 x 6 in fp64
+    mo, mc = (2, 6) if dtype == "f64" else (4, 2)
+    rel = 0.0 if dtype == "f64" else 1e-2
+    P, info = omni.solve_pcg(g_dev[0], g_dev[1], g_dev[2], m_dev, d, 0.0, mo, mc)
+    Po, io = omni_pcg.solve_pcg(g_or[0], g_or[1], g_or[2], m, *d, tol=0.0, max_outer=mo, max_cg=mc, inner_rel=rel)
+    valid = ~np.isnan(Po)
+    assert np.array_equal(np.isnan(P.cpu().numpy()), ~valid)
+    assert info["outer_iters"] == io["outer_iters"] == mo and info["cg_iters_total"] == io["cg_iters_total"]
+    err = rel_l2_after_mean_removal(P.cpu().numpy(), Po, valid)
+    assert err <= TOL_SOLVE[dtype], err
+    # eps_R of the returned field: equal up to rounding, above the floor the fp32 field's own rounding leaves (DESIGN.md 7)
+    assert abs(info["eps_R_final"] - io["eps_R_final"]) <= (5e-3 if dtype == "f32" else 1e-6) * io["eps_R_final"] + (5e-5 if dtype == "f32" else 1e-12)
+    # from a first guess (raw values: the guess fixes the constant)
+    rng = np.random.default_rng(3)
+    P0 = (0.1 * rng.normal(size=shape)).astype(np.float32 if dtype == "f32" else np.float64)
+    Pg, ig = omni.solve_pcg(g_dev[0], g_dev[1], g_dev[2], m_dev, d, 0.0, 2, 2, P_init=to_dev(P0))
+    Pog, iog = omni_pcg.solve_pcg(g_or[0], g_or[1], g_or[2], m, *d, tol=0.0, max_outer=2, max_cg=2, P_init=P0.astype(np.float64),
+                                  inner_rel=rel)
+    assert ig["cg_iters_total"] == iog["cg_iters_total"] == 4
+    scale = np.nanmax(np.abs(Pog))
+    assert np.nanmax(np.abs(Pg.cpu().numpy() - Pog)) <= (1e-10 if dtype == "f64" else 2e-4) * scale
+
+
+@pytest.mark.parametrize("dtype,tol", [("f64", 1e-8), ("f32", 1e-5)])
+def test_pcg_converged(oracle, dtype, tol):
+    """Converged omni_solve_pcg_* on stand-ins of configs 1 - 4: the oracle's operators certify eps_R of the returned
+    field (Eq. 41), the field equals the oracle's PCG result and omni_solve_direct's to tolerance level, and the
+    iteration count is the grid-independent handful the preconditioner is there for."""
+    from oracle import omni_pcg
+    for idx, n in ((1, 160), (3, 48), (2, 64), (4, 72)):
+        f = make_config(idx, n)
+        g_dev, g_or, m_dev, m = _inputs(f, dtype)
+        d = f["d"]
+        P, info = omni.solve_pcg(g_dev[0], g_dev[1], g_dev[2], m_dev, d, tol, 10, 100)
+        assert info["status"] == 0 and info["eps_R_final"] <= tol, (idx, info)
+        assert info["cg_iters_total"] <= 30, info
+        eps, _, _ = oracle.eps_R_of_field(g_or[0], g_or[1], g_or[2], m, P.cpu().numpy(), *d)
+        assert eps <= (1.05 if dtype == "f64" else 3.0) * tol, (idx, eps)
+        Po, io = omni_pcg.solve_pcg(g_or[0], g_or[1], g_or[2], m, *d, tol=tol, max_outer=10, max_cg=100,
+                                    inner_rel=0.0 if dtype == "f64" else 1e-2)
+        assert io["converged"] and abs(io["cg_iters_total"] - info["cg_iters_total"]) <= 2
+        valid = ~np.isnan(Po)
+        # both sides stop anywhere below tol: the fields agree to the accuracy tol buys (cf. test_direct_solve_converged)
+        bound = 2e-6 if dtype == "f64" else 2e-3
+        assert rel_l2_after_mean_removal(P.cpu().numpy(), Po, valid) <= bound
+        Pd, idd = omni.solve_direct(g_dev[0], g_dev[1], g_dev[2], m_dev, d, tol, 10, 5000)
+        assert idd["status"] == 0 and idd["cg_iters_total"] > 3 * info["cg_iters_total"]
+        assert rel_l2_after_mean_removal(P.cpu().numpy(), Pd.cpu().numpy(), valid) <= bound
