@@ -87,6 +87,45 @@ int omni_solve_host_f32(int nx, int ny, int nz, double dx, double dy, double dz,
                         const float* h_gx, const float* h_gy, const float* h_gz, const unsigned char* h_mask,
                         float* h_P_out, double tol, int max_outer, int max_cg, void* stream, omni_info* info);
 
+/* ---- one entry point with per-call options ---------------------------------------------------------------------
+ * omni_solve_ex_* runs Algorithm 1 (OMNI_METHOD_ALG1: what omni_solve_guess_* runs), CG on the fixed-point system
+ * (OMNI_METHOD_DIRECT: omni_solve_direct_*) or its multigrid-preconditioned form (OMNI_METHOD_PCG: omni_solve_pcg_*)
+ * with everything that is otherwise a process-wide setting passed IN THE CALL: two concurrent solves (threads,
+ * streams) never share a history buffer or a loop mode.  options == NULL: the process-wide defaults.  All pointers in
+ * omni_options are DEVICE memory owned by the caller and must stay valid until the solve has finished on `stream`.
+ *   loop_mode       -1: the process-wide setting (omni_set_loop_mode); 0..4 as described there
+ *   d_hist_eps_R    [hist_capacity] doubles: eps_R (Eq. 41 :442) at the i-th outer residual check (i = 0: first guess)
+ *   d_hist_cg_iters [hist_capacity] ints: CG iterations of the outer iteration that led to check i (0 for i = 0)
+ *   d_hist_eps_P    [hist_capacity] doubles: the pressure-update metric eps_P = ||P^i - P^(i-1)|| / ||P^i|| (Eq. 40 :438)
+ *                   of the update that led to check i (0 for i = 0); any of the three may be NULL
+ *   d_P64_out       [nx*ny*nz] doubles: the fp64 master pressure itself (NaN at missing cells).  The _f32 result
+ *                   d_P_out is this field rounded to fp32, and that rounding alone leaves a residual of about
+ *                   2^-24 |L||P| / ||S||, which on 1000-cell-wide grids exceeds tol = 1e-5; d_P64_out satisfies eps_R <= tol
+ *   d_status        one int: the final status, written by the device when the solve ends -- the way to learn about
+ *                   OMNI_NOT_CONVERGED / OMNI_ERR_BREAKDOWN after a call made with info == NULL (no synchronisation)
+ * struct_size must be sizeof(omni_options) (omni_options_init sets it, loop_mode = -1 and everything else to 0 / NULL);
+ * a mismatch, hist_capacity < 0, a history pointer with hist_capacity == 0 or an unknown method: OMNI_ERR_INVALID_ARG. */
+enum { OMNI_METHOD_ALG1 = 0, OMNI_METHOD_DIRECT = 1, OMNI_METHOD_PCG = 2 };
+typedef struct {
+    size_t struct_size;
+    int loop_mode;
+    int hist_capacity;
+    double* d_hist_eps_R;
+    int* d_hist_cg_iters;
+    double* d_hist_eps_P;
+    double* d_P64_out;
+    int* d_status;
+} omni_options;
+void omni_options_init(omni_options* options);
+int omni_solve_ex_f64(int nx, int ny, int nz, double dx, double dy, double dz,
+                      const double* d_gx, const double* d_gy, const double* d_gz, const unsigned char* d_mask,
+                      const double* d_P_init, double* d_P_out, double tol, int max_outer, int max_cg, int method,
+                      const omni_options* options, void* stream, omni_info* info);
+int omni_solve_ex_f32(int nx, int ny, int nz, double dx, double dy, double dz,
+                      const float* d_gx, const float* d_gy, const float* d_gz, const unsigned char* d_mask,
+                      const float* d_P_init, float* d_P_out, double tol, int max_outer, int max_cg, int method,
+                      const omni_options* options, void* stream, omni_info* info);
+
 /* ---- Algorithm 1 from a first guess ("initializing with a first guess for the pressure field") -------------
  * omni_solve_* with P^0 = d_P_init (device, [nz][ny][nx]; values at missing cells are ignored; NULL = zeros, i.e.
  * omni_solve_*) instead of P^0 = 0 (:139): the next volume of a time series starts from the previous one's pressure.
@@ -287,7 +326,8 @@ int omni_set_loop_mode(int mode);
  * check; info.outer_iters + 1 entries for a completed solve, the first `capacity` of them if there are more.  d_cg_iters
  * (device, `capacity` ints, may be NULL) receives next to it the CG iterations of the outer iteration that led to the
  * check (0 for i = 0) -- the quantity behind the falling cost per iteration of Fig. 13 (:489).  No host
- * synchronisation is added.  (NULL, NULL, 0) switches it off.  Process-wide setting (like omni_set_loop_mode); a cascade solve
+ * synchronisation is added.  (NULL, NULL, 0) switches it off.  Process-wide DEFAULT (like omni_set_loop_mode; the per-call form is
+ * omni_options of omni_solve_ex_*, which also offers eps_P of Eq. 40); a cascade solve
  * leaves the history of its finest level.  Returns OMNI_OK, or OMNI_ERR_INVALID_ARG for capacity < 0 or a NULL d_hist
  * with capacity > 0 or with d_cg_iters given. */
 int omni_set_history(double* d_hist, int* d_cg_iters, int capacity);
@@ -301,7 +341,7 @@ void omni_release_memory(void);
 int omni_profile_enable(int on);          /* returns the previous setting */
 void omni_profile_read(double* h_ms3, long long* h_count3, int reset);
 const char* omni_status_string(int status);
-int omni_version(void);                  /* 100 * major + minor; 101 added the _guess, _rans_source and history entry points, 102 omni_solve_pcg_* */
+int omni_version(void);                  /* 100 * major + minor; 101 added the _guess, _rans_source and history entry points, 102 omni_solve_pcg_*, 103 omni_solve_ex_* / omni_options */
 
 #ifdef __cplusplus
 }

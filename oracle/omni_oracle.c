@@ -387,14 +387,24 @@ typedef struct {
 static int solve_impl(int nx, int ny, int nz, double dx, double dy, double dz,
                       const double *gx, const double *gy, const double *gz, const unsigned char *mask,
                       const double *P_init, double *P_out, double tol, int max_outer, int max_cg, oracle_info *info,
-                      double *hist, int hist_cap);
+                      double *hist, int hist_cap, double *hist_P);
 
 int oracle_solve(int nx, int ny, int nz, double dx, double dy, double dz,
                  const double *gx, const double *gy, const double *gz, const unsigned char *mask,
                  double *P_out, double tol, int max_outer, int max_cg, oracle_info *info,
                  double *hist, int hist_cap)
 {
-    return solve_impl(nx, ny, nz, dx, dy, dz, gx, gy, gz, mask, NULL, P_out, tol, max_outer, max_cg, info, hist, hist_cap);
+    return solve_impl(nx, ny, nz, dx, dy, dz, gx, gy, gz, mask, NULL, P_out, tol, max_outer, max_cg, info, hist, hist_cap, NULL);
+}
+
+/* oracle_solve that also records the pressure-update metric of Eq. 40 (:438): hist_P[n] = ||P^n - P^{n-1}|| / ||P^n||
+ * for n >= 1 (entry 0 = 0: no update yet), next to hist[n] = eps_R of Eq. 41 at the same check. */
+int oracle_solve_hist(int nx, int ny, int nz, double dx, double dy, double dz,
+                      const double *gx, const double *gy, const double *gz, const unsigned char *mask,
+                      double *P_out, double tol, int max_outer, int max_cg, oracle_info *info,
+                      double *hist, double *hist_P, int hist_cap)
+{
+    return solve_impl(nx, ny, nz, dx, dy, dz, gx, gy, gz, mask, NULL, P_out, tol, max_outer, max_cg, info, hist, hist_cap, hist_P);
 }
 
 /* Algorithm 1 started from a first guess instead of P^0 = 0 ("initializing with a first guess for the pressure field",
@@ -404,7 +414,7 @@ int oracle_solve_guess(int nx, int ny, int nz, double dx, double dy, double dz,
                        const double *gx, const double *gy, const double *gz, const unsigned char *mask,
                        const double *P_init, double *P_out, double tol, int max_outer, int max_cg, oracle_info *info)
 {
-    return solve_impl(nx, ny, nz, dx, dy, dz, gx, gy, gz, mask, P_init, P_out, tol, max_outer, max_cg, info, NULL, 0);
+    return solve_impl(nx, ny, nz, dx, dy, dz, gx, gy, gz, mask, P_init, P_out, tol, max_outer, max_cg, info, NULL, 0, NULL);
 }
 
 /* The fixed point of Alg. 1 computed without the boundary iteration: at convergence P^{n+1} = P^n, so Eq. 12 reads
@@ -418,7 +428,7 @@ int oracle_solve_direct(int nx, int ny, int nz, double dx, double dy, double dz,
                         const double *P_init, double *P_out, double tol, int max_outer, int max_cg, oracle_info *info)
 {
     g_direct = 1;
-    int rc = solve_impl(nx, ny, nz, dx, dy, dz, gx, gy, gz, mask, P_init, P_out, tol, max_outer, max_cg, info, NULL, 0);
+    int rc = solve_impl(nx, ny, nz, dx, dy, dz, gx, gy, gz, mask, P_init, P_out, tol, max_outer, max_cg, info, NULL, 0, NULL);
     g_direct = 0;
     return rc;
 }
@@ -437,7 +447,7 @@ int oracle_solve_batch2d(int nx, int ny, int nb, double dx, double dy,
         for (int b = 0; b < nb; ++b) memcpy(m + (size_t)b * nx * ny, mask2d, (size_t)nx * ny);
     }
     g_batch2d = 1;
-    int rc = solve_impl(nx, ny, nb, dx, dy, 1.0, gx, gy, NULL, m, P_init, P_out, tol, max_outer, max_cg, info, NULL, 0);
+    int rc = solve_impl(nx, ny, nb, dx, dy, 1.0, gx, gy, NULL, m, P_init, P_out, tol, max_outer, max_cg, info, NULL, 0, NULL);
     g_batch2d = 0;
     free(m);
     return rc;
@@ -457,7 +467,7 @@ int oracle_solve_direct_batch2d(int nx, int ny, int nb, double dx, double dy,
 static int solve_impl(int nx, int ny, int nz, double dx, double dy, double dz,
                       const double *gx, const double *gy, const double *gz, const unsigned char *mask,
                       const double *P_init, double *P_out, double tol, int max_outer, int max_cg, oracle_info *info,
-                      double *hist, int hist_cap)
+                      double *hist, int hist_cap, double *hist_P)
 {
     i64 N = (i64)nx * ny * nz;
     size_t nb = sizeof(double) * (size_t)N;
@@ -466,8 +476,9 @@ static int solve_impl(int nx, int ny, int nz, double dx, double dy, double dz,
     double *S = (double *)malloc(nb), *P = (double *)calloc((size_t)N, sizeof(double));
     double *rhs = (double *)malloc(nb), *r = (double *)malloc(nb), *p = (double *)malloc(nb), *q = (double *)malloc(nb);
     double *tmp = (double *)malloc(nb);
+    double *Pold = hist_P ? (double *)malloc(nb) : NULL;
     int rc = -1;
-    if (!v || !w1 || !w0 || !w0C || !S || !P || !rhs || !r || !p || !q || !tmp) goto done;
+    if (!v || !w1 || !w0 || !w0C || !S || !P || !rhs || !r || !p || !q || !tmp || (hist_P && !Pold)) goto done;
     rc = 0;
 
     oracle_validity(nx, ny, nz, gx, gy, gz, mask, v);
@@ -489,7 +500,17 @@ static int solve_impl(int nx, int ny, int nz, double dx, double dy, double dz,
             for (i64 c = 0; c < N; ++c) { rhs[c] += S[c]; r[c] = rhs[c] - q[c]; }
             epsR = sqrt(dot(N, nx, r, r)) / normS;
             if (hist && n < hist_cap) hist[n] = epsR;
+            if (hist_P && n < hist_cap) {            /* Eq. 40 :438 for the update that led to this check */
+                if (n == 0) hist_P[0] = 0.0;
+                else {
+#pragma omp parallel for if (N > OMP_MIN_N)
+                    for (i64 c = 0; c < N; ++c) tmp[c] = P[c] - Pold[c];
+                    double nP = sqrt(dot(N, nx, P, P));
+                    hist_P[n] = nP > 0.0 ? sqrt(dot(N, nx, tmp, tmp)) / nP : 0.0;
+                }
+            }
             if (epsR <= tol || n == max_outer) break;
+            if (hist_P) memcpy(Pold, P, nb);
             /* Solve Eq. 12 for P^{n+1} by CG, first guess P^n (:489); inner threshold: reading A3.
              * Fixed-point variant (oracle_solve_direct): the same loop with the system L P = S; eps_R above is its
              * residual too (r0 = S - L P^n), so the outer loop only restarts a CG that hit max_cg. */
@@ -504,7 +525,7 @@ static int solve_impl(int nx, int ny, int nz, double dx, double dy, double dz,
         info->norm_S = normS; info->converged = (epsR <= tol);
     }
 done:
-    free(v); free(w1); free(w0); free(w0C); free(S); free(P); free(rhs); free(r); free(p); free(q); free(tmp);
+    free(v); free(w1); free(w0); free(w0C); free(S); free(P); free(rhs); free(r); free(p); free(q); free(tmp); free(Pold);
     return rc;
 }
 

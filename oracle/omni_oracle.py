@@ -159,6 +159,28 @@ def solve(gx, gy, gz, mask, dx, dy, dz, tol, max_outer, max_cg, hist_cap=0):
     return (P, d, hist) if hist_cap else (P, d)
 
 
+def solve_hist(gx, gy, gz, mask, dx, dy, dz, tol, max_outer, max_cg, hist_cap):
+    """Algorithm 1 with both convergence metrics recorded per outer check: eps_R (Eq. 41 :442) and the pressure-update
+    metric eps_P (Eq. 40 :438; entry 0 = 0).  Returns (P, info dict, hist_R, hist_P)."""
+    gx, gy = _f64(gx), _f64(gy)
+    nx, ny, nz = _dims(gx.shape)
+    gz = _f64(gz) if gz is not None else None
+    m = None if mask is None else np.ascontiguousarray(mask, dtype=np.uint8)
+    P = np.zeros(gx.shape)
+    info = Info()
+    hR, hP = np.full(hist_cap, np.nan), np.full(hist_cap, np.nan)
+    f = lib().oracle_solve_hist
+    f.restype = C.c_int
+    rc = f(C.c_int(nx), C.c_int(ny), C.c_int(nz), C.c_double(dx), C.c_double(dy), C.c_double(dz),
+           _p(gx), _p(gy), _p(gz if gz is not None else gx), _p(m), _p(P), C.c_double(tol), C.c_int(max_outer),
+           C.c_int(max_cg), C.byref(info), _p(hR), _p(hP), C.c_int(hist_cap))
+    if rc != 0:
+        raise MemoryError("oracle_solve_hist: allocation failed")
+    d = {"outer_iters": info.outer_iters, "cg_iters_total": info.cg_iters_total, "eps_R_final": info.eps_R_final,
+         "norm_S": info.norm_S, "converged": bool(info.converged)}
+    return P, d, hR, hP
+
+
 def solve_guess(gx, gy, gz, mask, dx, dy, dz, tol, max_outer, max_cg, P_init):
     """Algorithm 1 started from the first guess P_init (oracle_solve_guess).  Returns (P, info)."""
     gx, gy = _f64(gx), _f64(gy)

@@ -17,7 +17,7 @@ STATUS_NAMES = {0: "OMNI_OK", 1: "OMNI_NOT_CONVERGED", -1: "OMNI_ERR_INVALID_ARG
                 -3: "OMNI_ERR_ALLOC", -4: "OMNI_ERR_BREAKDOWN"}
 # every symbol include/omni.h declares
 SYMBOLS = ["omni_solve_f64", "omni_solve_f32", "omni_workspace_bytes", "omni_solve_f64_ws", "omni_solve_f32_ws",
-           "omni_solve_host_f64", "omni_solve_host_f32", "omni_solve_batch2d_f64", "omni_solve_batch2d_f32", "omni_solve_guess_f64", "omni_solve_guess_f32", "omni_solve_direct_f64", "omni_solve_direct_f32", "omni_solve_pcg_f64", "omni_solve_pcg_f32", "omni_solve_direct_batch2d_f64", "omni_solve_direct_batch2d_f32", "omni_solve_cascade_f64", "omni_solve_cascade_f32", "omni_velocity_source_f64", "omni_velocity_source_f32", "omni_rans_source_f64", "omni_rans_source_f32",
+           "omni_solve_host_f64", "omni_solve_host_f32", "omni_solve_batch2d_f64", "omni_solve_batch2d_f32", "omni_solve_guess_f64", "omni_solve_guess_f32", "omni_solve_direct_f64", "omni_solve_direct_f32", "omni_solve_pcg_f64", "omni_solve_pcg_f32", "omni_solve_ex_f64", "omni_solve_ex_f32", "omni_options_init", "omni_solve_direct_batch2d_f64", "omni_solve_direct_batch2d_f32", "omni_solve_cascade_f64", "omni_solve_cascade_f32", "omni_velocity_source_f64", "omni_velocity_source_f32", "omni_rans_source_f64", "omni_rans_source_f32",
            "omni_compressible_rans_source_f64", "omni_compressible_rans_source_f32", "omni_constants", "omni_source_f64", "omni_source_f32",
            "omni_apply_M_f64", "omni_apply_M_f32", "omni_residual_f64", "omni_residual_f32", "omni_launch_count",
            "omni_set_loop_mode", "omni_set_history", "omni_release_memory", "omni_profile_enable", "omni_profile_read", "omni_status_string", "omni_version"]
@@ -247,6 +247,51 @@ def solve_direct(gx, gy, gz, mask, d, tol, max_outer, max_cg, out=None, P_init=N
 def solve_pcg(gx, gy, gz, mask, d, tol, max_outer, max_cg, out=None, P_init=None):
     """omni_solve_pcg_*: the fixed point L P = S by multigrid-preconditioned CG (include/omni.h).  Returns (P, info dict)."""
     return solve_direct(gx, gy, gz, mask, d, tol, max_outer, max_cg, out=out, P_init=P_init, _entry="omni_solve_pcg")
+
+
+class Options(C.Structure):
+    """omni_options of include/omni.h."""
+    _fields_ = [("struct_size", C.c_size_t), ("loop_mode", C.c_int), ("hist_capacity", C.c_int),
+                ("d_hist_eps_R", C.c_void_p), ("d_hist_cg_iters", C.c_void_p), ("d_hist_eps_P", C.c_void_p),
+                ("d_P64_out", C.c_void_p), ("d_status", C.c_void_p)]
+
+
+METHODS = {"alg1": 0, "direct": 1, "pcg": 2}
+
+
+def solve_ex(gx, gy, gz, mask, d, tol, max_outer, max_cg, method="alg1", P_init=None, out=None, loop_mode=-1,
+             hist_eps_R=None, hist_cg_iters=None, hist_eps_P=None, P64_out=None, status=None, want_info=True):
+    """omni_solve_ex_*: one solve with per-call options (omni_options): loop mode, history buffers (CUDA float64 /
+    int32 tensors of one common length), the fp64 master pressure (CUDA float64 tensor shaped like gx) and a device
+    status word (CUDA int32 tensor with one element).  Returns (P, info dict or None)."""
+    import torch
+    sfx = _suffix(gx)
+    _check([gx, gy, gz, mask, out, P_init, hist_eps_R, hist_cg_iters, hist_eps_P, P64_out, status], "cuda")
+    _check_like(gx, [("gy", gy), ("gz", gz), ("out", out), ("P_init", P_init)], mask)
+    hs = [t for t in (hist_eps_R, hist_cg_iters, hist_eps_P) if t is not None]
+    cap = hs[0].numel() if hs else 0
+    for t, dt in ((hist_eps_R, torch.float64), (hist_cg_iters, torch.int32), (hist_eps_P, torch.float64)):
+        if t is not None and (t.dtype != dt or t.numel() != cap):
+            raise TypeError("history tensors: float64 / int32 / float64, one common length")
+    if P64_out is not None and (P64_out.dtype != torch.float64 or tuple(P64_out.shape) != tuple(gx.shape)):
+        raise TypeError("P64_out must be float64 with the shape of gx")
+    if status is not None and (status.dtype != torch.int32 or status.numel() != 1):
+        raise TypeError("status must be one int32")
+    o = Options()
+    lib().omni_options_init(C.byref(o))
+    o.loop_mode, o.hist_capacity = loop_mode, cap
+    o.d_hist_eps_R, o.d_hist_cg_iters, o.d_hist_eps_P = (None if t is None else t.data_ptr() for t in (hist_eps_R, hist_cg_iters, hist_eps_P))
+    o.d_P64_out = None if P64_out is None else P64_out.data_ptr()
+    o.d_status = None if status is None else status.data_ptr()
+    P = out if out is not None else torch.empty_like(gx)
+    info = Info()
+    with torch.cuda.device(gx.device):
+        fn = getattr(lib(), f"omni_solve_ex_{sfx}")
+        rc = fn(*_geom(gx, d), _ptr(gx), _ptr(gy), _ptr(gz), _ptr(mask), _ptr(P_init), _ptr(P), C.c_double(tol), C.c_int(max_outer),
+                C.c_int(max_cg), C.c_int(METHODS[method]), C.byref(o), _stream(gx.device), C.byref(info) if want_info else None)
+    if rc < 0:
+        raise OmniError(rc, f"omni_solve_ex_{sfx}")
+    return P, (info.as_dict() if want_info else None)
 
 
 def velocity_source(u, v, w, mask, d, rho=1.0, mu=0.0, dudt=None):

@@ -56,6 +56,26 @@ std::atomic<double*> g_hist{nullptr};     // omni_set_history: device buffer for
 std::atomic<int> g_hist_cap{0};
 std::atomic<int*> g_hist_k{nullptr};
 
+// Per-call options (omni_options of include/omni.h).  omni_solve_ex_* installs its caller's struct for the duration of
+// the call on the calling thread; every other entry point runs with the process-wide defaults the omni_set_* setters
+// maintain.  Nothing a call reads can be changed by another thread's call.
+struct CallOpts {
+    int loop_mode;
+    double* hist; int* hist_k; double* hist_p; int hist_cap;
+    double* P64;
+    int* status;
+};
+thread_local const CallOpts* tl_opts = nullptr;
+CallOpts current_opts()
+{
+    if (tl_opts) return *tl_opts;
+    CallOpts o;
+    o.loop_mode = g_loop_mode.load();
+    o.hist = g_hist.load(); o.hist_k = g_hist_k.load(); o.hist_p = nullptr; o.hist_cap = g_hist_cap.load();
+    o.P64 = nullptr; o.status = nullptr;
+    return o;
+}
+
 // optional per-kernel timing of the host-driven loop (omni_profile_*): CUDA events around every K2/K3/K4 launch
 std::atomic<int> g_profile{0};
 std::mutex g_prof_mu;
@@ -305,9 +325,9 @@ size_t partial_slots(const Geom& g)
 {
     // one fp64 slot per CTA and accumulator.  1D kernels: at most ceil(npad / 256) blocks.  Tile kernels: NACC x
     // (x tiles) x (y tiles) x (z segments) with at most nz segments; the finest tiling is K2's (64 cells x 8 rows,
-    // NACC = 2).  A thin cross-section with a long z axis has far more tile CTAs than npad / 256 (launch_tma checks).
+    // NACC = 4).  A thin cross-section with a long z axis has far more tile CTAs than npad / 256 (launch_tma checks).
     const size_t lin = (size_t)((g.npad + 255) / 256) * 2 + 64;
-    const size_t tile = (size_t)2 * (size_t)((g.px + 63) / 64) * (size_t)((g.ny + OMNI_BY - 1) / OMNI_BY) * (size_t)g.nz + 64;
+    const size_t tile = (size_t)4 * (size_t)((g.px + 63) / 64) * (size_t)((g.ny + OMNI_BY - 1) / OMNI_BY) * (size_t)g.nz + 64;
     return std::max(lin, tile);
 }
 
@@ -345,13 +365,14 @@ size_t carve(const Geom& g, char* base, Workspace<T>* w)
 }
 
 __global__ void init_scalars_kernel(Scalars* sc, double tol, int max_outer, int max_cg, double* hist = nullptr, int hist_cap = 0,
-                                    int* hist_k = nullptr, double inner_rel = 0.0)
+                                    int* hist_k = nullptr, double inner_rel = 0.0, double* hist_p = nullptr, int* status_out = nullptr)
 {
     Scalars s;
     memset(&s, 0, sizeof(s));
     s.tol = tol; s.max_outer = max_outer; s.max_cg = max_cg;
     s.inner_rel2 = inner_rel * inner_rel;
-    s.hist = hist; s.hist_k = hist_k; s.hist_cap = hist_cap; s.hist_n = 0;
+    s.hist = hist; s.hist_k = hist_k; s.hist_p = hist_p; s.hist_cap = hist_cap; s.hist_n = 0;
+    s.status_out = status_out;
     s.inner_go = 0; s.outer_go = 1; s.status = ST_OK;
     s.dzero = 1;                     // no CG iteration has run yet: the first K2 takes delta as zero
     s.bar_count = 2;                 // grid barrier of the loop kernel: set 0, tag 1 against zeroed slots (omni_persist.cuh)
@@ -1053,7 +1074,8 @@ int solve_ws(int nx, int ny, int nz, double dx, double dy, double dz, const T* g
     // floor the recursive residual at ~1e-4 ||r0|| on 1000-cell-wide grids), so it hands back to the fp64 refinement
     // after two digits (reading R-P1)
     const double inner_rel = (pcg && sizeof(T) == 4) ? OMNI_PCG_INNER_REL_F32 : 0.0;
-    init_scalars_kernel<<<1, 1, 0, st>>>(w.sc, tol, max_outer, max_cg, g_hist.load(), g_hist_cap.load(), g_hist_k.load(), inner_rel);
+    const CallOpts opt = current_opts();
+    init_scalars_kernel<<<1, 1, 0, st>>>(w.sc, tol, max_outer, max_cg, opt.hist, opt.hist_cap, opt.hist_k, inner_rel, opt.hist_p, opt.status);
     CK(cudaGetLastError());
     g_launches.fetch_add(1, std::memory_order_relaxed);
     int rc = setup_codes<T>(g, w, gx, gy, gz, mask, st);
@@ -1068,7 +1090,7 @@ int solve_ws(int nx, int ny, int nz, double dx, double dy, double dz, const T* g
         g_launches.fetch_add(2, std::memory_order_relaxed);
     }
 
-    int mode = g_loop_mode.load();
+    int mode = opt.loop_mode;
     if (mode == 0) mode = (g.npad <= persist_max_cells()) ? 3 : (g.npad <= loopk_max_cells()) ? 4 : 2;
     MgHier<T> mg;
     mg.mem = nullptr; mg.launches_per_cycle = 0;
@@ -1094,7 +1116,7 @@ int solve_ws(int nx, int ny, int nz, double dx, double dy, double dz, const T* g
     else if (mode == 2) rc = lop ? run_loop_graph<T, true>(g, w, H, K, st) : run_loop_graph<T, false>(g, w, H, K, st);
     if (rc != OMNI_OK) return rc;
 
-    finalize_kernel<T><<<blocks_for((long long)nx * ny * nz, 256), 256, 0, st>>>(g, w.P, w.P1, w.sc, w.link, P_out);
+    finalize_kernel<T><<<blocks_for((long long)nx * ny * nz, 256), 256, 0, st>>>(g, w.P, w.P1, w.sc, w.link, P_out, opt.P64);
     CK(cudaGetLastError());
     g_launches.fetch_add(1, std::memory_order_relaxed);
 
@@ -1549,6 +1571,56 @@ int omni_solve_pcg_f32(int nx, int ny, int nz, double dx, double dy, double dz, 
                               0, d_P_init, 1, 1);
 }
 
+void omni_options_init(omni_options* o)
+{
+    if (!o) return;
+    memset(o, 0, sizeof(*o));
+    o->struct_size = sizeof(omni_options);
+    o->loop_mode = -1;
+}
+
+extern "C++" {
+namespace {
+template <typename T>
+int solve_ex(int nx, int ny, int nz, double dx, double dy, double dz, const T* gx, const T* gy, const T* gz,
+             const unsigned char* mask, const T* P_init, T* P_out, double tol, int max_outer, int max_cg, int method,
+             const omni_options* o, void* stream, omni_info* info)
+{
+    if (method != OMNI_METHOD_ALG1 && method != OMNI_METHOD_DIRECT && method != OMNI_METHOD_PCG) return OMNI_ERR_INVALID_ARG;
+    CallOpts c = current_opts();
+    if (o) {
+        if (o->struct_size != sizeof(omni_options)) return OMNI_ERR_INVALID_ARG;
+        if (o->loop_mode > 4 || o->loop_mode < -1 || o->hist_capacity < 0) return OMNI_ERR_INVALID_ARG;
+        if (o->hist_capacity == 0 && (o->d_hist_eps_R || o->d_hist_cg_iters || o->d_hist_eps_P)) return OMNI_ERR_INVALID_ARG;
+        if (o->loop_mode >= 0) c.loop_mode = o->loop_mode;
+        c.hist = o->d_hist_eps_R; c.hist_k = o->d_hist_cg_iters; c.hist_p = o->d_hist_eps_P; c.hist_cap = o->hist_capacity;
+        c.P64 = o->d_P64_out; c.status = o->d_status;
+    }
+    tl_opts = &c;
+    const int rc = solve_alloc<T>(nx, ny, nz, dx, dy, dz, gx, gy, gz, mask, P_out, tol, max_outer, max_cg, stream, info, 0, P_init,
+                                  method != OMNI_METHOD_ALG1, method == OMNI_METHOD_PCG);
+    tl_opts = nullptr;
+    return rc;
+}
+}  // namespace
+}  // extern "C++"
+
+int omni_solve_ex_f64(int nx, int ny, int nz, double dx, double dy, double dz, const double* d_gx, const double* d_gy,
+                      const double* d_gz, const unsigned char* d_mask, const double* d_P_init, double* d_P_out, double tol,
+                      int max_outer, int max_cg, int method, const omni_options* options, void* stream, omni_info* info)
+{
+    return solve_ex<double>(nx, ny, nz, dx, dy, dz, d_gx, d_gy, d_gz, d_mask, d_P_init, d_P_out, tol, max_outer, max_cg, method,
+                            options, stream, info);
+}
+
+int omni_solve_ex_f32(int nx, int ny, int nz, double dx, double dy, double dz, const float* d_gx, const float* d_gy,
+                      const float* d_gz, const unsigned char* d_mask, const float* d_P_init, float* d_P_out, double tol,
+                      int max_outer, int max_cg, int method, const omni_options* options, void* stream, omni_info* info)
+{
+    return solve_ex<float>(nx, ny, nz, dx, dy, dz, d_gx, d_gy, d_gz, d_mask, d_P_init, d_P_out, tol, max_outer, max_cg, method,
+                           options, stream, info);
+}
+
 int omni_solve_cascade_f64(int nx, int ny, int nz, double dx, double dy, double dz, const double* d_gx, const double* d_gy,
                            const double* d_gz, const unsigned char* d_mask, double* d_P_out, double tol, int max_outer,
                            int max_cg, int levels, void* stream, omni_info* info)
@@ -1736,6 +1808,6 @@ const char* omni_status_string(int status)
     }
 }
 
-int omni_version(void) { return 102; }   // 101: omni_solve_guess_*, omni_set_history, omni_rans_source_*, omni_compressible_rans_source_*
+int omni_version(void) { return 103; }   // 101: omni_solve_guess_*, omni_set_history, omni_rans_source_*, omni_compressible_rans_source_*
 
 }  // extern "C"

@@ -91,16 +91,21 @@ struct Scalars {
     unsigned int bar_count;  // use count of the loop kernel's grid barrier, carried from one launch to the next (omni_loop.cuh)
     // optional residual history (omni_set_history): eps_R (Eq. 41) of every outer residual check, entry i = check i
     // and, optionally, the CG iterations the outer iteration before the check took (0 for the first check)
+    // and the pressure-update metric eps_P (Eq. 40 :438) of the update that led to the check (0 for the first check)
     double* hist;
     int* hist_k;
+    double* hist_p;
     int hist_cap, hist_n;
+    int* status_out;   // optional device word that receives the final status (omni_options::d_status)
 };
 
-__device__ __forceinline__ void record_history(Scalars* s, double epsR2, int k_prev)
+// dP2 = ||P^n - P^(n-1)||^2, P2 = ||P^n||^2 (Eq. 40); either 0 when nothing was folded
+__device__ __forceinline__ void record_history(Scalars* s, double epsR2, int k_prev, double dP2 = 0.0, double P2 = 0.0)
 {
-    if (s->hist != nullptr && s->hist_n < s->hist_cap) {
-        s->hist[s->hist_n] = (s->normS2 > 0.0) ? sqrt(epsR2 / s->normS2) : 0.0;
+    if (s->hist_n < s->hist_cap) {
+        if (s->hist != nullptr) s->hist[s->hist_n] = (s->normS2 > 0.0) ? sqrt(epsR2 / s->normS2) : 0.0;
         if (s->hist_k != nullptr) s->hist_k[s->hist_n] = k_prev;
+        if (s->hist_p != nullptr) s->hist_p[s->hist_n] = (P2 > 0.0) ? sqrt(dP2 / P2) : 0.0;
     }
     s->hist_n += 1;
 }
@@ -651,11 +656,12 @@ source_kernel(Geom g, const T* __restrict__ gx, const T* __restrict__ gy, const 
 // ------------------------------------------------------------------------------------------------ K7 finalize
 template <typename T>
 __global__ void finalize_kernel(Geom g, const double* P0, const double* P1, const Scalars* sc,
-                                const uint8_t* __restrict__ link, T* __restrict__ out)
+                                const uint8_t* __restrict__ link, T* __restrict__ out, double* __restrict__ out64)
 {
     const double* __restrict__ P = (sc->n & 1) ? P0 : P1;      // the last K2 wrote Pbuf[(n & 1) ^ 1]
     long long u = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     long long nuser = (long long)g.nx * g.ny * g.nz;
+    if (u == 0 && sc->status_out != nullptr) *sc->status_out = sc->status;
     if (u >= nuser) return;
     int i;
     long long row;
@@ -668,7 +674,9 @@ __global__ void finalize_kernel(Geom g, const double* P0, const double* P1, cons
         row = u / g.nx;
     }
     const long long pid = row * g.px + i;
-    out[u] = (link[pid] & LINK_VALID) ? (T)P[pid] : (T)nan("");
+    const bool ok = (link[pid] & LINK_VALID) != 0;
+    out[u] = ok ? (T)P[pid] : (T)nan("");
+    if (out64 != nullptr) out64[u] = ok ? P[pid] : nan("");      // the fp64 master pressure itself (omni_options::d_P64_out)
 }
 
 // copies between the caller's unpadded layout and the padded internal layout (step entry points only)

@@ -96,7 +96,7 @@ tma_loop_kernel(const Geom g, const ZSeg zs, const LoopArgs<K2, K3, K4> a, const
         // ------------------------------------------------------------------ K2: P += delta, r = S - L P, eps_R (Eq. 41)
         {
             const typename K2::Ctx c2(a.a2, n, dzero);
-            double acc[2] = { 0.0, 0.0 }, tot[2];
+            double acc[4] = { 0.0, 0.0, 0.0, 0.0 }, tot[2];
             LOOP_TRACE_BEGIN()
 #pragma unroll 1
             for (int h = 0; h < XR; ++h) {
@@ -111,10 +111,14 @@ tma_loop_kernel(const Geom g, const ZSeg zs, const LoopArgs<K2, K3, K4> a, const
             }
             fence_proxy_async_global();              // this phase's stores, before the release in the barrier
             LOOP_TRACE_MID()
-            if (!grid_allreduce<2, NT>(gs, a.slots, acc, tot)) { status = ST_BARRIER_TIMEOUT; break; }
+            const double acc01[2] = { acc[0], acc[1] }, acc23[2] = { acc[2], acc[3] };
+            double totp[2] = { 0.0, 0.0 };
+            if (!grid_allreduce<2, NT>(gs, a.slots, acc01, tot)) { status = ST_BARRIER_TIMEOUT; break; }
+            // Eq. 40 only when its history was asked for (grid-uniform): a second exchange
+            if (sc->hist_p != nullptr && !grid_allreduce<2, NT>(gs, a.slots, acc23, totp)) { status = ST_BARRIER_TIMEOUT; break; }
             LOOP_TRACE_END(trace_ph);
             epsR2 = tot[0];
-            if (blockIdx.x == 0 && threadIdx.x == 0) record_history(sc, tot[0], k);
+            if (blockIdx.x == 0 && threadIdx.x == 0) record_history(sc, tot[0], k, totp[0], totp[1]);
             if (!isfinite(tot[0])) { status = ST_BREAKDOWN; break; }
             if (tot[0] <= tol2S || n >= max_outer) { status = (tot[0] <= tol2S) ? ST_OK : ST_NOT_CONVERGED; break; }
             n += 1;

@@ -226,7 +226,8 @@ persist_kernel(const Geom g, const PersistArgs<T> a)
             const int par = n & 1;
             const double* Pin = a.Pbuf[par];
             double* Pout = a.Pbuf[par ^ 1];
-            double acc[2] = { 0.0, 0.0 };
+            double acc[2] = { 0.0, 0.0 }, accp[2] = { 0.0, 0.0 };
+            const bool want_p = sc->hist_p != nullptr;             // Eq. 40 history asked for (grid-uniform)
             RowTask<2> tk(g, lo2 + wfirst, nsx2, wstep, lane);
             for (int t = lo2 + wfirst; t < hi2; t += wstep, tk.next(g, lane)) {
                 auto val = [&](long long i, bool ok, double (&v)[2]) {
@@ -296,13 +297,22 @@ persist_kernel(const Geom g, const PersistArgs<T> a)
                     rn[i] = (T)rr;
                     acc[0] += rr * rr;
                     acc[1] += (double)rn[i] * (double)rn[i];
+                    if (want_p && (l & LINK_VALID)) accp[1] += vc[i] * vc[i];
+                }
+                if (want_p && !dzero) {
+                    T d[2];
+                    ldcg_chunk<T, 2>(a.delta + tk.idx, d);
+#pragma unroll
+                    for (int i = 0; i < 2; ++i)
+                        if ((lk >> (8 * i)) & LINK_VALID) accp[0] += (double)d[i] * (double)d[i];
                 }
                 st_chunk<T, 2>(a.r + tk.idx, rn);
             }
-            double tot[2];
+            double tot[2], totp[2] = { 0.0, 0.0 };
             if (!grid_allreduce<2, NT>(gs, a.slots, acc, tot)) { status = ST_BARRIER_TIMEOUT; break; }
+            if (want_p && !grid_allreduce<2, NT>(gs, a.slots, accp, totp)) { status = ST_BARRIER_TIMEOUT; break; }
             epsR2 = tot[0];
-            if (blockIdx.x == 0 && threadIdx.x == 0) record_history(sc, tot[0], k);
+            if (blockIdx.x == 0 && threadIdx.x == 0) record_history(sc, tot[0], k, totp[0], totp[1]);
             if (!isfinite(tot[0])) { status = ST_BREAKDOWN; break; }
             if (tot[0] <= tol2S || n >= max_outer) { status = (tot[0] <= tol2S) ? ST_OK : ST_NOT_CONVERGED; break; }
             n += 1;

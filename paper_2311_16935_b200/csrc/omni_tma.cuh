@@ -690,7 +690,8 @@ struct OpT2 {
         static constexpr int TILE_P = (BOX_P + 127) / 128 * 128, TILE_D = (BOX_D + 127) / 128 * 128;
         static constexpr int TILE_S = BY_ * BX * (int)sizeof(T);
     };
-    enum { V = 2, R = R_, D = D_, DMAX = D_, MINB = MINB_, NACC = 2, TICKET = 2, STAGE_BYTES = TG::TILE_P + TG::TILE_D + TG::TILE_S,
+    // accumulators: ||r0||^2 in fp64, ||r0 rounded to T||^2 (= rho of the CG), ||delta||^2 and ||P + delta||^2 (Eq. 40)
+    enum { V = 2, R = R_, D = D_, DMAX = D_, MINB = MINB_, NACC = 4, TICKET = 2, STAGE_BYTES = TG::TILE_P + TG::TILE_D + TG::TILE_S,
            SMEM_BYTES = D_ * STAGE_BYTES };
     static constexpr bool REV = false;
     struct Args {
@@ -753,10 +754,16 @@ struct OpT2 {
         v[0] = P[0] + (double)d[0];
         v[1] = P[1] + (double)d[1];
     }
+    __device__ static void delta_of(uint32_t st, int offD, bool dz, double (&dd)[V])
+    {
+        T d[2] = { T(0), T(0) };
+        if (!dz) lds_pair(st + TG::TILE_P + offD, d);
+        dd[0] = (double)d[0]; dd[1] = (double)d[1];
+    }
     template <bool CLEAN>
     __device__ static void emit(const Args& a, const Ctx& c, const State&, long long idx, int px, uint32_t sB, uint32_t sC, uint32_t sF,
                                 int warp, int lane, const bool (&out)[R], const uint32_t (&fb)[R], const uint32_t (&code)[R][V],
-                                const TC& lk_x, const int (&ycls)[R], int zcls, double (&acc)[2])
+                                const TC& lk_x, const int (&ycls)[R], int zcls, double (&acc)[4])
     {
         const int rowP0 = (warp * R + 1) * TG::PITCH_P, rowD0 = (warp * R + 1) * TG::PITCH_D;
         const int xP = (TG::HXP + lane * V) * 8, xD = (TG::HXD + lane * V) * (int)sizeof(T);
@@ -794,6 +801,8 @@ struct OpT2 {
             if (!CLEAN && fb[r]) lk = code[r][0];
             T S[2];
             lds_pair(sC + TG::TILE_P + TG::TILE_D + ((warp * R + r) * TG::BX + lane * V) * (int)sizeof(T), S);
+            double dd[V];
+            delta_of(sC, rowD + xD, c.dz, dd);
             T rn[V];
 #pragma unroll
             for (int i = 0; i < V; ++i) {
@@ -811,16 +820,17 @@ struct OpT2 {
                 rn[i] = (T)rr;
                 acc[0] += rr * rr;
                 acc[1] += (double)rn[i] * (double)rn[i];
+                if (l & LINK_VALID) { acc[2] += dd[i] * dd[i]; acc[3] += vc[i] * vc[i]; }
             }
             st_chunk<T, V>(a.r + cell, rn);
         }
     }
-    __device__ static void finalize(const Args& a, const double (&tot)[2])
+    __device__ static void finalize(const Args& a, const double (&tot)[4])
     {
         Scalars* s = a.sc;
         s->epsR2 = tot[0];
         if (!a.fold_delta) return;
-        record_history(s, tot[0], s->k);
+        record_history(s, tot[0], s->k, tot[2], tot[3]);
         if (!isfinite(tot[0])) {
             s->status = ST_BREAKDOWN; s->inner_go = 0; s->outer_go = 0;
             set_cond(a.cond, 0, 0);

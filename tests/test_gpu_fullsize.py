@@ -192,15 +192,21 @@ def test_converged_field_certified_by_oracle(oracle, idx, dtype):
     configs[4] by Alg. 1 takes about two minutes of GPU time (10 500 outer iterations)."""
     f, g_dev, g_or, mask, m_dev = _load(idx, dtype)
     d, tol = f["d"], TOL_CONV[dtype]
-    runs = [("alg1", lambda: omni.solve(g_dev[0], g_dev[1], g_dev[2], m_dev, d, tol, 400000, 16)),
+    P64 = torch.zeros(f["g"][0].shape, dtype=torch.float64, device="cuda") if dtype == "f32" else None
+    runs = [("alg1", lambda: omni.solve_ex(g_dev[0], g_dev[1], g_dev[2], m_dev, d, tol, 400000, 16, method="alg1", P64_out=P64)),
             ("cascade", lambda: omni.solve_cascade(g_dev[0], g_dev[1], g_dev[2], m_dev, d, tol, 20, 30000, levels=4)),
-            ("pcg", lambda: omni.solve_pcg(g_dev[0], g_dev[1], g_dev[2], m_dev, d, tol, 20, 300))]
+            ("pcg", lambda: omni.solve_ex(g_dev[0], g_dev[1], g_dev[2], m_dev, d, tol, 20, 300, method="pcg", P64_out=P64))]
     for name, fn in runs:
         P, info = fn()
         assert info["status"] == 0 and info["eps_R_final"] <= tol, (name, info)
         Pn = P.cpu().numpy()
         eps, nr, nS = oracle.eps_R_of_field(g_or[0], g_or[1], g_or[2], mask, Pn, *d)
         assert nS == pytest.approx(info["norm_S"], rel=1e-5 if dtype == "f32" else 1e-11)
+        if P64 is not None and name != "cascade":
+            # the fp64 master pressure of the fp32 solve (omni_options::d_P64_out) meets tol in the oracle's eyes
+            e64, _, _ = oracle.eps_R_of_field(g_or[0], g_or[1], g_or[2], mask, P64.cpu().numpy(), *d)
+            print(f"configs[{idx}] {dtype} {name}: oracle eps_R of the fp64 master pressure {e64:.3e}")
+            assert e64 <= 1.05 * tol, (name, e64)
         if dtype == "f64":
             bound = 1.05 * tol
         else:

@@ -931,3 +931,62 @@ def test_pcg_converged(oracle, dtype, tol):
         Pd, idd = omni.solve_direct(g_dev[0], g_dev[1], g_dev[2], m_dev, d, tol, 10, 5000)
         assert idd["status"] == 0 and idd["cg_iters_total"] > 3 * info["cg_iters_total"]
         assert rel_l2_after_mean_removal(P.cpu().numpy(), Pd.cpu().numpy(), valid) <= bound
+
+
+@pytest.mark.parametrize("loop", list(LOOPS))
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_solve_ex_options(oracle, dtype, loop):
+    """omni_solve_ex_* with per-call omni_options: the three history columns (eps_R of Eq. 41, CG iterations, eps_P of
+    Eq. 40) against oracle.solve_hist through every loop driver; the fp64 master pressure d_P64_out (the fp32 result
+    is its rounding, and the ORACLE's eps_R of it meets tol where the fp32 field's cannot); the device status word after
+    a call without info; the per-call loop mode leaves the process-wide one alone."""
+    f = make_field("lamb_oseen2d", (40, 52), seed=3, noise=0.05)
+    g_dev, g_or, m_dev, m = _inputs(f, dtype)
+    d = f["d"]
+    cap = 16
+    hR = torch.full((cap,), -1.0, dtype=torch.float64, device="cuda")
+    hP = torch.full((cap,), -1.0, dtype=torch.float64, device="cuda")
+    hK = torch.full((cap,), -1, dtype=torch.int32, device="cuda")
+    P64 = torch.zeros(f["g"][0].shape, dtype=torch.float64, device="cuda")
+    st = torch.full((1,), 77, dtype=torch.int32, device="cuda")
+    before = omni.set_loop_mode(0); omni.set_loop_mode(before)
+    P, info = omni.solve_ex(g_dev[0], g_dev[1], None, m_dev, d, 0.0, 12, 15, method="alg1", loop_mode=LOOPS[loop],
+                            hist_eps_R=hR, hist_cg_iters=hK, hist_eps_P=hP, P64_out=P64, status=st)
+    after = omni.set_loop_mode(0); omni.set_loop_mode(after)
+    assert before == after
+    Po, io, oR, oP = oracle.solve_hist(g_or[0], g_or[1], None, m, *d, tol=0.0, max_outer=12, max_cg=15, hist_cap=cap)
+    assert info["outer_iters"] == io["outer_iters"] == 12 and int(st.item()) == info["status"] == 1
+    r, p, k = hR.cpu().numpy(), hP.cpu().numpy(), hK.cpu().numpy()
+    rel = 2e-3 if dtype == "f32" else 1e-7
+    assert np.allclose(r[:13], oR[:13], rtol=rel) and np.all(r[13:] == -1.0)
+    assert p[0] == 0.0 and np.allclose(p[1:13], oP[1:13], rtol=rel) and np.all(p[13:] == -1.0)
+    assert k[0] == 0 and np.all(k[1:13] == 15)
+    valid = ~np.isnan(Po)
+    P64n = P64.cpu().numpy()
+    assert np.array_equal(np.isnan(P64n), ~valid)
+    assert np.array_equal(P.cpu().numpy(), P64n.astype(np.float32 if dtype == "f32" else np.float64), equal_nan=True)
+    assert rel_l2_after_mean_removal(P64n, Po, valid) <= TOL_SOLVE[dtype]
+    # no info: the call does not synchronise; the status word tells how it ended
+    st.fill_(77)
+    _, none = omni.solve_ex(g_dev[0], g_dev[1], None, m_dev, d, 1e-3, 100000, 16, method="pcg" if loop == "graph" else "direct",
+                            loop_mode=LOOPS[loop], status=st, want_info=False)
+    assert none is None
+    torch.cuda.synchronize()
+    assert int(st.item()) == 0
+
+
+@pytest.mark.parametrize("method", ["alg1", "direct", "pcg"])
+def test_fp64_master_pressure_meets_tol_where_fp32_output_cannot(oracle, method):
+    """configs[1] stand-in 384^2 in fp32, tol 1e-5: the oracle's eps_R (Eq. 41) of d_P64_out is <= 1.05 tol; of the fp32
+    result it is the larger rounding floor 2^-24 |L||P| / ||S|| (SURVEY 7 hard part 3) -- which is why the option exists."""
+    f = make_config(1, 384)
+    g_dev, g_or, m_dev, m = _inputs(f, "f32")
+    d, tol = f["d"], 1e-5
+    P64 = torch.zeros(f["g"][0].shape, dtype=torch.float64, device="cuda")
+    caps = {"alg1": (200000, 16), "direct": (20, 20000), "pcg": (20, 100)}[method]
+    P, info = omni.solve_ex(g_dev[0], g_dev[1], None, m_dev, d, tol, caps[0], caps[1], method=method, P64_out=P64)
+    assert info["status"] == 0 and info["eps_R_final"] <= tol
+    e64, _, _ = oracle.eps_R_of_field(g_or[0], g_or[1], None, m, P64.cpu().numpy(), *d)
+    e32, _, _ = oracle.eps_R_of_field(g_or[0], g_or[1], None, m, P.cpu().numpy(), *d)
+    assert e64 == pytest.approx(info["eps_R_final"], rel=1e-6) and e64 <= 1.05 * tol
+    assert e32 > e64

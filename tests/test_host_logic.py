@@ -85,7 +85,7 @@ def test_binding_rejects_mismatched_tensors_before_the_call():
 
 @pytest.mark.parametrize("dims", [(4, 1, 2000), (1, 1, 500), (4, 4, 4000), (8, 1, 2000), (500, 500, 500), (1024, 1024, 1)])
 def test_workspace_holds_one_reduction_slot_per_tile_cta(dims):
-    """thin cross-sections with a long z axis launch far more tile CTAs (x tiles * y tiles * z segments, two
+    """thin cross-sections with a long z axis launch far more tile CTAs (x tiles * y tiles * z segments, four
     accumulators in K2) than npad / 256; the workspace must grow with that bound, whatever segment count the device
     picks (at most nz)."""
     nx, ny, nz = dims
@@ -93,5 +93,25 @@ def test_workspace_holds_one_reduction_slot_per_tile_cta(dims):
         px = (nx + pad - 1) // pad * pad
         npad = px * ny * nz
         vectors = 5 * npad * cell + 2 * npad * 8 + npad * 5          # S r p0 p1 delta, P P1, link + wcode
-        worst_ctas = 2 * ((px + 63) // 64) * ((ny + 7) // 8) * nz
+        worst_ctas = 4 * ((px + 63) // 64) * ((ny + 7) // 8) * nz
         assert omni.workspace_bytes(nx, ny, nz, dt) >= vectors + 8 * worst_ctas
+
+
+def test_solve_ex_rejects_bad_options_before_enqueueing():
+    """omni_solve_ex_*: unknown method, a struct_size that is not this library's, a history pointer without capacity."""
+    L = omni.lib()
+    o = omni.Options()
+    L.omni_options_init(C.byref(o))
+    assert o.struct_size == C.sizeof(omni.Options) and o.loop_mode == -1 and o.hist_capacity == 0
+
+    def call(method, opt):
+        return L.omni_solve_ex_f64(C.c_int(4), C.c_int(4), C.c_int(1), C.c_double(1), C.c_double(1), C.c_double(1), C.c_void_p(8),
+                                   C.c_void_p(8), C.c_void_p(0), None, None, C.c_void_p(8), C.c_double(1e-8), C.c_int(1), C.c_int(1),
+                                   C.c_int(method), C.byref(opt) if opt is not None else None, None, None)
+    assert call(7, o) == -1
+    bad = omni.Options(); L.omni_options_init(C.byref(bad)); bad.struct_size = 8
+    assert call(0, bad) == -1
+    bad = omni.Options(); L.omni_options_init(C.byref(bad)); bad.d_hist_eps_R = 256
+    assert call(0, bad) == -1
+    bad = omni.Options(); L.omni_options_init(C.byref(bad)); bad.loop_mode = 9
+    assert call(0, bad) == -1

@@ -1029,3 +1029,25 @@ def test_pcg_oracle_pieces():
     assert plans[0] == [False, True, True] and np.allclose(levels[1].w, [0.1 * 4 / 4, 0.2 * 4 / 4, 0.3 * 4])
     assert levels[1].v.shape == (5, 8, 12) and plans[1] == [False, True, True] and levels[2].v.shape == (5, 4, 6)
     assert len(levels) == 3
+
+
+def test_eps_P_history_eq40(oracle):
+    """oracle.solve_hist records eps_P^n = ||P^n - P^(n-1)|| / ||P^n|| (Eq. 40 :438) next to eps_R (Eq. 41).  Pinned with
+    fields from SEPARATE truncated solves (max_outer = n - 1 and n give P^(n-1) and P^n of the same deterministic
+    iteration), and by the paper's own remark that both metrics decay at the same rate with eps_R the larger (:447)."""
+    f = make_field("lamb_oseen2d", (40, 52), seed=3, noise=0.05)
+    g, m, d = f["g"], f["mask"], f["d"]
+    P, info, hR, hP = oracle.solve_hist(g[0], g[1], None, m, *d, tol=0.0, max_outer=12, max_cg=15, hist_cap=16)
+    assert hP[0] == 0.0 and np.all(np.isnan(hP[13:])) and not np.isnan(hP[:13]).any()
+    _, _, hR0 = oracle.solve(g[0], g[1], None, m, *d, tol=0.0, max_outer=12, max_cg=15, hist_cap=16)
+    assert np.array_equal(hR[:13], hR0[:13])
+    prev = np.zeros_like(P)
+    for n in (1, 2, 5, 12):
+        Pa, _ = oracle.solve(g[0], g[1], None, m, *d, tol=0.0, max_outer=n - 1, max_cg=15)
+        Pb, _ = oracle.solve(g[0], g[1], None, m, *d, tol=0.0, max_outer=n, max_cg=15)
+        a, b = np.nan_to_num(Pa), np.nan_to_num(Pb)
+        assert hP[n] == pytest.approx(np.linalg.norm(b - a) / np.linalg.norm(b), rel=1e-10)
+    late = slice(6, 13)
+    rate_P = hP[late][1:] / hP[late][:-1]
+    rate_R = hR[late][1:] / hR[late][:-1]
+    assert np.allclose(rate_P, rate_R, rtol=0.15)
