@@ -223,6 +223,41 @@ int omni_solve_batch2d_f32(int nx, int ny, int nb, double dx, double dy, const f
                            const unsigned char* d_mask2d, const float* d_P_init, float* d_P_out, double tol,
                            int max_outer, int max_cg, void* stream, omni_info* info);
 
+/* ---- one solve on several ranks: z-slab sharding -------------------------------------
+ * The paper stops at one 16 GB GPU and names memory as the limit.  Here the grid is cut along z:
+ * rank s of nranks owns the planes [z0, z1) and works on the WINDOW [zlo, zhi) = its planes plus up to two halo planes
+ * per side (the stencil codes of Eq. 25 :266 read validity two planes away); omni_slab_plan (host only) returns both
+ * ranges: balanced, the first nz % nranks ranks own one plane more.  Per CG iteration each rank exchanges one halo
+ * plane of p and one of r with each neighbour and two scalars are all-reduced; per outer iteration the halo planes of
+ * delta, P and r and the four scalars of the boundary update.  Same kernels, same iteration, same stopping rules as
+ * omni_solve_* (method OMNI_METHOD_ALG1) / omni_solve_direct_* (OMNI_METHOD_DIRECT); the reductions add per-rank
+ * totals, so results equal the single-device ones to rounding and all ranks take identical decisions.
+ *
+ * omni_solve_slab_*: nlocal ranks of the solve live in THIS process on the current device; h_ranks[nlocal] are their
+ * rank numbers; h_gx / h_gy / h_gz / h_mask / h_P_out are HOST arrays of nlocal DEVICE pointers to each rank's window
+ * ([zhi - zlo][ny][nx], x fastest; h_mask may be NULL, or hold NULL entries = all valid).  P_out is written on the whole
+ * window; the owned planes are the result (halo planes hold the neighbours' values of an earlier iteration).
+ *   comm == NULL : all ranks are local (nlocal == nranks, h_ranks = 0..nranks-1): halo planes by device copies, the
+ *                  scalars by a summing kernel -- the sharded algorithm on one GPU (tests, grids split for other reasons)
+ *   comm != NULL : one rank per process (nlocal == 1), `comm` from omni_slab_comm_create: NCCL send / recv of the halo
+ *                  planes and ncclAllReduce of the scalars over NVLink.  libnccl.so.2 is loaded at run time; without it
+ *                  these calls return OMNI_ERR_CUDA.  omni_slab_unique_id (on rank 0) makes the 128-byte id every rank
+ *                  passes to omni_slab_comm_create (ship it with any host-side broadcast).
+ * nz >= nranks, nz >= 2 (3D only).  The loop is driven from the host (one synchronisation per outer iteration and per
+ * 16 CG iterations), so the call always synchronises; info may be NULL.  Status codes as omni_solve_*. */
+int omni_slab_plan(int nz, int nranks, int rank, int* z0, int* z1, int* zlo, int* zhi);
+int omni_slab_unique_id(char* h_id128);
+int omni_slab_comm_create(int rank, int nranks, const char* h_id128, void** comm);
+void omni_slab_comm_destroy(void* comm);
+int omni_solve_slab_f64(int nx, int ny, int nz, double dx, double dy, double dz, int nlocal, const int* h_ranks,
+                        const double* const* h_gx, const double* const* h_gy, const double* const* h_gz,
+                        const unsigned char* const* h_mask, double* const* h_P_out, double tol, int max_outer, int max_cg,
+                        int method, int nranks, void* comm, void* stream, omni_info* info);
+int omni_solve_slab_f32(int nx, int ny, int nz, double dx, double dy, double dz, int nlocal, const int* h_ranks,
+                        const float* const* h_gx, const float* const* h_gy, const float* const* h_gz,
+                        const unsigned char* const* h_mask, float* const* h_P_out, double tol, int max_outer, int max_cg,
+                        int method, int nranks, void* comm, void* stream, omni_info* info);
+
 /* ---- upstream of the path: the pressure gradient from a velocity field, Eq. 1 ----
  *   g = f(u) = -rho (du/dt + (u . grad) u) + mu lap u
  * with second-order central differences on the cell grid.  The paper does not fix the discretisation (reading R-V1,
@@ -341,7 +376,7 @@ void omni_release_memory(void);
 int omni_profile_enable(int on);          /* returns the previous setting */
 void omni_profile_read(double* h_ms3, long long* h_count3, int reset);
 const char* omni_status_string(int status);
-int omni_version(void);                  /* 100 * major + minor; 101 added the _guess, _rans_source and history entry points, 102 omni_solve_pcg_*, 103 omni_solve_ex_* / omni_options */
+int omni_version(void);                  /* 100 * major + minor; 101 added the _guess, _rans_source and history entry points, 102 omni_solve_pcg_*, 103 omni_solve_ex_* / omni_options, 104 omni_solve_slab_* */
 
 #ifdef __cplusplus
 }

@@ -115,7 +115,8 @@ static double far_face_constant(double da, double db, double dc)
  * z index is then 0, so all weights across planes vanish (Eq. 16/18 with c_xz = c_yz = c_zz = 0, F_z = 0) and no other
  * routine needs to know.  The flag is set only inside oracle_solve_batch2d (test infrastructure: not thread safe). */
 static int g_batch2d = 0;
-/* set by oracle_solve_direct around solve_impl: the inner systems are L P = S instead of Eq. 12 */
+/* set by oracle_solve_direct around solve_impl: the inner systems are L P = S instead of Eq. 12;
+ * 2: with the single-reduction recurrences of cg1_op */
 static int g_direct = 0;
 
 void oracle_constants(int nx, int ny, int nz, double dx, double dy, double dz, double *out)
@@ -366,6 +367,40 @@ static int cg_op(int direct, int nx, int ny, int nz, const unsigned char *v, con
     return k;
 }
 
+/* Single-reduction CG (Chronopoulos & Gear 1989; SURVEY 8(d) V5, 8(f) NEXT-2 i) for the SYMMETRIC system L x = rhs:
+ * the same iterates as cg_op in exact arithmetic, but both inner products of an iteration (r.r and (A r).r) are taken
+ * at the same point, so a parallel implementation synchronises once per iteration instead of twice.  s tracks A p by
+ * the recurrence s = A r + beta s; p.Ap is never formed: alpha = gamma / (delta - beta gamma / alpha_prev), which relies
+ * on A = A^T (it is NOT valid for the paper's nonsymmetric M).  Same stopping rule.  Work arrays r, p, q (= s), tmp, w. */
+static int cg1_op(int nx, int ny, int nz, const unsigned char *v, const double *w1, const double *w0,
+                  const double *w0C, const double *rhs, double *x, double thresh, int max_cg, double *r, double *p,
+                  double *s, double *tmp, double *w)
+{
+    i64 N = (i64)nx * ny * nz;
+    apply_op(1, nx, ny, nz, v, w1, w0, w0C, x, w, tmp);
+#pragma omp parallel for if (N > OMP_MIN_N)
+    for (i64 c = 0; c < N; ++c) { r[c] = rhs[c] - w[c]; p[c] = 0.0; s[c] = 0.0; }
+    apply_op(1, nx, ny, nz, v, w1, w0, w0C, r, w, tmp);
+    double gamma = dot(N, nx, r, r), delta = dot(N, nx, w, r), beta = 0.0, alpha = gamma / delta;
+    int k = 0;
+    while (sqrt(gamma) > thresh && gamma != 0.0 && k < max_cg) {
+#pragma omp parallel for if (N > OMP_MIN_N)
+        for (i64 c = 0; c < N; ++c) {
+            p[c] = r[c] + beta * p[c];
+            s[c] = w[c] + beta * s[c];
+            x[c] += alpha * p[c];
+            r[c] -= alpha * s[c];
+        }
+        apply_op(1, nx, ny, nz, v, w1, w0, w0C, r, w, tmp);
+        double gamma1 = dot(N, nx, r, r), delta1 = dot(N, nx, w, r);      /* the iteration's single reduction point */
+        beta = gamma1 / gamma;
+        alpha = gamma1 / (delta1 - beta * gamma1 / alpha);
+        gamma = gamma1;
+        ++k;
+    }
+    return k;
+}
+
 int oracle_cg(int nx, int ny, int nz, const unsigned char *v, const double *w1, const double *rhs, double *x,
               double thresh, int max_cg, double *r, double *p, double *q)
 {
@@ -433,6 +468,18 @@ int oracle_solve_direct(int nx, int ny, int nz, double dx, double dy, double dz,
     return rc;
 }
 
+/* oracle_solve_direct with the single-reduction CG recurrences (cg1_op) in the inner solves: same system, same outer
+ * loop and stopping rules; a different (in exact arithmetic identical) iteration. */
+int oracle_solve_direct_cg1(int nx, int ny, int nz, double dx, double dy, double dz,
+                            const double *gx, const double *gy, const double *gz, const unsigned char *mask,
+                            const double *P_init, double *P_out, double tol, int max_outer, int max_cg, oracle_info *info)
+{
+    g_direct = 2;
+    int rc = solve_impl(nx, ny, nz, dx, dy, dz, gx, gy, gz, mask, P_init, P_out, tol, max_outer, max_cg, info, NULL, 0, NULL);
+    g_direct = 0;
+    return rc;
+}
+
 /* nb snapshots [nb][ny][nx] on one mask [ny][nx] (NULL = all valid), optional first guess P_init [nb][ny][nx]
  * ("initialized to zero ... or any other arbitrary value"; NULL = 0).  eps_R and the CG scalars are those
  * of the stacked system. */
@@ -477,8 +524,9 @@ static int solve_impl(int nx, int ny, int nz, double dx, double dy, double dz,
     double *rhs = (double *)malloc(nb), *r = (double *)malloc(nb), *p = (double *)malloc(nb), *q = (double *)malloc(nb);
     double *tmp = (double *)malloc(nb);
     double *Pold = hist_P ? (double *)malloc(nb) : NULL;
+    double *wv = (g_direct == 2) ? (double *)malloc(nb) : NULL;
     int rc = -1;
-    if (!v || !w1 || !w0 || !w0C || !S || !P || !rhs || !r || !p || !q || !tmp || (hist_P && !Pold)) goto done;
+    if (!v || !w1 || !w0 || !w0C || !S || !P || !rhs || !r || !p || !q || !tmp || (hist_P && !Pold) || (g_direct == 2 && !wv)) goto done;
     rc = 0;
 
     oracle_validity(nx, ny, nz, gx, gy, gz, mask, v);
@@ -515,7 +563,8 @@ static int solve_impl(int nx, int ny, int nz, double dx, double dy, double dz,
              * Fixed-point variant (oracle_solve_direct): the same loop with the system L P = S; eps_R above is its
              * residual too (r0 = S - L P^n), so the outer loop only restarts a CG that hit max_cg. */
             if (g_direct) memcpy(rhs, S, nb);
-            cg_total += cg_op(g_direct, nx, ny, nz, v, w1, w0, w0C, rhs, P, 0.1 * tol * normS, max_cg, r, p, q, tmp);
+            if (g_direct == 2) cg_total += cg1_op(nx, ny, nz, v, w1, w0, w0C, rhs, P, 0.1 * tol * normS, max_cg, r, p, q, tmp, wv);
+            else cg_total += cg_op(g_direct, nx, ny, nz, v, w1, w0, w0C, rhs, P, 0.1 * tol * normS, max_cg, r, p, q, tmp);
             ++n;
         }
     }
@@ -525,7 +574,7 @@ static int solve_impl(int nx, int ny, int nz, double dx, double dy, double dz,
         info->norm_S = normS; info->converged = (epsR <= tol);
     }
 done:
-    free(v); free(w1); free(w0); free(w0C); free(S); free(P); free(rhs); free(r); free(p); free(q); free(tmp); free(Pold);
+    free(v); free(w1); free(w0); free(w0C); free(S); free(P); free(rhs); free(r); free(p); free(q); free(tmp); free(Pold); free(wv);
     return rc;
 }
 

@@ -203,8 +203,9 @@ def solve_guess(gx, gy, gz, mask, dx, dy, dz, tol, max_outer, max_cg, P_init):
                "norm_S": info.norm_S, "converged": bool(info.converged)}
 
 
-def solve_direct(gx, gy, gz, mask, dx, dy, dz, tol, max_outer, max_cg, P_init=None):
-    """Fixed point of Algorithm 1 by CG on L P = S (oracle_solve_direct; not the paper's iteration).  Returns (P, info)."""
+def solve_direct(gx, gy, gz, mask, dx, dy, dz, tol, max_outer, max_cg, P_init=None, single_reduction=False):
+    """Fixed point of Algorithm 1 by CG on L P = S (oracle_solve_direct; not the paper's iteration).  Returns (P, info).
+    single_reduction: the Chronopoulos-Gear recurrences (oracle_solve_direct_cg1) instead of the textbook ones."""
     gx, gy = _f64(gx), _f64(gy)
     nx, ny, nz = _dims(gx.shape)
     gz = _f64(gz) if gz is not None else None
@@ -214,7 +215,7 @@ def solve_direct(gx, gy, gz, mask, dx, dy, dz, tol, max_outer, max_cg, P_init=No
     P = np.zeros(gx.shape)
     info = Info()
     P0 = None if P_init is None else _f64(P_init)
-    f = lib().oracle_solve_direct
+    f = lib().oracle_solve_direct_cg1 if single_reduction else lib().oracle_solve_direct
     f.restype = C.c_int
     rc = f(C.c_int(nx), C.c_int(ny), C.c_int(nz), C.c_double(dx), C.c_double(dy), C.c_double(dz),
            _p(gx), _p(gy), _p(gz if gz is not None else gx), _p(m), _p(P0), _p(P), C.c_double(tol), C.c_int(max_outer),

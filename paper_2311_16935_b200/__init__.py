@@ -5,7 +5,8 @@ Importing the package does not load the library; the first call does, and fails 
 """
 from .binding import (Info, OmniError, SYMBOLS, apply_M, constants, launch_count, lib, profile_enable,  # noqa: F401
                       profile_read, release_memory, residual, set_loop_mode, solve, solve_batch2d, solve_cascade, solve_direct, source, status_string, velocity_source, version, workspace_bytes,
-                      rans_source, compressible_rans_source, solve_guess, set_history, solve_pcg, solve_ex, Options)
+                      rans_source, compressible_rans_source, solve_guess, set_history, solve_pcg, solve_ex, Options, slab_plan, solve_slab, solve_slab_rank, slab_comm_create,
+                      slab_comm_destroy)
 
 # the C names, for callers who think in terms of include/omni.h
 omni_solve = solve
@@ -15,6 +16,8 @@ omni_solve_guess = solve_guess
 omni_solve_cascade = solve_cascade
 omni_solve_pcg = solve_pcg
 omni_solve_ex = solve_ex
+omni_solve_slab = solve_slab
+omni_slab_plan = slab_plan
 omni_source = source
 omni_velocity_source = velocity_source
 omni_rans_source = rans_source

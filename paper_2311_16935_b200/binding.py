@@ -17,7 +17,8 @@ STATUS_NAMES = {0: "OMNI_OK", 1: "OMNI_NOT_CONVERGED", -1: "OMNI_ERR_INVALID_ARG
                 -3: "OMNI_ERR_ALLOC", -4: "OMNI_ERR_BREAKDOWN"}
 # every symbol include/omni.h declares
 SYMBOLS = ["omni_solve_f64", "omni_solve_f32", "omni_workspace_bytes", "omni_solve_f64_ws", "omni_solve_f32_ws",
-           "omni_solve_host_f64", "omni_solve_host_f32", "omni_solve_batch2d_f64", "omni_solve_batch2d_f32", "omni_solve_guess_f64", "omni_solve_guess_f32", "omni_solve_direct_f64", "omni_solve_direct_f32", "omni_solve_pcg_f64", "omni_solve_pcg_f32", "omni_solve_ex_f64", "omni_solve_ex_f32", "omni_options_init", "omni_solve_direct_batch2d_f64", "omni_solve_direct_batch2d_f32", "omni_solve_cascade_f64", "omni_solve_cascade_f32", "omni_velocity_source_f64", "omni_velocity_source_f32", "omni_rans_source_f64", "omni_rans_source_f32",
+           "omni_solve_host_f64", "omni_solve_host_f32", "omni_solve_batch2d_f64", "omni_solve_batch2d_f32", "omni_solve_guess_f64", "omni_solve_guess_f32", "omni_solve_direct_f64", "omni_solve_direct_f32", "omni_solve_pcg_f64", "omni_solve_pcg_f32", "omni_solve_ex_f64", "omni_solve_ex_f32", "omni_options_init", "omni_slab_plan", "omni_slab_unique_id", "omni_slab_comm_create", "omni_slab_comm_destroy",
+           "omni_solve_slab_f64", "omni_solve_slab_f32", "omni_solve_direct_batch2d_f64", "omni_solve_direct_batch2d_f32", "omni_solve_cascade_f64", "omni_solve_cascade_f32", "omni_velocity_source_f64", "omni_velocity_source_f32", "omni_rans_source_f64", "omni_rans_source_f32",
            "omni_compressible_rans_source_f64", "omni_compressible_rans_source_f32", "omni_constants", "omni_source_f64", "omni_source_f32",
            "omni_apply_M_f64", "omni_apply_M_f32", "omni_residual_f64", "omni_residual_f32", "omni_launch_count",
            "omni_set_loop_mode", "omni_set_history", "omni_release_memory", "omni_profile_enable", "omni_profile_read", "omni_status_string", "omni_version"]
@@ -292,6 +293,91 @@ def solve_ex(gx, gy, gz, mask, d, tol, max_outer, max_cg, method="alg1", P_init=
     if rc < 0:
         raise OmniError(rc, f"omni_solve_ex_{sfx}")
     return P, (info.as_dict() if want_info else None)
+
+
+def slab_plan(nz, nranks, rank):
+    """omni_slab_plan: (z0, z1, zlo, zhi) -- owned planes [z0, z1) and window [zlo, zhi) of `rank` (host only)."""
+    v = [C.c_int(0) for _ in range(4)]
+    rc = lib().omni_slab_plan(C.c_int(nz), C.c_int(nranks), C.c_int(rank), *[C.byref(x) for x in v])
+    if rc != 0:
+        raise OmniError(rc, "omni_slab_plan")
+    return tuple(x.value for x in v)
+
+
+def _slab_call(sfx, nx, ny, nz, d, ranks, wins, tol, max_outer, max_cg, method, nranks, comm, dev):
+    """wins: per local rank (gx, gy, gz, mask or None, P_out) window tensors.  Marshals the pointer arrays."""
+    n = len(ranks)
+    arr = lambda i: (C.c_void_p * n)(*[None if w[i] is None else w[i].data_ptr() for w in wins])
+    masks = arr(3) if any(w[3] is not None for w in wins) else None
+    info = Info()
+    fn = getattr(lib(), f"omni_solve_slab_{sfx}")
+    rc = fn(C.c_int(nx), C.c_int(ny), C.c_int(nz), C.c_double(float(d[0])), C.c_double(float(d[1])), C.c_double(float(d[2])),
+            C.c_int(n), (C.c_int * n)(*ranks), arr(0), arr(1), arr(2), masks, arr(4), C.c_double(tol), C.c_int(max_outer),
+            C.c_int(max_cg), C.c_int(METHODS[method]), C.c_int(nranks), C.c_void_p(comm), _stream(dev), C.byref(info))
+    if rc < 0:
+        raise OmniError(rc, f"omni_solve_slab_{sfx}")
+    return info.as_dict()
+
+
+def solve_slab(gx, gy, gz, mask, d, tol, max_outer, max_cg, nslabs, method="alg1"):
+    """omni_solve_slab_* with all `nslabs` ranks on this device (comm = NULL): the global CUDA tensors are cut into the
+    ranks' windows, solved as z-slabs with halo exchange, and the owned planes are put together again.  Returns (P, info)."""
+    import torch
+    sfx = _suffix(gx)
+    _check([gx, gy, gz, mask], "cuda")
+    _check_like(gx, [("gy", gy), ("gz", gz)], mask)
+    if gx.dim() != 3:
+        raise ValueError("z-slab sharding needs a 3D grid")
+    nz, ny, nx = gx.shape
+    plans = [slab_plan(nz, nslabs, r) for r in range(nslabs)]
+    wins = []
+    for (z0, z1, zlo, zhi) in plans:
+        wins.append((gx[zlo:zhi].contiguous(), gy[zlo:zhi].contiguous(), gz[zlo:zhi].contiguous(),
+                     None if mask is None else mask[zlo:zhi].contiguous(), torch.empty((zhi - zlo, ny, nx), dtype=gx.dtype, device=gx.device)))
+    with torch.cuda.device(gx.device):
+        info = _slab_call(sfx, nx, ny, nz, d, list(range(nslabs)), wins, tol, max_outer, max_cg, method, nslabs, None, gx.device)
+    P = torch.empty_like(gx)
+    for (z0, z1, zlo, zhi), w in zip(plans, wins):
+        P[z0:z1] = w[4][z0 - zlo:z1 - zlo]
+    return P, info
+
+
+def slab_comm_create(rank, nranks, broadcast):
+    """One NCCL communicator for omni_solve_slab_* with one rank per process.  `broadcast(bytes_or_None) -> bytes`
+    ships rank 0's 128-byte id to every rank (e.g. through torch.distributed.broadcast_object_list)."""
+    buf = C.create_string_buffer(128)
+    if rank == 0:
+        rc = lib().omni_slab_unique_id(buf)
+        if rc != 0:
+            raise OmniError(rc, "omni_slab_unique_id")
+    raw = broadcast(buf.raw if rank == 0 else None)
+    comm = C.c_void_p(0)
+    rc = lib().omni_slab_comm_create(C.c_int(rank), C.c_int(nranks), C.create_string_buffer(raw, 128), C.byref(comm))
+    if rc != 0:
+        raise OmniError(rc, "omni_slab_comm_create")
+    return comm.value
+
+
+def slab_comm_destroy(comm):
+    lib().omni_slab_comm_destroy(C.c_void_p(comm))
+
+
+def solve_slab_rank(gx_win, gy_win, gz_win, mask_win, d, nz, rank, nranks, comm, tol, max_outer, max_cg, method="alg1"):
+    """This process's rank of a sharded solve: *_win are the CUDA tensors of its window [zlo, zhi) (slab_plan); `comm` from
+    slab_comm_create.  Returns (P on the owned planes, info)."""
+    import torch
+    sfx = _suffix(gx_win)
+    _check([gx_win, gy_win, gz_win, mask_win], "cuda")
+    _check_like(gx_win, [("gy", gy_win), ("gz", gz_win)], mask_win)
+    z0, z1, zlo, zhi = slab_plan(nz, nranks, rank)
+    if gx_win.shape[0] != zhi - zlo:
+        raise ValueError(f"rank {rank} of {nranks}: the window holds planes [{zlo}, {zhi})")
+    _, ny, nx = gx_win.shape
+    out = torch.empty_like(gx_win)
+    with torch.cuda.device(gx_win.device):
+        info = _slab_call(sfx, nx, ny, nz, d, [rank], [(gx_win, gy_win, gz_win, mask_win, out)], tol, max_outer, max_cg, method,
+                          nranks, comm, gx_win.device)
+    return out[z0 - zlo:z1 - zlo], info
 
 
 def velocity_source(u, v, w, mask, d, rho=1.0, mu=0.0, dudt=None):

@@ -5,6 +5,7 @@
 #include "omni_persist.cuh"
 #include "omni_loop.cuh"
 #include "omni_mg.cuh"
+#include "omni_slab.cuh"
 #include "../../include/omni.h"
 
 #include <algorithm>
@@ -299,6 +300,7 @@ bool make_geom(int nx, int ny, int nz, int elem_size, Geom& g, int batch = 0)
     const long long npad = px * (long long)ny * (long long)nz;
     if (npad > (1LL << 40) || px > 0x7fffffff) return false;
     g.nx = nx; g.ny = ny; g.nz = nz; g.px = (int)px;
+    g.kz0 = 0; g.kz1 = nz;
     g.pplane = px * ny;
     g.npad = npad;
     const int naxes = (nz > 1 && !batch) ? 3 : 2;
@@ -365,7 +367,8 @@ size_t carve(const Geom& g, char* base, Workspace<T>* w)
 }
 
 __global__ void init_scalars_kernel(Scalars* sc, double tol, int max_outer, int max_cg, double* hist = nullptr, int hist_cap = 0,
-                                    int* hist_k = nullptr, double inner_rel = 0.0, double* hist_p = nullptr, int* status_out = nullptr)
+                                    int* hist_k = nullptr, double inner_rel = 0.0, double* hist_p = nullptr, int* status_out = nullptr,
+                                    int defer = 0)
 {
     Scalars s;
     memset(&s, 0, sizeof(s));
@@ -373,6 +376,7 @@ __global__ void init_scalars_kernel(Scalars* sc, double tol, int max_outer, int 
     s.inner_rel2 = inner_rel * inner_rel;
     s.hist = hist; s.hist_k = hist_k; s.hist_p = hist_p; s.hist_cap = hist_cap; s.hist_n = 0;
     s.status_out = status_out;
+    s.defer = defer;
     s.inner_go = 0; s.outer_go = 1; s.status = ST_OK;
     s.dzero = 1;                     // no CG iteration has run yet: the first K2 takes delta as zero
     s.bar_count = 2;                 // grid barrier of the loop kernel: set 0, tag 1 against zeroed slots (omni_persist.cuh)
@@ -417,13 +421,14 @@ MarchCfg tma_config(const Geom& g)
             if (cached) slots_cache[di.dev] = slots;
         }
     }
+    const int nzr = g.kz1 - g.kz0;                 // planes to emit (a slab: the planes it owns)
     const int ntx = (g.px + TG::BX - 1) / TG::BX, nty = (g.ny + TG::BY - 1) / TG::BY;
     const long long tiles = (long long)ntx * nty;
     int best = 1;
     double best_cost = 1e300;
-    for (int ns = 1; ns <= g.nz; ns = (ns < 16 ? ns + 1 : ns + ns / 8)) {
-        const int zlen = (g.nz + ns - 1) / ns;
-        const int nseg = (g.nz + zlen - 1) / zlen;
+    for (int ns = 1; ns <= nzr; ns = (ns < 16 ? ns + 1 : ns + ns / 8)) {
+        const int zlen = (nzr + ns - 1) / ns;
+        const int nseg = (nzr + zlen - 1) / zlen;
         const long long ctas = tiles * nseg;
         const long long waves = (ctas + slots - 1) / slots;
         // CTAs next to masked cells run the slower general loop: with fewer than three waves a few of them become
@@ -433,12 +438,12 @@ MarchCfg tma_config(const Geom& g)
         if (zlen <= 4) break;
     }
 #ifdef OMNI_TUNING   // tuning builds only: force the number of z segments from the environment
-    if (const char* ev = getenv("OMNI_NSEG")) { const int v = atoi(ev); if (v >= 1) best = v < g.nz ? v : g.nz; }
+    if (const char* ev = getenv("OMNI_NSEG")) { const int v = atoi(ev); if (v >= 1) best = v < nzr ? v : nzr; }
 #endif
     MarchCfg c;
     c.zs.n = 0;
-    c.zs.zlen = (g.nz + best - 1) / best;
-    int nseg = (g.nz + c.zs.zlen - 1) / c.zs.zlen;
+    c.zs.zlen = (nzr + best - 1) / best;
+    int nseg = (nzr + c.zs.zlen - 1) / c.zs.zlen;
     // Tapered z segments: CTAs are dispatched in blockIdx order, z slowest, so the segments of
     // later z indices start later.  Long segments first (few halo planes, few pipeline fills), short ones last: the
     // launch then drains in the time of a short CTA instead of about half a long one.  Each segment takes the
@@ -449,15 +454,15 @@ MarchCfg tma_config(const Geom& g)
     if (const char* ev = getenv("OMNI_TAPER_F")) taper_f = atof(ev);
     if (const char* ev = getenv("OMNI_TAPER_MIN")) taper_min = atoi(ev) > 1 ? atoi(ev) : 1;
 #endif
-    if (taper_f > 0.0 && (double)tiles * g.nz / slots >= 2.0 * taper_min) {
+    if (taper_f > 0.0 && (double)tiles * nzr / slots >= 2.0 * taper_min) {
         int k = 0, n = 0;
         bool ok = true;
         c.zs.k[0] = 0;
-        while (k < g.nz) {
-            const double rem = (double)(g.nz - k) * (double)tiles / slots;     // planes left per CTA slot
+        while (k < nzr) {
+            const double rem = (double)(nzr - k) * (double)tiles / slots;     // planes left per CTA slot
             int len = (int)(rem * taper_f + 0.5);
             if (len < taper_min) len = taper_min;
-            if (g.nz - k - len < (taper_min + 1) / 2) len = g.nz - k;
+            if (nzr - k - len < (taper_min + 1) / 2) len = nzr - k;
             if (n == ZSeg::MAXSEG) { ok = false; break; }
             k += len;
             c.zs.k[++n] = k;
@@ -1276,6 +1281,200 @@ int rans_source(bool compressible, int nx, int ny, int nz, double dx, double dy,
     return OMNI_OK;
 }
 
+// ------------------------------------------------------------------------------------------------ z-slab sharding (omni_slab.cuh)
+template <typename T>
+struct SlabRank {
+    int rank, z0, z1, zlo, zhi;
+    Geom g; Workspace<T> w; void* ws; TmaSet maps;
+    const T *gx, *gy, *gz; const uint8_t* mask; T* P_out;
+};
+
+// Halo exchange of one array: every rank's planes just outside its owned range receive the neighbour's outermost owned
+// plane.  comm == nullptr: all ranks are local (plane copies on the stream); else one local rank and NCCL.
+template <typename T, typename U, typename F>
+int slab_exchange(std::vector<SlabRank<T>>& R, int nranks, void* comm, F&& base, cudaStream_t st)
+{
+    if (!comm) {
+        for (int s = 0; s + 1 < (int)R.size(); ++s) {
+            SlabRank<T>&lo = R[s], &hi = R[s + 1];
+            U* a = base(lo); U* b = base(hi);
+            const size_t bytes = (size_t)lo.g.pplane * sizeof(U);
+            // lo's first plane above its range <- hi's first owned plane; hi's last plane below its range <- lo's last owned one
+            CK(cudaMemcpyAsync(a + (size_t)lo.g.kz1 * lo.g.pplane, b + (size_t)hi.g.kz0 * hi.g.pplane, bytes, cudaMemcpyDeviceToDevice, st));
+            CK(cudaMemcpyAsync(b + (size_t)(hi.g.kz0 - 1) * hi.g.pplane, a + (size_t)(lo.g.kz1 - 1) * lo.g.pplane, bytes, cudaMemcpyDeviceToDevice, st));
+        }
+        return OMNI_OK;
+    }
+    const NcclApi& N = nccl_api();
+    SlabRank<T>& r = R[0];
+    U* a = base(r);
+    const size_t bytes = (size_t)r.g.pplane * sizeof(U);
+    if (N.GroupStart() != 0) return OMNI_ERR_CUDA;
+    int bad = 0;
+    if (r.rank > 0) {
+        bad |= N.Send(a + (size_t)r.g.kz0 * r.g.pplane, bytes, NcclApi::Int8, r.rank - 1, comm, st);
+        bad |= N.Recv(a + (size_t)(r.g.kz0 - 1) * r.g.pplane, bytes, NcclApi::Int8, r.rank - 1, comm, st);
+    }
+    if (r.rank + 1 < nranks) {
+        bad |= N.Send(a + (size_t)(r.g.kz1 - 1) * r.g.pplane, bytes, NcclApi::Int8, r.rank + 1, comm, st);
+        bad |= N.Recv(a + (size_t)r.g.kz1 * r.g.pplane, bytes, NcclApi::Int8, r.rank + 1, comm, st);
+    }
+    bad |= N.GroupEnd();
+    return bad ? OMNI_ERR_CUDA : OMNI_OK;
+}
+
+// sum of Scalars::red_out[0..n) over all ranks, left in every rank's red_out
+template <typename T>
+int slab_allreduce(std::vector<SlabRank<T>>& R, void* comm, Scalars* const* d_scs, int n, cudaStream_t st)
+{
+    if (!comm) {
+        if (R.size() > 1) {
+            slab_sum_kernel<<<1, 32, 0, st>>>(d_scs, (int)R.size(), n);
+            g_launches.fetch_add(1, std::memory_order_relaxed);
+            CK(cudaGetLastError());
+        }
+        return OMNI_OK;
+    }
+    double* p = R[0].w.sc->red_out;            // device address of the member
+    return nccl_api().AllReduce(p, p, (size_t)n, NcclApi::Float64, NcclApi::Sum, comm, st) == 0 ? OMNI_OK : OMNI_ERR_CUDA;
+}
+
+// Alg. 1 (lop = 0) or CG on L P = S (lop = 1) on z-slabs; host-driven loop (one synchronisation per outer iteration and
+// per 16 CG iterations, like loop mode 1).  Local windows: d_g*, d_mask, d_P_out hold the planes [zlo, zhi) of each
+// local rank (omni_slab_plan); P_out is written on the whole window, the owned planes are the result.
+template <typename T>
+int solve_slab(int nx, int ny, int nz, double dx, double dy, double dz, int nlocal, const int* ranks, const T* const* gx,
+               const T* const* gy, const T* const* gz, const unsigned char* const* mask, T* const* P_out, double tol,
+               int max_outer, int max_cg, int lop, int nranks, void* comm, void* stream, omni_info* info)
+{
+    if (!valid_common(nx, ny, nz, dx, dy, dz, tol, max_outer, max_cg) || nz < 2 || nranks < 1 || nlocal < 1 || !ranks || !gx || !gy ||
+        !gz || !P_out)
+        return OMNI_ERR_INVALID_ARG;
+    if (comm ? (nlocal != 1 || !nccl_api().ok) : (nlocal != nranks)) return OMNI_ERR_INVALID_ARG;
+    cudaStream_t st = (cudaStream_t)stream;
+    std::vector<SlabRank<T>> R((size_t)nlocal);
+    HostConst H;
+    host_constants(3, dx, dy, dz, H);
+    int rc = OMNI_OK;
+    Scalars** d_scs = nullptr;
+    auto cleanup = [&]() {
+        for (auto& r : R)
+            if (r.ws) cudaFreeAsync(r.ws, st);
+        if (d_scs) cudaFreeAsync(d_scs, st);
+    };
+    for (auto& r : R) r.ws = nullptr;
+    for (int i = 0; i < nlocal && rc == OMNI_OK; ++i) {
+        SlabRank<T>& r = R[(size_t)i];
+        r.rank = ranks[i];
+        if ((!comm && r.rank != i) || !slab_plan(nz, nranks, r.rank, r.z0, r.z1, r.zlo, r.zhi) || !gx[i] || !gy[i] || !gz[i] || !P_out[i] ||
+            !make_geom(nx, ny, r.zhi - r.zlo, (int)sizeof(T), r.g)) { rc = OMNI_ERR_INVALID_ARG; break; }
+        r.g.kz0 = r.z0 - r.zlo; r.g.kz1 = r.z1 - r.zlo;
+        r.gx = gx[i]; r.gy = gy[i]; r.gz = gz[i]; r.mask = mask ? mask[i] : nullptr; r.P_out = P_out[i];
+        const size_t bytes = carve<T>(r.g, nullptr, nullptr);
+        if (pool_alloc(&r.ws, bytes, st) != cudaSuccess) { cudaGetLastError(); r.ws = nullptr; rc = OMNI_ERR_ALLOC; break; }
+        carve<T>(r.g, (char*)r.ws, &r.w);
+    }
+    if (rc != OMNI_OK) { cleanup(); return rc; }
+    std::vector<Scalars*> h_scs;
+    for (auto& r : R) h_scs.push_back(r.w.sc);
+    if (pool_alloc((void**)&d_scs, sizeof(Scalars*) * R.size(), st) != cudaSuccess) { cudaGetLastError(); d_scs = nullptr; cleanup(); return OMNI_ERR_ALLOC; }
+    cudaMemcpyAsync(d_scs, h_scs.data(), sizeof(Scalars*) * R.size(), cudaMemcpyHostToDevice, st);
+    cudaStreamSynchronize(st);            // h_scs is a host temporary
+
+    CondHandles ch{ 0, 0, 0 };
+    auto each = [&](auto&& fn) { for (auto& r : R) { if (rc == OMNI_OK) { const int e = fn(r); if (e != OMNI_OK) rc = e; } } };
+    // setup per rank: scalars (deferred finalize), validity / codes / source on the window, tensor maps
+    each([&](SlabRank<T>& r) {
+        const Coef<T> K = make_coef<T>(H, dx, dy, dz, r.g);
+        init_scalars_kernel<<<1, 1, 0, st>>>(r.w.sc, tol, max_outer, max_cg, nullptr, 0, nullptr, 0.0, nullptr, nullptr, 1);
+        g_launches.fetch_add(1, std::memory_order_relaxed);
+        int e = setup_codes<T>(r.g, r.w, r.gx, r.gy, r.gz, r.mask, st);
+        if (e == OMNI_OK) e = launch_source<T>(r.g, r.w, K, r.gx, r.gy, r.gz, st);
+        if (e == OMNI_OK && !make_tma_set<T>(r.g, r.w, r.maps)) e = OMNI_ERR_CUDA;
+        return e;
+    });
+    if (rc == OMNI_OK) rc = slab_allreduce<T>(R, comm, d_scs, 1, st);
+    each([&](SlabRank<T>& r) { source_finalize_kernel<<<1, 1, 0, st>>>(r.w.sc); g_launches.fetch_add(1, std::memory_order_relaxed); return OMNI_OK; });
+
+    auto launch_fin = [&](auto op_tag, SlabRank<T>& r, const auto& args) {
+        using Op = typename decltype(op_tag)::type;
+        op_finalize_kernel<Op><<<1, 1, 0, st>>>(args);
+        g_launches.fetch_add(1, std::memory_order_relaxed);
+        return cudaGetLastError() == cudaSuccess ? OMNI_OK : OMNI_ERR_CUDA;
+    };
+    Scalars h;
+    memset(&h, 0, sizeof(h));
+    h.outer_go = 1;
+    auto read_scalars = [&]() {
+        if (cudaMemcpyAsync(&h, R[0].w.sc, sizeof(Scalars), cudaMemcpyDeviceToHost, st) != cudaSuccess || cudaStreamSynchronize(st) != cudaSuccess)
+            rc = OMNI_ERR_CUDA;
+    };
+    if (rc == OMNI_OK) read_scalars();
+    for (long long it = 0; it <= (long long)max_outer && rc == OMNI_OK && h.outer_go; ++it) {
+        const int par = h.n & 1;                   // K2 reads Pbuf[par], writes Pbuf[par ^ 1]
+        // K2: halo planes of delta first (the correction of the last inner solve), then the fold + residual
+        if (it > 0) rc = slab_exchange<T, T>(R, nranks, comm, [](SlabRank<T>& r) { return r.w.delta; }, st);
+        each([&](SlabRank<T>& r) { return launch_tma<K2<T>>(r.g, k2_args<T>(r.g, r.w, H, ch, 1), r.maps, st) == cudaSuccess ? OMNI_OK : OMNI_ERR_CUDA; });
+        if (rc == OMNI_OK) rc = slab_allreduce<T>(R, comm, d_scs, 4, st);
+        each([&](SlabRank<T>& r) { return launch_fin(std::common_type<K2<T>>{}, r, k2_args<T>(r.g, r.w, H, ch, 1)); });
+        if (rc == OMNI_OK) rc = slab_exchange<T, double>(R, nranks, comm, [par](SlabRank<T>& r) { return par ? r.w.P : r.w.P1; }, st);
+        if (rc == OMNI_OK) rc = slab_exchange<T, T>(R, nranks, comm, [](SlabRank<T>& r) { return r.w.r; }, st);
+        if (rc == OMNI_OK) read_scalars();
+        if (rc != OMNI_OK || !h.outer_go) break;
+        // inner CG; the device decides when it ends (kernels of a finished loop return at once)
+        int k = 0;
+        while (k < max_cg && rc == OMNI_OK && h.inner_go) {
+            const int batch = (max_cg - k < 16) ? (max_cg - k) : 16;
+            for (int c = 0; c < batch && rc == OMNI_OK; ++c, ++k) {
+                const int pn = (k & 1) ^ 1;                 // K3 writes pbuf[pn]
+                each([&](SlabRank<T>& r) {
+                    const Coef<T> K = make_coef<T>(H, dx, dy, dz, r.g);
+                    cudaError_t e = lop ? launch_tma<K3<T, true>>(r.g, k3_args<T, true>(r.w, K, ch), r.maps, st)
+                                        : launch_tma<K3<T, false>>(r.g, k3_args<T, false>(r.w, K, ch), r.maps, st);
+                    return e == cudaSuccess ? OMNI_OK : OMNI_ERR_CUDA;
+                });
+                if (rc == OMNI_OK) rc = slab_allreduce<T>(R, comm, d_scs, 1, st);
+                each([&](SlabRank<T>& r) {
+                    const Coef<T> K = make_coef<T>(H, dx, dy, dz, r.g);
+                    return lop ? launch_fin(std::common_type<K3<T, true>>{}, r, k3_args<T, true>(r.w, K, ch))
+                               : launch_fin(std::common_type<K3<T, false>>{}, r, k3_args<T, false>(r.w, K, ch));
+                });
+                if (rc == OMNI_OK) rc = slab_exchange<T, T>(R, nranks, comm, [pn](SlabRank<T>& r) { return pn ? r.w.p1 : r.w.p0; }, st);
+                each([&](SlabRank<T>& r) {
+                    const Coef<T> K = make_coef<T>(H, dx, dy, dz, r.g);
+                    cudaError_t e = lop ? launch_tma<K4<T, true>>(r.g, k4_args<T, true>(r.w, K, ch), r.maps, st)
+                                        : launch_tma<K4<T, false>>(r.g, k4_args<T, false>(r.w, K, ch), r.maps, st);
+                    return e == cudaSuccess ? OMNI_OK : OMNI_ERR_CUDA;
+                });
+                if (rc == OMNI_OK) rc = slab_allreduce<T>(R, comm, d_scs, 1, st);
+                each([&](SlabRank<T>& r) {
+                    const Coef<T> K = make_coef<T>(H, dx, dy, dz, r.g);
+                    return lop ? launch_fin(std::common_type<K4<T, true>>{}, r, k4_args<T, true>(r.w, K, ch))
+                               : launch_fin(std::common_type<K4<T, false>>{}, r, k4_args<T, false>(r.w, K, ch));
+                });
+                if (rc == OMNI_OK) rc = slab_exchange<T, T>(R, nranks, comm, [](SlabRank<T>& r) { return r.w.r; }, st);
+            }
+            if (rc == OMNI_OK) read_scalars();
+        }
+        each([&](SlabRank<T>& r) { return launch_flush<T>(r.g, r.w, st) == cudaSuccess ? OMNI_OK : OMNI_ERR_CUDA; });
+    }
+    each([&](SlabRank<T>& r) {
+        finalize_kernel<T><<<blocks_for((long long)nx * ny * r.g.nz, 256), 256, 0, st>>>(r.g, r.w.P, r.w.P1, r.w.sc, r.w.link, r.P_out, nullptr);
+        g_launches.fetch_add(1, std::memory_order_relaxed);
+        return cudaGetLastError() == cudaSuccess ? OMNI_OK : OMNI_ERR_CUDA;
+    });
+    if (rc == OMNI_OK) read_scalars();
+    if (rc == OMNI_OK && info) {
+        info->outer_iters = h.n; info->cg_iters_total = h.cg_total; info->norm_S = std::sqrt(h.normS2);
+        info->eps_R_final = (h.normS2 > 0.0) ? std::sqrt(h.epsR2 / h.normS2) : 0.0;
+        info->status = h.status;
+    }
+    const int status = h.status;
+    cleanup();
+    if (rc == OMNI_ERR_CUDA) cudaGetLastError();
+    return rc == OMNI_OK ? status : rc;
+}
+
 template <typename T>
 int solve_host(int nx, int ny, int nz, double dx, double dy, double dz, const T* gx, const T* gy, const T* gz,
                const unsigned char* mask, T* P_out, double tol, int max_outer, int max_cg, void* stream, omni_info* info)
@@ -1683,6 +1882,60 @@ int omni_compressible_rans_source_f32(int nx, int ny, int nz, double dx, double 
                               d_gx, d_gy, d_gz, stream);
 }
 
+int omni_slab_plan(int nz, int nranks, int rank, int* z0, int* z1, int* zlo, int* zhi)
+{
+    int a, b, c, d;
+    if (!slab_plan(nz, nranks, rank, a, b, c, d)) return OMNI_ERR_INVALID_ARG;
+    if (z0) *z0 = a;
+    if (z1) *z1 = b;
+    if (zlo) *zlo = c;
+    if (zhi) *zhi = d;
+    return OMNI_OK;
+}
+
+int omni_slab_unique_id(char* h_id128)
+{
+    if (!h_id128 || !nccl_api().ok) return OMNI_ERR_CUDA;
+    NcclApi::UniqueId id;
+    if (nccl_api().GetUniqueId(&id) != 0) return OMNI_ERR_CUDA;
+    memcpy(h_id128, id.internal, 128);
+    return OMNI_OK;
+}
+
+int omni_slab_comm_create(int rank, int nranks, const char* h_id128, void** comm)
+{
+    if (!h_id128 || !comm || nranks < 1 || rank < 0 || rank >= nranks) return OMNI_ERR_INVALID_ARG;
+    if (!nccl_api().ok) return OMNI_ERR_CUDA;
+    NcclApi::UniqueId id;
+    memcpy(id.internal, h_id128, 128);
+    return nccl_api().CommInitRank(comm, nranks, id, rank) == 0 ? OMNI_OK : OMNI_ERR_CUDA;
+}
+
+void omni_slab_comm_destroy(void* comm)
+{
+    if (comm && nccl_api().ok) nccl_api().CommDestroy(comm);
+}
+
+int omni_solve_slab_f64(int nx, int ny, int nz, double dx, double dy, double dz, int nlocal, const int* h_ranks,
+                        const double* const* h_gx, const double* const* h_gy, const double* const* h_gz,
+                        const unsigned char* const* h_mask, double* const* h_P_out, double tol, int max_outer, int max_cg,
+                        int method, int nranks, void* comm, void* stream, omni_info* info)
+{
+    if (method != OMNI_METHOD_ALG1 && method != OMNI_METHOD_DIRECT) return OMNI_ERR_INVALID_ARG;
+    return solve_slab<double>(nx, ny, nz, dx, dy, dz, nlocal, h_ranks, h_gx, h_gy, h_gz, h_mask, h_P_out, tol, max_outer, max_cg,
+                              method == OMNI_METHOD_DIRECT, nranks, comm, stream, info);
+}
+
+int omni_solve_slab_f32(int nx, int ny, int nz, double dx, double dy, double dz, int nlocal, const int* h_ranks,
+                        const float* const* h_gx, const float* const* h_gy, const float* const* h_gz,
+                        const unsigned char* const* h_mask, float* const* h_P_out, double tol, int max_outer, int max_cg,
+                        int method, int nranks, void* comm, void* stream, omni_info* info)
+{
+    if (method != OMNI_METHOD_ALG1 && method != OMNI_METHOD_DIRECT) return OMNI_ERR_INVALID_ARG;
+    return solve_slab<float>(nx, ny, nz, dx, dy, dz, nlocal, h_ranks, h_gx, h_gy, h_gz, h_mask, h_P_out, tol, max_outer, max_cg,
+                             method == OMNI_METHOD_DIRECT, nranks, comm, stream, info);
+}
+
 int omni_constants(int nx, int ny, int nz, double dx, double dy, double dz, double* h_out13)
 {
     if (!h_out13 || !valid_common(nx, ny, nz, dx, dy, dz, 0.0, 0, 0)) return OMNI_ERR_INVALID_ARG;
@@ -1808,6 +2061,6 @@ const char* omni_status_string(int status)
     }
 }
 
-int omni_version(void) { return 103; }   // 101: omni_solve_guess_*, omni_set_history, omni_rans_source_*, omni_compressible_rans_source_*
+int omni_version(void) { return 104; }   // 101: omni_solve_guess_*, omni_set_history, omni_rans_source_*, omni_compressible_rans_source_*
 
 }  // extern "C"

@@ -33,6 +33,9 @@ struct Geom {
     // tile-plane flags for the K3/K4 tiles (tbx x tby cells): bit (k & 31) of tflags[(ty*ntx + tx)*twords + (k >> 5)]
     // is set iff some group of tile (tx, ty) is flagged in plane k; unset bits let a warp skip the per-row flag word
     int tbx, tby, ntx, nty, twords;
+    // z-slab sharding (omni_slab.cuh): the local grid is a window of the global one with up to two halo planes per
+    // side; the tile kernels emit, and the reductions count, only the planes [kz0, kz1) this rank owns (0, nz otherwise)
+    int kz0, kz1;
 };
 
 // stencil coefficients, already divided by A_tot (Eq. 10 :109), in the arithmetic type T
@@ -97,6 +100,10 @@ struct Scalars {
     double* hist_p;
     int hist_cap, hist_n;
     int* status_out;   // optional device word that receives the final status (omni_options::d_status)
+    // sharded solves: defer = 1 makes the reducing kernels leave their grid totals in red_out instead of acting on them;
+    // the totals are summed over the ranks and a one-thread kernel then runs the same finalize code on every rank
+    int defer;
+    double red_out[4];
 };
 
 // dP2 = ||P^n - P^(n-1)||^2, P2 = ||P^n||^2 (Eq. 40); either 0 when nothing was folded
@@ -584,6 +591,17 @@ __global__ void codes_worklist_kernel(Geom g, const uint8_t* __restrict__ vbyte,
     }
 }
 
+__device__ __forceinline__ void source_finalize(Scalars* sc, double n2)
+{
+    sc->normS2 = n2;
+    sc->thresh2 = (0.1 * sc->tol) * (0.1 * sc->tol) * n2;
+    sc->tol2S = sc->tol * sc->tol * n2;
+    if (!(n2 > 0.0)) {                 // zero (or NaN) source: P = 0, no iterations (A4)
+        sc->outer_go = 0; sc->inner_go = 0;
+        if (!isfinite(n2)) sc->status = ST_BREAKDOWN;
+    }
+}
+
 // ------------------------------------------------------------------------------------------------ K1 source
 // S_C = - sum_d v(C+d) sgn(d) (Delta_a t_a / 2) (g_a(C+d) + g_a(C))     (Eq. 9 :100, w^{n+1}+w^n = t_a)
 template <typename T>
@@ -617,6 +635,10 @@ source_kernel(Geom g, const T* __restrict__ gx, const T* __restrict__ gy, const 
             }
         }
         S[pid] = s;
+        if (g.kz0 > 0 || g.kz1 < g.nz) {                 // a slab counts the planes it owns
+            const int k = (int)(row / g.ny);
+            if (k < g.kz0 || k >= g.kz1) s = T(0);
+        }
         sq += (double)s * (double)s;
     }
     sq = warp_sum(sq);
@@ -642,13 +664,7 @@ source_kernel(Geom g, const T* __restrict__ gx, const T* __restrict__ gy, const 
             double n2 = 0.0;
             for (int w = 0; w < 8; ++w) n2 += red[w];
             sc->ticket[3] = 0;
-            sc->normS2 = n2;
-            sc->thresh2 = (0.1 * sc->tol) * (0.1 * sc->tol) * n2;
-            sc->tol2S = sc->tol * sc->tol * n2;
-            if (!(n2 > 0.0)) {                 // zero (or NaN) source: P = 0, no iterations (A4)
-                sc->outer_go = 0; sc->inner_go = 0;
-                if (!isfinite(n2)) sc->status = ST_BREAKDOWN;
-            }
+            if (sc->defer) sc->red_out[0] = n2; else source_finalize(sc, n2);
         }
     }
 }

@@ -77,7 +77,7 @@ tma_loop_kernel(const Geom g, const ZSeg zs, const LoopArgs<K2, K3, K4> a, const
     const int ntx2 = (g.px + K2::TG::BX - 1) / K2::TG::BX;
     const int tx = blockIdx.x % ntx, ty = (blockIdx.x / ntx) % nty, seg = blockIdx.x / (ntx * nty);
     const int k0 = zs.n ? zs.k[seg] : seg * zs.zlen;
-    const int k1 = zs.n ? zs.k[seg + 1] : min(g.nz, k0 + zs.zlen);
+    const int k1 = zs.n ? zs.k[seg + 1] : min(g.nz, k0 + zs.zlen);      // (never used on a slab: kz0 = 0, kz1 = nz)
 
     GridSync gs{ { 2u, 2u }, red, &flag, a.timeout_ns };
 

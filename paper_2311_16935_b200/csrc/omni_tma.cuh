@@ -297,14 +297,15 @@ template <bool REV>
 __device__ __forceinline__ void cta_column(const Geom& g, const ZSeg& zs, int& tx, int& ty, int& k0, int& k1)
 {
     const int bz = blockIdx.z;
+    const int nzr = g.kz1 - g.kz0;                   // planes to emit: all of them, or the ones a slab owns
     int lo = zs.n ? zs.k[bz] : bz * zs.zlen;
-    int hi = zs.n ? zs.k[bz + 1] : min(g.nz, lo + zs.zlen);
+    int hi = zs.n ? zs.k[bz + 1] : min(nzr, lo + zs.zlen);
     if (REV) {
         tx = gridDim.x - 1 - blockIdx.x; ty = gridDim.y - 1 - blockIdx.y;
-        k0 = g.nz - hi; k1 = g.nz - lo;
+        k0 = g.kz0 + nzr - hi; k1 = g.kz0 + nzr - lo;
     } else {
         tx = blockIdx.x; ty = blockIdx.y;
-        k0 = lo; k1 = hi;
+        k0 = g.kz0 + lo; k1 = g.kz0 + hi;
     }
 }
 
@@ -389,9 +390,25 @@ tma_kernel(const Geom g, const ZSeg zs, const typename Op::Args a, const __grid_
         }
         if (threadIdx.x == 0) {
             a.sc->ticket[Op::TICKET] = 0;
-            Op::finalize(a, tot);
+            if (a.sc->defer) {
+#pragma unroll
+                for (int i = 0; i < NACC; ++i) a.sc->red_out[i] = tot[i];      // summed over the ranks first (omni_slab.cuh)
+            } else {
+                Op::finalize(a, tot);
+            }
         }
     }
+}
+
+// sharded solves: the finalize step of Op on the rank-summed totals (one thread; every rank runs it on identical numbers)
+template <class Op>
+__global__ void op_finalize_kernel(const typename Op::Args a)
+{
+    if (!Op::active(a)) return;
+    double tot[Op::NACC];
+#pragma unroll
+    for (int i = 0; i < Op::NACC; ++i) tot[i] = a.sc->red_out[i];
+    Op::finalize(a, tot);
 }
 
 // ------------------------------------------------------------------------------------------------ K3 (TMA)

@@ -189,7 +189,8 @@ def test_converged_field_certified_by_oracle(oracle, idx, dtype):
     the fp64 master pressure rounded to fp32, and that rounding alone leaves a residual u |L||P| that grows with the
     grid (SURVEY 7 hard part 3), so the oracle's figure is bounded by tol plus that floor, the floor being evaluated by
     the oracle on the same field (the residual change under one more fp32 rounding of P_out has the same statistics).
-    configs[4] by Alg. 1 takes about two minutes of GPU time (10 500 outer iterations)."""
+    configs[4] by Alg. 1 takes about two minutes of GPU time (10 500 outer iterations): here only with OMNI_TEST_LONG=1;
+    the default bench.py line runs it and has the oracle certify it (section `converged`)."""
     f, g_dev, g_or, mask, m_dev = _load(idx, dtype)
     d, tol = f["d"], TOL_CONV[dtype]
     P64 = torch.zeros(f["g"][0].shape, dtype=torch.float64, device="cuda") if dtype == "f32" else None
@@ -197,6 +198,11 @@ def test_converged_field_certified_by_oracle(oracle, idx, dtype):
             ("cascade", lambda: omni.solve_cascade(g_dev[0], g_dev[1], g_dev[2], m_dev, d, tol, 20, 30000, levels=4)),
             ("pcg", lambda: omni.solve_ex(g_dev[0], g_dev[1], g_dev[2], m_dev, d, tol, 20, 300, method="pcg", P64_out=P64))]
     for name, fn in runs:
+        if name == "alg1" and idx == 4 and not LONG:
+            # two minutes of GPU time (10 500 outer iterations); the same run, oracle-certified, is part of the default
+            # bench.py line (section `converged`)
+            print("configs[4] by Alg. 1: set OMNI_TEST_LONG=1 to run it here; bench.py runs and certifies it")
+            continue
         P, info = fn()
         assert info["status"] == 0 and info["eps_R_final"] <= tol, (name, info)
         Pn = P.cpu().numpy()

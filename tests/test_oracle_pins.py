@@ -1051,3 +1051,30 @@ def test_eps_P_history_eq40(oracle):
     rate_P = hP[late][1:] / hP[late][:-1]
     rate_R = hR[late][1:] / hR[late][:-1]
     assert np.allclose(rate_P, rate_R, rtol=0.15)
+
+
+@pytest.mark.parametrize("shape,sp", [((9, 10), (1.0, 0.6, 1.0)), ((5, 5, 6), (1.0, 1.3, 0.8))])
+def test_single_reduction_cg_oracle(oracle, shape, sp):
+    """oracle_solve_direct_cg1 (Chronopoulos-Gear: one reduction point per iteration, NEXT-2 i) on the symmetric L:
+    its truncated iterates are those of a dense textbook CG written here (the two recurrences coincide in exact
+    arithmetic), it converges to pinv(L) S, and its drift from the two-reduction oracle stays at rounding level."""
+    g, mask, v, _, S, t = _pcg_case(oracle, shape, sp)
+    keep = v.ravel() == 1
+    Lk, Sk = _dense_laplacian(v, t)[np.ix_(keep, keep)], S.ravel()[keep]
+    for k in (1, 2, 5, 11):
+        x = np.zeros_like(Sk); r = Sk.copy(); pv = r.copy(); rho = r @ r
+        for _ in range(k):
+            q = Lk @ pv
+            al = rho / (pv @ q)
+            x += al * pv; r -= al * q
+            rho1 = r @ r
+            pv = r + (rho1 / rho) * pv
+            rho = rho1
+        Pk, ik = oracle.solve_direct(g[0], g[1], g[2], mask, *sp, tol=0.0, max_outer=1, max_cg=k, single_reduction=True)
+        assert ik["cg_iters_total"] == k
+        assert np.linalg.norm(Pk.ravel()[keep] - x) / np.linalg.norm(x) < 1e-10
+    P1, i1 = oracle.solve_direct(g[0], g[1], g[2], mask, *sp, tol=1e-11, max_outer=5, max_cg=2000, single_reduction=True)
+    P2, i2 = oracle.solve_direct(g[0], g[1], g[2], mask, *sp, tol=1e-11, max_outer=5, max_cg=2000)
+    assert i1["converged"] and i2["converged"] and abs(i1["cg_iters_total"] - i2["cg_iters_total"]) <= 3
+    a, b = np.nan_to_num(P1), np.nan_to_num(P2)
+    assert np.linalg.norm(a - b) / np.linalg.norm(b) < 1e-9
