@@ -103,6 +103,10 @@ int omni_solve_host_f32(int nx, int ny, int nz, double dx, double dy, double dz,
  *                   2^-24 |L||P| / ||S||, which on 1000-cell-wide grids exceeds tol = 1e-5; d_P64_out satisfies eps_R <= tol
  *   d_status        one int: the final status, written by the device when the solve ends -- the way to learn about
  *                   OMNI_NOT_CONVERGED / OMNI_ERR_BREAKDOWN after a call made with info == NULL (no synchronisation)
+ *   single_reduction  OMNI_METHOD_DIRECT in the persistent loop (mode 3: grids up to 1.5 M cells by default) only: the
+ *                   Chronopoulos-Gear recurrences, ONE grid barrier per CG iteration instead of two (SURVEY.md 8(f)
+ *                   NEXT-2 i).  In exact arithmetic the same iterates; it relies on L = L^T, so it does not exist for
+ *                   Algorithm 1, whose operator is not symmetric (A2).  Ignored elsewhere.
  * struct_size must be sizeof(omni_options) (omni_options_init sets it, loop_mode = -1 and everything else to 0 / NULL);
  * a mismatch, hist_capacity < 0, a history pointer with hist_capacity == 0 or an unknown method: OMNI_ERR_INVALID_ARG. */
 enum { OMNI_METHOD_ALG1 = 0, OMNI_METHOD_DIRECT = 1, OMNI_METHOD_PCG = 2 };
@@ -115,6 +119,7 @@ typedef struct {
     double* d_hist_eps_P;
     double* d_P64_out;
     int* d_status;
+    int single_reduction;
 } omni_options;
 void omni_options_init(omni_options* options);
 int omni_solve_ex_f64(int nx, int ny, int nz, double dx, double dy, double dz,

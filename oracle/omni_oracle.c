@@ -394,9 +394,11 @@ static int cg1_op(int nx, int ny, int nz, const unsigned char *v, const double *
         apply_op(1, nx, ny, nz, v, w1, w0, w0C, r, w, tmp);
         double gamma1 = dot(N, nx, r, r), delta1 = dot(N, nx, w, r);      /* the iteration's single reduction point */
         beta = gamma1 / gamma;
-        alpha = gamma1 / (delta1 - beta * gamma1 / alpha);
+        double den = delta1 - beta * gamma1 / alpha;                      /* stands for p.Ap > 0 */
         gamma = gamma1;
         ++k;
+        if (!(den > 0.0)) break;      /* the recurrences have lost their accuracy: the caller's outer loop restarts on the true residual */
+        alpha = gamma1 / den;
     }
     return k;
 }

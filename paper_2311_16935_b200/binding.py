@@ -254,14 +254,15 @@ class Options(C.Structure):
     """omni_options of include/omni.h."""
     _fields_ = [("struct_size", C.c_size_t), ("loop_mode", C.c_int), ("hist_capacity", C.c_int),
                 ("d_hist_eps_R", C.c_void_p), ("d_hist_cg_iters", C.c_void_p), ("d_hist_eps_P", C.c_void_p),
-                ("d_P64_out", C.c_void_p), ("d_status", C.c_void_p)]
+                ("d_P64_out", C.c_void_p), ("d_status", C.c_void_p), ("single_reduction", C.c_int)]
 
 
 METHODS = {"alg1": 0, "direct": 1, "pcg": 2}
 
 
 def solve_ex(gx, gy, gz, mask, d, tol, max_outer, max_cg, method="alg1", P_init=None, out=None, loop_mode=-1,
-             hist_eps_R=None, hist_cg_iters=None, hist_eps_P=None, P64_out=None, status=None, want_info=True):
+             hist_eps_R=None, hist_cg_iters=None, hist_eps_P=None, P64_out=None, status=None, want_info=True,
+             single_reduction=False):
     """omni_solve_ex_*: one solve with per-call options (omni_options): loop mode, history buffers (CUDA float64 /
     int32 tensors of one common length), the fp64 master pressure (CUDA float64 tensor shaped like gx) and a device
     status word (CUDA int32 tensor with one element).  Returns (P, info dict or None)."""
@@ -284,6 +285,7 @@ def solve_ex(gx, gy, gz, mask, d, tol, max_outer, max_cg, method="alg1", P_init=
     o.d_hist_eps_R, o.d_hist_cg_iters, o.d_hist_eps_P = (None if t is None else t.data_ptr() for t in (hist_eps_R, hist_cg_iters, hist_eps_P))
     o.d_P64_out = None if P64_out is None else P64_out.data_ptr()
     o.d_status = None if status is None else status.data_ptr()
+    o.single_reduction = 1 if single_reduction else 0
     P = out if out is not None else torch.empty_like(gx)
     info = Info()
     with torch.cuda.device(gx.device):

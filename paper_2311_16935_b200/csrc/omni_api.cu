@@ -3,6 +3,7 @@
 // loop driver (CUDA graph with device-side conditional WHILE nodes, or a host-driven debug loop).
 #include "omni_tma.cuh"
 #include "omni_persist.cuh"
+#include "omni_persist1.cuh"
 #include "omni_loop.cuh"
 #include "omni_mg.cuh"
 #include "omni_slab.cuh"
@@ -65,6 +66,7 @@ struct CallOpts {
     double* hist; int* hist_k; double* hist_p; int hist_cap;
     double* P64;
     int* status;
+    int single_reduction;
 };
 thread_local const CallOpts* tl_opts = nullptr;
 CallOpts current_opts()
@@ -73,7 +75,7 @@ CallOpts current_opts()
     CallOpts o;
     o.loop_mode = g_loop_mode.load();
     o.hist = g_hist.load(); o.hist_k = g_hist_k.load(); o.hist_p = nullptr; o.hist_cap = g_hist_cap.load();
-    o.P64 = nullptr; o.status = nullptr;
+    o.P64 = nullptr; o.status = nullptr; o.single_reduction = 0;
     return o;
 }
 
@@ -1025,6 +1027,61 @@ int run_loop_persist(const Geom& g, const Workspace<T>& w, const HostConst& H, c
                                                 : launch_persist<T, 1024, LOP>(g, w, H, K, nsm, st);
 }
 
+// Single-reduction CG for the fixed-point solve (omni_persist1.cuh): the persistent kernel with one grid barrier per
+// iteration.  Four more vectors (double-buffered r, w, s and p) come from the pool.  -100: cannot be co-scheduled.
+template <typename T, int NT>
+int launch_persist1(const Geom& g, const Workspace<T>& w, const HostConst& H, const Coef<T>& K, int nsm, cudaStream_t st)
+{
+    int occ = 0;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, persist_cg1_kernel<T, NT>, NT, 0) != cudaSuccess || occ < 1) {
+        cudaGetLastError();
+        return -100;
+    }
+    const size_t nb = align_up((size_t)g.npad * sizeof(T), 256);
+    char* extra = nullptr;
+    if (pool_alloc(&extra, 4 * nb, st) != cudaSuccess) { cudaGetLastError(); return OMNI_ERR_ALLOC; }
+    CK(cudaMemsetAsync(extra, 0, 4 * nb, st));
+    Persist1Args<T> A;
+    PersistArgs<T>& a = A.base;
+    a.r = w.r; a.pbuf[0] = w.p0; a.pbuf[1] = w.p1; a.delta = w.delta; a.S = w.S; a.Pbuf[0] = w.P; a.Pbuf[1] = w.P1;
+    a.link = w.link; a.wcode = w.wcode; a.flags = w.flags; a.K = K;
+    for (int i = 0; i < 3; ++i) a.t[i] = H.F[i] / H.Atot;
+    a.sc = w.sc; a.slots = w.slots;
+    a.timeout_ns = barrier_timeout_ns();
+    A.rb[0] = w.r; A.rb[1] = (T*)extra;
+    A.wb[0] = w.p0; A.wb[1] = w.p1;
+    A.sb[0] = (T*)(extra + nb); A.sb[1] = (T*)(extra + 2 * nb);
+    A.p = (T*)(extra + 3 * nb);
+    const long long tasks = (long long)g.ny * g.nz * ((g.nx + 63) / 64);
+    const int nw = NT / 32;
+    long long G = (tasks + nw - 1) / nw;
+    if (G > nsm) G = nsm;
+    if (G > PERSIST_MAX_CTAS) G = PERSIST_MAX_CTAS;
+    if (G < 1) G = 1;
+    CK(cudaMemsetAsync(w.slots, 0, (size_t)8 * G * sizeof(double), st));
+    Geom gg = g;
+    void* params[2] = { (void*)&gg, (void*)&A };
+    int rc = OMNI_OK;
+    if (cudaLaunchCooperativeKernel((const void*)persist_cg1_kernel<T, NT>, dim3((unsigned)G), dim3(NT), params, 0, st) != cudaSuccess) {
+        cudaGetLastError();
+        rc = -100;
+    } else {
+        g_launches.fetch_add(1, std::memory_order_relaxed);
+    }
+    cudaFreeAsync(extra, st);
+    return rc;
+}
+
+template <typename T>
+int run_loop_persist1(const Geom& g, const Workspace<T>& w, const HostConst& H, const Coef<T>& K, cudaStream_t st)
+{
+    const DevInfo di = device_info();
+    if (!di.coop || di.sms < 1) return -100;
+    if ((long long)g.ny * g.nz * ((g.nx + 63) / 64) >= (1LL << 31)) return -100;
+    return (g.npad <= OMNI_PERSIST_SMALL_CELLS) ? launch_persist1<T, 512>(g, w, H, K, di.sms, st)
+                                                : launch_persist1<T, 1024>(g, w, H, K, di.sms, st);
+}
+
 // loop selection: g_loop_mode 0 = automatic (persistent kernel for grids up to OMNI_PERSIST_MAX_CELLS padded cells, CUDA graph above),
 // 1 = host-driven, 2 = CUDA graph, 3 = persistent kernel
 long long persist_max_cells()
@@ -1110,7 +1167,9 @@ int solve_ws(int nx, int ny, int nz, double dx, double dy, double dz, const T* g
     }
     // lop: the CG kernels apply L instead of M (omni_solve_direct); everything else -- K2, scalars, loop control -- is shared
     if (mode == 3) {
-        rc = lop ? run_loop_persist<T, true>(g, w, H, K, st) : run_loop_persist<T, false>(g, w, H, K, st);
+        // fixed-point solve with omni_options::single_reduction: the one-barrier-per-iteration kernel (L = L^T only)
+        if (lop && opt.single_reduction) rc = run_loop_persist1<T>(g, w, H, K, st);
+        else rc = lop ? run_loop_persist<T, true>(g, w, H, K, st) : run_loop_persist<T, false>(g, w, H, K, st);
         if (rc == -100) mode = 2;
     }
     if (mode == 4) {
@@ -1793,7 +1852,7 @@ int solve_ex(int nx, int ny, int nz, double dx, double dy, double dz, const T* g
         if (o->hist_capacity == 0 && (o->d_hist_eps_R || o->d_hist_cg_iters || o->d_hist_eps_P)) return OMNI_ERR_INVALID_ARG;
         if (o->loop_mode >= 0) c.loop_mode = o->loop_mode;
         c.hist = o->d_hist_eps_R; c.hist_k = o->d_hist_cg_iters; c.hist_p = o->d_hist_eps_P; c.hist_cap = o->hist_capacity;
-        c.P64 = o->d_P64_out; c.status = o->d_status;
+        c.P64 = o->d_P64_out; c.status = o->d_status; c.single_reduction = o->single_reduction != 0;
     }
     tl_opts = &c;
     const int rc = solve_alloc<T>(nx, ny, nz, dx, dy, dz, gx, gy, gz, mask, P_out, tol, max_outer, max_cg, stream, info, 0, P_init,

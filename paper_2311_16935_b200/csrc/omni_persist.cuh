@@ -188,6 +188,97 @@ struct RowTask {
     }
 };
 
+// K2 phase of the persistent kernels on the row tasks [lo2, hi2) of this CTA: Pout = Pin + delta (unless dzero),
+// r = S - L Pout written to rout; acc = { ||r||^2 in fp64, ||r rounded to T||^2 }, accp = { ||delta||^2, ||Pout||^2 } if want_p
+template <typename T>
+__device__ __forceinline__ void persist_k2_rows(const Geom& g, const PersistArgs<T>& a, T* __restrict__ rout, const double* Pin,
+                                                double* Pout, bool dzero, bool want_p, int lo2, int hi2, int wfirst, int wstep,
+                                                int nsx2, int lane, double (&acc)[2], double (&accp)[2])
+{
+    const bool three = g.naxes == 3;
+    const long long pp = g.pplane;
+    RowTask<2> tk(g, lo2 + wfirst, nsx2, wstep, lane);
+    for (int t = lo2 + wfirst; t < hi2; t += wstep, tk.next(g, lane)) {
+        auto val = [&](long long i, bool ok, double (&v)[2]) {
+            v[0] = v[1] = 0.0;
+            if (ok) {
+                double P[2]; T d[2] = { T(0), T(0) };
+                ldcg_chunk<double, 2>(Pin + i, P);
+                if (!dzero) ldcg_chunk<T, 2>(a.delta + i, d);
+                v[0] = P[0] + (double)d[0];
+                v[1] = P[1] + (double)d[1];
+            }
+        };
+        auto val1 = [&](long long i) { return ldd(Pin + i) + (dzero ? 0.0 : (double)ldd(a.delta + i)); };
+        // every load of the task is issued before the first use
+        uint32_t fw = 0, lkb = 0;
+        T S[2] = { T(0), T(0) };
+        if (tk.out) {
+            fw = flag_bits<2>(a.flags, tk.idx);
+            lkb = *reinterpret_cast<const unsigned short*>(a.link + tk.idx);
+            ld_chunk<T, 2>(a.S + tk.idx, S);
+        }
+        double vm[2], vc[2], vp[2], vn[2], vs[2];
+        val(tk.idx, tk.inb, vc);
+        val(tk.idx + g.px, tk.inb && tk.j + 1 < g.ny, vn);
+        val(tk.idx - g.px, tk.inb && tk.j > 0, vs);
+        val(tk.idx + pp, tk.inb && three && tk.k + 1 < g.nz, vp);
+        val(tk.idx - pp, tk.inb && three && tk.k > 0, vm);
+        double xl = __shfl_up_sync(0xffffffffu, vc[1], 1);
+        double xr = __shfl_down_sync(0xffffffffu, vc[0], 1);
+        if (lane == 0) xl = (tk.x > 0) ? val1(tk.idx - 1) : 0.0;
+        if (lane == 31) xr = (tk.x + 2 < g.px) ? val1(tk.idx + 2) : 0.0;
+        if (!tk.out) continue;
+        st_chunk<double, 2>(Pout + tk.idx, vc);
+        uint32_t lk = 0;
+#pragma unroll
+        for (int i = 0; i < 2; ++i) {
+            const int gi = tk.x + i;
+            uint32_t l = 0x7fu;
+            if (!three) l &= ~48u;
+            if (g.fix[0]) {
+                if (gi == 0) l &= ~2u;
+                if (gi == g.nx - 1) l &= ~1u;
+                if (gi >= g.nx) l = 0;
+            }
+            lk |= l << (8 * i);
+        }
+        const int ycls = face_class(tk.j, g.ny, g.fix[1]), zcls = face_class(tk.k, g.nz, g.fix[2]);
+        if (ycls == 0) lk &= ~0x0808u;
+        if (ycls == 3) lk &= ~0x0404u;
+        if (zcls == 0) lk &= ~0x2020u;
+        if (zcls == 3) lk &= ~0x1010u;
+        if (fw) lk = lkb;
+        T rn[2];
+#pragma unroll
+        for (int i = 0; i < 2; ++i) {
+            const double w = (i == 0) ? xl : vc[0];
+            const double ee = (i == 1) ? xr : vc[1];
+            const uint32_t l = (lk >> (8 * i)) & 0xffu;
+            double LP = 0.0;
+            if (l & 1u) LP += a.t[0] * (vc[i] - ee);
+            if (l & 2u) LP += a.t[0] * (vc[i] - w);
+            if (l & 4u) LP += a.t[1] * (vc[i] - vn[i]);
+            if (l & 8u) LP += a.t[1] * (vc[i] - vs[i]);
+            if (l & 16u) LP += a.t[2] * (vc[i] - vp[i]);
+            if (l & 32u) LP += a.t[2] * (vc[i] - vm[i]);
+            const double rr = (l & LINK_VALID) ? ((double)S[i] - LP) : 0.0;
+            rn[i] = (T)rr;
+            acc[0] += rr * rr;
+            acc[1] += (double)rn[i] * (double)rn[i];
+            if (want_p && (l & LINK_VALID)) accp[1] += vc[i] * vc[i];
+        }
+        if (want_p && !dzero) {
+            T d[2];
+            ldcg_chunk<T, 2>(a.delta + tk.idx, d);
+#pragma unroll
+            for (int i = 0; i < 2; ++i)
+                if ((lk >> (8 * i)) & LINK_VALID) accp[0] += (double)d[i] * (double)d[i];
+        }
+        st_chunk<T, 2>(rout + tk.idx, rn);
+    }
+}
+
 template <typename T, int NT, bool LOP>
 __global__ void __launch_bounds__(NT, 1)
 persist_kernel(const Geom g, const PersistArgs<T> a)
@@ -228,86 +319,7 @@ persist_kernel(const Geom g, const PersistArgs<T> a)
             double* Pout = a.Pbuf[par ^ 1];
             double acc[2] = { 0.0, 0.0 }, accp[2] = { 0.0, 0.0 };
             const bool want_p = sc->hist_p != nullptr;             // Eq. 40 history asked for (grid-uniform)
-            RowTask<2> tk(g, lo2 + wfirst, nsx2, wstep, lane);
-            for (int t = lo2 + wfirst; t < hi2; t += wstep, tk.next(g, lane)) {
-                auto val = [&](long long i, bool ok, double (&v)[2]) {
-                    v[0] = v[1] = 0.0;
-                    if (ok) {
-                        double P[2]; T d[2] = { T(0), T(0) };
-                        ldcg_chunk<double, 2>(Pin + i, P);
-                        if (!dzero) ldcg_chunk<T, 2>(a.delta + i, d);
-                        v[0] = P[0] + (double)d[0];
-                        v[1] = P[1] + (double)d[1];
-                    }
-                };
-                auto val1 = [&](long long i) { return ldd(Pin + i) + (dzero ? 0.0 : (double)ldd(a.delta + i)); };
-                // every load of the task is issued before the first use
-                uint32_t fw = 0, lkb = 0;
-                T S[2] = { T(0), T(0) };
-                if (tk.out) {
-                    fw = flag_bits<2>(a.flags, tk.idx);
-                    lkb = *reinterpret_cast<const unsigned short*>(a.link + tk.idx);
-                    ld_chunk<T, 2>(a.S + tk.idx, S);
-                }
-                double vm[2], vc[2], vp[2], vn[2], vs[2];
-                val(tk.idx, tk.inb, vc);
-                val(tk.idx + g.px, tk.inb && tk.j + 1 < g.ny, vn);
-                val(tk.idx - g.px, tk.inb && tk.j > 0, vs);
-                val(tk.idx + pp, tk.inb && three && tk.k + 1 < g.nz, vp);
-                val(tk.idx - pp, tk.inb && three && tk.k > 0, vm);
-                double xl = __shfl_up_sync(0xffffffffu, vc[1], 1);
-                double xr = __shfl_down_sync(0xffffffffu, vc[0], 1);
-                if (lane == 0) xl = (tk.x > 0) ? val1(tk.idx - 1) : 0.0;
-                if (lane == 31) xr = (tk.x + 2 < g.px) ? val1(tk.idx + 2) : 0.0;
-                if (!tk.out) continue;
-                st_chunk<double, 2>(Pout + tk.idx, vc);
-                uint32_t lk = 0;
-#pragma unroll
-                for (int i = 0; i < 2; ++i) {
-                    const int gi = tk.x + i;
-                    uint32_t l = 0x7fu;
-                    if (!three) l &= ~48u;
-                    if (g.fix[0]) {
-                        if (gi == 0) l &= ~2u;
-                        if (gi == g.nx - 1) l &= ~1u;
-                        if (gi >= g.nx) l = 0;
-                    }
-                    lk |= l << (8 * i);
-                }
-                const int ycls = face_class(tk.j, g.ny, g.fix[1]), zcls = face_class(tk.k, g.nz, g.fix[2]);
-                if (ycls == 0) lk &= ~0x0808u;
-                if (ycls == 3) lk &= ~0x0404u;
-                if (zcls == 0) lk &= ~0x2020u;
-                if (zcls == 3) lk &= ~0x1010u;
-                if (fw) lk = lkb;
-                T rn[2];
-#pragma unroll
-                for (int i = 0; i < 2; ++i) {
-                    const double w = (i == 0) ? xl : vc[0];
-                    const double ee = (i == 1) ? xr : vc[1];
-                    const uint32_t l = (lk >> (8 * i)) & 0xffu;
-                    double LP = 0.0;
-                    if (l & 1u) LP += a.t[0] * (vc[i] - ee);
-                    if (l & 2u) LP += a.t[0] * (vc[i] - w);
-                    if (l & 4u) LP += a.t[1] * (vc[i] - vn[i]);
-                    if (l & 8u) LP += a.t[1] * (vc[i] - vs[i]);
-                    if (l & 16u) LP += a.t[2] * (vc[i] - vp[i]);
-                    if (l & 32u) LP += a.t[2] * (vc[i] - vm[i]);
-                    const double rr = (l & LINK_VALID) ? ((double)S[i] - LP) : 0.0;
-                    rn[i] = (T)rr;
-                    acc[0] += rr * rr;
-                    acc[1] += (double)rn[i] * (double)rn[i];
-                    if (want_p && (l & LINK_VALID)) accp[1] += vc[i] * vc[i];
-                }
-                if (want_p && !dzero) {
-                    T d[2];
-                    ldcg_chunk<T, 2>(a.delta + tk.idx, d);
-#pragma unroll
-                    for (int i = 0; i < 2; ++i)
-                        if ((lk >> (8 * i)) & LINK_VALID) accp[0] += (double)d[i] * (double)d[i];
-                }
-                st_chunk<T, 2>(a.r + tk.idx, rn);
-            }
+            persist_k2_rows<T>(g, a, a.r, Pin, Pout, dzero, want_p, lo2, hi2, wfirst, wstep, nsx2, lane, acc, accp);
             double tot[2], totp[2] = { 0.0, 0.0 };
             if (!grid_allreduce<2, NT>(gs, a.slots, acc, tot)) { status = ST_BARRIER_TIMEOUT; break; }
             if (want_p && !grid_allreduce<2, NT>(gs, a.slots, accp, totp)) { status = ST_BARRIER_TIMEOUT; break; }

@@ -988,8 +988,8 @@ def test_fp64_master_pressure_meets_tol_where_fp32_output_cannot(oracle, method)
     assert info["status"] == 0 and info["eps_R_final"] <= tol
     e64, _, _ = oracle.eps_R_of_field(g_or[0], g_or[1], None, m, P64.cpu().numpy(), *d)
     e32, _, _ = oracle.eps_R_of_field(g_or[0], g_or[1], None, m, P.cpu().numpy(), *d)
-    # the device forms S and r in fp32: near convergence r is 1e-5 of S, so S's own rounding shows at the per-cent level
-    assert e64 == pytest.approx(info["eps_R_final"], rel=3e-2) and e64 <= 1.05 * tol
+    # the device forms S and r in fp32 (2^-24 relative per entry of S): the two figures agree to a few 1e-7 of ||S||
+    assert abs(e64 - info["eps_R_final"]) <= 5e-7 and e64 <= 1.05 * tol
     assert e32 > e64
 
 
@@ -1044,3 +1044,34 @@ def test_slab_sharded_solve_converged(oracle, dtype, tol):
     assert abs(i1["cg_iters_total"] - info["cg_iters_total"]) <= 2
     valid = ~torch.isnan(P1).cpu().numpy()
     assert rel_l2_after_mean_removal(P.cpu().numpy(), P1.cpu().numpy(), valid) <= (2e-6 if dtype == "f64" else 2e-3)
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("kind,shape,frac", [("gaussians2d", (64, 64), None), ("lamb_oseen2d", (150, 130), None),
+                                             ("sphere3d", (40, 36, 44), None), ("fourier3d", (12, 30, 270), 0.15),
+                                             ("gaussians2d", (21, 132), None), ("fourier3d", (5, 4, 9), 0.2)])
+def test_single_reduction_cg_parity(oracle, dtype, kind, shape, frac):
+    """omni_options::single_reduction (Chronopoulos-Gear CG for the symmetric L in the persistent kernel, one grid barrier
+    per iteration; NEXT-2 i) against oracle_solve_direct_cg1 with fixed iteration counts, against the two-reduction
+    library result (same iterates in exact arithmetic: the drift is rounding), and converged."""
+    f = make_field(kind, shape, seed=7, noise=0.05, kmax=4.0)
+    mask = _random_mask(shape, 9, frac) if frac else None
+    g_dev, g_or, m_dev, m = _inputs(f, dtype, mask)
+    d = f["d"]
+    P, info = omni.solve_ex(g_dev[0], g_dev[1], g_dev[2], m_dev, d, 0.0, 2, 15, method="direct", loop_mode=3, single_reduction=True)
+    Po, io = oracle.solve_direct(g_or[0], g_or[1], g_or[2], m, *d, tol=0.0, max_outer=2, max_cg=15, single_reduction=True)
+    valid = ~np.isnan(Po)
+    assert np.array_equal(np.isnan(P.cpu().numpy()), ~valid)
+    assert info["outer_iters"] == io["outer_iters"] == 2 and info["cg_iters_total"] == io["cg_iters_total"] == 30
+    assert rel_l2_after_mean_removal(P.cpu().numpy(), Po, valid) <= TOL_SOLVE[dtype]
+    assert info["eps_R_final"] == pytest.approx(io["eps_R_final"], rel=5e-3 if dtype == "f32" else 1e-7)
+    P2, i2 = omni.solve_ex(g_dev[0], g_dev[1], g_dev[2], m_dev, d, 0.0, 2, 15, method="direct", loop_mode=3)
+    assert rel_l2_after_mean_removal(P.cpu().numpy(), P2.cpu().numpy(), valid) <= (1e-10 if dtype == "f64" else 2e-4)
+    tol = 1e-8 if dtype == "f64" else 1e-5
+    Pc, ic = omni.solve_ex(g_dev[0], g_dev[1], g_dev[2], m_dev, d, tol, 10, 5000, method="direct", loop_mode=3, single_reduction=True)
+    Pd, idd = omni.solve_ex(g_dev[0], g_dev[1], g_dev[2], m_dev, d, tol, 10, 5000, method="direct", loop_mode=3)
+    assert ic["status"] == 0 and ic["eps_R_final"] <= tol
+    # the single-reduction recurrences are numerically weaker (SURVEY 8(d) V5): in fp32 the recurred s = A p drifts and
+    # costs up to ~10 % more iterations (711 vs 653 on the 150 x 130 case); fp64 stays within a few iterations
+    assert abs(ic["cg_iters_total"] - idd["cg_iters_total"]) <= max(3, idd["cg_iters_total"] // (5 if dtype == "f32" else 20))
+    assert rel_l2_after_mean_removal(Pc.cpu().numpy(), Pd.cpu().numpy(), valid) <= (2e-6 if dtype == "f64" else 2e-3)
