@@ -16,7 +16,7 @@
 #include "omni_kernels.cuh"
 
 #ifndef OMNI_ZIGZAG
-#define OMNI_ZIGZAG 1      // K4 marches z downwards (0: every kernel marches upwards)
+#define OMNI_ZIGZAG 0      // 1: K4 marches z downwards (+3 % at 256^3 fp32, -4 % at 500^3: profiles/r2_loop_and_rows.md); 0: every kernel upwards
 #endif
 
 namespace omni {
@@ -717,12 +717,13 @@ struct OpT2 {
         int fold_delta;   // 0: residual of P as given (omni_residual); 1: inside the solve
     };
     struct Ctx {
-        int par; double* Pout; bool dz;
+        int par; double* Pout; bool dz, want_p;
         __device__ Ctx(const Args& a) : Ctx(a, a.sc->n, a.sc->dzero) {}
         __device__ Ctx(const Args& a, int n, int dzero)
         {
             par = a.fold_delta ? (n & 1) : 0; Pout = a.Pbuf[par ^ 1];
             dz = !a.fold_delta || dzero != 0;             // delta counts as zero: neither loaded nor added
+            want_p = a.sc->hist_p != nullptr;             // Eq. 40 history asked for: two more sums
         }
     };
     // thread constant: link bytes of an unflagged chunk as far as x decides (box faces normal to x, pad cells)
@@ -818,8 +819,8 @@ struct OpT2 {
             if (!CLEAN && fb[r]) lk = code[r][0];
             T S[2];
             lds_pair(sC + TG::TILE_P + TG::TILE_D + ((warp * R + r) * TG::BX + lane * V) * (int)sizeof(T), S);
-            double dd[V];
-            delta_of(sC, rowD + xD, c.dz, dd);
+            double dd[V] = { 0.0, 0.0 };
+            if (c.want_p) delta_of(sC, rowD + xD, c.dz, dd);
             T rn[V];
 #pragma unroll
             for (int i = 0; i < V; ++i) {
@@ -837,7 +838,7 @@ struct OpT2 {
                 rn[i] = (T)rr;
                 acc[0] += rr * rr;
                 acc[1] += (double)rn[i] * (double)rn[i];
-                if (l & LINK_VALID) { acc[2] += dd[i] * dd[i]; acc[3] += vc[i] * vc[i]; }
+                if (c.want_p && (l & LINK_VALID)) { acc[2] += dd[i] * dd[i]; acc[3] += vc[i] * vc[i]; }
             }
             st_chunk<T, V>(a.r + cell, rn);
         }
