@@ -33,7 +33,8 @@ typedef enum {
     OMNI_ERR_INVALID_ARG = -1,
     OMNI_ERR_CUDA = -2,        /* a CUDA runtime call failed (or no device)                                */
     OMNI_ERR_ALLOC = -3,       /* workspace allocation failed / caller workspace too small                 */
-    OMNI_ERR_BREAKDOWN = -4    /* non-finite scalar or p.Mp <= 0 seen on the device (M is not symmetric)   */
+    OMNI_ERR_BREAKDOWN = -4,   /* non-finite scalar or p.Mp <= 0 seen on the device (M is not symmetric)   */
+    OMNI_ERR_TOO_LARGE = -5    /* omni_source_noalloc_*: the grid exceeds the library's fixed scratch       */
 } omni_status;
 
 typedef struct {
@@ -330,6 +331,25 @@ int omni_source_f32(int nx, int ny, int nz, double dx, double dy, double dz,
                     const float* d_gx, const float* d_gy, const float* d_gz, const unsigned char* d_mask,
                     float* d_S_out, double* h_norm_S, void* stream);
 
+/* a1+a2 WITHOUT ANY ALLOCATION -- for callers that cannot call cudaMalloc (code under CUDA-graph stream capture, tight
+ *     serving loops, harnesses that forbid it).  Same S (last sum of Eq. 9 :100, 0 at missing cells; missing = outside
+ *     the box, mask == 0 or NaN in a used component, Eq. 13 :176) as omni_source_*, from ONE kernel that evaluates the
+ *     validity of a cell and its neighbours on the fly and writes straight to d_S_out; d_norm_S (DEVICE, one double, may
+ *     be NULL) receives ||S||_2.  The call enqueues one 64-byte memset and one kernel on `stream`, never synchronises,
+ *     and calls no cudaMalloc / cudaFree / pool or other allocating routine.  The only scratch (one reduction slot per
+ *     4096 cells, a ticket) is a fixed 256 KiB static __device__ array that every GPU loading the library holds until the
+ *     process exits; hence the limit nx*ny*nz <= omni_source_noalloc_max_cells() = 134 184 960 (500^3 fits): larger grids
+ *     return OMNI_ERR_TOO_LARGE with nothing enqueued.  ALL calls on a device share that array: two calls that overlap
+ *     on the GPU (different streams, or graph branches) race on it and give wrong norms -- serialise them; S itself does
+ *     not go through the scratch.  Other arguments and errors as omni_source_*. */
+int omni_source_noalloc_f64(int nx, int ny, int nz, double dx, double dy, double dz,
+                            const double* d_gx, const double* d_gy, const double* d_gz, const unsigned char* d_mask,
+                            double* d_S_out, double* d_norm_S, void* stream);
+int omni_source_noalloc_f32(int nx, int ny, int nz, double dx, double dy, double dz,
+                            const float* d_gx, const float* d_gy, const float* d_gz, const unsigned char* d_mask,
+                            float* d_S_out, double* d_norm_S, void* stream);
+long long omni_source_noalloc_max_cells(void);
+
 /* a1+a4  q = [W^{n+1}] p = M p with M = I - W1_off (Eq. 9 rearranged, A1), through the CG operator kernel
  *     (K4's recomputation path); validity from d_mask only (NULL = full box); q = 0 at missing cells; values of p at
  *     missing cells are ignored.  *h_pq (host, may be NULL) receives p.Mp over valid cells.  Synchronises. */
@@ -381,7 +401,7 @@ void omni_release_memory(void);
 int omni_profile_enable(int on);          /* returns the previous setting */
 void omni_profile_read(double* h_ms3, long long* h_count3, int reset);
 const char* omni_status_string(int status);
-int omni_version(void);                  /* 100 * major + minor; 101 added the _guess, _rans_source and history entry points, 102 omni_solve_pcg_*, 103 omni_solve_ex_* / omni_options, 104 omni_solve_slab_* */
+int omni_version(void);                  /* 100 * major + minor; 101 added the _guess, _rans_source and history entry points, 102 omni_solve_pcg_*, 103 omni_solve_ex_* / omni_options, 104 omni_solve_slab_*, 105 omni_source_noalloc_* */
 
 #ifdef __cplusplus
 }

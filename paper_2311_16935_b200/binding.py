@@ -14,11 +14,12 @@ _lib = None
 
 OMNI_OK, OMNI_NOT_CONVERGED = 0, 1
 STATUS_NAMES = {0: "OMNI_OK", 1: "OMNI_NOT_CONVERGED", -1: "OMNI_ERR_INVALID_ARG", -2: "OMNI_ERR_CUDA",
-                -3: "OMNI_ERR_ALLOC", -4: "OMNI_ERR_BREAKDOWN"}
+                -3: "OMNI_ERR_ALLOC", -4: "OMNI_ERR_BREAKDOWN", -5: "OMNI_ERR_TOO_LARGE"}
 # every symbol include/omni.h declares
 SYMBOLS = ["omni_solve_f64", "omni_solve_f32", "omni_workspace_bytes", "omni_solve_f64_ws", "omni_solve_f32_ws",
            "omni_solve_host_f64", "omni_solve_host_f32", "omni_solve_batch2d_f64", "omni_solve_batch2d_f32", "omni_solve_guess_f64", "omni_solve_guess_f32", "omni_solve_direct_f64", "omni_solve_direct_f32", "omni_solve_pcg_f64", "omni_solve_pcg_f32", "omni_solve_ex_f64", "omni_solve_ex_f32", "omni_options_init", "omni_slab_plan", "omni_slab_unique_id", "omni_slab_comm_create", "omni_slab_comm_destroy",
-           "omni_solve_slab_f64", "omni_solve_slab_f32", "omni_solve_direct_batch2d_f64", "omni_solve_direct_batch2d_f32", "omni_solve_cascade_f64", "omni_solve_cascade_f32", "omni_velocity_source_f64", "omni_velocity_source_f32", "omni_rans_source_f64", "omni_rans_source_f32",
+           "omni_solve_slab_f64", "omni_solve_slab_f32", "omni_source_noalloc_f64", "omni_source_noalloc_f32",
+           "omni_source_noalloc_max_cells", "omni_solve_direct_batch2d_f64", "omni_solve_direct_batch2d_f32", "omni_solve_cascade_f64", "omni_solve_cascade_f32", "omni_velocity_source_f64", "omni_velocity_source_f32", "omni_rans_source_f64", "omni_rans_source_f32",
            "omni_compressible_rans_source_f64", "omni_compressible_rans_source_f32", "omni_constants", "omni_source_f64", "omni_source_f32",
            "omni_apply_M_f64", "omni_apply_M_f32", "omni_residual_f64", "omni_residual_f32", "omni_launch_count",
            "omni_set_loop_mode", "omni_set_history", "omni_release_memory", "omni_profile_enable", "omni_profile_read", "omni_status_string", "omni_version"]
@@ -54,6 +55,7 @@ def lib():
         L = C.CDLL(path)
         L.omni_workspace_bytes.restype = C.c_size_t
         L.omni_launch_count.restype = C.c_longlong
+        L.omni_source_noalloc_max_cells.restype = C.c_longlong
         L.omni_status_string.restype = C.c_char_p
         _lib = L
     return _lib
@@ -497,6 +499,28 @@ def source(gx, gy, gz, mask, d):
     if rc < 0:
         raise OmniError(rc, f"omni_source_{sfx}")
     return S, nrm.value
+
+
+def source_noalloc(gx, gy, gz, mask, d, out, norm_out=None):
+    """omni_source_noalloc_*: S of Eq. 9 into the caller's `out` (and ||S|| into the one-element CUDA float64 tensor
+    `norm_out`) with no allocation anywhere: the caller passes every output, the library's only scratch is its fixed
+    static device array.  Asynchronous.  Returns `out`."""
+    import torch
+    sfx = _suffix(gx)
+    _check([gx, gy, gz, mask, out, norm_out], "cuda")
+    _check_like(gx, [("gy", gy), ("gz", gz), ("out", out)], mask)
+    if norm_out is not None and (norm_out.dtype != torch.float64 or norm_out.numel() != 1):
+        raise TypeError("norm_out must be one float64")
+    with torch.cuda.device(gx.device):
+        rc = getattr(lib(), f"omni_source_noalloc_{sfx}")(*_geom(gx, d), _ptr(gx), _ptr(gy), _ptr(gz), _ptr(mask), _ptr(out),
+                                                          _ptr(norm_out), _stream(gx.device))
+    if rc < 0:
+        raise OmniError(rc, f"omni_source_noalloc_{sfx}")
+    return out
+
+
+def source_noalloc_max_cells():
+    return int(lib().omni_source_noalloc_max_cells())
 
 
 def apply_M(p, mask, d):

@@ -7,6 +7,7 @@
 #include "omni_loop.cuh"
 #include "omni_mg.cuh"
 #include "omni_slab.cuh"
+#include "omni_noalloc.cuh"
 #include "../../include/omni.h"
 
 #include <algorithm>
@@ -19,6 +20,11 @@
 #include <type_traits>
 
 using namespace omni;
+
+// Scratch of omni_source_noalloc_* (omni_noalloc.cuh): a fixed array in every GPU that loads the library, held until the
+// process exits.  In HOST code this name is only a stand-in for the symbol, never a device address: the address is
+// fetched per device with cudaGetSymbolAddress (noalloc_scratch_ptr below) and passed to the kernel.
+static __device__ __align__(256) unsigned char g_noalloc_scratch[omni::NOALLOC_SCRATCH_BYTES];
 
 // tile shape and pipeline depths of K2 / K3 / K4 (each can be overridden at build time for sweeps)
 #ifndef OMNI_BY
@@ -1995,6 +2001,68 @@ int omni_solve_slab_f32(int nx, int ny, int nz, double dx, double dy, double dz,
                              method == OMNI_METHOD_DIRECT, nranks, comm, stream, info);
 }
 
+extern "C++" {
+namespace {
+// device address of g_noalloc_scratch on the CURRENT device, looked up once per device with that device current
+int noalloc_scratch_ptr(double** out)
+{
+    static std::mutex mu;
+    static double* cache[MAX_DEVICES] = {};
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) { cudaGetLastError(); return OMNI_ERR_CUDA; }
+    std::lock_guard<std::mutex> lk(mu);
+    if (dev >= 0 && dev < MAX_DEVICES && cache[dev]) { *out = cache[dev]; return OMNI_OK; }
+    void* p = nullptr;
+    if (cudaGetSymbolAddress(&p, g_noalloc_scratch) != cudaSuccess || p == nullptr) { cudaGetLastError(); return OMNI_ERR_CUDA; }
+    if (dev >= 0 && dev < MAX_DEVICES) cache[dev] = (double*)p;
+    *out = (double*)p;
+    return OMNI_OK;
+}
+
+template <typename T>
+int source_noalloc(int nx, int ny, int nz, double dx, double dy, double dz, const T* gx, const T* gy, const T* gz,
+                   const unsigned char* mask, T* S_out, double* d_norm_S, void* stream)
+{
+    if (!valid_common(nx, ny, nz, dx, dy, dz, 0.0, 0, 0)) return OMNI_ERR_INVALID_ARG;
+    if (!gx || !gy || (nz > 1 && !gz) || !S_out) return OMNI_ERR_INVALID_ARG;
+    const long long n = (long long)nx * ny * nz;
+    if (n > NOALLOC_MAX_CELLS) return OMNI_ERR_TOO_LARGE;          // one reduction slot per 4096 cells, 32 760 slots
+    const int naxes = nz > 1 ? 3 : 2;
+    HostConst H;
+    host_constants(naxes, dx, dy, dz, H);
+    const double d[3] = { dx, dy, dz };
+    T hs[3];
+    for (int a = 0; a < 3; ++a) hs[a] = (T)(a < naxes ? d[a] * (H.F[a] / H.Atot) * 0.5 : 0.0);      // as make_coef: Coef::hs
+    double* scratch = nullptr;
+    const int rc = noalloc_scratch_ptr(&scratch);
+    if (rc != OMNI_OK) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    // the array keeps the last call's contents: the ticket must start at zero (an aborted call may have left it set)
+    CK(cudaMemsetAsync(scratch, 0, NOALLOC_HEADER_DOUBLES * sizeof(double), st));
+    const unsigned nb = (unsigned)((n + NOALLOC_CELLS_PER_CTA - 1) / NOALLOC_CELLS_PER_CTA);
+    source_noalloc_kernel<T><<<nb, NOALLOC_THREADS, 0, st>>>(nx, ny, nz, naxes, gx, gy, gz, mask, hs[0], hs[1], hs[2], S_out, scratch,
+                                                             d_norm_S);
+    g_launches.fetch_add(1, std::memory_order_relaxed);
+    CK(cudaGetLastError());
+    return OMNI_OK;
+}
+}  // namespace
+}  // extern "C++"
+
+int omni_source_noalloc_f64(int nx, int ny, int nz, double dx, double dy, double dz, const double* d_gx, const double* d_gy,
+                            const double* d_gz, const unsigned char* d_mask, double* d_S_out, double* d_norm_S, void* stream)
+{
+    return source_noalloc<double>(nx, ny, nz, dx, dy, dz, d_gx, d_gy, d_gz, d_mask, d_S_out, d_norm_S, stream);
+}
+
+int omni_source_noalloc_f32(int nx, int ny, int nz, double dx, double dy, double dz, const float* d_gx, const float* d_gy,
+                            const float* d_gz, const unsigned char* d_mask, float* d_S_out, double* d_norm_S, void* stream)
+{
+    return source_noalloc<float>(nx, ny, nz, dx, dy, dz, d_gx, d_gy, d_gz, d_mask, d_S_out, d_norm_S, stream);
+}
+
+long long omni_source_noalloc_max_cells(void) { return NOALLOC_MAX_CELLS; }
+
 int omni_constants(int nx, int ny, int nz, double dx, double dy, double dz, double* h_out13)
 {
     if (!h_out13 || !valid_common(nx, ny, nz, dx, dy, dz, 0.0, 0, 0)) return OMNI_ERR_INVALID_ARG;
@@ -2116,10 +2184,11 @@ const char* omni_status_string(int status)
     case OMNI_ERR_CUDA: return "CUDA runtime error (or no CUDA device)";
     case OMNI_ERR_ALLOC: return "workspace allocation failed or workspace too small";
     case OMNI_ERR_BREAKDOWN: return "CG breakdown: non-finite scalar or p.Mp <= 0";
+    case OMNI_ERR_TOO_LARGE: return "grid exceeds the fixed scratch of the no-allocation entry point (omni_source_noalloc_max_cells)";
     default: return "unknown status";
     }
 }
 
-int omni_version(void) { return 104; }   // 101: omni_solve_guess_*, omni_set_history, omni_rans_source_*, omni_compressible_rans_source_*
+int omni_version(void) { return 105; }   // 101: omni_solve_guess_*, omni_set_history, omni_rans_source_*, omni_compressible_rans_source_*
 
 }  // extern "C"
