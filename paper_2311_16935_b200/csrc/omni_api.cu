@@ -831,7 +831,8 @@ int mg_build(const Geom& g, const Workspace<T>& w, const HostConst& H, MgHier<T>
         if (m == 0) break;
         MgLevel<T> C = {};
         C.nx = F.hx ? (F.nx + 1) / 2 : F.nx; C.ny = F.hy ? (F.ny + 1) / 2 : F.ny; C.nz = F.hz ? (F.nz + 1) / 2 : F.nz;
-        C.px = C.nx; C.pplane = (long long)C.px * C.ny; C.n = C.pplane * C.nz;
+        C.px = (C.nx + 3) / 4 * 4;            // rows padded to whole 4-cell chunks (pad cells: link 0, values 0)
+        C.pplane = (long long)C.px * C.ny; C.n = C.pplane * C.nz;
         const int h[3] = { F.hx, F.hy, F.hz };
         for (int a = 0; a < 3; ++a) {
             wd[a] = wd[a] * (double)(1 << m) * (h[a] ? 0.25 : 1.0);
@@ -858,9 +859,8 @@ int mg_build(const Geom& g, const Workspace<T>& w, const HostConst& H, MgHier<T>
     }
     uint8_t* vc = (uint8_t*)(base + o_vc);
     for (int l = 1; l < M.nlev; ++l) {
-        const unsigned nb = blocks_for(M.L[l].n, 256);
-        mg_coarse_valid_kernel<T><<<nb, 256, 0, st>>>(M.L[l - 1], M.L[l], vc);
-        mg_link_kernel<T><<<nb, 256, 0, st>>>(M.L[l], vc, (uint8_t*)(base + o_link[l]), g.naxes);
+        mg_coarse_valid_kernel<T><<<mg_grid(M.L[l]), mg_block(), 0, st>>>(M.L[l - 1], M.L[l], vc);
+        mg_link_kernel<T><<<mg_grid(M.L[l]), mg_block(), 0, st>>>(M.L[l], vc, (uint8_t*)(base + o_link[l]), g.naxes);
         g_launches.fetch_add(2, std::memory_order_relaxed);
     }
     CK(cudaGetLastError());
@@ -873,23 +873,31 @@ T* mg_vcycle(MgHier<T>& M, int l, cudaStream_t st)
 {
     const MgLevel<T>& L = M.L[l];
     const bool last = (l + 1 == M.nlev);
-    const unsigned nb = blocks_for(L.n, 256);
+    const dim3 nt = mg_block();
+    dim3 nb = mg_grid(L);
+    nb.x = (unsigned)((L.px / 4 + MG_BX - 1) / MG_BX);               // four cells of a row per thread
     T *cur = L.x, *oth = L.xt;
-    mg_jacobi_kernel<T, true><<<nb, 256, 0, st>>>(L, nullptr, cur);
+    mg_jacobi4_kernel<T, true><<<nb, nt, 0, st>>>(L, nullptr, cur);
     M.launches_per_cycle += 1;
     for (int sw = 1; sw < (last ? MG_NU_COARSEST : MG_NU); ++sw) {
-        mg_jacobi_kernel<T, false><<<nb, 256, 0, st>>>(L, cur, oth);
+        mg_jacobi4_kernel<T, false><<<nb, nt, 0, st>>>(L, cur, oth);
         std::swap(cur, oth);
         M.launches_per_cycle += 1;
     }
     if (last) return cur;
     const MgLevel<T>& C = M.L[l + 1];
-    mg_residual_restrict_kernel<T><<<blocks_for(C.n, 256), 256, 0, st>>>(L, C, cur);
+    if (L.hx) {                                                      // x halved: two coarse cells (one fine chunk) per thread
+        dim3 nc = mg_grid(C);
+        nc.x = (unsigned)((C.px / 2 + MG_BX - 1) / MG_BX);
+        mg_residual_restrict4_kernel<T><<<nc, nt, 0, st>>>(L, C, cur);
+    } else {
+        mg_residual_restrict_kernel<T><<<mg_grid(C), nt, 0, st>>>(L, C, cur);
+    }
     T* e = mg_vcycle<T>(M, l + 1, st);
-    mg_prolong_add_kernel<T><<<nb, 256, 0, st>>>(L, C, cur, e);
+    mg_prolong_add4_kernel<T><<<nb, nt, 0, st>>>(L, C, cur, e);
     M.launches_per_cycle += 2;
     for (int sw = 0; sw < MG_NU; ++sw) {
-        mg_jacobi_kernel<T, false><<<nb, 256, 0, st>>>(L, cur, oth);
+        mg_jacobi4_kernel<T, false><<<nb, nt, 0, st>>>(L, cur, oth);
         std::swap(cur, oth);
         M.launches_per_cycle += 1;
     }
@@ -2140,6 +2148,37 @@ int omni_debug_cta_trace(int which, unsigned long long* h_out, int n_ctas)
 #endif
 
 #ifdef OMNI_TUNING
+// tuning builds only: `reps` V-cycles of the multigrid preconditioner on b = S, launched one by one on the stream (outside
+// any graph, so that a profiler sees the level kernels by name)
+int omni_debug_vcycle_f32(int nx, int ny, int nz, double dx, double dy, double dz, const float* gx, const float* gy,
+                          const float* gz, const unsigned char* mask, int reps, void* stream)
+{
+    Geom g;
+    if (!make_geom(nx, ny, nz, 4, g)) return OMNI_ERR_INVALID_ARG;
+    cudaStream_t st = (cudaStream_t)stream;
+    const size_t bytes = carve<float>(g, nullptr, nullptr);
+    void* ws = nullptr;
+    if (pool_alloc(&ws, bytes, st) != cudaSuccess) return OMNI_ERR_ALLOC;
+    Workspace<float> w;
+    carve<float>(g, (char*)ws, &w);
+    HostConst H;
+    host_constants(g.naxes, dx, dy, dz, H);
+    const Coef<float> K = make_coef<float>(H, dx, dy, dz, g);
+    init_scalars_kernel<<<1, 1, 0, st>>>(w.sc, 1e-5, 1, 1);
+    int rc = setup_codes<float>(g, w, gx, gy, gz, mask, st);
+    if (rc == OMNI_OK) rc = launch_source<float>(g, w, K, gx, gy, gz, st);
+    MgHier<float> M;
+    if (rc == OMNI_OK) rc = mg_build<float>(g, w, H, M, st);
+    if (rc == OMNI_OK) {
+        cudaMemcpyAsync(w.r, w.S, (size_t)g.npad * 4, cudaMemcpyDeviceToDevice, st);
+        for (int i = 0; i < reps; ++i) mg_vcycle<float>(M, 0, st);
+        cudaFreeAsync(M.mem, st);
+    }
+    cudaStreamSynchronize(st);
+    cudaFreeAsync(ws, st);
+    return cudaGetLastError() == cudaSuccess ? rc : OMNI_ERR_CUDA;
+}
+
 // tuning builds only: per-CTA timeline of the loop kernel's first phases: h_out[phase][cta][3], returns the phase count
 int omni_debug_loop_trace(unsigned long long* h_out, int max_phases)
 {

@@ -9,7 +9,8 @@
 //   transfer  restriction = sum over the children, prolongation = the parent's value (transposes of each other)
 //   smoother  damped Jacobi x <- x + omega D^-1 (b - L x), omega = 0.8; 2 sweeps before and after the coarse-grid
 //             correction (the first from x = 0), 8 on the coarsest level
-// One thread per cell (per coarse cell in the restriction, which gathers its children in a fixed order: deterministic).
+// One thread per cell (per coarse cell in the restriction, which gathers its children in a fixed order: deterministic),
+// cell indices from a 3D launch (no integer division).
 // Bandwidth-bound elementwise / 7-point kernels on plain coalesced loads; neighbours come from L1 / L2.
 #pragma once
 #include "omni_kernels.cuh"
@@ -31,15 +32,25 @@ struct MgLevel {
     T *x, *xt, *b;               // iterate, second Jacobi buffer, right-hand side
 };
 
+// Launch shape of every level kernel: blocks of MG_BX x MG_BY threads over (x, y), one plane per blockIdx.z -- a
+// thread's cell comes from its indices, with no integer division (a linear index split by 64-bit / and % costs more than
+// the 7-point stencil itself and kept these kernels at a third of the memory roofline).
+constexpr int MG_BX = 64, MG_BY = 4;
 template <typename T>
-__device__ __forceinline__ bool mg_cell(const MgLevel<T>& L, long long c, int& i, int& j, int& k)
+inline dim3 mg_grid(const MgLevel<T>& L) { return dim3((unsigned)((L.px + MG_BX - 1) / MG_BX), (unsigned)((L.ny + MG_BY - 1) / MG_BY), (unsigned)L.nz); }
+inline dim3 mg_block() { return dim3(MG_BX, MG_BY, 1); }
+
+// the thread's cell (i, j, k) and linear index c in level L; false outside the array (i >= px or j >= ny);
+// cells with nx <= i < px are the pad cells of level 0
+template <typename T>
+__device__ __forceinline__ bool mg_cell(const MgLevel<T>& L, int& i, int& j, int& k, long long& c)
 {
-    if (c >= L.n) return false;
-    i = (int)(c % L.px);
-    const long long row = c / L.px;
-    j = (int)(row % L.ny);
-    k = (int)(row / L.ny);
-    return i < L.nx;
+    i = blockIdx.x * MG_BX + threadIdx.x;
+    j = blockIdx.y * MG_BY + threadIdx.y;
+    k = blockIdx.z;
+    if (i >= L.px || j >= L.ny) return false;
+    c = i + (long long)L.px * (j + (long long)L.ny * k);
+    return true;
 }
 
 // (D, L x) at cell c from its link byte
@@ -71,13 +82,13 @@ __device__ __forceinline__ T mg_diag(const MgLevel<T>& L, uint32_t l)
 
 // FIRST: xout = omega D^-1 b (a sweep from x = 0); else xout = xin + omega D^-1 (b - L xin).  0 at missing cells.
 template <typename T, bool FIRST>
-__global__ void __launch_bounds__(256)
+__global__ void __launch_bounds__(MG_BX * MG_BY)
 mg_jacobi_kernel(const MgLevel<T> L, const T* __restrict__ xin, T* __restrict__ xout)
 {
-    const long long c = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    long long c;
     int i, j, k;
-    if (c >= L.n) return;
-    if (!mg_cell(L, c, i, j, k)) { xout[c] = T(0); return; }
+    if (!mg_cell(L, i, j, k, c)) return;
+    if (i >= L.nx) { xout[c] = T(0); return; }
     const uint32_t l = L.link[c];
     T v = T(0);
     if (l & LINK_VALID) {
@@ -94,15 +105,140 @@ mg_jacobi_kernel(const MgLevel<T> L, const T* __restrict__ xin, T* __restrict__ 
     xout[c] = v;
 }
 
+// ---- the same sweep, four cells of a row per thread (rows are padded to a multiple of 4 cells on every level): 16 /
+// 32-byte loads, every neighbour load issued unconditionally (by position, not by link bit) so that a thread has ~10
+// independent loads in flight instead of a link -> neighbour chain; one cell per thread leaves the memory system at a
+// third of its bandwidth.  Link bits select the weights: a missing link contributes w = 0.
+template <typename T, bool FIRST>
+__global__ void __launch_bounds__(MG_BX * MG_BY)
+mg_jacobi4_kernel(const MgLevel<T> L, const T* __restrict__ xin, T* __restrict__ xout)
+{
+    const int i0 = (blockIdx.x * MG_BX + threadIdx.x) * 4, j = blockIdx.y * MG_BY + threadIdx.y, k = blockIdx.z;
+    if (i0 >= L.px || j >= L.ny) return;
+    const long long c = i0 + (long long)L.px * (j + (long long)L.ny * k);
+    const uint32_t lw = *reinterpret_cast<const uint32_t*>(L.link + c);
+    T b[4], v[4];
+    ld_chunk<T, 4>(L.b + c, b);
+    if (FIRST) {
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            const uint32_t l = (lw >> (8 * q)) & 0xffu;
+            const T D = mg_diag(L, l);
+            v[q] = ((l & LINK_VALID) && D > T(0)) ? (T)MG_OMEGA * (b[q] / D) : T(0);
+        }
+    } else {
+        T xc[4], xn[4], xs[4], xf[4], xb[4];
+        ld_chunk<T, 4>(xin + c, xc);
+        zero_chunk<T, 4>(xn); zero_chunk<T, 4>(xs); zero_chunk<T, 4>(xf); zero_chunk<T, 4>(xb);
+        if (j + 1 < L.ny) ld_chunk<T, 4>(xin + c + L.px, xn);
+        if (j > 0) ld_chunk<T, 4>(xin + c - L.px, xs);
+        if (k + 1 < L.nz) ld_chunk<T, 4>(xin + c + L.pplane, xf);
+        if (k > 0) ld_chunk<T, 4>(xin + c - L.pplane, xb);
+        const T xl = (i0 > 0) ? xin[c - 1] : T(0), xr = (i0 + 4 < L.px) ? xin[c + 4] : T(0);
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            const uint32_t l = (lw >> (8 * q)) & 0xffu;
+            const T e = (q == 3) ? xr : xc[q < 3 ? q + 1 : 3], w = (q == 0) ? xl : xc[q > 0 ? q - 1 : 0];
+            // same terms in the same order as mg_stencil; an absent link has weight 0
+            const T w0 = (l & 1u) ? L.w[0] : T(0), w1 = (l & 2u) ? L.w[0] : T(0), w2 = (l & 4u) ? L.w[1] : T(0);
+            const T w3 = (l & 8u) ? L.w[1] : T(0), w4 = (l & 16u) ? L.w[2] : T(0), w5 = (l & 32u) ? L.w[2] : T(0);
+            T D = T(0), Lx = T(0);
+            D += w0; Lx += w0 * (xc[q] - e);
+            D += w1; Lx += w1 * (xc[q] - w);
+            D += w2; Lx += w2 * (xc[q] - xn[q]);
+            D += w3; Lx += w3 * (xc[q] - xs[q]);
+            D += w4; Lx += w4 * (xc[q] - xf[q]);
+            D += w5; Lx += w5 * (xc[q] - xb[q]);
+            T r = T(0);
+            if (l & LINK_VALID) {
+                r = xc[q];
+                if (D > T(0)) r += (T)MG_OMEGA * ((b[q] - Lx) / D);
+            }
+            v[q] = r;
+        }
+    }
+    st_chunk<T, 4>(xout + c, v);
+}
+
+// coarse right-hand side with the x axis halved, two coarse cells = one 4-cell fine chunk per child row and thread;
+// children are added in the same (plane, row, cell) order as in mg_residual_restrict_kernel
+template <typename T>
+__global__ void __launch_bounds__(MG_BX * MG_BY)
+mg_residual_restrict4_kernel(const MgLevel<T> F, const MgLevel<T> C, const T* __restrict__ x)
+{
+    const int ci0 = (blockIdx.x * MG_BX + threadIdx.x) * 2, cj = blockIdx.y * MG_BY + threadIdx.y, ck = blockIdx.z;
+    if (ci0 >= C.px || cj >= C.ny) return;
+    const long long I = ci0 + (long long)C.px * (cj + (long long)C.ny * ck);
+    const int i0 = 2 * ci0;
+    T s[2] = { T(0), T(0) };
+    if (i0 < F.px) {
+        for (int dk = 0; dk <= F.hz; ++dk)
+            for (int dj = 0; dj <= F.hy; ++dj) {
+                const int j = (F.hy ? 2 * cj : cj) + dj, k = (F.hz ? 2 * ck : ck) + dk;
+                if (j >= F.ny || k >= F.nz) continue;
+                const long long c = i0 + (long long)F.px * (j + (long long)F.ny * k);
+                const uint32_t lw = *reinterpret_cast<const uint32_t*>(F.link + c);
+                if (!(lw & 0x40404040u)) continue;
+                T b[4], xc[4], xn[4], xs[4], xf[4], xb[4];
+                ld_chunk<T, 4>(F.b + c, b);
+                ld_chunk<T, 4>(x + c, xc);
+                zero_chunk<T, 4>(xn); zero_chunk<T, 4>(xs); zero_chunk<T, 4>(xf); zero_chunk<T, 4>(xb);
+                if (j + 1 < F.ny) ld_chunk<T, 4>(x + c + F.px, xn);
+                if (j > 0) ld_chunk<T, 4>(x + c - F.px, xs);
+                if (k + 1 < F.nz) ld_chunk<T, 4>(x + c + F.pplane, xf);
+                if (k > 0) ld_chunk<T, 4>(x + c - F.pplane, xb);
+                const T xl = (i0 > 0) ? x[c - 1] : T(0), xr = (i0 + 4 < F.px) ? x[c + 4] : T(0);
+#pragma unroll
+                for (int q = 0; q < 4; ++q) {
+                    const uint32_t l = (lw >> (8 * q)) & 0xffu;
+                    if (!(l & LINK_VALID)) continue;
+                    const T e = (q == 3) ? xr : xc[q < 3 ? q + 1 : 3], w = (q == 0) ? xl : xc[q > 0 ? q - 1 : 0];
+                    T Lx = T(0);
+                    if (l & 1u) Lx += F.w[0] * (xc[q] - e);
+                    if (l & 2u) Lx += F.w[0] * (xc[q] - w);
+                    if (l & 4u) Lx += F.w[1] * (xc[q] - xn[q]);
+                    if (l & 8u) Lx += F.w[1] * (xc[q] - xs[q]);
+                    if (l & 16u) Lx += F.w[2] * (xc[q] - xf[q]);
+                    if (l & 32u) Lx += F.w[2] * (xc[q] - xb[q]);
+                    s[q >> 1] += b[q] - Lx;
+                }
+            }
+    }
+    C.b[I] = (ci0 < C.nx) ? s[0] : T(0);
+    C.b[I + 1] = (ci0 + 1 < C.nx) ? s[1] : T(0);
+}
+
+// x += prolong(e), four fine cells per thread
+template <typename T>
+__global__ void __launch_bounds__(MG_BX * MG_BY)
+mg_prolong_add4_kernel(const MgLevel<T> F, const MgLevel<T> C, T* __restrict__ x, const T* __restrict__ e)
+{
+    const int i0 = (blockIdx.x * MG_BX + threadIdx.x) * 4, j = blockIdx.y * MG_BY + threadIdx.y, k = blockIdx.z;
+    if (i0 >= F.px || j >= F.ny) return;
+    const long long c = i0 + (long long)F.px * (j + (long long)F.ny * k);
+    const uint32_t lw = *reinterpret_cast<const uint32_t*>(F.link + c);
+    if (!(lw & 0x40404040u)) return;                              // no valid cell in the chunk
+    const long long I = (F.hx ? i0 >> 1 : i0) + (long long)C.px * ((F.hy ? j >> 1 : j) + (long long)C.ny * (F.hz ? k >> 1 : k));
+    T v[4];
+    ld_chunk<T, 4>(x + c, v);
+#pragma unroll
+    for (int q = 0; q < 4; ++q)
+        if ((lw >> (8 * q)) & LINK_VALID) {
+            const int ci = F.hx ? (q >> 1) : q;                   // parent of fine cell i0 + q relative to I
+            if ((F.hx ? ((i0 + q) >> 1) : (i0 + q)) < C.nx) v[q] += e[I + ci];
+        }
+    st_chunk<T, 4>(x + c, v);
+}
+
 // coarse right-hand side: b_c[I] = sum over the valid children C of I of (b - L x)_C, children in a fixed order
 template <typename T>
-__global__ void __launch_bounds__(256)
+__global__ void __launch_bounds__(MG_BX * MG_BY)
 mg_residual_restrict_kernel(const MgLevel<T> F, const MgLevel<T> C, const T* __restrict__ x)
 {
-    const long long I = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    long long I;
     int ci, cj, ck;
-    if (I >= C.n) return;
-    if (!mg_cell(C, I, ci, cj, ck)) { C.b[I] = T(0); return; }
+    if (!mg_cell(C, ci, cj, ck, I)) return;
+    if (ci >= C.nx) { C.b[I] = T(0); return; }
     T s = T(0);
     for (int dk = 0; dk <= F.hz; ++dk)
         for (int dj = 0; dj <= F.hy; ++dj)
@@ -121,12 +257,12 @@ mg_residual_restrict_kernel(const MgLevel<T> F, const MgLevel<T> C, const T* __r
 
 // x += prolong(e): every valid fine cell receives its parent's value
 template <typename T>
-__global__ void __launch_bounds__(256)
+__global__ void __launch_bounds__(MG_BX * MG_BY)
 mg_prolong_add_kernel(const MgLevel<T> F, const MgLevel<T> C, T* __restrict__ x, const T* __restrict__ e)
 {
-    const long long c = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    long long c;
     int i, j, k;
-    if (!mg_cell(F, c, i, j, k)) return;
+    if (!mg_cell(F, i, j, k, c) || i >= F.nx) return;
     if (!(F.link[c] & LINK_VALID)) return;
     const long long I = (F.hx ? i >> 1 : i) + (long long)C.px * ((F.hy ? j >> 1 : j) + (long long)C.ny * (F.hz ? k >> 1 : k));
     x[c] += e[I];
@@ -134,14 +270,14 @@ mg_prolong_add_kernel(const MgLevel<T> F, const MgLevel<T> C, T* __restrict__ x,
 
 // validity of the next level: a coarse cell is valid iff one of its children is
 template <typename T>
-__global__ void __launch_bounds__(256)
+__global__ void __launch_bounds__(MG_BX * MG_BY)
 mg_coarse_valid_kernel(const MgLevel<T> F, const MgLevel<T> C, uint8_t* __restrict__ vc)
 {
-    const long long I = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    long long I;
     int ci, cj, ck;
-    if (I >= C.n) return;
+    if (!mg_cell(C, ci, cj, ck, I)) return;
     uint8_t any = 0;
-    if (mg_cell(C, I, ci, cj, ck))
+    if (ci < C.nx)
         for (int dk = 0; dk <= F.hz; ++dk)
             for (int dj = 0; dj <= F.hy; ++dj)
                 for (int di = 0; di <= F.hx; ++di) {
@@ -154,14 +290,14 @@ mg_coarse_valid_kernel(const MgLevel<T> F, const MgLevel<T> C, uint8_t* __restri
 
 // link bytes of a level from its validity bytes (naxes = 2: no F / B links)
 template <typename T>
-__global__ void __launch_bounds__(256)
+__global__ void __launch_bounds__(MG_BX * MG_BY)
 mg_link_kernel(const MgLevel<T> C, const uint8_t* __restrict__ vc, uint8_t* __restrict__ link, int naxes)
 {
-    const long long I = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    long long I;
     int i, j, k;
-    if (I >= C.n) return;
+    if (!mg_cell(C, i, j, k, I)) return;
     uint32_t l = 0;
-    if (mg_cell(C, I, i, j, k) && vc[I]) {
+    if (i < C.nx && vc[I]) {
         l = LINK_VALID;
         if (i + 1 < C.nx && vc[I + 1]) l |= 1u;
         if (i > 0 && vc[I - 1]) l |= 2u;
