@@ -528,12 +528,28 @@ inline unsigned blocks_for(long long n, int bs) { return (unsigned)((n + bs - 1)
 
 // ------------------------------------------------------------------------------------------------ setup shared by all entry points
 
+// the caller's rows are whole 16-byte chunks of 4 cells: nx % 4 == 0, every given array 16-byte aligned (mask: 4-byte)
+template <typename A, typename B, typename Cc>
+bool rows_are_chunks(const Geom& g, const A* a, const B* b, const Cc* c, const unsigned char* mask)
+{
+    if (g.nx % 4 != 0 || g.nz > 65535 || (g.ny + SETUP_BY - 1) / SETUP_BY > 65535) return false;
+    const uintptr_t bits = (uintptr_t)a | (uintptr_t)b | (uintptr_t)c;
+    return (bits & 15) == 0 && ((uintptr_t)mask & 3) == 0;
+}
+inline dim3 setup_grid(const Geom& g)
+{
+    return dim3((unsigned)((g.px / 4 + SETUP_BX - 1) / SETUP_BX), (unsigned)((g.ny + SETUP_BY - 1) / SETUP_BY), (unsigned)g.nz);
+}
+
 template <typename T>
 int setup_codes(const Geom& g, const Workspace<T>& w, const T* gx, const T* gy, const T* gz, const uint8_t* mask,
                 cudaStream_t st)
 {
     uint8_t* vbyte = reinterpret_cast<uint8_t*>(w.p0);       // scratch: p0 is cleared afterwards
-    validity_kernel<T><<<blocks_for(g.npad, 256), 256, 0, st>>>(g, gx, gy, gz, mask, vbyte);
+    if (rows_are_chunks(g, gx, gy, gz, mask))
+        validity4_kernel<T><<<setup_grid(g), dim3(SETUP_BX, SETUP_BY), 0, st>>>(g, gx, gy, gz, mask, vbyte);
+    else
+        validity_kernel<T><<<blocks_for(g.npad, 256), 256, 0, st>>>(g, gx, gy, gz, mask, vbyte);
     CK(cudaGetLastError());
     CK(cudaMemsetAsync(w.tflags, 0, (size_t)g.ntx * g.nty * g.twords * 4, st));
     // work list of the groups that need the cell-by-cell decode: scratch in p1 (4 bytes per 4-cell group at most),
@@ -568,7 +584,13 @@ int launch_source(const Geom& g, const Workspace<T>& w, const Coef<T>& K, const 
 {
     unsigned nb = blocks_for(g.npad, 256);
     if (nb > 4736u) nb = 4736u;                 // 148 SMs x 8 CTAs x 4: the kernel is grid-stride
-    source_kernel<T><<<nb, 256, 0, st>>>(g, gx, gy, gz, w.link, K, w.S, w.sc, w.partial);
+    if (rows_are_chunks(g, gx, gy, gz, (const unsigned char*)nullptr)) {
+        const long long items = (long long)((g.ny + SETUP_BY - 1) / SETUP_BY) * g.nz;
+        if (items < (long long)nb) nb = (unsigned)items;
+        source4_kernel<T><<<nb, dim3(SETUP_BX, SETUP_BY), 0, st>>>(g, gx, gy, gz, w.link, K, w.S, w.sc, w.partial);
+    } else {
+        source_kernel<T><<<nb, 256, 0, st>>>(g, gx, gy, gz, w.link, K, w.S, w.sc, w.partial);
+    }
     g_launches.fetch_add(1, std::memory_order_relaxed);
     CK(cudaGetLastError());
     return OMNI_OK;
@@ -1194,7 +1216,10 @@ int solve_ws(int nx, int ny, int nz, double dx, double dy, double dz, const T* g
     else if (mode == 2) rc = lop ? run_loop_graph<T, true>(g, w, H, K, st) : run_loop_graph<T, false>(g, w, H, K, st);
     if (rc != OMNI_OK) return rc;
 
-    finalize_kernel<T><<<blocks_for((long long)nx * ny * nz, 256), 256, 0, st>>>(g, w.P, w.P1, w.sc, w.link, P_out, opt.P64);
+    if (rows_are_chunks(g, P_out, opt.P64, (const T*)nullptr, (const unsigned char*)nullptr))
+        finalize4_kernel<T><<<setup_grid(g), dim3(SETUP_BX, SETUP_BY), 0, st>>>(g, w.P, w.P1, w.sc, w.link, P_out, opt.P64);
+    else
+        finalize_kernel<T><<<blocks_for((long long)nx * ny * nz, 256), 256, 0, st>>>(g, w.P, w.P1, w.sc, w.link, P_out, opt.P64);
     CK(cudaGetLastError());
     g_launches.fetch_add(1, std::memory_order_relaxed);
 

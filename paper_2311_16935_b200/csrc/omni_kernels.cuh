@@ -695,6 +695,156 @@ __global__ void finalize_kernel(Geom g, const double* P0, const double* P1, cons
     if (out64 != nullptr) out64[u] = ok ? P[pid] : nan("");      // the fp64 master pressure itself (omni_options::d_P64_out)
 }
 
+// ------------------------------------------------------------------------------------------------ K0a / K1 / K7, four cells per thread
+// The one-cell-per-thread kernels above leave the memory system at 30-40 % of its bandwidth (few bytes in flight per
+// thread, an index division per cell, neighbour loads that wait for the link byte).  When the caller's rows are whole
+// 16-byte chunks (nx % 4 == 0, 16-byte aligned arrays) these variants take one 4-cell chunk per thread: vector loads,
+// (x, y, plane) from the launch indices, neighbour chunks loaded by POSITION before the link bits select the terms.
+// Same arithmetic per cell, same order.
+constexpr int SETUP_BX = 64, SETUP_BY = 4;
+
+template <typename T>
+__global__ void __launch_bounds__(SETUP_BX * SETUP_BY)
+validity4_kernel(Geom g, const T* __restrict__ gx, const T* __restrict__ gy, const T* __restrict__ gz,
+                 const uint8_t* __restrict__ mask, uint8_t* __restrict__ vbyte)
+{
+    const int i0 = (blockIdx.x * SETUP_BX + threadIdx.x) * 4, j = blockIdx.y * SETUP_BY + threadIdx.y, k = blockIdx.z;
+    if (i0 >= g.px || j >= g.ny) return;
+    const long long pid = i0 + (long long)g.px * (j + (long long)g.ny * k);
+    uint32_t ok = 0;
+    if (i0 < g.nx) {
+        const long long u = i0 + (long long)g.nx * (j + (long long)g.ny * k);
+        uint32_t m = 0x01010101u;
+        if (mask != nullptr) m = *reinterpret_cast<const uint32_t*>(mask + (g.batch ? i0 + (long long)g.nx * j : u));
+        T a[4], b[4], c[4];
+        zero_chunk<T, 4>(a); zero_chunk<T, 4>(b); zero_chunk<T, 4>(c);
+        if (gx != nullptr) {
+            ld_chunk<T, 4>(gx + u, a);
+            ld_chunk<T, 4>(gy + u, b);
+            if (g.naxes == 3) ld_chunk<T, 4>(gz + u, c);
+        }
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            uint32_t v = ((m >> (8 * q)) & 0xffu) != 0;
+            if (isnan(a[q]) || isnan(b[q]) || isnan(c[q])) v = 0;
+            ok |= v << (8 * q);
+        }
+    }
+    *reinterpret_cast<uint32_t*>(vbyte + pid) = ok;
+}
+
+// K1: blocks stride over (4-row group, plane) items, threads over the chunks of a row; one partial per block as in
+// source_kernel (same ticket, same finalize)
+template <typename T>
+__global__ void __launch_bounds__(SETUP_BX * SETUP_BY)
+source4_kernel(Geom g, const T* __restrict__ gx, const T* __restrict__ gy, const T* __restrict__ gz,
+               const uint8_t* __restrict__ link, Coef<T> K, T* __restrict__ S, Scalars* sc, double* partial)
+{
+    __shared__ double red[SETUP_BX * SETUP_BY / 32];
+    __shared__ int is_last;
+    const int nyb = (g.ny + SETUP_BY - 1) / SETUP_BY;
+    const long long items = (long long)nyb * g.nz;
+    const long long sy = g.nx, sz = (long long)g.nx * g.ny;
+    double sq = 0.0;
+    for (long long w = blockIdx.x; w < items; w += gridDim.x) {
+        const int k = (int)(w / nyb), j = (int)(w - (long long)k * nyb) * SETUP_BY + threadIdx.y;
+        if (j >= g.ny) continue;
+        const bool own = (k >= g.kz0 && k < g.kz1);                 // a slab counts the planes it owns
+        for (int i0 = threadIdx.x * 4; i0 < g.px; i0 += SETUP_BX * 4) {
+            const long long pid = i0 + (long long)g.px * (j + (long long)g.ny * k);
+            T s[4];
+            zero_chunk<T, 4>(s);
+            const uint32_t lw = *reinterpret_cast<const uint32_t*>(link + pid);
+            if (lw & 0x40404040u) {                                  // (implies i0 < nx)
+                const long long u = i0 + (long long)g.nx * (j + (long long)g.ny * k);
+                T xc[4], yc[4], yn[4], ys[4], zc[4], zf[4], zb[4];
+                ld_chunk<T, 4>(gx + u, xc);
+                ld_chunk<T, 4>(gy + u, yc);
+                zero_chunk<T, 4>(yn); zero_chunk<T, 4>(ys); zero_chunk<T, 4>(zc); zero_chunk<T, 4>(zf); zero_chunk<T, 4>(zb);
+                if (j + 1 < g.ny) ld_chunk<T, 4>(gy + u + sy, yn);
+                if (j > 0) ld_chunk<T, 4>(gy + u - sy, ys);
+                if (g.naxes == 3) {
+                    ld_chunk<T, 4>(gz + u, zc);
+                    if (k + 1 < g.nz) ld_chunk<T, 4>(gz + u + sz, zf);
+                    if (k > 0) ld_chunk<T, 4>(gz + u - sz, zb);
+                }
+                const T xl = (i0 > 0) ? gx[u - 1] : T(0), xr = (i0 + 4 < g.nx) ? gx[u + 4] : T(0);
+#pragma unroll
+                for (int q = 0; q < 4; ++q) {
+                    const uint32_t l = (lw >> (8 * q)) & 0xffu;
+                    if (!(l & LINK_VALID)) continue;
+                    const T e = (q == 3) ? xr : xc[q < 3 ? q + 1 : 3], wv = (q == 0) ? xl : xc[q > 0 ? q - 1 : 0];
+                    T v = T(0);
+                    if (l & 1u) v -= K.hs[0] * (e + xc[q]);
+                    if (l & 2u) v += K.hs[0] * (wv + xc[q]);
+                    if (l & 4u) v -= K.hs[1] * (yn[q] + yc[q]);
+                    if (l & 8u) v += K.hs[1] * (ys[q] + yc[q]);
+                    if (l & 16u) v -= K.hs[2] * (zf[q] + zc[q]);
+                    if (l & 32u) v += K.hs[2] * (zb[q] + zc[q]);
+                    s[q] = v;
+                }
+            }
+            st_chunk<T, 4>(S + pid, s);
+            if (own) {
+#pragma unroll
+                for (int q = 0; q < 4; ++q) sq += (double)s[q] * (double)s[q];
+            }
+        }
+    }
+    const int tid = threadIdx.y * SETUP_BX + threadIdx.x;
+    sq = warp_sum(sq);
+    if ((tid & 31) == 0) red[tid >> 5] = sq;
+    __syncthreads();
+    if (tid == 0) {
+        double t = 0.0;
+        for (int w = 0; w < SETUP_BX * SETUP_BY / 32; ++w) t += red[w];
+        partial[blockIdx.x] = t;
+        __threadfence();
+        is_last = (atomicAdd(&sc->ticket[3], 1u) == gridDim.x - 1);
+    }
+    __syncthreads();
+    if (is_last) {
+        __threadfence();
+        double t = 0.0;
+        for (unsigned int b = tid; b < gridDim.x; b += SETUP_BX * SETUP_BY) t += __ldcg(&partial[b]);
+        t = warp_sum(t);
+        __syncthreads();
+        if ((tid & 31) == 0) red[tid >> 5] = t;
+        __syncthreads();
+        if (tid == 0) {
+            double n2 = 0.0;
+            for (int w = 0; w < SETUP_BX * SETUP_BY / 32; ++w) n2 += red[w];
+            sc->ticket[3] = 0;
+            if (sc->defer) sc->red_out[0] = n2; else source_finalize(sc, n2);
+        }
+    }
+}
+
+template <typename T>
+__global__ void __launch_bounds__(SETUP_BX * SETUP_BY)
+finalize4_kernel(Geom g, const double* P0, const double* P1, const Scalars* sc, const uint8_t* __restrict__ link,
+                 T* __restrict__ out, double* __restrict__ out64)
+{
+    const double* __restrict__ P = (sc->n & 1) ? P0 : P1;      // the last K2 wrote Pbuf[(n & 1) ^ 1]
+    const int i0 = (blockIdx.x * SETUP_BX + threadIdx.x) * 4, j = blockIdx.y * SETUP_BY + threadIdx.y, k = blockIdx.z;
+    if (i0 == 0 && j == 0 && k == 0 && sc->status_out != nullptr) *sc->status_out = sc->status;
+    if (i0 >= g.nx || j >= g.ny) return;
+    const long long pid = i0 + (long long)g.px * (j + (long long)g.ny * k);
+    const long long u = i0 + (long long)g.nx * (j + (long long)g.ny * k);
+    const uint32_t lw = *reinterpret_cast<const uint32_t*>(link + pid);
+    double p[4], o64[4];
+    ld_chunk<double, 4>(P + pid, p);
+    T o[4];
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+        const bool ok = ((lw >> (8 * q)) & LINK_VALID) != 0;
+        o[q] = ok ? (T)p[q] : (T)nan("");
+        o64[q] = ok ? p[q] : nan("");
+    }
+    st_chunk<T, 4>(out + u, o);
+    if (out64 != nullptr) st_chunk<double, 4>(out64 + u, o64);
+}
+
 // copies between the caller's unpadded layout and the padded internal layout (step entry points only)
 template <typename TI, typename TO>
 __global__ void pad_copy_kernel(Geom g, const TI* __restrict__ in, TO* __restrict__ out, int to_padded,

@@ -41,9 +41,10 @@ source_noalloc_kernel(int nx, int ny, int nz, int naxes, const T* __restrict__ g
     for (int it = 0; it < NOALLOC_ITEMS; ++it) {
         const long long u = base + (long long)it * NOALLOC_THREADS;
         if (u >= n) break;
-        const int i = (int)(u % nx);
-        const long long row = u / nx;
-        const int j = (int)(row % ny), k = (int)(row / ny);
+        // n <= NOALLOC_MAX_CELLS < 2^31: 32-bit index arithmetic
+        const unsigned int u32 = (unsigned int)u, row = u32 / (unsigned int)nx;
+        const int i = (int)(u32 - row * (unsigned int)nx);
+        const int k = (int)(row / (unsigned int)ny), j = (int)(row - (unsigned int)k * (unsigned int)ny);
         T s = T(0);
         if (valid(u)) {
             // same terms, same order as source_kernel: E W N S (F B); faces to missing cells contribute nothing (Eq. 49 :656)
