@@ -111,20 +111,23 @@ static double far_face_constant(double da, double db, double dc)
  * out[4..12] = c[a][b] row-major  (Eq. 17 :207-212 / Eq. 32-35 :314-326 / A7)
  * nz == 1 -> 2D scheme: F_z = 0 and every c with a z index = 0. */
 /* Batched 2D snapshots (SURVEY NEXT-1; PAPER.md:365 "26 Taylor vortex snapshots", :503): nb independent 2D fields on
- * one mask are stacked along z and solved as ONE block-diagonal system with the 2D constants.  Every constant with a
- * z index is then 0, so all weights across planes vanish (Eq. 16/18 with c_xz = c_yz = c_zz = 0, F_z = 0) and no other
- * routine needs to know.  The flag is set only inside oracle_solve_batch2d (test infrastructure: not thread safe). */
-static int g_batch2d = 0;
-/* set by oracle_solve_direct around solve_impl: the inner systems are L P = S instead of Eq. 12;
- * 2: with the single-reduction recurrences of cg1_op */
-static int g_direct = 0;
+ * one mask are stacked along z and solved as ONE block-diagonal system with the 2D constants (scheme2d = 1 below although
+ * nz > 1).  Every constant with a z index is then 0, so all weights across planes vanish (Eq. 16/18 with c_xz = c_yz =
+ * c_zz = 0, F_z = 0) and no other routine needs to know.  The choices "2D scheme on a stack" and "inner systems L P = S"
+ * are explicit arguments of the internal routines (constants_impl, weights_impl, solve_impl): no hidden state. */
+static void constants_impl(int scheme2d, double dx, double dy, double dz, double *out);
 
 void oracle_constants(int nx, int ny, int nz, double dx, double dy, double dz, double *out)
 {
     (void)nx; (void)ny;
+    constants_impl(nz == 1, dx, dy, dz, out);
+}
+
+static void constants_impl(int scheme2d, double dx, double dy, double dz, double *out)
+{
     double F[3], c[3][3], Atot;
     memset(c, 0, sizeof c);
-    if (nz == 1 || g_batch2d) {
+    if (scheme2d) {
         double dd = sqrt(dx * dx + dy * dy);          /* :214 */
         F[0] = 2.0 * dy; F[1] = 2.0 * dx; F[2] = 0.0; /* Eq. 5 :75, :96 */
         Atot = 4.0 * (dx + dy);                       /* Eq. 8 :94 */
@@ -191,11 +194,20 @@ static inline int val(const unsigned char *v, int nx, int ny, int nz, int i, int
 
 /* w1[d*N + c] = w_d^{n+1}(c), w0[d*N + c] = w_d^{n}(c), w0C[c] = w_C^{n}(c); w_C^{n+1} = 0 (Eq. 11 :113).
  * Missing cells get all-zero weights. */
+static void weights_impl(int scheme2d, int nx, int ny, int nz, double dx, double dy, double dz, const unsigned char *v,
+                         double *w1, double *w0, double *w0C);
+
 void oracle_weights(int nx, int ny, int nz, double dx, double dy, double dz, const unsigned char *v,
                     double *w1, double *w0, double *w0C)
 {
+    weights_impl(nz == 1, nx, ny, nz, dx, dy, dz, v, w1, w0, w0C);
+}
+
+static void weights_impl(int scheme2d, int nx, int ny, int nz, double dx, double dy, double dz, const unsigned char *v,
+                         double *w1, double *w0, double *w0C)
+{
     double K[13];
-    oracle_constants(nx, ny, nz, dx, dy, dz, K);
+    constants_impl(scheme2d, dx, dy, dz, K);
     const double *F = K, Atot = K[3], *c = K + 4;
     i64 N = (i64)nx * ny * nz;
 #pragma omp parallel for collapse(2) if (N > OMP_MIN_N)
@@ -421,7 +433,9 @@ typedef struct {
 
 /* P_out: pressure at valid cells, NaN at missing cells (:158).  hist (may be NULL) receives eps_R of every outer
  * iteration visited, up to hist_cap entries.  Returns 0, or -1 on allocation failure. */
-static int solve_impl(int nx, int ny, int nz, double dx, double dy, double dz,
+/* scheme2d: 2D constants although nz > 1 (stacked snapshots); direct: 0 = Eq. 12 (Alg. 1), 1 = L P = S by textbook CG,
+ * 2 = L P = S by the single-reduction recurrences of cg1_op */
+static int solve_impl(int scheme2d, int direct, int nx, int ny, int nz, double dx, double dy, double dz,
                       const double *gx, const double *gy, const double *gz, const unsigned char *mask,
                       const double *P_init, double *P_out, double tol, int max_outer, int max_cg, oracle_info *info,
                       double *hist, int hist_cap, double *hist_P);
@@ -431,7 +445,7 @@ int oracle_solve(int nx, int ny, int nz, double dx, double dy, double dz,
                  double *P_out, double tol, int max_outer, int max_cg, oracle_info *info,
                  double *hist, int hist_cap)
 {
-    return solve_impl(nx, ny, nz, dx, dy, dz, gx, gy, gz, mask, NULL, P_out, tol, max_outer, max_cg, info, hist, hist_cap, NULL);
+    return solve_impl(nz == 1, 0, nx, ny, nz, dx, dy, dz, gx, gy, gz, mask, NULL, P_out, tol, max_outer, max_cg, info, hist, hist_cap, NULL);
 }
 
 /* oracle_solve that also records the pressure-update metric of Eq. 40 (:438): hist_P[n] = ||P^n - P^{n-1}|| / ||P^n||
@@ -441,7 +455,7 @@ int oracle_solve_hist(int nx, int ny, int nz, double dx, double dy, double dz,
                       double *P_out, double tol, int max_outer, int max_cg, oracle_info *info,
                       double *hist, double *hist_P, int hist_cap)
 {
-    return solve_impl(nx, ny, nz, dx, dy, dz, gx, gy, gz, mask, NULL, P_out, tol, max_outer, max_cg, info, hist, hist_cap, hist_P);
+    return solve_impl(nz == 1, 0, nx, ny, nz, dx, dy, dz, gx, gy, gz, mask, NULL, P_out, tol, max_outer, max_cg, info, hist, hist_cap, hist_P);
 }
 
 /* Algorithm 1 started from a first guess instead of P^0 = 0 ("initializing with a first guess for the pressure field",
@@ -451,7 +465,7 @@ int oracle_solve_guess(int nx, int ny, int nz, double dx, double dy, double dz,
                        const double *gx, const double *gy, const double *gz, const unsigned char *mask,
                        const double *P_init, double *P_out, double tol, int max_outer, int max_cg, oracle_info *info)
 {
-    return solve_impl(nx, ny, nz, dx, dy, dz, gx, gy, gz, mask, P_init, P_out, tol, max_outer, max_cg, info, NULL, 0, NULL);
+    return solve_impl(nz == 1, 0, nx, ny, nz, dx, dy, dz, gx, gy, gz, mask, P_init, P_out, tol, max_outer, max_cg, info, NULL, 0, NULL);
 }
 
 /* The fixed point of Alg. 1 computed without the boundary iteration: at convergence P^{n+1} = P^n, so Eq. 12 reads
@@ -464,10 +478,7 @@ int oracle_solve_direct(int nx, int ny, int nz, double dx, double dy, double dz,
                         const double *gx, const double *gy, const double *gz, const unsigned char *mask,
                         const double *P_init, double *P_out, double tol, int max_outer, int max_cg, oracle_info *info)
 {
-    g_direct = 1;
-    int rc = solve_impl(nx, ny, nz, dx, dy, dz, gx, gy, gz, mask, P_init, P_out, tol, max_outer, max_cg, info, NULL, 0, NULL);
-    g_direct = 0;
-    return rc;
+    return solve_impl(nz == 1, 1, nx, ny, nz, dx, dy, dz, gx, gy, gz, mask, P_init, P_out, tol, max_outer, max_cg, info, NULL, 0, NULL);
 }
 
 /* oracle_solve_direct with the single-reduction CG recurrences (cg1_op) in the inner solves: same system, same outer
@@ -476,18 +487,15 @@ int oracle_solve_direct_cg1(int nx, int ny, int nz, double dx, double dy, double
                             const double *gx, const double *gy, const double *gz, const unsigned char *mask,
                             const double *P_init, double *P_out, double tol, int max_outer, int max_cg, oracle_info *info)
 {
-    g_direct = 2;
-    int rc = solve_impl(nx, ny, nz, dx, dy, dz, gx, gy, gz, mask, P_init, P_out, tol, max_outer, max_cg, info, NULL, 0, NULL);
-    g_direct = 0;
-    return rc;
+    return solve_impl(nz == 1, 2, nx, ny, nz, dx, dy, dz, gx, gy, gz, mask, P_init, P_out, tol, max_outer, max_cg, info, NULL, 0, NULL);
 }
 
 /* nb snapshots [nb][ny][nx] on one mask [ny][nx] (NULL = all valid), optional first guess P_init [nb][ny][nx]
  * ("initialized to zero ... or any other arbitrary value"; NULL = 0).  eps_R and the CG scalars are those
  * of the stacked system. */
-int oracle_solve_batch2d(int nx, int ny, int nb, double dx, double dy,
-                         const double *gx, const double *gy, const unsigned char *mask2d, const double *P_init,
-                         double *P_out, double tol, int max_outer, int max_cg, oracle_info *info)
+static int solve_batch2d_impl(int direct, int nx, int ny, int nb, double dx, double dy,
+                              const double *gx, const double *gy, const unsigned char *mask2d, const double *P_init,
+                              double *P_out, double tol, int max_outer, int max_cg, oracle_info *info)
 {
     unsigned char *m = NULL;
     if (mask2d) {
@@ -495,11 +503,16 @@ int oracle_solve_batch2d(int nx, int ny, int nb, double dx, double dy,
         if (!m) return -1;
         for (int b = 0; b < nb; ++b) memcpy(m + (size_t)b * nx * ny, mask2d, (size_t)nx * ny);
     }
-    g_batch2d = 1;
-    int rc = solve_impl(nx, ny, nb, dx, dy, 1.0, gx, gy, NULL, m, P_init, P_out, tol, max_outer, max_cg, info, NULL, 0, NULL);
-    g_batch2d = 0;
+    int rc = solve_impl(1, direct, nx, ny, nb, dx, dy, 1.0, gx, gy, NULL, m, P_init, P_out, tol, max_outer, max_cg, info, NULL, 0, NULL);
     free(m);
     return rc;
+}
+
+int oracle_solve_batch2d(int nx, int ny, int nb, double dx, double dy,
+                         const double *gx, const double *gy, const unsigned char *mask2d, const double *P_init,
+                         double *P_out, double tol, int max_outer, int max_cg, oracle_info *info)
+{
+    return solve_batch2d_impl(0, nx, ny, nb, dx, dy, gx, gy, mask2d, P_init, P_out, tol, max_outer, max_cg, info);
 }
 
 /* oracle_solve_batch2d with the inner systems of oracle_solve_direct: CG on the block-diagonal L P = S of the stack */
@@ -507,13 +520,10 @@ int oracle_solve_direct_batch2d(int nx, int ny, int nb, double dx, double dy,
                                 const double *gx, const double *gy, const unsigned char *mask2d, const double *P_init,
                                 double *P_out, double tol, int max_outer, int max_cg, oracle_info *info)
 {
-    g_direct = 1;
-    int rc = oracle_solve_batch2d(nx, ny, nb, dx, dy, gx, gy, mask2d, P_init, P_out, tol, max_outer, max_cg, info);
-    g_direct = 0;
-    return rc;
+    return solve_batch2d_impl(1, nx, ny, nb, dx, dy, gx, gy, mask2d, P_init, P_out, tol, max_outer, max_cg, info);
 }
 
-static int solve_impl(int nx, int ny, int nz, double dx, double dy, double dz,
+static int solve_impl(int scheme2d, int direct, int nx, int ny, int nz, double dx, double dy, double dz,
                       const double *gx, const double *gy, const double *gz, const unsigned char *mask,
                       const double *P_init, double *P_out, double tol, int max_outer, int max_cg, oracle_info *info,
                       double *hist, int hist_cap, double *hist_P)
@@ -526,13 +536,13 @@ static int solve_impl(int nx, int ny, int nz, double dx, double dy, double dz,
     double *rhs = (double *)malloc(nb), *r = (double *)malloc(nb), *p = (double *)malloc(nb), *q = (double *)malloc(nb);
     double *tmp = (double *)malloc(nb);
     double *Pold = hist_P ? (double *)malloc(nb) : NULL;
-    double *wv = (g_direct == 2) ? (double *)malloc(nb) : NULL;
+    double *wv = (direct == 2) ? (double *)malloc(nb) : NULL;
     int rc = -1;
-    if (!v || !w1 || !w0 || !w0C || !S || !P || !rhs || !r || !p || !q || !tmp || (hist_P && !Pold) || (g_direct == 2 && !wv)) goto done;
+    if (!v || !w1 || !w0 || !w0C || !S || !P || !rhs || !r || !p || !q || !tmp || (hist_P && !Pold) || (direct == 2 && !wv)) goto done;
     rc = 0;
 
     oracle_validity(nx, ny, nz, gx, gy, gz, mask, v);
-    oracle_weights(nx, ny, nz, dx, dy, dz, v, w1, w0, w0C);
+    weights_impl(scheme2d, nx, ny, nz, dx, dy, dz, v, w1, w0, w0C);
     oracle_source(nx, ny, nz, dx, dy, dz, v, w1, w0, gx, gy, gz ? gz : gx, S);
     double normS = sqrt(dot(N, nx, S, S));
     if (P_init)
@@ -564,9 +574,9 @@ static int solve_impl(int nx, int ny, int nz, double dx, double dy, double dz,
             /* Solve Eq. 12 for P^{n+1} by CG, first guess P^n (:489); inner threshold: reading A3.
              * Fixed-point variant (oracle_solve_direct): the same loop with the system L P = S; eps_R above is its
              * residual too (r0 = S - L P^n), so the outer loop only restarts a CG that hit max_cg. */
-            if (g_direct) memcpy(rhs, S, nb);
-            if (g_direct == 2) cg_total += cg1_op(nx, ny, nz, v, w1, w0, w0C, rhs, P, 0.1 * tol * normS, max_cg, r, p, q, tmp, wv);
-            else cg_total += cg_op(g_direct, nx, ny, nz, v, w1, w0, w0C, rhs, P, 0.1 * tol * normS, max_cg, r, p, q, tmp);
+            if (direct) memcpy(rhs, S, nb);
+            if (direct == 2) cg_total += cg1_op(nx, ny, nz, v, w1, w0, w0C, rhs, P, 0.1 * tol * normS, max_cg, r, p, q, tmp, wv);
+            else cg_total += cg_op(direct, nx, ny, nz, v, w1, w0, w0C, rhs, P, 0.1 * tol * normS, max_cg, r, p, q, tmp);
             ++n;
         }
     }
