@@ -377,8 +377,11 @@ long long omni_launch_count(int reset);
  *   2  CUDA graph with device-side conditional WHILE nodes around the tile kernels K2 / K3 / K4
  *   3  one persistent cooperative kernel: phases separated by grid barriers that double as the reductions
  *      (state is L2-resident; falls back to mode 2 if the device cannot co-schedule the grid)
+ *   4  the whole iteration as ONE cooperative launch of the tile kernels' TMA pipeline (one column per CTA, the same
+ *      grid barriers between the K2 / K3 / K4 phases); correct and deterministic, measured slower than mode 2 at every
+ *      size (profiles/r2_loop_and_rows.md), never chosen automatically; falls back to mode 2 if its grid does not fit
  * The environment variable OMNI_PERSIST_MAX_CELLS overrides the automatic threshold.  Modes 1 and 2 give bit-identical
- * results; mode 3 sums its reductions in a different (fixed) order.  Returns the previous mode; other values are ignored. */
+ * results; modes 3 and 4 sum their reductions in a different (fixed) order.  Returns the previous mode; other values are ignored. */
 int omni_set_loop_mode(int mode);
 /* Convergence history (the momentum residual of Eq. 41, plotted in Fig. 10-13): registers a caller-owned
  * DEVICE buffer of `capacity` doubles that every solve enqueued afterwards fills on the device -- entry i = eps_R =
