@@ -185,7 +185,8 @@ int omni_solve_cascade_f32(int nx, int ny, int nz, double dx, double dy, double 
  * R-P1 of DESIGN.md; not the paper's iteration, which names only "CG").  Same system L P = S, same outer
  * loop (fp64 refinement: eps_R of Eq. 41 :442 re-evaluated from the fp64 master pressure, CG restarted on it), same
  * stopping rules, status codes and omni_info; cg_iters_total counts preconditioned iterations.  The V-cycle: levels
- * halving every axis that still has >= 8 cells (a coarse cell is valid iff one of its children is), link weights
+ * halving every axis that still has >= 8 cells and whose link weight is >= 0.7 of the largest such weight
+ * (semi-coarsening: anisotropic spacings cost no extra iterations; a coarse cell is valid iff one of its children is), link weights
  * w_{l+1}[a] = w_l[a] 2^m (1/4 along halved axes), restriction = sum over the children, prolongation = its transpose,
  * damped Jacobi (omega = 0.8), 2 sweeps before and after the coarse-grid correction, 8 on the coarsest level.  The
  * iteration count is nearly independent of the grid size (about 10 to eps_R <= 1e-5, 15 to 1e-8) at about 4 times the

@@ -7,8 +7,13 @@ DESIGN.md R-P1, restated step by step here.  Shares nothing with the CUDA path; 
 oracle legs may import it.
 
 Reading R-P1 (the algorithm, in the order executed):
-  levels   level 0 is the grid.  Level l+1 halves (ceil) every axis of level l that has >= 8 cells; a coarse cell is
-           valid iff one of its children is; coarsening stops when no axis qualifies (or after 16 levels).
+  levels   level 0 is the grid.  Level l+1 halves (ceil) every axis a of level l that has >= 8 cells AND is strongly
+           coupled on that level: w_l[a] >= 0.7 max_b w_l[b] (b over the axes with >= 8 cells).  Point smoothing only
+           removes error along strongly coupled axes, so a weakly coupled axis (t_a is proportional to 1 / Delta_a: the
+           axis with the larger spacing) is left alone until the halvings of the others -- each divides its own weight by
+           4 relative to the rest -- have made it strong (semi-coarsening; on isotropic grids every axis is halved on every
+           level).  A coarse cell is valid iff one of its children is; coarsening stops when no axis qualifies (or after
+           24 levels).
   operator (L_l x)_C = sum_d v_l(C+d) w_l[a] (x_C - x_{C+d}) on valid cells, 0 elsewhere.  w_0[a] = t_a = F_a / A_tot
            (Eq. 10 :109: w^{n+1} + w^n on a valid link); w_{l+1}[a] = w_l[a] * 2^m * (1/4 if axis a was halved else 1),
            m = number of halved axes: the Galerkin weight of piecewise-constant transfers (number of fine links between
@@ -35,8 +40,9 @@ from . import omni_oracle as _o
 OMEGA = 0.8
 NU = 2            # sweeps before and after the coarse-grid correction
 NU_COARSEST = 8
-MIN_COARSEN = 8   # an axis is halved while it has at least this many cells
-MAX_LEVELS = 16
+MIN_COARSEN = 8   # an axis is halved while it has at least this many cells ...
+THETA = 0.7       # ... and its link weight is at least this fraction of the largest weight among such axes
+MAX_LEVELS = 24
 
 
 def _shift(x, ax, s):
@@ -81,9 +87,14 @@ class Level:
         return x + OMEGA * self.Dinv * (b - self.apply(x))
 
 
-def coarsen_plan(shape):
-    """Which numpy axes of `shape` are halved to make the next level (those with >= MIN_COARSEN cells)."""
-    return [s >= MIN_COARSEN for s in shape]
+def coarsen_plan(shape, w):
+    """Which numpy axes of `shape` are halved to make the next level: those with >= MIN_COARSEN cells whose link weight
+    (w[a], a = 0 is x = the LAST numpy axis) is >= THETA times the largest weight among the axes with >= MIN_COARSEN cells."""
+    nd = len(shape)
+    ok = [s >= MIN_COARSEN for s in shape]
+    wax = [float(w[nd - 1 - ax]) for ax in range(nd)]
+    wmax = max([wa for wa, o in zip(wax, ok) if o], default=0.0)
+    return [bool(o and wa >= THETA * wmax) for wa, o in zip(wax, ok)]
 
 
 def restrict(r, halve):
@@ -113,7 +124,7 @@ def build_levels(v, w0):
     levels, plans = [Level(v.astype(bool), w0)], []
     while len(levels) < MAX_LEVELS:
         f = levels[-1]
-        halve = coarsen_plan(f.v.shape)
+        halve = coarsen_plan(f.v.shape, f.w)
         if not any(halve):
             break
         m = sum(halve)

@@ -848,7 +848,13 @@ int mg_build(const Geom& g, const Workspace<T>& w, const HostConst& H, MgHier<T>
     M.L[M.nlev++] = L0;
     while (M.nlev < MG_MAX_LEVELS) {
         MgLevel<T>& F = M.L[M.nlev - 1];
-        F.hx = F.nx >= MG_MIN_COARSEN; F.hy = F.ny >= MG_MIN_COARSEN; F.hz = (g.naxes == 3 && F.nz >= MG_MIN_COARSEN);
+        const bool ok[3] = { F.nx >= MG_MIN_COARSEN, F.ny >= MG_MIN_COARSEN, g.naxes == 3 && F.nz >= MG_MIN_COARSEN };
+        double wmax = 0.0;
+        for (int a = 0; a < 3; ++a)
+            if (ok[a] && wd[a] > wmax) wmax = wd[a];
+        F.hx = ok[0] && wd[0] >= MG_THETA * wmax;                    // strongly coupled axes only (reading R-P1)
+        F.hy = ok[1] && wd[1] >= MG_THETA * wmax;
+        F.hz = ok[2] && wd[2] >= MG_THETA * wmax;
         const int m = F.hx + F.hy + F.hz;
         if (m == 0) break;
         MgLevel<T> C = {};

@@ -3,7 +3,9 @@
 // only "CG"; this accelerates the separately named fixed-point solve of omni_solve_direct_*.
 //
 //   levels    level 0 = the grid (padded layout of the solver, its link bytes); level l+1 halves (ceil) every axis of
-//             level l with >= 8 cells; a coarse cell is valid iff one of its children is
+//             level l with >= 8 cells whose weight is >= 0.7 of the largest such weight (semi-coarsening: point smoothing
+//             only works along strongly coupled axes; t_a ~ 1 / Delta_a, so the axis with the larger spacing waits until
+//             the halvings of the others have made it strong); a coarse cell is valid iff one of its children is
 //   operator  (L_l x)_C = sum_d v_l(C+d) w_l[a] (x_C - x_{C+d}); w_0[a] = t_a = F_a / A_tot (Eq. 10 :109),
 //             w_{l+1}[a] = w_l[a] 2^m (1/4 if axis a was halved else 1), m = number of halved axes
 //   transfer  restriction = sum over the children, prolongation = the parent's value (transposes of each other)
@@ -17,8 +19,9 @@
 
 namespace omni {
 
-constexpr int MG_MAX_LEVELS = 16;
+constexpr int MG_MAX_LEVELS = 24;
 constexpr int MG_MIN_COARSEN = 8;
+constexpr double MG_THETA = 0.7;          // an axis is halved only while its weight is >= MG_THETA x the largest (semi-coarsening)
 constexpr int MG_NU = 2, MG_NU_COARSEST = 8;
 constexpr double MG_OMEGA = 0.8;
 

@@ -1012,7 +1012,17 @@ def test_pcg_oracle_pieces():
         r, e = rng.normal(size=shape), rng.normal(size=cshape)
         assert pcg.restrict(r, halve).shape == cshape
         assert np.sum(pcg.restrict(r, halve) * e) == pytest.approx(np.sum(r * pcg.prolong(e, halve, shape)), rel=1e-13)
-    assert pcg.coarsen_plan((5, 8, 17)) == [False, True, True]
+    assert pcg.coarsen_plan((5, 8, 17), [1.0, 1.0, 1.0]) == [False, True, True]
+    # semi-coarsening: only the strongly coupled axes (weight >= 0.7 of the largest among the axes long enough) are halved
+    assert pcg.coarsen_plan((40, 40, 40), [1.0, 0.69, 0.3]) == [False, False, True]       # w[0] is x = the last numpy axis
+    assert pcg.coarsen_plan((40, 40, 40), [0.3, 0.71, 1.0]) == [True, True, False]
+    assert pcg.coarsen_plan((40, 40, 4), [9.0, 0.71, 1.0]) == [True, True, False]         # x is too short to count
+    assert pcg.coarsen_plan((4, 4), [1.0, 1.0]) == [False, False]
+    # a halved axis loses a factor 4 against the others: the weak axis catches up and is halved on a later level
+    lv, pl = pcg.build_levels(np.ones((32, 32, 32), bool), [1.0, 0.5, 0.2])
+    assert pl[0] == [False, False, True] and np.allclose(lv[1].w, [0.5, 1.0, 0.4])
+    assert pl[1] == [False, True, False] and np.allclose(lv[2].w, [1.0, 0.5, 0.8])
+    assert pl[2] == [True, False, True] and np.allclose(lv[3].w, [1.0, 2.0, 0.8])
     v = rng.random((6, 7)) > 0.1
     levels, plans = pcg.build_levels(v, [0.3, 0.2])
     assert len(levels) == 1 and plans == []
@@ -1025,8 +1035,8 @@ def test_pcg_oracle_pieces():
     for _ in range(pcg.NU_COARSEST):
         z, term = z + term, G @ term
     assert np.abs(pcg.vcycle(levels, plans, 0, b).ravel() - z).max() < 1e-13
-    levels, plans = pcg.build_levels(np.ones((5, 16, 24), bool), [0.1, 0.2, 0.3])     # w[0] is x (24), w[2] is z (5)
-    assert plans[0] == [False, True, True] and np.allclose(levels[1].w, [0.1 * 4 / 4, 0.2 * 4 / 4, 0.3 * 4])
+    levels, plans = pcg.build_levels(np.ones((5, 16, 24), bool), [0.25, 0.25, 0.3])     # w[0] is x (24), w[2] is z (5: too short)
+    assert plans[0] == [False, True, True] and np.allclose(levels[1].w, [0.25 * 4 / 4, 0.25 * 4 / 4, 0.3 * 4])
     assert levels[1].v.shape == (5, 8, 12) and plans[1] == [False, True, True] and levels[2].v.shape == (5, 4, 6)
     assert len(levels) == 3
 
