@@ -212,6 +212,15 @@ int omni_solve_direct_batch2d_f32(int nx, int ny, int nb, double dx, double dy, 
                                   const unsigned char* d_mask2d, const float* d_P_init, float* d_P_out, double tol,
                                   int max_outer, int max_cg, void* stream, omni_info* info);
 
+/* ... and with the multigrid-preconditioned CG of omni_solve_pcg_* (the snapshot axis carries no links and is never
+ * coarsened; joint CG scalars and stopping tests over the stack, as for omni_solve_batch2d_*). */
+int omni_solve_pcg_batch2d_f64(int nx, int ny, int nb, double dx, double dy, const double* d_gx, const double* d_gy,
+                               const unsigned char* d_mask2d, const double* d_P_init, double* d_P_out, double tol,
+                               int max_outer, int max_cg, void* stream, omni_info* info);
+int omni_solve_pcg_batch2d_f32(int nx, int ny, int nb, double dx, double dy, const float* d_gx, const float* d_gy,
+                               const unsigned char* d_mask2d, const float* d_P_init, float* d_P_out, double tol,
+                               int max_outer, int max_cg, void* stream, omni_info* info);
+
 /* ---- batched 2D snapshots with an optional first guess (SURVEY.md 8(f) NEXT-1; time-resolved PIV: PAPER.md:365, :503) ----
  * nb independent 2D gradient fields [nb][ny][nx] on ONE mask [ny][nx] (NULL = all valid) are stacked and solved as one
  * block-diagonal system with the 2D scheme: stencil codes are built once, every stencil sweep serves all snapshots,
@@ -405,7 +414,7 @@ void omni_release_memory(void);
 int omni_profile_enable(int on);          /* returns the previous setting */
 void omni_profile_read(double* h_ms3, long long* h_count3, int reset);
 const char* omni_status_string(int status);
-int omni_version(void);                  /* 100 * major + minor; 101 added the _guess, _rans_source and history entry points, 102 omni_solve_pcg_*, 103 omni_solve_ex_* / omni_options, 104 omni_solve_slab_*, 105 omni_source_noalloc_* */
+int omni_version(void);                  /* 100 * major + minor; 101 added the _guess, _rans_source and history entry points, 102 omni_solve_pcg_*, 103 omni_solve_ex_* / omni_options, 104 omni_solve_slab_*, 105 omni_source_noalloc_*, 106 omni_solve_pcg_batch2d_* */
 
 #ifdef __cplusplus
 }

@@ -87,11 +87,12 @@ class Level:
         return x + OMEGA * self.Dinv * (b - self.apply(x))
 
 
-def coarsen_plan(shape, w):
+def coarsen_plan(shape, w, frozen_axes=()):
     """Which numpy axes of `shape` are halved to make the next level: those with >= MIN_COARSEN cells whose link weight
-    (w[a], a = 0 is x = the LAST numpy axis) is >= THETA times the largest weight among the axes with >= MIN_COARSEN cells."""
+    (w[a], a = 0 is x = the LAST numpy axis) is >= THETA times the largest weight among the axes with >= MIN_COARSEN cells;
+    numpy axes in `frozen_axes` (the snapshot axis of a stack of 2D fields) are never halved."""
     nd = len(shape)
-    ok = [s >= MIN_COARSEN for s in shape]
+    ok = [s >= MIN_COARSEN and ax not in frozen_axes for ax, s in enumerate(shape)]
     wax = [float(w[nd - 1 - ax]) for ax in range(nd)]
     wmax = max([wa for wa, o in zip(wax, ok) if o], default=0.0)
     return [bool(o and wa >= THETA * wmax) for wa, o in zip(wax, ok)]
@@ -120,11 +121,11 @@ def prolong(e, halve, fshape):
     return e[tuple(slice(0, s) for s in fshape)]
 
 
-def build_levels(v, w0):
+def build_levels(v, w0, frozen_axes=()):
     levels, plans = [Level(v.astype(bool), w0)], []
     while len(levels) < MAX_LEVELS:
         f = levels[-1]
-        halve = coarsen_plan(f.v.shape, f.w)
+        halve = coarsen_plan(f.v.shape, f.w, frozen_axes)
         if not any(halve):
             break
         m = sum(halve)
@@ -158,20 +159,12 @@ def face_weights(nd, dx, dy, dz):
     return [K["F"][a] / K["A_tot"] for a in range(nd)]
 
 
-def solve_pcg(gx, gy, gz, mask, dx, dy, dz, tol, max_outer, max_cg, P_init=None, return_iterates=False, inner_rel=0.0):
-    """Returns (P with NaN at missing cells, info dict) -- same conventions as omni_oracle.solve_direct.
-    inner_rel: an inner solve also stops once ||r|| <= inner_rel ||r0|| (0 = off; the fp32 library variant uses 1e-2,
-    because fp32 vectors cannot resolve more digits of one correction on large grids -- the outer refinement restarts)."""
-    gx = np.asarray(gx, dtype=np.float64)
-    nd = gx.ndim
-    v8 = _o.validity(gx, gy, gz, mask)
-    v = v8.astype(bool)
-    w1, w0, w0C = _o.weights(v8, dx, dy, dz)
-    z3 = lambda c: None if c is None else np.nan_to_num(np.asarray(c, dtype=np.float64))
-    S = _o.source(v8, w1, w0, z3(gx), z3(gy), z3(gz), dx, dy, dz)
-    levels, plans = build_levels(v, face_weights(nd, dx, dy, dz))
+def _pcg_core(v, S, w, tol, max_outer, max_cg, P_init, return_iterates, inner_rel, frozen_axes=()):
+    """The iteration of reading R-P1 on validity v (bool), source S and level-0 link weights w (w[0] is x); numpy axes
+    in `frozen_axes` are never coarsened (the snapshot axis of a stack)."""
+    levels, plans = build_levels(v, w, frozen_axes)
     L0 = levels[0]
-    P = np.zeros(gx.shape) if P_init is None else np.where(v, np.nan_to_num(np.asarray(P_init, dtype=np.float64)), 0.0)
+    P = np.zeros(v.shape) if P_init is None else np.where(v, np.nan_to_num(np.asarray(P_init, dtype=np.float64)), 0.0)
     normS = float(np.sqrt(np.sum(S * S)))
     n, cg_total, epsR, iterates = 0, 0, 0.0, []
     if normS > 0.0:
@@ -203,3 +196,31 @@ def solve_pcg(gx, gy, gz, mask, dx, dy, dz, tol, max_outer, max_cg, P_init=None,
             "levels": len(levels)}
     out = np.where(v, P, np.nan)
     return (out, info, iterates) if return_iterates else (out, info)
+
+
+def solve_pcg(gx, gy, gz, mask, dx, dy, dz, tol, max_outer, max_cg, P_init=None, return_iterates=False, inner_rel=0.0):
+    """Returns (P with NaN at missing cells, info dict) -- same conventions as omni_oracle.solve_direct.
+    inner_rel: an inner solve also stops once ||r|| <= inner_rel ||r0|| (0 = off; the fp32 library variant uses 1e-2,
+    because fp32 vectors cannot resolve more digits of one correction on large grids -- the outer refinement restarts)."""
+    gx = np.asarray(gx, dtype=np.float64)
+    nd = gx.ndim
+    v8 = _o.validity(gx, gy, gz, mask)
+    w1, w0, w0C = _o.weights(v8, dx, dy, dz)
+    z3 = lambda c: None if c is None else np.nan_to_num(np.asarray(c, dtype=np.float64))
+    S = _o.source(v8, w1, w0, z3(gx), z3(gy), z3(gz), dx, dy, dz)
+    return _pcg_core(v8.astype(bool), S, face_weights(nd, dx, dy, dz), tol, max_outer, max_cg, P_init, return_iterates, inner_rel)
+
+
+def solve_pcg_batch2d(gx, gy, mask2d, dx, dy, tol, max_outer, max_cg, P_init=None, inner_rel=0.0):
+    """nb stacked 2D snapshots (nb, ny, nx) on one mask (ny, nx), as omni_oracle.solve_batch2d with direct=True but with
+    the preconditioned iteration: ONE block-diagonal system (2D scheme per plane, no links across planes: weight 0 along
+    the snapshot axis, which is never coarsened), joint CG scalars and stopping tests over the stack."""
+    gx, gy = np.asarray(gx, dtype=np.float64), np.asarray(gy, dtype=np.float64)
+    nb = gx.shape[0]
+    v8 = np.stack([_o.validity(gx[b], gy[b], None, mask2d) for b in range(nb)])
+    S = np.zeros(gx.shape)
+    for b in range(nb):
+        w1, w0, w0C = _o.weights(v8[b], dx, dy)
+        S[b] = _o.source(v8[b], w1, w0, np.nan_to_num(gx[b]), np.nan_to_num(gy[b]), None, dx, dy)
+    w = face_weights(2, dx, dy, 1.0) + [0.0]
+    return _pcg_core(v8.astype(bool), S, w, tol, max_outer, max_cg, P_init, False, inner_rel, frozen_axes=(0,))

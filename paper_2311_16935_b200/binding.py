@@ -17,7 +17,7 @@ STATUS_NAMES = {0: "OMNI_OK", 1: "OMNI_NOT_CONVERGED", -1: "OMNI_ERR_INVALID_ARG
                 -3: "OMNI_ERR_ALLOC", -4: "OMNI_ERR_BREAKDOWN", -5: "OMNI_ERR_TOO_LARGE"}
 # every symbol include/omni.h declares
 SYMBOLS = ["omni_solve_f64", "omni_solve_f32", "omni_workspace_bytes", "omni_solve_f64_ws", "omni_solve_f32_ws",
-           "omni_solve_host_f64", "omni_solve_host_f32", "omni_solve_batch2d_f64", "omni_solve_batch2d_f32", "omni_solve_guess_f64", "omni_solve_guess_f32", "omni_solve_direct_f64", "omni_solve_direct_f32", "omni_solve_pcg_f64", "omni_solve_pcg_f32", "omni_solve_ex_f64", "omni_solve_ex_f32", "omni_options_init", "omni_slab_plan", "omni_slab_unique_id", "omni_slab_comm_create", "omni_slab_comm_destroy",
+           "omni_solve_host_f64", "omni_solve_host_f32", "omni_solve_batch2d_f64", "omni_solve_batch2d_f32", "omni_solve_guess_f64", "omni_solve_guess_f32", "omni_solve_direct_f64", "omni_solve_direct_f32", "omni_solve_pcg_f64", "omni_solve_pcg_f32", "omni_solve_pcg_batch2d_f64", "omni_solve_pcg_batch2d_f32", "omni_solve_ex_f64", "omni_solve_ex_f32", "omni_options_init", "omni_slab_plan", "omni_slab_unique_id", "omni_slab_comm_create", "omni_slab_comm_destroy",
            "omni_solve_slab_f64", "omni_solve_slab_f32", "omni_source_noalloc_f64", "omni_source_noalloc_f32",
            "omni_source_noalloc_max_cells", "omni_solve_direct_batch2d_f64", "omni_solve_direct_batch2d_f32", "omni_solve_cascade_f64", "omni_solve_cascade_f32", "omni_velocity_source_f64", "omni_velocity_source_f32", "omni_rans_source_f64", "omni_rans_source_f32",
            "omni_compressible_rans_source_f64", "omni_compressible_rans_source_f32", "omni_constants", "omni_source_f64", "omni_source_f32",
@@ -463,9 +463,9 @@ def solve_cascade(gx, gy, gz, mask, d, tol, max_outer, max_cg, levels=3, out=Non
     return P, info.as_dict()
 
 
-def solve_batch2d(gx, gy, mask2d, d, tol, max_outer, max_cg, P_init=None, out=None, direct=False):
-    """omni_solve_batch2d_* (direct=True: omni_solve_direct_batch2d_*): gx, gy (nb, ny, nx) CUDA tensors, mask2d
-    (ny, nx) uint8 or None, d = (dx, dy)."""
+def solve_batch2d(gx, gy, mask2d, d, tol, max_outer, max_cg, P_init=None, out=None, direct=False, pcg=False):
+    """omni_solve_batch2d_* (direct=True: omni_solve_direct_batch2d_*; pcg=True: omni_solve_pcg_batch2d_*): gx, gy
+    (nb, ny, nx) CUDA tensors, mask2d (ny, nx) uint8 or None, d = (dx, dy)."""
     import torch
     sfx = _suffix(gx)
     _check([gx, gy, mask2d, P_init, out], "cuda")
@@ -476,7 +476,8 @@ def solve_batch2d(gx, gy, mask2d, d, tol, max_outer, max_cg, P_init=None, out=No
     P = out if out is not None else torch.empty_like(gx)
     info = Info()
     with torch.cuda.device(gx.device):
-        fn = getattr(lib(), f"omni_solve_direct_batch2d_{sfx}" if direct else f"omni_solve_batch2d_{sfx}")
+        name = "omni_solve_pcg_batch2d" if pcg else "omni_solve_direct_batch2d" if direct else "omni_solve_batch2d"
+        fn = getattr(lib(), f"{name}_{sfx}")
         rc = fn(C.c_int(nx), C.c_int(ny), C.c_int(nb), C.c_double(float(d[0])), C.c_double(float(d[1])), _ptr(gx), _ptr(gy),
                 _ptr(mask2d), _ptr(P_init), _ptr(P), C.c_double(tol), C.c_int(max_outer), C.c_int(max_cg),
                 _stream(gx.device), C.byref(info))

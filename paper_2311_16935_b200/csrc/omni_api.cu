@@ -1808,6 +1808,24 @@ int omni_solve_batch2d_f32(int nx, int ny, int nb, double dx, double dy, const f
                               info, 1, d_P_init);
 }
 
+int omni_solve_pcg_batch2d_f64(int nx, int ny, int nb, double dx, double dy, const double* d_gx, const double* d_gy,
+                               const unsigned char* d_mask2d, const double* d_P_init, double* d_P_out, double tol,
+                               int max_outer, int max_cg, void* stream, omni_info* info)
+{
+    if (!d_gx || !d_gy || !d_P_out || nb < 1) return OMNI_ERR_INVALID_ARG;
+    return solve_alloc<double>(nx, ny, nb, dx, dy, 1.0, d_gx, d_gy, nullptr, d_mask2d, d_P_out, tol, max_outer, max_cg, stream,
+                               info, 1, d_P_init, 1, 1);
+}
+
+int omni_solve_pcg_batch2d_f32(int nx, int ny, int nb, double dx, double dy, const float* d_gx, const float* d_gy,
+                               const unsigned char* d_mask2d, const float* d_P_init, float* d_P_out, double tol,
+                               int max_outer, int max_cg, void* stream, omni_info* info)
+{
+    if (!d_gx || !d_gy || !d_P_out || nb < 1) return OMNI_ERR_INVALID_ARG;
+    return solve_alloc<float>(nx, ny, nb, dx, dy, 1.0, d_gx, d_gy, nullptr, d_mask2d, d_P_out, tol, max_outer, max_cg, stream,
+                              info, 1, d_P_init, 1, 1);
+}
+
 int omni_solve_direct_batch2d_f64(int nx, int ny, int nb, double dx, double dy, const double* d_gx, const double* d_gy,
                                   const unsigned char* d_mask2d, const double* d_P_init, double* d_P_out, double tol,
                                   int max_outer, int max_cg, void* stream, omni_info* info)
@@ -2259,6 +2277,6 @@ const char* omni_status_string(int status)
     }
 }
 
-int omni_version(void) { return 105; }   // 101: omni_solve_guess_*, omni_set_history, omni_rans_source_*, omni_compressible_rans_source_*
+int omni_version(void) { return 106; }   // 101: omni_solve_guess_*, omni_set_history, omni_rans_source_*, omni_compressible_rans_source_*
 
 }  // extern "C"

@@ -1075,3 +1075,42 @@ def test_single_reduction_cg_parity(oracle, dtype, kind, shape, frac):
     # costs up to ~10 % more iterations (711 vs 653 on the 150 x 130 case); fp64 stays within a few iterations
     assert abs(ic["cg_iters_total"] - idd["cg_iters_total"]) <= max(3, idd["cg_iters_total"] // (5 if dtype == "f32" else 20))
     assert rel_l2_after_mean_removal(Pc.cpu().numpy(), Pd.cpu().numpy(), valid) <= (2e-6 if dtype == "f64" else 2e-3)
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_pcg_batch2d(oracle, dtype):
+    """omni_solve_pcg_batch2d_*: the stacked snapshots with the multigrid-preconditioned CG against
+    oracle/omni_pcg.solve_pcg_batch2d (fixed counts, with and without a first guess), and converged: every snapshot's own
+    eps_R (oracle operators) within the bound the joint stopping rule gives, the fields equal to the unpreconditioned
+    stacked solve's."""
+    from oracle import omni_pcg
+    fs = [make_field("lamb_oseen2d", (45, 140), seed=s, noise=0.05) for s in range(4)]
+    np_dt = np.float32 if dtype == "f32" else np.float64
+    gx = np.stack([f["g"][0] for f in fs]).astype(np_dt); gy = np.stack([f["g"][1] for f in fs]).astype(np_dt)
+    m, d = fs[0]["mask"], fs[0]["d"]
+    gxd, gyd, md = to_dev(gx), to_dev(gy), to_dev(m)
+    mo, mc, rel = (2, 5, 0.0) if dtype == "f64" else (4, 2, 1e-2)
+    rng = np.random.default_rng(6)
+    P0 = (0.1 * rng.normal(size=gx.shape)).astype(np_dt)
+    for init in (None, P0):
+        P, info = omni.solve_batch2d(gxd, gyd, md, d, 0.0, mo, mc, P_init=None if init is None else to_dev(init), pcg=True)
+        Po, io = omni_pcg.solve_pcg_batch2d(gx.astype(np.float64), gy.astype(np.float64), m, d[0], d[1], 0.0, mo, mc,
+                                            P_init=None if init is None else init.astype(np.float64), inner_rel=rel)
+        assert info["cg_iters_total"] == io["cg_iters_total"] and info["outer_iters"] == io["outer_iters"] == mo
+        Pn = P.cpu().numpy()
+        assert np.array_equal(np.isnan(Pn), np.isnan(Po))
+        for b in range(4):
+            if init is None:
+                assert rel_l2_after_mean_removal(Pn[b], Po[b], ~np.isnan(Po[b])) <= TOL_SOLVE[dtype]
+            else:
+                assert np.nanmax(np.abs(Pn[b] - Po[b])) <= (1e-10 if dtype == "f64" else 2e-4) * np.nanmax(np.abs(Po[b]))
+    tol = 1e-5 if dtype == "f32" else 1e-8
+    Pc, ic = omni.solve_batch2d(gxd, gyd, md, d, tol, 20, 200, pcg=True)
+    assert ic["status"] == 0 and ic["eps_R_final"] <= tol and ic["cg_iters_total"] <= 40
+    Pd, idd = omni.solve_batch2d(gxd, gyd, md, d, tol, 20, 5000, direct=True)
+    assert idd["status"] == 0 and idd["cg_iters_total"] > 5 * ic["cg_iters_total"]
+    for b in range(4):
+        valid = ~torch.isnan(Pd[b]).cpu().numpy()
+        assert rel_l2_after_mean_removal(Pc[b].cpu().numpy(), Pd[b].cpu().numpy(), valid) <= (2e-6 if dtype == "f64" else 2e-3)
+        e_b, _, nS_b = oracle.eps_R_of_field(gx[b].astype(np.float64), gy[b].astype(np.float64), None, m, Pc[b].cpu().numpy(), d[0], d[1])
+        assert e_b * nS_b <= (1.05 if dtype == "f64" else 3.0) * tol * ic["norm_S"]

@@ -1088,3 +1088,29 @@ def test_single_reduction_cg_oracle(oracle, shape, sp):
     assert i1["converged"] and i2["converged"] and abs(i1["cg_iters_total"] - i2["cg_iters_total"]) <= 3
     a, b = np.nan_to_num(P1), np.nan_to_num(P2)
     assert np.linalg.norm(a - b) / np.linalg.norm(b) < 1e-9
+
+
+def test_pcg_batch2d_oracle_pins(oracle):
+    """solve_pcg_batch2d (stacked 2D snapshots, joint scalars): a stack of IDENTICAL snapshots reproduces the single
+    2D solve plane by plane with the same iteration counts (every inner product scales by nb, every ratio is unchanged);
+    nb = 1 equals solve_pcg on the 2D grid; different snapshots converge to the fields of the unpreconditioned stacked
+    solve (oracle.solve_batch2d direct=True, itself pinned to the dense pseudo-inverse)."""
+    from oracle import omni_pcg as pcg
+    fs = [make_field("lamb_oseen2d", (26, 41), seed=s, noise=0.05) for s in range(3)]
+    m, d = fs[0]["mask"], fs[0]["d"]
+    g0x, g0y = fs[0]["g"]
+    P1, i1 = pcg.solve_pcg(g0x, g0y, None, m, d[0], d[1], 1.0, tol=0.0, max_outer=2, max_cg=5)
+    Pb, ib = pcg.solve_pcg_batch2d(np.stack([g0x] * 3), np.stack([g0y] * 3), m, d[0], d[1], tol=0.0, max_outer=2, max_cg=5)
+    assert ib["cg_iters_total"] == i1["cg_iters_total"] == 10 and ib["norm_S"] == pytest.approx(np.sqrt(3) * i1["norm_S"], rel=1e-13)
+    for b in range(3):
+        assert np.nanmax(np.abs(Pb[b] - P1)) <= 1e-12 * np.nanmax(np.abs(P1))
+    Pn, in_ = pcg.solve_pcg_batch2d(g0x[None], g0y[None], m, d[0], d[1], tol=0.0, max_outer=2, max_cg=5)
+    assert np.array_equal(np.nan_to_num(Pn[0]), np.nan_to_num(P1))
+    gx = np.stack([f["g"][0] for f in fs]); gy = np.stack([f["g"][1] for f in fs])
+    Pc, ic = pcg.solve_pcg_batch2d(gx, gy, m, d[0], d[1], tol=1e-10, max_outer=5, max_cg=200)
+    Pd, idd = oracle.solve_batch2d(gx, gy, m, d[0], d[1], 1e-10, 5, 5000, direct=True)
+    assert ic["converged"] and idd["converged"] and ic["cg_iters_total"] * 4 < idd["cg_iters_total"]
+    for b in range(3):
+        valid = ~np.isnan(Pd[b])
+        a, c = Pc[b][valid] - Pc[b][valid].mean(), Pd[b][valid] - Pd[b][valid].mean()
+        assert np.linalg.norm(a - c) / np.linalg.norm(c) < 1e-7
