@@ -4,6 +4,7 @@
 #include "omni_tma.cuh"
 #include "omni_persist.cuh"
 #include "omni_persist1.cuh"
+#include "omni_resident.cuh"
 #include "omni_loop.cuh"
 #include "omni_mg.cuh"
 #include "omni_slab.cuh"
@@ -1069,6 +1070,56 @@ int run_loop_persist(const Geom& g, const Workspace<T>& w, const HostConst& H, c
                                                 : launch_persist<T, 1024, LOP>(g, w, H, K, nsm, st);
 }
 
+// SM-resident loop (omni_resident.cuh): the persistent loop with p in shared memory and r in registers for the whole
+// inner solve.  Returns -100 if the grid does not fit the SMs or the device cannot co-schedule it.
+template <typename T, bool LOP, bool RREG>
+int launch_resident(const Geom& g, const Workspace<T>& w, const HostConst& H, const Coef<T>& K, const ResidentPlan& pl, cudaStream_t st)
+{
+    const int G = pl.gy * pl.gz;
+    if (cudaFuncSetAttribute(resident_kernel<T, LOP, RREG>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem_bytes) != cudaSuccess) {
+        cudaGetLastError();
+        return -100;
+    }
+    int occ = 0;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, resident_kernel<T, LOP, RREG>, RES_NT, pl.smem_bytes) != cudaSuccess || occ < 1) {
+        cudaGetLastError();
+        return -100;
+    }
+    ResidentArgs<T> ra;
+    PersistArgs<T>& a = ra.a;
+    a.r = w.r; a.pbuf[0] = w.p0; a.pbuf[1] = w.p1; a.delta = w.delta; a.S = w.S; a.Pbuf[0] = w.P; a.Pbuf[1] = w.P1;
+    a.link = w.link; a.wcode = w.wcode; a.flags = w.flags; a.K = K;
+    for (int i = 0; i < 3; ++i) a.t[i] = H.F[i] / H.Atot;
+    a.sc = w.sc; a.slots = w.slots;
+    a.timeout_ns = barrier_timeout_ns();
+    ra.gy = pl.gy; ra.gz = pl.gz; ra.ly = pl.ly; ra.lz = pl.lz; ra.zpad = pl.zpad; ra.pxs = pl.pxs; ra.dres = pl.dres; ra.rpt = pl.rpt;
+    // the halo messages take the place of the two p buffers, which this loop does not use (carve: p1 follows p0); no
+    // message of an earlier solve may carry a live epoch
+    ra.xchg = (unsigned long long*)w.p0;
+    CK(cudaMemsetAsync(w.p0, 0, (size_t)2 * (size_t)g.npad * sizeof(T), st));
+    CK(cudaMemsetAsync(w.slots, 0, PERSIST_SLOT_BYTES, st));
+    Geom gg = g;
+    void* params[2] = { (void*)&gg, (void*)&ra };
+    if (cudaLaunchCooperativeKernel((const void*)resident_kernel<T, LOP, RREG>, dim3((unsigned)G), dim3(RES_NT), params, pl.smem_bytes, st) != cudaSuccess) {
+        cudaGetLastError();
+        return -100;
+    }
+    g_launches.fetch_add(1, std::memory_order_relaxed);
+    return OMNI_OK;
+}
+
+template <typename T, bool LOP>
+int run_loop_resident(const Geom& g, const Workspace<T>& w, const HostConst& H, const Coef<T>& K, cudaStream_t st)
+{
+    const DevInfo di = device_info();
+    if (!di.coop || di.sms < 1) return -100;
+    if (g.npad >= (1LL << 31) || (long long)g.ny * g.nz * ((g.nx + 63) / 64) >= (1LL << 31)) return -100;
+    ResidentPlan pl;
+    if (!resident_plan(g, (int)sizeof(T), di.sms < 148 ? di.sms : 148, pl)) return -100;     // relaxed slots: room for 148 CTAs
+    if (pl.gy * pl.gz > 148 || pl.gy * pl.gz > RES_NT) return -100;          // relaxed slots: RES_SLOT_OFFSET
+    return pl.rreg ? launch_resident<T, LOP, true>(g, w, H, K, pl, st) : launch_resident<T, LOP, false>(g, w, H, K, pl, st);
+}
+
 // Single-reduction CG for the fixed-point solve (omni_persist1.cuh): the persistent kernel with one grid barrier per
 // iteration.  Four more vectors (double-buffered r, w, s and p) come from the pool.  -100: cannot be co-scheduled.
 template <typename T, int NT>
@@ -1208,6 +1259,10 @@ int solve_ws(int nx, int ny, int nz, double dx, double dy, double dz, const T* g
         mode = -2;
     }
     // lop: the CG kernels apply L instead of M (omni_solve_direct); everything else -- K2, scalars, loop control -- is shared
+    if (mode == 5) {
+        rc = lop ? run_loop_resident<T, true>(g, w, H, K, st) : run_loop_resident<T, false>(g, w, H, K, st);
+        if (rc == -100) mode = 3;
+    }
     if (mode == 3) {
         // fixed-point solve with omni_options::single_reduction: the one-barrier-per-iteration kernel (L = L^T only)
         if (lop && opt.single_reduction) rc = run_loop_persist1<T>(g, w, H, K, st);
@@ -1911,7 +1966,7 @@ int solve_ex(int nx, int ny, int nz, double dx, double dy, double dz, const T* g
     CallOpts c = current_opts();
     if (o) {
         if (o->struct_size != sizeof(omni_options)) return OMNI_ERR_INVALID_ARG;
-        if (o->loop_mode > 4 || o->loop_mode < -1 || o->hist_capacity < 0) return OMNI_ERR_INVALID_ARG;
+        if (o->loop_mode > 5 || o->loop_mode < -1 || o->hist_capacity < 0) return OMNI_ERR_INVALID_ARG;
         if (o->hist_capacity == 0 && (o->d_hist_eps_R || o->d_hist_cg_iters || o->d_hist_eps_P)) return OMNI_ERR_INVALID_ARG;
         if (o->loop_mode >= 0) c.loop_mode = o->loop_mode;
         c.hist = o->d_hist_eps_R; c.hist_k = o->d_hist_cg_iters; c.hist_p = o->d_hist_eps_P; c.hist_cap = o->hist_capacity;
@@ -2259,7 +2314,7 @@ void omni_release_memory(void)
 
 int omni_set_loop_mode(int mode)
 {
-    if (mode < 0 || mode > 4) return g_loop_mode.load();
+    if (mode < 0 || mode > 5) return g_loop_mode.load();
     return g_loop_mode.exchange(mode);
 }
 
@@ -2279,4 +2334,14 @@ const char* omni_status_string(int status)
 
 int omni_version(void) { return 106; }   // 101: omni_solve_guess_*, omni_set_history, omni_rans_source_*, omni_compressible_rans_source_*
 
+#ifdef OMNI_RES_TRACE
+int omni_debug_res_trace(unsigned long long* out, int reset)
+{
+    unsigned long long z[16] = { 0 };
+    if (cudaMemcpyFromSymbol(out, omni::g_res_trace, sizeof(z)) != cudaSuccess) return -1;
+    z[15] = (unsigned long long)(reset > 0 ? reset - 1 : 0);      // reset = 1 + index of the CTA to trace
+    if (reset && cudaMemcpyToSymbol(omni::g_res_trace, z, sizeof(z)) != cudaSuccess) return -1;
+    return 0;
+}
+#endif
 }  // extern "C"

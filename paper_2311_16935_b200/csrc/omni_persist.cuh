@@ -29,14 +29,21 @@ constexpr int ST_BARRIER_TIMEOUT = -2;      // = OMNI_ERR_CUDA: a CTA waited lon
 #ifndef OMNI_PERSIST_LDCG
 #define OMNI_PERSIST_LDCG 0
 #endif
-template <typename T> __device__ __forceinline__ T ldd(const T* p) { return OMNI_PERSIST_LDCG ? __ldcg(p) : *reinterpret_cast<const volatile T*>(p); }
+template <typename T> __device__ __forceinline__ T ldd(const T* p)
+{
+    if (OMNI_PERSIST_LDCG == 2) return *p;
+    return OMNI_PERSIST_LDCG ? __ldcg(p) : *reinterpret_cast<const volatile T*>(p);
+}
 template <typename T, int V>
 __device__ __forceinline__ void ldcg_chunk(const T* p, T (&v)[V])
 {
     constexpr int BYTES = V * (int)sizeof(T);
     static_assert(BYTES == 8 || BYTES == 16, "persistent path moves 8- or 16-byte chunks");
     // plain (coherent) loads: never the non-coherent path, these arrays are rewritten by other CTAs between phases
-    if constexpr (BYTES == 8) {
+    if constexpr (OMNI_PERSIST_LDCG == 2) {
+        if constexpr (BYTES == 8) { const uint2 u = *reinterpret_cast<const uint2*>(p); memcpy(v, &u, 8); }
+        else { const uint4 u = *reinterpret_cast<const uint4*>(p); memcpy(v, &u, 16); }
+    } else if constexpr (BYTES == 8) {
         uint2 u;
         if (OMNI_PERSIST_LDCG) u = __ldcg(reinterpret_cast<const uint2*>(p));
         else asm volatile("ld.global.v2.u32 {%0, %1}, [%2];" : "=r"(u.x), "=r"(u.y) : "l"(p) : "memory");
@@ -78,20 +85,25 @@ struct GridSync {
     unsigned long long timeout_ns;
 };
 
+template <bool RELAXED = false>
 __device__ __forceinline__ void slot_publish(double* slot, double v, unsigned int tag)
 {
     const unsigned long long b = ((unsigned long long)__double_as_longlong(v) & ~1ULL) | tag;
-    asm volatile("st.release.gpu.global.u64 [%0], %1;" :: "l"(slot), "l"(b) : "memory");
+    if (RELAXED) asm volatile("st.relaxed.gpu.global.u64 [%0], %1;" :: "l"(slot), "l"(b) : "memory");
+    else asm volatile("st.release.gpu.global.u64 [%0], %1;" :: "l"(slot), "l"(b) : "memory");
 }
+// RELAXED (omni_resident.cuh): no data other than the slot itself crosses the barrier, so neither side needs a fence
+template <bool RELAXED = false>
 __device__ __forceinline__ bool slot_poll(const double* slot, unsigned int tag, double& v)
 {
     unsigned long long b;
-    asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(b) : "l"(slot) : "memory");
+    if (RELAXED) asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(b) : "l"(slot) : "memory");
+    else asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(b) : "l"(slot) : "memory");
     v = __longlong_as_double((long long)(b & ~1ULL));
     return (unsigned int)(b & 1ULL) == tag;
 }
 
-template <int NACC, int NT>
+template <int NACC, int NT, bool RELAXED = false>
 __device__ __forceinline__ bool grid_allreduce(GridSync& gs, double* slots, const double (&acc)[NACC], double (&tot)[NACC])
 {
     constexpr int R = NACC - 1;                                    // region: 0 for one accumulator, 1 for two
@@ -111,7 +123,7 @@ __device__ __forceinline__ bool grid_allreduce(GridSync& gs, double* slots, cons
 #pragma unroll
         for (int i = 0; i < NACC; ++i) {
             const double s = warp_sum(lane < NW ? gs.red[i * (NW + 1) + lane] : 0.0);
-            if (lane == 0) slot_publish(my + (size_t)i * G + blockIdx.x, s, tag);
+            if (lane == 0) slot_publish<RELAXED>(my + (size_t)i * G + blockIdx.x, s, tag);
         }
 #pragma unroll
         for (int i = 0; i < NACC; ++i) {
@@ -124,14 +136,14 @@ __device__ __forceinline__ bool grid_allreduce(GridSync& gs, double* slots, cons
                 for (int u = 0; u < PB; ++u) {
                     const unsigned int b = b0 + 32 * u;
                     v[u] = 0.0;
-                    got[u] = (b >= G) || slot_poll(my + (size_t)i * G + b, tag, v[u]);
+                    got[u] = (b >= G) || slot_poll<RELAXED>(my + (size_t)i * G + b, tag, v[u]);
                 }
 #pragma unroll
                 for (int u = 0; u < PB; ++u) {
                     if (!got[u]) {
                         const double* sl = my + (size_t)i * G + b0 + 32 * u;
                         const unsigned long long t0 = global_timer_ns();
-                        while (!slot_poll(sl, tag, v[u])) {
+                        while (!slot_poll<RELAXED>(sl, tag, v[u])) {
                             if (global_timer_ns() - t0 > gs.timeout_ns) { ok = 0; break; }
                         }
                     }

@@ -81,7 +81,7 @@ def test_source_and_operator_steps(oracle, dtype, shape, frac):
 
 
 # omni_set_loop_mode; the default (0) picks one of the three by grid size
-LOOPS = {"graph": 2, "persistent": 3, "loopk": 4}
+LOOPS = {"graph": 2, "persistent": 3, "loopk": 4, "resident": 5}
 
 
 @pytest.fixture(params=list(LOOPS))
