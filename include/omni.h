@@ -94,7 +94,7 @@ int omni_solve_host_f32(int nx, int ny, int nz, double dx, double dy, double dz,
  * with everything that is otherwise a process-wide setting passed IN THE CALL: two concurrent solves (threads,
  * streams) never share a history buffer or a loop mode.  options == NULL: the process-wide defaults.  All pointers in
  * omni_options are DEVICE memory owned by the caller and must stay valid until the solve has finished on `stream`.
- *   loop_mode       -1: the process-wide setting (omni_set_loop_mode); 0..4 as described there
+ *   loop_mode       -1: the process-wide setting (omni_set_loop_mode); 0..5 as described there
  *   d_hist_eps_R    [hist_capacity] doubles: eps_R (Eq. 41 :442) at the i-th outer residual check (i = 0: first guess)
  *   d_hist_cg_iters [hist_capacity] ints: CG iterations of the outer iteration that led to check i (0 for i = 0)
  *   d_hist_eps_P    [hist_capacity] doubles: the pressure-update metric eps_P = ||P^i - P^(i-1)|| / ||P^i|| (Eq. 40 :438)
@@ -382,7 +382,8 @@ int omni_residual_f32(int nx, int ny, int nz, double dx, double dy, double dz,
 /* Kernel launches issued by this library since the last reset (counts launches on any thread; for bench.py). */
 long long omni_launch_count(int reset);
 /* How the iteration (Alg. 1) is driven; every mode runs the same per-cell arithmetic.
- *   0  automatic (default): mode 3 for grids of up to 1.5 M padded cells, mode 2 above
+ *   0  automatic (default): mode 5 where the grid fits it with r in shared memory, else mode 3 for grids of up to
+ *      1.5 M padded cells, mode 2 above
  *   1  host-driven loop that synchronises once per outer iteration (debug / per-kernel profiling)
  *   2  CUDA graph with device-side conditional WHILE nodes around the tile kernels K2 / K3 / K4
  *   3  one persistent cooperative kernel: phases separated by grid barriers that double as the reductions
@@ -390,8 +391,15 @@ long long omni_launch_count(int reset);
  *   4  the whole iteration as ONE cooperative launch of the tile kernels' TMA pipeline (one column per CTA, the same
  *      grid barriers between the K2 / K3 / K4 phases); correct and deterministic, measured slower than mode 2 at every
  *      size (profiles/r2_loop_and_rows.md), never chosen automatically; falls back to mode 2 if its grid does not fit
- * The environment variable OMNI_PERSIST_MAX_CELLS overrides the automatic threshold.  Modes 1 and 2 give bit-identical
- * results; modes 3 and 4 sum their reductions in a different (fixed) order.  Returns the previous mode; other values are ignored. */
+ *   5  mode 3 with the CG vectors resident on the SMs for the whole inner solve: every CTA owns a box of grid rows, p of
+ *      the box and its halo in shared memory, r in shared memory or (where p alone fills it: 128^3 fp64) in registers;
+ *      per CG iteration only the halo rows of r travel, as self-validating messages, and the two grid barriers carry
+ *      nothing but the reduction (no fence).  For grids of up to about 2 M cells whose rows are at most 2048 (fp32) /
+ *      1024 (fp64) cells long; falls back to mode 3 where the grid does not fit.  Uses the workspace's two p vectors as
+ *      message buffer.
+ * The environment variable OMNI_PERSIST_MAX_CELLS overrides the threshold between modes 3 and 2, OMNI_RESIDENT=0 keeps mode
+ * 5 out of the automatic choice.  Modes 1 and 2 give bit-identical results; modes 3, 4 and 5 sum their reductions in a
+ * different (fixed) order.  Returns the previous mode; other values are ignored. */
 int omni_set_loop_mode(int mode);
 /* Convergence history (the momentum residual of Eq. 41, plotted in Fig. 10-13): registers a caller-owned
  * DEVICE buffer of `capacity` doubles that every solve enqueued afterwards fills on the device -- entry i = eps_R =

@@ -1175,8 +1175,9 @@ int run_loop_persist1(const Geom& g, const Workspace<T>& w, const HostConst& H, 
                                                 : launch_persist1<T, 1024>(g, w, H, K, di.sms, st);
 }
 
-// loop selection: g_loop_mode 0 = automatic (persistent kernel for grids up to OMNI_PERSIST_MAX_CELLS padded cells, CUDA graph above),
-// 1 = host-driven, 2 = CUDA graph, 3 = persistent kernel
+// loop selection: g_loop_mode 0 = automatic (SM-resident kernel where the grid fits the SMs, else the persistent kernel for grids up
+// to OMNI_PERSIST_MAX_CELLS padded cells, CUDA graph above), 1 = host-driven, 2 = CUDA graph, 3 = persistent kernel,
+// 4 = whole-solve tile loop kernel, 5 = SM-resident kernel
 long long persist_max_cells()
 {
     static long long v = -1;
@@ -1186,6 +1187,16 @@ long long persist_max_cells()
         if (v < 0) v = 0;
     }
     return v;
+}
+
+bool resident_enabled()
+{
+    static int v = -1;
+    if (v < 0) {
+        const char* e = getenv("OMNI_RESIDENT");
+        v = (e && atoi(e) == 0) ? 0 : 1;
+    }
+    return v != 0;
 }
 
 long long loopk_max_cells()
@@ -1246,7 +1257,17 @@ int solve_ws(int nx, int ny, int nz, double dx, double dy, double dz, const T* g
     }
 
     int mode = opt.loop_mode;
-    if (mode == 0) mode = (g.npad <= persist_max_cells()) ? 3 : (g.npad <= loopk_max_cells()) ? 4 : 2;
+    if (mode == 0) {
+        // automatic: the SM-resident loop wherever p AND r fit the SMs' shared memory (measured 1.1 - 2.2 x the persistent
+        // or graph loop on every such grid; with r in registers it does not win yet), else by size as before
+        ResidentPlan pl;
+        const DevInfo di = device_info();
+        const bool one_red = lop && opt.single_reduction;          // that option is the persistent loop's
+        if (!one_red && !pcg && resident_enabled() && di.coop && resident_plan(g, (int)sizeof(T), di.sms < 148 ? di.sms : 148, pl) && !pl.rreg)
+            mode = 5;
+        else
+            mode = (g.npad <= persist_max_cells()) ? 3 : (g.npad <= loopk_max_cells()) ? 4 : 2;
+    }
     MgHier<T> mg;
     mg.mem = nullptr; mg.launches_per_cycle = 0;
     if (pcg) {
