@@ -1072,16 +1072,16 @@ int run_loop_persist(const Geom& g, const Workspace<T>& w, const HostConst& H, c
 
 // SM-resident loop (omni_resident.cuh): the persistent loop with p in shared memory and r in registers for the whole
 // inner solve.  Returns -100 if the grid does not fit the SMs or the device cannot co-schedule it.
-template <typename T, bool LOP, bool RREG>
+template <typename T, bool LOP, int RM>
 int launch_resident(const Geom& g, const Workspace<T>& w, const HostConst& H, const Coef<T>& K, const ResidentPlan& pl, cudaStream_t st)
 {
     const int G = pl.gy * pl.gz;
-    if (cudaFuncSetAttribute(resident_kernel<T, LOP, RREG>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem_bytes) != cudaSuccess) {
+    if (cudaFuncSetAttribute(resident_kernel<T, LOP, RM>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem_bytes) != cudaSuccess) {
         cudaGetLastError();
         return -100;
     }
     int occ = 0;
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, resident_kernel<T, LOP, RREG>, RES_NT, pl.smem_bytes) != cudaSuccess || occ < 1) {
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, resident_kernel<T, LOP, RM>, RES_NT, pl.smem_bytes) != cudaSuccess || occ < 1) {
         cudaGetLastError();
         return -100;
     }
@@ -1100,7 +1100,7 @@ int launch_resident(const Geom& g, const Workspace<T>& w, const HostConst& H, co
     CK(cudaMemsetAsync(w.slots, 0, PERSIST_SLOT_BYTES, st));
     Geom gg = g;
     void* params[2] = { (void*)&gg, (void*)&ra };
-    if (cudaLaunchCooperativeKernel((const void*)resident_kernel<T, LOP, RREG>, dim3((unsigned)G), dim3(RES_NT), params, pl.smem_bytes, st) != cudaSuccess) {
+    if (cudaLaunchCooperativeKernel((const void*)resident_kernel<T, LOP, RM>, dim3((unsigned)G), dim3(RES_NT), params, pl.smem_bytes, st) != cudaSuccess) {
         cudaGetLastError();
         return -100;
     }
@@ -1117,7 +1117,10 @@ int run_loop_resident(const Geom& g, const Workspace<T>& w, const HostConst& H, 
     ResidentPlan pl;
     if (!resident_plan(g, (int)sizeof(T), di.sms < 148 ? di.sms : 148, pl)) return -100;     // relaxed slots: room for 148 CTAs
     if (pl.gy * pl.gz > 148 || pl.gy * pl.gz > RES_NT) return -100;          // relaxed slots: RES_SLOT_OFFSET
-    return pl.rreg ? launch_resident<T, LOP, true>(g, w, H, K, pl, st) : launch_resident<T, LOP, false>(g, w, H, K, pl, st);
+    if (!pl.rreg) return launch_resident<T, LOP, 0>(g, w, H, K, pl, st);
+    static const int rmode = getenv("OMNI_RESIDENT_R") ? atoi(getenv("OMNI_RESIDENT_R")) : 2;
+    if (rmode == 1 && pl.rpt <= RES_NI) return launch_resident<T, LOP, 1>(g, w, H, K, pl, st);
+    return launch_resident<T, LOP, 2>(g, w, H, K, pl, st);
 }
 
 // Single-reduction CG for the fixed-point solve (omni_persist1.cuh): the persistent kernel with one grid barrier per
@@ -1258,12 +1261,12 @@ int solve_ws(int nx, int ny, int nz, double dx, double dy, double dz, const T* g
 
     int mode = opt.loop_mode;
     if (mode == 0) {
-        // automatic: the SM-resident loop wherever p AND r fit the SMs' shared memory (measured 1.1 - 2.2 x the persistent
-        // or graph loop on every such grid; with r in registers it does not win yet), else by size as before
+        // automatic: the SM-resident loop wherever p fits the SMs' shared memory (measured 1.1 - 2.2 x the persistent or
+        // graph loop where r fits beside it, 1.2 - 1.35 x at 128^3 fp64 where r stays in L2), else by size as before
         ResidentPlan pl;
         const DevInfo di = device_info();
         const bool one_red = lop && opt.single_reduction;          // that option is the persistent loop's
-        if (!one_red && !pcg && resident_enabled() && di.coop && resident_plan(g, (int)sizeof(T), di.sms < 148 ? di.sms : 148, pl) && !pl.rreg)
+        if (!one_red && !pcg && resident_enabled() && di.coop && resident_plan(g, (int)sizeof(T), di.sms < 148 ? di.sms : 148, pl))
             mode = 5;
         else
             mode = (g.npad <= persist_max_cells()) ? 3 : (g.npad <= loopk_max_cells()) ? 4 : 2;

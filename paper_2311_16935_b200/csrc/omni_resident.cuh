@@ -147,12 +147,14 @@ __device__ __forceinline__ void res_for_rows(int nrt, F&& f)
     }
 }
 
-// RREG: r in registers (p alone fills the shared memory: 128^3 fp64), else r in shared memory beside p
-template <typename T, bool LOP, bool RREG>
+// where r of the box lives -- RM 0: shared memory, beside p; 1: registers (p alone fills the shared memory: 128^3 fp64);
+// 2: the global r array (through L2; same grids as 1)
+template <typename T, bool LOP, int RM>
 __global__ void __launch_bounds__(RES_NT, 1)
 resident_kernel(const Geom g, const ResidentArgs<T> ra)
 {
     constexpr int V = 16 / (int)sizeof(T), NT = RES_NT, NW = NT / 32, MW = (int)sizeof(T) / 4;
+    constexpr bool RREG = RM == 1;
     extern __shared__ __align__(16) unsigned char res_smem[];
     __shared__ double red[2 * (NW + 1)];
     __shared__ double sv[PERSIST_MAX_CTAS > NT ? NT : PERSIST_MAX_CTAS];
@@ -179,7 +181,7 @@ resident_kernel(const Geom g, const ResidentArgs<T> ra)
     const int p_elems = (ra.lz + 2 * zpad) * pls;
     // r (unless RREG) and delta (dres only) of this thread's row `it` at [(it * NT + tid) * V]
     T* const rsm = ps + p_elems;
-    T* const ds = rsm + (RREG ? 0 : ra.rpt * NT * V);
+    T* const ds = rsm + (RM != 0 ? 0 : ra.rpt * NT * V);
     // a thread owns x chunk xc of the rows [r_lo, r_lo + nrt) of the box (rows numbered y-fastest): NT / cpr row groups
     const int nrg = NT / cpr, grp = tid / cpr, xc = tid - grp * cpr, x = xc * V;
     const int rpg = (nrows + nrg - 1) / nrg;
@@ -230,20 +232,24 @@ resident_kernel(const Geom g, const ResidentArgs<T> ra)
     double rho = 0.0, beta = 0.0, alpha = 0.0, gamma = 0.0, epsR2 = 0.0, alpha_prev = 0.0;
     bool dzero = sc->dzero != 0;
     T rr[RREG ? RES_NI : 1][V];
-    auto r_ld = [&](int it, T (&v)[V]) {
-        if constexpr (RREG) {
+    auto r_ld = [&](int it, int jl, int kl, T (&v)[V]) {
+        if constexpr (RM == 1) {
 #pragma unroll
             for (int c = 0; c < V; ++c) v[c] = rr[it][c];
-        } else {
+        } else if constexpr (RM == 0) {
             ld_chunk<T, V>(rsm + (size_t)(it * NT + tid) * V, v);
+        } else {
+            ld_chunk<T, V>(a.r + cell_idx(jl, kl), v);             // this thread's own store (or K2's, behind a fenced barrier)
         }
     };
-    auto r_st = [&](int it, const T (&v)[V]) {
-        if constexpr (RREG) {
+    auto r_st = [&](int it, int jl, int kl, const T (&v)[V]) {
+        if constexpr (RM == 1) {
 #pragma unroll
             for (int c = 0; c < V; ++c) rr[it][c] = v[c];
-        } else {
+        } else if constexpr (RM == 0) {
             st_chunk<T, V>(rsm + (size_t)(it * NT + tid) * V, v);
+        } else {
+            st_chunk<T, V>(a.r + cell_idx(jl, kl), v);
         }
     };
 #ifdef OMNI_RES_TRACE
@@ -324,9 +330,11 @@ resident_kernel(const Geom g, const ResidentArgs<T> ra)
             st_chunk<T, V>(ps + i, z);
         }
         RES_ROWS_BEGIN
-            T v[V];
-            ldcg_chunk<T, V>(a.r + cell_idx(jl, kl), v);
-            r_st(it, v);
+            if constexpr (RM != 2) {
+                T v[V];
+                ldcg_chunk<T, V>(a.r + cell_idx(jl, kl), v);
+                r_st(it, jl, kl, v);
+            }
             (void)off;
         RES_ROWS_END
         __syncthreads();
@@ -390,7 +398,7 @@ resident_kernel(const Geom g, const ResidentArgs<T> ra)
                 RES_ROWS_BEGIN
                     T p[V], r[V];
                     ld_chunk<T, V>(ps + off, p);
-                    r_ld(it, r);
+                    r_ld(it, jl, kl, r);
 #pragma unroll
                     for (int c = 0; c < V; ++c) p[c] = r[c] + b * p[c];
                     st_chunk<T, V>(ps + off, p);
@@ -429,7 +437,7 @@ resident_kernel(const Geom g, const ResidentArgs<T> ra)
                 RES_ROWS_BEGIN
                     T q[V], r[V];
                     stencil(off, it, jl, kl, q);
-                    r_ld(it, r);
+                    r_ld(it, jl, kl, r);
                     if (ra.dres) {
                         T d[V];
                         T* dp = ds + (size_t)(it * NT + tid) * V;
@@ -449,7 +457,7 @@ resident_kernel(const Geom g, const ResidentArgs<T> ra)
                     }
 #pragma unroll
                     for (int c = 0; c < V; ++c) r[c] -= al * q[c];
-                    r_st(it, r);
+                    r_st(it, jl, kl, r);
                     acc[0] += dot_chunk(r, r);
                     if ((bndm >> it) & 1u) msg_send<T, V>(ra.xchg + cell_idx(jl, kl) * MW, r, epoch);
                     RES_CARRY_NEXT
@@ -508,7 +516,7 @@ resident_kernel(const Geom g, const ResidentArgs<T> ra)
 
 // ---- host side: the box decomposition.  Returns false if the grid does not fit the SMs' memory.
 struct ResidentPlan {
-    int gy, gz, ly, lz, zpad, pxs, dres, rpt, rreg;
+    int gy, gz, ly, lz, zpad, pxs, dres, rpt, rreg;    // rreg: r does not fit the shared memory beside p
     unsigned smem_bytes;
 };
 
@@ -532,7 +540,6 @@ inline bool resident_plan(const Geom& g, int elem_size, int nsm, ResidentPlan& b
         const long long v_bytes = rpt * RES_NT * 16;               // one more box vector (r, delta) in shared memory
         if (p_bytes > RES_SMEM_MAX) continue;
         const bool rreg = p_bytes + v_bytes > RES_SMEM_MAX;
-        if (rreg && rpt > RES_NI) continue;
         const long long halo_rows = (gy > 1 ? 2 * lz : 0) + ((three && gz > 1) ? 2 * ly : 0);
         // time of an iteration ~ rows a thread walks three times (update, two stencils) + halo rows the CTA updates
         const double cost = 3.0 * (double)rpt * (double)nrg + (double)halo_rows;
