@@ -1092,7 +1092,7 @@ int launch_resident(const Geom& g, const Workspace<T>& w, const HostConst& H, co
     for (int i = 0; i < 3; ++i) a.t[i] = H.F[i] / H.Atot;
     a.sc = w.sc; a.slots = w.slots;
     a.timeout_ns = barrier_timeout_ns();
-    ra.gy = pl.gy; ra.gz = pl.gz; ra.ly = pl.ly; ra.lz = pl.lz; ra.zpad = pl.zpad; ra.pxs = pl.pxs; ra.dres = pl.dres; ra.rpt = pl.rpt;
+    ra.gy = pl.gy; ra.gz = pl.gz; ra.ly = pl.ly; ra.lz = pl.lz; ra.zpad = pl.zpad; ra.pxs = pl.pxs; ra.dres = pl.dres; ra.qres = pl.qres; ra.rpt = pl.rpt;
     // the halo messages take the place of the two p buffers, which this loop does not use (carve: p1 follows p0); no
     // message of an earlier solve may carry a live epoch
     ra.xchg = (unsigned long long*)w.p0;

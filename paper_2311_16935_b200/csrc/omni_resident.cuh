@@ -54,6 +54,7 @@ struct ResidentArgs {
     int zpad;          // 1: 3D operator, the p array has a halo plane below and above
     int pxs;           // row pitch of the p array in cells: px + 2 chunks (a zero chunk left and right of every row)
     int dres;          // 1: delta lives in shared memory
+    int qres;          // 1: q = Op p of K3 is kept in shared memory for K4 (no second stencil pass)
     int rpt;           // rows per thread the shared r / delta arrays are laid out for
 };
 
@@ -67,13 +68,17 @@ __device__ __forceinline__ void msg_send(unsigned long long* m, const T (&v)[V],
     asm volatile("st.relaxed.gpu.global.v2.u64 [%0], {%1, %2};" :: "l"(m), "l"(e | w[0]), "l"(e | w[1]) : "memory");
     asm volatile("st.relaxed.gpu.global.v2.u64 [%0], {%1, %2};" :: "l"(m + 2), "l"(e | w[2]), "l"(e | w[3]) : "memory");
 }
-template <typename T, int V>
-__device__ __forceinline__ bool msg_try(const unsigned long long* m, T (&v)[V], uint32_t epoch)
+// the loads (in flight until msg_decode looks at them) ...
+__device__ __forceinline__ void msg_load(const unsigned long long* m, unsigned long long (&b)[4])
 {
-    unsigned long long b[4];
-    // weak L2 loads: every 8-byte word validates itself through its epoch
-    asm volatile("ld.global.cg.v2.u64 {%0, %1}, [%2];" : "=l"(b[0]), "=l"(b[1]) : "l"(m) : "memory");
-    asm volatile("ld.global.cg.v2.u64 {%0, %1}, [%2];" : "=l"(b[2]), "=l"(b[3]) : "l"(m + 2) : "memory");
+    // ld.global.cg is a strong L2 load on sm_100a (LDG.STRONG.GPU); every 8-byte word validates itself through its epoch
+    asm volatile("ld.relaxed.gpu.global.v2.u64 {%0, %1}, [%2];" : "=l"(b[0]), "=l"(b[1]) : "l"(m) : "memory");
+    asm volatile("ld.relaxed.gpu.global.v2.u64 {%0, %1}, [%2];" : "=l"(b[2]), "=l"(b[3]) : "l"(m + 2) : "memory");
+}
+// ... and their check: true iff all four words carry the expected epoch
+template <typename T, int V>
+__device__ __forceinline__ bool msg_decode(const unsigned long long (&b)[4], T (&v)[V], uint32_t epoch)
+{
     uint32_t w[4];
     bool ok = true;
 #pragma unroll
@@ -83,6 +88,13 @@ __device__ __forceinline__ bool msg_try(const unsigned long long* m, T (&v)[V], 
     }
     memcpy(v, w, 16);
     return ok;
+}
+template <typename T, int V>
+__device__ __forceinline__ bool msg_try(const unsigned long long* m, T (&v)[V], uint32_t epoch)
+{
+    unsigned long long b[4];
+    msg_load(m, b);
+    return msg_decode<T, V>(b, v, epoch);
 }
 
 // Relaxed grid barrier + all-reduce of one fp64 accumulator, for barriers that carry nothing but their own slot: no
@@ -182,6 +194,7 @@ resident_kernel(const Geom g, const ResidentArgs<T> ra)
     // r (unless RREG) and delta (dres only) of this thread's row `it` at [(it * NT + tid) * V]
     T* const rsm = ps + p_elems;
     T* const ds = rsm + (RM != 0 ? 0 : ra.rpt * NT * V);
+    T* const qs = ds + ra.rpt * NT * V;                    // qres only (implies dres)
     // a thread owns x chunk xc of the rows [r_lo, r_lo + nrt) of the box (rows numbered y-fastest): NT / cpr row groups
     const int nrg = NT / cpr, grp = tid / cpr, xc = tid - grp * cpr, x = xc * V;
     const int rpg = (nrows + nrg - 1) / nrg;
@@ -346,6 +359,8 @@ resident_kernel(const Geom g, const ResidentArgs<T> ra)
             {
                 const T b = (T)beta;
                 const uint32_t epoch = (uint32_t)cg_total;          // what the neighbours' last K4 stamped
+                // the halo, four chunks per thread in flight (updating the box's rows under these loads was tried: the
+                // registers it takes spill elsewhere and cost more than the latency it hides)
                 for (int h0 = tid; h0 < nhc; h0 += 4 * NT) {
                     T hr[4][V];
                     int hoff[4];
@@ -415,6 +430,7 @@ resident_kernel(const Geom g, const ResidentArgs<T> ra)
                     T q[V];
                     stencil(off, it, jl, kl, q);
                     acc[0] += dot_chunk(vc, q);
+                    if (ra.qres) st_chunk<T, V>(qs + (size_t)(it * NT + tid) * V, q);
                     RES_CARRY_NEXT
                 RES_ROWS_END
                 double tot[1];
@@ -436,7 +452,12 @@ resident_kernel(const Geom g, const ResidentArgs<T> ra)
                 carry = false;
                 RES_ROWS_BEGIN
                     T q[V], r[V];
-                    stencil(off, it, jl, kl, q);
+                    if (ra.qres) {
+                        ld_chunk<T, V>(qs + (size_t)(it * NT + tid) * V, q);
+                        ld_chunk<T, V>(ps + off, vc);
+                    } else {
+                        stencil(off, it, jl, kl, q);
+                    }
                     r_ld(it, jl, kl, r);
                     if (ra.dres) {
                         T d[V];
@@ -460,7 +481,7 @@ resident_kernel(const Geom g, const ResidentArgs<T> ra)
                     r_st(it, jl, kl, r);
                     acc[0] += dot_chunk(r, r);
                     if ((bndm >> it) & 1u) msg_send<T, V>(ra.xchg + cell_idx(jl, kl) * MW, r, epoch);
-                    RES_CARRY_NEXT
+                    if (!ra.qres) { RES_CARRY_NEXT }
                 RES_ROWS_END
                 double tot[1];
                 RES_T(4);
@@ -516,7 +537,7 @@ resident_kernel(const Geom g, const ResidentArgs<T> ra)
 
 // ---- host side: the box decomposition.  Returns false if the grid does not fit the SMs' memory.
 struct ResidentPlan {
-    int gy, gz, ly, lz, zpad, pxs, dres, rpt, rreg;    // rreg: r does not fit the shared memory beside p
+    int gy, gz, ly, lz, zpad, pxs, dres, qres, rpt, rreg;    // rreg: r does not fit the shared memory beside p
     unsigned smem_bytes;
 };
 
@@ -548,7 +569,8 @@ inline bool resident_plan(const Geom& g, int elem_size, int nsm, ResidentPlan& b
             best.gy = gy; best.gz = gz; best.ly = (int)ly; best.lz = (int)lz; best.zpad = zpad; best.pxs = (int)pxs;
             best.rpt = (int)rpt; best.rreg = rreg ? 1 : 0;
             best.dres = (!rreg && p_bytes + 2 * v_bytes <= RES_SMEM_MAX) ? 1 : 0;
-            best.smem_bytes = (unsigned)(p_bytes + (rreg ? 0 : v_bytes) + (best.dres ? v_bytes : 0));
+            best.qres = (!rreg && p_bytes + 3 * v_bytes <= RES_SMEM_MAX) ? 1 : 0;
+            best.smem_bytes = (unsigned)(p_bytes + (rreg ? 0 : v_bytes) + (best.dres ? v_bytes : 0) + (best.qres ? v_bytes : 0));
         }
     }
     return best_cost >= 0.0;
