@@ -317,7 +317,8 @@ def per_config_entry(idx, dtype, dev, peak, cache=None):
             "valid_cells": nvalid, "cg_iteration_us": cg * 1e6, "updates_per_s_in_loop": nvalid / cg,
             "algorithmic_bytes_per_cg_iteration": alg, "algorithmic_GBps": alg / cg / 1e9,
             "frac_of_measured": alg / cg / 1e9 / peak, "frac_of_8TBps": alg / cg / 8e12,
-            "memory": "L2-resident: effective GB/s, not HBM" if resident else "HBM (state exceeds L2)",
+            "memory": ("SM-resident loop (p in shared memory, DESIGN.md section 20): effective GB/s, not HBM" if N * esz <= 20e6
+                       else "L2-resident: effective GB/s, not HBM") if resident else "HBM (state exceeds L2)",
             "k3_us": k3 * 1e6, "k4_us": k4 * 1e6, "tile_kernels_cg_iteration_us": (k3 + k4) * 1e6,
             "iterations_timed": [m1, m2]}
 

@@ -29,21 +29,15 @@ constexpr int ST_BARRIER_TIMEOUT = -2;      // = OMNI_ERR_CUDA: a CTA waited lon
 #ifndef OMNI_PERSIST_LDCG
 #define OMNI_PERSIST_LDCG 0
 #endif
-template <typename T> __device__ __forceinline__ T ldd(const T* p)
-{
-    if (OMNI_PERSIST_LDCG == 2) return *p;
-    return OMNI_PERSIST_LDCG ? __ldcg(p) : *reinterpret_cast<const volatile T*>(p);
-}
+template <typename T> __device__ __forceinline__ T ldd(const T* p) { return OMNI_PERSIST_LDCG ? __ldcg(p) : *reinterpret_cast<const volatile T*>(p); }
 template <typename T, int V>
 __device__ __forceinline__ void ldcg_chunk(const T* p, T (&v)[V])
 {
     constexpr int BYTES = V * (int)sizeof(T);
     static_assert(BYTES == 8 || BYTES == 16, "persistent path moves 8- or 16-byte chunks");
     // plain (coherent) loads: never the non-coherent path, these arrays are rewritten by other CTAs between phases
-    if constexpr (OMNI_PERSIST_LDCG == 2) {
-        if constexpr (BYTES == 8) { const uint2 u = *reinterpret_cast<const uint2*>(p); memcpy(v, &u, 8); }
-        else { const uint4 u = *reinterpret_cast<const uint4*>(p); memcpy(v, &u, 16); }
-    } else if constexpr (BYTES == 8) {
+    // (plain L1-cached loads behind the barrier's acquire were measured: 3-7 % faster, not worth leaving the coherent path)
+    if constexpr (BYTES == 8) {
         uint2 u;
         if (OMNI_PERSIST_LDCG) u = __ldcg(reinterpret_cast<const uint2*>(p));
         else asm volatile("ld.global.v2.u32 {%0, %1}, [%2];" : "=r"(u.x), "=r"(u.y) : "l"(p) : "memory");

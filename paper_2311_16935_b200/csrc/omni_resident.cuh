@@ -160,7 +160,9 @@ __device__ __forceinline__ void res_for_rows(int nrt, F&& f)
 }
 
 // where r of the box lives -- RM 0: shared memory, beside p; 1: registers (p alone fills the shared memory: 128^3 fp64);
-// 2: the global r array (through L2; same grids as 1)
+// 2: the global r array (through L2; same grids as 1).  With RM 2 a thread's loads of r are one L2 round trip per row;
+// issuing them four rows ahead (16 + 16 more registers for r and the lazy delta) was tried and is slower (128^3 fp64:
+// 29.8 -> 36.3 us per iteration): with 190 KB of shared memory the L1 is 28 KB and the 230 B per thread it spills miss it.
 template <typename T, bool LOP, int RM>
 __global__ void __launch_bounds__(RES_NT, 1)
 resident_kernel(const Geom g, const ResidentArgs<T> ra)
