@@ -401,6 +401,15 @@ long long omni_launch_count(int reset);
  * 5 out of the automatic choice.  Modes 1 and 2 give bit-identical results; modes 3, 4 and 5 sum their reductions in a
  * different (fixed) order.  Returns the previous mode; other values are ignored. */
 int omni_set_loop_mode(int mode);
+/* The box decomposition loop mode 5 would use for this grid (host only, no CUDA call): 1 and
+ * out[0..11] = { gy, gz (boxes along y and z, gy * gz CTAs), ly, lz (rows and planes of the largest box), dynamic shared
+ * memory in bytes, rows per thread, r does not fit beside p (0 / 1), delta in shared memory, q in shared memory, weights of
+ * the y and z cuts, padded row pitch in cells }; 0 if the grid does not fit the SMs (mode 5 then falls back to mode 3);
+ * OMNI_ERR_INVALID_ARG for bad arguments.  elem_size 4 or 8, nsm = SMs to plan for, lop = 1 for the operator L of
+ * omni_solve_direct.  omni_resident_split(n, parts, i, wface) = first cell of part i when an axis of n cells is cut into
+ * `parts` boxes with that weight (i = parts: n). */
+int omni_resident_plan(int nx, int ny, int nz, int elem_size, int nsm, int lop, int* out);
+int omni_resident_split(int n, int parts, int i, int wface);
 /* Convergence history (the momentum residual of Eq. 41, plotted in Fig. 10-13): registers a caller-owned
  * DEVICE buffer of `capacity` doubles that every solve enqueued afterwards fills on the device -- entry i = eps_R =
  * ||S - L P^i|| / ||S|| at the i-th outer residual check (i = 0: the first guess), written by the kernel that evaluates the
@@ -422,7 +431,7 @@ void omni_release_memory(void);
 int omni_profile_enable(int on);          /* returns the previous setting */
 void omni_profile_read(double* h_ms3, long long* h_count3, int reset);
 const char* omni_status_string(int status);
-int omni_version(void);                  /* 100 * major + minor; 101 added the _guess, _rans_source and history entry points, 102 omni_solve_pcg_*, 103 omni_solve_ex_* / omni_options, 104 omni_solve_slab_*, 105 omni_source_noalloc_*, 106 omni_solve_pcg_batch2d_* */
+int omni_version(void);                  /* 100 * major + minor; 101 added the _guess, _rans_source and history entry points, 102 omni_solve_pcg_*, 103 omni_solve_ex_* / omni_options, 104 omni_solve_slab_*, 105 omni_source_noalloc_*, 106 omni_solve_pcg_batch2d_*, 107 loop mode 5, omni_resident_plan */
 
 #ifdef __cplusplus
 }

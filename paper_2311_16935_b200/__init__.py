@@ -6,7 +6,7 @@ Importing the package does not load the library; the first call does, and fails 
 from .binding import (Info, OmniError, SYMBOLS, apply_M, constants, launch_count, lib, profile_enable,  # noqa: F401
                       profile_read, release_memory, residual, set_loop_mode, solve, solve_batch2d, solve_cascade, solve_direct, source, status_string, velocity_source, version, workspace_bytes,
                       rans_source, compressible_rans_source, solve_guess, set_history, solve_pcg, solve_ex, Options, slab_plan, solve_slab, solve_slab_rank, slab_comm_create,
-                      slab_comm_destroy, source_noalloc, source_noalloc_max_cells)
+                      slab_comm_destroy, source_noalloc, source_noalloc_max_cells, resident_plan, resident_split)
 
 # the C names, for callers who think in terms of include/omni.h
 omni_solve = solve

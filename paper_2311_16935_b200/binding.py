@@ -22,7 +22,7 @@ SYMBOLS = ["omni_solve_f64", "omni_solve_f32", "omni_workspace_bytes", "omni_sol
            "omni_source_noalloc_max_cells", "omni_solve_direct_batch2d_f64", "omni_solve_direct_batch2d_f32", "omni_solve_cascade_f64", "omni_solve_cascade_f32", "omni_velocity_source_f64", "omni_velocity_source_f32", "omni_rans_source_f64", "omni_rans_source_f32",
            "omni_compressible_rans_source_f64", "omni_compressible_rans_source_f32", "omni_constants", "omni_source_f64", "omni_source_f32",
            "omni_apply_M_f64", "omni_apply_M_f32", "omni_residual_f64", "omni_residual_f32", "omni_launch_count",
-           "omni_set_loop_mode", "omni_set_history", "omni_release_memory", "omni_profile_enable", "omni_profile_read", "omni_status_string", "omni_version"]
+           "omni_set_loop_mode", "omni_resident_plan", "omni_resident_split", "omni_set_history", "omni_release_memory", "omni_profile_enable", "omni_profile_read", "omni_status_string", "omni_version"]
 
 
 class OmniError(RuntimeError):
@@ -77,6 +77,24 @@ def set_loop_mode(mode):
     """0 = automatic (default), 1 = host-driven debug loop, 2 = CUDA-graph loop, 3 = persistent cooperative kernel
     (include/omni.h).  Returns the previous mode."""
     return int(lib().omni_set_loop_mode(C.c_int(mode)))
+
+
+def resident_plan(nx, ny, nz, dtype="f32", nsm=148, lop=False):
+    """omni_resident_plan: the box decomposition of the SM-resident loop (loop mode 5) for this grid, or None if the grid
+    does not fit the SMs.  Host only."""
+    out = (C.c_int * 12)()
+    rc = lib().omni_resident_plan(C.c_int(nx), C.c_int(ny), C.c_int(nz), C.c_int(4 if dtype == "f32" else 8), C.c_int(nsm),
+                                  C.c_int(1 if lop else 0), out)
+    if rc < 0:
+        raise OmniError(rc, "omni_resident_plan")
+    if rc == 0:
+        return None
+    keys = ("gy", "gz", "ly", "lz", "smem_bytes", "rows_per_thread", "r_outside_smem", "delta_in_smem", "q_in_smem", "wy", "wz", "px")
+    return dict(zip(keys, list(out)))
+
+
+def resident_split(n, parts, i, wface=0):
+    return int(lib().omni_resident_split(C.c_int(n), C.c_int(parts), C.c_int(i), C.c_int(wface)))
 
 
 def set_history(buf, cg_iters=None):

@@ -1092,7 +1092,7 @@ int launch_resident(const Geom& g, const Workspace<T>& w, const HostConst& H, co
     for (int i = 0; i < 3; ++i) a.t[i] = H.F[i] / H.Atot;
     a.sc = w.sc; a.slots = w.slots;
     a.timeout_ns = barrier_timeout_ns();
-    ra.gy = pl.gy; ra.gz = pl.gz; ra.ly = pl.ly; ra.lz = pl.lz; ra.zpad = pl.zpad; ra.pxs = pl.pxs; ra.dres = pl.dres; ra.qres = pl.qres; ra.rpt = pl.rpt;
+    ra.gy = pl.gy; ra.gz = pl.gz; ra.ly = pl.ly; ra.lz = pl.lz; ra.zpad = pl.zpad; ra.pxs = pl.pxs; ra.dres = pl.dres; ra.qres = pl.qres; ra.rpt = pl.rpt; ra.wy = pl.wy; ra.wz = pl.wz;
     // the halo messages take the place of the two p buffers, which this loop does not use (carve: p1 follows p0); no
     // message of an earlier solve may carry a live epoch
     ra.xchg = (unsigned long long*)w.p0;
@@ -1115,7 +1115,7 @@ int run_loop_resident(const Geom& g, const Workspace<T>& w, const HostConst& H, 
     if (!di.coop || di.sms < 1) return -100;
     if (g.npad >= (1LL << 31) || (long long)g.ny * g.nz * ((g.nx + 63) / 64) >= (1LL << 31)) return -100;
     ResidentPlan pl;
-    if (!resident_plan(g, (int)sizeof(T), di.sms < 148 ? di.sms : 148, pl)) return -100;     // relaxed slots: room for 148 CTAs
+    if (!resident_plan(g, (int)sizeof(T), di.sms < 148 ? di.sms : 148, LOP, pl)) return -100;     // relaxed slots: room for 148 CTAs
     if (pl.gy * pl.gz > 148 || pl.gy * pl.gz > RES_NT) return -100;          // relaxed slots: RES_SLOT_OFFSET
     if (!pl.rreg) return launch_resident<T, LOP, 0>(g, w, H, K, pl, st);
     static const int rmode = getenv("OMNI_RESIDENT_R") ? atoi(getenv("OMNI_RESIDENT_R")) : 2;
@@ -1266,7 +1266,7 @@ int solve_ws(int nx, int ny, int nz, double dx, double dy, double dz, const T* g
         ResidentPlan pl;
         const DevInfo di = device_info();
         const bool one_red = lop && opt.single_reduction;          // that option is the persistent loop's
-        if (!one_red && !pcg && resident_enabled() && di.coop && resident_plan(g, (int)sizeof(T), di.sms < 148 ? di.sms : 148, pl))
+        if (!one_red && !pcg && resident_enabled() && di.coop && resident_plan(g, (int)sizeof(T), di.sms < 148 ? di.sms : 148, lop != 0, pl))
             mode = 5;
         else
             mode = (g.npad <= persist_max_cells()) ? 3 : (g.npad <= loopk_max_cells()) ? 4 : 2;
@@ -2356,7 +2356,20 @@ const char* omni_status_string(int status)
     }
 }
 
-int omni_version(void) { return 106; }   // 101: omni_solve_guess_*, omni_set_history, omni_rans_source_*, omni_compressible_rans_source_*
+int omni_resident_plan(int nx, int ny, int nz, int elem_size, int nsm, int lop, int* out)
+{
+    Geom g;
+    if ((elem_size != 4 && elem_size != 8) || !out || nsm < 1 || !make_geom(nx, ny, nz, elem_size, g, 0)) return OMNI_ERR_INVALID_ARG;
+    ResidentPlan pl;
+    if (!resident_plan(g, elem_size, nsm < 148 ? nsm : 148, lop != 0, pl)) return 0;
+    const int v[12] = { pl.gy, pl.gz, pl.ly, pl.lz, (int)pl.smem_bytes, pl.rpt, pl.rreg, pl.dres, pl.qres, pl.wy, pl.wz, g.px };
+    for (int i = 0; i < 12; ++i) out[i] = v[i];
+    return 1;
+}
+
+int omni_resident_split(int n, int parts, int i, int wface) { return res_split(n, parts, i, wface); }
+
+int omni_version(void) { return 107; }   // 101: omni_solve_guess_*, omni_set_history, omni_rans_source_*, omni_compressible_rans_source_*
 
 #ifdef OMNI_RES_TRACE
 int omni_debug_res_trace(unsigned long long* out, int reset)

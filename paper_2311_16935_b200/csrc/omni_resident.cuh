@@ -45,17 +45,39 @@ constexpr int RES_NT = 512;        // threads per CTA: up to 128 registers each,
 constexpr int RES_NI = 16;         // rows per thread (16-byte chunks of r: 64 registers)
 constexpr int RES_SMEM_MAX = 227 * 1024 - 1024;   // dynamic shared memory the plan may use (static: the barrier's scratch)
 
+// Start of part i when an axis of n cells is cut into `parts` boxes.  wface = 0: equal counts.  wface > 0 (operator M on an
+// axis with face classes): a cell costs 4, a cell of a face class (0, 1, n-2, n-1; they run the face correction of
+// DESIGN.md section 6 on top of the interior formula) 4 + wface, and the cuts equalise the cost, so that the boxes on the
+// faces of the grid -- for which every barrier would otherwise wait -- get fewer rows.  Only where every part keeps at
+// least four cells.
+__host__ __device__ inline int res_split(int n, int parts, int i, int wface)
+{
+    if (i <= 0) return 0;
+    if (i >= parts) return n;
+    if (wface <= 0 || n < 8 * parts) return (int)((long long)n * i / parts);
+    const long long total = 4LL * n + 4LL * wface;
+    const long long target = (total * i + parts - 1) / parts;          // smallest x with cost(x) >= target
+    auto cost = [&](long long x) { return 4 * x + (long long)wface * ((x < 2 ? x : 2) + (x > n - 2 ? x - (n - 2) : 0)); };
+    int lo = 0, hi = n;                                                 // cost(lo) < target <= cost(hi)
+    while (hi - lo > 1) {
+        const int mid = (lo + hi) / 2;
+        if (cost(mid) >= target) hi = mid; else lo = mid;
+    }
+    return hi;
+}
+
 template <typename T>
 struct ResidentArgs {
     PersistArgs<T> a;
     unsigned long long* xchg;   // halo messages: sizeof(T) / 4 words per cell, indexed like the padded grid; zero at launch
-    int gy, gz;        // CTA b owns rows j in [ny*by/gy, ny*(by+1)/gy) of planes k in [nz*bz/gz, nz*(bz+1)/gz), by = b % gy, bz = b / gy
+    int gy, gz;        // CTA b owns rows j in [res_split(ny, gy, by), res_split(ny, gy, by + 1)) of the planes k cut likewise by bz; by = b % gy, bz = b / gy
     int ly, lz;        // largest box (rows, planes): the extents of the shared p array
     int zpad;          // 1: 3D operator, the p array has a halo plane below and above
     int pxs;           // row pitch of the p array in cells: px + 2 chunks (a zero chunk left and right of every row)
     int dres;          // 1: delta lives in shared memory
     int qres;          // 1: q = Op p of K3 is kept in shared memory for K4 (no second stencil pass)
     int rpt;           // rows per thread the shared r / delta arrays are laid out for
+    int wy, wz;        // res_split weights of the y and z cuts
 };
 
 // one chunk (16 bytes of T) as four messages { payload, epoch }
@@ -186,8 +208,8 @@ resident_kernel(const Geom g, const ResidentArgs<T> ra)
     const int lo2 = (int)(ntask2 * blockIdx.x / gridDim.x), hi2 = (int)(ntask2 * (blockIdx.x + 1) / gridDim.x);
     // ---- the CG phases' share: this CTA's box
     const int by = (int)blockIdx.x % ra.gy, bz = (int)blockIdx.x / ra.gy;
-    const int j0 = (int)((long long)g.ny * by / ra.gy), j1 = (int)((long long)g.ny * (by + 1) / ra.gy);
-    const int k0 = (int)((long long)g.nz * bz / ra.gz), k1 = (int)((long long)g.nz * (bz + 1) / ra.gz);
+    const int j0 = res_split(g.ny, ra.gy, by, ra.wy), j1 = res_split(g.ny, ra.gy, by + 1, ra.wy);
+    const int k0 = res_split(g.nz, ra.gz, bz, ra.wz), k1 = res_split(g.nz, ra.gz, bz + 1, ra.wz);
     const int lyb = j1 - j0, lzb = k1 - k0, nrows = lyb * lzb;
     const int cpr = g.px / V;                              // chunks per row
     const int rs = ra.pxs, pls = (ra.ly + 2) * ra.pxs, zpad = ra.zpad;
@@ -539,11 +561,11 @@ resident_kernel(const Geom g, const ResidentArgs<T> ra)
 
 // ---- host side: the box decomposition.  Returns false if the grid does not fit the SMs' memory.
 struct ResidentPlan {
-    int gy, gz, ly, lz, zpad, pxs, dres, qres, rpt, rreg;    // rreg: r does not fit the shared memory beside p
+    int gy, gz, ly, lz, zpad, pxs, dres, qres, rpt, rreg, wy, wz;    // rreg: r does not fit the shared memory beside p
     unsigned smem_bytes;
 };
 
-inline bool resident_plan(const Geom& g, int elem_size, int nsm, ResidentPlan& best)
+inline bool resident_plan(const Geom& g, int elem_size, int nsm, bool lop, ResidentPlan& best)
 {
     const int V = 16 / elem_size;
     const long long cpr = g.px / V;
@@ -552,27 +574,51 @@ inline bool resident_plan(const Geom& g, int elem_size, int nsm, ResidentPlan& b
     const bool three = g.naxes == 3;
     const int zpad = three ? 1 : 0;
     const long long pxs = (long long)g.px + 2 * V;
+    // a row of a face class costs 1.75 x an interior row under M (measured per-CTA phase times);
+    // under L the two differ by one multiply
+    const bool fy = !lop && g.fix[1], fz = !lop && three && g.fix[2];
+    auto faces = [](int n, int a, int b) {                // cells of a face class in [a, b)
+        int c = 0;
+        for (int x : { 0, 1, n - 2, n - 1 }) c += (x >= a && x < b) ? 1 : 0;
+        return c;
+    };
     double best_cost = -1.0;
     for (int gy = 1; gy <= nsm && gy <= g.ny; ++gy) {
         int gz = nsm / gy;
         if (gz > g.nz) gz = g.nz;
         if (gz < 1) break;
-        const long long ly = (g.ny + gy - 1) / gy, lz = (g.nz + gz - 1) / gz;
-        const long long rpt = (ly * lz + nrg - 1) / nrg;           // rows per thread
-        const long long p_bytes = (lz + 2 * zpad) * (ly + 2) * pxs * elem_size;
-        const long long v_bytes = rpt * RES_NT * 16;               // one more box vector (r, delta) in shared memory
-        if (p_bytes > RES_SMEM_MAX) continue;
-        const bool rreg = p_bytes + v_bytes > RES_SMEM_MAX;
-        const long long halo_rows = (gy > 1 ? 2 * lz : 0) + ((three && gz > 1) ? 2 * ly : 0);
-        // time of an iteration ~ rows a thread walks three times (update, two stencils) + halo rows the CTA updates
-        const double cost = 3.0 * (double)rpt * (double)nrg + (double)halo_rows;
-        if (best_cost < 0.0 || cost < best_cost) {
-            best_cost = cost;
-            best.gy = gy; best.gz = gz; best.ly = (int)ly; best.lz = (int)lz; best.zpad = zpad; best.pxs = (int)pxs;
-            best.rpt = (int)rpt; best.rreg = rreg ? 1 : 0;
-            best.dres = (!rreg && p_bytes + 2 * v_bytes <= RES_SMEM_MAX) ? 1 : 0;
-            best.qres = (!rreg && p_bytes + 3 * v_bytes <= RES_SMEM_MAX) ? 1 : 0;
-            best.smem_bytes = (unsigned)(p_bytes + (rreg ? 0 : v_bytes) + (best.dres ? v_bytes : 0) + (best.qres ? v_bytes : 0));
+        for (int weighted = 0; weighted < 2; ++weighted) {
+            const int wy = (weighted && fy) ? 3 : 0, wz = (weighted && fz) ? 3 : 0;
+            if (weighted && !wy && !wz) continue;
+            long long ly = 0, lz = 0;                               // largest box
+            double worst = 0.0;                                     // rows per thread of the slowest box, in interior-row units
+            for (int bz = 0; bz < gz; ++bz) {
+                const int k0 = res_split(g.nz, gz, bz, wz), k1 = res_split(g.nz, gz, bz + 1, wz);
+                lz = std::max<long long>(lz, k1 - k0);
+                for (int by = 0; by < gy; ++by) {
+                    const int j0 = res_split(g.ny, gy, by, wy), j1 = res_split(g.ny, gy, by + 1, wy);
+                    ly = std::max<long long>(ly, j1 - j0);
+                    const double rows = (double)(((long long)(j1 - j0) * (k1 - k0) + nrg - 1) / nrg);
+                    const double f = 1.0 + (fy ? 0.75 * faces(g.ny, j0, j1) / (j1 - j0) : 0.0) + (fz ? 0.75 * faces(g.nz, k0, k1) / (k1 - k0) : 0.0);
+                    worst = std::max(worst, rows * f);
+                }
+            }
+            const long long rpt = (ly * lz + nrg - 1) / nrg;           // rows per thread of the largest box
+            const long long p_bytes = (lz + 2 * zpad) * (ly + 2) * pxs * elem_size;
+            const long long v_bytes = rpt * RES_NT * 16;               // one more box vector (r, delta, q) in shared memory
+            if (p_bytes > RES_SMEM_MAX) continue;
+            const bool rreg = p_bytes + v_bytes > RES_SMEM_MAX;
+            const long long halo_rows = (gy > 1 ? 2 * lz : 0) + ((three && gz > 1) ? 2 * ly : 0);
+            // time of an iteration ~ what the slowest thread walks three times (update, two stencils) + the halo rows a CTA updates
+            const double cost = 3.0 * worst * (double)nrg + (double)halo_rows;
+            if (best_cost < 0.0 || cost < best_cost) {
+                best_cost = cost;
+                best.gy = gy; best.gz = gz; best.ly = (int)ly; best.lz = (int)lz; best.zpad = zpad; best.pxs = (int)pxs;
+                best.rpt = (int)rpt; best.rreg = rreg ? 1 : 0; best.wy = wy; best.wz = wz;
+                best.dres = (!rreg && p_bytes + 2 * v_bytes <= RES_SMEM_MAX) ? 1 : 0;
+                best.qres = (!rreg && p_bytes + 3 * v_bytes <= RES_SMEM_MAX) ? 1 : 0;
+                best.smem_bytes = (unsigned)(p_bytes + (rreg ? 0 : v_bytes) + (best.dres ? v_bytes : 0) + (best.qres ? v_bytes : 0));
+            }
         }
     }
     return best_cost >= 0.0;

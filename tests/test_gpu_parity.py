@@ -442,18 +442,24 @@ def test_cascade_first_guess(oracle, dtype, tol, forced_loop):
         assert rel_l2_after_mean_removal(Pn, Po, valid) <= (1e-5 if dtype == "f64" else 5e-3)
 
 
+@pytest.mark.parametrize("coop", [3, 5])
 @pytest.mark.parametrize("dtype", ["f64", "f32"])
-def test_persistent_loop_stress(dtype):
-    """The persistent kernel's grid barrier under every mix of phases (max_cg = 0, 1, 2, 3, 16: the outer and the
-    inner barriers interleave differently), on grids from one CTA to one CTA per SM, repeated: every repetition gives
-    the same bits, the same iteration counts as the graph loop, and the same field to rounding."""
+def test_persistent_loop_stress(dtype, coop):
+    """The cooperative kernels' grid barriers (3: the persistent loop's fenced ones; 5: the SM-resident loop's fenced
+    and relaxed ones plus its halo messages) under every mix of phases (max_cg = 0, 1, 2, 3, 16: the outer and the inner
+    barriers interleave differently, the lazy delta is flushed at even and odd counts), on grids from one CTA to one CTA
+    per SM, repeated: every repetition gives the same bits, the same iteration counts as the graph loop, and the same
+    field to rounding.  (1030 x 1000 in fp64: r and delta beside p, no room for q; 100 x 108 x 120 in fp64: r beside p,
+    delta lazy in global memory; r outside the SM is covered at 128^3 fp64 by tests/test_gpu_fullsize.py.)"""
     cases = [("gaussians2d", (64, 64)), ("lamb_oseen2d", (700, 300)), ("sphere3d", (48, 40, 36)), ("fourier3d", (9, 19, 66))]
+    if coop == 5:
+        cases += [("lamb_oseen2d", (1030, 1000)), ("fourier3d", (100, 108, 120))]
     for kind, shape in cases:
         f = make_field(kind, shape, seed=3, noise=0.05, kmax=4.0)
         g_dev, _, m_dev, _ = _inputs(f, dtype)
         for max_outer, max_cg in ((3, 0), (12, 1), (9, 2), (7, 3), (5, 16)):
             out = {}
-            for mode, reps in ((2, 1), (3, 4)):
+            for mode, reps in ((2, 1), (coop, 4)):
                 prev = omni.set_loop_mode(mode)
                 try:
                     out[mode] = [omni.solve(g_dev[0], g_dev[1], g_dev[2], m_dev, f["d"], 0.0, max_outer, max_cg) for _ in range(reps)]
@@ -462,11 +468,11 @@ def test_persistent_loop_stress(dtype):
             Pg, ig = out[2][0]
             Pg = Pg.cpu().numpy()
             valid = ~np.isnan(Pg)
-            P0 = out[3][0][0].cpu().numpy()
-            for P, info in out[3]:
-                assert info == out[3][0][1], (kind, shape, max_outer, max_cg)
+            P0 = out[coop][0][0].cpu().numpy()
+            for P, info in out[coop]:
+                assert info == out[coop][0][1], (kind, shape, max_outer, max_cg)
                 assert np.array_equal(P.cpu().numpy(), P0, equal_nan=True), (kind, shape, max_outer, max_cg)
-            assert out[3][0][1]["cg_iters_total"] == ig["cg_iters_total"] and out[3][0][1]["outer_iters"] == ig["outer_iters"]
+            assert out[coop][0][1]["cg_iters_total"] == ig["cg_iters_total"] and out[coop][0][1]["outer_iters"] == ig["outer_iters"]
             if max_cg > 0:
                 assert rel_l2_after_mean_removal(P0, Pg, valid) <= (1e-11 if dtype == "f64" else 1e-5), (kind, shape, max_outer, max_cg)
             else:

@@ -115,3 +115,53 @@ def test_solve_ex_rejects_bad_options_before_enqueueing():
     assert call(0, bad) == -1
     bad = omni.Options(); L.omni_options_init(C.byref(bad)); bad.loop_mode = 9
     assert call(0, bad) == -1
+
+
+def test_resident_plan_invariants():
+    """The box decomposition of the SM-resident loop (host code of omni_resident.cuh through omni_resident_plan): the cuts
+    tile every axis with non-empty boxes, the largest box is the one the plan reports, the shared memory fits an SM, the
+    rows per thread cover the largest box; weighted cuts (operator M) never give a face box more rows than an interior one;
+    grids that cannot fit are refused."""
+    import paper_2311_16935_b200 as omni
+    cases = [(64, 64, 1), (130, 150, 1), (1024, 1024, 1), (2048, 700, 1), (32, 32, 32), (66, 19, 9), (128, 128, 128),
+             (130, 110, 101), (96, 96, 96), (500, 37, 41), (8, 3, 2)]
+    seen = 0
+    for nx, ny, nz in cases:
+        for dtype, esz in (("f32", 4), ("f64", 8)):
+            for lop in (False, True):
+                for nsm in (148, 132, 20):
+                    pl = omni.resident_plan(nx, ny, nz, dtype, nsm, lop)
+                    if pl is None:
+                        continue
+                    seen += 1
+                    V = 16 // esz
+                    assert pl["gy"] * pl["gz"] <= nsm and pl["gy"] <= ny and pl["gz"] <= nz
+                    assert pl["smem_bytes"] <= 226 * 1024
+                    cpr = pl["px"] // V
+                    assert pl["px"] % V == 0 and cpr <= 512
+                    nrg = 512 // cpr
+                    assert pl["rows_per_thread"] * nrg >= pl["ly"] * pl["lz"]
+                    three = nz > 1
+                    p_bytes = (pl["lz"] + (2 if three else 0)) * (pl["ly"] + 2) * (pl["px"] + 2 * V) * esz
+                    extra = (0 if pl["r_outside_smem"] else 1) + pl["delta_in_smem"] + pl["q_in_smem"]
+                    assert pl["smem_bytes"] == p_bytes + extra * pl["rows_per_thread"] * 512 * 16
+                    assert not (pl["r_outside_smem"] and (pl["delta_in_smem"] or pl["q_in_smem"]))
+                    if lop:
+                        assert pl["wy"] == 0 and pl["wz"] == 0
+                    for n, parts, w, big in ((ny, pl["gy"], pl["wy"], pl["ly"]), (nz, pl["gz"], pl["wz"], pl["lz"])):
+                        cuts = [omni.resident_split(n, parts, i, w) for i in range(parts + 1)]
+                        assert cuts[0] == 0 and cuts[-1] == n
+                        sizes = np.diff(cuts)
+                        assert (sizes >= 1).all() and sizes.max() == big
+                        if w > 0 and parts > 2:
+                            assert sizes[0] <= sizes[1:-1].min() + 1 and sizes[-1] <= sizes[1:-1].min() + 1
+    assert seen > 60
+    # rows longer than one chunk per thread, and grids whose p array cannot fit: no plan
+    assert omni.resident_plan(4096, 64, 1, "f32") is None and omni.resident_plan(1100, 900, 1, "f64") is None
+    assert omni.resident_plan(256, 256, 256, "f32") is None and omni.resident_plan(500, 500, 500, "f32") is None
+    # the weighted cut equalises cost: 128 cells in 8 parts, face cells cost 7 instead of 4
+    cuts = [omni.resident_split(128, 8, i, 3) for i in range(9)]
+    cost = lambda a, b: sum(7 if x in (0, 1, 126, 127) else 4 for x in range(a, b))
+    costs = [cost(cuts[i], cuts[i + 1]) for i in range(8)]
+    assert max(costs) - min(costs) <= 7 and cuts[1] < 16 and cuts[8] - cuts[7] < 16
+    assert [omni.resident_split(128, 8, i, 0) for i in range(9)] == list(range(0, 129, 16))
