@@ -402,9 +402,9 @@ long long omni_launch_count(int reset);
  * different (fixed) order.  Returns the previous mode; other values are ignored. */
 int omni_set_loop_mode(int mode);
 /* The box decomposition loop mode 5 would use for this grid (host only, no CUDA call): 1 and
- * out[0..11] = { gy, gz (boxes along y and z, gy * gz CTAs), ly, lz (rows and planes of the largest box), dynamic shared
+ * out[0..12] = { gy, gz (boxes along y and z, gy * gz CTAs), ly, lz (rows and planes of the largest box), dynamic shared
  * memory in bytes, rows per thread, r does not fit beside p (0 / 1), delta in shared memory, q in shared memory, weights of
- * the y and z cuts, padded row pitch in cells }; 0 if the grid does not fit the SMs (mode 5 then falls back to mode 3);
+ * the y and z cuts, padded row pitch in cells, r and delta in tensor memory (0 / 1) }; 0 if the grid does not fit the SMs (mode 5 then falls back to mode 3);
  * OMNI_ERR_INVALID_ARG for bad arguments.  elem_size 4 or 8, nsm = SMs to plan for, lop = 1 for the operator L of
  * omni_solve_direct.  omni_resident_split(n, parts, i, wface) = first cell of part i when an axis of n cells is cut into
  * `parts` boxes with that weight (i = parts: n). */

@@ -82,14 +82,14 @@ def set_loop_mode(mode):
 def resident_plan(nx, ny, nz, dtype="f32", nsm=148, lop=False):
     """omni_resident_plan: the box decomposition of the SM-resident loop (loop mode 5) for this grid, or None if the grid
     does not fit the SMs.  Host only."""
-    out = (C.c_int * 12)()
+    out = (C.c_int * 13)()
     rc = lib().omni_resident_plan(C.c_int(nx), C.c_int(ny), C.c_int(nz), C.c_int(4 if dtype == "f32" else 8), C.c_int(nsm),
                                   C.c_int(1 if lop else 0), out)
     if rc < 0:
         raise OmniError(rc, "omni_resident_plan")
     if rc == 0:
         return None
-    keys = ("gy", "gz", "ly", "lz", "smem_bytes", "rows_per_thread", "r_outside_smem", "delta_in_smem", "q_in_smem", "wy", "wz", "px")
+    keys = ("gy", "gz", "ly", "lz", "smem_bytes", "rows_per_thread", "r_outside_smem", "delta_in_smem", "q_in_smem", "wy", "wz", "px", "r_delta_in_tmem")
     return dict(zip(keys, list(out)))
 
 

@@ -1072,6 +1072,19 @@ int run_loop_persist(const Geom& g, const Workspace<T>& w, const HostConst& H, c
 
 // SM-resident loop (omni_resident.cuh): the persistent loop with p in shared memory and r in registers for the whole
 // inner solve.  Returns -100 if the grid does not fit the SMs or the device cannot co-schedule it.
+// OMNI_RESIDENT_TMEM = 0 / 2 keeps r and delta of the resident loop out of / always in tensor memory (A / B measurements).
+// The one combination it loses on is fp64 with the operator M (0.87-0.98 x: that instantiation runs out of registers), which
+// keeps r in shared memory / L2.
+bool resident_tmem(int elem_size, bool lop)
+{
+    static int v = -1;
+    if (v < 0) {
+        const char* e = getenv("OMNI_RESIDENT_TMEM");
+        v = e ? atoi(e) : 1;                                  // 0: never, 1: where it wins, 2: always
+    }
+    return v == 2 || (v == 1 && !(elem_size == 8 && !lop));
+}
+
 template <typename T, bool LOP, int RM>
 int launch_resident(const Geom& g, const Workspace<T>& w, const HostConst& H, const Coef<T>& K, const ResidentPlan& pl, cudaStream_t st)
 {
@@ -1115,8 +1128,9 @@ int run_loop_resident(const Geom& g, const Workspace<T>& w, const HostConst& H, 
     if (!di.coop || di.sms < 1) return -100;
     if (g.npad >= (1LL << 31) || (long long)g.ny * g.nz * ((g.nx + 63) / 64) >= (1LL << 31)) return -100;
     ResidentPlan pl;
-    if (!resident_plan(g, (int)sizeof(T), di.sms < 148 ? di.sms : 148, LOP, pl)) return -100;     // relaxed slots: room for 148 CTAs
+    if (!resident_plan(g, (int)sizeof(T), di.sms < 148 ? di.sms : 148, LOP, resident_tmem((int)sizeof(T), LOP), pl)) return -100;     // relaxed slots: room for 148 CTAs
     if (pl.gy * pl.gz > 148 || pl.gy * pl.gz > RES_NT) return -100;          // relaxed slots: RES_SLOT_OFFSET
+    if (pl.rtm) return launch_resident<T, LOP, 3>(g, w, H, K, pl, st);
     if (!pl.rreg) return launch_resident<T, LOP, 0>(g, w, H, K, pl, st);
     static const int rmode = getenv("OMNI_RESIDENT_R") ? atoi(getenv("OMNI_RESIDENT_R")) : 2;
     if (rmode == 1 && pl.rpt <= RES_NI) return launch_resident<T, LOP, 1>(g, w, H, K, pl, st);
@@ -1266,7 +1280,7 @@ int solve_ws(int nx, int ny, int nz, double dx, double dy, double dz, const T* g
         ResidentPlan pl;
         const DevInfo di = device_info();
         const bool one_red = lop && opt.single_reduction;          // that option is the persistent loop's
-        if (!one_red && !pcg && resident_enabled() && di.coop && resident_plan(g, (int)sizeof(T), di.sms < 148 ? di.sms : 148, lop != 0, pl))
+        if (!one_red && !pcg && resident_enabled() && di.coop && resident_plan(g, (int)sizeof(T), di.sms < 148 ? di.sms : 148, lop != 0, resident_tmem((int)sizeof(T), lop != 0), pl))
             mode = 5;
         else
             mode = (g.npad <= persist_max_cells()) ? 3 : (g.npad <= loopk_max_cells()) ? 4 : 2;
@@ -2361,9 +2375,9 @@ int omni_resident_plan(int nx, int ny, int nz, int elem_size, int nsm, int lop, 
     Geom g;
     if ((elem_size != 4 && elem_size != 8) || !out || nsm < 1 || !make_geom(nx, ny, nz, elem_size, g, 0)) return OMNI_ERR_INVALID_ARG;
     ResidentPlan pl;
-    if (!resident_plan(g, elem_size, nsm < 148 ? nsm : 148, lop != 0, pl)) return 0;
-    const int v[12] = { pl.gy, pl.gz, pl.ly, pl.lz, (int)pl.smem_bytes, pl.rpt, pl.rreg, pl.dres, pl.qres, pl.wy, pl.wz, g.px };
-    for (int i = 0; i < 12; ++i) out[i] = v[i];
+    if (!resident_plan(g, elem_size, nsm < 148 ? nsm : 148, lop != 0, resident_tmem(elem_size, lop != 0), pl)) return 0;
+    const int v[13] = { pl.gy, pl.gz, pl.ly, pl.lz, (int)pl.smem_bytes, pl.rpt, pl.rreg, pl.dres, pl.qres, pl.wy, pl.wz, g.px, pl.rtm };
+    for (int i = 0; i < 13; ++i) out[i] = v[i];
     return 1;
 }
 

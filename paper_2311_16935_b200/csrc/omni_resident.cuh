@@ -165,6 +165,46 @@ __device__ __forceinline__ bool grid_allreduce_relaxed(GridSync& gs, unsigned in
     return *late == 0;
 }
 
+// ---- Tensor memory as a per-thread scratchpad.  The 256 KB of TMEM of an SM (512 columns x 128 lanes x 32 bit) are the
+// accumulator store of tcgen05.mma; nothing here multiplies matrices, but tcgen05.ld / tcgen05.st move registers to and
+// from it with the 32x32b shape in which lane i of a warp owns TMEM lane 32 (warp % 4) + i: thread-private storage with
+// a 12-cycle load, exactly what r and delta need (CG touches them cell by cell).  The four warps that share a lane
+// quarter take 128 columns each: 32 chunks of 16 bytes per thread, RES_NI for r and RES_NI for delta.
+__device__ __forceinline__ void tmem_alloc512(uint32_t* smem_slot)        // one whole warp
+{
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;"
+                 :: "r"((uint32_t)__cvta_generic_to_shared(smem_slot)), "r"(512u) : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+}
+__device__ __forceinline__ void tmem_dealloc512(uint32_t base)            // one whole warp
+{
+    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" :: "r"(base), "r"(512u) : "memory");
+}
+// whole warp; the registers are valid after tmem_wait_ld (one wait covers every load issued before it)
+__device__ __forceinline__ void tmem_ld_raw(uint32_t taddr, uint32_t (&w)[4])
+{
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x4.b32 {%0, %1, %2, %3}, [%4];"
+                 : "=r"(w[0]), "=r"(w[1]), "=r"(w[2]), "=r"(w[3]) : "r"(taddr) : "memory");
+}
+__device__ __forceinline__ void tmem_wait_ld() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
+template <typename T, int V>
+__device__ __forceinline__ void tmem_ld_chunk(uint32_t taddr, T (&v)[V])
+{
+    uint32_t w[4];
+    tmem_ld_raw(taddr, w);
+    tmem_wait_ld();
+    memcpy(v, w, 16);
+}
+template <typename T, int V>
+__device__ __forceinline__ void tmem_st_chunk(uint32_t taddr, const T (&v)[V])   // whole warp
+{
+    uint32_t w[4];
+    memcpy(w, v, 16);
+    asm volatile("tcgen05.st.sync.aligned.32x32b.x4.b32 [%0], {%1, %2, %3, %4};"
+                 :: "r"(taddr), "r"(w[0]), "r"(w[1]), "r"(w[2]), "r"(w[3]) : "memory");
+}
+__device__ __forceinline__ void tmem_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
+
 // loop over the rows of a thread: unrolled when r lives in registers (static register indices), rolled otherwise
 template <bool UNROLL, typename F>
 __device__ __forceinline__ void res_for_rows(int nrt, F&& f)
@@ -185,12 +225,14 @@ __device__ __forceinline__ void res_for_rows(int nrt, F&& f)
 // 2: the global r array (through L2; same grids as 1).  With RM 2 a thread's loads of r are one L2 round trip per row;
 // issuing them four rows ahead (16 + 16 more registers for r and the lazy delta) was tried and is slower (128^3 fp64:
 // 29.8 -> 36.3 us per iteration): with 190 KB of shared memory the L1 is 28 KB and the 230 B per thread it spills miss it.
+//   3: r AND delta in tensor memory (tmem_* above): shared memory holds p and, where it fits, q.
 template <typename T, bool LOP, int RM>
 __global__ void __launch_bounds__(RES_NT, 1)
 resident_kernel(const Geom g, const ResidentArgs<T> ra)
 {
     constexpr int V = 16 / (int)sizeof(T), NT = RES_NT, NW = NT / 32, MW = (int)sizeof(T) / 4;
-    constexpr bool RREG = RM == 1;
+    constexpr bool RREG = RM == 1, RTM = RM == 3;
+    __shared__ uint32_t tmem_base_slot;
     extern __shared__ __align__(16) unsigned char res_smem[];
     __shared__ double red[2 * (NW + 1)];
     __shared__ double sv[PERSIST_MAX_CTAS > NT ? NT : PERSIST_MAX_CTAS];
@@ -218,7 +260,7 @@ resident_kernel(const Geom g, const ResidentArgs<T> ra)
     // r (unless RREG) and delta (dres only) of this thread's row `it` at [(it * NT + tid) * V]
     T* const rsm = ps + p_elems;
     T* const ds = rsm + (RM != 0 ? 0 : ra.rpt * NT * V);
-    T* const qs = ds + ra.rpt * NT * V;                    // qres only (implies dres)
+    T* const qs = RTM ? rsm : ds + ra.rpt * NT * V;        // qres only (RM 0: implies dres)
     // a thread owns x chunk xc of the rows [r_lo, r_lo + nrt) of the box (rows numbered y-fastest): NT / cpr row groups
     const int nrg = NT / cpr, grp = tid / cpr, xc = tid - grp * cpr, x = xc * V;
     const int rpg = (nrows + nrg - 1) / nrg;
@@ -233,10 +275,21 @@ resident_kernel(const Geom g, const ResidentArgs<T> ra)
     const int nC = (three && k0 > 0) ? lyb : 0, nD = (three && k1 < g.nz) ? lyb : 0;
     const int nhc = (nA + nB + nC + nD) * cpr;
 
+    // tcgen05.ld / st are warp-wide: with r in tensor memory every lane of a warp walks the same number of rows (the
+    // largest of the warp); `live` tells a lane whether row `it` is one of its own
+    int nloop = nrt;
+    if constexpr (RTM) {
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) nloop = max(nloop, __shfl_xor_sync(0xffffffffu, nloop, o));
+    }
+    // tensor-memory address of chunk `slot` (0 .. 31) of this thread: lane quarter of the warp, 128 columns per warp
+    uint32_t tm_base = 0;
+    auto tm_addr = [&](int slot) { return tm_base + (uint32_t)(slot * 4); };
 #define RES_ROWS_BEGIN                                                                                   \
     {                                                                                                    \
         int jl = jl0, kl = kl0, off = off0;                                                              \
-        res_for_rows<RREG>(nrt, [&](const int it) {
+        res_for_rows<RREG>(nloop, [&](const int it) {                                                    \
+            const bool live = it < nrt;
 #define RES_ROWS_END                                                                                     \
             jl += 1; off += rs;                                                                          \
             if (jl == lyb) { jl = 0; kl += 1; off += wrap; }                                             \
@@ -249,13 +302,24 @@ resident_kernel(const Geom g, const ResidentArgs<T> ra)
     //   bnd:  the row is on the box boundary: its r travels to a neighbour
     uint32_t fbm = 0, slowm = 0, bndm = 0;
     RES_ROWS_BEGIN
-        if (flag_bits<V>(a.flags, cell_idx(jl, kl))) fbm |= 1u << it;
-        if (face_class(j0 + jl, g.ny, g.fix[1]) >= 0 || face_class(k0 + kl, g.nz, g.fix[2]) >= 0) slowm |= 1u << it;
-        if ((jl == 0 && j0 > 0) || (jl == lyb - 1 && j1 < g.ny) || (three && ((kl == 0 && k0 > 0) || (kl == lzb - 1 && k1 < g.nz))))
-            bndm |= 1u << it;
+        if (live) {
+            if (flag_bits<V>(a.flags, cell_idx(jl, kl))) fbm |= 1u << it;
+            if (face_class(j0 + jl, g.ny, g.fix[1]) >= 0 || face_class(k0 + kl, g.nz, g.fix[2]) >= 0) slowm |= 1u << it;
+            if ((jl == 0 && j0 > 0) || (jl == lyb - 1 && j1 < g.ny) || (three && ((kl == 0 && k0 > 0) || (kl == lzb - 1 && k1 < g.nz))))
+                bndm |= 1u << it;
+        }
         (void)off;
     RES_ROWS_END
     slowm |= fbm;
+
+    if constexpr (RTM) {
+        // all 512 columns of this SM's tensor memory (one CTA per SM); released at the kernel's single exit below
+        if (warp == 0) tmem_alloc512(&tmem_base_slot);
+        asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+        __syncthreads();
+        asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+        tm_base = tmem_base_slot + ((uint32_t)(32 * (warp & 3)) << 16) + (uint32_t)(128 * (warp >> 2));
+    }
 
     GridSync gs{ { 2u, 2u }, red, &flag, a.timeout_ns };
     unsigned int rcount = 2u;                              // use count of the relaxed barrier (set = count & 1, tag = (count >> 1) & 1)
@@ -269,24 +333,35 @@ resident_kernel(const Geom g, const ResidentArgs<T> ra)
     double rho = 0.0, beta = 0.0, alpha = 0.0, gamma = 0.0, epsR2 = 0.0, alpha_prev = 0.0;
     bool dzero = sc->dzero != 0;
     T rr[RREG ? RES_NI : 1][V];
-    auto r_ld = [&](int it, int jl, int kl, T (&v)[V]) {
-        if constexpr (RM == 1) {
+    // r of row `it` (slots 0 .. RES_NI-1 of the thread's tensor memory with RM 3) and, RM 3 only, delta (slots RES_NI ..)
+    auto r_ld = [&](int it, int jl, int kl, bool live, T (&v)[V]) {
+        if constexpr (RM == 3) {
+            __syncwarp();
+            tmem_ld_chunk<T, V>(tm_addr(it), v);
+        } else if (live) {
+            if constexpr (RM == 1) {
 #pragma unroll
-            for (int c = 0; c < V; ++c) v[c] = rr[it][c];
-        } else if constexpr (RM == 0) {
-            ld_chunk<T, V>(rsm + (size_t)(it * NT + tid) * V, v);
-        } else {
-            ld_chunk<T, V>(a.r + cell_idx(jl, kl), v);             // this thread's own store (or K2's, behind a fenced barrier)
+                for (int c = 0; c < V; ++c) v[c] = rr[it][c];
+            } else if constexpr (RM == 0) {
+                ld_chunk<T, V>(rsm + (size_t)(it * NT + tid) * V, v);
+            } else {
+                ld_chunk<T, V>(a.r + cell_idx(jl, kl), v);         // this thread's own store (or K2's, behind a fenced barrier)
+            }
         }
     };
-    auto r_st = [&](int it, int jl, int kl, const T (&v)[V]) {
-        if constexpr (RM == 1) {
+    auto r_st = [&](int it, int jl, int kl, bool live, const T (&v)[V]) {
+        if constexpr (RM == 3) {
+            __syncwarp();
+            tmem_st_chunk<T, V>(tm_addr(it), v);
+        } else if (live) {
+            if constexpr (RM == 1) {
 #pragma unroll
-            for (int c = 0; c < V; ++c) rr[it][c] = v[c];
-        } else if constexpr (RM == 0) {
-            st_chunk<T, V>(rsm + (size_t)(it * NT + tid) * V, v);
-        } else {
-            st_chunk<T, V>(a.r + cell_idx(jl, kl), v);
+                for (int c = 0; c < V; ++c) rr[it][c] = v[c];
+            } else if constexpr (RM == 0) {
+                st_chunk<T, V>(rsm + (size_t)(it * NT + tid) * V, v);
+            } else {
+                st_chunk<T, V>(a.r + cell_idx(jl, kl), v);
+            }
         }
     };
 #ifdef OMNI_RES_TRACE
@@ -369,11 +444,13 @@ resident_kernel(const Geom g, const ResidentArgs<T> ra)
         RES_ROWS_BEGIN
             if constexpr (RM != 2) {
                 T v[V];
-                ldcg_chunk<T, V>(a.r + cell_idx(jl, kl), v);
-                r_st(it, jl, kl, v);
+                zero_chunk<T, V>(v);
+                if (live) ldcg_chunk<T, V>(a.r + cell_idx(jl, kl), v);
+                r_st(it, jl, kl, live, v);
             }
             (void)off;
         RES_ROWS_END
+        if constexpr (RTM) tmem_wait_st();
         __syncthreads();
         RES_T(0);
         // ------------------------------------------------------------------------------ inner CG on Op delta = r0
@@ -436,11 +513,13 @@ resident_kernel(const Geom g, const ResidentArgs<T> ra)
                 }
                 RES_ROWS_BEGIN
                     T p[V], r[V];
-                    ld_chunk<T, V>(ps + off, p);
-                    r_ld(it, jl, kl, r);
+                    r_ld(it, jl, kl, live, r);
+                    if (live) {
+                        ld_chunk<T, V>(ps + off, p);
 #pragma unroll
-                    for (int c = 0; c < V; ++c) p[c] = r[c] + b * p[c];
-                    st_chunk<T, V>(ps + off, p);
+                        for (int c = 0; c < V; ++c) p[c] = r[c] + b * p[c];
+                        st_chunk<T, V>(ps + off, p);
+                    }
                 RES_ROWS_END
             }
             __syncthreads();
@@ -451,11 +530,13 @@ resident_kernel(const Geom g, const ResidentArgs<T> ra)
                 double acc[1] = { 0.0 };
                 carry = false;
                 RES_ROWS_BEGIN
-                    T q[V];
-                    stencil(off, it, jl, kl, q);
-                    acc[0] += dot_chunk(vc, q);
-                    if (ra.qres) st_chunk<T, V>(qs + (size_t)(it * NT + tid) * V, q);
-                    RES_CARRY_NEXT
+                    if (live) {
+                        T q[V];
+                        stencil(off, it, jl, kl, q);
+                        acc[0] += dot_chunk(vc, q);
+                        if (ra.qres) st_chunk<T, V>(qs + (size_t)(it * NT + tid) * V, q);
+                        RES_CARRY_NEXT
+                    }
                 RES_ROWS_END
                 double tot[1];
                 RES_T(2);
@@ -476,37 +557,61 @@ resident_kernel(const Geom g, const ResidentArgs<T> ra)
                 carry = false;
                 RES_ROWS_BEGIN
                     T q[V], r[V];
-                    if (ra.qres) {
-                        ld_chunk<T, V>(qs + (size_t)(it * NT + tid) * V, q);
-                        ld_chunk<T, V>(ps + off, vc);
+                    zero_chunk<T, V>(q);
+                    if (live) {
+                        if (ra.qres) {
+                            ld_chunk<T, V>(qs + (size_t)(it * NT + tid) * V, q);
+                            ld_chunk<T, V>(ps + off, vc);
+                        } else {
+                            stencil(off, it, jl, kl, q);
+                        }
+                    }
+                    if constexpr (RTM) {
+                        // r and delta of the row: two loads, one wait
+                        uint32_t wr[4], wd[4] = { 0u, 0u, 0u, 0u };
+                        __syncwarp();
+                        tmem_ld_raw(tm_addr(it), wr);
+                        if (k != 0) tmem_ld_raw(tm_addr(RES_NI + it), wd);
+                        tmem_wait_ld();
+                        T d[V];
+                        memcpy(r, wr, 16);
+                        memcpy(d, wd, 16);
+                        if (live) {
+#pragma unroll
+                            for (int c = 0; c < V; ++c) d[c] += al * vc[c];
+                        }
+                        tmem_st_chunk<T, V>(tm_addr(RES_NI + it), d);
                     } else {
-                        stencil(off, it, jl, kl, q);
+                        r_ld(it, jl, kl, live, r);
                     }
-                    r_ld(it, jl, kl, r);
-                    if (ra.dres) {
-                        T d[V];
-                        T* dp = ds + (size_t)(it * NT + tid) * V;
-                        if (k == 0) zero_chunk<T, V>(d);
-                        else ld_chunk<T, V>(dp, d);
+                    if (live) {
+                        if constexpr (RTM) {
+                        } else if (ra.dres) {
+                            T d[V];
+                            T* dp = ds + (size_t)(it * NT + tid) * V;
+                            if (k == 0) zero_chunk<T, V>(d);
+                            else ld_chunk<T, V>(dp, d);
 #pragma unroll
-                        for (int c = 0; c < V; ++c) d[c] += al * vc[c];
-                        st_chunk<T, V>(dp, d);
-                    } else if (odd) {
-                        T d[V];
-                        T* dp = a.delta + cell_idx(jl, kl);
-                        if (k == 1) zero_chunk<T, V>(d);
-                        else ld_chunk<T, V>(dp, d);             // this thread's own store of two iterations ago
+                            for (int c = 0; c < V; ++c) d[c] += al * vc[c];
+                            st_chunk<T, V>(dp, d);
+                        } else if (odd) {
+                            T d[V];
+                            T* dp = a.delta + cell_idx(jl, kl);
+                            if (k == 1) zero_chunk<T, V>(d);
+                            else ld_chunk<T, V>(dp, d);             // this thread's own store of two iterations ago
 #pragma unroll
-                        for (int c = 0; c < V; ++c) d[c] += c1 * vc[c] - c2 * r[c];
-                        st_chunk<T, V>(dp, d);
+                            for (int c = 0; c < V; ++c) d[c] += c1 * vc[c] - c2 * r[c];
+                            st_chunk<T, V>(dp, d);
+                        }
+#pragma unroll
+                        for (int c = 0; c < V; ++c) r[c] -= al * q[c];
+                        acc[0] += dot_chunk(r, r);
+                        if ((bndm >> it) & 1u) msg_send<T, V>(ra.xchg + cell_idx(jl, kl) * MW, r, epoch);
+                        if (!ra.qres) { RES_CARRY_NEXT }
                     }
-#pragma unroll
-                    for (int c = 0; c < V; ++c) r[c] -= al * q[c];
-                    r_st(it, jl, kl, r);
-                    acc[0] += dot_chunk(r, r);
-                    if ((bndm >> it) & 1u) msg_send<T, V>(ra.xchg + cell_idx(jl, kl) * MW, r, epoch);
-                    if (!ra.qres) { RES_CARRY_NEXT }
+                    r_st(it, jl, kl, live, r);
                 RES_ROWS_END
+                if constexpr (RTM) tmem_wait_st();
                 double tot[1];
                 RES_T(4);
                 if (!grid_allreduce_relaxed<NT>(gs, rcount, a.slots, sv, &halo_late, acc[0], tot[0])) { status = ST_BARRIER_TIMEOUT; stop_all = true; break; }
@@ -526,21 +631,25 @@ resident_kernel(const Geom g, const ResidentArgs<T> ra)
         {
             const bool pend = (k & 1) != 0;        // k iterations done; the last one (index k - 1) was even: its update is pending
             const T al = (T)alpha;
-            if (ra.dres || pend) {
+            if (RTM || ra.dres || pend) {
                 RES_ROWS_BEGIN
                     T d[V];
-                    T* dp = a.delta + cell_idx(jl, kl);
-                    if (ra.dres) {
-                        ld_chunk<T, V>(ds + (size_t)(it * NT + tid) * V, d);
-                    } else {
-                        T p[V];
-                        ld_chunk<T, V>(ps + off, p);
-                        if (k == 1) zero_chunk<T, V>(d);
-                        else ld_chunk<T, V>(dp, d);
+                    if constexpr (RTM) { __syncwarp(); tmem_ld_chunk<T, V>(tm_addr(RES_NI + it), d); }
+                    if (live) {
+                        T* dp = a.delta + cell_idx(jl, kl);
+                        if constexpr (RTM) {
+                        } else if (ra.dres) {
+                            ld_chunk<T, V>(ds + (size_t)(it * NT + tid) * V, d);
+                        } else {
+                            T p[V];
+                            ld_chunk<T, V>(ps + off, p);
+                            if (k == 1) zero_chunk<T, V>(d);
+                            else ld_chunk<T, V>(dp, d);
 #pragma unroll
-                        for (int c = 0; c < V; ++c) d[c] += al * p[c];
+                            for (int c = 0; c < V; ++c) d[c] += al * p[c];
+                        }
+                        st_chunk<T, V>(dp, d);
                     }
-                    st_chunk<T, V>(dp, d);
                 RES_ROWS_END
             }
             // K2 reads delta of other CTAs' cells: a fenced barrier
@@ -552,6 +661,12 @@ resident_kernel(const Geom g, const ResidentArgs<T> ra)
 #undef RES_ROWS_END
 #undef RES_CARRY_NEXT
 
+    if constexpr (RTM) {
+        tmem_wait_st();
+        asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+        __syncthreads();
+        if (warp == 0) tmem_dealloc512(tmem_base_slot);
+    }
     if (blockIdx.x == 0 && tid == 0) {
         sc->n = n; sc->k = k; sc->cg_total = cg_total; sc->status = status;
         sc->rho = rho; sc->beta = beta; sc->alpha = alpha; sc->gamma = gamma; sc->epsR2 = epsR2;
@@ -561,11 +676,11 @@ resident_kernel(const Geom g, const ResidentArgs<T> ra)
 
 // ---- host side: the box decomposition.  Returns false if the grid does not fit the SMs' memory.
 struct ResidentPlan {
-    int gy, gz, ly, lz, zpad, pxs, dres, qres, rpt, rreg, wy, wz;    // rreg: r does not fit the shared memory beside p
+    int gy, gz, ly, lz, zpad, pxs, dres, qres, rpt, rreg, wy, wz, rtm;   // rtm: r and delta in tensor memory    // rreg: r does not fit the shared memory beside p
     unsigned smem_bytes;
 };
 
-inline bool resident_plan(const Geom& g, int elem_size, int nsm, bool lop, ResidentPlan& best)
+inline bool resident_plan(const Geom& g, int elem_size, int nsm, bool lop, bool allow_tm, ResidentPlan& best)
 {
     const int V = 16 / elem_size;
     const long long cpr = g.px / V;
@@ -606,17 +721,18 @@ inline bool resident_plan(const Geom& g, int elem_size, int nsm, bool lop, Resid
             const long long rpt = (ly * lz + nrg - 1) / nrg;           // rows per thread of the largest box
             const long long p_bytes = (lz + 2 * zpad) * (ly + 2) * pxs * elem_size;
             const long long v_bytes = rpt * RES_NT * 16;               // one more box vector (r, delta, q) in shared memory
-            if (p_bytes > RES_SMEM_MAX) continue;
-            const bool rreg = p_bytes + v_bytes > RES_SMEM_MAX;
+            if (p_bytes > RES_SMEM_MAX || rpt > 32) continue;       // (one mask bit per row of a thread)
+            const bool rtm = allow_tm && rpt <= RES_NI;              // r and delta fit the thread's share of tensor memory
+            const bool rreg = rtm || p_bytes + v_bytes > RES_SMEM_MAX;
             const long long halo_rows = (gy > 1 ? 2 * lz : 0) + ((three && gz > 1) ? 2 * ly : 0);
             // time of an iteration ~ what the slowest thread walks three times (update, two stencils) + the halo rows a CTA updates
             const double cost = 3.0 * worst * (double)nrg + (double)halo_rows;
             if (best_cost < 0.0 || cost < best_cost) {
                 best_cost = cost;
                 best.gy = gy; best.gz = gz; best.ly = (int)ly; best.lz = (int)lz; best.zpad = zpad; best.pxs = (int)pxs;
-                best.rpt = (int)rpt; best.rreg = rreg ? 1 : 0; best.wy = wy; best.wz = wz;
+                best.rpt = (int)rpt; best.rreg = rreg ? 1 : 0; best.wy = wy; best.wz = wz; best.rtm = rtm ? 1 : 0;
                 best.dres = (!rreg && p_bytes + 2 * v_bytes <= RES_SMEM_MAX) ? 1 : 0;
-                best.qres = (!rreg && p_bytes + 3 * v_bytes <= RES_SMEM_MAX) ? 1 : 0;
+                best.qres = rtm ? (p_bytes + v_bytes <= RES_SMEM_MAX ? 1 : 0) : (!rreg && p_bytes + 3 * v_bytes <= RES_SMEM_MAX) ? 1 : 0;
                 best.smem_bytes = (unsigned)(p_bytes + (rreg ? 0 : v_bytes) + (best.dres ? v_bytes : 0) + (best.qres ? v_bytes : 0));
             }
         }

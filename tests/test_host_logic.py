@@ -145,7 +145,10 @@ def test_resident_plan_invariants():
                     p_bytes = (pl["lz"] + (2 if three else 0)) * (pl["ly"] + 2) * (pl["px"] + 2 * V) * esz
                     extra = (0 if pl["r_outside_smem"] else 1) + pl["delta_in_smem"] + pl["q_in_smem"]
                     assert pl["smem_bytes"] == p_bytes + extra * pl["rows_per_thread"] * 512 * 16
-                    assert not (pl["r_outside_smem"] and (pl["delta_in_smem"] or pl["q_in_smem"]))
+                    assert not (pl["r_outside_smem"] and pl["delta_in_smem"])
+                    assert not (pl["q_in_smem"] and pl["r_outside_smem"] and not pl["r_delta_in_tmem"])
+                    if pl["r_delta_in_tmem"]:                         # a thread's share of tensor memory: 16 + 16 chunks
+                        assert pl["rows_per_thread"] <= 16 and pl["r_outside_smem"] == 1
                     if lop:
                         assert pl["wy"] == 0 and pl["wz"] == 0
                     for n, parts, w, big in ((ny, pl["gy"], pl["wy"], pl["ly"]), (nz, pl["gz"], pl["wz"], pl["lz"])):
