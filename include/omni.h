@@ -392,13 +392,14 @@ long long omni_launch_count(int reset);
  *      grid barriers between the K2 / K3 / K4 phases); correct and deterministic, measured slower than mode 2 at every
  *      size (profiles/r2_loop_and_rows.md), never chosen automatically; falls back to mode 2 if its grid does not fit
  *   5  mode 3 with the CG vectors resident on the SMs for the whole inner solve: every CTA owns a box of grid rows, p of
- *      the box and its halo in shared memory, r in shared memory or (where p alone fills it: 128^3 fp64) in registers;
+ *      the box and its halo in shared memory, r and delta in the SM's tensor memory (tcgen05.ld / st as a thread-private
+ *      scratchpad), else in shared memory or, where p alone fills it, behind L2;
  *      per CG iteration only the halo rows of r travel, as self-validating messages, and the two grid barriers carry
  *      nothing but the reduction (no fence).  For grids of up to about 2 M cells whose rows are at most 2048 (fp32) /
  *      1024 (fp64) cells long; falls back to mode 3 where the grid does not fit.  Uses the workspace's two p vectors as
  *      message buffer.
  * The environment variable OMNI_PERSIST_MAX_CELLS overrides the threshold between modes 3 and 2, OMNI_RESIDENT=0 keeps mode
- * 5 out of the automatic choice.  Modes 1 and 2 give bit-identical results; modes 3, 4 and 5 sum their reductions in a
+ * 5 out of the automatic choice, OMNI_RESIDENT_TMEM=0 keeps it out of tensor memory.  Modes 1 and 2 give bit-identical results; modes 3, 4 and 5 sum their reductions in a
  * different (fixed) order.  Returns the previous mode; other values are ignored. */
 int omni_set_loop_mode(int mode);
 /* The box decomposition loop mode 5 would use for this grid (host only, no CUDA call): 1 and
