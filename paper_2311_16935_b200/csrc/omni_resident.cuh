@@ -1,25 +1,27 @@
 // omni_resident.cuh -- the persistent loop of omni_persist.cuh with the CG vectors kept ON THE SM between iterations,
-// for grids small enough that the direction vector p fits the shared memory of the whole GPU (148 x 227 KB) and the
-// residual r its register files: 1024 x 1024 (2D) and 128^3 (3D) in both precisions.
+// for grids small enough that the direction vector p fits the shared memory of the whole GPU (148 x 227 KB): up to
+// 1024 x 1024 (2D) and 128^3 (3D) in both precisions.
 //
 // omni_persist.cuh streams every vector through L2 in every phase and crosses two fenced grid barriers per CG
-// iteration; at these sizes an iteration is bound by those round trips (a fence.acq_rel.gpu alone costs about 2 us),
+// iteration; at these sizes an iteration is bound by those round trips (a fenced barrier of 148 CTAs costs 3.9 us),
 // not by bandwidth.  Here each CTA owns a BOX of grid rows, [j0, j1) x [k0, k1) with the whole x extent, for the
-// entire inner solve:
+// entire inner solve; a thread owns one 16-byte x chunk of consecutive rows of the box:
 //   * p of the box and of the one-row / one-plane halo around it lives in shared memory (the stencil M p, Eq. 12 :119,
 //     reads neighbours from there);
-//   * r of the box lives in registers (CG touches r cell by cell only): a thread owns one 16-byte x chunk of up to
-//     RES_NI consecutive rows of the box;
-//   * delta (the CG solution, Alg. 1 :146) lives in shared memory when it fits beside p, else in global memory and is
-//     touched every second iteration (lazy, as in the tile kernel K4: delta += alpha_{k-1} p_{k-1} + alpha_k p_k with
-//     p_{k-1} = (p_k - r_k) / beta_k recovered from what is on chip);
+//   * r and delta (the CG solution, Alg. 1 :146) are touched cell by cell by their thread only.  They live in the SM's
+//     TENSOR MEMORY, used as a thread-private scratchpad through tcgen05.ld / st (RM 3, at most RES_NI rows per thread), which
+//     leaves the shared memory to p and to q = Op p.  Otherwise (more rows per thread; fp64 with the operator M, whose
+//     tensor-memory instantiation runs out of registers): r in shared memory beside p (RM 0), behind L2 where p alone fills
+//     the shared memory (RM 2), or in registers (RM 1, on request); delta in shared memory when it fits, else in global
+//     memory and touched every second iteration (lazy, as in the tile kernel K4: delta += alpha_{k-1} p_{k-1} + alpha_k p_k
+//     with p_{k-1} = (p_k - r_k) / beta_k recovered from what is on chip);
 //   * per CG iteration the only global traffic is the halo of r: K4 sends r of the box's boundary rows to the
 //     neighbours, which form p_new = r + beta p_old on their halo themselves (p_old of the halo is in their shared
 //     memory), so no p ever travels.  The rows travel as self-validating 8-byte messages { 32 payload bits, 32-bit
 //     epoch = number of the CG iteration that wrote them } (the scheme of NCCL's low-latency protocol): a reader polls
 //     until the epoch is the one it expects, so the exchange needs no fence, and the two grid barriers of an iteration
 //     -- which remain, as the deterministic all-reduce of gamma and rho' -- carry nothing but their own slot and are
-//     relaxed (omni_persist.cuh: RELAXED).  The fenced barriers remain around K2, once per outer iteration.
+//     relaxed (grid_allreduce_relaxed below: 1.6 us).  The fenced barriers remain around K2, once per outer iteration.
 // Phase order, arithmetic per cell (apply_op_chunk of omni_kernels.cuh), stopping rules and the K2 phase (outer update
 // through L2, persist_k2_rows) are those of persist_kernel; the reductions differ from it only in the order in which
 // cells are added (fp32: a chunk's four products are added in fp32 first, as in the tile kernels, A9).
@@ -43,7 +45,7 @@ __device__ unsigned long long g_res_trace[16];
 
 constexpr int RES_NT = 512;        // threads per CTA: up to 128 registers each, half of them hold r
 constexpr int RES_NI = 16;         // rows per thread (16-byte chunks of r: 64 registers)
-constexpr int RES_SMEM_MAX = 227 * 1024 - 1024;   // dynamic shared memory the plan may use (static: the barrier's scratch)
+constexpr int RES_SMEM_MAX = (227 - 5) * 1024;    // dynamic shared memory the plan may use (static: 4.4 KB of barrier scratch)
 
 // Start of part i when an axis of n cells is cut into `parts` boxes.  wface = 0: equal counts.  wface > 0 (operator M on an
 // axis with face classes): a cell costs 4, a cell of a face class (0, 1, n-2, n-1; they run the face correction of
@@ -703,7 +705,8 @@ inline bool resident_plan(const Geom& g, int elem_size, int nsm, bool lop, bool 
         if (gz > g.nz) gz = g.nz;
         if (gz < 1) break;
         for (int weighted = 0; weighted < 2; ++weighted) {
-            const int wy = (weighted && fy) ? 3 : 0, wz = (weighted && fz) ? 3 : 0;
+            // (under L the weighted cut costs nothing and only matters where it makes the largest box small enough to fit)
+            const int wy = (weighted && g.fix[1]) ? 3 : 0, wz = (weighted && three && g.fix[2]) ? 3 : 0;
             if (weighted && !wy && !wz) continue;
             long long ly = 0, lz = 0;                               // largest box
             double worst = 0.0;                                     // rows per thread of the slowest box, in interior-row units
