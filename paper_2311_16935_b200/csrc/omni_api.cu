@@ -1073,28 +1073,37 @@ int run_loop_persist(const Geom& g, const Workspace<T>& w, const HostConst& H, c
 // SM-resident loop (omni_resident.cuh): the persistent loop with p in shared memory and r in registers for the whole
 // inner solve.  Returns -100 if the grid does not fit the SMs or the device cannot co-schedule it.
 // OMNI_RESIDENT_TMEM = 0 / 2 keeps r and delta of the resident loop out of / always in tensor memory (A / B measurements).
-// The one combination it loses on is fp64 with the operator M (0.87-0.98 x: that instantiation runs out of registers), which
-// keeps r in shared memory / L2.
-bool resident_tmem(int elem_size, bool lop)
+// The one combination it loses on is fp64 with the operator M in the masked (non-uniform) form (0.87-0.98 x), which keeps r in
+// shared memory / L2.
+int resident_tmem_policy()
 {
     static int v = -1;
     if (v < 0) {
         const char* e = getenv("OMNI_RESIDENT_TMEM");
         v = e ? atoi(e) : 1;                                  // 0: never, 1: where it wins, 2: always
     }
-    return v == 2 || (v == 1 && !(elem_size == 8 && !lop));
+    return v;
 }
 
-template <typename T, bool LOP, int RM>
+// the plan the resident loop runs: with tensor memory unless that needs the masked form for fp64 with M
+bool resident_plan_auto(const Geom& g, int elem_size, int nsm, bool lop, ResidentPlan& pl)
+{
+    const int pol = resident_tmem_policy();
+    if (!resident_plan(g, elem_size, nsm, lop, pol != 0, pl)) return false;
+    if (pol == 1 && pl.rtm && !pl.uni && elem_size == 8 && !lop) return resident_plan(g, elem_size, nsm, lop, false, pl);
+    return true;
+}
+
+template <typename T, bool LOP, int RM, bool UNI = true>
 int launch_resident(const Geom& g, const Workspace<T>& w, const HostConst& H, const Coef<T>& K, const ResidentPlan& pl, cudaStream_t st)
 {
     const int G = pl.gy * pl.gz;
-    if (cudaFuncSetAttribute(resident_kernel<T, LOP, RM>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem_bytes) != cudaSuccess) {
+    if (cudaFuncSetAttribute(resident_kernel<T, LOP, RM, UNI>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem_bytes) != cudaSuccess) {
         cudaGetLastError();
         return -100;
     }
     int occ = 0;
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, resident_kernel<T, LOP, RM>, RES_NT, pl.smem_bytes) != cudaSuccess || occ < 1) {
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, resident_kernel<T, LOP, RM, UNI>, RES_NT, pl.smem_bytes) != cudaSuccess || occ < 1) {
         cudaGetLastError();
         return -100;
     }
@@ -1113,7 +1122,7 @@ int launch_resident(const Geom& g, const Workspace<T>& w, const HostConst& H, co
     CK(cudaMemsetAsync(w.slots, 0, PERSIST_SLOT_BYTES, st));
     Geom gg = g;
     void* params[2] = { (void*)&gg, (void*)&ra };
-    if (cudaLaunchCooperativeKernel((const void*)resident_kernel<T, LOP, RM>, dim3((unsigned)G), dim3(RES_NT), params, pl.smem_bytes, st) != cudaSuccess) {
+    if (cudaLaunchCooperativeKernel((const void*)resident_kernel<T, LOP, RM, UNI>, dim3((unsigned)G), dim3(RES_NT), params, pl.smem_bytes, st) != cudaSuccess) {
         cudaGetLastError();
         return -100;
     }
@@ -1128,9 +1137,9 @@ int run_loop_resident(const Geom& g, const Workspace<T>& w, const HostConst& H, 
     if (!di.coop || di.sms < 1) return -100;
     if (g.npad >= (1LL << 31) || (long long)g.ny * g.nz * ((g.nx + 63) / 64) >= (1LL << 31)) return -100;
     ResidentPlan pl;
-    if (!resident_plan(g, (int)sizeof(T), di.sms < 148 ? di.sms : 148, LOP, resident_tmem((int)sizeof(T), LOP), pl)) return -100;     // relaxed slots: room for 148 CTAs
+    if (!resident_plan_auto(g, (int)sizeof(T), di.sms < 148 ? di.sms : 148, LOP, pl)) return -100;     // relaxed slots: room for 148 CTAs
     if (pl.gy * pl.gz > 148 || pl.gy * pl.gz > RES_NT) return -100;          // relaxed slots: RES_SLOT_OFFSET
-    if (pl.rtm) return launch_resident<T, LOP, 3>(g, w, H, K, pl, st);
+    if (pl.rtm) return pl.uni ? launch_resident<T, LOP, 3, true>(g, w, H, K, pl, st) : launch_resident<T, LOP, 3, false>(g, w, H, K, pl, st);
     if (!pl.rreg) return launch_resident<T, LOP, 0>(g, w, H, K, pl, st);
     static const int rmode = getenv("OMNI_RESIDENT_R") ? atoi(getenv("OMNI_RESIDENT_R")) : 2;
     if (rmode == 1 && pl.rpt <= RES_NI) return launch_resident<T, LOP, 1>(g, w, H, K, pl, st);
@@ -1280,7 +1289,7 @@ int solve_ws(int nx, int ny, int nz, double dx, double dy, double dz, const T* g
         ResidentPlan pl;
         const DevInfo di = device_info();
         const bool one_red = lop && opt.single_reduction;          // that option is the persistent loop's
-        if (!one_red && !pcg && resident_enabled() && di.coop && resident_plan(g, (int)sizeof(T), di.sms < 148 ? di.sms : 148, lop != 0, resident_tmem((int)sizeof(T), lop != 0), pl))
+        if (!one_red && !pcg && resident_enabled() && di.coop && resident_plan_auto(g, (int)sizeof(T), di.sms < 148 ? di.sms : 148, lop != 0, pl))
             mode = 5;
         else
             mode = (g.npad <= persist_max_cells()) ? 3 : (g.npad <= loopk_max_cells()) ? 4 : 2;
@@ -2375,7 +2384,7 @@ int omni_resident_plan(int nx, int ny, int nz, int elem_size, int nsm, int lop, 
     Geom g;
     if ((elem_size != 4 && elem_size != 8) || !out || nsm < 1 || !make_geom(nx, ny, nz, elem_size, g, 0)) return OMNI_ERR_INVALID_ARG;
     ResidentPlan pl;
-    if (!resident_plan(g, elem_size, nsm < 148 ? nsm : 148, lop != 0, resident_tmem(elem_size, lop != 0), pl)) return 0;
+    if (!resident_plan_auto(g, elem_size, nsm < 148 ? nsm : 148, lop != 0, pl)) return 0;
     const int v[13] = { pl.gy, pl.gz, pl.ly, pl.lz, (int)pl.smem_bytes, pl.rpt, pl.rreg, pl.dres, pl.qres, pl.wy, pl.wz, g.px, pl.rtm };
     for (int i = 0; i < 13; ++i) out[i] = v[i];
     return 1;

@@ -228,10 +228,14 @@ __device__ __forceinline__ void res_for_rows(int nrt, F&& f)
 // issuing them four rows ahead (16 + 16 more registers for r and the lazy delta) was tried and is slower (128^3 fp64:
 // 29.8 -> 36.3 us per iteration): with 190 KB of shared memory the L1 is 28 KB and the 230 B per thread it spills miss it.
 //   3: r AND delta in tensor memory (tmem_* above): shared memory holds p and, where it fits, q.
-template <typename T, bool LOP, int RM>
+// UNI (RM 3 only; true otherwise): the host has checked that in every box all lanes of a warp own the same number of rows
+// (resident_uniform), so the warp-wide tcgen05 instructions need no per-lane mask.  Without it the row loops run to the
+// warp's longest lane under a `live` predicate, which costs the stencil loops a third more instructions.
+template <typename T, bool LOP, int RM, bool UNI = true>
 __global__ void __launch_bounds__(RES_NT, 1)
 resident_kernel(const Geom g, const ResidentArgs<T> ra)
 {
+    static_assert(RM == 3 || UNI, "only the tensor-memory variant has a masked form");
     constexpr int V = 16 / (int)sizeof(T), NT = RES_NT, NW = NT / 32, MW = (int)sizeof(T) / 4;
     constexpr bool RREG = RM == 1, RTM = RM == 3;
     __shared__ uint32_t tmem_base_slot;
@@ -280,7 +284,7 @@ resident_kernel(const Geom g, const ResidentArgs<T> ra)
     // tcgen05.ld / st are warp-wide: with r in tensor memory every lane of a warp walks the same number of rows (the
     // largest of the warp); `live` tells a lane whether row `it` is one of its own
     int nloop = nrt;
-    if constexpr (RTM) {
+    if constexpr (!UNI) {
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) nloop = max(nloop, __shfl_xor_sync(0xffffffffu, nloop, o));
     }
@@ -291,7 +295,7 @@ resident_kernel(const Geom g, const ResidentArgs<T> ra)
     {                                                                                                    \
         int jl = jl0, kl = kl0, off = off0;                                                              \
         res_for_rows<RREG>(nloop, [&](const int it) {                                                    \
-            const bool live = it < nrt;
+            const bool live = UNI || it < nrt;
 #define RES_ROWS_END                                                                                     \
             jl += 1; off += rs;                                                                          \
             if (jl == lyb) { jl = 0; kl += 1; off += wrap; }                                             \
@@ -676,9 +680,32 @@ resident_kernel(const Geom g, const ResidentArgs<T> ra)
     }
 }
 
+// ---- host side: does every warp of every box own the same number of rows in all its lanes?  (the thread -> rows map of the kernel)
+inline bool resident_uniform(const Geom& g, int elem_size, int gy, int gz, int wy, int wz)
+{
+    const int V = 16 / elem_size, cpr = g.px / V, nrg = RES_NT / cpr;
+    for (int bz = 0; bz < gz; ++bz)
+        for (int by = 0; by < gy; ++by) {
+            const int nrows = (res_split(g.ny, gy, by + 1, wy) - res_split(g.ny, gy, by, wy)) *
+                              (res_split(g.nz, gz, bz + 1, wz) - res_split(g.nz, gz, bz, wz));
+            const int rpg = (nrows + nrg - 1) / nrg;
+            for (int w = 0; w < RES_NT / 32; ++w) {
+                int first = -1;
+                for (int l = 0; l < 32; ++l) {
+                    const int tid = 32 * w + l, grp = tid / cpr, x = (tid - grp * cpr) * V;
+                    const int r_lo = std::min(grp * rpg, nrows);
+                    const int nrt = (grp < nrg && x < g.nx) ? std::min(rpg, nrows - r_lo) : 0;
+                    if (l == 0) first = nrt;
+                    else if (nrt != first) return false;
+                }
+            }
+        }
+    return true;
+}
+
 // ---- host side: the box decomposition.  Returns false if the grid does not fit the SMs' memory.
 struct ResidentPlan {
-    int gy, gz, ly, lz, zpad, pxs, dres, qres, rpt, rreg, wy, wz, rtm;   // rtm: r and delta in tensor memory    // rreg: r does not fit the shared memory beside p
+    int gy, gz, ly, lz, zpad, pxs, dres, qres, rpt, rreg, wy, wz, rtm, uni;   // rtm: r and delta in tensor memory; uni: resident_uniform    // rreg: r does not fit the shared memory beside p
     unsigned smem_bytes;
 };
 
@@ -740,6 +767,7 @@ inline bool resident_plan(const Geom& g, int elem_size, int nsm, bool lop, bool 
             }
         }
     }
+    if (best_cost >= 0.0) best.uni = resident_uniform(g, elem_size, best.gy, best.gz, best.wy, best.wz) ? 1 : 0;
     return best_cost >= 0.0;
 }
 
