@@ -1072,26 +1072,42 @@ int run_loop_persist(const Geom& g, const Workspace<T>& w, const HostConst& H, c
 
 // SM-resident loop (omni_resident.cuh): the persistent loop with p in shared memory and r in registers for the whole
 // inner solve.  Returns -100 if the grid does not fit the SMs or the device cannot co-schedule it.
-// OMNI_RESIDENT_TMEM = 0 / 2 keeps r and delta of the resident loop out of / always in tensor memory (A / B measurements).
-// The one combination it loses on is fp64 with the operator M in the masked (non-uniform) form (0.87-0.98 x), which keeps r in
-// shared memory / L2.
+// OMNI_RESIDENT_TMEM=0 keeps r and delta of the resident loop out of tensor memory (A / B measurements).
 int resident_tmem_policy()
 {
     static int v = -1;
     if (v < 0) {
         const char* e = getenv("OMNI_RESIDENT_TMEM");
-        v = e ? atoi(e) : 1;                                  // 0: never, 1: where it wins, 2: always
+        v = e ? atoi(e) : 1;                                  // 0: never, else wherever a thread has at most RES_NI rows
     }
     return v;
 }
 
-// the plan the resident loop runs: with tensor memory unless that needs the masked form for fp64 with M
+
+// The search walks every box of every candidate grid (1 - 2 ms of host time at 1024^2 or 128^3): its results are kept, keyed
+// by what they depend on; the last few geometries of a process cover the solves it repeats.
 bool resident_plan_auto(const Geom& g, int elem_size, int nsm, bool lop, ResidentPlan& pl)
 {
-    const int pol = resident_tmem_policy();
-    if (!resident_plan(g, elem_size, nsm, lop, pol != 0, pl)) return false;
-    if (pol == 1 && pl.rtm && !pl.uni && elem_size == 8 && !lop) return resident_plan(g, elem_size, nsm, lop, false, pl);
-    return true;
+    struct Entry { int nx, ny, nz, naxes, fix1, fix2, esz, nsm, lop, ok; ResidentPlan pl; };
+    static std::mutex mu;
+    static std::vector<Entry> cache;
+    const Entry key = { g.nx, g.ny, g.nz, g.naxes, g.fix[1], g.fix[2], elem_size, nsm, lop ? 1 : 0, 0, ResidentPlan() };
+    {
+        std::lock_guard<std::mutex> lk(mu);
+        for (const Entry& e : cache)
+            if (e.nx == key.nx && e.ny == key.ny && e.nz == key.nz && e.naxes == key.naxes && e.fix1 == key.fix1 && e.fix2 == key.fix2 &&
+                e.esz == key.esz && e.nsm == key.nsm && e.lop == key.lop) {
+                pl = e.pl;
+                return e.ok != 0;
+            }
+    }
+    Entry e = key;
+    e.ok = resident_plan(g, elem_size, nsm, lop, resident_tmem_policy() != 0, e.pl) ? 1 : 0;
+    pl = e.pl;
+    std::lock_guard<std::mutex> lk(mu);
+    if (cache.size() >= 32) cache.erase(cache.begin());
+    cache.push_back(e);
+    return e.ok != 0;
 }
 
 template <typename T, bool LOP, int RM, bool UNI = true>

@@ -10,8 +10,7 @@
 //     reads neighbours from there);
 //   * r and delta (the CG solution, Alg. 1 :146) are touched cell by cell by their thread only.  They live in the SM's
 //     TENSOR MEMORY, used as a thread-private scratchpad through tcgen05.ld / st (RM 3, at most RES_NI rows per thread), which
-//     leaves the shared memory to p and to q = Op p.  Otherwise (more rows per thread; fp64 with the operator M, whose
-//     tensor-memory instantiation runs out of registers): r in shared memory beside p (RM 0), behind L2 where p alone fills
+//     leaves the shared memory to p and to q = Op p.  Otherwise (more rows per thread): r in shared memory beside p (RM 0), behind L2 where p alone fills
 //     the shared memory (RM 2), or in registers (RM 1, on request); delta in shared memory when it fits, else in global
 //     memory and touched every second iteration (lazy, as in the tile kernel K4: delta += alpha_{k-1} p_{k-1} + alpha_k p_k
 //     with p_{k-1} = (p_k - r_k) / beta_k recovered from what is on chip);
@@ -43,8 +42,8 @@ __device__ unsigned long long g_res_trace[16];
 #define RES_T(i) do { } while (0)
 #endif
 
-constexpr int RES_NT = 512;        // threads per CTA: up to 128 registers each, half of them hold r
-constexpr int RES_NI = 16;         // rows per thread (16-byte chunks of r: 64 registers)
+constexpr int RES_NT = 512;        // threads per CTA: up to 128 registers each
+constexpr int RES_NI = 16;         // rows per thread whose r and delta fit the thread's share of tensor memory (and, RM 1, 64 registers)
 constexpr int RES_SMEM_MAX = (227 - 5) * 1024;    // dynamic shared memory the plan may use (static: 4.4 KB of barrier scratch)
 
 // Start of part i when an axis of n cells is cut into `parts` boxes.  wface = 0: equal counts.  wface > 0 (operator M on an
@@ -95,7 +94,8 @@ __device__ __forceinline__ void msg_send(unsigned long long* m, const T (&v)[V],
 // the loads (in flight until msg_decode looks at them) ...
 __device__ __forceinline__ void msg_load(const unsigned long long* m, unsigned long long (&b)[4])
 {
-    // ld.global.cg is a strong L2 load on sm_100a (LDG.STRONG.GPU); every 8-byte word validates itself through its epoch
+    // strong L2 loads (weak ones may be hoisted out of a polling loop or served from L1); every 8-byte word validates itself
+    // through its epoch
     asm volatile("ld.relaxed.gpu.global.v2.u64 {%0, %1}, [%2];" : "=l"(b[0]), "=l"(b[1]) : "l"(m) : "memory");
     asm volatile("ld.relaxed.gpu.global.v2.u64 {%0, %1}, [%2];" : "=l"(b[2]), "=l"(b[3]) : "l"(m + 2) : "memory");
 }
@@ -229,8 +229,8 @@ __device__ __forceinline__ void res_for_rows(int nrt, F&& f)
 // 29.8 -> 36.3 us per iteration): with 190 KB of shared memory the L1 is 28 KB and the 230 B per thread it spills miss it.
 //   3: r AND delta in tensor memory (tmem_* above): shared memory holds p and, where it fits, q.
 // UNI (RM 3 only; true otherwise): the host has checked that in every box all lanes of a warp own the same number of rows
-// (resident_uniform), so the warp-wide tcgen05 instructions need no per-lane mask.  Without it the row loops run to the
-// warp's longest lane under a `live` predicate, which costs the stencil loops a third more instructions.
+// (resident_uniform), so the warp-wide tcgen05 instructions need no per-lane mask.  Without it the row loops that touch
+// tensor memory run to the warp's longest lane under a `live` predicate.
 template <typename T, bool LOP, int RM, bool UNI = true>
 __global__ void __launch_bounds__(RES_NT, 1)
 resident_kernel(const Geom g, const ResidentArgs<T> ra)
@@ -301,13 +301,19 @@ resident_kernel(const Geom g, const ResidentArgs<T> ra)
             if (jl == lyb) { jl = 0; kl += 1; off += wrap; }                                             \
         });                                                                                              \
     }
+    // the same walk for loops without warp-wide instructions: every lane stops after its own rows, no mask
+#define RES_ROWS_BEGIN_LANE                                                                              \
+    {                                                                                                    \
+        int jl = jl0, kl = kl0, off = off0;                                                              \
+        res_for_rows<RREG>(nrt, [&](const int it) {                                                      \
+            constexpr bool live = true;
 
     // per row of this thread, one bit each (the codes and the box never change during a solve):
     //   slow: the chunk is flagged (mask / NaN changed a code) or the row lies in a face class of the grid -- everything
     //         else is the interior formula (plus the x-edge correction in the two or three threads that hold such cells)
     //   bnd:  the row is on the box boundary: its r travels to a neighbour
     uint32_t fbm = 0, slowm = 0, bndm = 0;
-    RES_ROWS_BEGIN
+    RES_ROWS_BEGIN_LANE
         if (live) {
             if (flag_bits<V>(a.flags, cell_idx(jl, kl))) fbm |= 1u << it;
             if (face_class(j0 + jl, g.ny, g.fix[1]) >= 0 || face_class(k0 + kl, g.nz, g.fix[2]) >= 0) slowm |= 1u << it;
@@ -535,7 +541,7 @@ resident_kernel(const Geom g, const ResidentArgs<T> ra)
             {
                 double acc[1] = { 0.0 };
                 carry = false;
-                RES_ROWS_BEGIN
+                RES_ROWS_BEGIN_LANE
                     if (live) {
                         T q[V];
                         stencil(off, it, jl, kl, q);
@@ -664,6 +670,7 @@ resident_kernel(const Geom g, const ResidentArgs<T> ra)
         }
     }
 #undef RES_ROWS_BEGIN
+#undef RES_ROWS_BEGIN_LANE
 #undef RES_ROWS_END
 #undef RES_CARRY_NEXT
 
