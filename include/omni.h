@@ -395,8 +395,9 @@ long long omni_launch_count(int reset);
  *      the box and its halo in shared memory, r and delta in the SM's tensor memory (tcgen05.ld / st as a thread-private
  *      scratchpad), else in shared memory or, where p alone fills it, behind L2;
  *      per CG iteration only the halo rows of r travel, as self-validating messages, and the two grid barriers carry
- *      nothing but the reduction (no fence).  For grids of up to about 2 M cells whose rows are at most 2048 (fp32) /
- *      1024 (fp64) cells long; falls back to mode 3 where the grid does not fit.  Uses the workspace's two p vectors as
+ *      nothing but the reduction (no fence).  For grids whose p fits the shared memory of the SMs (on a 148-SM B200 up to about
+ *      5 M cells in fp32, 2.5 M in fp64: 2048^2, 160^3 / 1448 x 1024, 136^3) and whose rows are at most 2048 (fp32) / 1024
+ *      (fp64) cells long; falls back to mode 3 where the grid does not fit.  Uses the workspace's two p vectors as
  *      message buffer.
  * The environment variable OMNI_PERSIST_MAX_CELLS overrides the threshold between modes 3 and 2, OMNI_RESIDENT=0 keeps mode
  * 5 out of the automatic choice, OMNI_RESIDENT_TMEM=0 keeps it out of tensor memory.  Modes 1 and 2 give bit-identical results; modes 3, 4 and 5 sum their reductions in a

@@ -1120,3 +1120,27 @@ def test_pcg_batch2d(oracle, dtype):
         assert rel_l2_after_mean_removal(Pc[b].cpu().numpy(), Pd[b].cpu().numpy(), valid) <= (2e-6 if dtype == "f64" else 2e-3)
         e_b, _, nS_b = oracle.eps_R_of_field(gx[b].astype(np.float64), gy[b].astype(np.float64), None, m, Pc[b].cpu().numpy(), d[0], d[1])
         assert e_b * nS_b <= (1.05 if dtype == "f64" else 3.0) * tol * ic["norm_S"]
+
+
+def test_automatic_loop_choice():
+    """Which loop the automatic mode takes, shown by bit-identical results: the SM-resident kernel (5) where the grid fits
+    the SMs, the persistent kernel (3) where its rows are too long for one chunk per thread, the CUDA graph over the tile
+    kernels (2) where p no longer fits the shared memory of the SMs."""
+    cases = [("gaussians2d", (96, 80), "f32", 5), ("fourier3d", (20, 33, 140), "f64", 5),
+             ("lamb_oseen2d", (40, 2100), "f64", 3), ("fourier3d", (200, 190, 200), "f32", 2)]
+    for kind, shape, dtype, expect in cases:
+        f = make_field(kind, shape, seed=2, noise=0.05, kmax=4.0)
+        g_dev, _, m_dev, _ = _inputs(f, dtype)
+        nx = shape[-1]
+        plan = omni.resident_plan(nx, shape[-2], shape[0] if len(shape) == 3 else 1, dtype)
+        assert (plan is not None) == (expect == 5), (shape, dtype, plan)
+        P0, i0 = omni.solve(g_dev[0], g_dev[1], g_dev[2], m_dev, f["d"], 0.0, 3, 7)
+        out = {}
+        for mode in (2, 3, 5):
+            prev = omni.set_loop_mode(mode)
+            try:
+                out[mode] = omni.solve(g_dev[0], g_dev[1], g_dev[2], m_dev, f["d"], 0.0, 3, 7)[0]
+            finally:
+                omni.set_loop_mode(prev)
+        assert torch.equal(torch.nan_to_num(P0), torch.nan_to_num(out[expect])), (shape, dtype, expect)
+        assert i0["cg_iters_total"] == 21
