@@ -107,7 +107,9 @@ int omni_solve_host_f32(int nx, int ny, int nz, double dx, double dy, double dz,
  *   single_reduction  OMNI_METHOD_DIRECT in the persistent loop (mode 3: grids up to 1.5 M cells by default) only: the
  *                   Chronopoulos-Gear recurrences, ONE grid barrier per CG iteration instead of two (SURVEY.md 8(f)
  *                   NEXT-2 i).  In exact arithmetic the same iterates; it relies on L = L^T, so it does not exist for
- *                   Algorithm 1, whose operator is not symmetric (A2).  Ignored elsewhere.
+ *                   Algorithm 1, whose operator is not symmetric (A2).  Ignored elsewhere.  It selects mode 3 even
+ *                   where the automatic choice would be the SM-resident loop (mode 5), which is faster with its two
+ *                   relaxed barriers: a numerical variant, not a speed-up.
  * struct_size must be sizeof(omni_options) (omni_options_init sets it, loop_mode = -1 and everything else to 0 / NULL);
  * a mismatch, hist_capacity < 0, a history pointer with hist_capacity == 0 or an unknown method: OMNI_ERR_INVALID_ARG. */
 enum { OMNI_METHOD_ALG1 = 0, OMNI_METHOD_DIRECT = 1, OMNI_METHOD_PCG = 2 };
